@@ -1,0 +1,24 @@
+import os
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def pytest_configure(config):
+    config.addinivalue_line("markers", "gpu: needs a CUDA device (B200); run with -m gpu")
+
+
+@pytest.fixture(scope="session")
+def rot128():
+    import workloads as W
+    return W.rotations(20260624, 128)
+
+
+@pytest.fixture(scope="session")
+def tab128(rot128):
+    from oracle import oracle as O
+    return O.Tables(rot128, 128)

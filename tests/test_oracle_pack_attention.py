@@ -1,0 +1,207 @@
+"""Pins for the oracle's packer (BGTQ-v1 physical layout) and attention (CPU only).
+
+Byte accounting: PAPER.md:837 (96 B ideal at 3 bits); split merge: PAPER.md:120.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+from scipy.special import softmax as scipy_softmax
+
+from oracle import oracle as O
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "layout_fields.txt")
+
+
+def test_golden_field_positions():
+    n = 0
+    for line in open(GOLDEN):
+        line = line.strip()
+        if not line or line.startswith("#"):
+            continue
+        parts = line.split()
+        b, k, idx = int(parts[0]), int(parts[1]), int(parts[2])
+        want = [int(x, 16) for x in parts[3:]]
+        assert len(want) == b
+        W = np.zeros(8, dtype=np.uint32)
+        O.put_field(W, b, k, idx)
+        assert W[:b].tolist() == want, line
+        assert not W[b:].any()
+        assert O.get_field(W, b, k) == idx
+        n += 1
+    assert n >= 20
+
+
+@pytest.mark.parametrize("b", range(1, 9))
+def test_unit_is_a_bijection(b):
+    """Every one of the 32*b bits of a unit belongs to exactly one slot; round trip for all values."""
+    seen = np.zeros(b, dtype=np.uint32)
+    for k in range(32):
+        W = np.zeros(8, dtype=np.uint32)
+        # all-ones field pattern that survives the width-4 recoding: put every idx, OR the footprints
+        foot = np.zeros(8, dtype=np.uint32)
+        for idx in range(1 << b):
+            W[:] = 0
+            O.put_field(W, b, k, idx)
+            assert O.get_field(W, b, k) == idx
+            foot |= W
+        assert not foot[b:].any()
+        assert not (seen & foot[:b]).any()        # disjoint from other slots
+        seen |= foot[:b]
+        assert sum(bin(int(x)).count("1") for x in foot[:b]) == b
+    assert np.all(seen == 0xFFFFFFFF)
+    # writing one slot never disturbs the others
+    rng = np.random.default_rng(b)
+    vals = rng.integers(0, 1 << b, 32)
+    W = np.zeros(8, dtype=np.uint32)
+    for k in rng.permutation(32):
+        O.put_field(W, b, int(k), int(vals[k]))
+    for k in rng.permutation(32):
+        O.put_field(W, b, int(k), int(vals[k]))   # overwrite in place
+    assert [O.get_field(W, b, k) for k in range(32)] == vals.tolist()
+
+
+def _random_head(rng, bits, b_v, T, d=128):
+    groups = O.groups_from_bits(bits, d, 0)
+    kdim = sum(g.m for g in groups)
+    kidx = np.zeros((T, kdim), np.uint8)
+    o = 0
+    for g in groups:
+        kidx[:, o:o + g.m] = rng.integers(0, 1 << g.width, (T, g.m))
+        o += g.m
+    return O.QuantizedHead(groups, b_v, kidx, rng.integers(0, 0x7C00, (T, len(groups))).astype(np.uint16),
+                           rng.integers(0, 1 << b_v, (T, d)).astype(np.uint8),
+                           rng.integers(0, 0x7C00, T).astype(np.uint16))
+
+
+@pytest.mark.parametrize("bits_kind", ["mixed", "uniform3", "all8", "zeros_and_ones", "ragged"])
+def test_region_round_trip_and_accounting(bits_kind):
+    rng = np.random.default_rng(5)
+    d = 128
+    if bits_kind == "mixed":
+        bits = rng.integers(0, 9, 64)
+    elif bits_kind == "uniform3":
+        bits = np.full(64, 3)
+    elif bits_kind == "all8":
+        bits = np.full(64, 8)
+    elif bits_kind == "zeros_and_ones":
+        bits = np.array([0, 1] * 32)
+    else:
+        bits = np.array([1] * 1 + [2] * 3 + [3] * 33 + [4] * 13 + [5] * 7 + [6] * 5 + [7] * 1 + [8] * 1)
+    b_v = 3
+    T = 128 * 2 + 37                       # two full tiles and a ragged tail
+    q = _random_head(rng, bits, b_v, T)
+    region = O.pack_region(q, d)
+    geo = O.tile_geometry(q.groups, d, b_v)
+    n_g = len(q.groups)
+    # bytes/token == 2*sum(b_i)/8 + 16*b_V + 2*(n_g+1): zero padding anywhere
+    assert geo["stride"] == 32 * int(bits.sum()) + 128 * (16 * b_v + 2 * (n_g + 1))
+    assert O.token_bytes(q.groups, d, b_v) == 2 * int(bits.sum()) / 8 + 16 * b_v + 2 * (n_g + 1)
+    assert region.size == 3 * geo["stride"]
+    u = O.unpack_region(region, q.groups, d, b_v, T)
+    assert np.array_equal(u.kidx, q.kidx) and np.array_equal(u.knorm, q.knorm)
+    assert np.array_equal(u.vidx, q.vidx) and np.array_equal(u.vnorm, q.vnorm)
+    # appending token by token gives the same bytes as packing at once (append preserves neighbours)
+    region2 = np.zeros_like(region)
+    for (t0, t1) in [(0, 1), (1, 100), (100, 129), (129, T)]:
+        part = O.QuantizedHead(q.groups, b_v, q.kidx[t0:t1], q.knorm[t0:t1], q.vidx[t0:t1], q.vnorm[t0:t1])
+        O.pack_region(part, d, region2, t_offset=t0)
+    assert np.array_equal(region, region2)
+    # slots of tokens beyond T stay zero: a full third tile of zero codes only differs there
+    full = O.unpack_region(region, q.groups, d, b_v, 3 * 128)
+    # (zero bits decode to idx 0 except in width-4 groups, whose sign-magnitude zero is idx 8)
+    o = 0
+    for g in q.groups:
+        assert np.all(full.kidx[T:, o:o + g.m] == (8 if g.width == 4 else 0))
+        o += g.m
+    assert not full.vnorm[T:].any() and not full.knorm[T:].any()
+
+
+def test_ideal_three_bit_bytes():
+    """pure 3-bit K+V codes are 48+48 = 96 bytes per token and KV head at D=128."""
+    groups = O.groups_from_bits([3] * 64, 128, 0)
+    geo = O.tile_geometry(groups, 128, 3)
+    assert geo["kcode"] // 128 == 48 and (geo["stride"] - geo["vcode_off"]) // 128 == 48
+    assert O.token_bytes(groups, 128, 3) == 96 + 2 * 2      # + one K-group norm + one V norm (fp16)
+
+
+def test_single_code_lands_where_the_spec_says():
+    """K coord u of token tau in a full half-step: word (unit + 4*(plane*32+lane)), lane=(tau&7)*4+((u&7)>>1),
+    slot=(tau>>4)*4+((tau>>3)&1)*2+(u&1); V coord u: unit J*2+rho, lane (u&7)*4+((tau&7)>>1),
+    slot (tau>>4)*4+((tau>>3)&1)*2+(tau&1).  Byte-level check with 8-bit K and V codes."""
+    d = 128
+    groups = O.groups_from_bits([8] * 64, d, 0)
+    geo = O.tile_geometry(groups, d, 8)
+    for tau, u in [(0, 0), (1, 0), (8, 1), (17, 10), (127, 127), (77, 64)]:
+        q = O.QuantizedHead(groups, 8, np.zeros((128, 128), np.uint8), np.zeros((128, 1), np.uint16),
+                            np.zeros((128, d), np.uint8), np.zeros(128, np.uint16))
+        q.kidx[tau, u] = 0xA5
+        q.vidx[tau, u] = 0x5A
+        region = O.pack_region(q, d)
+        nz = np.nonzero(region)[0].tolist()
+        lane = (tau & 7) * 4 + ((u & 7) >> 1)
+        slot = (tau >> 4) * 4 + ((tau >> 3) & 1) * 2 + (u & 1)
+        kbyte = (u >> 3) * 8 * 128 + 4 * ((slot >> 2) * 32 + lane) + (slot & 3)
+        J, g, rho = u >> 4, u & 7, (u >> 3) & 1
+        vlane = g * 4 + ((tau & 7) >> 1)
+        vslot = (tau >> 4) * 4 + ((tau >> 3) & 1) * 2 + (tau & 1)
+        vbyte = geo["vcode_off"] + (J * 2 + rho) * 8 * 128 + 4 * ((vslot >> 2) * 32 + vlane) + (vslot & 3)
+        assert nz == sorted([kbyte, vbyte])
+        assert region[kbyte] == 0xA5 and region[vbyte] == 0x5A
+
+
+def test_attention_is_textbook_softmax():
+    rng = np.random.default_rng(3)
+    T, d = 300, 128
+    K, V, q = rng.standard_normal((T, d)), rng.standard_normal((T, d)), rng.standard_normal(d)
+    scale = 1.0 / math.sqrt(d)
+    ref = scipy_softmax(scale * (K @ q)) @ V
+    assert np.allclose(O.attention(q, K, V, scale), ref, rtol=1e-12, atol=1e-14)
+    # T = 1 -> the value itself; all-equal logits -> the mean of the values
+    assert np.allclose(O.attention(q, K[:1], V[:1], scale), V[0], rtol=1e-15)
+    assert np.allclose(O.attention(np.zeros(d), K, V, scale), V.mean(0), rtol=1e-12)
+    # huge logits do not overflow (max subtraction)
+    out = O.attention(q * 1e4, K, V, 1.0)
+    assert np.all(np.isfinite(out))
+
+
+@pytest.mark.parametrize("splits", [2, 3, 7, 300])
+def test_split_merge_is_exact(splits):
+    rng = np.random.default_rng(4)
+    T, d = 300, 128
+    K, V, q = rng.standard_normal((T, d)) * 3, rng.standard_normal((T, d)), rng.standard_normal(d)
+    scale = 0.3
+    full = O.attention(q, K, V, scale)
+    edges = np.linspace(0, T, splits + 1).astype(int)
+    parts = [O.attention_partial(q, K[a:b], V[a:b], scale) for a, b in zip(edges[:-1], edges[1:]) if b > a]
+    assert np.allclose(O.merge_partials(parts), full, rtol=1e-12, atol=1e-14)
+
+
+def test_decode_attention_head_equals_rotated_domain_form(tab128):
+    """The plain definition (de-rotate every key) equals the folded form the GPU uses (rotate q once,
+    de-rotate the output once): q'=Pi q/sqrt(m), logits from codes, out = Pi^T acc/sqrt(d)."""
+    import workloads as W
+    d = 128
+    rng = np.random.default_rng(8)
+    scales = W.block_scales(0, 1, 64)
+    k = W.pre_rope_gaussian(0, 2, 200, 1, d, scales)[:, 0].astype(np.float32).astype(np.float64)
+    v = W.values_gaussian(0, 3, 200, 1, d)[:, 0].astype(np.float32).astype(np.float64)
+    bits = O.allocate(2 * scales[0], 192, 0, 8)
+    qh = O.quantize_head(k, v, bits, 3, tab128)
+    qv = rng.standard_normal((2, d))
+    scale = 1 / math.sqrt(d)
+    plain = O.decode_attention_head(qv, qh, tab128, d, scale)
+    for a in range(2):
+        logits = np.zeros(200)
+        o = 0
+        for gi, g in enumerate(qh.groups):
+            qp = tab128.Pi(g.m).astype(np.float64) @ qv[a, g.coords] / math.sqrt(g.m)
+            h = qh.knorm[:, gi].view(np.float16).astype(np.float64)
+            logits += h * (tab128.C(g.width)[qh.kidx[:, o:o + g.m]] @ qp)
+            o += g.m
+        p = scipy_softmax(scale * logits)
+        hv = qh.vnorm.view(np.float16).astype(np.float64)
+        acc = (p * hv) @ tab128.C(3)[qh.vidx]
+        folded = tab128.Pi(d).astype(np.float64).T @ acc / math.sqrt(d)
+        assert np.allclose(folded, plain[a], rtol=1e-10, atol=1e-12)

@@ -1,0 +1,133 @@
+"""Pins for the oracle's TQ-MSE encoder/decoder and the rotation table (CPU only).
+
+Rate law and constants: PAPER.md:49; grouping: PAPER.md:108; Lemma 2: PAPER.md:396.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import workloads as W
+from oracle import codebook as cb
+from oracle import oracle as O
+
+C_TQ = math.sqrt(3.0) * math.pi / 2.0
+
+
+def test_rotations_orthogonal_and_fold_identity(rot128):
+    offs = W.rotation_offsets(128)
+    rng = np.random.default_rng(0)
+    for m in (2, 4, 6, 26, 64, 128):
+        Pi = rot128[offs[m]:offs[m] + m * m].reshape(m, m).astype(np.float64)
+        assert np.max(np.abs(Pi @ Pi.T - np.eye(m))) < 1e-6          # fp32-rounded orthogonal
+        # fold: q^T (h Pi^T c / sqrt(m)) == (Pi q)^T (h c / sqrt(m))
+        q, c, h = rng.standard_normal(m), rng.standard_normal(m), 1.7
+        assert q @ (h * (Pi.T @ c) / math.sqrt(m)) == pytest.approx((Pi @ q) @ (h * c / math.sqrt(m)), rel=1e-12)
+
+
+@pytest.mark.parametrize("b", range(1, 9))
+def test_rate_law_m128(b, tab128):
+    """mean ||x - xhat||^2 / ||x||^2 <= C_TQ 4^-b and ~ D(b) (before the fp16 norm matters)."""
+    rng = np.random.default_rng(b)
+    n = 1500 if b < 6 else 6000
+    rel = np.empty(n)
+    for i in range(n):
+        x = (rng.standard_normal(128) * 3.0).astype(np.float32).astype(np.float64)
+        idx, h, r = O.quantize_group(x, b, tab128)
+        xh = O.dequantize_group(idx, h, b, tab128)
+        rel[i] = np.sum((x - xh) ** 2) / np.sum(x * x)
+        assert idx.max() < (1 << b)
+        assert h == O.f16_bits(math.sqrt(float(np.sum(x * x)))) or abs(h - O.f16_bits(math.sqrt(float(np.sum(x * x))))) <= 1
+    D = cb.distortion(cb.lloyd_max_levels(b))
+    assert rel.mean() <= C_TQ * 4.0 ** (-b)
+    assert rel.mean() == pytest.approx(D, rel=0.06)
+
+
+def test_error_falls_with_bits_and_small_groups(tab128):
+    rng = np.random.default_rng(42)
+    for m in (2, 4, 10, 26):
+        x = rng.standard_normal((400, m)).astype(np.float32).astype(np.float64)
+        prev = None
+        for b in range(1, 9):
+            e = 0.0
+            for row in x:
+                idx, h, _ = O.quantize_group(row, b, tab128)
+                e += np.sum((row - O.dequantize_group(idx, h, b, tab128)) ** 2) / np.sum(row * row)
+            e /= len(x)
+            if prev is not None:
+                assert e < prev          # reconstruction error strictly falls as bits rise
+            prev = e
+
+
+def test_codes_are_nearest_centroid(tab128):
+    """Brute force: idx_j = argmin_k |z_j/sigma - C_k| (thresholds are midpoints)."""
+    rng = np.random.default_rng(1)
+    for m, b in [(128, 3), (26, 5), (8, 8), (2, 1), (64, 2)]:
+        x = rng.standard_normal(m).astype(np.float32).astype(np.float64)
+        idx, h, r = O.quantize_group(x, b, tab128)
+        z = tab128.Pi(m).astype(np.float64) @ x
+        sigma = np.linalg.norm(x) / math.sqrt(m)
+        want = np.argmin(np.abs(z[:, None] / sigma - tab128.C(b)[None, :]), axis=1)
+        assert np.array_equal(idx, want)
+        assert r == pytest.approx(np.linalg.norm(x), rel=1e-14)
+
+
+def test_zero_vector_and_saturating_norm(tab128):
+    idx, h, r = O.quantize_group(np.zeros(16), 4, tab128)
+    assert idx.tolist() == [0] * 16 and h == 0 and r == 0.0
+    assert np.array_equal(O.dequantize_group(idx, h, 4, tab128), np.zeros(16))
+    big = np.full(4, 1.0e6)
+    idx, h, _ = O.quantize_group(big, 2, tab128)
+    assert h == 0x7BFF                       # saturates to 65504 (Q10)
+
+
+def test_lemma2_bound_and_one_group_is_uniform(tab128):
+    """Per-block accounting bound holds for every (q, k, k_hat); a schedule with
+    one width is plain uniform TQ-MSE over the whole head."""
+    rng = np.random.default_rng(7)
+    d = 128
+    a, b = O.pair_indices(d, 0)
+    scales = W.block_scales(0, 1, 64)
+    k_pre = W.pre_rope_gaussian(0, 2, 20, 1, d, scales)
+    q_pre = W.pre_rope_gaussian(0, 1, 20, 1, d, scales)
+    pos_k = np.arange(20, dtype=np.float64)
+    k_post = O.rope(k_pre, pos_k, 1e4, 0)[:, 0].astype(np.float32).astype(np.float64)
+    s, _, _ = O.block_energy(q_pre, k_pre, 0)
+    bits = O.allocate(s[0], 192, 0, 8)
+    qh = O.quantize_head(k_post, k_post, bits, 3, tab128, 0)
+    K_hat, _ = O.dequantize_head(qh, tab128, d)
+    n_pos = 50.0
+    q_post = O.rope(q_pre[:1], np.array([n_pos]), 1e4, 0)[0, 0]
+    for t in range(20):
+        err = abs(q_post @ k_post[t] - q_post @ K_hat[t])
+        e = k_post[t] - K_hat[t]                   # block norms are rotation invariant
+        bound = np.sum(np.sqrt(q_post[a] ** 2 + q_post[b] ** 2) * np.sqrt(e[a] ** 2 + e[b] ** 2))
+        assert err <= bound * (1 + 1e-12)
+    # uniform: all blocks width 3 -> one group of 128 coords == quantising the permuted vector
+    qu = O.quantize_head(k_post, k_post, [3] * 64, 3, tab128, 0)
+    assert len(qu.groups) == 1 and qu.groups[0].m == 128
+    perm = qu.groups[0].coords
+    for t in range(3):
+        idx, h, _ = O.quantize_group(k_post[t, perm], 3, tab128)
+        assert np.array_equal(idx, qu.kidx[t]) and h == qu.knorm[t, 0]
+    # width-0 blocks decode to exactly zero (Q3)
+    z = np.nonzero(bits == 0)[0]
+    if len(z):
+        assert np.all(K_hat[:, a[z]] == 0) and np.all(K_hat[:, b[z]] == 0)
+
+
+def test_block_gtq_beats_uniform_on_logit_error(tab128):
+    """Sanity echo of Table 1's direction on the synthetic profile."""
+    d = 128
+    scales = W.block_scales(0, 1, 64)
+    k_pre = W.pre_rope_gaussian(0, 2, 64, 1, d, scales)
+    q_pre = W.pre_rope_gaussian(0, 1, 64, 1, d, scales)
+    k_post = O.rope(k_pre, np.arange(64, dtype=np.float64), 1e4, 0)[:, 0].astype(np.float32).astype(np.float64)
+    q_post = O.rope(q_pre, np.full(64, 64.0), 1e4, 0)[:, 0]
+    s, _, _ = O.block_energy(q_pre, k_pre, 0)
+    bits = O.allocate(s[0], 192, 0, 8)
+    Kb, _ = O.dequantize_head(O.quantize_head(k_post, k_post, bits, 3, tab128), tab128, d)
+    Ku, _ = O.dequantize_head(O.quantize_head(k_post, k_post, [3] * 64, 3, tab128), tab128, d)
+    mae_b = np.mean(np.abs(q_post @ (k_post - Kb).T))
+    mae_u = np.mean(np.abs(q_post @ (k_post - Ku).T))
+    assert mae_b < 0.7 * mae_u
