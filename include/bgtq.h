@@ -1,0 +1,153 @@
+/*
+ * bgtq.h -- C-ABI of the B200-native Block-GTQ packed-cache decode path.
+ *
+ * Paper: "RoPE-Aware Bit Allocation for KV-Cache Quantization" (arxiv/paper_2606_24033);
+ * citations are PAPER.md:<line>; "Qn" are the readings listed in DESIGN.md section 2.
+ *
+ * Conventions (all entry points):
+ *   - return value is a bgtq_status (0 = ok, <0 = error); nothing throws or aborts;
+ *     bgtq_last_error() returns a thread-local description of the last failure.
+ *   - pointers marked [device] are CUDA device pointers owned by the caller (PyTorch owns the
+ *     memory); pointers marked [host] are plain host memory.  The library allocates device memory
+ *     only inside bgtq_layout_create (small static metadata) and frees it in bgtq_layout_destroy.
+ *   - device work is asynchronous on the caller's `stream` (a cudaStream_t passed as void*;
+ *     NULL = default stream).  No hidden synchronisation.
+ *   - tensors are dense row-major with the listed shapes.  K and q are POST-RoPE (the paper
+ *     quantises after rotary), so no positions cross this boundary.
+ *   - GQA map: query head a uses KV head a / (n_q_heads / n_kv_heads)   (Q18).
+ *   - there is no CPU fallback: every device entry point needs an sm_100a GPU.
+ */
+#ifndef BGTQ_H
+#define BGTQ_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    BGTQ_OK = 0,
+    BGTQ_EINVAL = -1,     /* bad argument (shape, enum, null pointer, negative/NaN score) */
+    BGTQ_EBUDGET = -2,    /* B not in [L*b_min, L*b_max] */
+    BGTQ_ECAPACITY = -3,  /* n_new or batch exceeds what the cache was sized for */
+    BGTQ_EWORKSPACE = -4, /* workspace too small */
+    BGTQ_ECUDA = -5       /* a CUDA runtime call failed */
+} bgtq_status;
+
+typedef enum { BGTQ_F32 = 0, BGTQ_BF16 = 1 } bgtq_dtype;
+/* which coordinates form RoPE block i (Q1): HALF = (i, i+d_h/2), INTERLEAVED = (2i, 2i+1) */
+typedef enum { BGTQ_PAIR_HALF = 0, BGTQ_PAIR_INTERLEAVED = 1 } bgtq_pairing;
+/* score kinds; QK_AVG is Eq. 1 / Eq. 4 */
+typedef enum { BGTQ_QK_AVG = 0, BGTQ_QK_MAX = 1, BGTQ_QK_PRODUCT = 2, BGTQ_K_ONLY = 3,
+               BGTQ_Q_ONLY = 4 } bgtq_score;
+
+#define BGTQ_TILE_TOKENS 128   /* tokens per packed tile */
+#define BGTQ_MAX_WIDTH 8       /* widest code, bits per coordinate */
+
+const char *bgtq_last_error(void);
+
+/* TQ-MSE scalar codebook C_b (Q7): the 2^b levels of the Lloyd-Max quantiser of N(0,1),
+ * ascending, symmetric, rounded to fp16-representable values; b = 0 is {0}.  PAPER.md:49, 114.
+ * levels [host] receives 2^b floats.  Computed by the library itself (csrc/codebook.cpp). */
+int bgtq_codebook(int b, float *levels);
+
+/* ---- a1: block-energy score, Eq. 1 = Eq. 4, Alg. 2.
+ *   Eq[h][i] = 1/(n_q*G) sum_t sum_{g in G(h)} (q[t][g][a(i)]^2 + q[t][g][b(i)]^2)   (square, then mean)
+ *   Ek[h][i] = 1/n_k     sum_t               (k[t][h][a(i)]^2 + k[t][h][b(i)]^2)
+ *   scores[h][i] = kind(Eq, Ek);  QK_AVG = (Eq+Ek)/2.  n_q and n_k are independent (Q15).
+ * q [device] [n_q, n_q_heads, d_h], k [device] [n_k, n_kv_heads, d_h], both of dtype `dt`.
+ * scores [device] float [n_kv_heads, d_h/2]; eq_out / ek_out [device] same shape, may be NULL.
+ * workspace [device], at least bgtq_block_energy_workspace_bytes(...) bytes; contents scratch.
+ * Deterministic (fixed reduction order).  One layer per call. */
+size_t bgtq_block_energy_workspace_bytes(int n_q_heads, int n_kv_heads, int d_h);
+int bgtq_block_energy(const void *q, int64_t n_q, const void *k, int64_t n_k, int dt,
+                      int n_q_heads, int n_kv_heads, int d_h, int pairing, int kind,
+                      float *scores, float *eq_out, float *ek_out,
+                      void *workspace, size_t workspace_bytes, void *stream);
+
+/* ---- a2: greedy marginal-gain allocation, Alg. 1, optimal by Thm. 1.
+ * Per head: b_i = b_min; repeat B - L*b_min times: give one bit to the block with the largest
+ * Delta_i = 3/4 * s_i * 4^-b_i among those with b_i < b_max; ties -> smallest i (Q4).
+ * scores float [n_heads, n_blocks]; bits uint8 [n_heads, n_blocks], sum_i bits = total_bits_B.
+ * on_device = 0: both pointers [host], runs on the calling thread (stream ignored; negative or
+ *   NaN scores -> BGTQ_EINVAL).  on_device = 1: both [device], one warp per head, asynchronous
+ *   (a negative/NaN score is treated as 0 there). */
+int bgtq_allocate(const float *scores, int n_heads, int n_blocks, int b_min, int b_max,
+                  int total_bits_B, uint8_t *bits, int on_device, void *stream);
+
+/* ---- a3: same-width grouping -> static layout metadata.
+ * bits [host] uint8 [n_layers, n_kv_heads, d_h/2] (widths 0..8; width 0 = block not stored,
+ *   decodes to 0, Q3).  Groups G_w = {i : bits_i = w}, w ascending; coordinates inside a group
+ *   [a(i1), b(i1), a(i2), ...] (Q9).  b_v: uniform V width (1..8).
+ * rotations [host] float: the TQ-MSE rotation table (Q8), Pi^(m) for m = 2,4,..,d_h,
+ *   row-major Pi^(m)[j][k] at offset sum_{m'<m, m' even} m'^2 + j*m + k.  It is a random draw of the
+ *   method and therefore an INPUT (data), copied to the device.
+ * The physical format is "BGTQ-v1": tile of 128 tokens =
+ *   [K codes | K norms (fp16) per group | V norms (fp16) | V codes], no padding;
+ *   bytes per token = 16*bbar_K + 16*b_V + 2*(n_groups+1) at d_h = 128.
+ * d_h must be 128.  The layout owns a few hundred KB of device memory. */
+typedef struct bgtq_layout bgtq_layout;
+int bgtq_layout_create(const uint8_t *bits, int n_layers, int n_kv_heads, int n_q_heads, int d_h,
+                       int b_v, int pairing, const float *rotations, bgtq_layout **out);
+void bgtq_layout_destroy(bgtq_layout *layout);
+
+/* Sizes.  cache: one buffer for all layers, order [layer][sequence][head][tile], which the CALLER
+ * allocates and ZERO-INITIALISES once (cudaMemset); max_tokens is the per-sequence capacity
+ * (rounded up to whole tiles).  token_bytes: tile stride / 128 of (layer, kv_head) -- the
+ * roofline input.  workspace: scratch for bgtq_decode_attention (n_layers_per_call = 1 for the
+ * per-layer call). */
+size_t bgtq_cache_bytes(const bgtq_layout *layout, int batch, int64_t max_tokens);
+double bgtq_token_bytes(const bgtq_layout *layout, int layer, int kv_head);
+size_t bgtq_workspace_bytes(const bgtq_layout *layout, int batch, int n_layers_per_call);
+/* byte offset of the packed region of (layer, sequence, kv_head) inside the cache, and its tile
+ * stride; for tests and tools that compare regions with the oracle's packer. */
+int64_t bgtq_region_offset(const bgtq_layout *layout, int layer, int seq, int kv_head, int batch,
+                           int64_t max_tokens);
+int64_t bgtq_tile_stride(const bgtq_layout *layout, int layer, int kv_head);
+
+/* ---- a4: quantize-on-append.  TQ-MSE per same-width K group and for
+ * V as one group; code streams + fp16 norms written in the layout the decode kernel reads
+ * (PAPER.md:112, 122).  Arithmetic is the exact fp64 sequence of DESIGN.md section 3 (codes,
+ * norms and bytes are bit-exact against the oracle).
+ * k_new, v_new [device] [batch, n_new, n_kv_heads, d_h] of dtype dt (post-RoPE K).
+ * seq_len [device] int32 [batch]: tokens already cached; sequence s receives its n_new tokens at
+ *   positions seq_len[s] .. seq_len[s]+n_new-1 and, if advance_seq_len != 0, seq_len[s] is advanced
+ *   by n_new (by a kernel on `stream`; a model appends to every layer with the same seq_len and
+ *   advances on the last).  Tokens that would not fit in max_tokens are dropped and seq_len
+ *   saturates (BGTQ_ECAPACITY if n_new > max_tokens is detectable on the host).
+ * Only the fields of the new tokens change.  One layer per call. */
+int bgtq_quantize_append(const bgtq_layout *layout, int layer, void *cache, const void *k_new,
+                         const void *v_new, int dt, int batch, int n_new, int32_t *seq_len,
+                         int advance_seq_len, int64_t max_tokens, void *stream);
+
+/* ---- a5 + a6: split-KV decode attention over the packed cache with the exact
+ * log-sum-exp merge across splits and the V de-rotation.  For every sequence s and
+ * query head a:  out = softmax_t(softmax_scale * <q, khat_t>) . vhat_t  over t in [0, seq_len[s]),
+ * khat/vhat the dequantised cache (never materialised).  seq_len[s] = 0 gives zeros.
+ * q [device] bf16 [n_layers_per_call, batch, n_q_heads, d_h]; out [device] bf16, same shape.
+ * bgtq_decode_attention: one layer.  bgtq_decode_attention_layers: layers
+ *   [layer0, layer0+n_layers) as independent problems in ONE launch (BASELINE.json cfg2
+ *   "36 independent layers").
+ * workspace [device] >= bgtq_workspace_bytes(layout, batch, n_layers). */
+int bgtq_decode_attention(const bgtq_layout *layout, int layer, const void *cache, const void *q,
+                          const int32_t *seq_len, int batch, int64_t max_tokens,
+                          float softmax_scale, void *out, void *workspace, size_t workspace_bytes,
+                          void *stream);
+int bgtq_decode_attention_layers(const bgtq_layout *layout, int layer0, int n_layers,
+                                 const void *cache, const void *q, const int32_t *seq_len,
+                                 int batch, int64_t max_tokens, float softmax_scale, void *out,
+                                 void *workspace, size_t workspace_bytes, void *stream);
+
+/* ---- test hooks (used by tests/ only; synchronous) */
+/* decode one unit (b words per lane, 32 lanes, plane-major as in a tile) with the kernel's own
+ * unpack routine: words [host] uint32 [b*32] -> values [host] float [32 lanes][32 slots]. */
+int bgtq_debug_decode_unit(int b, const uint32_t *words, float *values);
+/* number of kernels launched by this library since load (bench.py's gpu_launches). */
+int64_t bgtq_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BGTQ_H */

@@ -1,0 +1,243 @@
+"""Thin ctypes binding of libbgtq.so (include/bgtq.h): argument marshalling only.
+
+Every step of the hot path runs in the library's CUDA kernels; PyTorch supplies device memory
+and streams.  There is NO CPU fallback: importing this module without a built libbgtq.so raises,
+and every device entry point needs a CUDA tensor.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libbgtq.so")
+
+F32, BF16 = 0, 1
+PAIR_HALF, PAIR_INTERLEAVED = 0, 1
+QK_AVG, QK_MAX, QK_PRODUCT, K_ONLY, Q_ONLY = range(5)
+TILE_TOKENS = 128
+
+# every symbol include/bgtq.h declares (tests check the library exports each one)
+SYMBOLS = [
+    "bgtq_last_error", "bgtq_codebook", "bgtq_block_energy_workspace_bytes", "bgtq_block_energy",
+    "bgtq_allocate", "bgtq_layout_create", "bgtq_layout_destroy", "bgtq_cache_bytes",
+    "bgtq_token_bytes", "bgtq_workspace_bytes", "bgtq_region_offset", "bgtq_tile_stride",
+    "bgtq_quantize_append", "bgtq_decode_attention", "bgtq_decode_attention_layers",
+    "bgtq_debug_decode_unit", "bgtq_launch_count",
+]
+
+
+class BgtqError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"bgtq error {code}: {msg}")
+        self.code = code
+
+
+def _load() -> C.CDLL:
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(
+            f"{LIB_PATH} not found: build it with `python -m paper_2606_24033_b200.build` "
+            "(there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    vp, i32, i64, f32, sz = C.c_void_p, C.c_int, C.c_int64, C.c_float, C.c_size_t
+    lib.bgtq_last_error.restype = C.c_char_p
+    lib.bgtq_last_error.argtypes = []
+    lib.bgtq_launch_count.restype = i64
+    lib.bgtq_launch_count.argtypes = []
+    lib.bgtq_codebook.restype = i32
+    lib.bgtq_codebook.argtypes = [i32, vp]
+    lib.bgtq_block_energy_workspace_bytes.restype = sz
+    lib.bgtq_block_energy_workspace_bytes.argtypes = [i32, i32, i32]
+    lib.bgtq_block_energy.restype = i32
+    lib.bgtq_block_energy.argtypes = [vp, i64, vp, i64, i32, i32, i32, i32, i32, i32, vp, vp, vp, vp, sz, vp]
+    lib.bgtq_allocate.restype = i32
+    lib.bgtq_allocate.argtypes = [vp, i32, i32, i32, i32, i32, vp, i32, vp]
+    lib.bgtq_layout_create.restype = i32
+    lib.bgtq_layout_create.argtypes = [vp, i32, i32, i32, i32, i32, i32, vp, C.POINTER(vp)]
+    lib.bgtq_layout_destroy.restype = None
+    lib.bgtq_layout_destroy.argtypes = [vp]
+    lib.bgtq_cache_bytes.restype = sz
+    lib.bgtq_cache_bytes.argtypes = [vp, i32, i64]
+    lib.bgtq_token_bytes.restype = C.c_double
+    lib.bgtq_token_bytes.argtypes = [vp, i32, i32]
+    lib.bgtq_workspace_bytes.restype = sz
+    lib.bgtq_workspace_bytes.argtypes = [vp, i32, i32]
+    lib.bgtq_region_offset.restype = i64
+    lib.bgtq_region_offset.argtypes = [vp, i32, i32, i32, i32, i64]
+    lib.bgtq_tile_stride.restype = i64
+    lib.bgtq_tile_stride.argtypes = [vp, i32, i32]
+    lib.bgtq_quantize_append.restype = i32
+    lib.bgtq_quantize_append.argtypes = [vp, i32, vp, vp, vp, i32, i32, i32, vp, i32, i64, vp]
+    lib.bgtq_decode_attention.restype = i32
+    lib.bgtq_decode_attention.argtypes = [vp, i32, vp, vp, vp, i32, i64, f32, vp, vp, sz, vp]
+    lib.bgtq_decode_attention_layers.restype = i32
+    lib.bgtq_decode_attention_layers.argtypes = [vp, i32, i32, vp, vp, vp, i32, i64, f32, vp, vp, sz, vp]
+    lib.bgtq_debug_decode_unit.restype = i32
+    lib.bgtq_debug_decode_unit.argtypes = [i32, vp, vp]
+    return lib
+
+
+_lib = _load()
+
+
+def lib() -> C.CDLL:
+    return _lib
+
+
+def _check(rc: int) -> None:
+    if rc != 0:
+        raise BgtqError(rc, _lib.bgtq_last_error().decode())
+
+
+def _stream() -> int:
+    return torch.cuda.current_stream().cuda_stream
+
+
+def _dev(t: torch.Tensor, dtype=None) -> int:
+    if not t.is_cuda:
+        raise ValueError("expected a CUDA tensor (no CPU fallback)")
+    if not t.is_contiguous():
+        raise ValueError("expected a contiguous tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise ValueError(f"expected dtype {dtype}, got {t.dtype}")
+    return t.data_ptr()
+
+
+def _dt(t: torch.Tensor) -> int:
+    if t.dtype == torch.float32:
+        return F32
+    if t.dtype == torch.bfloat16:
+        return BF16
+    raise ValueError("activations must be float32 or bfloat16")
+
+
+def launch_count() -> int:
+    return int(_lib.bgtq_launch_count())
+
+
+def codebook(b: int) -> np.ndarray:
+    """bgtq_codebook: the 2^b fp16-representable Lloyd-Max levels (float32)."""
+    out = np.zeros(1 << b, dtype=np.float32)
+    _check(_lib.bgtq_codebook(b, out.ctypes.data))
+    return out
+
+
+def block_energy(q: torch.Tensor, k: torch.Tensor, pairing: int = PAIR_HALF, kind: int = QK_AVG,
+                 return_parts: bool = False):
+    """bgtq_block_energy.  q [N_q, H_q, d_h], k [N_k, H_kv, d_h] (CUDA, same dtype) ->
+    scores [H_kv, d_h/2] float32 (and Eq, Ek)."""
+    nq, Hq, d = q.shape
+    nk, Hkv, d2 = k.shape
+    assert d == d2 and _dt(q) == _dt(k)
+    L = d // 2
+    scores = torch.empty((Hkv, L), dtype=torch.float32, device=k.device)
+    eq = torch.empty_like(scores) if return_parts else None
+    ek = torch.empty_like(scores) if return_parts else None
+    nws = int(_lib.bgtq_block_energy_workspace_bytes(Hq, Hkv, d))
+    ws = torch.empty(nws, dtype=torch.uint8, device=k.device)
+    _check(_lib.bgtq_block_energy(_dev(q) if nq else None, nq, _dev(k) if nk else None, nk, _dt(k), Hq, Hkv, d,
+                                  pairing, kind, _dev(scores), _dev(eq) if return_parts else None,
+                                  _dev(ek) if return_parts else None, _dev(ws), nws, _stream()))
+    return (scores, eq, ek) if return_parts else scores
+
+
+def allocate(scores, total_bits: int, b_min: int, b_max: int):
+    """bgtq_allocate.  scores [n_heads, L] float32: a CUDA tensor runs the device kernel and returns
+    a CUDA uint8 tensor; a numpy array runs the library's host variant."""
+    if isinstance(scores, torch.Tensor):
+        n_heads, L = scores.shape
+        bits = torch.empty((n_heads, L), dtype=torch.uint8, device=scores.device)
+        _check(_lib.bgtq_allocate(_dev(scores, torch.float32), n_heads, L, b_min, b_max, total_bits,
+                                  _dev(bits), 1, _stream()))
+        return bits
+    s = np.ascontiguousarray(scores, dtype=np.float32)
+    n_heads, L = s.shape
+    bits = np.zeros((n_heads, L), dtype=np.uint8)
+    _check(_lib.bgtq_allocate(s.ctypes.data, n_heads, L, b_min, b_max, total_bits, bits.ctypes.data, 0, None))
+    return bits
+
+
+class Layout:
+    """bgtq_layout: static metadata of the packed cache for an allocation bits[n_layers, H_kv, L]."""
+
+    def __init__(self, bits: np.ndarray, n_q_heads: int, d_h: int, b_v: int, rotations: np.ndarray,
+                 pairing: int = PAIR_HALF):
+        bits = np.ascontiguousarray(bits, dtype=np.uint8)
+        assert bits.ndim == 3
+        self.n_layers, self.n_kv_heads, _ = bits.shape
+        self.n_q_heads, self.d_h, self.b_v = n_q_heads, d_h, b_v
+        rot = np.ascontiguousarray(rotations, dtype=np.float32)
+        h = C.c_void_p()
+        _check(_lib.bgtq_layout_create(bits.ctypes.data, self.n_layers, self.n_kv_heads, n_q_heads, d_h, b_v,
+                                       pairing, rot.ctypes.data, C.byref(h)))
+        self._h = h
+
+    def __del__(self):
+        h = getattr(self, "_h", None)
+        if h:
+            _lib.bgtq_layout_destroy(h)
+            self._h = None
+
+    def cache_bytes(self, batch: int, max_tokens: int) -> int:
+        return int(_lib.bgtq_cache_bytes(self._h, batch, max_tokens))
+
+    def token_bytes(self, layer: int, kv_head: int) -> float:
+        return float(_lib.bgtq_token_bytes(self._h, layer, kv_head))
+
+    def workspace_bytes(self, batch: int, n_layers: int = 1) -> int:
+        return int(_lib.bgtq_workspace_bytes(self._h, batch, n_layers))
+
+    def region_offset(self, layer: int, seq: int, kv_head: int, batch: int, max_tokens: int) -> int:
+        return int(_lib.bgtq_region_offset(self._h, layer, seq, kv_head, batch, max_tokens))
+
+    def tile_stride(self, layer: int, kv_head: int) -> int:
+        return int(_lib.bgtq_tile_stride(self._h, layer, kv_head))
+
+    def new_cache(self, batch: int, max_tokens: int, device="cuda") -> torch.Tensor:
+        """Zero-initialised cache buffer (torch owns the memory)."""
+        return torch.zeros(self.cache_bytes(batch, max_tokens), dtype=torch.uint8, device=device)
+
+    def new_workspace(self, batch: int, n_layers: int = 1, device="cuda") -> torch.Tensor:
+        return torch.empty(self.workspace_bytes(batch, n_layers), dtype=torch.uint8, device=device)
+
+
+def quantize_append(layout: Layout, layer: int, cache: torch.Tensor, k_new: torch.Tensor,
+                    v_new: torch.Tensor, seq_len: torch.Tensor, max_tokens: int,
+                    advance_seq_len: bool = True) -> None:
+    """bgtq_quantize_append.  k_new, v_new [batch, n_new, H_kv, d_h]; seq_len int32 [batch] (CUDA)."""
+    batch, n_new, Hkv, d = k_new.shape
+    assert v_new.shape == k_new.shape and Hkv == layout.n_kv_heads and d == layout.d_h
+    assert _dt(k_new) == _dt(v_new)
+    _check(_lib.bgtq_quantize_append(layout._h, layer, _dev(cache, torch.uint8), _dev(k_new), _dev(v_new),
+                                     _dt(k_new), batch, n_new, _dev(seq_len, torch.int32),
+                                     1 if advance_seq_len else 0, max_tokens, _stream()))
+
+
+def decode_attention(layout: Layout, layer: int, cache: torch.Tensor, q: torch.Tensor,
+                     seq_len: torch.Tensor, max_tokens: int, softmax_scale: float,
+                     workspace: torch.Tensor, out: Optional[torch.Tensor] = None,
+                     n_layers: int = 1) -> torch.Tensor:
+    """bgtq_decode_attention (n_layers = 1: q [batch, H_q, d_h]) or bgtq_decode_attention_layers
+    (q [n_layers, batch, H_q, d_h], layers layer..layer+n_layers-1 in one launch).  bf16 in / out."""
+    if out is None:
+        out = torch.empty_like(q)
+    batch = q.shape[-3]
+    assert q.shape[-2] == layout.n_q_heads and q.shape[-1] == layout.d_h
+    _check(_lib.bgtq_decode_attention_layers(layout._h, layer, n_layers, _dev(cache, torch.uint8),
+                                             _dev(q, torch.bfloat16), _dev(seq_len, torch.int32), batch,
+                                             max_tokens, float(softmax_scale), _dev(out, torch.bfloat16),
+                                             _dev(workspace, torch.uint8), workspace.numel(), _stream()))
+    return out
+
+
+def debug_decode_unit(b: int, words: np.ndarray) -> np.ndarray:
+    """Test hook: decode one unit (uint32 [b, 32] plane-major) with the kernel's unpack routine ->
+    float32 [32 lanes, 32 slots]."""
+    w = np.ascontiguousarray(words, dtype=np.uint32).reshape(b * 32)
+    out = np.zeros((32, 32), dtype=np.float32)
+    _check(_lib.bgtq_debug_decode_unit(b, w.ctypes.data, out.ctypes.data))
+    return out

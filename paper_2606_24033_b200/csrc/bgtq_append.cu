@@ -1,0 +1,280 @@
+// bgtq_append.cu -- quantize-on-append: TQ-MSE per same-width K group and for V
+// (PAPER.md:49, 108), packed into the BGTQ-v1 tile layout.
+//
+// Exactness: the arithmetic is the fp64 sequence of DESIGN.md section 3 -- fma chains in index
+// order, IEEE sqrt / divide, strict '>' against tau_k * sigma -- written with explicit
+// round-to-nearest intrinsics so the compiler cannot contract or reorder it.
+//
+// One CTA owns one (sequence, KV head, 128-token tile): it stages the tile in shared memory
+// (loading the older tokens if the tile is partly filled), processes the new tokens in sub-batches
+// of 16 (one m-tile of the decode kernel's fragment order), and writes the tile back with
+// coalesced 16-byte stores.  No global atomics; every rotation row is read once per 16 tokens.
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
+
+#include "bgtq_internal.h"
+
+namespace bgtq {
+
+#define CUDA_TRY(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) return cuda_fail(e_, #expr); } while (0)
+
+constexpr int kAppendThreads = 256;
+constexpr int kSub = 16;                       // tokens per sub-batch
+constexpr int kMaxUnits = 2 * kMaxKSteps;
+
+struct UnitDesc { int off; int b; int nc; int ustart; };   // ustart: grouped-order coordinate of slot q=0,c=0
+
+// position of bit `bit` of the field of slot k in a unit of width b (DESIGN.md section 4 table)
+__device__ __forceinline__ void field_bit_pos(int b, int k, int bit, int &word, int &pos)
+{
+    if (b == 1) { word = 0; pos = (15 - (k >> 1)) + 16 * (k & 1); }
+    else if (b == 2) {
+        int kk = k & 15, Q = kk >> 2, e = kk & 3;
+        word = k >> 4; pos = 4 * ((Q & 1) * 4 + e) + 2 * (Q >> 1) + bit;
+    } else if (b == 3 || (b == 4 && bit < 3)) {
+        if (k < 24) { word = k >> 3; pos = 4 * (k & 7) + bit; }
+        else { word = bit; pos = 4 * (k - 24) + 3; }
+    } else if (b == 4) { word = 3; pos = 8 * (k & 3) + 7 - (k >> 2); }
+    else { int s = b * k + bit; word = s >> 5; pos = s & 31; }
+}
+
+// write code idx into slot k of the unit whose word w lives at base[w * wstride] (32-bit words)
+__device__ __forceinline__ void put_field(uint32_t *base, int wstride, int b, int k, unsigned idx)
+{
+    unsigned f = idx;
+    if (b == 4) f = idx >= 8 ? (idx - 8) : (8u | (7u - idx));       // sign-magnitude storage
+    for (int bit = 0; bit < b; ++bit) {
+        int word, pos;
+        field_bit_pos(b, k, bit, word, pos);
+        uint32_t v = base[word * wstride];
+        v = (v & ~(1u << pos)) | (((f >> bit) & 1u) << pos);
+        base[word * wstride] = v;
+    }
+}
+
+__device__ __forceinline__ double to_f64(float v) { return (double)v; }
+__device__ __forceinline__ double to_f64(__nv_bfloat16 v) { return (double)__bfloat162float(v); }
+
+template <typename T>
+__global__ void __launch_bounds__(kAppendThreads)
+quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__ cache,
+                       const T *__restrict__ k_new, const T *__restrict__ v_new,
+                       const double *__restrict__ cb64, const float *__restrict__ rot_t, int batch,
+                       int n_new, int Hkv, const int32_t *__restrict__ seq_len, int64_t n_cap,
+                       int64_t max_tokens)
+{
+    extern __shared__ __align__(16) unsigned char smem[];
+    const int tid = threadIdx.x;
+    const int h = blockIdx.y, s = blockIdx.z;
+    const HeadMeta &M = metas[h];
+    const int64_t t0 = seq_len[s];
+    const int64_t t_end = min(t0 + (int64_t)n_new, max_tokens);
+    const int64_t tile = t0 / kTile + blockIdx.x;
+    const int64_t tile_lo = tile * kTile;
+    const int64_t lo = max(t0, tile_lo), hi = min(t_end, tile_lo + kTile);
+    if (lo >= hi) return;
+
+    const int stride = M.tile_stride, ng = M.n_groups, kdim = M.kdim, b_v = M.b_v;
+    // shared memory carve-up
+    double *xs = reinterpret_cast<double *>(smem);                       // [16][256]
+    double *tau = xs + kSub * 256;                                       // [512] thresholds (C_b at 2^b-1)
+    double *sigma = tau + 512;                                           // [16][9]
+    uint16_t *nrm = reinterpret_cast<uint16_t *>(sigma + kSub * 9);      // [16][9] (+pad)
+    uint8_t *idxs = reinterpret_cast<uint8_t *>(nrm + kSub * 9 + 8);     // [16][256]
+    UnitDesc *units = reinterpret_cast<UnitDesc *>(idxs + kSub * 256);   // [32]
+    int *n_units_p = reinterpret_cast<int *>(units + kMaxUnits);
+    uint32_t *tbuf = reinterpret_cast<uint32_t *>(n_units_p + 4);        // tile, `stride` bytes
+
+    uint8_t *gtile = cache + n_cap * ((int64_t)batch * M.layer_prefix + (int64_t)s * M.layer_sum + M.head_prefix) + tile * stride;
+    {   // stage the tile: older tokens present -> load, else start from zeros
+        const bool has_old = tile_lo < t0;
+        const uint4 *src = reinterpret_cast<const uint4 *>(gtile);
+        uint4 *dst = reinterpret_cast<uint4 *>(tbuf);
+        for (int i = tid; i < stride / 16; i += kAppendThreads)
+            dst[i] = has_old ? src[i] : make_uint4(0, 0, 0, 0);
+    }
+    // thresholds tau_k = (C[k] + C[k+1]) / 2 (exact in fp64); stored at the level's flat index
+    for (int i = tid; i < 511; i += kAppendThreads) {
+        double c0 = cb64[i], c1 = cb64[i + 1 < 511 ? i + 1 : i];
+        tau[i] = __dmul_rn(__dadd_rn(c0, c1), 0.5);
+    }
+    if (tid == 0) {  // list of half-step units of the K code section
+        int n = 0, j = 0;
+        for (int ks = 0; ks < M.n_ksteps; ++ks) {
+            const KStep &K = M.ksteps[ks];
+            int g = K.flags >> 4;
+            if (K.flags & 1) j = 0;
+            units[n++] = UnitDesc{K.off0, K.b, K.nc0, M.gstart[g] + 8 * j};
+            ++j;
+            if (K.off1 != 0xFFFF) { units[n++] = UnitDesc{K.off1, K.b, K.nc1, M.gstart[g] + 8 * j}; ++j; }
+        }
+        *n_units_p = n;
+    }
+    __syncthreads();
+    const int n_units = *n_units_p;
+
+    // this thread's row of the rotation: col < kdim -> K group row, col >= 128 -> V row
+    const int col = tid;
+    int my_m = 0, my_r = 0, my_x0 = 0, my_g = 0, my_b = 0;
+    if (col >= 128) { my_m = kDh; my_r = col - 128; my_x0 = 128; my_g = ng; my_b = b_v; }
+    else if (col < kdim) {
+        int g = 0;
+        while (g + 1 < ng && col >= M.gstart[g + 1]) ++g;
+        my_m = M.gm[g]; my_r = col - M.gstart[g]; my_x0 = M.gstart[g]; my_g = g; my_b = M.gb[g];
+    }
+    const float *myrot = rot_t + rot_offset(my_m > 0 ? my_m : 2) + my_r;
+
+    for (int i = 0; i < kTile / kSub; ++i) {
+        const int64_t base = tile_lo + i * kSub;
+        const int64_t nlo = max(lo, base), nhi = min(hi, base + kSub);
+        if (nlo >= nhi) continue;
+        // ---- 1. gather the sub-batch: xs[tt][0..127] = K in grouped order, xs[tt][128..255] = V
+        for (int e = tid; e < kSub * 256; e += kAppendThreads) {
+            int tt = e >> 8, c = e & 255;
+            int64_t tok = base + tt;
+            double v = 0.0;
+            if (tok >= nlo && tok < nhi) {
+                int64_t row = (((int64_t)s * n_new + (tok - t0)) * Hkv + h) * kDh;
+                if (c >= 128) v = to_f64(v_new[row + (c - 128)]);
+                else if (c < kdim) v = to_f64(k_new[row + M.coords[c]]);
+            }
+            xs[e] = v;
+        }
+        __syncthreads();
+        // ---- 2. radii: ss = fma chain, r = sqrt(ss), sigma = r / sqrt(m), h = fp16_rne_sat(r)
+        if (tid < kSub * (ng + 1)) {
+            int tt = tid / (ng + 1), g = tid % (ng + 1);
+            int x0 = g < ng ? M.gstart[g] : 128, m = g < ng ? M.gm[g] : kDh;
+            const double *x = xs + tt * 256 + x0;
+            double ss = 0.0;
+            for (int j = 0; j < m; ++j) ss = __fma_rn(x[j], x[j], ss);
+            double r = __dsqrt_rn(ss);
+            sigma[tt * 9 + g] = __ddiv_rn(r, __dsqrt_rn((double)m));
+            __half hv = __double2half(r);
+            uint16_t hb = __half_as_ushort(hv);
+            if (r >= 65520.0) hb = 0x7BFF;
+            nrm[tt * 9 + g] = hb;
+        }
+        // ---- 3. rotation: z[tt] = fma chain over k of Pi[r][k] * x_k, 16 tokens per rotation read
+        double z[kSub];
+#pragma unroll
+        for (int tt = 0; tt < kSub; ++tt) z[tt] = 0.0;
+        if (my_m > 0) {
+            const double *x = xs + my_x0;
+            for (int k = 0; k < my_m; ++k) {
+                double pi = (double)__ldg(myrot + (size_t)k * my_m);
+#pragma unroll
+                for (int tt = 0; tt < kSub; ++tt) z[tt] = __fma_rn(pi, x[tt * 256 + k], z[tt]);
+            }
+        }
+        __syncthreads();
+        // ---- 4. scalar quantise: idx = #{k : z > tau_k * sigma}; the predicate is monotone in k
+        if (my_m > 0) {
+            const double *tb = tau + ((1 << my_b) - 1);
+            const int nthr = (1 << my_b) - 1;
+#pragma unroll
+            for (int tt = 0; tt < kSub; ++tt) {
+                double sg = sigma[tt * 9 + my_g];
+                int a = 0, c = nthr;
+                while (a < c) {
+                    int mid = (a + c) >> 1;
+                    if (z[tt] > __dmul_rn(tb[mid], sg)) a = mid + 1; else c = mid;
+                }
+                idxs[tt * 256 + col] = (uint8_t)a;
+            }
+        }
+        __syncthreads();
+        // ---- 5. pack the sub-batch's fields; each (unit, lane) word set has exactly one owner
+        const int kitems = n_units * 32;
+        for (int it = tid; it < kitems + 16 * 32; it += kAppendThreads) {
+            if (it < kitems) {
+                const UnitDesc U = units[it >> 5];
+                const int lp = it & 31, lanes = 8 * U.nc;
+                if (lp >= lanes) continue;
+                const int g8 = lp / U.nc, c = lp % U.nc;
+                uint32_t *wbase = tbuf + (U.off >> 2) + lp;
+                for (int p = 0; p < 2; ++p) {
+                    int tt = 8 * p + g8;
+                    int64_t tok = base + tt;
+                    if (tok < nlo || tok >= nhi) continue;
+                    for (int q = 0; q < 2; ++q)
+                        put_field(wbase, lanes, U.b, i * 4 + p * 2 + q, idxs[tt * 256 + U.ustart + 2 * c + q]);
+                }
+            } else {
+                const int v = it - kitems, unit = v >> 5, lane = v & 31;   // unit = 2J + rho
+                const int gq = lane >> 2, c = lane & 3;
+                const int u = 16 * (unit >> 1) + 8 * (unit & 1) + gq;
+                uint32_t *wbase = tbuf + ((M.vcode_off + unit * 128 * b_v) >> 2) + lane;
+                for (int o = 0; o < 2; ++o)
+                    for (int e = 0; e < 2; ++e) {
+                        int tt = 8 * o + 2 * c + e;
+                        int64_t tok = base + tt;
+                        if (tok < nlo || tok >= nhi) continue;
+                        put_field(wbase, 32, b_v, i * 4 + o * 2 + e, idxs[tt * 256 + 128 + u]);
+                    }
+            }
+        }
+        if (tid < kSub * (ng + 1)) {   // fp16 norms: token tau at entry (tau&7)*16 + (tau>>4)*2 + ((tau>>3)&1)
+            int tt = tid / (ng + 1), g = tid % (ng + 1);
+            int64_t tok = base + tt;
+            if (tok >= nlo && tok < nhi) {
+                int t128 = i * kSub + tt;
+                int slot = (t128 & 7) * 16 + (t128 >> 4) * 2 + ((t128 >> 3) & 1);
+                int off = g < ng ? M.knorm_off + 256 * g : M.vnorm_off;
+                reinterpret_cast<uint16_t *>(reinterpret_cast<uint8_t *>(tbuf) + off)[slot] = nrm[tt * 9 + g];
+            }
+        }
+        __syncthreads();
+    }
+    {   // write the tile back
+        uint4 *dst = reinterpret_cast<uint4 *>(gtile);
+        const uint4 *src = reinterpret_cast<const uint4 *>(tbuf);
+        for (int i = tid; i < stride / 16; i += kAppendThreads) dst[i] = src[i];
+    }
+}
+
+__global__ void advance_seq_len_kernel(int32_t *seq_len, int batch, int n_new, int64_t max_tokens)
+{
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s < batch) {
+        int64_t v = (int64_t)seq_len[s] + n_new;
+        seq_len[s] = (int32_t)(v > max_tokens ? max_tokens : v);
+    }
+}
+
+static size_t append_smem_bytes(int max_stride)
+{
+    return (size_t)kSub * 256 * 8 + 512 * 8 + kSub * 9 * 8 + (kSub * 9 + 8) * 2 + kSub * 256 +
+           kMaxUnits * sizeof(UnitDesc) + 16 + (size_t)max_stride + 64;
+}
+
+int launch_quantize_append(const bgtq_layout *lay, int layer, void *cache, const void *k_new,
+                           const void *v_new, int dt, int batch, int n_new, int32_t *seq_len,
+                           int advance, int64_t max_tokens, cudaStream_t st)
+{
+    const int64_t n_cap = (max_tokens + kTile - 1) / kTile;
+    const size_t smem = append_smem_bytes(lay->max_stride);
+    dim3 grid((n_new + kTile - 1) / kTile + 1, lay->n_kv_heads, batch);
+    const HeadMeta *metas = lay->d_meta + (size_t)layer * lay->n_kv_heads;
+    if (dt == BGTQ_F32) {
+        CUDA_TRY(cudaFuncSetAttribute(quantize_append_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        quantize_append_kernel<float><<<grid, kAppendThreads, smem, st>>>(
+            metas, (uint8_t *)cache, (const float *)k_new, (const float *)v_new, lay->d_cb64, lay->d_rot_t,
+            batch, n_new, lay->n_kv_heads, seq_len, n_cap, n_cap * kTile);
+    } else {
+        CUDA_TRY(cudaFuncSetAttribute(quantize_append_kernel<__nv_bfloat16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        quantize_append_kernel<__nv_bfloat16><<<grid, kAppendThreads, smem, st>>>(
+            metas, (uint8_t *)cache, (const __nv_bfloat16 *)k_new, (const __nv_bfloat16 *)v_new, lay->d_cb64,
+            lay->d_rot_t, batch, n_new, lay->n_kv_heads, seq_len, n_cap, n_cap * kTile);
+    }
+    count_launch();
+    CUDA_TRY(cudaGetLastError());
+    if (advance) {
+        advance_seq_len_kernel<<<(batch + 127) / 128, 128, 0, st>>>(seq_len, batch, n_new, n_cap * kTile);
+        count_launch();
+        CUDA_TRY(cudaGetLastError());
+    }
+    return BGTQ_OK;
+}
+
+}  // namespace bgtq

@@ -1,0 +1,708 @@
+// bgtq_decode.cu -- split-KV decode attention over the packed cache and the exact
+// log-sum-exp combine + V de-rotation (a6).  PAPER.md:114, 120.  Hand-written for sm_100a.
+//
+// Algebra: the TQ-MSE rotation is folded into the query once per call
+//   q'_g = Pi^(m_g) q_g * (scale*log2(e)/sqrt(m_g))          (prologue kernel)
+// so that  log2e*logit_t = sum_g h_{t,g} * sum_j q'_{g,j} C_{b_g}[idx_{t,g,j}]  -- no key is ever
+// de-rotated and no fp16 K/V tile exists outside registers.  V is accumulated in the rotated
+// domain and de-rotated once per query head after the cross-split merge.
+//
+// Mapping: one WARP owns one 128-token tile at a time.  The tile is one contiguous range of the
+// cache and is staged into the warp's private shared-memory buffer by two TMA bulk copies
+// (cp.async.bulk + mbarrier): [K codes|K norms] and [V norms|V codes]; the K half of the next
+// tile is requested as soon as QK^T of the current one is done, the V half after PV, so the copy
+// engine runs one half-tile ahead of the math of every warp.  Codes are laid out in mma.sync
+// fragment order: tokens are the M dimension of QK^T (A = unpacked codes, fp16
+// exact; B = q' for the <= 8 query heads of the GQA group), dims are the M dimension of PV.
+// Work is split over ALL warps of the grid in equal contiguous ranges of the global tile list
+// [layer][sequence][kv head][tile] (flash-decoding along the key axis); a warp writes
+// one partial (max, sum, acc[128]) per (pair, warp) it touches.
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
+
+#include "bgtq_internal.h"
+
+namespace bgtq {
+
+#define CUDA_TRY(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) return cuda_fail(e_, #expr); } while (0)
+
+constexpr int kMaxWarpsPerSM = 16;
+constexpr int kMaxBatch = 256;
+constexpr int kQfHalves = kMaxKSteps * 8 * 16;      // fp16 q' fragments per (layer, seq, kv head)
+constexpr int kPartialFloats = 8 * 130;             // (m, l, acc[128]) for 8 head slots
+
+// ---------------------------------------------------------------- small PTX wrappers
+__device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t s)
+{
+    uint32_t r;
+    asm("prmt.b32 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(s));
+    return r;
+}
+__device__ __forceinline__ void mma16816(float (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2,
+                                         uint32_t a3, uint32_t b0, uint32_t b1)
+{
+    asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                 : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+                 : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ uint32_t movmatrix_trans(uint32_t x)
+{
+    uint32_t r;
+    asm volatile("movmatrix.sync.aligned.m8n8.trans.b16 %0, %1;" : "=r"(r) : "r"(x));
+    return r;
+}
+__device__ __forceinline__ float fast_exp2(float x)
+{
+    float r;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+__device__ __forceinline__ uint32_t pack_half2(float lo, float hi)
+{
+    uint32_t r;
+    asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+    return r;
+}
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    uint32_t done;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\t"
+                     "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+                     "selp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+    } while (!done);
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async()
+{
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+
+// ---------------------------------------------------------------- unit decoders
+// A unit = B words per lane holding 32 slots.  Output: 16 half2 registers,
+// h[j] = (slot 2j, slot 2j+1) as fp16 codebook values (exact: the codebook is fp16).
+// pools[]: byte planes of the small codebooks for PRMT lookups, built once per CTA:
+//   [0]      b=1: (0x8000 | +c) in both halves
+//   [1],[2]  b=2: low bytes / high bytes of levels 0..3
+//   [3..6]   b=3: low bytes of levels 0..3, 4..7; high bytes of levels 0..3, 4..7
+//   [7..10]  b=4: same for the 8 magnitudes C_4[8..15] (codes are stored sign-magnitude)
+// lut: fp16 bits of the flat codebook table in shared memory (C_b at 2^b - 1), for b >= 5.
+template <int B>
+__device__ __forceinline__ void decode_unit(const uint32_t (&w)[B], const uint32_t *pools,
+                                            const uint16_t *lut, uint32_t (&h)[16])
+{
+    if constexpr (B == 1) {
+        const uint32_t mag = pools[0];
+#pragma unroll
+        for (int j = 0; j < 16; ++j) h[j] = ((w[0] << j) & 0x80008000u) ^ mag;
+    } else if constexpr (B == 2) {
+        const uint32_t LO = pools[1], HI = pools[2];
+#pragma unroll
+        for (int wi = 0; wi < 2; ++wi)
+#pragma unroll
+            for (int hf = 0; hf < 2; ++hf) {
+                const uint32_t t = (w[wi] >> (2 * hf)) & 0x33333333u;
+#pragma unroll
+                for (int ql = 0; ql < 2; ++ql) {
+                    const uint32_t sel = ql ? (t >> 16) : t;
+                    const uint32_t lo4 = prmt(LO, 0, sel), hi4 = prmt(HI, 0, sel);
+                    const int Q = hf * 2 + ql;
+                    h[wi * 8 + 2 * Q] = prmt(lo4, hi4, 0x5140);
+                    h[wi * 8 + 2 * Q + 1] = prmt(lo4, hi4, 0x7362);
+                }
+            }
+    } else if constexpr (B == 3 || B == 4) {
+        const int pb = B == 3 ? 3 : 7;
+        const uint32_t LOa = pools[pb], LOb = pools[pb + 1], HIa = pools[pb + 2], HIb = pools[pb + 3];
+        uint32_t t[4];
+        t[0] = w[0] & 0x77777777u;
+        t[1] = w[1] & 0x77777777u;
+        t[2] = w[2] & 0x77777777u;
+        t[3] = ((w[0] >> 3) & 0x11111111u) | ((w[1] >> 2) & 0x22222222u) | ((w[2] >> 1) & 0x44444444u);
+#pragma unroll
+        for (int wi = 0; wi < 4; ++wi)
+#pragma unroll
+            for (int hf = 0; hf < 2; ++hf) {
+                const uint32_t sel = hf ? (t[wi] >> 16) : t[wi];
+                uint32_t lo4 = prmt(LOa, LOb, sel), hi4 = prmt(HIa, HIb, sel);
+                if constexpr (B == 4) hi4 ^= (w[3] << (2 * wi + hf)) & 0x80808080u;   // sign of slot 4Q+e: bit 8e+7-Q
+                h[wi * 4 + 2 * hf] = prmt(lo4, hi4, 0x5140);
+                h[wi * 4 + 2 * hf + 1] = prmt(lo4, hi4, 0x7362);
+            }
+    } else {
+        const uint16_t *T = lut + ((1 << B) - 1);
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+            uint32_t v[2];
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const int o = B * (2 * j + e), wi = o >> 5, sh = o & 31;
+                uint32_t x;
+                if (sh + B <= 32) x = w[wi] >> sh;
+                else x = __funnelshift_r(w[wi], w[wi + 1 < B ? wi + 1 : wi], sh);
+                v[e] = T[x & ((1u << B) - 1)];
+            }
+            h[j] = v[0] | (v[1] << 16);
+        }
+    }
+}
+
+__device__ __forceinline__ void build_pools(const uint16_t *cb16, uint32_t *pools)
+{
+    // cb16: flat fp16 table in shared memory; one thread fills all pools (tiny)
+    pools[0] = (0x8000u | cb16[1 + 1]) * 0x10001u;
+    auto plane = [&](int base, int hi) {
+        uint32_t r = 0;
+        for (int k = 0; k < 4; ++k) r |= (uint32_t)((cb16[base + k] >> (hi ? 8 : 0)) & 0xFF) << (8 * k);
+        return r;
+    };
+    pools[1] = plane(3, 0);  pools[2] = plane(3, 1);
+    pools[3] = plane(7, 0);  pools[4] = plane(11, 0); pools[5] = plane(7, 1);  pools[6] = plane(11, 1);
+    pools[7] = plane(15 + 8, 0); pools[8] = plane(15 + 12, 0); pools[9] = plane(15 + 8, 1); pools[10] = plane(15 + 12, 1);
+}
+
+// ---------------------------------------------------------------- work partition
+// Global tile list [layer][sequence][kv head][tile]; pre[] = prefix sums of tiles per sequence.
+struct Sched {
+    int n_layers, batch, Hkv;
+    int tiles_sum;          // sum over sequences of ceil(seq_len/128)
+    int total;              // n_layers * Hkv * tiles_sum
+    int per_warp;           // ceil(total / n_warps)
+};
+
+__device__ __forceinline__ void build_prefix(const int32_t *seq_len, int batch, int64_t cap_tokens, int *pre)
+{
+    // called by one thread; batch <= kMaxBatch
+    int acc = 0;
+    pre[0] = 0;
+    for (int b = 0; b < batch; ++b) {
+        int64_t n = seq_len[b];
+        n = n < 0 ? 0 : (n > cap_tokens ? cap_tokens : n);
+        acc += (int)((n + kTile - 1) / kTile);
+        pre[b + 1] = acc;
+    }
+}
+
+__device__ __forceinline__ Sched make_sched(int n_layers, int batch, int Hkv, const int *pre, int n_warps)
+{
+    Sched s;
+    s.n_layers = n_layers; s.batch = batch; s.Hkv = Hkv;
+    s.tiles_sum = pre[batch];
+    s.total = n_layers * Hkv * s.tiles_sum;
+    s.per_warp = s.total > 0 ? (s.total + n_warps - 1) / n_warps : 1;
+    return s;
+}
+
+struct TilePos { int l, b, h, t, tiles_b, pair, pair_start; };
+
+__device__ __forceinline__ TilePos locate(int x, const Sched &s, const int *pre)
+{
+    TilePos p;
+    const int per_layer = s.Hkv * s.tiles_sum;
+    p.l = x / per_layer;
+    const int r = x - p.l * per_layer;
+    int b = 0;
+    while (b + 1 < s.batch && r >= pre[b + 1] * s.Hkv) ++b;
+    p.b = b;
+    p.tiles_b = pre[b + 1] - pre[b];
+    const int r2 = r - pre[b] * s.Hkv;
+    p.h = r2 / p.tiles_b;
+    p.t = r2 - p.h * p.tiles_b;
+    p.pair = (p.l * s.batch + b) * s.Hkv + p.h;
+    p.pair_start = x - p.t;
+    return p;
+}
+
+// ---------------------------------------------------------------- prologue: Q-side rotation fold
+// q'_g = Pi^(m_g) q_g * (scale*log2e/sqrt(m_g))  ("Q-side rotation"), rounded to fp16 and
+// written in B-fragment order: qf[pair][kstep][head slot n (8)][16 coords of the k-step], zero padded.
+__global__ void __launch_bounds__(128)
+qfold_kernel(const HeadMeta *__restrict__ metas, const float *__restrict__ rot_t,
+             const __nv_bfloat16 *__restrict__ q, int batch, int Hkv, int Hq, float scale_log2e,
+             __half *__restrict__ qf)
+{
+    const int pair = blockIdx.x;                       // (l*batch + b)*Hkv + h  (l relative to layer0)
+    const int h = pair % Hkv, lb = pair / Hkv, l = lb / batch;
+    const int G = Hq / Hkv;
+    const HeadMeta &M = metas[l * Hkv + h];
+    __shared__ float qs[8 * kDh];
+    __shared__ int ksbase[kMaxGroups];
+    const int tid = threadIdx.x;
+    for (int e = tid; e < G * kDh; e += 128)
+        qs[e] = __bfloat162float(q[((size_t)lb * Hq + h * G) * kDh + e]);
+    if (tid == 0)
+        for (int ks = 0; ks < M.n_ksteps; ++ks)
+            if (M.ksteps[ks].flags & 1) ksbase[M.ksteps[ks].flags >> 4] = ks;
+    __half *out = qf + (size_t)pair * kQfHalves;
+    for (int e = tid; e < kQfHalves; e += 128) out[e] = __float2half(0.f);
+    __syncthreads();
+    if (tid < M.kdim) {
+        int g = 0;
+        while (g + 1 < M.n_groups && tid >= M.gstart[g + 1]) ++g;
+        const int m = M.gm[g], x0 = M.gstart[g], r = tid - x0;
+        const float *T = rot_t + rot_offset(m) + r;
+        const float sc = scale_log2e / sqrtf((float)m);
+        const int ks = ksbase[g] + (r >> 4), kap = r & 15;
+        for (int n = 0; n < G; ++n) {
+            float acc = 0.f;
+            for (int k = 0; k < m; ++k) acc = fmaf(__ldg(T + (size_t)k * m), qs[n * kDh + M.coords[x0 + k]], acc);
+            out[(ks * 8 + n) * 16 + kap] = __float2half_rn(acc * sc);
+        }
+    }
+}
+
+// ---------------------------------------------------------------- the decode kernel
+struct DecodeParams {
+    const HeadMeta *metas;      // [n_layers][Hkv], first layer of this call
+    const uint8_t *cache;
+    const __half *qf;           // q' fragments, [pair][kQfHalves]
+    const int32_t *seq_len;
+    const uint16_t *cb16;
+    float *partials;            // [n_warps + n_pairs][8][130]
+    int64_t n_cap;              // tiles of capacity per sequence
+    int n_layers, batch, Hkv, G;
+    int buf_bytes;              // per-warp tile buffer
+};
+
+struct WarpState {
+    float m[2], l[2];           // running max (log2 domain) and partial sum for heads 2c, 2c+1
+    float O[8][4];              // PV accumulators: [J] -> dims 16J+g8 (+8), heads 2c, 2c+1
+};
+
+// QK^T of one k16 step: two units of width B -> 8 m-tiles
+template <int B>
+__device__ __forceinline__ void qk_step(const uint32_t *tile, uint32_t d0, uint32_t d1, int g8, int c,
+                                        uint32_t bq0, uint32_t bq1, const uint32_t *pools,
+                                        const uint16_t *lut, float (&A)[8][4])
+{
+    const int off0 = d0 & 0xFFFF, off1 = d0 >> 16;
+    const int nc0 = (d1 >> 8) & 0xFF, nc1 = (d1 >> 16) & 0xFF;
+    uint32_t w0[B], w1[B], h0[16], h1[16];
+    {
+        const bool act = c < nc0;
+        const uint32_t *wp = tile + (off0 >> 2) + g8 * nc0 + c;
+#pragma unroll
+        for (int w = 0; w < B; ++w) w0[w] = act ? wp[w * 8 * nc0] : 0u;
+    }
+    {
+        const bool act = c < nc1;
+        const uint32_t *wp = tile + (off1 >> 2) + g8 * nc1 + c;
+#pragma unroll
+        for (int w = 0; w < B; ++w) w1[w] = act ? wp[w * 8 * nc1] : 0u;
+    }
+    decode_unit<B>(w0, pools, lut, h0);
+    decode_unit<B>(w1, pools, lut, h1);
+#pragma unroll
+    for (int i = 0; i < 8; ++i) mma16816(A[i], h0[2 * i], h0[2 * i + 1], h1[2 * i], h1[2 * i + 1], bq0, bq1);
+}
+
+// PV of one tile: 16 units of width B -> O[J] += V^T[16 dims x 128 tokens] . P[128 tokens x 8 heads]
+template <int B>
+__device__ __forceinline__ void pv_tile(const uint32_t *vcodes, int lane, const uint32_t (&bP)[8][2],
+                                        const uint32_t *pools, const uint16_t *lut, float (&O)[8][4])
+{
+#pragma unroll 1
+    for (int J = 0; J < 8; ++J) {
+        uint32_t w0[B], w1[B], h0[16], h1[16];
+        const uint32_t *wp = vcodes + (2 * J) * 32 * B + lane;
+#pragma unroll
+        for (int w = 0; w < B; ++w) { w0[w] = wp[w * 32]; w1[w] = wp[32 * B + w * 32]; }
+        decode_unit<B>(w0, pools, lut, h0);
+        decode_unit<B>(w1, pools, lut, h1);
+#pragma unroll
+        for (int kp = 0; kp < 8; ++kp)
+            mma16816(O[J], h0[2 * kp], h1[2 * kp], h0[2 * kp + 1], h1[2 * kp + 1], bP[kp][0], bP[kp][1]);
+    }
+}
+
+template <int W>
+__global__ void __launch_bounds__(W * 32, 1)
+decode_kernel(const DecodeParams P)
+{
+    extern __shared__ __align__(128) unsigned char smem[];
+    // carve-up: [lut16 1024 B][pools 64 B][pre (kMaxBatch+1) ints][barriers W*2*8][tile buffers]
+    uint16_t *lut = reinterpret_cast<uint16_t *>(smem);
+    uint32_t *pools = reinterpret_cast<uint32_t *>(smem + 1024);
+    int *pre = reinterpret_cast<int *>(smem + 1024 + 64);
+    uint64_t *bars = reinterpret_cast<uint64_t *>(smem + 1024 + 64 + ((kMaxBatch + 1) * 4 + 12) / 16 * 16);
+    unsigned char *bufs = reinterpret_cast<unsigned char *>(bars + 2 * W);
+    bufs = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(bufs) + 127) & ~uintptr_t(127));
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int g8 = lane >> 2, c = lane & 3;
+    for (int i = tid; i < 512; i += W * 32) lut[i] = P.cb16[i < 511 ? i : 510];
+    if (tid == 0) build_prefix(P.seq_len, P.batch, P.n_cap * kTile, pre);
+    __syncthreads();
+    if (tid == 0) build_pools(lut, pools);
+    const uint32_t kbar = smem_u32(&bars[2 * warp]), vbar = smem_u32(&bars[2 * warp + 1]);
+    if (lane == 0) {
+        mbar_init(kbar, 1);
+        mbar_init(vbar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        fence_proxy_async();
+    }
+    __syncthreads();
+
+    const int n_warps = gridDim.x * W;
+    const int gw = blockIdx.x * W + warp;
+    const Sched S = make_sched(P.n_layers, P.batch, P.Hkv, pre, n_warps);
+    int x = gw * S.per_warp;
+    const int x_end = min(S.total, x + S.per_warp);
+    if (x >= x_end) return;
+
+    uint32_t *tile = reinterpret_cast<uint32_t *>(bufs + (size_t)warp * P.buf_bytes);
+    const uint32_t tile_s = smem_u32(tile);
+    uint32_t kphase = 0, vphase = 0;
+
+    // source address and byte counts of a global tile index (lane 0 only needs them)
+    auto issue = [&](int xg, bool want_k, bool want_v) {
+        const TilePos tp = locate(xg, S, pre);
+        const HeadMeta &M = P.metas[tp.l * P.Hkv + tp.h];
+        const uint8_t *src = P.cache + P.n_cap * ((int64_t)P.batch * M.layer_prefix + (int64_t)tp.b * M.layer_sum + M.head_prefix) +
+                             (int64_t)tp.t * M.tile_stride;
+        const uint32_t kbytes = M.vnorm_off, vbytes = M.tile_stride - M.vnorm_off;
+        fence_proxy_async();
+        if (want_k) { mbar_expect_tx(kbar, kbytes); bulk_g2s(tile_s, src, kbytes, kbar); }
+        if (want_v) { mbar_expect_tx(vbar, vbytes); bulk_g2s(tile_s + kbytes, src + kbytes, vbytes, vbar); }
+    };
+    if (lane == 0) issue(x, true, true);
+
+    while (x < x_end) {
+        // ---------------- segment = the part of one (layer, sequence, kv head) inside this warp's range
+        const TilePos tp = locate(x, S, pre);
+        const HeadMeta &M = P.metas[tp.l * P.Hkv + tp.h];
+        const int seg_end = min(x_end, tp.pair_start + tp.tiles_b);
+        const int n_ksteps = M.n_ksteps, b_v = M.b_v;
+        const int knorm_off = M.knorm_off, vnorm_off = M.vnorm_off, vcode_off = M.vcode_off;
+        int64_t slen = P.seq_len[tp.b];
+        slen = slen > P.n_cap * kTile ? P.n_cap * kTile : slen;
+        // lane ks keeps the descriptor of k-step ks
+        uint32_t desc0 = 0, desc1 = 0;
+        if (lane < n_ksteps) {
+            const KStep K = M.ksteps[lane];
+            desc0 = (uint32_t)K.off0 | ((uint32_t)K.off1 << 16);
+            desc1 = (uint32_t)K.b | ((uint32_t)K.nc0 << 8) | ((uint32_t)K.nc1 << 16) | ((uint32_t)K.flags << 24);
+        }
+        const uint32_t *qfp = reinterpret_cast<const uint32_t *>(P.qf + (size_t)tp.pair * kQfHalves) + g8 * 8 + c;
+
+        WarpState st;
+        st.m[0] = st.m[1] = -INFINITY;
+        st.l[0] = st.l[1] = 0.f;
+#pragma unroll
+        for (int J = 0; J < 8; ++J) st.O[J][0] = st.O[J][1] = st.O[J][2] = st.O[J][3] = 0.f;
+
+        for (int t = tp.t; x < seg_end; ++x, ++t) {
+            // ======== QK^T
+            mbar_wait(kbar, kphase);
+            kphase ^= 1;
+            float Sc[8][4], A[8][4];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) Sc[i][0] = Sc[i][1] = Sc[i][2] = Sc[i][3] = 0.f;
+#pragma unroll 1
+            for (int ks = 0; ks < n_ksteps; ++ks) {
+                const uint32_t d0 = __shfl_sync(0xFFFFFFFFu, desc0, ks);
+                const uint32_t d1 = __shfl_sync(0xFFFFFFFFu, desc1, ks);
+                const int flags = d1 >> 24;
+                if (flags & 1) {
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) A[i][0] = A[i][1] = A[i][2] = A[i][3] = 0.f;
+                }
+                const uint32_t bq0 = __ldg(qfp + ks * 64), bq1 = __ldg(qfp + ks * 64 + 4);
+                switch (d1 & 0xFF) {
+                case 1: qk_step<1>(tile, d0, d1, g8, c, bq0, bq1, pools, lut, A); break;
+                case 2: qk_step<2>(tile, d0, d1, g8, c, bq0, bq1, pools, lut, A); break;
+                case 3: qk_step<3>(tile, d0, d1, g8, c, bq0, bq1, pools, lut, A); break;
+                case 4: qk_step<4>(tile, d0, d1, g8, c, bq0, bq1, pools, lut, A); break;
+                case 5: qk_step<5>(tile, d0, d1, g8, c, bq0, bq1, pools, lut, A); break;
+                case 6: qk_step<6>(tile, d0, d1, g8, c, bq0, bq1, pools, lut, A); break;
+                case 7: qk_step<7>(tile, d0, d1, g8, c, bq0, bq1, pools, lut, A); break;
+                default: qk_step<8>(tile, d0, d1, g8, c, bq0, bq1, pools, lut, A); break;
+                }
+                if (flags & 2) {   // group finished: scale by the fp16 group norms (fp32, on the accumulators)
+                    const uint4 *np = reinterpret_cast<const uint4 *>(
+                        reinterpret_cast<const unsigned char *>(tile) + knorm_off + 256 * (flags >> 4) + g8 * 32);
+                    const uint4 n0 = np[0], n1 = np[1];
+                    const uint32_t nw[8] = {n0.x, n0.y, n0.z, n0.w, n1.x, n1.y, n1.z, n1.w};
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const float2 nf = __half22float2(*reinterpret_cast<const __half2 *>(&nw[i]));
+                        Sc[i][0] = fmaf(nf.x, A[i][0], Sc[i][0]);
+                        Sc[i][1] = fmaf(nf.x, A[i][1], Sc[i][1]);
+                        Sc[i][2] = fmaf(nf.y, A[i][2], Sc[i][2]);
+                        Sc[i][3] = fmaf(nf.y, A[i][3], Sc[i][3]);
+                    }
+                }
+            }
+            __syncwarp();
+            if (lane == 0 && x + 1 < seg_end) issue(x + 1, true, false);    // K half of the next tile (same layout only)
+
+            // ======== mask the ragged tail, online softmax (log2 domain)
+            const int n_valid = (int)min((int64_t)kTile, slen - (int64_t)t * kTile);
+            if (n_valid < kTile) {
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    if (16 * i + g8 >= n_valid) Sc[i][0] = Sc[i][1] = -INFINITY;
+                    if (16 * i + 8 + g8 >= n_valid) Sc[i][2] = Sc[i][3] = -INFINITY;
+                }
+            }
+            float mx0 = -INFINITY, mx1 = -INFINITY;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                mx0 = fmaxf(mx0, fmaxf(Sc[i][0], Sc[i][2]));
+                mx1 = fmaxf(mx1, fmaxf(Sc[i][1], Sc[i][3]));
+            }
+#pragma unroll
+            for (int o = 4; o < 32; o <<= 1) {
+                mx0 = fmaxf(mx0, __shfl_xor_sync(0xFFFFFFFFu, mx0, o));
+                mx1 = fmaxf(mx1, __shfl_xor_sync(0xFFFFFFFFu, mx1, o));
+            }
+            const float mn0 = fmaxf(st.m[0], mx0), mn1 = fmaxf(st.m[1], mx1);
+            const float al0 = fast_exp2(st.m[0] - mn0), al1 = fast_exp2(st.m[1] - mn1);
+            st.m[0] = mn0; st.m[1] = mn1;
+            float ls0 = 0.f, ls1 = 0.f;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                Sc[i][0] = fast_exp2(Sc[i][0] - mn0); Sc[i][2] = fast_exp2(Sc[i][2] - mn0);
+                Sc[i][1] = fast_exp2(Sc[i][1] - mn1); Sc[i][3] = fast_exp2(Sc[i][3] - mn1);
+                ls0 += Sc[i][0] + Sc[i][2];
+                ls1 += Sc[i][1] + Sc[i][3];
+            }
+            st.l[0] = fmaf(st.l[0], al0, ls0);
+            st.l[1] = fmaf(st.l[1], al1, ls1);
+#pragma unroll
+            for (int J = 0; J < 8; ++J) { st.O[J][0] *= al0; st.O[J][2] *= al0; st.O[J][1] *= al1; st.O[J][3] *= al1; }
+
+            // ======== P * (V norm) -> fp16 B fragments (8x8 transposes), then PV
+            mbar_wait(vbar, vphase);
+            vphase ^= 1;
+            uint32_t bP[8][2];
+            {
+                const uint4 *np = reinterpret_cast<const uint4 *>(reinterpret_cast<const unsigned char *>(tile) + vnorm_off + g8 * 32);
+                const uint4 n0 = np[0], n1 = np[1];
+                const uint32_t nw[8] = {n0.x, n0.y, n0.z, n0.w, n1.x, n1.y, n1.z, n1.w};
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    const float2 nf = __half22float2(*reinterpret_cast<const __half2 *>(&nw[i]));
+                    bP[i][0] = movmatrix_trans(pack_half2(Sc[i][0] * nf.x, Sc[i][1] * nf.x));
+                    bP[i][1] = movmatrix_trans(pack_half2(Sc[i][2] * nf.y, Sc[i][3] * nf.y));
+                }
+            }
+            const uint32_t *vcodes = tile + (vcode_off >> 2);
+            switch (b_v) {
+            case 1: pv_tile<1>(vcodes, lane, bP, pools, lut, st.O); break;
+            case 2: pv_tile<2>(vcodes, lane, bP, pools, lut, st.O); break;
+            case 3: pv_tile<3>(vcodes, lane, bP, pools, lut, st.O); break;
+            case 4: pv_tile<4>(vcodes, lane, bP, pools, lut, st.O); break;
+            case 5: pv_tile<5>(vcodes, lane, bP, pools, lut, st.O); break;
+            case 6: pv_tile<6>(vcodes, lane, bP, pools, lut, st.O); break;
+            case 7: pv_tile<7>(vcodes, lane, bP, pools, lut, st.O); break;
+            default: pv_tile<8>(vcodes, lane, bP, pools, lut, st.O); break;
+            }
+            __syncwarp();
+            if (lane == 0 && x + 1 < x_end) issue(x + 1, x + 1 >= seg_end, true);   // V half (and K when the layout changes)
+        }
+
+        // ---------------- write this warp's partial for the pair: slot = warp + pair (unique, see combine)
+        float l0 = st.l[0], l1 = st.l[1];
+#pragma unroll
+        for (int o = 4; o < 32; o <<= 1) {
+            l0 += __shfl_xor_sync(0xFFFFFFFFu, l0, o);
+            l1 += __shfl_xor_sync(0xFFFFFFFFu, l1, o);
+        }
+        float *rec = P.partials + (size_t)(gw + tp.pair) * kPartialFloats;
+        const int n0 = 2 * c, n1 = 2 * c + 1;
+        if (n0 < P.G) {
+            float *r0 = rec + n0 * 130;
+            if (g8 == 0) { r0[0] = st.m[0]; r0[1] = l0; }
+#pragma unroll
+            for (int J = 0; J < 8; ++J) { r0[2 + 16 * J + g8] = st.O[J][0]; r0[2 + 16 * J + 8 + g8] = st.O[J][2]; }
+        }
+        if (n1 < P.G) {
+            float *r1 = rec + n1 * 130;
+            if (g8 == 0) { r1[0] = st.m[1]; r1[1] = l1; }
+#pragma unroll
+            for (int J = 0; J < 8; ++J) { r1[2 + 16 * J + g8] = st.O[J][1]; r1[2 + 16 * J + 8 + g8] = st.O[J][3]; }
+        }
+    }
+}
+
+// ---------------------------------------------------------------- a6: exact LSE merge + V de-rotation
+// M = max_w m_w; l = sum_w l_w 2^(m_w-M); o' = sum_w acc_w 2^(m_w-M) / l, then
+// out = Pi^(128)^T o' / sqrt(128)  (dequantisation of V, applied once because it is linear) -> bf16.
+__global__ void __launch_bounds__(128)
+combine_kernel(const float *__restrict__ partials, const int32_t *__restrict__ seq_len,
+               const float *__restrict__ rot128, int n_layers, int batch, int Hkv, int G, int64_t n_cap,
+               int n_warps, __nv_bfloat16 *__restrict__ out)
+{
+    __shared__ int pre[kMaxBatch + 1];
+    __shared__ float o[kDh];
+    const int pair = blockIdx.x / G, n = blockIdx.x % G;
+    const int h = pair % Hkv, lb = pair / Hkv, b = lb % batch, l = lb / batch;
+    const int d = threadIdx.x;
+    if (d == 0) build_prefix(seq_len, batch, n_cap * kTile, pre);
+    __syncthreads();
+    const Sched S = make_sched(n_layers, batch, Hkv, pre, n_warps);
+    const int tiles_b = pre[b + 1] - pre[b];
+    __nv_bfloat16 *dst = out + ((size_t)lb * Hkv * G + h * G + n) * kDh;
+    if (tiles_b == 0) { dst[d] = __float2bfloat16(0.f); return; }
+    const int start = l * (Hkv * S.tiles_sum) + pre[b] * Hkv + h * tiles_b;
+    const int w0 = start / S.per_warp, w1 = (start + tiles_b - 1) / S.per_warp;
+    float Mx = -INFINITY;
+    for (int w = w0; w <= w1; ++w) Mx = fmaxf(Mx, partials[(size_t)(w + pair) * kPartialFloats + n * 130]);
+    float acc = 0.f, lsum = 0.f;
+    for (int w = w0; w <= w1; ++w) {
+        const float *rec = partials + (size_t)(w + pair) * kPartialFloats + n * 130;
+        const float f = exp2f(rec[0] - Mx);
+        lsum = fmaf(rec[1], f, lsum);
+        acc = fmaf(rec[2 + d], f, acc);
+    }
+    o[d] = acc / lsum;
+    __syncthreads();
+    float r = 0.f;
+#pragma unroll 8
+    for (int j = 0; j < kDh; ++j) r = fmaf(__ldg(rot128 + j * kDh + d), o[j], r);
+    dst[d] = __float2bfloat16(r * 0.08838834764831845f);     // 1/sqrt(128)
+}
+
+// ---------------------------------------------------------------- host side
+static int pick_warps(int buf_bytes)
+{
+    const int avail = 227 * 1024 - 2128 - 512;
+    const int cands[4] = {16, 12, 8, 4};
+    for (int i = 0; i < 4; ++i)
+        if ((size_t)cands[i] * (buf_bytes + 16) <= (size_t)avail) return cands[i];
+    return 0;
+}
+static size_t decode_smem(int W, int buf_bytes) { return 2128 + 16 * W + 128 + (size_t)W * buf_bytes; }
+
+size_t decode_ws_bytes(const bgtq_layout *lay, int batch, int n_layers)
+{
+    const size_t pairs = (size_t)n_layers * batch * lay->n_kv_heads;
+    const size_t qf = pairs * kQfHalves * sizeof(__half);
+    const size_t slots = (size_t)lay->sm_count * kMaxWarpsPerSM + pairs;
+    return qf + slots * kPartialFloats * sizeof(float);
+}
+
+template <int W>
+static int launch_decode_w(const DecodeParams &P, int grid, size_t smem, cudaStream_t st)
+{
+    CUDA_TRY(cudaFuncSetAttribute(decode_kernel<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    decode_kernel<W><<<grid, W * 32, smem, st>>>(P);
+    return BGTQ_OK;
+}
+
+int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *cache, const void *q,
+                  const int32_t *seq_len, int batch, int64_t max_tokens, float scale, void *out,
+                  void *ws, size_t, cudaStream_t st)
+{
+    if (batch > kMaxBatch) { set_error("bgtq_decode_attention: batch > 256"); return BGTQ_EINVAL; }
+    const int Hkv = lay->n_kv_heads, Hq = lay->n_q_heads, G = Hq / Hkv;
+    const int64_t n_cap = (max_tokens + kTile - 1) / kTile;
+    if ((double)n_layers * batch * Hkv * (double)n_cap >= 2.0e9) { set_error("bgtq_decode_attention: too many tiles for one call"); return BGTQ_EINVAL; }
+    const int pairs = n_layers * batch * Hkv;
+    __half *qf = reinterpret_cast<__half *>(ws);
+    float *partials = reinterpret_cast<float *>(reinterpret_cast<unsigned char *>(ws) + (size_t)pairs * kQfHalves * sizeof(__half));
+    const HeadMeta *metas = lay->d_meta + (size_t)layer0 * Hkv;
+
+    qfold_kernel<<<pairs, 128, 0, st>>>(metas, lay->d_rot_t, (const __nv_bfloat16 *)q, batch, Hkv, Hq,
+                                        scale * 1.4426950408889634f, qf);
+    count_launch();
+    CUDA_TRY(cudaGetLastError());
+
+    const int buf_bytes = (lay->max_stride + 127) / 128 * 128;
+    const int W = pick_warps(buf_bytes);
+    if (!W) { set_error("bgtq_decode_attention: tile does not fit shared memory"); return BGTQ_EINVAL; }
+    DecodeParams P;
+    P.metas = metas; P.cache = (const uint8_t *)cache; P.qf = qf; P.seq_len = seq_len; P.cb16 = lay->d_cb16;
+    P.partials = partials; P.n_cap = n_cap; P.n_layers = n_layers; P.batch = batch; P.Hkv = Hkv; P.G = G;
+    P.buf_bytes = buf_bytes;
+    const int grid = lay->sm_count;
+    const size_t smem = decode_smem(W, buf_bytes);
+    int rc;
+    switch (W) {
+    case 16: rc = launch_decode_w<16>(P, grid, smem, st); break;
+    case 12: rc = launch_decode_w<12>(P, grid, smem, st); break;
+    case 8: rc = launch_decode_w<8>(P, grid, smem, st); break;
+    default: rc = launch_decode_w<4>(P, grid, smem, st); break;
+    }
+    if (rc != BGTQ_OK) return rc;
+    count_launch();
+    CUDA_TRY(cudaGetLastError());
+
+    combine_kernel<<<pairs * G, 128, 0, st>>>(partials, seq_len, lay->d_rot + rot_offset(kDh), n_layers, batch,
+                                              Hkv, G, n_cap, grid * W, (__nv_bfloat16 *)out);
+    count_launch();
+    CUDA_TRY(cudaGetLastError());
+    return BGTQ_OK;
+}
+
+// ---------------------------------------------------------------- test hook: the kernel's unpack routine
+template <int B>
+__device__ void debug_decode_b(const uint32_t *words, const uint32_t *pools, const uint16_t *lut, float *values)
+{
+    const int lane = threadIdx.x;
+    uint32_t w[B], h[16];
+    for (int i = 0; i < B; ++i) w[i] = words[i * 32 + lane];
+    decode_unit<B>(w, pools, lut, h);
+    for (int j = 0; j < 16; ++j) {
+        const float2 f = __half22float2(*reinterpret_cast<const __half2 *>(&h[j]));
+        values[lane * 32 + 2 * j] = f.x;
+        values[lane * 32 + 2 * j + 1] = f.y;
+    }
+}
+__global__ void debug_decode_kernel(int b, const uint32_t *words, const uint16_t *cb16, float *values)
+{
+    __shared__ uint16_t lut[512];
+    __shared__ uint32_t pools[16];
+    for (int i = threadIdx.x; i < 511; i += 32) lut[i] = cb16[i];
+    __syncwarp();
+    if (threadIdx.x == 0) build_pools(lut, pools);
+    __syncwarp();
+    switch (b) {
+    case 1: debug_decode_b<1>(words, pools, lut, values); break;
+    case 2: debug_decode_b<2>(words, pools, lut, values); break;
+    case 3: debug_decode_b<3>(words, pools, lut, values); break;
+    case 4: debug_decode_b<4>(words, pools, lut, values); break;
+    case 5: debug_decode_b<5>(words, pools, lut, values); break;
+    case 6: debug_decode_b<6>(words, pools, lut, values); break;
+    case 7: debug_decode_b<7>(words, pools, lut, values); break;
+    default: debug_decode_b<8>(words, pools, lut, values); break;
+    }
+}
+
+int debug_decode_unit(int b, const uint32_t *words, float *values)
+{
+    uint32_t *dw = nullptr; float *dv = nullptr; uint16_t *dcb = nullptr;
+    std::vector<uint16_t> cb16(512, 0);
+    for (int bb = 0; bb <= BGTQ_MAX_WIDTH; ++bb) {
+        double lv[256];
+        codebook_levels(bb, lv);
+        for (int k = 0; k < (1 << bb); ++k) cb16[(1 << bb) - 1 + k] = __half_as_ushort(__double2half(lv[k]));
+    }
+    cudaError_t e = cudaMalloc(&dw, b * 32 * 4);
+    if (e == cudaSuccess) e = cudaMalloc(&dv, 32 * 32 * 4);
+    if (e == cudaSuccess) e = cudaMalloc(&dcb, 512 * 2);
+    if (e == cudaSuccess) e = cudaMemcpy(dw, words, b * 32 * 4, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(dcb, cb16.data(), 512 * 2, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) { debug_decode_kernel<<<1, 32>>>(b, dw, dcb, dv); count_launch(); e = cudaGetLastError(); }
+    if (e == cudaSuccess) e = cudaMemcpy(values, dv, 32 * 32 * 4, cudaMemcpyDeviceToHost);
+    cudaFree(dw); cudaFree(dv); cudaFree(dcb);
+    if (e != cudaSuccess) return cuda_fail(e, "bgtq_debug_decode_unit");
+    return BGTQ_OK;
+}
+
+}  // namespace bgtq

@@ -1,0 +1,328 @@
+// bgtq_host.cu -- host side of the C-ABI: argument checks, layout build, host
+// allocator (a2), sizes.  No arithmetic of the hot path runs here except Alg. 1's host variant.
+#include <atomic>
+#include <cmath>
+#include <cstring>
+#include <new>
+
+#include <cuda_fp16.h>
+
+#include "bgtq_internal.h"
+
+namespace bgtq {
+
+static thread_local std::string g_err;
+static std::atomic<int64_t> g_launches{0};
+
+void set_error(const std::string &msg) { g_err = msg; }
+int cuda_fail(cudaError_t e, const char *what)
+{
+    set_error(std::string(what) + ": " + cudaGetErrorString(e));
+    return BGTQ_ECUDA;
+}
+void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+
+}  // namespace bgtq
+
+using namespace bgtq;
+
+#define FAIL(code, msg) do { set_error(msg); return (code); } while (0)
+#define CUDA_TRY(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) return cuda_fail(e_, #expr); } while (0)
+
+extern "C" const char *bgtq_last_error(void) { return g_err.c_str(); }
+extern "C" int64_t bgtq_launch_count(void) { return g_launches.load(); }
+
+extern "C" int bgtq_codebook(int b, float *levels)
+{
+    if (b < 0 || b > BGTQ_MAX_WIDTH || !levels) FAIL(BGTQ_EINVAL, "bgtq_codebook: b in 0..8, levels != NULL");
+    double tmp[256];
+    codebook_levels(b, tmp);
+    for (int k = 0; k < (1 << b); ++k) levels[k] = (float)tmp[k];
+    return BGTQ_OK;
+}
+
+// ------------------------------------------------------------------ a2, host variant
+// Alg. 1 with a linear arg-max; key = 3/4 * s * 4^-b in fp64 (exact: a power-of-two
+// scaling of an fp32 value); ties -> smallest index (Q4); zero scores served last in index order (Q5).
+static int allocate_host(const float *scores, int n_heads, int L, int b_min, int b_max, int B,
+                         uint8_t *bits)
+{
+    for (int h = 0; h < n_heads; ++h) {
+        const float *s = scores + (size_t)h * L;
+        uint8_t *b = bits + (size_t)h * L;
+        for (int i = 0; i < L; ++i) {
+            if (!(s[i] >= 0.0f) || std::isinf(s[i])) FAIL(BGTQ_EINVAL, "bgtq_allocate: scores must be finite and >= 0");
+            b[i] = (uint8_t)b_min;
+        }
+        for (int extra = B - L * b_min; extra > 0; --extra) {
+            int best = -1;
+            double bestkey = -1.0;
+            for (int i = 0; i < L; ++i) {
+                if (b[i] >= b_max) continue;
+                double key = 0.75 * std::ldexp((double)s[i], -2 * (int)b[i]);
+                if (key > bestkey) { bestkey = key; best = i; }
+            }
+            if (best < 0) break;
+            b[best] += 1;
+        }
+    }
+    return BGTQ_OK;
+}
+
+extern "C" int bgtq_allocate(const float *scores, int n_heads, int n_blocks, int b_min, int b_max,
+                             int total_bits_B, uint8_t *bits, int on_device, void *stream)
+{
+    if (!scores || !bits || n_heads < 0 || n_blocks <= 0) FAIL(BGTQ_EINVAL, "bgtq_allocate: null pointer or bad shape");
+    if (b_min < 0 || b_max > BGTQ_MAX_WIDTH || b_min > b_max) FAIL(BGTQ_EINVAL, "bgtq_allocate: need 0 <= b_min <= b_max <= 8");
+    if (total_bits_B < n_blocks * b_min || total_bits_B > n_blocks * b_max)
+        FAIL(BGTQ_EBUDGET, "bgtq_allocate: B outside [L*b_min, L*b_max]");
+    if (n_heads == 0) return BGTQ_OK;
+    if (!on_device) return allocate_host(scores, n_heads, n_blocks, b_min, b_max, total_bits_B, bits);
+    if (n_blocks > 1024) FAIL(BGTQ_EINVAL, "bgtq_allocate: device path supports n_blocks <= 1024");
+    return launch_allocate(scores, n_heads, n_blocks, b_min, b_max, total_bits_B, bits, (cudaStream_t)stream);
+}
+
+// ------------------------------------------------------------------ a1 wrapper
+extern "C" size_t bgtq_block_energy_workspace_bytes(int n_q_heads, int n_kv_heads, int d_h)
+{
+    if (n_q_heads <= 0 || n_kv_heads <= 0 || d_h <= 0) return 0;
+    return block_energy_ws_bytes(n_q_heads, n_kv_heads, d_h);
+}
+
+extern "C" int bgtq_block_energy(const void *q, int64_t n_q, const void *k, int64_t n_k, int dt,
+                                 int n_q_heads, int n_kv_heads, int d_h, int pairing, int kind,
+                                 float *scores, float *eq_out, float *ek_out, void *workspace,
+                                 size_t workspace_bytes, void *stream)
+{
+    if (!scores || !workspace) FAIL(BGTQ_EINVAL, "bgtq_block_energy: null scores/workspace");
+    if (n_q < 0 || n_k < 0 || (n_q > 0 && !q) || (n_k > 0 && !k)) FAIL(BGTQ_EINVAL, "bgtq_block_energy: bad q/k");
+    if (dt != BGTQ_F32 && dt != BGTQ_BF16) FAIL(BGTQ_EINVAL, "bgtq_block_energy: dtype");
+    if (n_kv_heads <= 0 || n_q_heads <= 0 || n_q_heads % n_kv_heads) FAIL(BGTQ_EINVAL, "bgtq_block_energy: heads");
+    if (d_h <= 0 || d_h % 8 || d_h > 1024) FAIL(BGTQ_EINVAL, "bgtq_block_energy: d_h must be a multiple of 8, <= 1024");
+    if (pairing != BGTQ_PAIR_HALF && pairing != BGTQ_PAIR_INTERLEAVED) FAIL(BGTQ_EINVAL, "bgtq_block_energy: pairing");
+    if (kind < 0 || kind > BGTQ_Q_ONLY) FAIL(BGTQ_EINVAL, "bgtq_block_energy: score kind");
+    if (workspace_bytes < block_energy_ws_bytes(n_q_heads, n_kv_heads, d_h)) FAIL(BGTQ_EWORKSPACE, "bgtq_block_energy: workspace too small");
+    return launch_block_energy(q, n_q, k, n_k, dt, n_q_heads, n_kv_heads, d_h, pairing, kind, scores,
+                               eq_out, ek_out, workspace, workspace_bytes, (cudaStream_t)stream);
+}
+
+// ------------------------------------------------------------------ a3: layout build
+// Grouping, tile geometry and the k-step program of DESIGN.md section 4.
+static void build_head_meta(const uint8_t *bits, int d_h, int b_v, int pairing, HeadMeta &m)
+{
+    std::memset(&m, 0, sizeof(m));
+    const int L = d_h / 2;
+    m.b_v = b_v;
+    int ng = 0, kdim = 0, off = 0, nks = 0;
+    for (int w = 1; w <= BGTQ_MAX_WIDTH; ++w) {
+        int cnt = 0;
+        for (int i = 0; i < L; ++i)
+            if (bits[i] == w) {
+                int a = pairing == BGTQ_PAIR_HALF ? i : 2 * i;
+                int b = pairing == BGTQ_PAIR_HALF ? i + L : 2 * i + 1;
+                m.coords[kdim + cnt++] = (uint8_t)a;
+                m.coords[kdim + cnt++] = (uint8_t)b;
+            }
+        if (!cnt) continue;
+        m.gb[ng] = (uint8_t)w;
+        m.gm[ng] = (uint16_t)cnt;
+        m.gstart[ng] = (uint16_t)kdim;
+        m.goff[ng] = off;
+        // half-steps of 8 coordinates; full one = 128*w bytes, trailing partial (r coords) = 16*r*w
+        int n_half = (cnt + 7) / 8;
+        for (int j = 0; j < n_half; j += 2) {
+            KStep &ks = m.ksteps[nks++];
+            int r0 = cnt - 8 * j >= 8 ? 8 : cnt - 8 * j;
+            ks.off0 = (uint16_t)(off + j * 128 * w);
+            ks.nc0 = (uint8_t)(r0 / 2);
+            if (j + 1 < n_half) {
+                int r1 = cnt - 8 * (j + 1) >= 8 ? 8 : cnt - 8 * (j + 1);
+                ks.off1 = (uint16_t)(off + (j + 1) * 128 * w);
+                ks.nc1 = (uint8_t)(r1 / 2);
+            } else {
+                ks.off1 = 0xFFFF;
+                ks.nc1 = 0;
+            }
+            ks.b = (uint8_t)w;
+            ks.flags = (uint8_t)((j == 0 ? 1 : 0) | (j + 2 >= n_half ? 2 : 0) | (ng << 4));
+        }
+        off += 16 * cnt * w;
+        kdim += cnt;
+        ++ng;
+    }
+    m.n_groups = ng;
+    m.kdim = kdim;
+    m.n_ksteps = nks;
+    m.kcode_bytes = off;
+    m.knorm_off = off;
+    m.vnorm_off = off + 256 * ng;
+    m.vcode_off = m.vnorm_off + 256;
+    m.tile_stride = m.vcode_off + 16 * d_h * b_v;
+}
+
+extern "C" int bgtq_layout_create(const uint8_t *bits, int n_layers, int n_kv_heads, int n_q_heads,
+                                  int d_h, int b_v, int pairing, const float *rotations,
+                                  bgtq_layout **out)
+{
+    if (!bits || !rotations || !out) FAIL(BGTQ_EINVAL, "bgtq_layout_create: null pointer");
+    if (d_h != kDh) FAIL(BGTQ_EINVAL, "bgtq_layout_create: d_h must be 128");
+    if (n_layers <= 0 || n_kv_heads <= 0 || n_q_heads <= 0 || n_q_heads % n_kv_heads)
+        FAIL(BGTQ_EINVAL, "bgtq_layout_create: bad layer/head counts");
+    if (n_q_heads / n_kv_heads > 8) FAIL(BGTQ_EINVAL, "bgtq_layout_create: GQA group size must be <= 8");
+    if (b_v < 1 || b_v > BGTQ_MAX_WIDTH) FAIL(BGTQ_EINVAL, "bgtq_layout_create: b_v in 1..8");
+    if (pairing != BGTQ_PAIR_HALF && pairing != BGTQ_PAIR_INTERLEAVED) FAIL(BGTQ_EINVAL, "bgtq_layout_create: pairing");
+    const int L = d_h / 2;
+    for (size_t i = 0; i < (size_t)n_layers * n_kv_heads * L; ++i)
+        if (bits[i] > BGTQ_MAX_WIDTH) FAIL(BGTQ_EINVAL, "bgtq_layout_create: widths must be 0..8");
+
+    bgtq_layout *lay = new (std::nothrow) bgtq_layout();
+    if (!lay) FAIL(BGTQ_EINVAL, "bgtq_layout_create: out of host memory");
+    lay->n_layers = n_layers; lay->n_kv_heads = n_kv_heads; lay->n_q_heads = n_q_heads;
+    lay->d_h = d_h; lay->b_v = b_v; lay->pairing = pairing;
+    lay->d_meta = nullptr; lay->d_rot = nullptr; lay->d_rot_t = nullptr; lay->d_cb16 = nullptr; lay->d_cb64 = nullptr;
+    lay->meta.resize((size_t)n_layers * n_kv_heads);
+    int64_t prefix = 0;
+    lay->max_stride = 0;
+    for (int l = 0; l < n_layers; ++l) {
+        int64_t lsum = 0;
+        for (int h = 0; h < n_kv_heads; ++h) {
+            HeadMeta &m = lay->meta[(size_t)l * n_kv_heads + h];
+            build_head_meta(bits + ((size_t)l * n_kv_heads + h) * L, d_h, b_v, pairing, m);
+            m.layer_prefix = prefix;
+            m.head_prefix = lsum;
+            lsum += m.tile_stride;
+            if (m.tile_stride > lay->max_stride) lay->max_stride = m.tile_stride;
+        }
+        for (int h = 0; h < n_kv_heads; ++h) lay->meta[(size_t)l * n_kv_heads + h].layer_sum = lsum;
+        prefix += lsum;
+    }
+    lay->total_stride_sum = prefix;
+
+    // device copies: metadata, rotation table (both orientations), codebooks
+    const int64_t rot_n = rot_offset(d_h + 2);
+    std::vector<float> rot_t((size_t)rot_n);
+    for (int m = 2; m <= d_h; m += 2) {
+        const float *P = rotations + rot_offset(m);
+        float *T = rot_t.data() + rot_offset(m);
+        for (int j = 0; j < m; ++j)
+            for (int k = 0; k < m; ++k) T[(size_t)k * m + j] = P[(size_t)j * m + k];
+    }
+    std::vector<uint16_t> cb16(512, 0);
+    std::vector<double> cb64(512, 0.0);
+    for (int b = 0; b <= BGTQ_MAX_WIDTH; ++b) {
+        double lv[256];
+        codebook_levels(b, lv);
+        for (int k = 0; k < (1 << b); ++k) {
+            cb64[(1 << b) - 1 + k] = lv[k];
+            __half hv = __double2half(lv[k]);
+            uint16_t u;
+            std::memcpy(&u, &hv, 2);
+            cb16[(1 << b) - 1 + k] = u;
+        }
+    }
+    cudaError_t e = cudaSuccess;
+    int dev = 0;
+    if (e == cudaSuccess) e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&lay->sm_count, cudaDevAttrMultiProcessorCount, dev);
+    if (e == cudaSuccess) e = cudaMalloc(&lay->d_meta, lay->meta.size() * sizeof(HeadMeta));
+    if (e == cudaSuccess) e = cudaMalloc(&lay->d_rot, rot_n * sizeof(float));
+    if (e == cudaSuccess) e = cudaMalloc(&lay->d_rot_t, rot_n * sizeof(float));
+    if (e == cudaSuccess) e = cudaMalloc(&lay->d_cb16, 512 * sizeof(uint16_t));
+    if (e == cudaSuccess) e = cudaMalloc(&lay->d_cb64, 512 * sizeof(double));
+    if (e == cudaSuccess) e = cudaMemcpy(lay->d_meta, lay->meta.data(), lay->meta.size() * sizeof(HeadMeta), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(lay->d_rot, rotations, rot_n * sizeof(float), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(lay->d_rot_t, rot_t.data(), rot_n * sizeof(float), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(lay->d_cb16, cb16.data(), 512 * sizeof(uint16_t), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(lay->d_cb64, cb64.data(), 512 * sizeof(double), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) {
+        bgtq_layout_destroy(lay);
+        return cuda_fail(e, "bgtq_layout_create");
+    }
+    *out = lay;
+    return BGTQ_OK;
+}
+
+extern "C" void bgtq_layout_destroy(bgtq_layout *lay)
+{
+    if (!lay) return;
+    cudaFree(lay->d_meta); cudaFree(lay->d_rot); cudaFree(lay->d_rot_t);
+    cudaFree(lay->d_cb16); cudaFree(lay->d_cb64);
+    delete lay;
+}
+
+static inline int64_t n_cap_tiles(int64_t max_tokens) { return (max_tokens + kTile - 1) / kTile; }
+
+extern "C" size_t bgtq_cache_bytes(const bgtq_layout *lay, int batch, int64_t max_tokens)
+{
+    if (!lay || batch <= 0 || max_tokens <= 0) return 0;
+    return (size_t)(n_cap_tiles(max_tokens) * batch * lay->total_stride_sum);
+}
+extern "C" double bgtq_token_bytes(const bgtq_layout *lay, int layer, int kv_head)
+{
+    if (!lay || layer < 0 || layer >= lay->n_layers || kv_head < 0 || kv_head >= lay->n_kv_heads) return 0.0;
+    return lay->meta[(size_t)layer * lay->n_kv_heads + kv_head].tile_stride / (double)kTile;
+}
+extern "C" int64_t bgtq_tile_stride(const bgtq_layout *lay, int layer, int kv_head)
+{
+    if (!lay || layer < 0 || layer >= lay->n_layers || kv_head < 0 || kv_head >= lay->n_kv_heads) return -1;
+    return lay->meta[(size_t)layer * lay->n_kv_heads + kv_head].tile_stride;
+}
+extern "C" int64_t bgtq_region_offset(const bgtq_layout *lay, int layer, int seq, int kv_head,
+                                      int batch, int64_t max_tokens)
+{
+    if (!lay || layer < 0 || layer >= lay->n_layers || kv_head < 0 || kv_head >= lay->n_kv_heads ||
+        seq < 0 || seq >= batch || max_tokens <= 0) return -1;
+    const HeadMeta &m = lay->meta[(size_t)layer * lay->n_kv_heads + kv_head];
+    return n_cap_tiles(max_tokens) * ((int64_t)batch * m.layer_prefix + (int64_t)seq * m.layer_sum + m.head_prefix);
+}
+extern "C" size_t bgtq_workspace_bytes(const bgtq_layout *lay, int batch, int n_layers_per_call)
+{
+    if (!lay || batch <= 0 || n_layers_per_call <= 0) return 0;
+    return decode_ws_bytes(lay, batch, n_layers_per_call);
+}
+
+// ------------------------------------------------------------------ a4 / a5 wrappers
+extern "C" int bgtq_quantize_append(const bgtq_layout *lay, int layer, void *cache, const void *k_new,
+                                    const void *v_new, int dt, int batch, int n_new, int32_t *seq_len,
+                                    int advance_seq_len, int64_t max_tokens, void *stream)
+{
+    if (!lay || !cache || !seq_len) FAIL(BGTQ_EINVAL, "bgtq_quantize_append: null pointer");
+    if (layer < 0 || layer >= lay->n_layers) FAIL(BGTQ_EINVAL, "bgtq_quantize_append: layer out of range");
+    if (dt != BGTQ_F32 && dt != BGTQ_BF16) FAIL(BGTQ_EINVAL, "bgtq_quantize_append: dtype");
+    if (batch <= 0 || n_new < 0 || max_tokens <= 0) FAIL(BGTQ_EINVAL, "bgtq_quantize_append: batch/n_new/max_tokens");
+    if (n_new > max_tokens) FAIL(BGTQ_ECAPACITY, "bgtq_quantize_append: n_new exceeds max_tokens");
+    if (n_new == 0) return BGTQ_OK;
+    if (!k_new || !v_new) FAIL(BGTQ_EINVAL, "bgtq_quantize_append: null k_new/v_new");
+    return launch_quantize_append(lay, layer, cache, k_new, v_new, dt, batch, n_new, seq_len,
+                                  advance_seq_len, max_tokens, (cudaStream_t)stream);
+}
+
+extern "C" int bgtq_decode_attention_layers(const bgtq_layout *lay, int layer0, int n_layers,
+                                            const void *cache, const void *q, const int32_t *seq_len,
+                                            int batch, int64_t max_tokens, float softmax_scale,
+                                            void *out, void *workspace, size_t workspace_bytes,
+                                            void *stream)
+{
+    if (!lay || !cache || !q || !seq_len || !out || !workspace) FAIL(BGTQ_EINVAL, "bgtq_decode_attention: null pointer");
+    if (layer0 < 0 || n_layers <= 0 || layer0 + n_layers > lay->n_layers) FAIL(BGTQ_EINVAL, "bgtq_decode_attention: layer range");
+    if (batch <= 0 || max_tokens <= 0) FAIL(BGTQ_EINVAL, "bgtq_decode_attention: batch/max_tokens");
+    if (!(softmax_scale > 0.0f) || std::isinf(softmax_scale)) FAIL(BGTQ_EINVAL, "bgtq_decode_attention: softmax_scale must be finite and > 0");
+    if (workspace_bytes < decode_ws_bytes(lay, batch, n_layers)) FAIL(BGTQ_EWORKSPACE, "bgtq_decode_attention: workspace too small");
+    return launch_decode(lay, layer0, n_layers, cache, q, seq_len, batch, max_tokens, softmax_scale,
+                         out, workspace, workspace_bytes, (cudaStream_t)stream);
+}
+
+extern "C" int bgtq_decode_attention(const bgtq_layout *lay, int layer, const void *cache, const void *q,
+                                     const int32_t *seq_len, int batch, int64_t max_tokens,
+                                     float softmax_scale, void *out, void *workspace,
+                                     size_t workspace_bytes, void *stream)
+{
+    return bgtq_decode_attention_layers(lay, layer, 1, cache, q, seq_len, batch, max_tokens,
+                                        softmax_scale, out, workspace, workspace_bytes, stream);
+}
+
+extern "C" int bgtq_debug_decode_unit(int b, const uint32_t *words, float *values)
+{
+    if (b < 1 || b > BGTQ_MAX_WIDTH || !words || !values) FAIL(BGTQ_EINVAL, "bgtq_debug_decode_unit: bad argument");
+    return debug_decode_unit(b, words, values);
+}

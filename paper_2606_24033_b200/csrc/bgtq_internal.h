@@ -1,0 +1,87 @@
+// bgtq_internal.h -- shared declarations of the library's translation units (not installed).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+
+#include "../../include/bgtq.h"
+
+namespace bgtq {
+
+constexpr int kDh = 128;          // head dimension the kernels are written for
+constexpr int kTile = 128;        // tokens per tile
+constexpr int kMaxGroups = 8;
+constexpr int kMaxKSteps = 16;    // sum_g ceil(m_g/16) <= 8 + 7
+
+// One k16 step of the QK^T product: two half-step units (8 coordinates each) of one group.
+struct KStep {
+    uint16_t off0;     // byte offset of the first unit inside the tile
+    uint16_t off1;     // second unit, 0xFFFF if the group ends after the first
+    uint8_t b;         // code width of the group
+    uint8_t nc0;       // lanes per 8-token row holding data in unit 0 (4 = full, 1..3 partial)
+    uint8_t nc1;       // same for unit 1 (0 if absent)
+    uint8_t flags;     // bit0 first step of its group, bit1 last step; bits 4..7 group index
+};
+
+// Static layout metadata of one (layer, KV head)   ("static layout metadata")
+struct HeadMeta {
+    int32_t n_groups, kdim, n_ksteps, b_v;
+    int32_t tile_stride, kcode_bytes, knorm_off, vnorm_off, vcode_off, pad0;
+    int64_t layer_prefix;   // sum of tile strides of all heads of all earlier layers
+    int64_t layer_sum;      // sum of tile strides of the heads of this layer
+    int64_t head_prefix;    // sum of tile strides of earlier heads of this layer
+    int32_t goff[kMaxGroups];      // byte offset of the group's codes inside the tile
+    uint16_t gm[kMaxGroups];       // coordinates in the group
+    uint16_t gstart[kMaxGroups];   // first grouped-order coordinate of the group
+    uint16_t grot[kMaxGroups];     // unused / reserved
+    uint8_t gb[kMaxGroups];        // width of the group
+    uint8_t coords[kDh];           // grouped order -> original coordinate (Q9)
+    KStep ksteps[kMaxKSteps];
+};
+
+}  // namespace bgtq
+
+struct bgtq_layout {
+    int n_layers, n_kv_heads, n_q_heads, d_h, b_v, pairing;
+    int max_stride;                       // largest tile stride over all heads
+    std::vector<bgtq::HeadMeta> meta;     // host copy, [layer][kv_head]
+    int64_t total_stride_sum;             // sum of tile strides over all (layer, head)
+    bgtq::HeadMeta *d_meta;               // device copy
+    float *d_rot;                         // rotation table, row-major Pi^(m)[j][k]
+    float *d_rot_t;                       // transposed: Pi^(m)[j][k] stored at [k][j]
+    uint16_t *d_cb16;                     // fp16 bits of the 511 codebook levels (C_b at 2^b-1)
+    double *d_cb64;                       // same levels as fp64
+    int sm_count;
+};
+
+namespace bgtq {
+
+void set_error(const std::string &msg);
+int cuda_fail(cudaError_t e, const char *what);
+void count_launch(int n = 1);
+void codebook_levels(int b, double *levels);
+
+__host__ __device__ inline int64_t rot_offset(int m)  // element offset of Pi^(m), m even: sum of m'^2, m' = 2,4,..,m-2
+{
+    const int64_t n = m / 2;
+    return 4 * ((n - 1) * n * (2 * n - 1) / 6);
+}
+
+// implemented in the .cu files
+int launch_block_energy(const void *q, int64_t n_q, const void *k, int64_t n_k, int dt, int Hq,
+                        int Hkv, int d_h, int pairing, int kind, float *scores, float *eq_out,
+                        float *ek_out, void *ws, size_t ws_bytes, cudaStream_t st);
+size_t block_energy_ws_bytes(int Hq, int Hkv, int d_h);
+int launch_allocate(const float *scores, int n_heads, int L, int b_min, int b_max, int B,
+                    uint8_t *bits, cudaStream_t st);
+int launch_quantize_append(const bgtq_layout *lay, int layer, void *cache, const void *k_new,
+                           const void *v_new, int dt, int batch, int n_new, int32_t *seq_len,
+                           int advance, int64_t max_tokens, cudaStream_t st);
+int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *cache,
+                  const void *q, const int32_t *seq_len, int batch, int64_t max_tokens,
+                  float scale, void *out, void *ws, size_t ws_bytes, cudaStream_t st);
+size_t decode_ws_bytes(const bgtq_layout *lay, int batch, int n_layers);
+int debug_decode_unit(int b, const uint32_t *words, float *values);
+
+}  // namespace bgtq

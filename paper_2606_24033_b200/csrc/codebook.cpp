@@ -1,0 +1,122 @@
+// codebook.cpp -- the library's own TQ-MSE scalar codebooks (reading Q7).
+//
+// C_b = Lloyd-Max (MSE-optimal) 2^b-level quantiser of N(0,1): each level is the conditional
+// mean of its cell, thresholds are midpoints.  This is the scalar quantiser whose
+// high-resolution distortion is the paper's C_TQ * 4^-b, C_TQ = sqrt(3)*pi/2.
+// Levels are symmetric, ascending, rounded to fp16 ("shared fp16 codebook").
+//
+// Solver: damped Newton on the centroid equations of the positive half, long double, with a
+// tridiagonal (Thomas) solve.  Shares nothing with oracle/codebook.py; tests compare the two
+// tables value by value.
+#include <cmath>
+#include <cstdint>
+#include <vector>
+
+namespace bgtq {
+
+namespace {
+const long double kInvSqrt2Pi = 0.39894228040143267793994605993438L;
+const long double kSqrt2 = 1.41421356237309504880168872420970L;
+
+long double pdf(long double x) { return std::isinf(x) ? 0.0L : kInvSqrt2Pi * expl(-0.5L * x * x); }
+// P(a < X < b), 0 <= a < b, through erfc so the tail keeps relative accuracy
+long double mass(long double a, long double b)
+{
+    long double ea = erfcl(a / kSqrt2);
+    long double eb = std::isinf(b) ? 0.0L : erfcl(b / kSqrt2);
+    return 0.5L * (ea - eb);
+}
+
+// positive levels c[0..n) of the symmetric 2n-level quantiser
+std::vector<long double> solve_positive(int n)
+{
+    std::vector<long double> c(n), t(n + 1), F(n), lo(n), di(n), up(n), step(n), cn(n);
+    // start: equal-probability cells of the half-normal, level = cell centroid
+    {
+        // invert the half-normal CDF by bisection
+        std::vector<long double> edge(n + 1);
+        edge[0] = 0.0L;
+        for (int k = 1; k < n; ++k) {
+            long double target = (long double)k / n, a = 0.0L, b = 40.0L;
+            for (int it = 0; it < 200; ++it) {
+                long double mid = 0.5L * (a + b);
+                if (1.0L - erfcl(mid / kSqrt2) < target) a = mid; else b = mid;
+            }
+            edge[k] = 0.5L * (a + b);
+        }
+        edge[n] = INFINITY;
+        for (int k = 0; k < n; ++k) c[k] = (pdf(edge[k]) - pdf(edge[k + 1])) / mass(edge[k], edge[k + 1]);
+    }
+    for (int iter = 0; iter < 500; ++iter) {
+        t[0] = 0.0L;
+        for (int k = 1; k < n; ++k) t[k] = 0.5L * (c[k - 1] + c[k]);
+        t[n] = INFINITY;
+        long double resid = 0.0L;
+        for (int k = 0; k < n; ++k) {
+            long double a = t[k], b = t[k + 1];
+            long double P = mass(a, b);
+            long double g = (pdf(a) - pdf(b)) / P;                 // centroid of the cell
+            long double dga = pdf(a) * (g - a) / P;                // d g / d a
+            long double dgb = std::isinf(b) ? 0.0L : pdf(b) * (b - g) / P;   // d g / d b
+            F[k] = c[k] - g;
+            lo[k] = 0.0L; up[k] = 0.0L; di[k] = 1.0L;
+            if (k > 0) { lo[k] -= 0.5L * dga; di[k] -= 0.5L * dga; }
+            if (k + 1 < n) { di[k] -= 0.5L * dgb; up[k] -= 0.5L * dgb; }
+            resid = fmaxl(resid, fabsl(F[k]));
+        }
+        if (resid < 1e-17L) break;
+        // Thomas algorithm: J * step = F
+        std::vector<long double> cp(n), dp(n);
+        cp[0] = up[0] / di[0];
+        dp[0] = F[0] / di[0];
+        for (int k = 1; k < n; ++k) {
+            long double den = di[k] - lo[k] * cp[k - 1];
+            cp[k] = up[k] / den;
+            dp[k] = (F[k] - lo[k] * dp[k - 1]) / den;
+        }
+        step[n - 1] = dp[n - 1];
+        for (int k = n - 2; k >= 0; --k) step[k] = dp[k] - cp[k] * step[k + 1];
+        long double lam = 1.0L;
+        for (;;) {
+            bool ok = true;
+            for (int k = 0; k < n; ++k) cn[k] = c[k] - lam * step[k];
+            if (!(cn[0] > 0.0L)) ok = false;
+            for (int k = 1; k < n && ok; ++k) if (!(cn[k] > cn[k - 1])) ok = false;
+            if (ok || lam < 1e-8L) break;
+            lam *= 0.5L;
+        }
+        c = cn;
+    }
+    return c;
+}
+
+// fp64 -> fp16 round-to-nearest-even (finite, |x| < 65504), returned as the fp16 value in double
+double round_to_f16(double x)
+{
+    if (x == 0.0) return 0.0;
+    int e;
+    double f = frexp(fabs(x), &e);            // |x| = f * 2^e, f in [0.5, 1)
+    int E = e - 1;                            // exponent of the leading bit
+    int q = (E < -14) ? -24 : E - 10;         // quantum 2^q (subnormal quantum is 2^-24)
+    double scaled = ldexp(fabs(x), -q);       // exact
+    double r = nearbyint(scaled);             // default mode: ties-to-even
+    (void)f;
+    double v = ldexp(r, q);
+    return x < 0 ? -v : v;
+}
+}  // namespace
+
+// levels[0 .. 2^b): ascending, fp16-representable
+void codebook_levels(int b, double *levels)
+{
+    if (b == 0) { levels[0] = 0.0; return; }
+    int n = 1 << (b - 1);
+    std::vector<long double> pos = solve_positive(n);
+    for (int k = 0; k < n; ++k) {
+        double v = round_to_f16((double)pos[k]);
+        levels[n + k] = v;
+        levels[n - 1 - k] = -v;
+    }
+}
+
+}  // namespace bgtq
