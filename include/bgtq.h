@@ -121,6 +121,11 @@ int64_t bgtq_tile_stride(const bgtq_layout *layout, int layer, int kv_head);
 int bgtq_quantize_append(const bgtq_layout *layout, int layer, void *cache, const void *k_new,
                          const void *v_new, int dt, int batch, int n_new, int32_t *seq_len,
                          int advance_seq_len, int64_t max_tokens, void *stream);
+/* the same for layers [layer0, layer0+n_layers) in ONE launch (a decode step appends one token to
+ * every layer): k_new, v_new [n_layers, batch, n_new, n_kv_heads, d_h]. */
+int bgtq_quantize_append_layers(const bgtq_layout *layout, int layer0, int n_layers, void *cache,
+                                const void *k_new, const void *v_new, int dt, int batch, int n_new,
+                                int32_t *seq_len, int advance_seq_len, int64_t max_tokens, void *stream);
 
 /* ---- a5 + a6: split-KV decode attention over the packed cache with the exact
  * log-sum-exp merge across splits and the V de-rotation.  For every sequence s and
@@ -144,6 +149,12 @@ int bgtq_decode_attention_layers(const bgtq_layout *layout, int layer0, int n_la
 /* decode one unit (b words per lane, 32 lanes, plane-major as in a tile) with the kernel's own
  * unpack routine: words [host] uint32 [b*32] -> values [host] float [32 lanes][32 slots]. */
 int bgtq_debug_decode_unit(int b, const uint32_t *words, float *values);
+/* measurement hook for bench.py's roofline: while enabled, every decode call records a CUDA event
+ * pair on its stream around the split-KV decode kernel alone (not the q-fold / combine kernels);
+ * _read synchronises those events, returns the summed milliseconds and the number of launches
+ * since the last read, and resets.  Do not enable during stream capture. */
+void bgtq_profile_decode(int enable);
+int bgtq_profile_decode_read(double *ms_sum, int *count);
 /* number of kernels launched by this library since load (bench.py's gpu_launches). */
 int64_t bgtq_launch_count(void);
 

@@ -26,7 +26,8 @@ SYMBOLS = [
     "bgtq_last_error", "bgtq_codebook", "bgtq_block_energy_workspace_bytes", "bgtq_block_energy",
     "bgtq_allocate", "bgtq_layout_create", "bgtq_layout_destroy", "bgtq_cache_bytes",
     "bgtq_token_bytes", "bgtq_workspace_bytes", "bgtq_region_offset", "bgtq_tile_stride",
-    "bgtq_quantize_append", "bgtq_decode_attention", "bgtq_decode_attention_layers",
+    "bgtq_quantize_append", "bgtq_quantize_append_layers", "bgtq_profile_decode",
+    "bgtq_profile_decode_read", "bgtq_decode_attention", "bgtq_decode_attention_layers",
     "bgtq_debug_decode_unit", "bgtq_launch_count",
 ]
 
@@ -72,6 +73,12 @@ def _load() -> C.CDLL:
     lib.bgtq_tile_stride.argtypes = [vp, i32, i32]
     lib.bgtq_quantize_append.restype = i32
     lib.bgtq_quantize_append.argtypes = [vp, i32, vp, vp, vp, i32, i32, i32, vp, i32, i64, vp]
+    lib.bgtq_quantize_append_layers.restype = i32
+    lib.bgtq_quantize_append_layers.argtypes = [vp, i32, i32, vp, vp, vp, i32, i32, i32, vp, i32, i64, vp]
+    lib.bgtq_profile_decode.restype = None
+    lib.bgtq_profile_decode.argtypes = [i32]
+    lib.bgtq_profile_decode_read.restype = i32
+    lib.bgtq_profile_decode_read.argtypes = [vp, vp]
     lib.bgtq_decode_attention.restype = i32
     lib.bgtq_decode_attention.argtypes = [vp, i32, vp, vp, vp, i32, i64, f32, vp, vp, sz, vp]
     lib.bgtq_decode_attention_layers.restype = i32
@@ -207,14 +214,32 @@ class Layout:
 
 def quantize_append(layout: Layout, layer: int, cache: torch.Tensor, k_new: torch.Tensor,
                     v_new: torch.Tensor, seq_len: torch.Tensor, max_tokens: int,
-                    advance_seq_len: bool = True) -> None:
-    """bgtq_quantize_append.  k_new, v_new [batch, n_new, H_kv, d_h]; seq_len int32 [batch] (CUDA)."""
-    batch, n_new, Hkv, d = k_new.shape
+                    advance_seq_len: bool = True, n_layers: int = 1) -> None:
+    """bgtq_quantize_append (k_new, v_new [batch, n_new, H_kv, d_h]) or, with n_layers > 1,
+    bgtq_quantize_append_layers ([n_layers, batch, n_new, H_kv, d_h]); seq_len int32 [batch] (CUDA)."""
+    batch, n_new, Hkv, d = k_new.shape[-4:]
     assert v_new.shape == k_new.shape and Hkv == layout.n_kv_heads and d == layout.d_h
     assert _dt(k_new) == _dt(v_new)
+    if k_new.dim() == 5:
+        assert k_new.shape[0] == n_layers
+        _check(_lib.bgtq_quantize_append_layers(layout._h, layer, n_layers, _dev(cache, torch.uint8), _dev(k_new),
+                                                _dev(v_new), _dt(k_new), batch, n_new, _dev(seq_len, torch.int32),
+                                                1 if advance_seq_len else 0, max_tokens, _stream()))
+        return
     _check(_lib.bgtq_quantize_append(layout._h, layer, _dev(cache, torch.uint8), _dev(k_new), _dev(v_new),
                                      _dt(k_new), batch, n_new, _dev(seq_len, torch.int32),
                                      1 if advance_seq_len else 0, max_tokens, _stream()))
+
+
+def profile_decode(enable: bool) -> None:
+    _lib.bgtq_profile_decode(1 if enable else 0)
+
+
+def profile_decode_read():
+    """-> (summed milliseconds of the decode kernel alone, launches) since the last read."""
+    ms, n = C.c_double(0.0), C.c_int(0)
+    _check(_lib.bgtq_profile_decode_read(C.byref(ms), C.byref(n)))
+    return float(ms.value), int(n.value)
 
 
 def decode_attention(layout: Layout, layer: int, cache: torch.Tensor, q: torch.Tensor,
@@ -227,6 +252,13 @@ def decode_attention(layout: Layout, layer: int, cache: torch.Tensor, q: torch.T
         out = torch.empty_like(q)
     batch = q.shape[-3]
     assert q.shape[-2] == layout.n_q_heads and q.shape[-1] == layout.d_h
+    if q.dim() == 3:
+        _check(_lib.bgtq_decode_attention(layout._h, layer, _dev(cache, torch.uint8), _dev(q, torch.bfloat16),
+                                          _dev(seq_len, torch.int32), batch, max_tokens, float(softmax_scale),
+                                          _dev(out, torch.bfloat16), _dev(workspace, torch.uint8),
+                                          workspace.numel(), _stream()))
+        return out
+    assert q.shape[0] == n_layers
     _check(_lib.bgtq_decode_attention_layers(layout._h, layer, n_layers, _dev(cache, torch.uint8),
                                              _dev(q, torch.bfloat16), _dev(seq_len, torch.int32), batch,
                                              max_tokens, float(softmax_scale), _dev(out, torch.bfloat16),

@@ -65,8 +65,8 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
 {
     extern __shared__ __align__(16) unsigned char smem[];
     const int tid = threadIdx.x;
-    const int h = blockIdx.y, s = blockIdx.z;
-    const HeadMeta &M = metas[h];
+    const int h = blockIdx.y % Hkv, lrel = blockIdx.y / Hkv, s = blockIdx.z;
+    const HeadMeta &M = metas[blockIdx.y];
     const int64_t t0 = seq_len[s];
     const int64_t t_end = min(t0 + (int64_t)n_new, max_tokens);
     const int64_t tile = t0 / kTile + blockIdx.x;
@@ -134,7 +134,7 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
             int64_t tok = base + tt;
             double v = 0.0;
             if (tok >= nlo && tok < nhi) {
-                int64_t row = (((int64_t)s * n_new + (tok - t0)) * Hkv + h) * kDh;
+                int64_t row = ((((int64_t)lrel * batch + s) * n_new + (tok - t0)) * Hkv + h) * kDh;
                 if (c >= 128) v = to_f64(v_new[row + (c - 128)]);
                 else if (c < kdim) v = to_f64(k_new[row + M.coords[c]]);
             }
@@ -248,21 +248,26 @@ static size_t append_smem_bytes(int max_stride)
            kMaxUnits * sizeof(UnitDesc) + 16 + (size_t)max_stride + 64;
 }
 
-int launch_quantize_append(const bgtq_layout *lay, int layer, void *cache, const void *k_new,
+int launch_quantize_append(const bgtq_layout *lay, int layer, int n_layers, void *cache, const void *k_new,
                            const void *v_new, int dt, int batch, int n_new, int32_t *seq_len,
                            int advance, int64_t max_tokens, cudaStream_t st)
 {
+    static bool attr_set = false;
     const int64_t n_cap = (max_tokens + kTile - 1) / kTile;
     const size_t smem = append_smem_bytes(lay->max_stride);
-    dim3 grid((n_new + kTile - 1) / kTile + 1, lay->n_kv_heads, batch);
+    dim3 grid((n_new + kTile - 1) / kTile + 1, lay->n_kv_heads * n_layers, batch);
     const HeadMeta *metas = lay->d_meta + (size_t)layer * lay->n_kv_heads;
+    if (!attr_set) {   // once per process, outside any stream capture
+        const int maxs = (int)append_smem_bytes(16 * kDh * 8 + 256 * 9 + 16 * kDh * 8);
+        CUDA_TRY(cudaFuncSetAttribute(quantize_append_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, maxs));
+        CUDA_TRY(cudaFuncSetAttribute(quantize_append_kernel<__nv_bfloat16>, cudaFuncAttributeMaxDynamicSharedMemorySize, maxs));
+        attr_set = true;
+    }
     if (dt == BGTQ_F32) {
-        CUDA_TRY(cudaFuncSetAttribute(quantize_append_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         quantize_append_kernel<float><<<grid, kAppendThreads, smem, st>>>(
             metas, (uint8_t *)cache, (const float *)k_new, (const float *)v_new, lay->d_cb64, lay->d_rot_t,
             batch, n_new, lay->n_kv_heads, seq_len, n_cap, n_cap * kTile);
     } else {
-        CUDA_TRY(cudaFuncSetAttribute(quantize_append_kernel<__nv_bfloat16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         quantize_append_kernel<__nv_bfloat16><<<grid, kAppendThreads, smem, st>>>(
             metas, (uint8_t *)cache, (const __nv_bfloat16 *)k_new, (const __nv_bfloat16 *)v_new, lay->d_cb64,
             lay->d_rot_t, batch, n_new, lay->n_kv_heads, seq_len, n_cap, n_cap * kTile);

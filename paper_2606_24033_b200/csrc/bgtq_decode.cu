@@ -20,6 +20,9 @@
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
 
+#include <utility>
+#include <vector>
+
 #include "bgtq_internal.h"
 
 namespace bgtq {
@@ -597,11 +600,49 @@ size_t decode_ws_bytes(const bgtq_layout *lay, int batch, int n_layers)
     return qf + slots * kPartialFloats * sizeof(float);
 }
 
+// measurement hook (bgtq_profile_decode): event pairs around the decode kernel only
+static bool g_prof = false;
+static std::vector<std::pair<cudaEvent_t, cudaEvent_t>> g_prof_events;
+static size_t g_prof_used = 0;
+
+void profile_decode_enable(int enable) { g_prof = enable != 0; }
+int profile_decode_read(double *ms_sum, int *count)
+{
+    double sum = 0.0;
+    for (size_t i = 0; i < g_prof_used; ++i) {
+        float ms = 0.f;
+        CUDA_TRY(cudaEventSynchronize(g_prof_events[i].second));
+        CUDA_TRY(cudaEventElapsedTime(&ms, g_prof_events[i].first, g_prof_events[i].second));
+        sum += ms;
+    }
+    *ms_sum = sum;
+    *count = (int)g_prof_used;
+    g_prof_used = 0;
+    return BGTQ_OK;
+}
+
 template <int W>
 static int launch_decode_w(const DecodeParams &P, int grid, size_t smem, cudaStream_t st)
 {
-    CUDA_TRY(cudaFuncSetAttribute(decode_kernel<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    static bool attr_set = false;
+    if (!attr_set) {   // once per process, outside any stream capture
+        CUDA_TRY(cudaFuncSetAttribute(decode_kernel<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        attr_set = true;
+    }
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (g_prof) {
+        if (g_prof_used == g_prof_events.size()) {
+            CUDA_TRY(cudaEventCreate(&e0));
+            CUDA_TRY(cudaEventCreate(&e1));
+            g_prof_events.emplace_back(e0, e1);
+        }
+        e0 = g_prof_events[g_prof_used].first;
+        e1 = g_prof_events[g_prof_used].second;
+        ++g_prof_used;
+        CUDA_TRY(cudaEventRecord(e0, st));
+    }
     decode_kernel<W><<<grid, W * 32, smem, st>>>(P);
+    if (g_prof) CUDA_TRY(cudaEventRecord(e1, st));
     return BGTQ_OK;
 }
 

@@ -282,19 +282,35 @@ extern "C" size_t bgtq_workspace_bytes(const bgtq_layout *lay, int batch, int n_
 }
 
 // ------------------------------------------------------------------ a4 / a5 wrappers
+extern "C" int bgtq_quantize_append_layers(const bgtq_layout *lay, int layer0, int n_layers, void *cache,
+                                           const void *k_new, const void *v_new, int dt, int batch, int n_new,
+                                           int32_t *seq_len, int advance_seq_len, int64_t max_tokens, void *stream)
+{
+    if (!lay || !cache || !seq_len) FAIL(BGTQ_EINVAL, "bgtq_quantize_append: null pointer");
+    if (layer0 < 0 || n_layers <= 0 || layer0 + n_layers > lay->n_layers) FAIL(BGTQ_EINVAL, "bgtq_quantize_append: layer out of range");
+    if (dt != BGTQ_F32 && dt != BGTQ_BF16) FAIL(BGTQ_EINVAL, "bgtq_quantize_append: dtype");
+    if (batch <= 0 || n_new < 0 || max_tokens <= 0) FAIL(BGTQ_EINVAL, "bgtq_quantize_append: batch/n_new/max_tokens");
+    if (batch > 65535 || (int64_t)n_layers * lay->n_kv_heads > 65535) FAIL(BGTQ_EINVAL, "bgtq_quantize_append: batch or layers*heads > 65535");
+    if (n_new > max_tokens) FAIL(BGTQ_ECAPACITY, "bgtq_quantize_append: n_new exceeds max_tokens");
+    if (n_new == 0) return BGTQ_OK;
+    if (!k_new || !v_new) FAIL(BGTQ_EINVAL, "bgtq_quantize_append: null k_new/v_new");
+    return launch_quantize_append(lay, layer0, n_layers, cache, k_new, v_new, dt, batch, n_new, seq_len,
+                                  advance_seq_len, max_tokens, (cudaStream_t)stream);
+}
+
 extern "C" int bgtq_quantize_append(const bgtq_layout *lay, int layer, void *cache, const void *k_new,
                                     const void *v_new, int dt, int batch, int n_new, int32_t *seq_len,
                                     int advance_seq_len, int64_t max_tokens, void *stream)
 {
-    if (!lay || !cache || !seq_len) FAIL(BGTQ_EINVAL, "bgtq_quantize_append: null pointer");
-    if (layer < 0 || layer >= lay->n_layers) FAIL(BGTQ_EINVAL, "bgtq_quantize_append: layer out of range");
-    if (dt != BGTQ_F32 && dt != BGTQ_BF16) FAIL(BGTQ_EINVAL, "bgtq_quantize_append: dtype");
-    if (batch <= 0 || n_new < 0 || max_tokens <= 0) FAIL(BGTQ_EINVAL, "bgtq_quantize_append: batch/n_new/max_tokens");
-    if (n_new > max_tokens) FAIL(BGTQ_ECAPACITY, "bgtq_quantize_append: n_new exceeds max_tokens");
-    if (n_new == 0) return BGTQ_OK;
-    if (!k_new || !v_new) FAIL(BGTQ_EINVAL, "bgtq_quantize_append: null k_new/v_new");
-    return launch_quantize_append(lay, layer, cache, k_new, v_new, dt, batch, n_new, seq_len,
-                                  advance_seq_len, max_tokens, (cudaStream_t)stream);
+    return bgtq_quantize_append_layers(lay, layer, 1, cache, k_new, v_new, dt, batch, n_new, seq_len,
+                                       advance_seq_len, max_tokens, stream);
+}
+
+extern "C" void bgtq_profile_decode(int enable) { profile_decode_enable(enable); }
+extern "C" int bgtq_profile_decode_read(double *ms_sum, int *count)
+{
+    if (!ms_sum || !count) FAIL(BGTQ_EINVAL, "bgtq_profile_decode_read: null pointer");
+    return profile_decode_read(ms_sum, count);
 }
 
 extern "C" int bgtq_decode_attention_layers(const bgtq_layout *lay, int layer0, int n_layers,

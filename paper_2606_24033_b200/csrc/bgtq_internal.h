@@ -75,7 +75,7 @@ int launch_block_energy(const void *q, int64_t n_q, const void *k, int64_t n_k, 
 size_t block_energy_ws_bytes(int Hq, int Hkv, int d_h);
 int launch_allocate(const float *scores, int n_heads, int L, int b_min, int b_max, int B,
                     uint8_t *bits, cudaStream_t st);
-int launch_quantize_append(const bgtq_layout *lay, int layer, void *cache, const void *k_new,
+int launch_quantize_append(const bgtq_layout *lay, int layer, int n_layers, void *cache, const void *k_new,
                            const void *v_new, int dt, int batch, int n_new, int32_t *seq_len,
                            int advance, int64_t max_tokens, cudaStream_t st);
 int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *cache,
@@ -83,5 +83,7 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
                   float scale, void *out, void *ws, size_t ws_bytes, cudaStream_t st);
 size_t decode_ws_bytes(const bgtq_layout *lay, int batch, int n_layers);
 int debug_decode_unit(int b, const uint32_t *words, float *values);
+void profile_decode_enable(int enable);
+int profile_decode_read(double *ms_sum, int *count);
 
 }  // namespace bgtq
