@@ -142,7 +142,7 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
         }
         __syncthreads();
         // ---- 2. radii: ss = fma chain, r = sqrt(ss), sigma = r / sqrt(m), h = fp16_rne_sat(r)
-        if (tid < kSub * (ng + 1)) {
+        if (tid < kSub * (ng + 1) && base + tid / (ng + 1) >= nlo && base + tid / (ng + 1) < nhi) {
             int tt = tid / (ng + 1), g = tid % (ng + 1);
             int x0 = g < ng ? M.gstart[g] : 128, m = g < ng ? M.gm[g] : kDh;
             const double *x = xs + tt * 256 + x0;
@@ -155,16 +155,47 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
             if (r >= 65520.0) hb = 0x7BFF;
             nrm[tt * 9 + g] = hb;
         }
-        // ---- 3. rotation: z[tt] = fma chain over k of Pi[r][k] * x_k, 16 tokens per rotation read
+        // ---- 3. rotation: z[tt] = fma chain over k of Pi[r][k] * x_k (k ascending: the oracle's order).
+        //      Rotation rows are read 4 at a time ahead of the chain; a single new token (decode-time
+        //      append) takes the scalar path so that the step is latency- not throughput-shaped.
+        const int tt_lo = (int)(nlo - base), tt_hi = (int)(nhi - base);
         double z[kSub];
 #pragma unroll
         for (int tt = 0; tt < kSub; ++tt) z[tt] = 0.0;
         if (my_m > 0) {
             const double *x = xs + my_x0;
-            for (int k = 0; k < my_m; ++k) {
-                double pi = (double)__ldg(myrot + (size_t)k * my_m);
+            if (tt_hi - tt_lo == 1) {
+                const double *x1 = x + tt_lo * 256;
+                double zz = 0.0;
+                int k = 0;
+                for (; k + 8 <= my_m; k += 8) {
+                    float pf[8];
 #pragma unroll
-                for (int tt = 0; tt < kSub; ++tt) z[tt] = __fma_rn(pi, x[tt * 256 + k], z[tt]);
+                    for (int u = 0; u < 8; ++u) pf[u] = __ldg(myrot + (size_t)(k + u) * my_m);
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) zz = __fma_rn((double)pf[u], x1[k + u], zz);
+                }
+                for (; k < my_m; ++k) zz = __fma_rn((double)__ldg(myrot + (size_t)k * my_m), x1[k], zz);
+#pragma unroll
+                for (int tt = 0; tt < kSub; ++tt) if (tt == tt_lo) z[tt] = zz;
+            } else {
+                int k = 0;
+                for (; k + 4 <= my_m; k += 4) {
+                    float pf[4];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) pf[u] = __ldg(myrot + (size_t)(k + u) * my_m);
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const double pi = (double)pf[u];
+#pragma unroll
+                        for (int tt = 0; tt < kSub; ++tt) z[tt] = __fma_rn(pi, x[tt * 256 + k + u], z[tt]);
+                    }
+                }
+                for (; k < my_m; ++k) {
+                    const double pi = (double)__ldg(myrot + (size_t)k * my_m);
+#pragma unroll
+                    for (int tt = 0; tt < kSub; ++tt) z[tt] = __fma_rn(pi, x[tt * 256 + k], z[tt]);
+                }
             }
         }
         __syncthreads();
@@ -174,6 +205,7 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
             const int nthr = (1 << my_b) - 1;
 #pragma unroll
             for (int tt = 0; tt < kSub; ++tt) {
+                if (tt < tt_lo || tt >= tt_hi) continue;
                 double sg = sigma[tt * 9 + my_g];
                 int a = 0, c = nthr;
                 while (a < c) {

@@ -44,7 +44,7 @@ __device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t s)
 __device__ __forceinline__ void mma16816(float (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2,
                                          uint32_t a3, uint32_t b0, uint32_t b1)
 {
-    asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+    asm("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
                  : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
                  : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
 }
@@ -232,7 +232,8 @@ __device__ __forceinline__ TilePos locate(int x, const Sched &s, const int *pre)
 
 // ---------------------------------------------------------------- prologue: Q-side rotation fold
 // q'_g = Pi^(m_g) q_g * (scale*log2e/sqrt(m_g))  ("Q-side rotation"), rounded to fp16 and
-// written in B-fragment order: qf[pair][kstep][head slot n (8)][16 coords of the k-step], zero padded.
+// written in B-fragment order: qf[pair][kstep][head slot n (8)][c (4)][coords 2c, 2c+1, 8+2c, 9+2c], i.e. one
+// 8-byte load per lane (n*4+c) and k-step; zero padded.
 __global__ void __launch_bounds__(128)
 qfold_kernel(const HeadMeta *__restrict__ metas, const float *__restrict__ rot_t,
              const __nv_bfloat16 *__restrict__ q, int batch, int Hkv, int Hq, float scale_log2e,
@@ -260,11 +261,28 @@ qfold_kernel(const HeadMeta *__restrict__ metas, const float *__restrict__ rot_t
         const float *T = rot_t + rot_offset(m) + r;
         const float sc = scale_log2e / sqrtf((float)m);
         const int ks = ksbase[g] + (r >> 4), kap = r & 15;
-        for (int n = 0; n < G; ++n) {
-            float acc = 0.f;
-            for (int k = 0; k < m; ++k) acc = fmaf(__ldg(T + (size_t)k * m), qs[n * kDh + M.coords[x0 + k]], acc);
-            out[(ks * 8 + n) * 16 + kap] = __float2half_rn(acc * sc);
+        float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+        const uint8_t *co = M.coords + x0;
+        int k = 0;
+        for (; k + 4 <= m; k += 4) {                    // m is even; rotation rows read 4 ahead of the FMAs
+            float tv[4];
+            int cc[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) { tv[u] = __ldg(T + (size_t)(k + u) * m); cc[u] = co[k + u]; }
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+#pragma unroll
+                for (int n = 0; n < 8; ++n) if (n < G) acc[n] = fmaf(tv[u], qs[n * kDh + cc[u]], acc[n]);
         }
+        for (; k < m; ++k) {
+            const float tv = __ldg(T + (size_t)k * m);
+            const int cc = co[k];
+#pragma unroll
+            for (int n = 0; n < 8; ++n) if (n < G) acc[n] = fmaf(tv, qs[n * kDh + cc], acc[n]);
+        }
+#pragma unroll
+        for (int n = 0; n < 8; ++n)
+            if (n < G) out[((ks * 8 + n) * 4 + ((kap & 7) >> 1)) * 4 + (kap >> 3) * 2 + (kap & 1)] = __float2half_rn(acc[n] * sc);
     }
 }
 
@@ -281,36 +299,59 @@ struct DecodeParams {
     int buf_bytes;              // per-warp tile buffer
 };
 
-struct WarpState {
-    float m[2], l[2];           // running max (log2 domain) and partial sum for heads 2c, 2c+1
-    float O[8][4];              // PV accumulators: [J] -> dims 16J+g8 (+8), heads 2c, 2c+1
-};
+constexpr int kSmemHdr = 2560;  // [lut16 1024][pools 64][pre 1040][mbarriers 256], then the tile buffers
 
-// QK^T of one k16 step: two units of width B -> 8 m-tiles
+// load the B words of one unit for this lane.  FULL: 32 lanes per word plane (stride 32 words).
 template <int B>
-__device__ __forceinline__ void qk_step(const uint32_t *tile, uint32_t d0, uint32_t d1, int g8, int c,
-                                        uint32_t bq0, uint32_t bq1, const uint32_t *pools,
-                                        const uint16_t *lut, float (&A)[8][4])
+__device__ __forceinline__ void load_unit_full(const uint32_t *unit, int lane, uint32_t (&w)[B])
 {
-    const int off0 = d0 & 0xFFFF, off1 = d0 >> 16;
-    const int nc0 = (d1 >> 8) & 0xFF, nc1 = (d1 >> 16) & 0xFF;
-    uint32_t w0[B], w1[B], h0[16], h1[16];
-    {
-        const bool act = c < nc0;
-        const uint32_t *wp = tile + (off0 >> 2) + g8 * nc0 + c;
 #pragma unroll
-        for (int w = 0; w < B; ++w) w0[w] = act ? wp[w * 8 * nc0] : 0u;
+    for (int i = 0; i < B; ++i) w[i] = unit[i * 32 + lane];
+}
+// trailing partial half-step: only lanes c < nc hold data, compacted to 8*nc lanes per plane
+template <int B>
+__device__ __forceinline__ void load_unit_partial(const uint32_t *unit, int g8, int c, int nc, uint32_t (&w)[B])
+{
+    const bool act = c < nc;
+    const uint32_t *wp = unit + g8 * nc + c;
+#pragma unroll
+    for (int i = 0; i < B; ++i) w[i] = act ? wp[i * 8 * nc] : 0u;
+}
+
+// QK^T of one same-width group: all its k16 steps, 8 m-tiles each.  m = coordinates in the
+// group; units of 8 coordinates are contiguous (128*B bytes each), only the last may be partial.
+template <int B>
+__device__ __forceinline__ void qk_group(const uint32_t *gcodes, int m, int lane, const uint2 *qfp,
+                                         const uint32_t *pools, const uint16_t *lut, float (&A)[8][4])
+{
+    const int g8 = lane >> 2, c = lane & 3;
+    const int n_full = m >> 3, rem = (m & 7) >> 1;         // full units; lanes per row in the partial one
+    const int n_half = n_full + (rem ? 1 : 0);
+#pragma unroll 1
+    for (int j = 0; j < n_half; j += 2) {
+        uint32_t w0[B], w1[B], h0[16], h1[16];
+        const uint32_t *u0 = gcodes + j * 32 * B;
+        const uint2 bq = __ldg(qfp + (j >> 1) * 32);
+        if (j + 1 < n_full) {                               // common case: two full units
+            load_unit_full<B>(u0, lane, w0);
+            load_unit_full<B>(u0 + 32 * B, lane, w1);
+            decode_unit<B>(w0, pools, lut, h0);
+            decode_unit<B>(w1, pools, lut, h1);
+        } else {
+            if (j < n_full) load_unit_full<B>(u0, lane, w0);
+            else load_unit_partial<B>(u0, g8, c, rem, w0);
+            decode_unit<B>(w0, pools, lut, h0);
+            if (j + 1 < n_half) {                           // second unit is the partial one
+                load_unit_partial<B>(u0 + 32 * B, g8, c, rem, w1);
+                decode_unit<B>(w1, pools, lut, h1);
+            } else {
+#pragma unroll
+                for (int i = 0; i < 16; ++i) h1[i] = 0u;
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < 8; ++i) mma16816(A[i], h0[2 * i], h0[2 * i + 1], h1[2 * i], h1[2 * i + 1], bq.x, bq.y);
     }
-    {
-        const bool act = c < nc1;
-        const uint32_t *wp = tile + (off1 >> 2) + g8 * nc1 + c;
-#pragma unroll
-        for (int w = 0; w < B; ++w) w1[w] = act ? wp[w * 8 * nc1] : 0u;
-    }
-    decode_unit<B>(w0, pools, lut, h0);
-    decode_unit<B>(w1, pools, lut, h1);
-#pragma unroll
-    for (int i = 0; i < 8; ++i) mma16816(A[i], h0[2 * i], h0[2 * i + 1], h1[2 * i], h1[2 * i + 1], bq0, bq1);
 }
 
 // PV of one tile: 16 units of width B -> O[J] += V^T[16 dims x 128 tokens] . P[128 tokens x 8 heads]
@@ -321,9 +362,9 @@ __device__ __forceinline__ void pv_tile(const uint32_t *vcodes, int lane, const 
 #pragma unroll 1
     for (int J = 0; J < 8; ++J) {
         uint32_t w0[B], w1[B], h0[16], h1[16];
-        const uint32_t *wp = vcodes + (2 * J) * 32 * B + lane;
-#pragma unroll
-        for (int w = 0; w < B; ++w) { w0[w] = wp[w * 32]; w1[w] = wp[32 * B + w * 32]; }
+        const uint32_t *u0 = vcodes + (2 * J) * 32 * B;
+        load_unit_full<B>(u0, lane, w0);
+        load_unit_full<B>(u0 + 32 * B, lane, w1);
         decode_unit<B>(w0, pools, lut, h0);
         decode_unit<B>(w1, pools, lut, h1);
 #pragma unroll
@@ -337,13 +378,10 @@ __global__ void __launch_bounds__(W * 32, 1)
 decode_kernel(const DecodeParams P)
 {
     extern __shared__ __align__(128) unsigned char smem[];
-    // carve-up: [lut16 1024 B][pools 64 B][pre (kMaxBatch+1) ints][barriers W*2*8][tile buffers]
     uint16_t *lut = reinterpret_cast<uint16_t *>(smem);
     uint32_t *pools = reinterpret_cast<uint32_t *>(smem + 1024);
     int *pre = reinterpret_cast<int *>(smem + 1024 + 64);
-    uint64_t *bars = reinterpret_cast<uint64_t *>(smem + 1024 + 64 + ((kMaxBatch + 1) * 4 + 12) / 16 * 16);
-    unsigned char *bufs = reinterpret_cast<unsigned char *>(bars + 2 * W);
-    bufs = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(bufs) + 127) & ~uintptr_t(127));
+    uint64_t *bars = reinterpret_cast<uint64_t *>(smem + 1024 + 64 + 1040 + 176);   // 2304, 8-byte aligned
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int g8 = lane >> 2, c = lane & 3;
@@ -367,12 +405,11 @@ decode_kernel(const DecodeParams P)
     const int x_end = min(S.total, x + S.per_warp);
     if (x >= x_end) return;
 
-    uint32_t *tile = reinterpret_cast<uint32_t *>(bufs + (size_t)warp * P.buf_bytes);
+    const uint32_t *tile = reinterpret_cast<const uint32_t *>(smem + kSmemHdr + warp * P.buf_bytes);
     const uint32_t tile_s = smem_u32(tile);
     uint32_t kphase = 0, vphase = 0;
 
-    // source address and byte counts of a global tile index (lane 0 only needs them)
-    auto issue = [&](int xg, bool want_k, bool want_v) {
+    auto issue = [&](int xg, bool want_k, bool want_v) {      // lane 0: request (half of) global tile xg
         const TilePos tp = locate(xg, S, pre);
         const HeadMeta &M = P.metas[tp.l * P.Hkv + tp.h];
         const uint8_t *src = P.cache + P.n_cap * ((int64_t)P.batch * M.layer_prefix + (int64_t)tp.b * M.layer_sum + M.head_prefix) +
@@ -389,65 +426,62 @@ decode_kernel(const DecodeParams P)
         const TilePos tp = locate(x, S, pre);
         const HeadMeta &M = P.metas[tp.l * P.Hkv + tp.h];
         const int seg_end = min(x_end, tp.pair_start + tp.tiles_b);
-        const int n_ksteps = M.n_ksteps, b_v = M.b_v;
+        const int n_groups = M.n_groups, b_v = M.b_v;
         const int knorm_off = M.knorm_off, vnorm_off = M.vnorm_off, vcode_off = M.vcode_off;
         int64_t slen = P.seq_len[tp.b];
         slen = slen > P.n_cap * kTile ? P.n_cap * kTile : slen;
-        // lane ks keeps the descriptor of k-step ks
-        uint32_t desc0 = 0, desc1 = 0;
-        if (lane < n_ksteps) {
-            const KStep K = M.ksteps[lane];
-            desc0 = (uint32_t)K.off0 | ((uint32_t)K.off1 << 16);
-            desc1 = (uint32_t)K.b | ((uint32_t)K.nc0 << 8) | ((uint32_t)K.nc1 << 16) | ((uint32_t)K.flags << 24);
+        // lane g keeps the descriptor of group g: code offset | m << 16 | b << 24 | first k-step << 28
+        uint32_t gdesc = 0;
+        if (lane < n_groups) {
+            int ksb = 0;
+            for (int g = 0; g < lane; ++g) ksb += (M.gm[g] + 15) >> 4;
+            gdesc = (uint32_t)M.goff[lane] | ((uint32_t)(M.gm[lane] & 0xFF) << 16) | ((uint32_t)M.gb[lane] << 24) | ((uint32_t)ksb << 28);
         }
-        const uint32_t *qfp = reinterpret_cast<const uint32_t *>(P.qf + (size_t)tp.pair * kQfHalves) + g8 * 8 + c;
+        const uint2 *qfp = reinterpret_cast<const uint2 *>(P.qf + (size_t)tp.pair * kQfHalves) + lane;
 
-        WarpState st;
-        st.m[0] = st.m[1] = -INFINITY;
-        st.l[0] = st.l[1] = 0.f;
+        float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;   // heads 2c, 2c+1 (log2 domain)
+        float O[8][4];
 #pragma unroll
-        for (int J = 0; J < 8; ++J) st.O[J][0] = st.O[J][1] = st.O[J][2] = st.O[J][3] = 0.f;
+        for (int J = 0; J < 8; ++J) O[J][0] = O[J][1] = O[J][2] = O[J][3] = 0.f;
 
         for (int t = tp.t; x < seg_end; ++x, ++t) {
             // ======== QK^T
             mbar_wait(kbar, kphase);
             kphase ^= 1;
-            float Sc[8][4], A[8][4];
+            float Sc[8][4];
 #pragma unroll
             for (int i = 0; i < 8; ++i) Sc[i][0] = Sc[i][1] = Sc[i][2] = Sc[i][3] = 0.f;
 #pragma unroll 1
-            for (int ks = 0; ks < n_ksteps; ++ks) {
-                const uint32_t d0 = __shfl_sync(0xFFFFFFFFu, desc0, ks);
-                const uint32_t d1 = __shfl_sync(0xFFFFFFFFu, desc1, ks);
-                const int flags = d1 >> 24;
-                if (flags & 1) {
+            for (int g = 0; g < n_groups; ++g) {
+                const uint32_t d = __shfl_sync(0xFFFFFFFFu, gdesc, g);
+                int m = (d >> 16) & 0xFF;
+                m = m ? m : 128;
+                const uint32_t *gcodes = tile + ((d & 0xFFFF) >> 2);
+                const uint2 *qg = qfp + (d >> 28) * 32;
+                float A[8][4];
 #pragma unroll
-                    for (int i = 0; i < 8; ++i) A[i][0] = A[i][1] = A[i][2] = A[i][3] = 0.f;
+                for (int i = 0; i < 8; ++i) A[i][0] = A[i][1] = A[i][2] = A[i][3] = 0.f;
+                switch ((d >> 24) & 0xF) {
+                case 1: qk_group<1>(gcodes, m, lane, qg, pools, lut, A); break;
+                case 2: qk_group<2>(gcodes, m, lane, qg, pools, lut, A); break;
+                case 3: qk_group<3>(gcodes, m, lane, qg, pools, lut, A); break;
+                case 4: qk_group<4>(gcodes, m, lane, qg, pools, lut, A); break;
+                case 5: qk_group<5>(gcodes, m, lane, qg, pools, lut, A); break;
+                case 6: qk_group<6>(gcodes, m, lane, qg, pools, lut, A); break;
+                case 7: qk_group<7>(gcodes, m, lane, qg, pools, lut, A); break;
+                default: qk_group<8>(gcodes, m, lane, qg, pools, lut, A); break;
                 }
-                const uint32_t bq0 = __ldg(qfp + ks * 64), bq1 = __ldg(qfp + ks * 64 + 4);
-                switch (d1 & 0xFF) {
-                case 1: qk_step<1>(tile, d0, d1, g8, c, bq0, bq1, pools, lut, A); break;
-                case 2: qk_step<2>(tile, d0, d1, g8, c, bq0, bq1, pools, lut, A); break;
-                case 3: qk_step<3>(tile, d0, d1, g8, c, bq0, bq1, pools, lut, A); break;
-                case 4: qk_step<4>(tile, d0, d1, g8, c, bq0, bq1, pools, lut, A); break;
-                case 5: qk_step<5>(tile, d0, d1, g8, c, bq0, bq1, pools, lut, A); break;
-                case 6: qk_step<6>(tile, d0, d1, g8, c, bq0, bq1, pools, lut, A); break;
-                case 7: qk_step<7>(tile, d0, d1, g8, c, bq0, bq1, pools, lut, A); break;
-                default: qk_step<8>(tile, d0, d1, g8, c, bq0, bq1, pools, lut, A); break;
-                }
-                if (flags & 2) {   // group finished: scale by the fp16 group norms (fp32, on the accumulators)
-                    const uint4 *np = reinterpret_cast<const uint4 *>(
-                        reinterpret_cast<const unsigned char *>(tile) + knorm_off + 256 * (flags >> 4) + g8 * 32);
-                    const uint4 n0 = np[0], n1 = np[1];
-                    const uint32_t nw[8] = {n0.x, n0.y, n0.z, n0.w, n1.x, n1.y, n1.z, n1.w};
+                // scale by the fp16 group norms (fp32, on the accumulators)
+                const uint4 *np = reinterpret_cast<const uint4 *>(tile + ((knorm_off + 256 * g + g8 * 32) >> 2));
+                const uint4 n0 = np[0], n1 = np[1];
+                const uint32_t nw[8] = {n0.x, n0.y, n0.z, n0.w, n1.x, n1.y, n1.z, n1.w};
 #pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        const float2 nf = __half22float2(*reinterpret_cast<const __half2 *>(&nw[i]));
-                        Sc[i][0] = fmaf(nf.x, A[i][0], Sc[i][0]);
-                        Sc[i][1] = fmaf(nf.x, A[i][1], Sc[i][1]);
-                        Sc[i][2] = fmaf(nf.y, A[i][2], Sc[i][2]);
-                        Sc[i][3] = fmaf(nf.y, A[i][3], Sc[i][3]);
-                    }
+                for (int i = 0; i < 8; ++i) {
+                    const float2 nf = __half22float2(*reinterpret_cast<const __half2 *>(&nw[i]));
+                    Sc[i][0] = fmaf(nf.x, A[i][0], Sc[i][0]);
+                    Sc[i][1] = fmaf(nf.x, A[i][1], Sc[i][1]);
+                    Sc[i][2] = fmaf(nf.y, A[i][2], Sc[i][2]);
+                    Sc[i][3] = fmaf(nf.y, A[i][3], Sc[i][3]);
                 }
             }
             __syncwarp();
@@ -473,9 +507,9 @@ decode_kernel(const DecodeParams P)
                 mx0 = fmaxf(mx0, __shfl_xor_sync(0xFFFFFFFFu, mx0, o));
                 mx1 = fmaxf(mx1, __shfl_xor_sync(0xFFFFFFFFu, mx1, o));
             }
-            const float mn0 = fmaxf(st.m[0], mx0), mn1 = fmaxf(st.m[1], mx1);
-            const float al0 = fast_exp2(st.m[0] - mn0), al1 = fast_exp2(st.m[1] - mn1);
-            st.m[0] = mn0; st.m[1] = mn1;
+            const float mn0 = fmaxf(m0, mx0), mn1 = fmaxf(m1, mx1);
+            const float al0 = fast_exp2(m0 - mn0), al1 = fast_exp2(m1 - mn1);
+            m0 = mn0; m1 = mn1;
             float ls0 = 0.f, ls1 = 0.f;
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
@@ -484,17 +518,19 @@ decode_kernel(const DecodeParams P)
                 ls0 += Sc[i][0] + Sc[i][2];
                 ls1 += Sc[i][1] + Sc[i][3];
             }
-            st.l[0] = fmaf(st.l[0], al0, ls0);
-            st.l[1] = fmaf(st.l[1], al1, ls1);
+            l0 = fmaf(l0, al0, ls0);
+            l1 = fmaf(l1, al1, ls1);
+            if (__any_sync(0xFFFFFFFFu, al0 != 1.f || al1 != 1.f)) {
 #pragma unroll
-            for (int J = 0; J < 8; ++J) { st.O[J][0] *= al0; st.O[J][2] *= al0; st.O[J][1] *= al1; st.O[J][3] *= al1; }
+                for (int J = 0; J < 8; ++J) { O[J][0] *= al0; O[J][2] *= al0; O[J][1] *= al1; O[J][3] *= al1; }
+            }
 
             // ======== P * (V norm) -> fp16 B fragments (8x8 transposes), then PV
             mbar_wait(vbar, vphase);
             vphase ^= 1;
             uint32_t bP[8][2];
             {
-                const uint4 *np = reinterpret_cast<const uint4 *>(reinterpret_cast<const unsigned char *>(tile) + vnorm_off + g8 * 32);
+                const uint4 *np = reinterpret_cast<const uint4 *>(tile + ((vnorm_off + g8 * 32) >> 2));
                 const uint4 n0 = np[0], n1 = np[1];
                 const uint32_t nw[8] = {n0.x, n0.y, n0.z, n0.w, n1.x, n1.y, n1.z, n1.w};
 #pragma unroll
@@ -506,21 +542,20 @@ decode_kernel(const DecodeParams P)
             }
             const uint32_t *vcodes = tile + (vcode_off >> 2);
             switch (b_v) {
-            case 1: pv_tile<1>(vcodes, lane, bP, pools, lut, st.O); break;
-            case 2: pv_tile<2>(vcodes, lane, bP, pools, lut, st.O); break;
-            case 3: pv_tile<3>(vcodes, lane, bP, pools, lut, st.O); break;
-            case 4: pv_tile<4>(vcodes, lane, bP, pools, lut, st.O); break;
-            case 5: pv_tile<5>(vcodes, lane, bP, pools, lut, st.O); break;
-            case 6: pv_tile<6>(vcodes, lane, bP, pools, lut, st.O); break;
-            case 7: pv_tile<7>(vcodes, lane, bP, pools, lut, st.O); break;
-            default: pv_tile<8>(vcodes, lane, bP, pools, lut, st.O); break;
+            case 1: pv_tile<1>(vcodes, lane, bP, pools, lut, O); break;
+            case 2: pv_tile<2>(vcodes, lane, bP, pools, lut, O); break;
+            case 3: pv_tile<3>(vcodes, lane, bP, pools, lut, O); break;
+            case 4: pv_tile<4>(vcodes, lane, bP, pools, lut, O); break;
+            case 5: pv_tile<5>(vcodes, lane, bP, pools, lut, O); break;
+            case 6: pv_tile<6>(vcodes, lane, bP, pools, lut, O); break;
+            case 7: pv_tile<7>(vcodes, lane, bP, pools, lut, O); break;
+            default: pv_tile<8>(vcodes, lane, bP, pools, lut, O); break;
             }
             __syncwarp();
             if (lane == 0 && x + 1 < x_end) issue(x + 1, x + 1 >= seg_end, true);   // V half (and K when the layout changes)
         }
 
         // ---------------- write this warp's partial for the pair: slot = warp + pair (unique, see combine)
-        float l0 = st.l[0], l1 = st.l[1];
 #pragma unroll
         for (int o = 4; o < 32; o <<= 1) {
             l0 += __shfl_xor_sync(0xFFFFFFFFu, l0, o);
@@ -530,15 +565,15 @@ decode_kernel(const DecodeParams P)
         const int n0 = 2 * c, n1 = 2 * c + 1;
         if (n0 < P.G) {
             float *r0 = rec + n0 * 130;
-            if (g8 == 0) { r0[0] = st.m[0]; r0[1] = l0; }
+            if (g8 == 0) { r0[0] = m0; r0[1] = l0; }
 #pragma unroll
-            for (int J = 0; J < 8; ++J) { r0[2 + 16 * J + g8] = st.O[J][0]; r0[2 + 16 * J + 8 + g8] = st.O[J][2]; }
+            for (int J = 0; J < 8; ++J) { r0[2 + 16 * J + g8] = O[J][0]; r0[2 + 16 * J + 8 + g8] = O[J][2]; }
         }
         if (n1 < P.G) {
             float *r1 = rec + n1 * 130;
-            if (g8 == 0) { r1[0] = st.m[1]; r1[1] = l1; }
+            if (g8 == 0) { r1[0] = m1; r1[1] = l1; }
 #pragma unroll
-            for (int J = 0; J < 8; ++J) { r1[2 + 16 * J + g8] = st.O[J][1]; r1[2 + 16 * J + 8 + g8] = st.O[J][3]; }
+            for (int J = 0; J < 8; ++J) { r1[2 + 16 * J + g8] = O[J][1]; r1[2 + 16 * J + 8 + g8] = O[J][3]; }
         }
     }
 }
@@ -564,14 +599,17 @@ combine_kernel(const float *__restrict__ partials, const int32_t *__restrict__ s
     if (tiles_b == 0) { dst[d] = __float2bfloat16(0.f); return; }
     const int start = l * (Hkv * S.tiles_sum) + pre[b] * Hkv + h * tiles_b;
     const int w0 = start / S.per_warp, w1 = (start + tiles_b - 1) / S.per_warp;
-    float Mx = -INFINITY;
-    for (int w = w0; w <= w1; ++w) Mx = fmaxf(Mx, partials[(size_t)(w + pair) * kPartialFloats + n * 130]);
-    float acc = 0.f, lsum = 0.f;
+    float Mx = -INFINITY, acc = 0.f, lsum = 0.f;       // single pass, running max (exact: PAPER.md:120)
+    const float *rec0 = partials + (size_t)pair * kPartialFloats + n * 130;
+#pragma unroll 4
     for (int w = w0; w <= w1; ++w) {
-        const float *rec = partials + (size_t)(w + pair) * kPartialFloats + n * 130;
-        const float f = exp2f(rec[0] - Mx);
-        lsum = fmaf(rec[1], f, lsum);
-        acc = fmaf(rec[2 + d], f, acc);
+        const float *rec = rec0 + (size_t)w * kPartialFloats;
+        const float mw = rec[0], lw = rec[1], aw = rec[2 + d];
+        const float Mn = fmaxf(Mx, mw);
+        const float fo = exp2f(Mx - Mn), fw = exp2f(mw - Mn);
+        lsum = fmaf(lsum, fo, lw * fw);
+        acc = fmaf(acc, fo, aw * fw);
+        Mx = Mn;
     }
     o[d] = acc / lsum;
     __syncthreads();
@@ -584,13 +622,13 @@ combine_kernel(const float *__restrict__ partials, const int32_t *__restrict__ s
 // ---------------------------------------------------------------- host side
 static int pick_warps(int buf_bytes)
 {
-    const int avail = 227 * 1024 - 2128 - 512;
+    const int avail = 227 * 1024 - kSmemHdr;
     const int cands[4] = {16, 12, 8, 4};
     for (int i = 0; i < 4; ++i)
-        if ((size_t)cands[i] * (buf_bytes + 16) <= (size_t)avail) return cands[i];
+        if ((size_t)cands[i] * buf_bytes <= (size_t)avail) return cands[i];
     return 0;
 }
-static size_t decode_smem(int W, int buf_bytes) { return 2128 + 16 * W + 128 + (size_t)W * buf_bytes; }
+static size_t decode_smem(int W, int buf_bytes) { return kSmemHdr + (size_t)W * buf_bytes; }
 
 size_t decode_ws_bytes(const bgtq_layout *lay, int batch, int n_layers)
 {
