@@ -20,6 +20,7 @@
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
 
+#include <cstdlib>
 #include <utility>
 #include <vector>
 
@@ -147,21 +148,39 @@ __device__ __forceinline__ void decode_unit(const uint32_t (&w)[B], const uint32
                 h[wi * 4 + 2 * hf + 1] = prmt(lo4, hi4, 0x7362);
             }
     } else {
-        const uint16_t *T = lut + ((1 << B) - 1);
+        // byte offset of the table entry straight from the bit stream: one shift (funnel when the
+        // field straddles two words) + one mask, then LDS [offset + constant table address].
+        auto field_off = [&](int o, int nbits, int scale_log2) -> uint32_t {   // ((stream >> o) & (2^nbits-1)) << scale_log2
+            const int wi = o >> 5, sh = (o & 31) - scale_log2;
+            uint32_t x;
+            if (sh < 0) x = w[wi] << (-sh);
+            else if (sh + scale_log2 + nbits <= 32) x = w[wi] >> sh;
+            else x = __funnelshift_r(w[wi], w[wi + 1 < B ? wi + 1 : wi], sh);
+            return x & (((1u << nbits) - 1) << scale_log2);
+        };
+        if constexpr (B == 5) {      // pair table: 1024 half2 entries indexed by two adjacent 5-bit codes
+            const char *T2 = reinterpret_cast<const char *>(lut + 512);
 #pragma unroll
-        for (int j = 0; j < 16; ++j) {
-            uint32_t v[2];
+            for (int j = 0; j < 16; ++j) h[j] = *reinterpret_cast<const uint32_t *>(T2 + field_off(10 * j, 10, 2));
+        } else {
+            const char *T = reinterpret_cast<const char *>(lut + ((1 << B) - 1));
 #pragma unroll
-            for (int e = 0; e < 2; ++e) {
-                const int o = B * (2 * j + e), wi = o >> 5, sh = o & 31;
-                uint32_t x;
-                if (sh + B <= 32) x = w[wi] >> sh;
-                else x = __funnelshift_r(w[wi], w[wi + 1 < B ? wi + 1 : wi], sh);
-                v[e] = T[x & ((1u << B) - 1)];
+            for (int j = 0; j < 16; ++j) {
+                const uint32_t v0 = *reinterpret_cast<const uint16_t *>(T + field_off(B * (2 * j), B, 1));
+                const uint32_t v1 = *reinterpret_cast<const uint16_t *>(T + field_off(B * (2 * j + 1), B, 1));
+                h[j] = prmt(v0, v1, 0x5410);
             }
-            h[j] = v[0] | (v[1] << 16);
         }
     }
+}
+
+constexpr int kLutHalves = 512 + 2048;     // flat fp16 codebooks (C_b at 2^b-1) + the 5-bit pair table
+__device__ __forceinline__ void build_lut(const uint16_t *cb16_global, uint16_t *lut, int tid, int nthreads)
+{
+    for (int i = tid; i < 512; i += nthreads) lut[i] = cb16_global[i < 511 ? i : 510];
+    uint32_t *pair = reinterpret_cast<uint32_t *>(lut + 512);
+    for (int i = tid; i < 1024; i += nthreads)
+        pair[i] = (uint32_t)cb16_global[31 + (i & 31)] | ((uint32_t)cb16_global[31 + (i >> 5)] << 16);
 }
 
 __device__ __forceinline__ void build_pools(const uint16_t *cb16, uint32_t *pools)
@@ -299,7 +318,8 @@ struct DecodeParams {
     int buf_bytes;              // per-warp tile buffer
 };
 
-constexpr int kSmemHdr = 2560;  // [lut16 1024][pools 64][pre 1040][mbarriers 256], then the tile buffers
+constexpr int kSmemHdr = 0;      // dynamic shared memory holds only the tile buffers (tables are static)
+constexpr int kStaticSmem = 8 * 1024;   // upper bound of the kernel's static shared memory
 
 // load the B words of one unit for this lane.  FULL: 32 lanes per word plane (stride 32 words).
 template <int B>
@@ -321,33 +341,38 @@ __device__ __forceinline__ void load_unit_partial(const uint32_t *unit, int g8, 
 // QK^T of one same-width group: all its k16 steps, 8 m-tiles each.  m = coordinates in the
 // group; units of 8 coordinates are contiguous (128*B bytes each), only the last may be partial.
 template <int B>
-__device__ __forceinline__ void qk_group(const uint32_t *gcodes, int m, int lane, const uint2 *qfp,
+__device__ __forceinline__ void qk_group(const uint32_t *gcodes, int m, int lane, const uint2 *__restrict__ qfp,
                                          const uint32_t *pools, const uint16_t *lut, float (&A)[8][4])
 {
     const int g8 = lane >> 2, c = lane & 3;
     const int n_full = m >> 3, rem = (m & 7) >> 1;         // full units; lanes per row in the partial one
-    const int n_half = n_full + (rem ? 1 : 0);
+    const uint32_t *u0 = gcodes;
 #pragma unroll 1
-    for (int j = 0; j < n_half; j += 2) {
+    for (int jp = n_full >> 1; jp > 0; --jp) {              // pairs of full units: the tight loop
         uint32_t w0[B], w1[B], h0[16], h1[16];
-        const uint32_t *u0 = gcodes + j * 32 * B;
-        const uint2 bq = __ldg(qfp + (j >> 1) * 32);
-        if (j + 1 < n_full) {                               // common case: two full units
-            load_unit_full<B>(u0, lane, w0);
-            load_unit_full<B>(u0 + 32 * B, lane, w1);
-            decode_unit<B>(w0, pools, lut, h0);
+        const uint2 bq = __ldg(qfp);
+        load_unit_full<B>(u0, lane, w0);
+        load_unit_full<B>(u0 + 32 * B, lane, w1);
+        decode_unit<B>(w0, pools, lut, h0);
+        decode_unit<B>(w1, pools, lut, h1);
+#pragma unroll
+        for (int i = 0; i < 8; ++i) mma16816(A[i], h0[2 * i], h0[2 * i + 1], h1[2 * i], h1[2 * i + 1], bq.x, bq.y);
+        u0 += 64 * B;
+        qfp += 32;
+    }
+    if ((n_full & 1) | rem) {                               // tail k-step: full+partial, full+none or partial+none
+        uint32_t w0[B], h0[16], h1[16];
+        const uint2 bq = __ldg(qfp);
+        if (n_full & 1) load_unit_full<B>(u0, lane, w0);
+        else load_unit_partial<B>(u0, g8, c, rem, w0);
+        decode_unit<B>(w0, pools, lut, h0);
+        if ((n_full & 1) && rem) {
+            uint32_t w1[B];
+            load_unit_partial<B>(u0 + 32 * B, g8, c, rem, w1);
             decode_unit<B>(w1, pools, lut, h1);
         } else {
-            if (j < n_full) load_unit_full<B>(u0, lane, w0);
-            else load_unit_partial<B>(u0, g8, c, rem, w0);
-            decode_unit<B>(w0, pools, lut, h0);
-            if (j + 1 < n_half) {                           // second unit is the partial one
-                load_unit_partial<B>(u0 + 32 * B, g8, c, rem, w1);
-                decode_unit<B>(w1, pools, lut, h1);
-            } else {
 #pragma unroll
-                for (int i = 0; i < 16; ++i) h1[i] = 0u;
-            }
+            for (int i = 0; i < 16; ++i) h1[i] = 0u;
         }
 #pragma unroll
         for (int i = 0; i < 8; ++i) mma16816(A[i], h0[2 * i], h0[2 * i + 1], h1[2 * i], h1[2 * i + 1], bq.x, bq.y);
@@ -377,15 +402,15 @@ template <int W>
 __global__ void __launch_bounds__(W * 32, 1)
 decode_kernel(const DecodeParams P)
 {
-    extern __shared__ __align__(128) unsigned char smem[];
-    uint16_t *lut = reinterpret_cast<uint16_t *>(smem);
-    uint32_t *pools = reinterpret_cast<uint32_t *>(smem + 1024);
-    int *pre = reinterpret_cast<int *>(smem + 1024 + 64);
-    uint64_t *bars = reinterpret_cast<uint64_t *>(smem + 1024 + 64 + 1040 + 176);   // 2304, 8-byte aligned
+    extern __shared__ __align__(128) unsigned char smem[];       // the per-warp tile buffers only
+    __shared__ __align__(16) uint16_t lut[kLutHalves];            // static: constant LDS addresses for the LUTs
+    __shared__ uint32_t pools[16];
+    __shared__ int pre[kMaxBatch + 1];
+    __shared__ __align__(8) uint64_t bars[2 * W];
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int g8 = lane >> 2, c = lane & 3;
-    for (int i = tid; i < 512; i += W * 32) lut[i] = P.cb16[i < 511 ? i : 510];
+    build_lut(P.cb16, lut, tid, W * 32);
     if (tid == 0) build_prefix(P.seq_len, P.batch, P.n_cap * kTile, pre);
     __syncthreads();
     if (tid == 0) build_pools(lut, pools);
@@ -409,17 +434,21 @@ decode_kernel(const DecodeParams P)
     const uint32_t tile_s = smem_u32(tile);
     uint32_t kphase = 0, vphase = 0;
 
-    auto issue = [&](int xg, bool want_k, bool want_v) {      // lane 0: request (half of) global tile xg
-        const TilePos tp = locate(xg, S, pre);
-        const HeadMeta &M = P.metas[tp.l * P.Hkv + tp.h];
-        const uint8_t *src = P.cache + P.n_cap * ((int64_t)P.batch * M.layer_prefix + (int64_t)tp.b * M.layer_sum + M.head_prefix) +
-                             (int64_t)tp.t * M.tile_stride;
-        const uint32_t kbytes = M.vnorm_off, vbytes = M.tile_stride - M.vnorm_off;
+    // lane 0 requests (a half of) a tile: K half = [K codes | K norms], V half = [V norms | V codes]
+    auto issue_at = [&](const uint8_t *src, uint32_t kbytes, uint32_t vbytes, bool want_k, bool want_v) {
         fence_proxy_async();
         if (want_k) { mbar_expect_tx(kbar, kbytes); bulk_g2s(tile_s, src, kbytes, kbar); }
         if (want_v) { mbar_expect_tx(vbar, vbytes); bulk_g2s(tile_s + kbytes, src + kbytes, vbytes, vbar); }
     };
-    if (lane == 0) issue(x, true, true);
+    auto tile_src = [&](const TilePos &tp, const HeadMeta &M) -> const uint8_t * {
+        return P.cache + P.n_cap * ((int64_t)P.batch * M.layer_prefix + (int64_t)tp.b * M.layer_sum + M.head_prefix) +
+               (int64_t)tp.t * M.tile_stride;
+    };
+    {
+        const TilePos tp0 = locate(x, S, pre);
+        const HeadMeta &M0 = P.metas[tp0.l * P.Hkv + tp0.h];
+        if (lane == 0) issue_at(tile_src(tp0, M0), M0.vnorm_off, M0.tile_stride - M0.vnorm_off, true, true);
+    }
 
     while (x < x_end) {
         // ---------------- segment = the part of one (layer, sequence, kv head) inside this warp's range
@@ -438,6 +467,8 @@ decode_kernel(const DecodeParams P)
             gdesc = (uint32_t)M.goff[lane] | ((uint32_t)(M.gm[lane] & 0xFF) << 16) | ((uint32_t)M.gb[lane] << 24) | ((uint32_t)ksb << 28);
         }
         const uint2 *qfp = reinterpret_cast<const uint2 *>(P.qf + (size_t)tp.pair * kQfHalves) + lane;
+        const uint8_t *src = tile_src(tp, M);                     // current tile of this segment (advanced per tile)
+        const uint32_t stride = M.tile_stride, kbytes = M.vnorm_off, vbytes = stride - kbytes;
 
         float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;   // heads 2c, 2c+1 (log2 domain)
         float O[8][4];
@@ -485,7 +516,8 @@ decode_kernel(const DecodeParams P)
                 }
             }
             __syncwarp();
-            if (lane == 0 && x + 1 < seg_end) issue(x + 1, true, false);    // K half of the next tile (same layout only)
+            src += stride;
+            if (lane == 0 && x + 1 < seg_end) issue_at(src, kbytes, vbytes, true, false);   // K half of the next tile (same layout only)
 
             // ======== mask the ragged tail, online softmax (log2 domain)
             const int n_valid = (int)min((int64_t)kTile, slen - (int64_t)t * kTile);
@@ -552,7 +584,13 @@ decode_kernel(const DecodeParams P)
             default: pv_tile<8>(vcodes, lane, bP, pools, lut, O); break;
             }
             __syncwarp();
-            if (lane == 0 && x + 1 < x_end) issue(x + 1, x + 1 >= seg_end, true);   // V half (and K when the layout changes)
+            if (x + 1 < seg_end) {
+                if (lane == 0) issue_at(src, kbytes, vbytes, false, true);                   // V half of the next tile
+            } else if (x + 1 < x_end) {                                                      // next segment: other layout
+                const TilePos tn = locate(x + 1, S, pre);
+                const HeadMeta &Mn = P.metas[tn.l * P.Hkv + tn.h];
+                if (lane == 0) issue_at(tile_src(tn, Mn), Mn.vnorm_off, Mn.tile_stride - Mn.vnorm_off, true, true);
+            }
         }
 
         // ---------------- write this warp's partial for the pair: slot = warp + pair (unique, see combine)
@@ -622,10 +660,12 @@ combine_kernel(const float *__restrict__ partials, const int32_t *__restrict__ s
 // ---------------------------------------------------------------- host side
 static int pick_warps(int buf_bytes)
 {
-    const int avail = 227 * 1024 - kSmemHdr;
+    const int avail = 227 * 1024 - kStaticSmem;
     const int cands[4] = {16, 12, 8, 4};
+    int cap = 16;
+    if (const char *e = getenv("BGTQ_DECODE_WARPS")) cap = atoi(e);   // tuning knob (warps per CTA upper bound)
     for (int i = 0; i < 4; ++i)
-        if ((size_t)cands[i] * buf_bytes <= (size_t)avail) return cands[i];
+        if (cands[i] <= cap && (size_t)cands[i] * buf_bytes <= (size_t)avail) return cands[i];
     return 0;
 }
 static size_t decode_smem(int W, int buf_bytes) { return kSmemHdr + (size_t)W * buf_bytes; }
@@ -664,7 +704,7 @@ static int launch_decode_w(const DecodeParams &P, int grid, size_t smem, cudaStr
 {
     static bool attr_set = false;
     if (!attr_set) {   // once per process, outside any stream capture
-        CUDA_TRY(cudaFuncSetAttribute(decode_kernel<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        CUDA_TRY(cudaFuncSetAttribute(decode_kernel<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - kStaticSmem));
         attr_set = true;
     }
     cudaEvent_t e0 = nullptr, e1 = nullptr;
@@ -745,9 +785,9 @@ __device__ void debug_decode_b(const uint32_t *words, const uint32_t *pools, con
 }
 __global__ void debug_decode_kernel(int b, const uint32_t *words, const uint16_t *cb16, float *values)
 {
-    __shared__ uint16_t lut[512];
+    __shared__ __align__(16) uint16_t lut[kLutHalves];
     __shared__ uint32_t pools[16];
-    for (int i = threadIdx.x; i < 511; i += 32) lut[i] = cb16[i];
+    build_lut(cb16, lut, threadIdx.x, 32);
     __syncwarp();
     if (threadIdx.x == 0) build_pools(lut, pools);
     __syncwarp();
