@@ -168,6 +168,13 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
                 const double *x1 = x + tt_lo * 256;
                 double zz = 0.0;
                 int k = 0;
+                for (; k + 32 <= my_m; k += 32) {            // 32 independent loads in flight, then the chain
+                    float pf[32];
+#pragma unroll
+                    for (int u = 0; u < 32; ++u) pf[u] = __ldg(myrot + (size_t)(k + u) * my_m);
+#pragma unroll
+                    for (int u = 0; u < 32; ++u) zz = __fma_rn((double)pf[u], x1[k + u], zz);
+                }
                 for (; k + 8 <= my_m; k += 8) {
                     float pf[8];
 #pragma unroll

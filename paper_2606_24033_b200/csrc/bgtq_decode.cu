@@ -49,6 +49,14 @@ __device__ __forceinline__ void mma16816(float (&c)[4], uint32_t a0, uint32_t a1
                  : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
                  : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
 }
+// same with C = 0 (the zero register): starts an accumulator without a separate zero-fill
+__device__ __forceinline__ void mma16816_z(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2,
+                                           uint32_t a3, uint32_t b0, uint32_t b1)
+{
+    asm("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%10,%10,%10,%10};"
+        : "=f"(d[0]), "=f"(d[1]), "=f"(d[2]), "=f"(d[3])
+        : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1), "f"(0.f));
+}
 __device__ __forceinline__ uint32_t movmatrix_trans(uint32_t x)
 {
     uint32_t r;
@@ -96,6 +104,30 @@ __device__ __forceinline__ void fence_proxy_async()
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 }
 
+// Optional: shifts issued to the FMA pipe (IMAD) instead of the ALU pipe (tuning switches)
+__device__ __forceinline__ uint32_t shl_k(uint32_t x, int k)
+{
+#ifdef BGTQ_SHL_FMA
+    uint32_t r;
+    asm("mul.lo.u32 %0, %1, %2;" : "=r"(r) : "r"(x), "r"(1u << k));
+    return r;
+#else
+    return x << k;
+#endif
+}
+__device__ __forceinline__ uint32_t shr16(uint32_t x)
+{
+#ifdef BGTQ_SHR16_FMA
+    uint32_t r;
+    asm("mul.hi.u32 %0, %1, %2;" : "=r"(r) : "r"(x), "r"(0x10000u));
+    return r;
+#elif defined(BGTQ_SHR16_PRMT)
+    return prmt(x, 0u, 0x4432);
+#else
+    return x >> 16;
+#endif
+}
+
 // ---------------------------------------------------------------- unit decoders
 // A unit = B words per lane holding 32 slots.  Output: 16 half2 registers,
 // h[j] = (slot 2j, slot 2j+1) as fp16 codebook values (exact: the codebook is fp16).
@@ -112,7 +144,7 @@ __device__ __forceinline__ void decode_unit(const uint32_t (&w)[B], const uint32
     if constexpr (B == 1) {
         const uint32_t mag = pools[0];
 #pragma unroll
-        for (int j = 0; j < 16; ++j) h[j] = ((w[0] << j) & 0x80008000u) ^ mag;
+        for (int j = 0; j < 16; ++j) h[j] = ((j ? shl_k(w[0], j) : w[0]) & 0x80008000u) ^ mag;
     } else if constexpr (B == 2) {
         const uint32_t LO = pools[1], HI = pools[2];
 #pragma unroll
@@ -122,7 +154,7 @@ __device__ __forceinline__ void decode_unit(const uint32_t (&w)[B], const uint32
                 const uint32_t t = (w[wi] >> (2 * hf)) & 0x33333333u;
 #pragma unroll
                 for (int ql = 0; ql < 2; ++ql) {
-                    const uint32_t sel = ql ? (t >> 16) : t;
+                    const uint32_t sel = ql ? shr16(t) : t;
                     const uint32_t lo4 = prmt(LO, 0, sel), hi4 = prmt(HI, 0, sel);
                     const int Q = hf * 2 + ql;
                     h[wi * 8 + 2 * Q] = prmt(lo4, hi4, 0x5140);
@@ -141,9 +173,9 @@ __device__ __forceinline__ void decode_unit(const uint32_t (&w)[B], const uint32
         for (int wi = 0; wi < 4; ++wi)
 #pragma unroll
             for (int hf = 0; hf < 2; ++hf) {
-                const uint32_t sel = hf ? (t[wi] >> 16) : t[wi];
+                const uint32_t sel = hf ? shr16(t[wi]) : t[wi];
                 uint32_t lo4 = prmt(LOa, LOb, sel), hi4 = prmt(HIa, HIb, sel);
-                if constexpr (B == 4) hi4 ^= (w[3] << (2 * wi + hf)) & 0x80808080u;   // sign of slot 4Q+e: bit 8e+7-Q
+                if constexpr (B == 4) hi4 ^= ((2 * wi + hf) ? shl_k(w[3], 2 * wi + hf) : w[3]) & 0x80808080u;   // sign of slot 4Q+e: bit 8e+7-Q
                 h[wi * 4 + 2 * hf] = prmt(lo4, hi4, 0x5140);
                 h[wi * 4 + 2 * hf + 1] = prmt(lo4, hi4, 0x7362);
             }
@@ -283,13 +315,13 @@ qfold_kernel(const HeadMeta *__restrict__ metas, const float *__restrict__ rot_t
         float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
         const uint8_t *co = M.coords + x0;
         int k = 0;
-        for (; k + 4 <= m; k += 4) {                    // m is even; rotation rows read 4 ahead of the FMAs
-            float tv[4];
-            int cc[4];
+        for (; k + 16 <= m; k += 16) {                  // 16 independent rotation loads in flight per thread
+            float tv[16];
+            int cc[16];
 #pragma unroll
-            for (int u = 0; u < 4; ++u) { tv[u] = __ldg(T + (size_t)(k + u) * m); cc[u] = co[k + u]; }
+            for (int u = 0; u < 16; ++u) { tv[u] = __ldg(T + (size_t)(k + u) * m); cc[u] = co[k + u]; }
 #pragma unroll
-            for (int u = 0; u < 4; ++u)
+            for (int u = 0; u < 16; ++u)
 #pragma unroll
                 for (int n = 0; n < 8; ++n) if (n < G) acc[n] = fmaf(tv[u], qs[n * kDh + cc[u]], acc[n]);
         }
@@ -347,6 +379,7 @@ __device__ __forceinline__ void qk_group(const uint32_t *gcodes, int m, int lane
     const int g8 = lane >> 2, c = lane & 3;
     const int n_full = m >> 3, rem = (m & 7) >> 1;         // full units; lanes per row in the partial one
     const uint32_t *u0 = gcodes;
+    bool first = true;                                      // the group's first k-step starts the accumulators (C = 0)
 #pragma unroll 1
     for (int jp = n_full >> 1; jp > 0; --jp) {              // pairs of full units: the tight loop
         uint32_t w0[B], w1[B], h0[16], h1[16];
@@ -355,8 +388,14 @@ __device__ __forceinline__ void qk_group(const uint32_t *gcodes, int m, int lane
         load_unit_full<B>(u0 + 32 * B, lane, w1);
         decode_unit<B>(w0, pools, lut, h0);
         decode_unit<B>(w1, pools, lut, h1);
+        if (first) {
 #pragma unroll
-        for (int i = 0; i < 8; ++i) mma16816(A[i], h0[2 * i], h0[2 * i + 1], h1[2 * i], h1[2 * i + 1], bq.x, bq.y);
+            for (int i = 0; i < 8; ++i) mma16816_z(A[i], h0[2 * i], h0[2 * i + 1], h1[2 * i], h1[2 * i + 1], bq.x, bq.y);
+            first = false;
+        } else {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) mma16816(A[i], h0[2 * i], h0[2 * i + 1], h1[2 * i], h1[2 * i + 1], bq.x, bq.y);
+        }
         u0 += 64 * B;
         qfp += 32;
     }
@@ -374,8 +413,13 @@ __device__ __forceinline__ void qk_group(const uint32_t *gcodes, int m, int lane
 #pragma unroll
             for (int i = 0; i < 16; ++i) h1[i] = 0u;
         }
+        if (first) {
 #pragma unroll
-        for (int i = 0; i < 8; ++i) mma16816(A[i], h0[2 * i], h0[2 * i + 1], h1[2 * i], h1[2 * i + 1], bq.x, bq.y);
+            for (int i = 0; i < 8; ++i) mma16816_z(A[i], h0[2 * i], h0[2 * i + 1], h1[2 * i], h1[2 * i + 1], bq.x, bq.y);
+        } else {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) mma16816(A[i], h0[2 * i], h0[2 * i + 1], h1[2 * i], h1[2 * i + 1], bq.x, bq.y);
+        }
     }
 }
 
@@ -489,9 +533,7 @@ decode_kernel(const DecodeParams P)
                 m = m ? m : 128;
                 const uint32_t *gcodes = tile + ((d & 0xFFFF) >> 2);
                 const uint2 *qg = qfp + (d >> 28) * 32;
-                float A[8][4];
-#pragma unroll
-                for (int i = 0; i < 8; ++i) A[i][0] = A[i][1] = A[i][2] = A[i][3] = 0.f;
+                float A[8][4];                               // started by the group's first k-step (m >= 2)
                 switch ((d >> 24) & 0xF) {
                 case 1: qk_group<1>(gcodes, m, lane, qg, pools, lut, A); break;
                 case 2: qk_group<2>(gcodes, m, lane, qg, pools, lut, A); break;
@@ -639,7 +681,7 @@ combine_kernel(const float *__restrict__ partials, const int32_t *__restrict__ s
     const int w0 = start / S.per_warp, w1 = (start + tiles_b - 1) / S.per_warp;
     float Mx = -INFINITY, acc = 0.f, lsum = 0.f;       // single pass, running max (exact: PAPER.md:120)
     const float *rec0 = partials + (size_t)pair * kPartialFloats + n * 130;
-#pragma unroll 4
+#pragma unroll 8
     for (int w = w0; w <= w1; ++w) {
         const float *rec = rec0 + (size_t)w * kPartialFloats;
         const float mw = rec[0], lw = rec[1], aw = rec[2 + d];
@@ -652,7 +694,7 @@ combine_kernel(const float *__restrict__ partials, const int32_t *__restrict__ s
     o[d] = acc / lsum;
     __syncthreads();
     float r = 0.f;
-#pragma unroll 8
+#pragma unroll 32
     for (int j = 0; j < kDh; ++j) r = fmaf(__ldg(rot128 + j * kDh + d), o[j], r);
     dst[d] = __float2bfloat16(r * 0.08838834764831845f);     // 1/sqrt(128)
 }
@@ -742,7 +784,7 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
     count_launch();
     CUDA_TRY(cudaGetLastError());
 
-    const int buf_bytes = (lay->max_stride + 127) / 128 * 128;
+    const int buf_bytes = (lay->max_stride + 127) / 128 * 128;   // 128-byte aligned tile buffers
     const int W = pick_warps(buf_bytes);
     if (!W) { set_error("bgtq_decode_attention: tile does not fit shared memory"); return BGTQ_EINVAL; }
     DecodeParams P;
