@@ -235,8 +235,14 @@ struct Sched {
     int n_layers, batch, Hkv;
     int tiles_sum;          // sum over sequences of ceil(seq_len/128)
     int total;              // n_layers * Hkv * tiles_sum
-    int per_warp;           // ceil(total / n_warps)
+    int n_ctas, W;          // balanced two-level split: CTA c owns [cta_lo(c), cta_lo(c+1)), its W warps split that evenly
 };
+__device__ __forceinline__ int cta_lo(const Sched &s, int c) { return (int)(((int64_t)c * s.total) / s.n_ctas); }
+__device__ __forceinline__ int warp_lo(const Sched &s, int c, int w)
+{
+    const int lo = cta_lo(s, c), len = cta_lo(s, c + 1) - lo;
+    return lo + (int)(((int64_t)w * len) / s.W);
+}
 
 __device__ __forceinline__ void build_prefix(const int32_t *seq_len, int batch, int64_t cap_tokens, int *pre)
 {
@@ -251,13 +257,13 @@ __device__ __forceinline__ void build_prefix(const int32_t *seq_len, int batch, 
     }
 }
 
-__device__ __forceinline__ Sched make_sched(int n_layers, int batch, int Hkv, const int *pre, int n_warps)
+__device__ __forceinline__ Sched make_sched(int n_layers, int batch, int Hkv, const int *pre, int n_ctas, int W)
 {
     Sched s;
     s.n_layers = n_layers; s.batch = batch; s.Hkv = Hkv;
     s.tiles_sum = pre[batch];
     s.total = n_layers * Hkv * s.tiles_sum;
-    s.per_warp = s.total > 0 ? (s.total + n_warps - 1) / n_warps : 1;
+    s.n_ctas = n_ctas; s.W = W;
     return s;
 }
 
@@ -290,20 +296,23 @@ qfold_kernel(const HeadMeta *__restrict__ metas, const float *__restrict__ rot_t
              const __nv_bfloat16 *__restrict__ q, int batch, int Hkv, int Hq, float scale_log2e,
              __half *__restrict__ qf)
 {
-    const int pair = blockIdx.x;                       // (l*batch + b)*Hkv + h  (l relative to layer0)
-    const int h = pair % Hkv, lb = pair / Hkv, l = lb / batch;
     const int G = Hq / Hkv;
+    const int pair = blockIdx.x / G, n = blockIdx.x % G;   // one block per (pair, query head of the group)
+    const int h = pair % Hkv, lb = pair / Hkv, l = lb / batch;
     const HeadMeta &M = metas[l * Hkv + h];
-    __shared__ float qs[8 * kDh];
+    __shared__ float qs[kDh];
     __shared__ int ksbase[kMaxGroups];
     const int tid = threadIdx.x;
-    for (int e = tid; e < G * kDh; e += 128)
-        qs[e] = __bfloat162float(q[((size_t)lb * Hq + h * G) * kDh + e]);
+    qs[tid] = __bfloat162float(q[((size_t)lb * Hq + h * G + n) * kDh + tid]);
     if (tid == 0)
         for (int ks = 0; ks < M.n_ksteps; ++ks)
             if (M.ksteps[ks].flags & 1) ksbase[M.ksteps[ks].flags >> 4] = ks;
-    __half *out = qf + (size_t)pair * kQfHalves;
-    for (int e = tid; e < kQfHalves; e += 128) out[e] = __float2half(0.f);
+    // zero padding: this head's slots (and, from block n = 0, the unused head slots n >= G)
+    uint2 *out2 = reinterpret_cast<uint2 *>(qf + (size_t)pair * kQfHalves);     // [kstep][8][4] of 4 halves
+    for (int e = tid; e < kMaxKSteps * 32; e += 128) {
+        const int nn = (e >> 2) & 7;
+        if (nn == n || (n == 0 && nn >= G)) out2[e] = make_uint2(0u, 0u);
+    }
     __syncthreads();
     if (tid < M.kdim) {
         int g = 0;
@@ -312,28 +321,19 @@ qfold_kernel(const HeadMeta *__restrict__ metas, const float *__restrict__ rot_t
         const float *T = rot_t + rot_offset(m) + r;
         const float sc = scale_log2e / sqrtf((float)m);
         const int ks = ksbase[g] + (r >> 4), kap = r & 15;
-        float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
         const uint8_t *co = M.coords + x0;
+        float acc = 0.f;
         int k = 0;
         for (; k + 16 <= m; k += 16) {                  // 16 independent rotation loads in flight per thread
             float tv[16];
-            int cc[16];
 #pragma unroll
-            for (int u = 0; u < 16; ++u) { tv[u] = __ldg(T + (size_t)(k + u) * m); cc[u] = co[k + u]; }
+            for (int u = 0; u < 16; ++u) tv[u] = __ldg(T + (size_t)(k + u) * m);
 #pragma unroll
-            for (int u = 0; u < 16; ++u)
-#pragma unroll
-                for (int n = 0; n < 8; ++n) if (n < G) acc[n] = fmaf(tv[u], qs[n * kDh + cc[u]], acc[n]);
+            for (int u = 0; u < 16; ++u) acc = fmaf(tv[u], qs[co[k + u]], acc);
         }
-        for (; k < m; ++k) {
-            const float tv = __ldg(T + (size_t)k * m);
-            const int cc = co[k];
-#pragma unroll
-            for (int n = 0; n < 8; ++n) if (n < G) acc[n] = fmaf(tv, qs[n * kDh + cc], acc[n]);
-        }
-#pragma unroll
-        for (int n = 0; n < 8; ++n)
-            if (n < G) out[((ks * 8 + n) * 4 + ((kap & 7) >> 1)) * 4 + (kap >> 3) * 2 + (kap & 1)] = __float2half_rn(acc[n] * sc);
+        for (; k < m; ++k) acc = fmaf(__ldg(T + (size_t)k * m), qs[co[k]], acc);
+        __half *out = qf + (size_t)pair * kQfHalves;
+        out[((ks * 8 + n) * 4 + ((kap & 7) >> 1)) * 4 + (kap >> 3) * 2 + (kap & 1)] = __float2half_rn(acc * sc);
     }
 }
 
@@ -467,12 +467,23 @@ decode_kernel(const DecodeParams P)
     }
     __syncthreads();
 
-    const int n_warps = gridDim.x * W;
     const int gw = blockIdx.x * W + warp;
-    const Sched S = make_sched(P.n_layers, P.batch, P.Hkv, pre, n_warps);
-    int x = gw * S.per_warp;
-    const int x_end = min(S.total, x + S.per_warp);
-    if (x >= x_end) return;
+    const Sched S = make_sched(P.n_layers, P.batch, P.Hkv, pre, gridDim.x, W);
+    int x = warp_lo(S, blockIdx.x, warp);
+    const int x_end = warp_lo(S, blockIdx.x, warp + 1);
+    // CTA-level merge: when the whole CTA range lies inside one (layer, sequence, kv head) pair, the warps'
+    // partials are merged in shared memory and ONE partial per CTA goes to HBM (slot of the CTA's warp 0).
+    bool merged = false;
+    int merged_pair = 0;
+    {
+        const int c_lo = cta_lo(S, blockIdx.x), c_hi = cta_lo(S, blockIdx.x + 1);
+        if (c_lo < c_hi) {
+            const TilePos tc = locate(c_lo, S, pre);
+            merged = c_hi <= tc.pair_start + tc.tiles_b;
+            merged_pair = tc.pair;
+        }
+    }
+    if (!merged && x >= x_end) return;
 
     const uint32_t *tile = reinterpret_cast<const uint32_t *>(smem + kSmemHdr + warp * P.buf_bytes);
     const uint32_t tile_s = smem_u32(tile);
@@ -488,10 +499,13 @@ decode_kernel(const DecodeParams P)
         return P.cache + P.n_cap * ((int64_t)P.batch * M.layer_prefix + (int64_t)tp.b * M.layer_sum + M.head_prefix) +
                (int64_t)tp.t * M.tile_stride;
     };
-    {
+    if (x < x_end) {
         const TilePos tp0 = locate(x, S, pre);
         const HeadMeta &M0 = P.metas[tp0.l * P.Hkv + tp0.h];
         if (lane == 0) issue_at(tile_src(tp0, M0), M0.vnorm_off, M0.tile_stride - M0.vnorm_off, true, true);
+    } else {                                   // idle warp of a merged CTA: contributes an empty partial
+        float *rec = reinterpret_cast<float *>(smem + kSmemHdr + warp * P.buf_bytes);
+        for (int i = lane; i < kPartialFloats; i += 32) rec[i] = (i % 130 == 0) ? -INFINITY : 0.f;
     }
 
     while (x < x_end) {
@@ -641,7 +655,8 @@ decode_kernel(const DecodeParams P)
             l0 += __shfl_xor_sync(0xFFFFFFFFu, l0, o);
             l1 += __shfl_xor_sync(0xFFFFFFFFu, l1, o);
         }
-        float *rec = P.partials + (size_t)(gw + tp.pair) * kPartialFloats;
+        float *rec = merged ? reinterpret_cast<float *>(smem + kSmemHdr + warp * P.buf_bytes)
+                            : P.partials + (size_t)(gw + tp.pair) * kPartialFloats;
         const int n0 = 2 * c, n1 = 2 * c + 1;
         if (n0 < P.G) {
             float *r0 = rec + n0 * 130;
@@ -656,6 +671,29 @@ decode_kernel(const DecodeParams P)
             for (int J = 0; J < 8; ++J) { r1[2 + 16 * J + g8] = O[J][1]; r1[2 + 16 * J + 8 + g8] = O[J][3]; }
         }
     }
+    if (merged) {      // exact log-sum-exp merge of the W warp partials, one record per CTA
+        __syncthreads();
+        const float *all = reinterpret_cast<const float *>(smem + kSmemHdr);
+        const int fstride = P.buf_bytes >> 2;
+        float *dst = P.partials + (size_t)(blockIdx.x * W + merged_pair) * kPartialFloats;
+        for (int e = tid; e < 8 * 128; e += W * 32) {
+            const int n = e >> 7, dd = e & 127;
+            if (n >= P.G) continue;
+            float Mx = -INFINITY;
+#pragma unroll
+            for (int w = 0; w < W; ++w) Mx = fmaxf(Mx, all[w * fstride + n * 130]);
+            float acc = 0.f, ls = 0.f;
+#pragma unroll
+            for (int w = 0; w < W; ++w) {
+                const float *r = all + w * fstride + n * 130;
+                const float f = fast_exp2(r[0] - Mx);
+                acc = fmaf(r[2 + dd], f, acc);
+                ls = fmaf(r[1], f, ls);
+            }
+            dst[n * 130 + 2 + dd] = acc;
+            if (dd == 0) { dst[n * 130] = Mx; dst[n * 130 + 1] = ls; }
+        }
+    }
 }
 
 // ---------------------------------------------------------------- a6: exact LSE merge + V de-rotation
@@ -664,32 +702,62 @@ decode_kernel(const DecodeParams P)
 __global__ void __launch_bounds__(128)
 combine_kernel(const float *__restrict__ partials, const int32_t *__restrict__ seq_len,
                const float *__restrict__ rot128, int n_layers, int batch, int Hkv, int G, int64_t n_cap,
-               int n_warps, __nv_bfloat16 *__restrict__ out)
+               int n_ctas, int W, __nv_bfloat16 *__restrict__ out)
 {
+    constexpr int kMaxSlots = 1024;
     __shared__ int pre[kMaxBatch + 1];
     __shared__ float o[kDh];
+    __shared__ int slots[kMaxSlots];
     const int pair = blockIdx.x / G, n = blockIdx.x % G;
     const int h = pair % Hkv, lb = pair / Hkv, b = lb % batch, l = lb / batch;
     const int d = threadIdx.x;
     if (d == 0) build_prefix(seq_len, batch, n_cap * kTile, pre);
     __syncthreads();
-    const Sched S = make_sched(n_layers, batch, Hkv, pre, n_warps);
+    const Sched S = make_sched(n_layers, batch, Hkv, pre, n_ctas, W);
     const int tiles_b = pre[b + 1] - pre[b];
     __nv_bfloat16 *dst = out + ((size_t)lb * Hkv * G + h * G + n) * kDh;
     if (tiles_b == 0) { dst[d] = __float2bfloat16(0.f); return; }
-    const int start = l * (Hkv * S.tiles_sum) + pre[b] * Hkv + h * tiles_b;
-    const int w0 = start / S.per_warp, w1 = (start + tiles_b - 1) / S.per_warp;
-    float Mx = -INFINITY, acc = 0.f, lsum = 0.f;       // single pass, running max (exact: PAPER.md:120)
+    const int start = l * (Hkv * S.tiles_sum) + pre[b] * Hkv + h * tiles_b, stop = start + tiles_b;
+    // CTAs whose range meets [start, stop): the decode kernel's balanced split, recomputed
+    int c0 = (int)(((int64_t)start * S.n_ctas) / S.total), c1 = (int)(((int64_t)(stop - 1) * S.n_ctas) / S.total);
+    while (c0 + 1 < S.n_ctas && cta_lo(S, c0 + 1) <= start) ++c0;
+    while (c0 > 0 && cta_lo(S, c0) > start) --c0;
+    while (c1 + 1 < S.n_ctas && cta_lo(S, c1 + 1) <= stop - 1) ++c1;
+    while (c1 > 0 && cta_lo(S, c1) > stop - 1) --c1;
+    // slot list in a fixed order: [warps of the first CTA][interior CTAs][warps of the last CTA].  Interior
+    // CTAs lie wholly inside the pair, so they merged their warps (one record at the slot of warp 0); a CTA
+    // straddling the pair boundary left one record per warp.
+    float Mx = -INFINITY, acc = 0.f, lsum = 0.f;       // single pass with a running max (exact: PAPER.md:120)
     const float *rec0 = partials + (size_t)pair * kPartialFloats + n * 130;
+    auto edge_slot = [&](int c, int w) -> int {         // record of warp w of boundary CTA c, or -1
+        const int lo = cta_lo(S, c), hi = cta_lo(S, c + 1);
+        if (lo >= start && hi <= stop) return (w == 0 && lo < hi) ? c * W : -1;
+        if (w >= W) return -1;
+        const int wl = warp_lo(S, c, w), wh = warp_lo(S, c, w + 1);
+        return (wl < wh && wl < stop && wh > start) ? c * W + w : -1;
+    };
+    const int n_int = c1 - c0 - 1 > 0 ? c1 - c0 - 1 : 0;
+    const int n_ent = 16 + n_int + (c1 > c0 ? 16 : 0);
+    for (int eb = 0; eb < n_ent; eb += kMaxSlots) {
+        const int ne = min(kMaxSlots, n_ent - eb);
+        __syncthreads();
+        for (int e = d; e < ne; e += 128) {
+            const int ge = eb + e;
+            slots[e] = ge < 16 ? edge_slot(c0, ge) : (ge < 16 + n_int ? edge_slot(c0 + 1 + ge - 16, 0) : edge_slot(c1, ge - 16 - n_int));
+        }
+        __syncthreads();
 #pragma unroll 8
-    for (int w = w0; w <= w1; ++w) {
-        const float *rec = rec0 + (size_t)w * kPartialFloats;
-        const float mw = rec[0], lw = rec[1], aw = rec[2 + d];
-        const float Mn = fmaxf(Mx, mw);
-        const float fo = exp2f(Mx - Mn), fw = exp2f(mw - Mn);
-        lsum = fmaf(lsum, fo, lw * fw);
-        acc = fmaf(acc, fo, aw * fw);
-        Mx = Mn;
+        for (int e = 0; e < ne; ++e) {
+            const int sl = slots[e];
+            const float *rec = rec0 + (size_t)(sl < 0 ? 0 : sl) * kPartialFloats;
+            const float mw = sl < 0 ? -INFINITY : rec[0];
+            const float lw = sl < 0 ? 0.f : rec[1], aw = sl < 0 ? 0.f : rec[2 + d];
+            const float Mn = fmaxf(Mx, mw);
+            const float fo = Mn == -INFINITY ? 0.f : exp2f(Mx - Mn), fw = Mn == -INFINITY ? 0.f : exp2f(mw - Mn);
+            lsum = fmaf(lsum, fo, lw * fw);
+            acc = fmaf(acc, fo, aw * fw);
+            Mx = Mn;
+        }
     }
     o[d] = acc / lsum;
     __syncthreads();
@@ -779,7 +847,7 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
     float *partials = reinterpret_cast<float *>(reinterpret_cast<unsigned char *>(ws) + (size_t)pairs * kQfHalves * sizeof(__half));
     const HeadMeta *metas = lay->d_meta + (size_t)layer0 * Hkv;
 
-    qfold_kernel<<<pairs, 128, 0, st>>>(metas, lay->d_rot_t, (const __nv_bfloat16 *)q, batch, Hkv, Hq,
+    qfold_kernel<<<pairs * G, 128, 0, st>>>(metas, lay->d_rot_t, (const __nv_bfloat16 *)q, batch, Hkv, Hq,
                                         scale * 1.4426950408889634f, qf);
     count_launch();
     CUDA_TRY(cudaGetLastError());
@@ -805,7 +873,7 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
     CUDA_TRY(cudaGetLastError());
 
     combine_kernel<<<pairs * G, 128, 0, st>>>(partials, seq_len, lay->d_rot + rot_offset(kDh), n_layers, batch,
-                                              Hkv, G, n_cap, grid * W, (__nv_bfloat16 *)out);
+                                              Hkv, G, n_cap, grid, W, (__nv_bfloat16 *)out);
     count_launch();
     CUDA_TRY(cudaGetLastError());
     return BGTQ_OK;
