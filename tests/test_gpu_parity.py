@@ -202,3 +202,118 @@ def test_attention_empty_sequence_is_zero(P):
     q = _cuda(p.q_post[None], torch.bfloat16)
     out = P.decode_attention(lay, 0, cache, q, seq, 128, 0.1, lay.new_workspace(1))
     assert torch.all(out == 0)
+
+
+# ----------------------------------------------------------------------------- batched layers / sequences
+def test_layers_batched_and_ragged_batch(P, tab128):
+    """bgtq_quantize_append_layers + bgtq_decode_attention_layers over 3 layers x 2 sequences of different
+    lengths (one launch) == per-layer calls == oracle, with a different allocation per (layer, head)."""
+    Lyr, B, Hq, Hkv, d = 3, 2, 8, 2, 128
+    lens = [389, 150]
+    probs = [[H.make_problem(60 + 10 * l + b, lens[b], Hq, Hkv, 3, 3, 1, 8, rope_base=1e6) for b in range(B)] for l in range(Lyr)]
+    for l in range(Lyr):                       # one allocation per layer (from sequence 0's statistics)
+        for b in range(B):
+            probs[l][b].bits = probs[l][0].bits
+    bits = np.stack([probs[l][0].bits for l in range(Lyr)])
+    lay = P.Layout(bits, Hq, d, 3, probs[0][0].rot)
+    max_tokens = 512
+    cache = lay.new_cache(B, max_tokens)
+    seq = torch.zeros(B, dtype=torch.int32, device="cuda")
+    # first 150 tokens of both sequences in one layers-batched call, then the rest of sequence 0 per layer
+    k0 = np.stack([np.stack([probs[l][b].k_post[:150] for b in range(B)]) for l in range(Lyr)])
+    v0 = np.stack([np.stack([probs[l][b].v[:150] for b in range(B)]) for l in range(Lyr)])
+    P.quantize_append(lay, 0, cache, _cuda(k0, torch.float32), _cuda(v0, torch.float32), seq, max_tokens, n_layers=Lyr)
+    assert seq.tolist() == [150, 150]
+    rest = lens[0] - 150
+    for l in range(Lyr):
+        kk = np.zeros((B, rest, Hkv, d)); vv = np.zeros((B, rest, Hkv, d))
+        kk[0] = probs[l][0].k_post[150:]; vv[0] = probs[l][0].v[150:]
+        seq_l = torch.tensor([150, max_tokens], dtype=torch.int32, device="cuda")   # sequence 1 is "full": nothing appended
+        P.quantize_append(lay, l, cache, _cuda(kk, torch.float32), _cuda(vv, torch.float32), seq_l, max_tokens,
+                          advance_seq_len=False)
+    seq = torch.tensor(lens, dtype=torch.int32, device="cuda")
+    host = cache.cpu().numpy()
+    heads = [[H.oracle_heads(probs[l][b], tab128) for b in range(B)] for l in range(Lyr)]
+    n_cap = max_tokens // 128
+    for l in range(Lyr):
+        for b in range(B):
+            for h in range(Hkv):
+                stride = lay.tile_stride(l, h)
+                off = lay.region_offset(l, b, h, B, max_tokens)
+                exp = np.zeros(n_cap * stride, dtype=np.uint8)
+                O.pack_region(heads[l][b][h], d, exp)
+                assert np.array_equal(host[off:off + n_cap * stride], exp), (l, b, h)
+    scale = 1.0 / math.sqrt(d)
+    q = np.stack([np.stack([probs[l][b].q_post for b in range(B)]) for l in range(Lyr)])       # [Lyr,B,Hq,d]
+    qd = _cuda(q, torch.bfloat16)
+    out_b = P.decode_attention(lay, 0, cache, qd, seq, max_tokens, scale, lay.new_workspace(B, Lyr), n_layers=Lyr)
+    ws1 = lay.new_workspace(B, 1)
+    out_l = torch.stack([P.decode_attention(lay, l, cache, qd[l].contiguous(), seq, max_tokens, scale, ws1) for l in range(Lyr)])
+    torch.cuda.synchronize()
+    for l in range(Lyr):
+        for b in range(B):
+            exp, rv = H.oracle_attention(probs[l][b], heads[l][b], tab128, scale)
+            for name, out in (("batched", out_b), ("per-layer", out_l)):
+                got = out[l, b].double().cpu().numpy()
+                err = max(np.max(np.abs(got[a] - exp[a])) / rv[a // (Hq // Hkv)] for a in range(Hq))
+                assert err <= 2e-3, (name, l, b, err)
+
+
+def test_gpu_generator_rope_matches_oracle(P):
+    """workloads/gpu_synth.py shapes inputs only, but its RoPE is still checked against the oracle's."""
+    from workloads import gpu_synth as GS
+    x = torch.randn((50, 3, 128), dtype=torch.float64, device="cuda")
+    pos = torch.arange(1000, 1050, dtype=torch.float64, device="cuda")
+    got = GS.rope_half(x, pos, 1e6).cpu().numpy()
+    exp = O.rope(x.cpu().numpy(), pos.cpu().numpy(), 1e6)
+    assert np.max(np.abs(got - exp)) < 1e-9
+
+
+@pytest.mark.timeout(900)
+def test_full_size_128k_sampled_head(P, tab128):
+    """BASELINE.json configs[2] at full context (131,072 tokens) in the launch configuration bench.py times
+    (layers batched in one launch): the packed region and the attention output of one sampled
+    (layer, KV head) are checked against the oracle run on the SAME input tensors (copied to the host)."""
+    from workloads import gpu_synth as GS
+    shp = W.CONFIGS[2]
+    Lyr, T, d, Hq, Hkv = 2, 131072, shp.d_h, shp.n_q_heads, shp.n_kv_heads
+    kv, scores, scales_all = [], [], []
+    for l in range(Lyr):
+        ks, vs = [], []
+        for c0 in range(0, T, 32768):
+            k, v, scales = GS.layer_kv(shp.seed0 + l, 32768, Hkv, d, shp.rope_base, "cuda", t0=c0, chunk_tag=c0 // 32768)
+            ks.append(k); vs.append(v)
+        k, v = torch.cat(ks), torch.cat(vs)
+        qcal = GS.layer_queries(shp.seed0 + l, shp.n_cal, Hq, scales, d, shp.rope_base, 0, "cuda", tag=4)
+        scores.append(P.block_energy(qcal, k))
+        kv.append((k, v)); scales_all.append(scales)
+    bits = P.allocate(torch.cat(scores), shp.b_k * 64, shp.b_min, shp.b_max).cpu().numpy().reshape(Lyr, Hkv, 64)
+    lay = P.Layout(bits, Hq, d, shp.b_v, tab128.rot)
+    max_tokens = T
+    cache = lay.new_cache(1, max_tokens)
+    seq = torch.zeros(1, dtype=torch.int32, device="cuda")
+    for l in range(Lyr):
+        seq.zero_()
+        P.quantize_append(lay, l, cache, kv[l][0][None].contiguous(), kv[l][1][None].contiguous(), seq, max_tokens)
+    q = torch.stack([GS.layer_queries(shp.seed0 + l, 1, Hq, scales_all[l], d, shp.rope_base, T, "cuda", tag=3,
+                                      dtype=torch.bfloat16) for l in range(Lyr)])
+    scale = 1.0 / math.sqrt(d)
+    out = P.decode_attention(lay, 0, cache, q, seq, max_tokens, scale, lay.new_workspace(1, Lyr), n_layers=Lyr)
+    torch.cuda.synchronize()
+    l, h = 1, 1                                                    # the sampled (layer, KV head)
+    k_h = kv[l][0][:, h].double().cpu().numpy()
+    v_h = kv[l][1][:, h].double().cpu().numpy()
+    head = O.quantize_head(k_h, v_h, bits[l, h], shp.b_v, tab128)
+    stride = lay.tile_stride(l, h)
+    off = lay.region_offset(l, 0, h, 1, max_tokens)
+    exp = np.zeros((T // 128) * stride, dtype=np.uint8)
+    O.pack_region(head, d, exp)
+    got = cache[off:off + exp.size].cpu().numpy()
+    assert np.array_equal(got, exp), "packed region differs at full size"
+    G = Hq // Hkv
+    q_h = q[l, 0, h * G:(h + 1) * G].double().cpu().numpy()
+    ref = O.decode_attention_head(q_h, head, tab128, d, scale)
+    _, V = O.dequantize_head(head, tab128, d)
+    rv = math.sqrt(np.mean(np.sum(V * V, axis=1)))
+    err = np.max(np.abs(out[l, 0, h * G:(h + 1) * G].double().cpu().numpy() - ref)) / rv
+    assert err <= 2e-3, err
