@@ -100,7 +100,7 @@ class ClockSampler:
                         self.reasons.add(name)
             except Exception:
                 pass
-            self._stop.wait(0.02)
+            self._stop.wait(0.002)
 
     def __enter__(self):
         if self._nv is not None:
@@ -406,7 +406,7 @@ def run_ours(args):
         one_pass, nbytes, t_quant = oracle_sample(args, T_s)
         one_pass()
         reps, tt = 0, 0.0
-        while tt < 10.0 and reps < 50:
+        while tt < 12.0 and reps < 400:
             tt += one_pass()
             reps += 1
         cpu_baseline = {"value": nbytes / (tt / reps) / 1e9, "unit": "GB/s", "cores": blas_threads(), "kind": "oracle",
