@@ -137,7 +137,7 @@ __device__ __forceinline__ uint32_t shr16(uint32_t x)
 //   [3..6]   b=3: low bytes of levels 0..3, 4..7; high bytes of levels 0..3, 4..7
 //   [7..10]  b=4: same for the 8 magnitudes C_4[8..15] (codes are stored sign-magnitude)
 // lut: fp16 bits of the flat codebook table in shared memory (C_b at 2^b - 1), for b >= 5.
-template <int B>
+template <int B, bool P5 = true>
 __device__ __forceinline__ void decode_unit(const uint32_t (&w)[B], const uint32_t *pools,
                                             const uint16_t *lut, uint32_t (&h)[16])
 {
@@ -190,7 +190,7 @@ __device__ __forceinline__ void decode_unit(const uint32_t (&w)[B], const uint32
             else x = __funnelshift_r(w[wi], w[wi + 1 < B ? wi + 1 : wi], sh);
             return x & (((1u << nbits) - 1) << scale_log2);
         };
-        if constexpr (B == 5) {      // pair table: 1024 half2 entries indexed by two adjacent 5-bit codes
+        if constexpr (B == 5 && P5) {      // pair table: 1024 half2 entries indexed by two adjacent 5-bit codes
             const char *T2 = reinterpret_cast<const char *>(lut + 512);
 #pragma unroll
             for (int j = 0; j < 16; ++j) h[j] = *reinterpret_cast<const uint32_t *>(T2 + field_off(10 * j, 10, 2));
@@ -207,11 +207,11 @@ __device__ __forceinline__ void decode_unit(const uint32_t (&w)[B], const uint32
 }
 
 constexpr int kLutHalves = 512 + 2048;     // flat fp16 codebooks (C_b at 2^b-1) + the 5-bit pair table
-__device__ __forceinline__ void build_lut(const uint16_t *cb16_global, uint16_t *lut, int tid, int nthreads)
+__device__ __forceinline__ void build_lut(const uint16_t *cb16_global, uint16_t *lut, int tid, int nthreads, bool pair5 = true)
 {
     for (int i = tid; i < 512; i += nthreads) lut[i] = cb16_global[i < 511 ? i : 510];
     uint32_t *pair = reinterpret_cast<uint32_t *>(lut + 512);
-    for (int i = tid; i < 1024; i += nthreads)
+    for (int i = tid; i < (pair5 ? 1024 : 0); i += nthreads)
         pair[i] = (uint32_t)cb16_global[31 + (i & 31)] | ((uint32_t)cb16_global[31 + (i >> 5)] << 16);
 }
 
@@ -372,7 +372,7 @@ __device__ __forceinline__ void load_unit_partial(const uint32_t *unit, int g8, 
 
 // QK^T of one same-width group: all its k16 steps, 8 m-tiles each.  m = coordinates in the
 // group; units of 8 coordinates are contiguous (128*B bytes each), only the last may be partial.
-template <int B>
+template <int B, bool P5>
 __device__ __forceinline__ void qk_group(const uint32_t *gcodes, int m, int lane, const uint2 *__restrict__ qfp,
                                          const uint32_t *pools, const uint16_t *lut, float (&A)[8][4])
 {
@@ -386,8 +386,8 @@ __device__ __forceinline__ void qk_group(const uint32_t *gcodes, int m, int lane
         const uint2 bq = __ldg(qfp);
         load_unit_full<B>(u0, lane, w0);
         load_unit_full<B>(u0 + 32 * B, lane, w1);
-        decode_unit<B>(w0, pools, lut, h0);
-        decode_unit<B>(w1, pools, lut, h1);
+        decode_unit<B, P5>(w0, pools, lut, h0);
+        decode_unit<B, P5>(w1, pools, lut, h1);
         if (first) {
 #pragma unroll
             for (int i = 0; i < 8; ++i) mma16816_z(A[i], h0[2 * i], h0[2 * i + 1], h1[2 * i], h1[2 * i + 1], bq.x, bq.y);
@@ -404,11 +404,11 @@ __device__ __forceinline__ void qk_group(const uint32_t *gcodes, int m, int lane
         const uint2 bq = __ldg(qfp);
         if (n_full & 1) load_unit_full<B>(u0, lane, w0);
         else load_unit_partial<B>(u0, g8, c, rem, w0);
-        decode_unit<B>(w0, pools, lut, h0);
+        decode_unit<B, P5>(w0, pools, lut, h0);
         if ((n_full & 1) && rem) {
             uint32_t w1[B];
             load_unit_partial<B>(u0 + 32 * B, g8, c, rem, w1);
-            decode_unit<B>(w1, pools, lut, h1);
+            decode_unit<B, P5>(w1, pools, lut, h1);
         } else {
 #pragma unroll
             for (int i = 0; i < 16; ++i) h1[i] = 0u;
@@ -424,7 +424,7 @@ __device__ __forceinline__ void qk_group(const uint32_t *gcodes, int m, int lane
 }
 
 // PV of one tile: 16 units of width B -> O[J] += V^T[16 dims x 128 tokens] . P[128 tokens x 8 heads]
-template <int B>
+template <int B, bool P5>
 __device__ __forceinline__ void pv_tile(const uint32_t *vcodes, int lane, const uint32_t (&bP)[8][2],
                                         const uint32_t *pools, const uint16_t *lut, float (&O)[8][4])
 {
@@ -434,8 +434,8 @@ __device__ __forceinline__ void pv_tile(const uint32_t *vcodes, int lane, const 
         const uint32_t *u0 = vcodes + (2 * J) * 32 * B;
         load_unit_full<B>(u0, lane, w0);
         load_unit_full<B>(u0 + 32 * B, lane, w1);
-        decode_unit<B>(w0, pools, lut, h0);
-        decode_unit<B>(w1, pools, lut, h1);
+        decode_unit<B, P5>(w0, pools, lut, h0);
+        decode_unit<B, P5>(w1, pools, lut, h1);
 #pragma unroll
         for (int kp = 0; kp < 8; ++kp)
             mma16816(O[J], h0[2 * kp], h1[2 * kp], h0[2 * kp + 1], h1[2 * kp + 1], bP[kp][0], bP[kp][1]);
@@ -447,14 +447,15 @@ __global__ void __launch_bounds__(W * 32, 1)
 decode_kernel(const DecodeParams P)
 {
     extern __shared__ __align__(128) unsigned char smem[];       // the per-warp tile buffers only
-    __shared__ __align__(16) uint16_t lut[kLutHalves];            // static: constant LDS addresses for the LUTs
+    constexpr bool P5 = W < 16;                                   // the 4 KB 5-bit pair table is dropped where 16 tile buffers need the room
+    __shared__ __align__(16) uint16_t lut[P5 ? kLutHalves : 512]; // static: constant LDS addresses for the LUTs
     __shared__ uint32_t pools[16];
     __shared__ int pre[kMaxBatch + 1];
     __shared__ __align__(8) uint64_t bars[2 * W];
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int g8 = lane >> 2, c = lane & 3;
-    build_lut(P.cb16, lut, tid, W * 32);
+    build_lut(P.cb16, lut, tid, W * 32, P5);
     if (tid == 0) build_prefix(P.seq_len, P.batch, P.n_cap * kTile, pre);
     __syncthreads();
     if (tid == 0) build_pools(lut, pools);
@@ -549,14 +550,14 @@ decode_kernel(const DecodeParams P)
                 const uint2 *qg = qfp + (d >> 28) * 32;
                 float A[8][4];                               // started by the group's first k-step (m >= 2)
                 switch ((d >> 24) & 0xF) {
-                case 1: qk_group<1>(gcodes, m, lane, qg, pools, lut, A); break;
-                case 2: qk_group<2>(gcodes, m, lane, qg, pools, lut, A); break;
-                case 3: qk_group<3>(gcodes, m, lane, qg, pools, lut, A); break;
-                case 4: qk_group<4>(gcodes, m, lane, qg, pools, lut, A); break;
-                case 5: qk_group<5>(gcodes, m, lane, qg, pools, lut, A); break;
-                case 6: qk_group<6>(gcodes, m, lane, qg, pools, lut, A); break;
-                case 7: qk_group<7>(gcodes, m, lane, qg, pools, lut, A); break;
-                default: qk_group<8>(gcodes, m, lane, qg, pools, lut, A); break;
+                case 1: qk_group<1, P5>(gcodes, m, lane, qg, pools, lut, A); break;
+                case 2: qk_group<2, P5>(gcodes, m, lane, qg, pools, lut, A); break;
+                case 3: qk_group<3, P5>(gcodes, m, lane, qg, pools, lut, A); break;
+                case 4: qk_group<4, P5>(gcodes, m, lane, qg, pools, lut, A); break;
+                case 5: qk_group<5, P5>(gcodes, m, lane, qg, pools, lut, A); break;
+                case 6: qk_group<6, P5>(gcodes, m, lane, qg, pools, lut, A); break;
+                case 7: qk_group<7, P5>(gcodes, m, lane, qg, pools, lut, A); break;
+                default: qk_group<8, P5>(gcodes, m, lane, qg, pools, lut, A); break;
                 }
                 // scale by the fp16 group norms (fp32, on the accumulators)
                 const uint4 *np = reinterpret_cast<const uint4 *>(tile + ((knorm_off + 256 * g + g8 * 32) >> 2));
@@ -630,14 +631,14 @@ decode_kernel(const DecodeParams P)
             }
             const uint32_t *vcodes = tile + (vcode_off >> 2);
             switch (b_v) {
-            case 1: pv_tile<1>(vcodes, lane, bP, pools, lut, O); break;
-            case 2: pv_tile<2>(vcodes, lane, bP, pools, lut, O); break;
-            case 3: pv_tile<3>(vcodes, lane, bP, pools, lut, O); break;
-            case 4: pv_tile<4>(vcodes, lane, bP, pools, lut, O); break;
-            case 5: pv_tile<5>(vcodes, lane, bP, pools, lut, O); break;
-            case 6: pv_tile<6>(vcodes, lane, bP, pools, lut, O); break;
-            case 7: pv_tile<7>(vcodes, lane, bP, pools, lut, O); break;
-            default: pv_tile<8>(vcodes, lane, bP, pools, lut, O); break;
+            case 1: pv_tile<1, P5>(vcodes, lane, bP, pools, lut, O); break;
+            case 2: pv_tile<2, P5>(vcodes, lane, bP, pools, lut, O); break;
+            case 3: pv_tile<3, P5>(vcodes, lane, bP, pools, lut, O); break;
+            case 4: pv_tile<4, P5>(vcodes, lane, bP, pools, lut, O); break;
+            case 5: pv_tile<5, P5>(vcodes, lane, bP, pools, lut, O); break;
+            case 6: pv_tile<6, P5>(vcodes, lane, bP, pools, lut, O); break;
+            case 7: pv_tile<7, P5>(vcodes, lane, bP, pools, lut, O); break;
+            default: pv_tile<8, P5>(vcodes, lane, bP, pools, lut, O); break;
             }
             __syncwarp();
             if (x + 1 < seg_end) {
@@ -772,8 +773,9 @@ static int pick_warps(int buf_bytes)
 {
     const int avail = 227 * 1024 - kStaticSmem;
     const int cands[4] = {16, 12, 8, 4};
-    int cap = 16;
+    int cap = 12;   // measured: 16 warps at 128 registers (spills, no pair table) is slower than 12 at 168
     if (const char *e = getenv("BGTQ_DECODE_WARPS")) cap = atoi(e);   // tuning knob (warps per CTA upper bound)
+    if (cap >= 16 && (size_t)16 * buf_bytes <= (size_t)(227 * 1024 - 2560)) return 16;   // W = 16 runs without the pair table
     for (int i = 0; i < 4; ++i)
         if (cands[i] <= cap && (size_t)cands[i] * buf_bytes <= (size_t)avail) return cands[i];
     return 0;
@@ -814,7 +816,7 @@ static int launch_decode_w(const DecodeParams &P, int grid, size_t smem, cudaStr
 {
     static bool attr_set = false;
     if (!attr_set) {   // once per process, outside any stream capture
-        CUDA_TRY(cudaFuncSetAttribute(decode_kernel<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - kStaticSmem));
+        CUDA_TRY(cudaFuncSetAttribute(decode_kernel<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - (W == 16 ? 2560 : kStaticSmem)));
         attr_set = true;
     }
     cudaEvent_t e0 = nullptr, e1 = nullptr;
@@ -830,6 +832,16 @@ static int launch_decode_w(const DecodeParams &P, int grid, size_t smem, cudaStr
         CUDA_TRY(cudaEventRecord(e0, st));
     }
     decode_kernel<W><<<grid, W * 32, smem, st>>>(P);
+    {
+        cudaError_t le = cudaPeekAtLastError();
+        if (le != cudaSuccess) {
+            cudaFuncAttributes fa;
+            cudaFuncGetAttributes(&fa, decode_kernel<W>);
+            set_error(std::string("decode launch: ") + cudaGetErrorString(le) + " regs=" + std::to_string(fa.numRegs) + " maxthr=" + std::to_string(fa.maxThreadsPerBlock) + " static=" + std::to_string(fa.sharedSizeBytes) + " dyn=" + std::to_string(smem) + " maxdyn=" + std::to_string(fa.maxDynamicSharedSizeBytes));
+            cudaGetLastError();
+            return BGTQ_ECUDA;
+        }
+    }
     if (g_prof) CUDA_TRY(cudaEventRecord(e1, st));
     return BGTQ_OK;
 }
