@@ -49,6 +49,10 @@ def parse_args():
     ap.add_argument("--layers", type=int, default=36)
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config supplying the head shape")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--alloc", default="greedy", choices=["greedy", "uniform", "paper_like"],
+                    help="K allocation: greedy = Block-GTQ from the library's energy->allocate path (the metric's workload); "
+                         "uniform = one group at b_k bits (uniform TQ-MSE, PAPER.md:108); paper_like = greedy on scores whose "
+                         "histogram resembles the paper's Qwen2.5-3B row (Table 8, PAPER.md:476)")
     return ap.parse_args()
 
 
@@ -62,6 +66,7 @@ def workload_config(args):
         "rope_base": shp.rope_base, "batch": 1,
         "step": "append 1 token to every layer + decode attention over every layer (one launch each, CUDA graph)",
         "l2": "inputs larger than L2 (per-step footprint ~1 GB >> 126 MB); no flush needed",
+        "alloc": args.alloc,
     }
 
 
@@ -226,6 +231,11 @@ def build_workload(args, P, torch, device, seed_shift: int = 0):
     torch.cuda.synchronize()
     t_alloc = e0.elapsed_time(e1)
     bits = bits_d.cpu().numpy().reshape(Lyr, Hkv, d // 2)
+    if args.alloc == "uniform":                                   # comparison path: uniform TQ-MSE (one group)
+        bits = np.full_like(bits, shp.b_k)
+    elif args.alloc == "paper_like":                              # labelled extra profile, not a BASELINE config
+        sc = torch.from_numpy(W.paper_like_scores(shp.seed0, Lyr * Hkv, d // 2).astype(np.float32)).to(device)
+        bits = P.allocate(sc, shp.b_k * (d // 2), shp.b_min, shp.b_max).cpu().numpy().reshape(Lyr, Hkv, d // 2)
     t0 = time.perf_counter()
     rot = W.rotations(ROT_SEED, d)
     lay = P.Layout(bits, Hq, d, shp.b_v, rot)

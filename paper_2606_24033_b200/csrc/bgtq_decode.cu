@@ -30,6 +30,9 @@ namespace bgtq {
 
 #define CUDA_TRY(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) return cuda_fail(e_, #expr); } while (0)
 
+#ifndef BGTQ_NO_P5
+#define BGTQ_NO_P5 0
+#endif
 constexpr int kMaxWarpsPerSM = 16;
 constexpr int kMaxBatch = 256;
 constexpr int kQfHalves = kMaxKSteps * 8 * 16;      // fp16 q' fragments per (layer, seq, kv head)
@@ -447,7 +450,7 @@ __global__ void __launch_bounds__(W * 32, 1)
 decode_kernel(const DecodeParams P)
 {
     extern __shared__ __align__(128) unsigned char smem[];       // the per-warp tile buffers only
-    constexpr bool P5 = W < 16;                                   // the 4 KB 5-bit pair table is dropped where 16 tile buffers need the room
+    constexpr bool P5 = W < 16 && !BGTQ_NO_P5;                                   // the 4 KB 5-bit pair table is dropped where 16 tile buffers need the room
     __shared__ __align__(16) uint16_t lut[P5 ? kLutHalves : 512]; // static: constant LDS addresses for the LUTs
     __shared__ uint32_t pools[16];
     __shared__ int pre[kMaxBatch + 1];
