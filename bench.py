@@ -49,6 +49,8 @@ def parse_args():
     ap.add_argument("--layers", type=int, default=36)
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config supplying the head shape")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--compare-fp16", action="store_true",
+                    help="also time the fp16-cache comparison kernel (bgtq_fp16_decode_attention) on the same K, V")
     ap.add_argument("--alloc", default="greedy", choices=["greedy", "uniform", "paper_like"],
                     help="K allocation: greedy = Block-GTQ from the library's energy->allocate path (the metric's workload); "
                          "uniform = one group at b_k bits (uniform TQ-MSE, PAPER.md:108); paper_like = greedy on scores whose "
@@ -264,10 +266,18 @@ def build_workload(args, P, torch, device, seed_shift: int = 0):
     v_new = torch.randn_like(k_new)
     tok_bytes = sum(lay.token_bytes(l, h) for l in range(Lyr) for h in range(Hkv))
     ws = lay.new_workspace(1, Lyr, device)
+    fp16 = None
+    if getattr(args, "compare_fp16", False):                     # comparison path: the same K, V as a plain fp16 cache
+        k16 = torch.zeros((Lyr, 1, Hkv, max_tokens, d), dtype=torch.float16, device=device)
+        v16 = torch.zeros_like(k16)
+        for l in range(Lyr):
+            k16[l, 0, :, :T] = kv[l][0].permute(1, 0, 2).to(torch.float16)
+            v16[l, 0, :, :T] = kv[l][1].permute(1, 0, 2).to(torch.float16)
+        fp16 = (k16, v16)
     del kv
     torch.cuda.empty_cache()
     return dict(lay=lay, cache=cache, seq=seq, q=q, k_new=k_new, v_new=v_new, ws=ws, max_tokens=max_tokens,
-                tok_bytes=tok_bytes, bits=bits, scale=1.0 / math.sqrt(d),
+                tok_bytes=tok_bytes, bits=bits, scale=1.0 / math.sqrt(d), fp16=fp16,
                 setup={"block_energy_ms": t_energy, "allocate_ms": t_alloc, "layout_create_ms": t_layout,
                        "cache_fill_ms": t_fill, "cache_fill_tokens_per_s": Lyr * T / (t_fill * 1e-3),
                        "cache_bytes": int(cache.numel()),
@@ -365,6 +375,41 @@ def run_ours(args):
                     "kernel_us": k_ms * 1e3, "algorithmic_bytes_per_launch": alg_bytes,
                     "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS}
 
+        # ---- comparison: own split-KV kernel over an fp16 cache of the same K, V (PAPER.md:308-310 restated on this box)
+        comparison = None
+        if wl["fp16"] is not None:
+            k16, v16 = wl["fp16"]
+            o16 = torch.empty_like(q)
+            for _ in range(3):
+                P.fp16_decode_attention(k16, v16, q, seq, wl["scale"], out=o16)
+            c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            n16 = 10
+            c0.record(stream)
+            for _ in range(n16):
+                P.fp16_decode_attention(k16, v16, q, seq, wl["scale"], out=o16)
+            c1.record(stream)
+            stream.synchronize()
+            us16 = c0.elapsed_time(c1) / n16 * 1e3
+            P.decode_attention(lay, 0, cache, q, seq, wl["max_tokens"], wl["scale"], ws, out=out, n_layers=Lyr)
+            stream.synchronize()
+            rel = float((out.float() - o16.float()).abs().max() / o16.float().abs().max())
+            bytes16 = int(seq.item()) * Lyr * W.CONFIGS[args.config].n_kv_heads * 512
+            comparison = {"fp16_cache_attention_us": us16, "fp16_cache_GBs": bytes16 / (us16 * 1e-6) / 1e9,
+                          "fp16_cache_bytes": bytes16, "packed_attention_us": k_ms * 1e3 + 0.0,
+                          "speedup_packed_vs_fp16_attention_call": None, "compression_vs_fp16": 512.0 * Lyr * W.CONFIGS[args.config].n_kv_heads / wl["tok_bytes"],
+                          "max_rel_diff_packed_vs_fp16_outputs": rel,
+                          "note": "fp16 call = fp16_decode_kernel + combine; packed = decode_kernel alone (q-fold + combine add ~25 us)"}
+            p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            p0.record(stream)
+            for _ in range(n16):
+                P.decode_attention(lay, 0, cache, q, seq, wl["max_tokens"], wl["scale"], ws, out=out, n_layers=Lyr)
+            p1.record(stream)
+            stream.synchronize()
+            usp = p0.elapsed_time(p1) / n16 * 1e3
+            comparison["packed_attention_call_us"] = usp
+            comparison["speedup_packed_vs_fp16_attention_call"] = us16 / usp
+            del k16, v16
+
         # ---- per-layer-launch variant (model-faithful dependency order), device-timed, for the record
         per_layer_us = None
         if world == 1:
@@ -437,6 +482,7 @@ def run_ours(args):
             "e2e": {"value": e2e_val, "unit": "GB/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": e2e_ms},
             "gpu_launches": int(launches_per_step) * args.steps, "gpu_launches_per_step": int(launches_per_step),
+            "comparison": comparison,
         }))
     if world > 1:
         dist.destroy_process_group()

@@ -145,6 +145,17 @@ int bgtq_decode_attention_layers(const bgtq_layout *layout, int layer0, int n_la
                                  int batch, int64_t max_tokens, float softmax_scale, void *out,
                                  void *workspace, size_t workspace_bytes, void *stream);
 
+/* ---- comparison path (NOT part of the method): the same split-KV decode attention over a
+ * plain fp16 cache, so that the paper's "packed cache vs fp16" claims can be restated on
+ * this box without a third-party system.  k_cache, v_cache [device] fp16
+ * [n_layers, batch, n_kv_heads, max_tokens, d_h] (max_tokens a multiple of 128); q, out bf16
+ * [n_layers, batch, n_q_heads, d_h]; out = softmax(scale * q.K^T) V over tokens [0, seq_len[s]). */
+size_t bgtq_fp16_workspace_bytes(int batch, int n_layers, int n_kv_heads);
+int bgtq_fp16_decode_attention(int n_layers, int batch, int n_q_heads, int n_kv_heads, int d_h,
+                               const void *k_cache, const void *v_cache, const void *q,
+                               const int32_t *seq_len, int64_t max_tokens, float softmax_scale,
+                               void *out, void *workspace, size_t workspace_bytes, void *stream);
+
 /* ---- test hooks (used by tests/ only; synchronous) */
 /* decode one unit (b words per lane, 32 lanes, plane-major as in a tile) with the kernel's own
  * unpack routine: words [host] uint32 [b*32] -> values [host] float [32 lanes][32 slots]. */

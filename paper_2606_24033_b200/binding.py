@@ -28,7 +28,7 @@ SYMBOLS = [
     "bgtq_token_bytes", "bgtq_workspace_bytes", "bgtq_region_offset", "bgtq_tile_stride",
     "bgtq_quantize_append", "bgtq_quantize_append_layers", "bgtq_profile_decode",
     "bgtq_profile_decode_read", "bgtq_decode_attention", "bgtq_decode_attention_layers",
-    "bgtq_debug_decode_unit", "bgtq_launch_count",
+    "bgtq_fp16_workspace_bytes", "bgtq_fp16_decode_attention", "bgtq_debug_decode_unit", "bgtq_launch_count",
 ]
 
 
@@ -83,6 +83,10 @@ def _load() -> C.CDLL:
     lib.bgtq_decode_attention.argtypes = [vp, i32, vp, vp, vp, i32, i64, f32, vp, vp, sz, vp]
     lib.bgtq_decode_attention_layers.restype = i32
     lib.bgtq_decode_attention_layers.argtypes = [vp, i32, i32, vp, vp, vp, i32, i64, f32, vp, vp, sz, vp]
+    lib.bgtq_fp16_workspace_bytes.restype = sz
+    lib.bgtq_fp16_workspace_bytes.argtypes = [i32, i32, i32]
+    lib.bgtq_fp16_decode_attention.restype = i32
+    lib.bgtq_fp16_decode_attention.argtypes = [i32, i32, i32, i32, i32, vp, vp, vp, vp, i64, f32, vp, vp, sz, vp]
     lib.bgtq_debug_decode_unit.restype = i32
     lib.bgtq_debug_decode_unit.argtypes = [i32, vp, vp]
     return lib
@@ -263,6 +267,23 @@ def decode_attention(layout: Layout, layer: int, cache: torch.Tensor, q: torch.T
                                              _dev(q, torch.bfloat16), _dev(seq_len, torch.int32), batch,
                                              max_tokens, float(softmax_scale), _dev(out, torch.bfloat16),
                                              _dev(workspace, torch.uint8), workspace.numel(), _stream()))
+    return out
+
+
+def fp16_decode_attention(k_cache: torch.Tensor, v_cache: torch.Tensor, q: torch.Tensor, seq_len: torch.Tensor,
+                          softmax_scale: float, workspace: Optional[torch.Tensor] = None,
+                          out: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """bgtq_fp16_decode_attention (comparison path).  k_cache, v_cache fp16 [n_layers, batch, H_kv, max_tokens, 128];
+    q bf16 [n_layers, batch, H_q, 128]."""
+    n_layers, batch, Hkv, max_tokens, d = k_cache.shape
+    Hq = q.shape[-2]
+    if out is None:
+        out = torch.empty_like(q)
+    if workspace is None:
+        workspace = torch.empty(int(_lib.bgtq_fp16_workspace_bytes(batch, n_layers, Hkv)), dtype=torch.uint8, device=q.device)
+    _check(_lib.bgtq_fp16_decode_attention(n_layers, batch, Hq, Hkv, d, _dev(k_cache, torch.float16), _dev(v_cache, torch.float16),
+                                           _dev(q, torch.bfloat16), _dev(seq_len, torch.int32), max_tokens, float(softmax_scale),
+                                           _dev(out, torch.bfloat16), _dev(workspace, torch.uint8), workspace.numel(), _stream()))
     return out
 
 

@@ -765,10 +765,233 @@ combine_kernel(const float *__restrict__ partials, const int32_t *__restrict__ s
     }
     o[d] = acc / lsum;
     __syncthreads();
+    if (rot128 == nullptr) { dst[d] = __float2bfloat16(o[d]); return; }    // fp16-cache comparison path: no rotation
     float r = 0.f;
 #pragma unroll 32
     for (int j = 0; j < kDh; ++j) r = fmaf(__ldg(rot128 + j * kDh + d), o[j], r);
     dst[d] = __float2bfloat16(r * 0.08838834764831845f);     // 1/sqrt(128)
+}
+
+// ---------------------------------------------------------------- comparison path: fp16 KV cache
+// Not part of the method: an own split-KV decode kernel over a plain fp16 cache
+// k_cache, v_cache [layer][sequence][kv head][token][128], same scheduler, same partial/combine format,
+// so that "packed Block-GTQ cache vs fp16 cache" can be restated on this box without any
+// third-party system.  HBM-bound by construction: 512 bytes per token per KV head.
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void *src)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void ldmatrix_x4(uint32_t (&r)[4], uint32_t addr)
+{
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
+}
+__device__ __forceinline__ void ldmatrix_x4_trans(uint32_t (&r)[4], uint32_t addr)
+{
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
+}
+
+struct Fp16Params {
+    const __half *k_cache, *v_cache;
+    const __nv_bfloat16 *q;     // [n_layers][batch][Hq][128]
+    const int32_t *seq_len;
+    float *partials;
+    int64_t n_cap;
+    int n_layers, batch, Hkv, G;
+    float scale_log2e;
+};
+
+constexpr int kSubTok = 32;                       // tokens per staged sub-tile (4 per 128-token scheduling tile)
+constexpr int kFp16Warps = 12;
+constexpr int kFp16Buf = 2 * kSubTok * kDh * 2;   // K and V sub-tile, 16 KB per warp
+
+__global__ void __launch_bounds__(kFp16Warps * 32, 1)
+fp16_decode_kernel(const Fp16Params P)
+{
+    constexpr int W = kFp16Warps;
+    extern __shared__ __align__(128) unsigned char smem[];
+    __shared__ int pre[kMaxBatch + 1];
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int g8 = lane >> 2, c = lane & 3;
+    if (tid == 0) build_prefix(P.seq_len, P.batch, P.n_cap * kTile, pre);
+    __syncthreads();
+    const Sched S = make_sched(P.n_layers, P.batch, P.Hkv, pre, gridDim.x, W);
+    int x = warp_lo(S, blockIdx.x, warp);
+    const int x_end = warp_lo(S, blockIdx.x, warp + 1);
+    bool merged = false;
+    int merged_pair = 0;
+    {
+        const int c_lo = cta_lo(S, blockIdx.x), c_hi = cta_lo(S, blockIdx.x + 1);
+        if (c_lo < c_hi) {
+            const TilePos tc = locate(c_lo, S, pre);
+            merged = c_hi <= tc.pair_start + tc.tiles_b;
+            merged_pair = tc.pair;
+        }
+    }
+    if (!merged && x >= x_end) return;
+    unsigned char *buf = smem + warp * kFp16Buf;
+    const uint32_t kbuf = smem_u32(buf), vbuf = kbuf + kSubTok * kDh * 2;
+    const int gw = blockIdx.x * W + warp;
+    if (x >= x_end) {
+        float *rec = reinterpret_cast<float *>(buf);
+        for (int i = lane; i < kPartialFloats; i += 32) rec[i] = (i % 130 == 0) ? -INFINITY : 0.f;
+    }
+    // stage 32 tokens x 128 halves with a 16-byte-chunk XOR swizzle (chunk ^= token & 7): conflict-free ldmatrix
+    auto stage = [&](uint32_t dst, const __half *src) {      // src: first token of the sub-tile, row pitch 256 B
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+            const int ch = i * 32 + lane, tok = ch >> 4, cc = ch & 15;
+            cp_async16(dst + tok * 256 + ((cc ^ (tok & 7)) << 4), src + tok * kDh + cc * 8);
+        }
+    };
+    while (x < x_end) {
+        const TilePos tp = locate(x, S, pre);
+        const int seg_end = min(x_end, tp.pair_start + tp.tiles_b);
+        int64_t slen = P.seq_len[tp.b];
+        slen = slen > P.n_cap * kTile ? P.n_cap * kTile : slen;
+        const size_t row0 = ((size_t)tp.pair * P.n_cap * kTile) * kDh;       // pair = (l*batch+b)*Hkv+h
+        const __half *kp = P.k_cache + row0, *vp = P.v_cache + row0;
+        // q fragments: B[k = dim][n = head]; lane (n = g8, c) holds dims 16ks+2c,+1 and 16ks+8+2c,+1
+        uint32_t bq[8][2];
+        {
+            const int l = tp.pair / (P.batch * P.Hkv), b = (tp.pair / P.Hkv) % P.batch, h = tp.pair % P.Hkv;
+            const __nv_bfloat16 *qh = P.q + (((size_t)l * P.batch + b) * P.Hkv * P.G + h * P.G + g8) * kDh;
+#pragma unroll
+            for (int ks = 0; ks < 8; ++ks)
+#pragma unroll
+                for (int hf = 0; hf < 2; ++hf) {
+                    float a = 0.f, bb = 0.f;
+                    if (g8 < P.G) {
+                        a = __bfloat162float(qh[16 * ks + 8 * hf + 2 * c]) * P.scale_log2e;
+                        bb = __bfloat162float(qh[16 * ks + 8 * hf + 2 * c + 1]) * P.scale_log2e;
+                    }
+                    bq[ks][hf] = pack_half2(a, bb);
+                }
+        }
+        float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;
+        float O[8][4];
+#pragma unroll
+        for (int J = 0; J < 8; ++J) O[J][0] = O[J][1] = O[J][2] = O[J][3] = 0.f;
+        const int64_t tok_lo = (int64_t)tp.t * kTile, tok_hi = min(slen, (int64_t)(tp.t + (seg_end - x)) * kTile);
+        const int n_sub = (int)((tok_hi - tok_lo + kSubTok - 1) / kSubTok);
+        stage(kbuf, kp + tok_lo * kDh);
+        asm volatile("cp.async.commit_group;" ::: "memory");
+        stage(vbuf, vp + tok_lo * kDh);
+        asm volatile("cp.async.commit_group;" ::: "memory");
+        for (int s = 0; s < n_sub; ++s) {
+            const int64_t t0 = tok_lo + (int64_t)s * kSubTok;
+            asm volatile("cp.async.wait_group 1;" ::: "memory");
+            __syncwarp();
+            float Sc[2][4];
+#pragma unroll
+            for (int i = 0; i < 2; ++i) {
+                Sc[i][0] = Sc[i][1] = Sc[i][2] = Sc[i][3] = 0.f;
+#pragma unroll
+                for (int ks = 0; ks < 8; ++ks) {
+                    uint32_t a[4];
+                    const int tok = 16 * i + (lane & 7) + 8 * ((lane >> 3) & 1), ch = 2 * ks + (lane >> 4);
+                    ldmatrix_x4(a, kbuf + tok * 256 + ((ch ^ (tok & 7)) << 4));
+                    mma16816(Sc[i], a[0], a[1], a[2], a[3], bq[ks][0], bq[ks][1]);
+                }
+            }
+            __syncwarp();
+            if (s + 1 < n_sub) stage(kbuf, kp + (t0 + kSubTok) * kDh);
+            asm volatile("cp.async.commit_group;" ::: "memory");
+            const int n_valid = (int)min((int64_t)kSubTok, slen - t0);
+            if (n_valid < kSubTok) {
+#pragma unroll
+                for (int i = 0; i < 2; ++i) {
+                    if (16 * i + g8 >= n_valid) Sc[i][0] = Sc[i][1] = -INFINITY;
+                    if (16 * i + 8 + g8 >= n_valid) Sc[i][2] = Sc[i][3] = -INFINITY;
+                }
+            }
+            float mx0 = fmaxf(fmaxf(Sc[0][0], Sc[0][2]), fmaxf(Sc[1][0], Sc[1][2]));
+            float mx1 = fmaxf(fmaxf(Sc[0][1], Sc[0][3]), fmaxf(Sc[1][1], Sc[1][3]));
+#pragma unroll
+            for (int o = 4; o < 32; o <<= 1) {
+                mx0 = fmaxf(mx0, __shfl_xor_sync(0xFFFFFFFFu, mx0, o));
+                mx1 = fmaxf(mx1, __shfl_xor_sync(0xFFFFFFFFu, mx1, o));
+            }
+            const float mn0 = fmaxf(m0, mx0), mn1 = fmaxf(m1, mx1);
+            const float al0 = fast_exp2(m0 - mn0), al1 = fast_exp2(m1 - mn1);
+            m0 = mn0; m1 = mn1;
+            float ls0 = 0.f, ls1 = 0.f;
+            uint32_t bP[2][2];
+#pragma unroll
+            for (int i = 0; i < 2; ++i) {
+                Sc[i][0] = fast_exp2(Sc[i][0] - mn0); Sc[i][2] = fast_exp2(Sc[i][2] - mn0);
+                Sc[i][1] = fast_exp2(Sc[i][1] - mn1); Sc[i][3] = fast_exp2(Sc[i][3] - mn1);
+                ls0 += Sc[i][0] + Sc[i][2];
+                ls1 += Sc[i][1] + Sc[i][3];
+                bP[i][0] = movmatrix_trans(pack_half2(Sc[i][0], Sc[i][1]));
+                bP[i][1] = movmatrix_trans(pack_half2(Sc[i][2], Sc[i][3]));
+            }
+            l0 = fmaf(l0, al0, ls0);
+            l1 = fmaf(l1, al1, ls1);
+#pragma unroll
+            for (int J = 0; J < 8; ++J) { O[J][0] *= al0; O[J][2] *= al0; O[J][1] *= al1; O[J][3] *= al1; }
+            asm volatile("cp.async.wait_group 1;" ::: "memory");
+            __syncwarp();
+#pragma unroll
+            for (int J = 0; J < 8; ++J)
+#pragma unroll
+                for (int kp2 = 0; kp2 < 2; ++kp2) {
+                    uint32_t a[4];
+                    const int blk = lane >> 3, tok = 16 * kp2 + (lane & 7) + 8 * (blk >> 1), ch = 2 * J + (blk & 1);
+                    ldmatrix_x4_trans(a, vbuf + tok * 256 + ((ch ^ (tok & 7)) << 4));
+                    mma16816(O[J], a[0], a[1], a[2], a[3], bP[kp2][0], bP[kp2][1]);
+                }
+            __syncwarp();
+            if (s + 1 < n_sub) stage(vbuf, vp + (t0 + kSubTok) * kDh);
+            asm volatile("cp.async.commit_group;" ::: "memory");
+        }
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        x = seg_end;
+#pragma unroll
+        for (int o = 4; o < 32; o <<= 1) {
+            l0 += __shfl_xor_sync(0xFFFFFFFFu, l0, o);
+            l1 += __shfl_xor_sync(0xFFFFFFFFu, l1, o);
+        }
+        __syncwarp();
+        float *rec = merged ? reinterpret_cast<float *>(buf) : P.partials + (size_t)(gw + tp.pair) * kPartialFloats;
+        const int n0 = 2 * c, n1 = 2 * c + 1;
+        if (n0 < P.G) {
+            float *r0 = rec + n0 * 130;
+            if (g8 == 0) { r0[0] = m0; r0[1] = l0; }
+#pragma unroll
+            for (int J = 0; J < 8; ++J) { r0[2 + 16 * J + g8] = O[J][0]; r0[2 + 16 * J + 8 + g8] = O[J][2]; }
+        }
+        if (n1 < P.G) {
+            float *r1 = rec + n1 * 130;
+            if (g8 == 0) { r1[0] = m1; r1[1] = l1; }
+#pragma unroll
+            for (int J = 0; J < 8; ++J) { r1[2 + 16 * J + g8] = O[J][1]; r1[2 + 16 * J + 8 + g8] = O[J][3]; }
+        }
+    }
+    if (merged) {
+        __syncthreads();
+        const float *all = reinterpret_cast<const float *>(smem);
+        const int fstride = kFp16Buf >> 2;
+        float *dst = P.partials + (size_t)(blockIdx.x * W + merged_pair) * kPartialFloats;
+        for (int e = tid; e < 8 * 128; e += W * 32) {
+            const int n = e >> 7, dd = e & 127;
+            if (n >= P.G) continue;
+            float Mx = -INFINITY;
+#pragma unroll
+            for (int w = 0; w < W; ++w) Mx = fmaxf(Mx, all[w * fstride + n * 130]);
+            float acc = 0.f, ls = 0.f;
+#pragma unroll
+            for (int w = 0; w < W; ++w) {
+                const float *r = all + w * fstride + n * 130;
+                const float f = fast_exp2(r[0] - Mx);
+                acc = fmaf(r[2 + dd], f, acc);
+                ls = fmaf(r[1], f, ls);
+            }
+            dst[n * 130 + 2 + dd] = acc;
+            if (dd == 0) { dst[n * 130] = Mx; dst[n * 130 + 1] = ls; }
+        }
+    }
 }
 
 // ---------------------------------------------------------------- host side
@@ -889,6 +1112,44 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
 
     combine_kernel<<<pairs * G, 128, 0, st>>>(partials, seq_len, lay->d_rot + rot_offset(kDh), n_layers, batch,
                                               Hkv, G, n_cap, grid, W, (__nv_bfloat16 *)out);
+    count_launch();
+    CUDA_TRY(cudaGetLastError());
+    return BGTQ_OK;
+}
+
+// ---------------------------------------------------------------- host side of the fp16 comparison path
+size_t fp16_ws_bytes(int sm_count, int batch, int n_layers, int Hkv)
+{
+    return ((size_t)sm_count * kMaxWarpsPerSM + (size_t)n_layers * batch * Hkv) * kPartialFloats * sizeof(float);
+}
+
+int launch_fp16_decode(int n_layers, int batch, int Hq, int Hkv, const void *k_cache, const void *v_cache,
+                       const void *q, const int32_t *seq_len, int64_t max_tokens, float scale, void *out,
+                       void *ws, size_t ws_bytes, cudaStream_t st)
+{
+    static int sm_count = 0;
+    static bool attr_set = false;
+    if (!sm_count) {
+        int dev = 0;
+        CUDA_TRY(cudaGetDevice(&dev));
+        CUDA_TRY(cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev));
+    }
+    if (batch > kMaxBatch) { set_error("bgtq_fp16_decode_attention: batch > 256"); return BGTQ_EINVAL; }
+    if (ws_bytes < fp16_ws_bytes(sm_count, batch, n_layers, Hkv)) { set_error("bgtq_fp16_decode_attention: workspace too small"); return BGTQ_EWORKSPACE; }
+    const size_t smem = (size_t)kFp16Warps * kFp16Buf;
+    if (!attr_set) {
+        CUDA_TRY(cudaFuncSetAttribute(fp16_decode_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_set = true;
+    }
+    Fp16Params P;
+    P.k_cache = (const __half *)k_cache; P.v_cache = (const __half *)v_cache; P.q = (const __nv_bfloat16 *)q;
+    P.seq_len = seq_len; P.partials = (float *)ws; P.n_cap = (max_tokens + kTile - 1) / kTile;
+    P.n_layers = n_layers; P.batch = batch; P.Hkv = Hkv; P.G = Hq / Hkv; P.scale_log2e = scale * 1.4426950408889634f;
+    fp16_decode_kernel<<<sm_count, kFp16Warps * 32, smem, st>>>(P);
+    count_launch();
+    CUDA_TRY(cudaGetLastError());
+    combine_kernel<<<n_layers * batch * Hkv * P.G, 128, 0, st>>>(P.partials, seq_len, nullptr, n_layers, batch, Hkv, P.G,
+                                                                 P.n_cap, sm_count, kFp16Warps, (__nv_bfloat16 *)out);
     count_launch();
     CUDA_TRY(cudaGetLastError());
     return BGTQ_OK;

@@ -337,6 +337,29 @@ extern "C" int bgtq_decode_attention(const bgtq_layout *lay, int layer, const vo
                                         softmax_scale, out, workspace, workspace_bytes, stream);
 }
 
+extern "C" size_t bgtq_fp16_workspace_bytes(int batch, int n_layers, int n_kv_heads)
+{
+    if (batch <= 0 || n_layers <= 0 || n_kv_heads <= 0) return 0;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) sms = 256;
+    return fp16_ws_bytes(sms, batch, n_layers, n_kv_heads);
+}
+
+extern "C" int bgtq_fp16_decode_attention(int n_layers, int batch, int n_q_heads, int n_kv_heads, int d_h,
+                                          const void *k_cache, const void *v_cache, const void *q,
+                                          const int32_t *seq_len, int64_t max_tokens, float softmax_scale,
+                                          void *out, void *workspace, size_t workspace_bytes, void *stream)
+{
+    if (!k_cache || !v_cache || !q || !seq_len || !out || !workspace) FAIL(BGTQ_EINVAL, "bgtq_fp16_decode_attention: null pointer");
+    if (d_h != kDh) FAIL(BGTQ_EINVAL, "bgtq_fp16_decode_attention: d_h must be 128");
+    if (n_layers <= 0 || batch <= 0 || n_kv_heads <= 0 || n_q_heads % n_kv_heads || n_q_heads / n_kv_heads > 8 || n_q_heads <= 0)
+        FAIL(BGTQ_EINVAL, "bgtq_fp16_decode_attention: bad shape (GQA group <= 8)");
+    if (max_tokens <= 0 || max_tokens % BGTQ_TILE_TOKENS) FAIL(BGTQ_EINVAL, "bgtq_fp16_decode_attention: max_tokens must be a positive multiple of 128");
+    if (!(softmax_scale > 0.0f)) FAIL(BGTQ_EINVAL, "bgtq_fp16_decode_attention: softmax_scale");
+    return launch_fp16_decode(n_layers, batch, n_q_heads, n_kv_heads, k_cache, v_cache, q, seq_len, max_tokens,
+                              softmax_scale, out, workspace, workspace_bytes, (cudaStream_t)stream);
+}
+
 extern "C" int bgtq_debug_decode_unit(int b, const uint32_t *words, float *values)
 {
     if (b < 1 || b > BGTQ_MAX_WIDTH || !words || !values) FAIL(BGTQ_EINVAL, "bgtq_debug_decode_unit: bad argument");

@@ -317,3 +317,29 @@ def test_full_size_128k_sampled_head(P, tab128):
     rv = math.sqrt(np.mean(np.sum(V * V, axis=1)))
     err = np.max(np.abs(out[l, 0, h * G:(h + 1) * G].double().cpu().numpy() - ref)) / rv
     assert err <= 2e-3, err
+
+
+# ----------------------------------------------------------------------------- comparison path (not the method)
+@pytest.mark.parametrize("lens", [[1], [300, 77], [1000, 129, 0]])
+def test_fp16_comparison_kernel_vs_plain_attention(P, lens):
+    """bgtq_fp16_decode_attention against the textbook definition evaluated in fp64 on the same fp16 cache."""
+    torch.manual_seed(3)
+    Lyr, B, Hq, Hkv, d, cap = 2, len(lens), 16, 2, 128, 1024
+    k = torch.randn(Lyr, B, Hkv, cap, d, device="cuda").to(torch.float16)
+    v = torch.randn(Lyr, B, Hkv, cap, d, device="cuda").to(torch.float16)
+    q = torch.randn(Lyr, B, Hq, d, device="cuda").to(torch.bfloat16)
+    seq = torch.tensor(lens, dtype=torch.int32, device="cuda")
+    scale = 1.0 / math.sqrt(d)
+    out = P.fp16_decode_attention(k, v, q, seq, scale).double().cpu().numpy()
+    G = Hq // Hkv
+    for l in range(Lyr):
+        for b in range(B):
+            T = lens[b]
+            for a in range(Hq):
+                if T == 0:
+                    assert np.all(out[l, b, a] == 0)
+                    continue
+                K = k[l, b, a // G, :T].double().cpu().numpy()
+                V = v[l, b, a // G, :T].double().cpu().numpy()
+                ref = O.attention(q[l, b, a].double().cpu().numpy(), K, V, scale)
+                assert np.max(np.abs(out[l, b, a] - ref)) <= 2e-3 * math.sqrt(d), (l, b, a)
