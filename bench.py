@@ -217,12 +217,15 @@ def build_workload(args, P, torch, device, seed_shift: int = 0):
         k = torch.cat(ks) if len(ks) > 1 else ks[0]
         v = torch.cat(vs) if len(vs) > 1 else vs[0]
         qcal = GS.layer_queries(seed, shp.n_cal, Hq, scales, d, shp.rope_base, 0, device, tag=4)
+        P.block_energy(qcal, k)                                   # warm-up (allocator, caches)
         e0, e1 = ev(), ev()
         e0.record()
         scores.append(P.block_energy(qcal, k))
         e1.record()
         torch.cuda.synchronize()
         t_energy += e0.elapsed_time(e1)
+        energy_bytes = energy_bytes + qcal.numel() * qcal.element_size() + k.numel() * k.element_size() if l else \
+            qcal.numel() * qcal.element_size() + k.numel() * k.element_size()
         kv.append((k, v))
         scales_all.append(scales)
     s_all = torch.cat(scores)                                   # [Lyr*Hkv, 64]
@@ -278,7 +281,7 @@ def build_workload(args, P, torch, device, seed_shift: int = 0):
     torch.cuda.empty_cache()
     return dict(lay=lay, cache=cache, seq=seq, q=q, k_new=k_new, v_new=v_new, ws=ws, max_tokens=max_tokens,
                 tok_bytes=tok_bytes, bits=bits, scale=1.0 / math.sqrt(d), fp16=fp16,
-                setup={"block_energy_ms": t_energy, "allocate_ms": t_alloc, "layout_create_ms": t_layout,
+                setup={"block_energy_ms": t_energy, "block_energy_GBs": energy_bytes / (t_energy * 1e-3) / 1e9, "allocate_ms": t_alloc, "layout_create_ms": t_layout,
                        "cache_fill_ms": t_fill, "cache_fill_tokens_per_s": Lyr * T / (t_fill * 1e-3),
                        "cache_bytes": int(cache.numel()),
                        "packed_bytes_per_token_per_kv_head": tok_bytes / (Lyr * Hkv)})

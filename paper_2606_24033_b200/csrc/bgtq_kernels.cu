@@ -38,34 +38,56 @@ __global__ void __launch_bounds__(kEnergyThreads)
 energy_partial_kernel(const T *__restrict__ x, int64_t n, int row_elems, int n_chunks,
                       float *__restrict__ partial)
 {
-    const int col0 = (blockIdx.y * kEnergyThreads + threadIdx.x) * 8;
-    if (col0 >= row_elems) return;
+    // A row (one token, all heads) is row_elems/8 threads wide; when that is narrower than the CTA the spare
+    // threads take other tokens of the chunk (token lanes) and a fixed-order shared-memory reduction joins them.
+    __shared__ float red[kEnergyThreads * 8];
+    const int row_threads = row_elems / 8;
+    const int ct = row_threads < kEnergyThreads ? row_threads : kEnergyThreads;   // column threads in this CTA
+    const int TS = kEnergyThreads / ct;                                            // token lanes
+    const int tsub = threadIdx.x / ct, cidx = threadIdx.x % ct;
+    const int col0 = (blockIdx.y * ct + cidx) * 8;
+    const bool active = tsub < TS && col0 < row_elems;
     const int c = blockIdx.x;
     const int64_t per = (n + n_chunks - 1) / n_chunks;
     const int64_t t_lo = c * per, t_hi = min(n, t_lo + per);
     float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-    const T *p = x + t_lo * row_elems + col0;
-    int64_t t = t_lo;
-    for (; t + 4 <= t_hi; t += 4) {      // four independent 16/32-byte loads in flight per thread
-        float v[4][8];
+    if (active) {
+        const int64_t step = (int64_t)TS * row_elems;
+        const T *p = x + (t_lo + tsub) * row_elems + col0;
+        int64_t t = t_lo + tsub;
+        for (; t + 3 * TS < t_hi; t += 4 * TS) {      // four independent 16/32-byte loads in flight per thread
+            float v[4][8];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) load8(p + (int64_t)u * row_elems, v[u]);
+            for (int u = 0; u < 4; ++u) load8(p + u * step, v[u]);
 #pragma unroll
-        for (int u = 0; u < 4; ++u)
+            for (int u = 0; u < 4; ++u)
 #pragma unroll
-            for (int e = 0; e < 8; ++e) acc[e] = fmaf(v[u][e], v[u][e], acc[e]);
-        p += 4 * (int64_t)row_elems;
+                for (int e = 0; e < 8; ++e) acc[e] = fmaf(v[u][e], v[u][e], acc[e]);
+            p += 4 * step;
+        }
+        for (; t < t_hi; t += TS) {
+            float v[8];
+            load8(p, v);
+#pragma unroll
+            for (int e = 0; e < 8; ++e) acc[e] = fmaf(v[e], v[e], acc[e]);
+            p += step;
+        }
     }
-    for (; t < t_hi; ++t) {
-        float v[8];
-        load8(p, v);
+    if (TS > 1) {
 #pragma unroll
-        for (int e = 0; e < 8; ++e) acc[e] = fmaf(v[e], v[e], acc[e]);
-        p += row_elems;
+        for (int e = 0; e < 8; ++e) red[threadIdx.x * 8 + e] = acc[e];
+        __syncthreads();
+        if (tsub == 0 && active) {
+            for (int s2 = 1; s2 < TS; ++s2)
+#pragma unroll
+                for (int e = 0; e < 8; ++e) acc[e] += red[(s2 * ct + cidx) * 8 + e];
+        }
     }
-    float *o = partial + (int64_t)c * row_elems + col0;
-    reinterpret_cast<float4 *>(o)[0] = make_float4(acc[0], acc[1], acc[2], acc[3]);
-    reinterpret_cast<float4 *>(o)[1] = make_float4(acc[4], acc[5], acc[6], acc[7]);
+    if (tsub == 0 && active) {
+        float *o = partial + (int64_t)c * row_elems + col0;
+        reinterpret_cast<float4 *>(o)[0] = make_float4(acc[0], acc[1], acc[2], acc[3]);
+        reinterpret_cast<float4 *>(o)[1] = make_float4(acc[4], acc[5], acc[6], acc[7]);
+    }
 }
 
 // one CTA of 128 threads per (kv head h, block i): fixed-order fp64 reduction of the partials
@@ -139,7 +161,7 @@ int launch_block_energy(const void *q, int64_t n_q, const void *k, int64_t n_k, 
     const int cq = energy_chunks(n_q), ck = energy_chunks(n_k);
     const int rq = Hq * d_h, rk = Hkv * d_h;
     if (n_q > 0) {
-        dim3 grid(cq, (rq / 8 + kEnergyThreads - 1) / kEnergyThreads);
+        dim3 grid(cq, (rq / 8 + kEnergyThreads - 1) / kEnergyThreads);   // narrow rows: one slab, spare threads take tokens
         if (dt == BGTQ_F32) energy_partial_kernel<float><<<grid, kEnergyThreads, 0, st>>>((const float *)q, n_q, rq, cq, pq);
         else energy_partial_kernel<__nv_bfloat16><<<grid, kEnergyThreads, 0, st>>>((const __nv_bfloat16 *)q, n_q, rq, cq, pq);
         count_launch();
