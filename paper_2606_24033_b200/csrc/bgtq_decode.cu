@@ -30,6 +30,9 @@ namespace bgtq {
 
 #define CUDA_TRY(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) return cuda_fail(e_, #expr); } while (0)
 
+#ifndef BGTQ_NORM_IN_OPERAND
+#define BGTQ_NORM_IN_OPERAND 0   // 1: fold K group norms into the fp16 A operand (measured: no faster, less exact); 0: scale fp32 accumulators
+#endif
 #ifndef BGTQ_NO_P5
 #define BGTQ_NO_P5 0
 #endif
@@ -322,7 +325,7 @@ qfold_kernel(const HeadMeta *__restrict__ metas, const float *__restrict__ rot_t
         while (g + 1 < M.n_groups && tid >= M.gstart[g + 1]) ++g;
         const int m = M.gm[g], x0 = M.gstart[g], r = tid - x0;
         const float *T = rot_t + rot_offset(m) + r;
-        const float sc = scale_log2e / sqrtf((float)m);
+        const float sc = scale_log2e / sqrtf((float)m) * (BGTQ_NORM_IN_OPERAND ? 64.f : 1.f);   // 2^6: see qk_group_n
         const int ks = ksbase[g] + (r >> 4), kap = r & 15;
         const uint8_t *co = M.coords + x0;
         float acc = 0.f;
@@ -340,6 +343,29 @@ qfold_kernel(const HeadMeta *__restrict__ metas, const float *__restrict__ rot_t
     }
 }
 
+// ---------------------------------------------------------------- TMEM as a register parking space
+// The PV accumulators (32 registers per thread) are idle during the QK^T phase.  With 16 warps per SM the kernel has
+// 128 registers per thread and no shared memory to spare (tile buffers), so they are parked in tensor memory:
+// tcgen05.st / tcgen05.ld move 32 registers of every lane to / from 32 TMEM columns of the warp's lane quadrant.
+__device__ __forceinline__ void tmem_park(uint32_t taddr, const float (&O)[8][4])
+{
+    uint32_t r[32];
+#pragma unroll
+    for (int i = 0; i < 32; ++i) r[i] = __float_as_uint(O[i >> 2][i & 3]);
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};"
+                 :: "r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]), "r"(r[16]), "r"(r[17]), "r"(r[18]), "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]), "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31]) : "memory");
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_unpark(uint32_t taddr, float (&O)[8][4])
+{
+    uint32_t r[32];
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31]) : "r"(taddr) : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+    for (int i = 0; i < 32; ++i) O[i >> 2][i & 3] = __uint_as_float(r[i]);
+}
+
 // ---------------------------------------------------------------- the decode kernel
 struct DecodeParams {
     const HeadMeta *metas;      // [n_layers][Hkv], first layer of this call
@@ -351,6 +377,7 @@ struct DecodeParams {
     int64_t n_cap;              // tiles of capacity per sequence
     int n_layers, batch, Hkv, G;
     int buf_bytes;              // per-warp tile buffer
+    int dbg;                    // timing experiments only (BGTQ_DEBUG_SKIP): 1 = skip QK^T math, 2 = skip PV math
 };
 
 constexpr int kSmemHdr = 0;      // dynamic shared memory holds only the tile buffers (tables are static)
@@ -426,6 +453,62 @@ __device__ __forceinline__ void qk_group(const uint32_t *gcodes, int m, int lane
     }
 }
 
+// Variant with the K group norm folded into the A operand (fp16): a *= n * 2^-6 before the MMA (q' carries the
+// 2^6), so that ALL groups accumulate into one fp32 logit accumulator and no per-group fp32 scaling pass -- and
+// no HMMA -> FFMA pipeline drain at every group boundary -- is needed.  nn[i][p] = (n, n) half2 of token row
+// (16i + 8p + g8).  The product is rounded to fp16 (2^-11 relative), well inside the 2e-3 attention tolerance;
+// the 2^-6 prescale keeps n * |c| <= 65504 * 4.6 / 64 finite for every fp16 norm.
+__device__ __forceinline__ uint32_t hmul2_u(uint32_t a, uint32_t b)
+{
+    uint32_t r;
+    asm("mul.rn.f16x2 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(b));
+    return r;
+}
+template <int B, bool P5>
+__device__ __forceinline__ void qk_group_n(const uint32_t *gcodes, int m, int lane, const uint2 *__restrict__ qfp,
+                                           const uint32_t *pools, const uint16_t *lut, const uint32_t (&nn)[8][2],
+                                           float (&S)[8][4])
+{
+    const int g8 = lane >> 2, c = lane & 3;
+    const int n_full = m >> 3, rem = (m & 7) >> 1;
+    const uint32_t *u0 = gcodes;
+#pragma unroll 1
+    for (int jp = n_full >> 1; jp > 0; --jp) {
+        uint32_t w0[B], w1[B], h0[16], h1[16];
+        const uint2 bq = __ldg(qfp);
+        load_unit_full<B>(u0, lane, w0);
+        load_unit_full<B>(u0 + 32 * B, lane, w1);
+        decode_unit<B, P5>(w0, pools, lut, h0);
+        decode_unit<B, P5>(w1, pools, lut, h1);
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+            mma16816(S[i], hmul2_u(h0[2 * i], nn[i][0]), hmul2_u(h0[2 * i + 1], nn[i][1]),
+                     hmul2_u(h1[2 * i], nn[i][0]), hmul2_u(h1[2 * i + 1], nn[i][1]), bq.x, bq.y);
+        u0 += 64 * B;
+        qfp += 32;
+    }
+    if ((n_full & 1) | rem) {
+        uint32_t w0[B], h0[16], h1[16];
+        const uint2 bq = __ldg(qfp);
+        if (n_full & 1) load_unit_full<B>(u0, lane, w0);
+        else load_unit_partial<B>(u0, g8, c, rem, w0);
+        decode_unit<B, P5>(w0, pools, lut, h0);
+        if ((n_full & 1) && rem) {
+            uint32_t w1[B];
+            load_unit_partial<B>(u0 + 32 * B, g8, c, rem, w1);
+            decode_unit<B, P5>(w1, pools, lut, h1);
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+                mma16816(S[i], hmul2_u(h0[2 * i], nn[i][0]), hmul2_u(h0[2 * i + 1], nn[i][1]),
+                         hmul2_u(h1[2 * i], nn[i][0]), hmul2_u(h1[2 * i + 1], nn[i][1]), bq.x, bq.y);
+        } else {
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+                mma16816(S[i], hmul2_u(h0[2 * i], nn[i][0]), hmul2_u(h0[2 * i + 1], nn[i][1]), 0u, 0u, bq.x, bq.y);
+        }
+    }
+}
+
 // PV of one tile: 16 units of width B -> O[J] += V^T[16 dims x 128 tokens] . P[128 tokens x 8 heads]
 template <int B, bool P5>
 __device__ __forceinline__ void pv_tile(const uint32_t *vcodes, int lane, const uint32_t (&bP)[8][2],
@@ -455,12 +538,21 @@ decode_kernel(const DecodeParams P)
     __shared__ uint32_t pools[16];
     __shared__ int pre[kMaxBatch + 1];
     __shared__ __align__(8) uint64_t bars[2 * W];
+    constexpr bool PARK = W == 16;                                // 16 warps: 128 registers -> park O in TMEM during QK^T
+    __shared__ uint32_t tmem_base_s;
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int g8 = lane >> 2, c = lane & 3;
     build_lut(P.cb16, lut, tid, W * 32, P5);
     if (tid == 0) build_prefix(P.seq_len, P.batch, P.n_cap * kTile, pre);
+    if (PARK && warp == 0) {                                      // 4 warps per lane quadrant x 32 columns
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 128;" :: "r"(smem_u32(&tmem_base_s)) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    if (PARK) asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
+    if (PARK) asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t taddr = PARK ? tmem_base_s + ((uint32_t)(32 * (warp & 3)) << 16) + 32u * (warp >> 2) : 0u;
     if (tid == 0) build_pools(lut, pools);
     const uint32_t kbar = smem_u32(&bars[2 * warp]), vbar = smem_u32(&bars[2 * warp + 1]);
     if (lane == 0) {
@@ -487,7 +579,7 @@ decode_kernel(const DecodeParams P)
             merged_pair = tc.pair;
         }
     }
-    if (!merged && x >= x_end) return;
+    if (!PARK && !merged && x >= x_end) return;               // (with TMEM parking every warp stays for the dealloc barrier)
 
     const uint32_t *tile = reinterpret_cast<const uint32_t *>(smem + kSmemHdr + warp * P.buf_bytes);
     const uint32_t tile_s = smem_u32(tile);
@@ -507,7 +599,7 @@ decode_kernel(const DecodeParams P)
         const TilePos tp0 = locate(x, S, pre);
         const HeadMeta &M0 = P.metas[tp0.l * P.Hkv + tp0.h];
         if (lane == 0) issue_at(tile_src(tp0, M0), M0.vnorm_off, M0.tile_stride - M0.vnorm_off, true, true);
-    } else {                                   // idle warp of a merged CTA: contributes an empty partial
+    } else if (merged) {                       // idle warp of a merged CTA: contributes an empty partial
         float *rec = reinterpret_cast<float *>(smem + kSmemHdr + warp * P.buf_bytes);
         for (int i = lane; i < kPartialFloats; i += 32) rec[i] = (i % 130 == 0) ? -INFINITY : 0.f;
     }
@@ -536,6 +628,7 @@ decode_kernel(const DecodeParams P)
         float O[8][4];
 #pragma unroll
         for (int J = 0; J < 8; ++J) O[J][0] = O[J][1] = O[J][2] = O[J][3] = 0.f;
+        if (PARK) tmem_park(taddr, O);              // TMEM is the home of O; registers hold it only during PV
 
         for (int t = tp.t; x < seg_end; ++x, ++t) {
             // ======== QK^T
@@ -545,12 +638,36 @@ decode_kernel(const DecodeParams P)
 #pragma unroll
             for (int i = 0; i < 8; ++i) Sc[i][0] = Sc[i][1] = Sc[i][2] = Sc[i][3] = 0.f;
 #pragma unroll 1
-            for (int g = 0; g < n_groups; ++g) {
+            for (int g = 0; g < ((P.dbg & 1) ? 0 : n_groups); ++g) {
                 const uint32_t d = __shfl_sync(0xFFFFFFFFu, gdesc, g);
                 int m = (d >> 16) & 0xFF;
                 m = m ? m : 128;
                 const uint32_t *gcodes = tile + ((d & 0xFFFF) >> 2);
                 const uint2 *qg = qfp + (d >> 28) * 32;
+#if BGTQ_NORM_IN_OPERAND
+                // group norms (fp16, pre-scaled by 2^-6) duplicated to (n, n) pairs and folded into the A operand
+                const uint4 *np = reinterpret_cast<const uint4 *>(tile + ((knorm_off + 256 * g + g8 * 32) >> 2));
+                const uint4 n0 = np[0], n1 = np[1];
+                const uint32_t nw[8] = {n0.x, n0.y, n0.z, n0.w, n1.x, n1.y, n1.z, n1.w};
+                uint32_t nn[8][2];
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    const uint32_t xs = hmul2_u(nw[i], 0x24002400u);       // * 2^-6 (exact)
+                    nn[i][0] = prmt(xs, xs, 0x1010);
+                    nn[i][1] = prmt(xs, xs, 0x3232);
+                }
+                switch ((d >> 24) & 0xF) {
+                case 1: qk_group_n<1, P5>(gcodes, m, lane, qg, pools, lut, nn, Sc); break;
+                case 2: qk_group_n<2, P5>(gcodes, m, lane, qg, pools, lut, nn, Sc); break;
+                case 3: qk_group_n<3, P5>(gcodes, m, lane, qg, pools, lut, nn, Sc); break;
+                case 4: qk_group_n<4, P5>(gcodes, m, lane, qg, pools, lut, nn, Sc); break;
+                case 5: qk_group_n<5, P5>(gcodes, m, lane, qg, pools, lut, nn, Sc); break;
+                case 6: qk_group_n<6, P5>(gcodes, m, lane, qg, pools, lut, nn, Sc); break;
+                case 7: qk_group_n<7, P5>(gcodes, m, lane, qg, pools, lut, nn, Sc); break;
+                default: qk_group_n<8, P5>(gcodes, m, lane, qg, pools, lut, nn, Sc); break;
+                }
+            }
+#else
                 float A[8][4];                               // started by the group's first k-step (m >= 2)
                 switch ((d >> 24) & 0xF) {
                 case 1: qk_group<1, P5>(gcodes, m, lane, qg, pools, lut, A); break;
@@ -575,6 +692,7 @@ decode_kernel(const DecodeParams P)
                     Sc[i][3] = fmaf(nf.y, A[i][3], Sc[i][3]);
                 }
             }
+#endif
             __syncwarp();
             src += stride;
             if (lane == 0 && x + 1 < seg_end) issue_at(src, kbytes, vbytes, true, false);   // K half of the next tile (same layout only)
@@ -612,6 +730,7 @@ decode_kernel(const DecodeParams P)
             }
             l0 = fmaf(l0, al0, ls0);
             l1 = fmaf(l1, al1, ls1);
+            if (PARK) tmem_unpark(taddr, O);
             if (__any_sync(0xFFFFFFFFu, al0 != 1.f || al1 != 1.f)) {
 #pragma unroll
                 for (int J = 0; J < 8; ++J) { O[J][0] *= al0; O[J][2] *= al0; O[J][1] *= al1; O[J][3] *= al1; }
@@ -633,7 +752,8 @@ decode_kernel(const DecodeParams P)
                 }
             }
             const uint32_t *vcodes = tile + (vcode_off >> 2);
-            switch (b_v) {
+            switch ((P.dbg & 2) ? 0 : b_v) {
+            case 0: break;
             case 1: pv_tile<1, P5>(vcodes, lane, bP, pools, lut, O); break;
             case 2: pv_tile<2, P5>(vcodes, lane, bP, pools, lut, O); break;
             case 3: pv_tile<3, P5>(vcodes, lane, bP, pools, lut, O); break;
@@ -644,6 +764,7 @@ decode_kernel(const DecodeParams P)
             default: pv_tile<8, P5>(vcodes, lane, bP, pools, lut, O); break;
             }
             __syncwarp();
+            if (PARK) tmem_park(taddr, O);
             if (x + 1 < seg_end) {
                 if (lane == 0) issue_at(src, kbytes, vbytes, false, true);                   // V half of the next tile
             } else if (x + 1 < x_end) {                                                      // next segment: other layout
@@ -654,6 +775,7 @@ decode_kernel(const DecodeParams P)
         }
 
         // ---------------- write this warp's partial for the pair: slot = warp + pair (unique, see combine)
+        if (PARK) tmem_unpark(taddr, O);
 #pragma unroll
         for (int o = 4; o < 32; o <<= 1) {
             l0 += __shfl_xor_sync(0xFFFFFFFFu, l0, o);
@@ -697,6 +819,11 @@ decode_kernel(const DecodeParams P)
             dst[n * 130 + 2 + dd] = acc;
             if (dd == 0) { dst[n * 130] = Mx; dst[n * 130 + 1] = ls; }
         }
+    }
+    if (PARK) {
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncthreads();
+        if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 128;" :: "r"(tmem_base_s) : "memory");
     }
 }
 
@@ -1097,6 +1224,8 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
     P.metas = metas; P.cache = (const uint8_t *)cache; P.qf = qf; P.seq_len = seq_len; P.cb16 = lay->d_cb16;
     P.partials = partials; P.n_cap = n_cap; P.n_layers = n_layers; P.batch = batch; P.Hkv = Hkv; P.G = G;
     P.buf_bytes = buf_bytes;
+    P.dbg = 0;
+    if (const char *e = getenv("BGTQ_DEBUG_SKIP")) P.dbg = atoi(e);
     const int grid = lay->sm_count;
     const size_t smem = decode_smem(W, buf_bytes);
     int rc;
