@@ -377,7 +377,6 @@ struct DecodeParams {
     int64_t n_cap;              // tiles of capacity per sequence
     int n_layers, batch, Hkv, G;
     int buf_bytes;              // per-warp tile buffer
-    int dbg;                    // timing experiments only (BGTQ_DEBUG_SKIP): 1 = skip QK^T math, 2 = skip PV math
 };
 
 constexpr int kSmemHdr = 0;      // dynamic shared memory holds only the tile buffers (tables are static)
@@ -638,7 +637,7 @@ decode_kernel(const DecodeParams P)
 #pragma unroll
             for (int i = 0; i < 8; ++i) Sc[i][0] = Sc[i][1] = Sc[i][2] = Sc[i][3] = 0.f;
 #pragma unroll 1
-            for (int g = 0; g < ((P.dbg & 1) ? 0 : n_groups); ++g) {
+            for (int g = 0; g < n_groups; ++g) {
                 const uint32_t d = __shfl_sync(0xFFFFFFFFu, gdesc, g);
                 int m = (d >> 16) & 0xFF;
                 m = m ? m : 128;
@@ -752,8 +751,7 @@ decode_kernel(const DecodeParams P)
                 }
             }
             const uint32_t *vcodes = tile + (vcode_off >> 2);
-            switch ((P.dbg & 2) ? 0 : b_v) {
-            case 0: break;
+            switch (b_v) {
             case 1: pv_tile<1, P5>(vcodes, lane, bP, pools, lut, O); break;
             case 2: pv_tile<2, P5>(vcodes, lane, bP, pools, lut, O); break;
             case 3: pv_tile<3, P5>(vcodes, lane, bP, pools, lut, O); break;
@@ -1224,8 +1222,6 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
     P.metas = metas; P.cache = (const uint8_t *)cache; P.qf = qf; P.seq_len = seq_len; P.cb16 = lay->d_cb16;
     P.partials = partials; P.n_cap = n_cap; P.n_layers = n_layers; P.batch = batch; P.Hkv = Hkv; P.G = G;
     P.buf_bytes = buf_bytes;
-    P.dbg = 0;
-    if (const char *e = getenv("BGTQ_DEBUG_SKIP")) P.dbg = atoi(e);
     const int grid = lay->sm_count;
     const size_t smem = decode_smem(W, buf_bytes);
     int rc;
