@@ -45,8 +45,9 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--ctx", type=int, default=131072)
-    ap.add_argument("--layers", type=int, default=36)
+    ap.add_argument("--ctx", type=int, default=None, help="cached tokens per sequence (default: the config's first context)")
+    ap.add_argument("--layers", type=int, default=None, help="layers (default: the config's)")
+    ap.add_argument("--batch", type=int, default=None, help="sequences (default: the config's)")
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config supplying the head shape")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--compare-fp16", action="store_true",
@@ -55,17 +56,22 @@ def parse_args():
                     help="K allocation: greedy = Block-GTQ from the library's energy->allocate path (the metric's workload); "
                          "uniform = one group at b_k bits (uniform TQ-MSE, PAPER.md:108); paper_like = greedy on scores whose "
                          "histogram resembles the paper's Qwen2.5-3B row (Table 8, PAPER.md:476)")
-    return ap.parse_args()
+    args = ap.parse_args()
+    shp = W.CONFIGS[args.config]
+    args.ctx = args.ctx or shp.contexts[0]
+    args.layers = args.layers or shp.n_layers
+    args.batch = args.batch or shp.batch
+    return args
 
 
 def workload_config(args):
     shp = W.CONFIGS[args.config]
     return {
         "workload": f"BASELINE.json configs[{args.config}] ({shp.name}) at ctx {args.ctx}: {args.layers} independent layers, "
-                    f"{shp.n_q_heads}q/{shp.n_kv_heads}kv heads, d_h {shp.d_h}, K{shp.b_k}V{shp.b_v}, batch 1",
+                    f"{shp.n_q_heads}q/{shp.n_kv_heads}kv heads, d_h {shp.d_h}, K{shp.b_k}V{shp.b_v}, batch {args.batch}",
         "ctx": args.ctx, "layers": args.layers, "n_q_heads": shp.n_q_heads, "n_kv_heads": shp.n_kv_heads,
         "d_h": shp.d_h, "b_k": shp.b_k, "b_v": shp.b_v, "b_min": shp.b_min, "b_max": shp.b_max,
-        "rope_base": shp.rope_base, "batch": 1,
+        "rope_base": shp.rope_base, "batch": args.batch,
         "step": "append 1 token to every layer + decode attention over every layer (one launch each, CUDA graph)",
         "l2": "inputs larger than L2 (per-step footprint ~1 GB >> 126 MB); no flush needed",
         "alloc": args.alloc,
@@ -199,35 +205,41 @@ def run_reference(args):
 # ----------------------------------------------------------------------------- GPU arm
 def build_workload(args, P, torch, device, seed_shift: int = 0):
     """Calibrate (energy -> allocate -> layout) and fill the packed cache through the library.
-    Returns a dict with everything a step needs plus setup timings."""
+    Two passes over seeded generators (pass 1: block energy per layer; pass 2: regenerate and append), so only one
+    layer of fp32 K, V is resident at a time.  Returns everything a step needs plus setup timings."""
     from workloads import gpu_synth as GS
     shp = W.CONFIGS[args.config]
-    Lyr, T, d, Hq, Hkv = args.layers, args.ctx, shp.d_h, shp.n_q_heads, shp.n_kv_heads
+    Lyr, T, d, Hq, Hkv, B = args.layers, args.ctx, shp.d_h, shp.n_q_heads, shp.n_kv_heads, args.batch
     chunk = 32768
     ev = lambda: torch.cuda.Event(enable_timing=True)
-    kv, scales_all, scores = [], [], []
-    t_energy = 0.0
+
+    def seed_of(l, b):
+        return shp.seed0 + l + 1000 * seed_shift + 100000 * b
+
+    def gen_chunk(l, b, c0, n):
+        return GS.layer_kv(seed_of(l, b), n, Hkv, d, shp.rope_base, device, t0=c0, chunk_tag=c0 // chunk)
+
+    # ---- pass 1: block energy from n_cal calibration queries and the T keys of sequence 0 of every layer
+    scales_all, scores = [], []
+    t_energy, energy_bytes = 0.0, 0
     for l in range(Lyr):
-        seed = shp.seed0 + l + 1000 * seed_shift
-        ks, vs = [], []
+        ks = []
         for c0 in range(0, T, chunk):
-            k, v, scales = GS.layer_kv(seed, min(chunk, T - c0), Hkv, d, shp.rope_base, device, t0=c0, chunk_tag=c0 // chunk)
+            k, _, scales = gen_chunk(l, 0, c0, min(chunk, T - c0))
             ks.append(k)
-            vs.append(v)
         k = torch.cat(ks) if len(ks) > 1 else ks[0]
-        v = torch.cat(vs) if len(vs) > 1 else vs[0]
-        qcal = GS.layer_queries(seed, shp.n_cal, Hq, scales, d, shp.rope_base, 0, device, tag=4)
-        P.block_energy(qcal, k)                                   # warm-up (allocator, caches)
+        qcal = GS.layer_queries(seed_of(l, 0), shp.n_cal, Hq, scales, d, shp.rope_base, 0, device, tag=4)
+        if l == 0:
+            P.block_energy(qcal, k)                               # warm-up (allocator, caches)
         e0, e1 = ev(), ev()
         e0.record()
         scores.append(P.block_energy(qcal, k))
         e1.record()
         torch.cuda.synchronize()
         t_energy += e0.elapsed_time(e1)
-        energy_bytes = energy_bytes + qcal.numel() * qcal.element_size() + k.numel() * k.element_size() if l else \
-            qcal.numel() * qcal.element_size() + k.numel() * k.element_size()
-        kv.append((k, v))
+        energy_bytes += qcal.numel() * qcal.element_size() + k.numel() * k.element_size()
         scales_all.append(scales)
+        del k, ks
     s_all = torch.cat(scores)                                   # [Lyr*Hkv, 64]
     e0, e1 = ev(), ev()
     e0.record()
@@ -246,45 +258,53 @@ def build_workload(args, P, torch, device, seed_shift: int = 0):
     lay = P.Layout(bits, Hq, d, shp.b_v, rot)
     t_layout = (time.perf_counter() - t0) * 1e3
     max_tokens = T + 4096
-    cache = lay.new_cache(1, max_tokens, device)
-    seq = torch.zeros(1, dtype=torch.int32, device=device)
-    e0, e1 = ev(), ev()
-    e0.record()
-    for l in range(Lyr):
-        k, v = kv[l]
-        for c0 in range(0, T, chunk):
-            seq.zero_()
-            seq += c0
-            P.quantize_append(lay, l, cache, k[None, c0:c0 + chunk].contiguous(), v[None, c0:c0 + chunk].contiguous(),
-                              seq, max_tokens, advance_seq_len=True)
-    e1.record()
-    torch.cuda.synchronize()
-    t_fill = e0.elapsed_time(e1)
-    assert int(seq.item()) == T
-    # the decode-step inputs: one query and one new token per layer
-    q = torch.stack([GS.layer_queries(shp.seed0 + l + 1000 * seed_shift, 1, Hq, scales_all[l], d, shp.rope_base, T, device,
-                                      tag=3, dtype=torch.bfloat16) for l in range(Lyr)])          # [Lyr,1,Hq,d]
-    k_new = torch.stack([GS.layer_kv(shp.seed0 + l + 1000 * seed_shift, 1, Hkv, d, shp.rope_base, device, t0=T, chunk_tag=99)[0][None]
-                         for l in range(Lyr)]).contiguous()                                         # [Lyr,1,1,Hkv,d]
-    v_new = torch.randn_like(k_new)
-    tok_bytes = sum(lay.token_bytes(l, h) for l in range(Lyr) for h in range(Hkv))
-    ws = lay.new_workspace(1, Lyr, device)
+    cache = lay.new_cache(B, max_tokens, device)
+    seq = torch.zeros(B, dtype=torch.int32, device=device)
     fp16 = None
     if getattr(args, "compare_fp16", False):                     # comparison path: the same K, V as a plain fp16 cache
-        k16 = torch.zeros((Lyr, 1, Hkv, max_tokens, d), dtype=torch.float16, device=device)
-        v16 = torch.zeros_like(k16)
-        for l in range(Lyr):
-            k16[l, 0, :, :T] = kv[l][0].permute(1, 0, 2).to(torch.float16)
-            v16[l, 0, :, :T] = kv[l][1].permute(1, 0, 2).to(torch.float16)
-        fp16 = (k16, v16)
-    del kv
+        fp16 = (torch.zeros((Lyr, B, Hkv, max_tokens, d), dtype=torch.float16, device=device),
+                torch.zeros((Lyr, B, Hkv, max_tokens, d), dtype=torch.float16, device=device))
+    # ---- pass 2: regenerate layer by layer and fill the cache through bgtq_quantize_append (timed without the generation)
+    t_fill = 0.0
+    for l in range(Lyr):
+        for c0 in range(0, T, chunk):
+            n = min(chunk, T - c0)
+            kb, vb = [], []
+            for b in range(B):
+                k, v, _ = gen_chunk(l, b, c0, n)
+                kb.append(k)
+                vb.append(v)
+            k = torch.stack(kb) if B > 1 else kb[0][None]
+            v = torch.stack(vb) if B > 1 else vb[0][None]
+            seq.fill_(c0)
+            e0, e1 = ev(), ev()
+            e0.record()
+            P.quantize_append(lay, l, cache, k, v, seq, max_tokens, advance_seq_len=True)
+            e1.record()
+            torch.cuda.synchronize()
+            t_fill += e0.elapsed_time(e1)
+            if fp16 is not None:
+                fp16[0][l, :, :, c0:c0 + n] = k.permute(0, 2, 1, 3).to(torch.float16)
+                fp16[1][l, :, :, c0:c0 + n] = v.permute(0, 2, 1, 3).to(torch.float16)
+            del k, v, kb, vb
+    assert seq.tolist() == [T] * B
+    # the decode-step inputs: one query and one new token per (layer, sequence)
+    q = torch.stack([torch.cat([GS.layer_queries(seed_of(l, b), 1, Hq, scales_all[l], d, shp.rope_base, T, device, tag=3,
+                                                 dtype=torch.bfloat16) for b in range(B)]) for l in range(Lyr)])   # [Lyr,B,Hq,d]
+    k_new = torch.stack([torch.stack([gen_chunk(l, b, T, 1)[0] for b in range(B)]) for l in range(Lyr)]).contiguous()  # [Lyr,B,1,Hkv,d]
+    v_new = torch.randn_like(k_new)
+    tok_bytes = B * sum(lay.token_bytes(l, h) for l in range(Lyr) for h in range(Hkv))
+    ws = lay.new_workspace(B, Lyr, device)
     torch.cuda.empty_cache()
+    n_th = Lyr * B * T * Hkv
     return dict(lay=lay, cache=cache, seq=seq, q=q, k_new=k_new, v_new=v_new, ws=ws, max_tokens=max_tokens,
                 tok_bytes=tok_bytes, bits=bits, scale=1.0 / math.sqrt(d), fp16=fp16,
-                setup={"block_energy_ms": t_energy, "block_energy_GBs": energy_bytes / (t_energy * 1e-3) / 1e9, "allocate_ms": t_alloc, "layout_create_ms": t_layout,
-                       "cache_fill_ms": t_fill, "cache_fill_tokens_per_s": Lyr * T / (t_fill * 1e-3),
+                setup={"block_energy_ms": t_energy, "block_energy_GBs": energy_bytes / (t_energy * 1e-3) / 1e9,
+                       "allocate_ms": t_alloc, "allocate_heads": Lyr * Hkv, "layout_create_ms": t_layout,
+                       "cache_fill_ms": t_fill, "cache_fill_tokens_per_s": Lyr * B * T / (t_fill * 1e-3),
+                       "append_codes_per_s": n_th * 2 * d / (t_fill * 1e-3),
                        "cache_bytes": int(cache.numel()),
-                       "packed_bytes_per_token_per_kv_head": tok_bytes / (Lyr * Hkv)})
+                       "packed_bytes_per_token_per_kv_head": tok_bytes / (Lyr * Hkv * B)})
 
 
 def run_ours(args):
@@ -324,7 +344,7 @@ def run_ours(args):
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
-        seq_start = int(seq.item())
+        seq_start = int(seq[0].item())
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         with ClockSampler(local) as clk:
             e0.record(stream)
@@ -357,7 +377,7 @@ def run_ours(args):
         k_ms, k_n = P.profile_decode_read()
         P.profile_decode(False)
         k_ms /= max(k_n, 1)
-        seq_now = int(seq.item())
+        seq_now = int(seq[0].item())
         alg_bytes = seq_now * wl["tok_bytes"]
         peak, peak_src = 6650.0, "fallback"
         try:
@@ -396,10 +416,10 @@ def run_ours(args):
             P.decode_attention(lay, 0, cache, q, seq, wl["max_tokens"], wl["scale"], ws, out=out, n_layers=Lyr)
             stream.synchronize()
             rel = float((out.float() - o16.float()).abs().max() / o16.float().abs().max())
-            bytes16 = int(seq.item()) * Lyr * W.CONFIGS[args.config].n_kv_heads * 512
+            bytes16 = int(seq[0].item()) * args.batch * Lyr * W.CONFIGS[args.config].n_kv_heads * 512
             comparison = {"fp16_cache_attention_us": us16, "fp16_cache_GBs": bytes16 / (us16 * 1e-6) / 1e9,
                           "fp16_cache_bytes": bytes16, "packed_attention_us": k_ms * 1e3 + 0.0,
-                          "speedup_packed_vs_fp16_attention_call": None, "compression_vs_fp16": 512.0 * Lyr * W.CONFIGS[args.config].n_kv_heads / wl["tok_bytes"],
+                          "speedup_packed_vs_fp16_attention_call": None, "compression_vs_fp16": 512.0 * args.batch * Lyr * W.CONFIGS[args.config].n_kv_heads / wl["tok_bytes"],
                           "max_rel_diff_packed_vs_fp16_outputs": rel,
                           "note": "fp16 call = fp16_decode_kernel + combine; packed = decode_kernel alone (q-fold + combine add ~25 us)"}
             p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -417,7 +437,7 @@ def run_ours(args):
         per_layer_us = None
         if world == 1:
             g2 = torch.cuda.CUDAGraph()
-            wsl = lay.new_workspace(1, 1, device)
+            wsl = lay.new_workspace(args.batch, 1, device)
             with torch.cuda.graph(g2, stream=stream):
                 for l in range(Lyr):
                     P.decode_attention(lay, l, cache, q[l], seq, wl["max_tokens"], wl["scale"], wsl, out=out[l])
@@ -453,7 +473,7 @@ def run_ours(args):
             t = torch.tensor([e2e_ms], device=device, dtype=torch.float64)
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             e2e_ms = float(t.item())
-        seq_e2e = int(seq.item()) - n_e2e / 2.0
+        seq_e2e = int(seq[0].item()) - n_e2e / 2.0
         e2e_val = world * (seq_e2e * wl["tok_bytes"] + io_bytes) / (e2e_ms * 1e-3) / 1e9
         h2d = (hq.numel() * 2 + hk.numel() * 4 + hv.numel() * 4)
         d2h = hout.numel() * 2
