@@ -347,15 +347,20 @@ def run_ours(args):
         seq_start = int(seq[0].item())
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         with ClockSampler(local) as clk:
+            marks = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
             e0.record(stream)
-            for _ in range(args.steps):
+            for i in range(args.steps):
                 graph.replay()
+                marks[i].record(stream)
             e1.record(stream)
             stream.synchronize()
         torch.cuda.synchronize()
         if world > 1:
             dist.barrier()
         ms = e0.elapsed_time(e1)
+        per = np.array([(e0 if i == 0 else marks[i - 1]).elapsed_time(marks[i]) * 1e3 for i in range(args.steps)])
+        step_stats = {"median": float(np.median(per)), "mean": float(per.mean()), "p5": float(np.percentile(per, 5)),
+                      "p95": float(np.percentile(per, 95))}
         if world > 1:
             t = torch.tensor([ms], device=device, dtype=torch.float64)
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -498,7 +503,7 @@ def run_ours(args):
         cfg["per_layer_launch_us_per_step"] = per_layer_us
         print(json.dumps({
             "metric": METRIC, "value": value, "unit": "GB/s", "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms_step, "us_per_step": ms_step * 1e3,
+            "warmup": args.warmup, "ms_per_step": ms_step, "us_per_step": ms_step * 1e3, "step_us_stats": step_stats,
             "pct_of_8TBs": 100.0 * value / world / NOMINAL_HBM_GBS, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f16 codes x bf16 query, f32 accumulate (append: f64)", "data": "synthetic",
             "config": cfg, "clocks": clk.summary(), "roofline": roofline, "cpu_baseline": cpu_baseline,

@@ -343,3 +343,39 @@ def test_fp16_comparison_kernel_vs_plain_attention(P, lens):
                 V = v[l, b, a // G, :T].double().cpu().numpy()
                 ref = O.attention(q[l, b, a].double().cpu().numpy(), K, V, scale)
                 assert np.max(np.abs(out[l, b, a] - ref)) <= 2e-3 * math.sqrt(d), (l, b, a)
+
+
+@pytest.mark.timeout(600)
+def test_cfg1_append_then_attend(P, tab128):
+    """BASELINE.json configs[1]: Qwen2.5-3B layer, 32,768 cached tokens; per step one token goes through
+    bgtq_quantize_append and the query attends over T+1 tokens (Q13).  One KV head is checked against the oracle."""
+    from workloads import gpu_synth as GS
+    shp = W.CONFIGS[1]
+    T, d, Hq, Hkv = shp.contexts[0], shp.d_h, shp.n_q_heads, shp.n_kv_heads
+    k, v, scales = GS.layer_kv(shp.seed0, T + 1, Hkv, d, shp.rope_base, "cuda")
+    qcal = GS.layer_queries(shp.seed0, shp.n_cal, Hq, scales, d, shp.rope_base, 0, "cuda", tag=4)
+    bits = P.allocate(P.block_energy(qcal, k[:T].contiguous()), shp.b_k * 64, shp.b_min, shp.b_max).cpu().numpy()
+    lay = P.Layout(bits[None], Hq, d, shp.b_v, tab128.rot)
+    max_tokens = T + 128
+    cache = lay.new_cache(1, max_tokens)
+    seq = torch.zeros(1, dtype=torch.int32, device="cuda")
+    P.quantize_append(lay, 0, cache, k[None, :T].contiguous(), v[None, :T].contiguous(), seq, max_tokens)
+    P.quantize_append(lay, 0, cache, k[None, T:].contiguous(), v[None, T:].contiguous(), seq, max_tokens)   # the decode-step append
+    assert int(seq.item()) == T + 1
+    q = GS.layer_queries(shp.seed0, 1, Hq, scales, d, shp.rope_base, T, "cuda", tag=3, dtype=torch.bfloat16)
+    scale = 1.0 / math.sqrt(d)
+    out = P.decode_attention(lay, 0, cache, q, seq, max_tokens, scale, lay.new_workspace(1))
+    torch.cuda.synchronize()
+    h = 1
+    head = O.quantize_head(k[:, h].double().cpu().numpy(), v[:, h].double().cpu().numpy(), bits[h], shp.b_v, tab128)
+    stride = lay.tile_stride(0, h)
+    off = lay.region_offset(0, 0, h, 1, max_tokens)
+    exp = np.zeros(((max_tokens + 127) // 128) * stride, dtype=np.uint8)
+    O.pack_region(head, d, exp)
+    assert np.array_equal(cache[off:off + exp.size].cpu().numpy(), exp)
+    G = Hq // Hkv
+    ref = O.decode_attention_head(q[0, h * G:(h + 1) * G].double().cpu().numpy(), head, tab128, d, scale)
+    _, V = O.dequantize_head(head, tab128, d)
+    rv = math.sqrt(np.mean(np.sum(V * V, axis=1)))
+    err = np.max(np.abs(out[0, h * G:(h + 1) * G].double().cpu().numpy() - ref)) / rv
+    assert err <= 2e-3, err
