@@ -380,3 +380,19 @@ def decode_attention_head(q_post: np.ndarray, qh: QuantizedHead, tab: Tables, d_
     dequantised cache (the slow plain definition: every key is de-rotated)."""
     K, V = dequantize_head(qh, tab, d_h)
     return np.stack([attention(q_post[a], K, V, scale) for a in range(q_post.shape[0])])
+
+
+def prefill_attention_head(q_post: np.ndarray, qh: QuantizedHead, tab: Tables, d_h: int, scale: float,
+                           pos0: int) -> np.ndarray:
+    """Causal prefill attention over the (fully dequantised) packed cache: query token i of the
+    chunk sits at position pos0 + i and attends to cached tokens [0, pos0 + i] (itself included; the chunk's K, V
+    are already in the cache).  q_post[n_q, G, d_h] -> out[n_q, G, d_h].  The plain definition: one exact softmax
+    per (query token, head), nothing shared between rows."""
+    K, V = dequantize_head(qh, tab, d_h)
+    n_q, G, _ = q_post.shape
+    out = np.zeros((n_q, G, d_h))
+    for i in range(n_q):
+        T = pos0 + i + 1
+        for a in range(G):
+            out[i, a] = attention(q_post[i, a], K[:T], V[:T], scale)
+    return out

@@ -205,3 +205,24 @@ def test_decode_attention_head_equals_rotated_domain_form(tab128):
         acc = (p * hv) @ tab128.C(3)[qh.vidx]
         folded = tab128.Pi(d).astype(np.float64).T @ acc / math.sqrt(d)
         assert np.allclose(folded, plain[a], rtol=1e-10, atol=1e-12)
+
+
+def test_prefill_oracle_rows_are_decode_steps(tab128):
+    """causal prefill row i == the decode-step attention over the first pos0+i+1 cached tokens; the
+    first row of a chunk starting at 0 is exactly vhat_0 (softmax over one token)."""
+    import workloads as W
+    from oracle import oracle as O
+    rng = np.random.default_rng(9)
+    T, d = 40, 128
+    k = rng.standard_normal((T, d)); v = rng.standard_normal((T, d))
+    bits = np.array([3] * 64, dtype=np.uint8); bits[:8] = 5; bits[8:16] = 1
+    head = O.quantize_head(k, v, bits, 3, tab128)
+    q = rng.standard_normal((T, 2, d))
+    out = O.prefill_attention_head(q, head, tab128, d, 0.1, 0)
+    K, V = O.dequantize_head(head, tab128, d)
+    assert np.allclose(out[0, 0], V[0], atol=1e-12) and np.allclose(out[0, 1], V[0], atol=1e-12)
+    for i in (5, 39):
+        for a in range(2):
+            assert np.allclose(out[i, a], O.attention(q[i, a], K[:i + 1], V[:i + 1], 0.1), atol=1e-12)
+    out2 = O.prefill_attention_head(q[30:], head, tab128, d, 0.1, 30)        # a later chunk of the same sequence
+    assert np.allclose(out2, out[30:], atol=1e-12)
