@@ -145,6 +145,16 @@ int bgtq_decode_attention_layers(const bgtq_layout *layout, int layer0, int n_la
                                  int batch, int64_t max_tokens, float softmax_scale, void *out,
                                  void *workspace, size_t workspace_bytes, void *stream);
 
+/* ---- NEXT #1: causal prefill attention over the packed cache.  The chunk's K, V are
+ * already in the cache (bgtq_quantize_append first): query token i of sequence s sits at position
+ * seq_len[s] - n_q + i and attends to cached tokens [0, that position] (itself included).
+ * q, out [device] bf16 [batch, n_q, n_q_heads, d_h] (post-RoPE q); seq_len [device] int32 [batch] >= n_q.
+ * GQA group must be 1, 2, 4 or 8.  First cut on the legacy mma.sync tensor path. */
+size_t bgtq_prefill_workspace_bytes(const bgtq_layout *layout, int batch, int n_q);
+int bgtq_prefill_attention(const bgtq_layout *layout, int layer, const void *cache, const void *q,
+                           const int32_t *seq_len, int batch, int n_q, int64_t max_tokens, float softmax_scale,
+                           void *out, void *workspace, size_t workspace_bytes, void *stream);
+
 /* ---- comparison path (NOT part of the method): the same split-KV decode attention over a
  * plain fp16 cache, so that the paper's "packed cache vs fp16" claims can be restated on
  * this box without a third-party system.  k_cache, v_cache [device] fp16

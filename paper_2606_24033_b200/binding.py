@@ -28,7 +28,7 @@ SYMBOLS = [
     "bgtq_token_bytes", "bgtq_workspace_bytes", "bgtq_region_offset", "bgtq_tile_stride",
     "bgtq_quantize_append", "bgtq_quantize_append_layers", "bgtq_profile_decode",
     "bgtq_profile_decode_read", "bgtq_decode_attention", "bgtq_decode_attention_layers",
-    "bgtq_fp16_workspace_bytes", "bgtq_fp16_decode_attention", "bgtq_debug_decode_unit", "bgtq_launch_count",
+    "bgtq_prefill_workspace_bytes", "bgtq_prefill_attention", "bgtq_fp16_workspace_bytes", "bgtq_fp16_decode_attention", "bgtq_debug_decode_unit", "bgtq_launch_count",
 ]
 
 
@@ -83,6 +83,10 @@ def _load() -> C.CDLL:
     lib.bgtq_decode_attention.argtypes = [vp, i32, vp, vp, vp, i32, i64, f32, vp, vp, sz, vp]
     lib.bgtq_decode_attention_layers.restype = i32
     lib.bgtq_decode_attention_layers.argtypes = [vp, i32, i32, vp, vp, vp, i32, i64, f32, vp, vp, sz, vp]
+    lib.bgtq_prefill_workspace_bytes.restype = sz
+    lib.bgtq_prefill_workspace_bytes.argtypes = [vp, i32, i32]
+    lib.bgtq_prefill_attention.restype = i32
+    lib.bgtq_prefill_attention.argtypes = [vp, i32, vp, vp, vp, i32, i32, i64, f32, vp, vp, sz, vp]
     lib.bgtq_fp16_workspace_bytes.restype = sz
     lib.bgtq_fp16_workspace_bytes.argtypes = [i32, i32, i32]
     lib.bgtq_fp16_decode_attention.restype = i32
@@ -267,6 +271,22 @@ def decode_attention(layout: Layout, layer: int, cache: torch.Tensor, q: torch.T
                                              _dev(q, torch.bfloat16), _dev(seq_len, torch.int32), batch,
                                              max_tokens, float(softmax_scale), _dev(out, torch.bfloat16),
                                              _dev(workspace, torch.uint8), workspace.numel(), _stream()))
+    return out
+
+
+def prefill_attention(layout: Layout, layer: int, cache: torch.Tensor, q: torch.Tensor, seq_len: torch.Tensor,
+                      max_tokens: int, softmax_scale: float, workspace: Optional[torch.Tensor] = None,
+                      out: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """bgtq_prefill_attention: causal attention of the last n_q cached tokens' queries.  q bf16 [batch, n_q, H_q, d_h]."""
+    batch, n_q, Hq, d = q.shape
+    assert Hq == layout.n_q_heads and d == layout.d_h
+    if out is None:
+        out = torch.empty_like(q)
+    if workspace is None:
+        workspace = torch.empty(int(_lib.bgtq_prefill_workspace_bytes(layout._h, batch, n_q)), dtype=torch.uint8, device=q.device)
+    _check(_lib.bgtq_prefill_attention(layout._h, layer, _dev(cache, torch.uint8), _dev(q, torch.bfloat16),
+                                       _dev(seq_len, torch.int32), batch, n_q, max_tokens, float(softmax_scale),
+                                       _dev(out, torch.bfloat16), _dev(workspace, torch.uint8), workspace.numel(), _stream()))
     return out
 
 

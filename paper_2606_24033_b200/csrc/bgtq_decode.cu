@@ -300,7 +300,7 @@ __device__ __forceinline__ TilePos locate(int x, const Sched &s, const int *pre)
 __global__ void __launch_bounds__(128)
 qfold_kernel(const HeadMeta *__restrict__ metas, const float *__restrict__ rot_t,
              const __nv_bfloat16 *__restrict__ q, int batch, int Hkv, int Hq, float scale_log2e,
-             __half *__restrict__ qf)
+             __half *__restrict__ qf, int plain)
 {
     const int G = Hq / Hkv;
     const int pair = blockIdx.x / G, n = blockIdx.x % G;   // one block per (pair, query head of the group)
@@ -315,11 +315,14 @@ qfold_kernel(const HeadMeta *__restrict__ metas, const float *__restrict__ rot_t
             if (M.ksteps[ks].flags & 1) ksbase[M.ksteps[ks].flags >> 4] = ks;
     // zero padding: this head's slots (and, from block n = 0, the unused head slots n >= G)
     uint2 *out2 = reinterpret_cast<uint2 *>(qf + (size_t)pair * kQfHalves);     // [kstep][8][4] of 4 halves
-    for (int e = tid; e < kMaxKSteps * 32; e += 128) {
-        const int nn = (e >> 2) & 7;
-        if (nn == n || (n == 0 && nn >= G)) out2[e] = make_uint2(0u, 0u);
-    }
+    if (!plain)
+        for (int e = tid; e < kMaxKSteps * 32; e += 128) {
+            const int nn = (e >> 2) & 7;
+            if (nn == n || (n == 0 && nn >= G)) out2[e] = make_uint2(0u, 0u);
+        }
     __syncthreads();
+    // plain layout (prefill): q'[pair][head slot n][128] in grouped coordinate order, zero beyond kdim
+    if (plain && tid >= M.kdim) qf[((size_t)pair * 8 + n) * kDh + tid] = __float2half(0.f);
     if (tid < M.kdim) {
         int g = 0;
         while (g + 1 < M.n_groups && tid >= M.gstart[g + 1]) ++g;
@@ -339,7 +342,8 @@ qfold_kernel(const HeadMeta *__restrict__ metas, const float *__restrict__ rot_t
         }
         for (; k < m; ++k) acc = fmaf(__ldg(T + (size_t)k * m), qs[co[k]], acc);
         __half *out = qf + (size_t)pair * kQfHalves;
-        out[((ks * 8 + n) * 4 + ((kap & 7) >> 1)) * 4 + (kap >> 3) * 2 + (kap & 1)] = __float2half_rn(acc * sc);
+        if (plain) qf[((size_t)pair * 8 + n) * kDh + tid] = __float2half_rn(acc * sc);
+        else out[((ks * 8 + n) * 4 + ((kap & 7) >> 1)) * 4 + (kap >> 3) * 2 + (kap & 1)] = __float2half_rn(acc * sc);
     }
 }
 
@@ -1211,7 +1215,7 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
     const HeadMeta *metas = lay->d_meta + (size_t)layer0 * Hkv;
 
     qfold_kernel<<<pairs * G, 128, 0, st>>>(metas, lay->d_rot_t, (const __nv_bfloat16 *)q, batch, Hkv, Hq,
-                                        scale * 1.4426950408889634f, qf);
+                                        scale * 1.4426950408889634f, qf, 0);
     count_launch();
     CUDA_TRY(cudaGetLastError());
 
@@ -1275,6 +1279,351 @@ int launch_fp16_decode(int n_layers, int batch, int Hq, int Hkv, const void *k_c
     CUDA_TRY(cudaGetLastError());
     combine_kernel<<<n_layers * batch * Hkv * P.G, 128, 0, st>>>(P.partials, seq_len, nullptr, n_layers, batch, Hkv, P.G,
                                                                  P.n_cap, sm_count, kFp16Warps, (__nv_bfloat16 *)out);
+    count_launch();
+    CUDA_TRY(cudaGetLastError());
+    return BGTQ_OK;
+}
+
+// ---------------------------------------------------------------- NEXT #1: prefill attention over the packed cache
+// "each program owns a tile of queries, streams the compressed K/V tiles, decodes them into
+// kernel-local temporaries ... and accumulates under a causal mask with an online softmax".  First cut: a CTA owns
+// 16*(8/G) query tokens x the G query heads of one KV head; every 128-token packed tile is staged by one TMA bulk
+// copy, unpacked ONCE by all 8 warps into shared memory as fp16 (K^ with its group norms, in grouped coordinate
+// order; V^T with its token norms, both in the rotated domain), and then consumed FlashAttention-2 style with
+// ldmatrix + mma.sync by the 8 warps (16 query rows each).  The rotation stays folded: queries arrive as q'
+// (plain layout of qfold_kernel), the output is de-rotated by derotate_kernel.  The unpack is amortised over 128
+// query rows, so this kernel is bound by the (legacy) tensor path, not by the ALU unpack.
+struct PrefillParams {
+    const HeadMeta *metas;      // [Hkv] of the layer
+    const uint8_t *cache;
+    const __half *qp;           // q' plain: [batch*n_q][Hkv][8][128]
+    const int32_t *seq_len;
+    const uint16_t *cb16;
+    float *opart;               // [batch*n_q][Hq][128] fp32, rotated domain, normalised
+    int64_t n_cap;
+    int batch, n_q, Hkv, G, raw_bytes;
+};
+
+struct PUnit { int off, b, nc, ustart, group; };
+
+template <int B>
+__device__ __forceinline__ void prefill_decode_k(const uint32_t *raw, const PUnit &U, int lane, const uint32_t *pools,
+                                                 const uint16_t *lut, const __half *kn, unsigned char *khat)
+{
+    const int g8 = lane >> 2, c = lane & 3;
+    uint32_t w[B], h[16];
+    if (U.nc == 4) load_unit_full<B>(raw + (U.off >> 2), lane, w);
+    else load_unit_partial<B>(raw + (U.off >> 2), g8, c, U.nc, w);
+    decode_unit<B, true>(w, pools, lut, h);
+    if (c < U.nc) {
+        const int col = U.ustart + 2 * c, chunk = col >> 3;
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+#pragma unroll
+            for (int p = 0; p < 2; ++p) {
+                const int tok = 16 * i + 8 * p + g8;
+                const uint32_t n2 = (uint32_t)__half_as_ushort(kn[U.group * 128 + tok]) * 0x10001u;
+                const uint32_t v = hmul2_u(h[2 * i + p], n2);
+                *reinterpret_cast<uint32_t *>(khat + tok * 256 + ((chunk ^ (tok & 7)) << 4) + (col & 7) * 2) = v;
+            }
+    }
+}
+
+template <int B>
+__device__ __forceinline__ void prefill_decode_v(const uint32_t *vcodes, int J, int lane, const uint32_t *pools,
+                                                 const uint16_t *lut, const __half *vn, unsigned char *vhat_t)
+{
+    const int gq = lane >> 2, c = lane & 3;
+#pragma unroll
+    for (int rho = 0; rho < 2; ++rho) {
+        uint32_t w[B], h[16];
+        load_unit_full<B>(vcodes + (2 * J + rho) * 32 * B, lane, w);
+        decode_unit<B, true>(w, pools, lut, h);
+        const int dim = 16 * J + 8 * rho + gq;
+#pragma unroll
+        for (int kp = 0; kp < 8; ++kp)
+#pragma unroll
+            for (int o = 0; o < 2; ++o) {
+                const int tok = 16 * kp + 8 * o + 2 * c;                       // tokens tok, tok+1
+                const uint32_t n2 = *reinterpret_cast<const uint32_t *>(vn + tok);
+                const uint32_t v = hmul2_u(h[2 * kp + o], n2);
+                const int chunk = tok >> 3;
+                *reinterpret_cast<uint32_t *>(vhat_t + dim * 256 + ((chunk ^ (dim & 7)) << 4) + (tok & 7) * 2) = v;
+            }
+    }
+}
+
+__global__ void __launch_bounds__(256, 1)
+prefill_kernel(const PrefillParams P)
+{
+    extern __shared__ __align__(128) unsigned char smem[];
+    __shared__ __align__(16) uint16_t lut[kLutHalves];
+    __shared__ uint32_t pools[16];
+    __shared__ __align__(8) uint64_t bar;
+    __shared__ PUnit units[2 * kMaxKSteps];
+    __shared__ int n_units_s;
+    __shared__ __align__(16) __half kn[kMaxGroups * 128];
+    __shared__ __align__(16) __half vn[128];
+    unsigned char *khat = smem;                       // [128 tokens][128 coords] fp16, 16-byte chunks XOR-swizzled
+    unsigned char *vhat_t = smem + 32768;             // [128 dims][128 tokens] fp16, swizzled
+    uint32_t *raw = reinterpret_cast<uint32_t *>(smem + 65536);
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g8 = lane >> 2, c = lane & 3;
+    const int h = blockIdx.y, b = blockIdx.z, G = P.G;
+    const HeadMeta &M = P.metas[h];
+    const int TQ = 16 * (8 / G);
+    const int n = warp % G, sb = warp / G;                         // head within the group, 16-token sub-block
+    int64_t slen = P.seq_len[b];
+    slen = slen > P.n_cap * kTile ? P.n_cap * kTile : slen;
+    const int i_first = blockIdx.x * TQ;
+    const int i_last = min(P.n_q, i_first + TQ) - 1;
+    const int64_t pos0 = slen - P.n_q;                              // position of query token 0
+    if (i_first >= P.n_q || pos0 < 0) return;
+    const int n_tiles = (int)((pos0 + i_last) / kTile) + 1;
+
+    build_lut(P.cb16, lut, tid, 256, true);
+    for (int i = tid; i < 65536 / 16; i += 256) reinterpret_cast<uint4 *>(smem)[i] = make_uint4(0, 0, 0, 0);
+    if (tid == 0) {
+        int nu = 0, j = 0;
+        for (int ks = 0; ks < M.n_ksteps; ++ks) {
+            const KStep &K = M.ksteps[ks];
+            const int g = K.flags >> 4;
+            if (K.flags & 1) j = 0;
+            units[nu++] = PUnit{K.off0, K.b, K.nc0, M.gstart[g] + 8 * j, g};
+            ++j;
+            if (K.off1 != 0xFFFF) { units[nu++] = PUnit{K.off1, K.b, K.nc1, M.gstart[g] + 8 * j, g}; ++j; }
+        }
+        n_units_s = nu;
+        mbar_init(smem_u32(&bar), 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        fence_proxy_async();
+    }
+    __syncthreads();
+    if (tid == 0) build_pools(lut, pools);
+    const int n_units = n_units_s, ng = M.n_groups, b_v = M.b_v;
+    const uint8_t *region = P.cache + P.n_cap * ((int64_t)P.batch * M.layer_prefix + (int64_t)b * M.layer_sum + M.head_prefix);
+    const uint32_t bar_s = smem_u32(&bar), raw_s = smem_u32(raw);
+    if (tid == 0) { mbar_expect_tx(bar_s, M.tile_stride); bulk_g2s(raw_s, region, M.tile_stride, bar_s); }
+
+    // this warp's 16 query rows: tokens i_first + sb*16 + {g8, g8+8}, head n; A fragments of q' for 8 k-steps
+    const int ti0 = i_first + sb * 16 + g8, ti1 = ti0 + 8;
+    const int64_t p0 = pos0 + ti0, p1 = pos0 + ti1;
+    uint32_t Qa[8][4];
+    {
+        const bool v0 = warp < 8 / G * G && ti0 < P.n_q, v1 = warp < 8 / G * G && ti1 < P.n_q;
+        const __half *q0 = P.qp + ((((size_t)b * P.n_q + (v0 ? ti0 : 0)) * P.Hkv + h) * 8 + n) * kDh;
+        const __half *q1 = P.qp + ((((size_t)b * P.n_q + (v1 ? ti1 : 0)) * P.Hkv + h) * 8 + n) * kDh;
+#pragma unroll
+        for (int ks = 0; ks < 8; ++ks) {
+            Qa[ks][0] = v0 ? *reinterpret_cast<const uint32_t *>(q0 + 16 * ks + 2 * c) : 0u;
+            Qa[ks][1] = v1 ? *reinterpret_cast<const uint32_t *>(q1 + 16 * ks + 2 * c) : 0u;
+            Qa[ks][2] = v0 ? *reinterpret_cast<const uint32_t *>(q0 + 16 * ks + 8 + 2 * c) : 0u;
+            Qa[ks][3] = v1 ? *reinterpret_cast<const uint32_t *>(q1 + 16 * ks + 8 + 2 * c) : 0u;
+        }
+    }
+    float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;
+    float O[16][4];
+#pragma unroll
+    for (int nd = 0; nd < 16; ++nd) O[nd][0] = O[nd][1] = O[nd][2] = O[nd][3] = 0.f;
+    const uint32_t khat_s = smem_u32(khat), vhat_s = smem_u32(vhat_t);
+    uint32_t phase = 0;
+
+    for (int t = 0; t < n_tiles; ++t) {
+        // ---- stage + unpack tile t (all warps)
+        mbar_wait(bar_s, phase);
+        phase ^= 1;
+        for (int idx = tid; idx < (ng + 1) * 128; idx += 256) {      // linearise the norm rows
+            const int tau = idx & 127, g = idx >> 7;
+            const int slot = (tau & 7) * 16 + (tau >> 4) * 2 + ((tau >> 3) & 1);
+            const int off = g < ng ? M.knorm_off + 256 * g : M.vnorm_off;
+            const __half v = reinterpret_cast<const __half *>(reinterpret_cast<const unsigned char *>(raw) + off)[slot];
+            if (g < ng) kn[g * 128 + tau] = v; else vn[tau] = v;
+        }
+        __syncthreads();
+        for (int u = warp; u < n_units; u += 8) {
+            const PUnit U = units[u];
+            switch (U.b) {
+            case 1: prefill_decode_k<1>(raw, U, lane, pools, lut, kn, khat); break;
+            case 2: prefill_decode_k<2>(raw, U, lane, pools, lut, kn, khat); break;
+            case 3: prefill_decode_k<3>(raw, U, lane, pools, lut, kn, khat); break;
+            case 4: prefill_decode_k<4>(raw, U, lane, pools, lut, kn, khat); break;
+            case 5: prefill_decode_k<5>(raw, U, lane, pools, lut, kn, khat); break;
+            case 6: prefill_decode_k<6>(raw, U, lane, pools, lut, kn, khat); break;
+            case 7: prefill_decode_k<7>(raw, U, lane, pools, lut, kn, khat); break;
+            default: prefill_decode_k<8>(raw, U, lane, pools, lut, kn, khat); break;
+            }
+        }
+        {
+            const uint32_t *vcodes = raw + (M.vcode_off >> 2);
+            switch (b_v) {
+            case 1: prefill_decode_v<1>(vcodes, warp, lane, pools, lut, vn, vhat_t); break;
+            case 2: prefill_decode_v<2>(vcodes, warp, lane, pools, lut, vn, vhat_t); break;
+            case 3: prefill_decode_v<3>(vcodes, warp, lane, pools, lut, vn, vhat_t); break;
+            case 4: prefill_decode_v<4>(vcodes, warp, lane, pools, lut, vn, vhat_t); break;
+            case 5: prefill_decode_v<5>(vcodes, warp, lane, pools, lut, vn, vhat_t); break;
+            case 6: prefill_decode_v<6>(vcodes, warp, lane, pools, lut, vn, vhat_t); break;
+            case 7: prefill_decode_v<7>(vcodes, warp, lane, pools, lut, vn, vhat_t); break;
+            default: prefill_decode_v<8>(vcodes, warp, lane, pools, lut, vn, vhat_t); break;
+            }
+        }
+        __syncthreads();
+        if (tid == 0 && t + 1 < n_tiles) {                          // raw buffer is free: request the next tile
+            fence_proxy_async();
+            mbar_expect_tx(bar_s, M.tile_stride);
+            bulk_g2s(raw_s, region + (int64_t)(t + 1) * M.tile_stride, M.tile_stride, bar_s);
+        }
+        // ---- S = q' . K^T for this warp's 16 rows x 128 tokens of the tile (log2 domain)
+        float S[16][4];
+#pragma unroll
+        for (int nt = 0; nt < 16; ++nt) {
+            S[nt][0] = S[nt][1] = S[nt][2] = S[nt][3] = 0.f;
+#pragma unroll
+            for (int ks = 0; ks < 8; ks += 2) {
+                uint32_t r[4];
+                const int tok = 8 * nt + (lane & 7), ch = 2 * ks + (lane >> 3);
+                ldmatrix_x4(r, khat_s + tok * 256 + ((ch ^ (tok & 7)) << 4));
+                mma16816(S[nt], Qa[ks][0], Qa[ks][1], Qa[ks][2], Qa[ks][3], r[0], r[1]);
+                mma16816(S[nt], Qa[ks + 1][0], Qa[ks + 1][1], Qa[ks + 1][2], Qa[ks + 1][3], r[2], r[3]);
+            }
+        }
+        // ---- causal mask + online softmax per row (rows g8 and g8+8; columns 2c, 2c+1 of every n-tile)
+        const int64_t col0 = (int64_t)t * kTile + 2 * c;
+        if (col0 + 126 > (p0 < p1 ? p0 : p1)) {
+#pragma unroll
+            for (int nt = 0; nt < 16; ++nt) {
+                const int64_t j = col0 + 8 * nt;
+                if (j > p0) S[nt][0] = -INFINITY;
+                if (j + 1 > p0) S[nt][1] = -INFINITY;
+                if (j > p1) S[nt][2] = -INFINITY;
+                if (j + 1 > p1) S[nt][3] = -INFINITY;
+            }
+        }
+        float mx0 = -INFINITY, mx1 = -INFINITY;
+#pragma unroll
+        for (int nt = 0; nt < 16; ++nt) {
+            mx0 = fmaxf(mx0, fmaxf(S[nt][0], S[nt][1]));
+            mx1 = fmaxf(mx1, fmaxf(S[nt][2], S[nt][3]));
+        }
+#pragma unroll
+        for (int o = 1; o < 4; o <<= 1) {
+            mx0 = fmaxf(mx0, __shfl_xor_sync(0xFFFFFFFFu, mx0, o));
+            mx1 = fmaxf(mx1, __shfl_xor_sync(0xFFFFFFFFu, mx1, o));
+        }
+        const float mn0 = fmaxf(m0, mx0), mn1 = fmaxf(m1, mx1);
+        // a row whose causal prefix has not started yet (cannot happen: tile 0 always holds token 0) would give -inf
+        const float al0 = fast_exp2(m0 - mn0), al1 = fast_exp2(m1 - mn1);
+        m0 = mn0; m1 = mn1;
+        float ls0 = 0.f, ls1 = 0.f;
+#pragma unroll
+        for (int nt = 0; nt < 16; ++nt) {
+            S[nt][0] = fast_exp2(S[nt][0] - mn0); S[nt][1] = fast_exp2(S[nt][1] - mn0);
+            S[nt][2] = fast_exp2(S[nt][2] - mn1); S[nt][3] = fast_exp2(S[nt][3] - mn1);
+            ls0 += S[nt][0] + S[nt][1];
+            ls1 += S[nt][2] + S[nt][3];
+        }
+        l0 = fmaf(l0, al0, ls0);
+        l1 = fmaf(l1, al1, ls1);
+#pragma unroll
+        for (int nd = 0; nd < 16; ++nd) { O[nd][0] *= al0; O[nd][1] *= al0; O[nd][2] *= al1; O[nd][3] *= al1; }
+        // ---- O += P . V^   (A = P from the S fragments, B = V^T[dim][token] via ldmatrix)
+#pragma unroll
+        for (int kp = 0; kp < 8; ++kp) {
+            const uint32_t a0 = pack_half2(S[2 * kp][0], S[2 * kp][1]), a1 = pack_half2(S[2 * kp][2], S[2 * kp][3]);
+            const uint32_t a2 = pack_half2(S[2 * kp + 1][0], S[2 * kp + 1][1]), a3 = pack_half2(S[2 * kp + 1][2], S[2 * kp + 1][3]);
+#pragma unroll
+            for (int nd = 0; nd < 16; nd += 2) {
+                uint32_t r[4];
+                const int dim = 8 * (nd + (lane >> 4)) + (lane & 7), ch = 2 * kp + ((lane >> 3) & 1);
+                ldmatrix_x4(r, vhat_s + dim * 256 + ((ch ^ (dim & 7)) << 4));
+                mma16816(O[nd], a0, a1, a2, a3, r[0], r[1]);
+                mma16816(O[nd + 1], a0, a1, a2, a3, r[2], r[3]);
+            }
+        }
+        __syncthreads();                                              // K^/V^ are overwritten by the next tile
+    }
+    // ---- normalise and store the rotated-domain output rows (fp32); derotate_kernel finishes them
+#pragma unroll
+    for (int o = 1; o < 4; o <<= 1) {
+        l0 += __shfl_xor_sync(0xFFFFFFFFu, l0, o);
+        l1 += __shfl_xor_sync(0xFFFFFFFFu, l1, o);
+    }
+    const float i0 = 1.f / l0, i1 = 1.f / l1;
+    if (ti0 < P.n_q) {
+        float *dst = P.opart + (((size_t)b * P.n_q + ti0) * (P.Hkv * G) + h * G + n) * kDh;
+#pragma unroll
+        for (int nd = 0; nd < 16; ++nd) *reinterpret_cast<float2 *>(dst + 8 * nd + 2 * c) = make_float2(O[nd][0] * i0, O[nd][1] * i0);
+    }
+    if (ti1 < P.n_q) {
+        float *dst = P.opart + (((size_t)b * P.n_q + ti1) * (P.Hkv * G) + h * G + n) * kDh;
+#pragma unroll
+        for (int nd = 0; nd < 16; ++nd) *reinterpret_cast<float2 *>(dst + 8 * nd + 2 * c) = make_float2(O[nd][2] * i1, O[nd][3] * i1);
+    }
+}
+
+// out[row][k] = sum_j Pi^(128)[j][k] * o'[row][j] / sqrt(128)  ->  bf16  (the V de-rotation, once per output row)
+__global__ void __launch_bounds__(128)
+derotate_kernel(const float *__restrict__ opart, const float *__restrict__ rot128, int64_t n_rows,
+                __nv_bfloat16 *__restrict__ out)
+{
+    __shared__ float o[4][kDh];
+    const int d = threadIdx.x;
+    const int64_t row0 = (int64_t)blockIdx.x * 4;
+#pragma unroll
+    for (int r = 0; r < 4; ++r) o[r][d] = row0 + r < n_rows ? opart[(row0 + r) * kDh + d] : 0.f;
+    __syncthreads();
+    float acc[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll 16
+    for (int j = 0; j < kDh; ++j) {
+        const float p = __ldg(rot128 + j * kDh + d);
+#pragma unroll
+        for (int r = 0; r < 4; ++r) acc[r] = fmaf(p, o[r][j], acc[r]);
+    }
+#pragma unroll
+    for (int r = 0; r < 4; ++r)
+        if (row0 + r < n_rows) out[(row0 + r) * kDh + d] = __float2bfloat16(acc[r] * 0.08838834764831845f);
+}
+
+size_t prefill_ws_bytes(const bgtq_layout *lay, int batch, int n_q)
+{
+    const size_t rows = (size_t)batch * n_q;
+    return rows * lay->n_kv_heads * 8 * kDh * sizeof(__half) + rows * lay->n_q_heads * kDh * sizeof(float);
+}
+
+int launch_prefill(const bgtq_layout *lay, int layer, const void *cache, const void *q, const int32_t *seq_len,
+                   int batch, int n_q, int64_t max_tokens, float scale, void *out, void *ws, size_t ws_bytes,
+                   cudaStream_t st)
+{
+    static bool attr_set = false;
+    const int Hkv = lay->n_kv_heads, Hq = lay->n_q_heads, G = Hq / Hkv;
+    if (G != 1 && G != 2 && G != 4 && G != 8) { set_error("bgtq_prefill_attention: GQA group must be 1, 2, 4 or 8"); return BGTQ_EINVAL; }
+    if (ws_bytes < prefill_ws_bytes(lay, batch, n_q)) { set_error("bgtq_prefill_attention: workspace too small"); return BGTQ_EWORKSPACE; }
+    if (batch > 65535 || (int64_t)batch * n_q * Hkv > 0x7FFFFFFF / 8) { set_error("bgtq_prefill_attention: too many rows"); return BGTQ_EINVAL; }
+    const size_t rows = (size_t)batch * n_q;
+    __half *qp = reinterpret_cast<__half *>(ws);
+    float *opart = reinterpret_cast<float *>(reinterpret_cast<unsigned char *>(ws) + rows * Hkv * 8 * kDh * sizeof(__half));
+    const HeadMeta *metas = lay->d_meta + (size_t)layer * Hkv;
+    // q' for every query token: the decode q-fold with (batch * n_q) rows, plain layout
+    qfold_kernel<<<(unsigned)(rows * Hkv * G), 128, 0, st>>>(metas, lay->d_rot_t, (const __nv_bfloat16 *)q, (int)rows, Hkv, Hq,
+                                                             scale * 1.4426950408889634f, qp, 1);
+    count_launch();
+    CUDA_TRY(cudaGetLastError());
+    const int raw_bytes = (lay->max_stride + 127) / 128 * 128;
+    const size_t smem = 65536 + (size_t)raw_bytes;
+    if (!attr_set) {
+        CUDA_TRY(cudaFuncSetAttribute(prefill_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 65536 + 40 * 1024));
+        attr_set = true;
+    }
+    PrefillParams P;
+    P.metas = metas; P.cache = (const uint8_t *)cache; P.qp = qp; P.seq_len = seq_len; P.cb16 = lay->d_cb16;
+    P.opart = opart; P.n_cap = (max_tokens + kTile - 1) / kTile; P.batch = batch; P.n_q = n_q; P.Hkv = Hkv; P.G = G;
+    P.raw_bytes = raw_bytes;
+    const int TQ = 16 * (8 / G);
+    dim3 grid((n_q + TQ - 1) / TQ, Hkv, batch);
+    prefill_kernel<<<grid, 256, smem, st>>>(P);
+    count_launch();
+    CUDA_TRY(cudaGetLastError());
+    derotate_kernel<<<(unsigned)((rows * Hq + 3) / 4), 128, 0, st>>>(opart, lay->d_rot + rot_offset(kDh), (int64_t)(rows * Hq),
+                                                                      (__nv_bfloat16 *)out);
     count_launch();
     CUDA_TRY(cudaGetLastError());
     return BGTQ_OK;

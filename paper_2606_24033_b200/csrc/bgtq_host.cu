@@ -337,6 +337,25 @@ extern "C" int bgtq_decode_attention(const bgtq_layout *lay, int layer, const vo
                                         softmax_scale, out, workspace, workspace_bytes, stream);
 }
 
+extern "C" size_t bgtq_prefill_workspace_bytes(const bgtq_layout *lay, int batch, int n_q)
+{
+    if (!lay || batch <= 0 || n_q <= 0) return 0;
+    return prefill_ws_bytes(lay, batch, n_q);
+}
+
+extern "C" int bgtq_prefill_attention(const bgtq_layout *lay, int layer, const void *cache, const void *q,
+                                      const int32_t *seq_len, int batch, int n_q, int64_t max_tokens,
+                                      float softmax_scale, void *out, void *workspace, size_t workspace_bytes,
+                                      void *stream)
+{
+    if (!lay || !cache || !q || !seq_len || !out || !workspace) FAIL(BGTQ_EINVAL, "bgtq_prefill_attention: null pointer");
+    if (layer < 0 || layer >= lay->n_layers) FAIL(BGTQ_EINVAL, "bgtq_prefill_attention: layer out of range");
+    if (batch <= 0 || n_q <= 0 || max_tokens <= 0 || n_q > max_tokens) FAIL(BGTQ_EINVAL, "bgtq_prefill_attention: batch/n_q/max_tokens");
+    if (!(softmax_scale > 0.0f) || std::isinf(softmax_scale)) FAIL(BGTQ_EINVAL, "bgtq_prefill_attention: softmax_scale");
+    return launch_prefill(lay, layer, cache, q, seq_len, batch, n_q, max_tokens, softmax_scale, out, workspace,
+                          workspace_bytes, (cudaStream_t)stream);
+}
+
 extern "C" size_t bgtq_fp16_workspace_bytes(int batch, int n_layers, int n_kv_heads)
 {
     if (batch <= 0 || n_layers <= 0 || n_kv_heads <= 0) return 0;

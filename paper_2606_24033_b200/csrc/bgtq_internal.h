@@ -83,6 +83,10 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
                   float scale, void *out, void *ws, size_t ws_bytes, cudaStream_t st);
 size_t decode_ws_bytes(const bgtq_layout *lay, int batch, int n_layers);
 int debug_decode_unit(int b, const uint32_t *words, float *values);
+size_t prefill_ws_bytes(const bgtq_layout *lay, int batch, int n_q);
+int launch_prefill(const bgtq_layout *lay, int layer, const void *cache, const void *q, const int32_t *seq_len,
+                   int batch, int n_q, int64_t max_tokens, float scale, void *out, void *ws, size_t ws_bytes,
+                   cudaStream_t st);
 size_t fp16_ws_bytes(int sm_count, int batch, int n_layers, int Hkv);
 int launch_fp16_decode(int n_layers, int batch, int Hq, int Hkv, const void *k_cache, const void *v_cache,
                        const void *q, const int32_t *seq_len, int64_t max_tokens, float scale, void *out,

@@ -379,3 +379,29 @@ def test_cfg1_append_then_attend(P, tab128):
     rv = math.sqrt(np.mean(np.sum(V * V, axis=1)))
     err = np.max(np.abs(out[0, h * G:(h + 1) * G].double().cpu().numpy() - ref)) / rv
     assert err <= 2e-3, err
+
+
+# ----------------------------------------------------------------------------- NEXT #1: prefill attention
+@pytest.mark.parametrize("T,n_q,Hq,Hkv,bk,bv", [(40, 40, 8, 1, 3, 3), (300, 77, 16, 2, 3, 3), (333, 333, 8, 2, 2, 2),
+                                              (260, 5, 4, 1, 3, 4)])
+def test_prefill_attention_vs_oracle(P, tab128, T, n_q, Hq, Hkv, bk, bv):
+    """bgtq_prefill_attention: causal attention of the last n_q tokens' queries over the packed cache
+    against the oracle's plain definition, row by row."""
+    p = H.make_problem(70 + T, T, Hq, Hkv, bk, bv, 1, 8, rope_base=1e6)
+    lay, cache, seq, heads = _append_and_compare(P, p, tab128, [T], ((T + 127) // 128) * 128, "f32")
+    max_tokens = ((T + 127) // 128) * 128
+    rng = np.random.default_rng(T)
+    scales = W.block_scales(70 + T, Hkv, 64)
+    q_pre = W.pre_rope_gaussian(70 + T, 9, n_q, Hq, 128, scales)
+    q_post = W.round_to_bf16(O.rope(q_pre, np.arange(T - n_q, T, dtype=np.float64), 1e6)).astype(np.float64)   # [n_q,Hq,d]
+    scale = 1.0 / math.sqrt(128)
+    out = P.prefill_attention(lay, 0, cache, _cuda(q_post[None], torch.bfloat16), seq, max_tokens, scale)
+    torch.cuda.synchronize()
+    got = out[0].double().cpu().numpy()
+    G = Hq // Hkv
+    for h in range(Hkv):
+        ref = O.prefill_attention_head(q_post[:, h * G:(h + 1) * G], heads[h], tab128, 128, scale, T - n_q)
+        _, V = O.dequantize_head(heads[h], tab128, 128)
+        rv = math.sqrt(np.mean(np.sum(V * V, axis=1)))
+        err = np.max(np.abs(got[:, h * G:(h + 1) * G] - ref)) / rv
+        assert err <= 2e-3, (h, err)
