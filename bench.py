@@ -50,6 +50,8 @@ def parse_args():
     ap.add_argument("--batch", type=int, default=None, help="sequences (default: the config's)")
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config supplying the head shape")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--prefill-chunk", type=int, default=0,
+                    help="also time bgtq_prefill_attention for the last N cached tokens of layer 0 (NEXT #1, first cut)")
     ap.add_argument("--compare-fp16", action="store_true",
                     help="also time the fp16-cache comparison kernel (bgtq_fp16_decode_attention) on the same K, V")
     ap.add_argument("--alloc", default="greedy", choices=["greedy", "uniform", "paper_like"],
@@ -438,6 +440,28 @@ def run_ours(args):
             comparison["speedup_packed_vs_fp16_attention_call"] = us16 / usp
             del k16, v16
 
+        # ---- NEXT #1: causal prefill attention of the last N cached tokens (layer 0), device-timed
+        prefill = None
+        if args.prefill_chunk > 0:
+            from workloads import gpu_synth as GS
+            shp_ = W.CONFIGS[args.config]
+            nq = min(args.prefill_chunk, int(seq[0].item()))
+            qpf = torch.randn((args.batch, nq, shp_.n_q_heads, shp_.d_h), device=device, dtype=torch.float32).to(torch.bfloat16)
+            for _ in range(2):
+                opf = P.prefill_attention(lay, 0, cache, qpf, seq, wl["max_tokens"], wl["scale"])
+            f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            f0.record(stream)
+            for _ in range(3):
+                opf = P.prefill_attention(lay, 0, cache, qpf, seq, wl["max_tokens"], wl["scale"])
+            f1.record(stream)
+            stream.synchronize()
+            ms_pf = f0.elapsed_time(f1) / 3
+            T_now = int(seq[0].item())
+            pairs = args.batch * sum(T_now - nq + i + 1 for i in range(nq))          # causal (query, key) pairs per head
+            flops = pairs * shp_.n_q_heads * 4 * shp_.d_h
+            prefill = {"n_q": nq, "ms": ms_pf, "tflops": flops / (ms_pf * 1e-3) / 1e12,
+                       "note": "layer 0, q-fold + prefill_kernel + derotate; 4*d_h flop per (query, key, head) pair"}
+
         # ---- per-layer-launch variant (model-faithful dependency order), device-timed, for the record
         per_layer_us = None
         if world == 1:
@@ -510,7 +534,7 @@ def run_ours(args):
             "e2e": {"value": e2e_val, "unit": "GB/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": e2e_ms},
             "gpu_launches": int(launches_per_step) * args.steps, "gpu_launches_per_step": int(launches_per_step),
-            "comparison": comparison,
+            "comparison": comparison, "prefill": prefill,
         }))
     if world > 1:
         dist.destroy_process_group()
