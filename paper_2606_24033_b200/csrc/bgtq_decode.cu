@@ -409,18 +409,30 @@ template <int B, bool P5>
 __device__ __forceinline__ void qk_group(const uint32_t *gcodes, int m, int lane, const uint2 *__restrict__ qfp,
                                          const uint32_t *pools, const uint16_t *lut, float (&A)[8][4])
 {
+    // One loop over the group's k16 steps.  A unit holds 8 coordinates; only the group's last unit may be partial
+    // (nc = lanes per token row that hold data: 4 = full) and the last k-step may lack its second unit (nc1 = 0).
+    // A single loader covers full and partial units (word w of lane g8*nc+c at w*8*nc), so every width
+    // instantiates the unpack twice instead of five times (smaller code, one path).
     const int g8 = lane >> 2, c = lane & 3;
-    const int n_full = m >> 3, rem = (m & 7) >> 1;         // full units; lanes per row in the partial one
+    const int n_full = m >> 3, rem = (m & 7) >> 1, n_half = n_full + (rem ? 1 : 0);
     const uint32_t *u0 = gcodes;
     bool first = true;                                      // the group's first k-step starts the accumulators (C = 0)
 #pragma unroll 1
-    for (int jp = n_full >> 1; jp > 0; --jp) {              // pairs of full units: the tight loop
-        uint32_t w0[B], w1[B], h0[16], h1[16];
+    for (int j = 0; j < n_half; j += 2) {
+        const int nc0 = j < n_full ? 4 : rem;
+        const int nc1 = j + 1 < n_half ? (j + 1 < n_full ? 4 : rem) : 0;
+        uint32_t w0[B], h0[16], h1[16];
         const uint2 bq = __ldg(qfp);
-        load_unit_full<B>(u0, lane, w0);
-        load_unit_full<B>(u0 + 32 * B, lane, w1);
+        load_unit_partial<B>(u0, g8, c, nc0, w0);
         decode_unit<B, P5>(w0, pools, lut, h0);
-        decode_unit<B, P5>(w1, pools, lut, h1);
+        if (nc1) {
+            uint32_t w1[B];
+            load_unit_partial<B>(u0 + 32 * B, g8, c, nc1, w1);
+            decode_unit<B, P5>(w1, pools, lut, h1);
+        } else {
+#pragma unroll
+            for (int i = 0; i < 16; ++i) h1[i] = 0u;
+        }
         if (first) {
 #pragma unroll
             for (int i = 0; i < 8; ++i) mma16816_z(A[i], h0[2 * i], h0[2 * i + 1], h1[2 * i], h1[2 * i + 1], bq.x, bq.y);
@@ -431,28 +443,6 @@ __device__ __forceinline__ void qk_group(const uint32_t *gcodes, int m, int lane
         }
         u0 += 64 * B;
         qfp += 32;
-    }
-    if ((n_full & 1) | rem) {                               // tail k-step: full+partial, full+none or partial+none
-        uint32_t w0[B], h0[16], h1[16];
-        const uint2 bq = __ldg(qfp);
-        if (n_full & 1) load_unit_full<B>(u0, lane, w0);
-        else load_unit_partial<B>(u0, g8, c, rem, w0);
-        decode_unit<B, P5>(w0, pools, lut, h0);
-        if ((n_full & 1) && rem) {
-            uint32_t w1[B];
-            load_unit_partial<B>(u0 + 32 * B, g8, c, rem, w1);
-            decode_unit<B, P5>(w1, pools, lut, h1);
-        } else {
-#pragma unroll
-            for (int i = 0; i < 16; ++i) h1[i] = 0u;
-        }
-        if (first) {
-#pragma unroll
-            for (int i = 0; i < 8; ++i) mma16816_z(A[i], h0[2 * i], h0[2 * i + 1], h1[2 * i], h1[2 * i + 1], bq.x, bq.y);
-        } else {
-#pragma unroll
-            for (int i = 0; i < 8; ++i) mma16816(A[i], h0[2 * i], h0[2 * i + 1], h1[2 * i], h1[2 * i + 1], bq.x, bq.y);
-        }
     }
 }
 
