@@ -405,3 +405,33 @@ def test_prefill_attention_vs_oracle(P, tab128, T, n_q, Hq, Hkv, bk, bv):
         rv = math.sqrt(np.mean(np.sum(V * V, axis=1)))
         err = np.max(np.abs(got[:, h * G:(h + 1) * G] - ref)) / rv
         assert err <= 2e-3, (h, err)
+
+
+# ----------------------------------------------------------------------------- randomised allocations
+@pytest.mark.parametrize("seed", [0, 1, 2, 3, 4, 5])
+def test_random_allocations_append_and_attention(P, tab128, seed):
+    """Arbitrary width patterns (not only greedy outputs): every width 0..8 present, tiny groups of one block,
+    a single 8-bit group, many zero-width blocks ... packed bytes bit-exact and attention within tolerance."""
+    rng = np.random.default_rng(1000 + seed)
+    Hq, Hkv, T = 8, 2, 200 + 37 * seed
+    p = H.make_problem(80 + seed, T, Hq, Hkv, 3, 1 + (seed % 8), 1, 8, rope_base=1e4)
+    pats = [rng.integers(0, 9, size=64), rng.integers(1, 9, size=64)]
+    if seed == 1:
+        pats[0] = np.array([0] * 60 + [8, 7, 6, 5])               # almost everything dropped, tiny wide groups
+    if seed == 2:
+        pats[1] = np.full(64, 8)
+    if seed == 3:
+        pats[0] = np.array(list(range(1, 9)) * 8)                  # 8 groups of 16 coordinates
+    if seed == 4:
+        pats[1] = np.array([1] * 63 + [4])                         # a one-block group
+    p.bits = np.stack(pats).astype(np.uint8)
+    max_tokens = ((T + 127) // 128) * 128
+    lay, cache, seq, heads = _append_and_compare(P, p, tab128, [T - 3, 3], max_tokens, "f32")
+    scale = 1.0 / math.sqrt(p.d_h)
+    out = P.decode_attention(lay, 0, cache, _cuda(p.q_post[None], torch.bfloat16), seq, max_tokens, scale, lay.new_workspace(1))
+    torch.cuda.synchronize()
+    exp, rv = H.oracle_attention(p, heads, tab128, scale)
+    got = out[0].double().cpu().numpy()
+    G = Hq // Hkv
+    err = max(np.max(np.abs(got[a] - exp[a])) / max(rv[a // G], 1e-30) for a in range(Hq))
+    assert err <= 2e-3, err
