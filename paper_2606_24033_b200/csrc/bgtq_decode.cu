@@ -579,8 +579,9 @@ decode_kernel(const DecodeParams P)
     uint32_t kphase = 0, vphase = 0;
 
     // lane 0 requests (a half of) a tile: K half = [K codes | K norms], V half = [V norms | V codes]
+    // (the buffer was only READ through the generic proxy since its last fill, and __syncwarp orders those reads
+    // before the copy is issued, so no cross-proxy fence is needed -- the usual consumer-release -> TMA pattern)
     auto issue_at = [&](const uint8_t *src, uint32_t kbytes, uint32_t vbytes, bool want_k, bool want_v) {
-        fence_proxy_async();
         if (want_k) { mbar_expect_tx(kbar, kbytes); bulk_g2s(tile_s, src, kbytes, kbar); }
         if (want_v) { mbar_expect_tx(vbar, vbytes); bulk_g2s(tile_s + kbytes, src + kbytes, vbytes, vbar); }
     };
