@@ -1344,7 +1344,7 @@ __device__ __forceinline__ void prefill_decode_v(const uint32_t *vcodes, int J, 
     }
 }
 
-__global__ void __launch_bounds__(256, 1)
+__global__ void __launch_bounds__(256, 2)
 prefill_kernel(const PrefillParams P)
 {
     extern __shared__ __align__(128) unsigned char smem[];
@@ -1353,6 +1353,8 @@ prefill_kernel(const PrefillParams P)
     __shared__ __align__(8) uint64_t bar;
     __shared__ PUnit units[2 * kMaxKSteps];
     __shared__ int n_units_s;
+    __shared__ uint32_t tmem_base_s;                  // O (64 registers per thread) lives in tensor memory outside the PV phase,
+                                                      // which brings the kernel under 128 registers -> two CTAs per SM
     __shared__ __align__(16) __half kn[kMaxGroups * 128];
     __shared__ __align__(16) __half vn[128];
     unsigned char *khat = smem;                       // [128 tokens][128 coords] fp16, 16-byte chunks XOR-swizzled
@@ -1373,6 +1375,11 @@ prefill_kernel(const PrefillParams P)
     const int n_tiles = (int)((pos0 + i_last) / kTile) + 1;
 
     build_lut(P.cb16, lut, tid, 256, true);
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 128;" :: "r"(smem_u32(&tmem_base_s)) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     for (int i = tid; i < 65536 / 16; i += 256) reinterpret_cast<uint4 *>(smem)[i] = make_uint4(0, 0, 0, 0);
     if (tid == 0) {
         int nu = 0, j = 0;
@@ -1390,6 +1397,8 @@ prefill_kernel(const PrefillParams P)
         fence_proxy_async();
     }
     __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t taddr = tmem_base_s + ((uint32_t)(32 * (warp & 3)) << 16) + 64u * (warp >> 2);
     if (tid == 0) build_pools(lut, pools);
     const int n_units = n_units_s, ng = M.n_groups, b_v = M.b_v;
     const uint8_t *region = P.cache + P.n_cap * ((int64_t)P.batch * M.layer_prefix + (int64_t)b * M.layer_sum + M.head_prefix);
@@ -1416,6 +1425,8 @@ prefill_kernel(const PrefillParams P)
     float O[16][4];
 #pragma unroll
     for (int nd = 0; nd < 16; ++nd) O[nd][0] = O[nd][1] = O[nd][2] = O[nd][3] = 0.f;
+    tmem_park(taddr, reinterpret_cast<float (&)[8][4]>(O[0]));
+    tmem_park(taddr + 32, reinterpret_cast<float (&)[8][4]>(O[8]));
     const uint32_t khat_s = smem_u32(khat), vhat_s = smem_u32(vhat_t);
     uint32_t phase = 0;
 
@@ -1514,13 +1525,17 @@ prefill_kernel(const PrefillParams P)
         }
         l0 = fmaf(l0, al0, ls0);
         l1 = fmaf(l1, al1, ls1);
+        uint32_t Pp[16][2];                                           // P as fp16 A fragments; S is dead from here
+#pragma unroll
+        for (int nt = 0; nt < 16; ++nt) { Pp[nt][0] = pack_half2(S[nt][0], S[nt][1]); Pp[nt][1] = pack_half2(S[nt][2], S[nt][3]); }
+        tmem_unpark(taddr, reinterpret_cast<float (&)[8][4]>(O[0]));
+        tmem_unpark(taddr + 32, reinterpret_cast<float (&)[8][4]>(O[8]));
 #pragma unroll
         for (int nd = 0; nd < 16; ++nd) { O[nd][0] *= al0; O[nd][1] *= al0; O[nd][2] *= al1; O[nd][3] *= al1; }
         // ---- O += P . V^   (A = P from the S fragments, B = V^T[dim][token] via ldmatrix)
 #pragma unroll
         for (int kp = 0; kp < 8; ++kp) {
-            const uint32_t a0 = pack_half2(S[2 * kp][0], S[2 * kp][1]), a1 = pack_half2(S[2 * kp][2], S[2 * kp][3]);
-            const uint32_t a2 = pack_half2(S[2 * kp + 1][0], S[2 * kp + 1][1]), a3 = pack_half2(S[2 * kp + 1][2], S[2 * kp + 1][3]);
+            const uint32_t a0 = Pp[2 * kp][0], a1 = Pp[2 * kp][1], a2 = Pp[2 * kp + 1][0], a3 = Pp[2 * kp + 1][1];
 #pragma unroll
             for (int nd = 0; nd < 16; nd += 2) {
                 uint32_t r[4];
@@ -1530,8 +1545,12 @@ prefill_kernel(const PrefillParams P)
                 mma16816(O[nd + 1], a0, a1, a2, a3, r[2], r[3]);
             }
         }
+        tmem_park(taddr, reinterpret_cast<float (&)[8][4]>(O[0]));
+        tmem_park(taddr + 32, reinterpret_cast<float (&)[8][4]>(O[8]));
         __syncthreads();                                              // K^/V^ are overwritten by the next tile
     }
+    tmem_unpark(taddr, reinterpret_cast<float (&)[8][4]>(O[0]));
+    tmem_unpark(taddr + 32, reinterpret_cast<float (&)[8][4]>(O[8]));
     // ---- normalise and store the rotated-domain output rows (fp32); derotate_kernel finishes them
 #pragma unroll
     for (int o = 1; o < 4; o <<= 1) {
@@ -1549,6 +1568,9 @@ prefill_kernel(const PrefillParams P)
 #pragma unroll
         for (int nd = 0; nd < 16; ++nd) *reinterpret_cast<float2 *>(dst + 8 * nd + 2 * c) = make_float2(O[nd][2] * i1, O[nd][3] * i1);
     }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 128;" :: "r"(tmem_base_s) : "memory");
 }
 
 // out[row][k] = sum_j Pi^(128)[j][k] * o'[row][j] / sqrt(128)  ->  bf16  (the V de-rotation, once per output row)
