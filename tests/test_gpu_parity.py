@@ -435,3 +435,10 @@ def test_random_allocations_append_and_attention(P, tab128, seed):
     G = Hq // Hkv
     err = max(np.max(np.abs(got[a] - exp[a])) / max(rv[a // G], 1e-30) for a in range(Hq))
     assert err <= 2e-3, err
+
+
+@pytest.mark.parametrize("Hq,Hkv,bk,bv,T", [(4, 2, 1, 1, 260), (6, 2, 4, 4, 200), (5, 1, 2, 8, 130), (2, 2, 6, 5, 140), (16, 2, 3, 2, 515)])
+def test_attention_more_shapes_and_budgets(P, tab128, Hq, Hkv, bk, bv, T):
+    """GQA groups 1, 2, 3, 5, 8 and budgets K1V1 .. K6V5 / V8 (greedy allocation at that budget)."""
+    err = _attention_case(P, tab128, 90 + T, T, Hq, Hkv, bk, bv, 1, 8, base=5e5)
+    assert err.max() <= 2e-3, err
