@@ -235,6 +235,14 @@ __device__ __forceinline__ void build_pools(const uint16_t *cb16, uint32_t *pool
     pools[7] = plane(15 + 8, 0); pools[8] = plane(15 + 12, 0); pools[9] = plane(15 + 8, 1); pools[10] = plane(15 + 12, 1);
 }
 
+// ---------------------------------------------------------------- programmatic dependent launch
+// qfold -> decode -> combine are launched back to back on one stream.  decode and combine are launched with the
+// programmatic-stream-serialization attribute: their CTAs may start while the previous kernel is still running
+// (pdl_trigger in that kernel), run their prologue (LUTs, prefix sums, slot lists), and block in pdl_wait until the
+// previous kernel has completed and its writes are visible.  Nothing written by a predecessor is read before pdl_wait.
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 // ---------------------------------------------------------------- work partition
 // Global tile list [layer][sequence][kv head][tile]; pre[] = prefix sums of tiles per sequence.
 struct Sched {
@@ -302,6 +310,7 @@ qfold_kernel(const HeadMeta *__restrict__ metas, const float *__restrict__ rot_t
              const __nv_bfloat16 *__restrict__ q, int batch, int Hkv, int Hq, float scale_log2e,
              __half *__restrict__ qf, int plain)
 {
+    pdl_trigger();
     const int G = Hq / Hkv;
     const int pair = blockIdx.x / G, n = blockIdx.x % G;   // one block per (pair, query head of the group)
     const int h = pair % Hkv, lb = pair / Hkv, l = lb / batch;
@@ -536,6 +545,7 @@ decode_kernel(const DecodeParams P)
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int g8 = lane >> 2, c = lane & 3;
+    pdl_trigger();
     build_lut(P.cb16, lut, tid, W * 32, P5);
     if (tid == 0) build_prefix(P.seq_len, P.batch, P.n_cap * kTile, pre);
     if (PARK && warp == 0) {                                      // 4 warps per lane quadrant x 32 columns
@@ -555,6 +565,7 @@ decode_kernel(const DecodeParams P)
         fence_proxy_async();
     }
     __syncthreads();
+    pdl_wait();                                                   // q' (qfold_kernel) is complete from here on
 
     const int gw = blockIdx.x * W + warp;
     const Sched S = make_sched(P.n_layers, P.batch, P.Hkv, pre, gridDim.x, W);
@@ -828,13 +839,16 @@ combine_kernel(const float *__restrict__ partials, const int32_t *__restrict__ s
                const float *__restrict__ rot128, int n_layers, int batch, int Hkv, int G, int64_t n_cap,
                int n_ctas, int W, __nv_bfloat16 *__restrict__ out)
 {
-    constexpr int kMaxSlots = 1024;
+    constexpr int kMaxSlots = 1024;                     // 32 + n_ctas entries at most (host checks n_ctas)
     __shared__ int pre[kMaxBatch + 1];
     __shared__ float o[kDh];
     __shared__ int slots[kMaxSlots];
+    __shared__ float wgt[kMaxSlots];
+    __shared__ float red[4][kDh + 4];
+    __shared__ float wred[2][4];
     const int pair = blockIdx.x / G, n = blockIdx.x % G;
     const int h = pair % Hkv, lb = pair / Hkv, b = lb % batch, l = lb / batch;
-    const int d = threadIdx.x;
+    const int d = threadIdx.x, lane = d & 31, wq = d >> 5;
     if (d == 0) build_prefix(seq_len, batch, n_cap * kTile, pre);
     __syncthreads();
     const Sched S = make_sched(n_layers, batch, Hkv, pre, n_ctas, W);
@@ -851,7 +865,6 @@ combine_kernel(const float *__restrict__ partials, const int32_t *__restrict__ s
     // slot list in a fixed order: [warps of the first CTA][interior CTAs][warps of the last CTA].  Interior
     // CTAs lie wholly inside the pair, so they merged their warps (one record at the slot of warp 0); a CTA
     // straddling the pair boundary left one record per warp.
-    float Mx = -INFINITY, acc = 0.f, lsum = 0.f;       // single pass with a running max (exact: PAPER.md:120)
     const float *rec0 = partials + (size_t)pair * kPartialFloats + n * 130;
     auto edge_slot = [&](int c, int w) -> int {         // record of warp w of boundary CTA c, or -1
         const int lo = cta_lo(S, c), hi = cta_lo(S, c + 1);
@@ -861,29 +874,51 @@ combine_kernel(const float *__restrict__ partials, const int32_t *__restrict__ s
         return (wl < wh && wl < stop && wh > start) ? c * W + w : -1;
     };
     const int n_int = c1 - c0 - 1 > 0 ? c1 - c0 - 1 : 0;
-    const int n_ent = 16 + n_int + (c1 > c0 ? 16 : 0);
-    for (int eb = 0; eb < n_ent; eb += kMaxSlots) {
-        const int ne = min(kMaxSlots, n_ent - eb);
-        __syncthreads();
-        for (int e = d; e < ne; e += 128) {
-            const int ge = eb + e;
-            slots[e] = ge < 16 ? edge_slot(c0, ge) : (ge < 16 + n_int ? edge_slot(c0 + 1 + ge - 16, 0) : edge_slot(c1, ge - 16 - n_int));
-        }
-        __syncthreads();
-#pragma unroll 8
-        for (int e = 0; e < ne; ++e) {
-            const int sl = slots[e];
-            const float *rec = rec0 + (size_t)(sl < 0 ? 0 : sl) * kPartialFloats;
-            const float mw = sl < 0 ? -INFINITY : rec[0];
-            const float lw = sl < 0 ? 0.f : rec[1], aw = sl < 0 ? 0.f : rec[2 + d];
-            const float Mn = fmaxf(Mx, mw);
-            const float fo = Mn == -INFINITY ? 0.f : exp2f(Mx - Mn), fw = Mn == -INFINITY ? 0.f : exp2f(mw - Mn);
-            lsum = fmaf(lsum, fo, lw * fw);
-            acc = fmaf(acc, fo, aw * fw);
-            Mx = Mn;
-        }
+    const int n_ent = min(kMaxSlots, 16 + n_int + (c1 > c0 ? 16 : 0));
+    pdl_wait();                                         // the decode kernel's partials are complete from here on
+    // pass 1: every record's running max -> M, then its weight 2^(m - M) and the merged sum l.  All loads are
+    // independent (one record per thread), and the order of every reduction is fixed, so the result does not depend
+    // on timing.
+    float mloc = -INFINITY;
+    for (int e = d; e < n_ent; e += 128) {
+        const int sl = e < 16 ? edge_slot(c0, e) : (e < 16 + n_int ? edge_slot(c0 + 1 + e - 16, 0) : edge_slot(c1, e - 16 - n_int));
+        slots[e] = sl;
+        const float mw = sl < 0 ? -INFINITY : rec0[(size_t)sl * kPartialFloats];
+        wgt[e] = mw;
+        mloc = fmaxf(mloc, mw);
     }
-    o[d] = acc / lsum;
+#pragma unroll
+    for (int s = 16; s; s >>= 1) mloc = fmaxf(mloc, __shfl_xor_sync(0xffffffffu, mloc, s));
+    if (lane == 0) wred[0][wq] = mloc;
+    __syncthreads();
+    const float Mx = fmaxf(fmaxf(wred[0][0], wred[0][1]), fmaxf(wred[0][2], wred[0][3]));
+    float lloc = 0.f;
+    for (int e = d; e < n_ent; e += 128) {
+        const int sl = slots[e];
+        const float mw = wgt[e];
+        const float f = (sl < 0 || mw == -INFINITY) ? 0.f : exp2f(mw - Mx);
+        wgt[e] = f;
+        if (f != 0.f) lloc = fmaf(rec0[(size_t)sl * kPartialFloats + 1], f, lloc);
+    }
+#pragma unroll
+    for (int s = 16; s; s >>= 1) lloc += __shfl_xor_sync(0xffffffffu, lloc, s);
+    if (lane == 0) wred[1][wq] = lloc;
+    __syncthreads();
+    const float lsum = (wred[1][0] + wred[1][1]) + (wred[1][2] + wred[1][3]);
+    // pass 2: warp wq accumulates records wq, wq+4, ...; a lane owns dims 2*lane, 2*lane+1, 64+2*lane, 65+2*lane
+    float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
+#pragma unroll 4
+    for (int e = wq; e < n_ent; e += 4) {
+        const float f = wgt[e];
+        if (f == 0.f) continue;
+        const float *rec = rec0 + (size_t)slots[e] * kPartialFloats + 2;
+        const float2 lo = *reinterpret_cast<const float2 *>(rec + 2 * lane);
+        const float2 hi = *reinterpret_cast<const float2 *>(rec + 64 + 2 * lane);
+        a0 = fmaf(lo.x, f, a0); a1 = fmaf(lo.y, f, a1); a2 = fmaf(hi.x, f, a2); a3 = fmaf(hi.y, f, a3);
+    }
+    red[wq][2 * lane] = a0; red[wq][2 * lane + 1] = a1; red[wq][64 + 2 * lane] = a2; red[wq][65 + 2 * lane] = a3;
+    __syncthreads();
+    o[d] = ((red[0][d] + red[1][d]) + (red[2][d] + red[3][d])) / lsum;
     __syncthreads();
     if (rot128 == nullptr) { dst[d] = __float2bfloat16(o[d]); return; }    // fp16-cache comparison path: no rotation
     float r = 0.f;
@@ -1177,7 +1212,15 @@ static int launch_decode_w(const DecodeParams &P, int grid, size_t smem, cudaStr
         ++g_prof_used;
         CUDA_TRY(cudaEventRecord(e0, st));
     }
-    decode_kernel<W><<<grid, W * 32, smem, st>>>(P);
+    {
+        cudaLaunchConfig_t cfg = {};
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = g_prof ? 0 : 1;
+        cfg.gridDim = dim3(grid); cfg.blockDim = dim3(W * 32); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        cudaLaunchKernelEx(&cfg, decode_kernel<W>, P);
+    }
     {
         cudaError_t le = cudaPeekAtLastError();
         if (le != cudaSuccess) {
@@ -1230,8 +1273,16 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
     count_launch();
     CUDA_TRY(cudaGetLastError());
 
-    combine_kernel<<<pairs * G, 128, 0, st>>>(partials, seq_len, lay->d_rot + rot_offset(kDh), n_layers, batch,
-                                              Hkv, G, n_cap, grid, W, (__nv_bfloat16 *)out);
+    {
+        cudaLaunchConfig_t cfg = {};
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = g_prof ? 0 : 1;
+        cfg.gridDim = dim3(pairs * G); cfg.blockDim = dim3(128); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        cudaLaunchKernelEx(&cfg, combine_kernel, (const float *)partials, seq_len, (const float *)(lay->d_rot + rot_offset(kDh)),
+                           n_layers, batch, Hkv, G, n_cap, grid, W, (__nv_bfloat16 *)out);
+    }
     count_launch();
     CUDA_TRY(cudaGetLastError());
     return BGTQ_OK;
