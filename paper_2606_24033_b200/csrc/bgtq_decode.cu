@@ -565,7 +565,6 @@ decode_kernel(const DecodeParams P)
         fence_proxy_async();
     }
     __syncthreads();
-    pdl_wait();                                                   // q' (qfold_kernel) is complete from here on
 
     const int gw = blockIdx.x * W + warp;
     const Sched S = make_sched(P.n_layers, P.batch, P.Hkv, pre, gridDim.x, W);
@@ -608,6 +607,9 @@ decode_kernel(const DecodeParams P)
         float *rec = reinterpret_cast<float *>(smem + kSmemHdr + warp * P.buf_bytes);
         for (int i = lane; i < kPartialFloats; i += 32) rec[i] = (i % 130 == 0) ? -INFINITY : 0.f;
     }
+    // The first tile is already in flight (the cache was complete before qfold_kernel started: it is launched without
+    // the attribute); q' and the partial-record workspace may be touched only after the predecessor has completed.
+    pdl_wait();
 
     while (x < x_end) {
         // ---------------- segment = the part of one (layer, sequence, kv head) inside this warp's range
