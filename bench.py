@@ -54,6 +54,8 @@ def parse_args():
                     help="also time bgtq_prefill_attention for the last N cached tokens of layer 0 (NEXT #1, first cut)")
     ap.add_argument("--compare-fp16", action="store_true",
                     help="also time the fp16-cache comparison kernel (bgtq_fp16_decode_attention) on the same K, V")
+    ap.add_argument("--paged", action="store_true",
+                    help="also time bgtq_decode_attention_paged on a scattered-page copy of the same cache")
     ap.add_argument("--alloc", default="greedy", choices=["greedy", "uniform", "paper_like"],
                     help="K allocation: greedy = Block-GTQ from the library's energy->allocate path (the metric's workload); "
                          "uniform = one group at b_k bits (uniform TQ-MSE, PAPER.md:108); paper_like = greedy on scores whose "
@@ -440,6 +442,45 @@ def run_ours(args):
             comparison["speedup_packed_vs_fp16_attention_call"] = us16 / usp
             del k16, v16
 
+        # ---- NEXT #4: the same attention over a paged copy of the cache (random page table), device-timed
+        paged = None
+        if args.paged:
+            shp_ = W.CONFIGS[args.config]
+            n_cap = (wl["max_tokens"] + 127) // 128
+            n_pages = args.batch * n_cap
+            gen = torch.Generator(device="cpu")
+            gen.manual_seed(1234)
+            table = torch.randperm(n_pages, generator=gen).to(torch.int32).reshape(args.batch, n_cap).to(device)
+            pc = torch.empty(lay.paged_cache_bytes(n_pages), dtype=torch.uint8, device=device)
+            for l in range(Lyr):                          # harness-side scatter of the contiguous tiles into pages
+                for h in range(shp_.n_kv_heads):
+                    st_, po = lay.tile_stride(l, h), lay.paged_pool_offset(l, h, n_pages)
+                    pool = pc[po:po + n_pages * st_].view(n_pages, st_)
+                    for b in range(args.batch):
+                        ro = lay.region_offset(l, b, h, args.batch, wl["max_tokens"])
+                        pool[table[b].long()] = cache[ro:ro + n_cap * st_].view(n_cap, st_)
+            outp = torch.empty_like(q)
+            tms = {}
+            for name in ("contiguous", "paged"):
+                def call():
+                    if name == "paged":
+                        P.decode_attention_paged(lay, 0, pc, q, seq, table, n_pages, wl["scale"], ws, out=outp, n_layers=Lyr)
+                    else:
+                        P.decode_attention(lay, 0, cache, q, seq, wl["max_tokens"], wl["scale"], ws, out=out, n_layers=Lyr)
+                for _ in range(3):
+                    call()
+                g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                g0.record(stream)
+                for _ in range(10):
+                    call()
+                g1.record(stream)
+                stream.synchronize()
+                tms[name] = g0.elapsed_time(g1) / 10 * 1e3
+            paged = {"attention_call_us": tms["paged"], "contiguous_attention_call_us": tms["contiguous"],
+                     "n_pages": n_pages, "outputs_bit_identical": bool(torch.equal(out, outp)),
+                     "note": "random page table over batch*ceil(max_tokens/128) pages; same tiles, scattered"}
+            del pc
+
         # ---- NEXT #1: causal prefill attention of the last N cached tokens (layer 0), device-timed
         prefill = None
         if args.prefill_chunk > 0:
@@ -534,7 +575,7 @@ def run_ours(args):
             "e2e": {"value": e2e_val, "unit": "GB/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": e2e_ms},
             "gpu_launches": int(launches_per_step) * args.steps, "gpu_launches_per_step": int(launches_per_step),
-            "comparison": comparison, "prefill": prefill,
+            "comparison": comparison, "prefill": prefill, "paged": paged,
         }))
     if world > 1:
         dist.destroy_process_group()

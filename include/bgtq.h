@@ -145,6 +145,29 @@ int bgtq_decode_attention_layers(const bgtq_layout *layout, int layer0, int n_la
                                  int batch, int64_t max_tokens, float softmax_scale, void *out,
                                  void *workspace, size_t workspace_bytes, void *stream);
 
+/* ---- SURVEY.md 8(f).4 "paged sequences": the same two calls over a PAGED cache.
+ * The cache is a set of pools, one per (layer, kv head), each of n_pages pages; a page is one
+ * 128-token tile of that head (bgtq_tile_stride bytes, the same tile format as the contiguous
+ * layout).  Pool (layer, kv_head) starts at byte bgtq_paged_pool_offset(...).
+ * page_table [device] int32 [batch, table_stride]: page_table[s][j] = page that holds tokens
+ * [128 j, 128 j + 128) of sequence s, the same index in every (layer, head) pool (one logical block
+ * id per 128 tokens, as in a paged serving cache).  Entries are read only for tiles below
+ * ceil(seq_len[s]/128) (decode) or touched by the new tokens (append); they must be in
+ * [0, n_pages) and distinct across live tiles -- not checked on the device.  Capacity per sequence
+ * is 128 * table_stride tokens; everything else (arguments, arithmetic, results) is as for the
+ * contiguous calls above: a paged cache holds byte-identical tiles, only their addresses differ. */
+size_t bgtq_paged_cache_bytes(const bgtq_layout *layout, int64_t n_pages);
+int64_t bgtq_paged_pool_offset(const bgtq_layout *layout, int layer, int kv_head, int64_t n_pages);
+int bgtq_quantize_append_paged(const bgtq_layout *layout, int layer0, int n_layers, void *cache,
+                               const void *k_new, const void *v_new, int dt, int batch, int n_new,
+                               int32_t *seq_len, int advance_seq_len, const int32_t *page_table,
+                               int table_stride, int64_t n_pages, void *stream);
+int bgtq_decode_attention_paged(const bgtq_layout *layout, int layer0, int n_layers, const void *cache,
+                                const void *q, const int32_t *seq_len, int batch,
+                                const int32_t *page_table, int table_stride, int64_t n_pages,
+                                float softmax_scale, void *out, void *workspace,
+                                size_t workspace_bytes, void *stream);
+
 /* ---- NEXT #1: causal prefill attention over the packed cache.  The chunk's K, V are
  * already in the cache (bgtq_quantize_append first): query token i of sequence s sits at position
  * seq_len[s] - n_q + i and attends to cached tokens [0, that position] (itself included).

@@ -29,6 +29,7 @@ SYMBOLS = [
     "bgtq_quantize_append", "bgtq_quantize_append_layers", "bgtq_profile_decode",
     "bgtq_profile_decode_read", "bgtq_decode_attention", "bgtq_decode_attention_layers",
     "bgtq_prefill_workspace_bytes", "bgtq_prefill_attention", "bgtq_fp16_workspace_bytes", "bgtq_fp16_decode_attention", "bgtq_debug_decode_unit", "bgtq_launch_count",
+    "bgtq_paged_cache_bytes", "bgtq_paged_pool_offset", "bgtq_quantize_append_paged", "bgtq_decode_attention_paged",
 ]
 
 
@@ -93,6 +94,14 @@ def _load() -> C.CDLL:
     lib.bgtq_fp16_decode_attention.argtypes = [i32, i32, i32, i32, i32, vp, vp, vp, vp, i64, f32, vp, vp, sz, vp]
     lib.bgtq_debug_decode_unit.restype = i32
     lib.bgtq_debug_decode_unit.argtypes = [i32, vp, vp]
+    lib.bgtq_paged_cache_bytes.restype = sz
+    lib.bgtq_paged_cache_bytes.argtypes = [vp, i64]
+    lib.bgtq_paged_pool_offset.restype = i64
+    lib.bgtq_paged_pool_offset.argtypes = [vp, i32, i32, i64]
+    lib.bgtq_quantize_append_paged.restype = i32
+    lib.bgtq_quantize_append_paged.argtypes = [vp, i32, i32, vp, vp, vp, i32, i32, i32, vp, i32, vp, i32, i64, vp]
+    lib.bgtq_decode_attention_paged.restype = i32
+    lib.bgtq_decode_attention_paged.argtypes = [vp, i32, i32, vp, vp, vp, i32, vp, i32, i64, f32, vp, vp, sz, vp]
     return lib
 
 
@@ -209,6 +218,12 @@ class Layout:
     def region_offset(self, layer: int, seq: int, kv_head: int, batch: int, max_tokens: int) -> int:
         return int(_lib.bgtq_region_offset(self._h, layer, seq, kv_head, batch, max_tokens))
 
+    def paged_cache_bytes(self, n_pages: int) -> int:
+        return int(_lib.bgtq_paged_cache_bytes(self._h, n_pages))
+
+    def paged_pool_offset(self, layer: int, kv_head: int, n_pages: int) -> int:
+        return int(_lib.bgtq_paged_pool_offset(self._h, layer, kv_head, n_pages))
+
     def tile_stride(self, layer: int, kv_head: int) -> int:
         return int(_lib.bgtq_tile_stride(self._h, layer, kv_head))
 
@@ -237,6 +252,40 @@ def quantize_append(layout: Layout, layer: int, cache: torch.Tensor, k_new: torc
     _check(_lib.bgtq_quantize_append(layout._h, layer, _dev(cache, torch.uint8), _dev(k_new), _dev(v_new),
                                      _dt(k_new), batch, n_new, _dev(seq_len, torch.int32),
                                      1 if advance_seq_len else 0, max_tokens, _stream()))
+
+
+def quantize_append_paged(layout: Layout, layer: int, cache: torch.Tensor, k_new: torch.Tensor,
+                          v_new: torch.Tensor, seq_len: torch.Tensor, page_table: torch.Tensor, n_pages: int,
+                          advance_seq_len: bool = True, n_layers: int = 1) -> None:
+    """bgtq_quantize_append_paged: k_new, v_new [batch, n_new, H_kv, d_h] (n_layers = 1) or
+    [n_layers, batch, n_new, H_kv, d_h]; page_table int32 [batch, table_stride] (CUDA)."""
+    batch, n_new, Hkv, d = k_new.shape[-4:]
+    assert v_new.shape == k_new.shape and Hkv == layout.n_kv_heads and d == layout.d_h
+    assert _dt(k_new) == _dt(v_new)
+    assert k_new.dim() == 4 and n_layers == 1 or k_new.dim() == 5 and k_new.shape[0] == n_layers
+    assert page_table.dim() == 2 and page_table.shape[0] == batch
+    _check(_lib.bgtq_quantize_append_paged(layout._h, layer, n_layers, _dev(cache, torch.uint8), _dev(k_new), _dev(v_new),
+                                           _dt(k_new), batch, n_new, _dev(seq_len, torch.int32),
+                                           1 if advance_seq_len else 0, _dev(page_table, torch.int32),
+                                           page_table.shape[1], n_pages, _stream()))
+
+
+def decode_attention_paged(layout: Layout, layer: int, cache: torch.Tensor, q: torch.Tensor, seq_len: torch.Tensor,
+                           page_table: torch.Tensor, n_pages: int, softmax_scale: float, workspace: torch.Tensor,
+                           out: Optional[torch.Tensor] = None, n_layers: int = 1) -> torch.Tensor:
+    """bgtq_decode_attention_paged: q bf16 [batch, H_q, d_h] (n_layers = 1) or [n_layers, batch, H_q, d_h]."""
+    if out is None:
+        out = torch.empty_like(q)
+    batch = q.shape[-3]
+    assert q.shape[-2] == layout.n_q_heads and q.shape[-1] == layout.d_h
+    assert q.dim() == 3 and n_layers == 1 or q.dim() == 4 and q.shape[0] == n_layers
+    assert page_table.dim() == 2 and page_table.shape[0] == batch
+    _check(_lib.bgtq_decode_attention_paged(layout._h, layer, n_layers, _dev(cache, torch.uint8), _dev(q, torch.bfloat16),
+                                            _dev(seq_len, torch.int32), batch, _dev(page_table, torch.int32),
+                                            page_table.shape[1], n_pages, float(softmax_scale),
+                                            _dev(out, torch.bfloat16), _dev(workspace, torch.uint8),
+                                            workspace.numel(), _stream()))
+    return out
 
 
 def profile_decode(enable: bool) -> None:

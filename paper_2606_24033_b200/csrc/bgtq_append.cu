@@ -61,7 +61,7 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
                        const T *__restrict__ k_new, const T *__restrict__ v_new,
                        const double *__restrict__ cb64, const float *__restrict__ rot_t, int batch,
                        int n_new, int Hkv, const int32_t *__restrict__ seq_len, int64_t n_cap,
-                       int64_t max_tokens)
+                       int64_t max_tokens, const int32_t *__restrict__ pages, int pstride, int64_t n_pages)
 {
     extern __shared__ __align__(16) unsigned char smem[];
     const int tid = threadIdx.x;
@@ -85,7 +85,8 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
     int *n_units_p = reinterpret_cast<int *>(units + kMaxUnits);
     uint32_t *tbuf = reinterpret_cast<uint32_t *>(n_units_p + 4);        // tile, `stride` bytes
 
-    uint8_t *gtile = cache + n_cap * ((int64_t)batch * M.layer_prefix + (int64_t)s * M.layer_sum + M.head_prefix) + tile * stride;
+    uint8_t *gtile = pages ? cache + n_pages * ((int64_t)M.layer_prefix + M.head_prefix) + (int64_t)pages[(int64_t)s * pstride + tile] * stride
+                           : cache + n_cap * ((int64_t)batch * M.layer_prefix + (int64_t)s * M.layer_sum + M.head_prefix) + tile * stride;
     {   // stage the tile: older tokens present -> load, else start from zeros
         const bool has_old = tile_lo < t0;
         const uint4 *src = reinterpret_cast<const uint4 *>(gtile);
@@ -289,7 +290,7 @@ static size_t append_smem_bytes(int max_stride)
 
 int launch_quantize_append(const bgtq_layout *lay, int layer, int n_layers, void *cache, const void *k_new,
                            const void *v_new, int dt, int batch, int n_new, int32_t *seq_len,
-                           int advance, int64_t max_tokens, cudaStream_t st)
+                           int advance, int64_t max_tokens, const PageMap *pm, cudaStream_t st)
 {
     static bool attr_set = false;
     const int64_t n_cap = (max_tokens + kTile - 1) / kTile;
@@ -305,11 +306,13 @@ int launch_quantize_append(const bgtq_layout *lay, int layer, int n_layers, void
     if (dt == BGTQ_F32) {
         quantize_append_kernel<float><<<grid, kAppendThreads, smem, st>>>(
             metas, (uint8_t *)cache, (const float *)k_new, (const float *)v_new, lay->d_cb64, lay->d_rot_t,
-            batch, n_new, lay->n_kv_heads, seq_len, n_cap, n_cap * kTile);
+            batch, n_new, lay->n_kv_heads, seq_len, n_cap, n_cap * kTile, pm ? pm->table : nullptr,
+            pm ? pm->table_stride : 0, pm ? pm->n_pages : 0);
     } else {
         quantize_append_kernel<__nv_bfloat16><<<grid, kAppendThreads, smem, st>>>(
             metas, (uint8_t *)cache, (const __nv_bfloat16 *)k_new, (const __nv_bfloat16 *)v_new, lay->d_cb64,
-            lay->d_rot_t, batch, n_new, lay->n_kv_heads, seq_len, n_cap, n_cap * kTile);
+            lay->d_rot_t, batch, n_new, lay->n_kv_heads, seq_len, n_cap, n_cap * kTile, pm ? pm->table : nullptr,
+            pm ? pm->table_stride : 0, pm ? pm->n_pages : 0);
     }
     count_launch();
     CUDA_TRY(cudaGetLastError());

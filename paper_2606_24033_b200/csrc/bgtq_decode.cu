@@ -33,6 +33,9 @@ namespace bgtq {
 #ifndef BGTQ_NORM_IN_OPERAND
 #define BGTQ_NORM_IN_OPERAND 0   // 1: fold K group norms into the fp16 A operand (measured: no faster, less exact); 0: scale fp32 accumulators
 #endif
+#ifndef BGTQ_TIMING
+#define BGTQ_TIMING 0
+#endif
 #ifndef BGTQ_NO_P5
 #define BGTQ_NO_P5 0
 #endif
@@ -390,6 +393,9 @@ struct DecodeParams {
     int64_t n_cap;              // tiles of capacity per sequence
     int n_layers, batch, Hkv, G;
     int buf_bytes;              // per-warp tile buffer
+    const int32_t *pages;       // paged cache: [batch][pstride] page index per tile (nullptr: contiguous layout)
+    int pstride;
+    int64_t n_pages;
 };
 
 constexpr int kSmemHdr = 0;      // dynamic shared memory holds only the tile buffers (tables are static)
@@ -530,7 +536,7 @@ __device__ __forceinline__ void pv_tile(const uint32_t *vcodes, int lane, const 
     }
 }
 
-template <int W>
+template <int W, bool PAGED>
 __global__ void __launch_bounds__(W * 32, 1)
 decode_kernel(const DecodeParams P)
 {
@@ -546,6 +552,14 @@ decode_kernel(const DecodeParams P)
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int g8 = lane >> 2, c = lane & 3;
     pdl_trigger();
+#if BGTQ_TIMING
+    unsigned long long tst[10];
+    auto TS = [&](int i) { asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tst[i])); };
+    for (int i = 0; i < 10; ++i) tst[i] = 0;
+    TS(0);
+#else
+    auto TS = [&](int) {};
+#endif
     build_lut(P.cb16, lut, tid, W * 32, P5);
     if (tid == 0) build_prefix(P.seq_len, P.batch, P.n_cap * kTile, pre);
     if (PARK && warp == 0) {                                      // 4 warps per lane quadrant x 32 columns
@@ -565,6 +579,7 @@ decode_kernel(const DecodeParams P)
         fence_proxy_async();
     }
     __syncthreads();
+    TS(1);
 
     const int gw = blockIdx.x * W + warp;
     const Sched S = make_sched(P.n_layers, P.batch, P.Hkv, pre, gridDim.x, W);
@@ -596,6 +611,9 @@ decode_kernel(const DecodeParams P)
         if (want_v) { mbar_expect_tx(vbar, vbytes); bulk_g2s(tile_s + kbytes, src + kbytes, vbytes, vbar); }
     };
     auto tile_src = [&](const TilePos &tp, const HeadMeta &M) -> const uint8_t * {
+        if (PAGED)
+            return P.cache + P.n_pages * ((int64_t)M.layer_prefix + M.head_prefix) +
+                   (int64_t)__ldg(P.pages + (int64_t)tp.b * P.pstride + tp.t) * M.tile_stride;
         return P.cache + P.n_cap * ((int64_t)P.batch * M.layer_prefix + (int64_t)tp.b * M.layer_sum + M.head_prefix) +
                (int64_t)tp.t * M.tile_stride;
     };
@@ -609,7 +627,9 @@ decode_kernel(const DecodeParams P)
     }
     // The first tile is already in flight (the cache was complete before qfold_kernel started: it is launched without
     // the attribute); q' and the partial-record workspace may be touched only after the predecessor has completed.
+    TS(2);
     pdl_wait();
+    TS(3);
 
     while (x < x_end) {
         // ---------------- segment = the part of one (layer, sequence, kv head) inside this warp's range
@@ -630,6 +650,8 @@ decode_kernel(const DecodeParams P)
         const uint2 *qfp = reinterpret_cast<const uint2 *>(P.qf + (size_t)tp.pair * kQfHalves) + lane;
         const uint8_t *src = tile_src(tp, M);                     // current tile of this segment (advanced per tile)
         const uint32_t stride = M.tile_stride, kbytes = M.vnorm_off, vbytes = stride - kbytes;
+        const uint8_t *pool = P.cache + P.n_pages * ((int64_t)M.layer_prefix + M.head_prefix);   // paged layout only
+        const int32_t *prow = P.pages + (int64_t)tp.b * P.pstride;
 
         float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;   // heads 2c, 2c+1 (log2 domain)
         float O[8][4];
@@ -639,8 +661,11 @@ decode_kernel(const DecodeParams P)
 
         for (int t = tp.t; x < seg_end; ++x, ++t) {
             // ======== QK^T
+            // paged: the next tile's page index is fetched a whole QK^T ahead of the copy that needs it
+            const int next_page = (PAGED && x + 1 < seg_end) ? __ldg(prow + t + 1) : 0;
             mbar_wait(kbar, kphase);
             kphase ^= 1;
+            TS(4);
             float Sc[8][4];
 #pragma unroll
             for (int i = 0; i < 8; ++i) Sc[i][0] = Sc[i][1] = Sc[i][2] = Sc[i][3] = 0.f;
@@ -701,9 +726,10 @@ decode_kernel(const DecodeParams P)
             }
 #endif
             __syncwarp();
-            src += stride;
+            src = PAGED ? pool + (int64_t)next_page * stride : src + stride;
             if (lane == 0 && x + 1 < seg_end) issue_at(src, kbytes, vbytes, true, false);   // K half of the next tile (same layout only)
 
+            TS(5);
             // ======== mask the ragged tail, online softmax (log2 domain)
             const int n_valid = (int)min((int64_t)kTile, slen - (int64_t)t * kTile);
             if (n_valid < kTile) {
@@ -746,6 +772,7 @@ decode_kernel(const DecodeParams P)
             // ======== P * (V norm) -> fp16 B fragments (8x8 transposes), then PV
             mbar_wait(vbar, vphase);
             vphase ^= 1;
+            TS(6);
             uint32_t bP[8][2];
             {
                 const uint4 *np = reinterpret_cast<const uint4 *>(tile + ((vnorm_off + g8 * 32) >> 2));
@@ -770,6 +797,7 @@ decode_kernel(const DecodeParams P)
             default: pv_tile<8, P5>(vcodes, lane, bP, pools, lut, O); break;
             }
             __syncwarp();
+            TS(7);
             if (PARK) tmem_park(taddr, O);
             if (x + 1 < seg_end) {
                 if (lane == 0) issue_at(src, kbytes, vbytes, false, true);                   // V half of the next tile
@@ -803,6 +831,7 @@ decode_kernel(const DecodeParams P)
             for (int J = 0; J < 8; ++J) { r1[2 + 16 * J + g8] = O[J][1]; r1[2 + 16 * J + 8 + g8] = O[J][3]; }
         }
     }
+    TS(8);
     if (merged) {      // exact log-sum-exp merge of the W warp partials, one record per CTA
         __syncthreads();
         const float *all = reinterpret_cast<const float *>(smem + kSmemHdr);
@@ -826,6 +855,12 @@ decode_kernel(const DecodeParams P)
             if (dd == 0) { dst[n * 130] = Mx; dst[n * 130 + 1] = ls; }
         }
     }
+#if BGTQ_TIMING
+    TS(9);
+    if (lane == 0 && (blockIdx.x % 37) == 5 && warp < 2)
+        printf("cta %d warp %d: prologue %llu issue %llu pdlwait %llu ktile %llu qk %llu softmax+vwait %llu pv %llu tail %llu merge %llu total %llu\n", blockIdx.x, warp,
+               tst[1] - tst[0], tst[2] - tst[1], tst[3] - tst[2], tst[4] - tst[3], tst[5] - tst[4], tst[6] - tst[5], tst[7] - tst[6], tst[8] - tst[7], tst[9] - tst[8], tst[9] - tst[0]);
+#endif
     if (PARK) {
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
         __syncthreads();
@@ -1194,12 +1229,12 @@ int profile_decode_read(double *ms_sum, int *count)
     return BGTQ_OK;
 }
 
-template <int W>
+template <int W, bool PAGED>
 static int launch_decode_w(const DecodeParams &P, int grid, size_t smem, cudaStream_t st)
 {
     static bool attr_set = false;
     if (!attr_set) {   // once per process, outside any stream capture
-        CUDA_TRY(cudaFuncSetAttribute(decode_kernel<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - (W == 16 ? 2560 : kStaticSmem)));
+        CUDA_TRY(cudaFuncSetAttribute(decode_kernel<W, PAGED>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - (W == 16 ? 2560 : kStaticSmem)));
         attr_set = true;
     }
     cudaEvent_t e0 = nullptr, e1 = nullptr;
@@ -1221,13 +1256,13 @@ static int launch_decode_w(const DecodeParams &P, int grid, size_t smem, cudaStr
         at[0].val.programmaticStreamSerializationAllowed = g_prof ? 0 : 1;
         cfg.gridDim = dim3(grid); cfg.blockDim = dim3(W * 32); cfg.dynamicSmemBytes = smem; cfg.stream = st;
         cfg.attrs = at; cfg.numAttrs = 1;
-        cudaLaunchKernelEx(&cfg, decode_kernel<W>, P);
+        cudaLaunchKernelEx(&cfg, decode_kernel<W, PAGED>, P);
     }
     {
         cudaError_t le = cudaPeekAtLastError();
         if (le != cudaSuccess) {
             cudaFuncAttributes fa;
-            cudaFuncGetAttributes(&fa, decode_kernel<W>);
+            cudaFuncGetAttributes(&fa, decode_kernel<W, PAGED>);
             set_error(std::string("decode launch: ") + cudaGetErrorString(le) + " regs=" + std::to_string(fa.numRegs) + " maxthr=" + std::to_string(fa.maxThreadsPerBlock) + " static=" + std::to_string(fa.sharedSizeBytes) + " dyn=" + std::to_string(smem) + " maxdyn=" + std::to_string(fa.maxDynamicSharedSizeBytes));
             cudaGetLastError();
             return BGTQ_ECUDA;
@@ -1239,7 +1274,7 @@ static int launch_decode_w(const DecodeParams &P, int grid, size_t smem, cudaStr
 
 int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *cache, const void *q,
                   const int32_t *seq_len, int batch, int64_t max_tokens, float scale, void *out,
-                  void *ws, size_t, cudaStream_t st)
+                  void *ws, size_t, const PageMap *pm, cudaStream_t st)
 {
     if (batch > kMaxBatch) { set_error("bgtq_decode_attention: batch > 256"); return BGTQ_EINVAL; }
     const int Hkv = lay->n_kv_heads, Hq = lay->n_q_heads, G = Hq / Hkv;
@@ -1262,14 +1297,24 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
     P.metas = metas; P.cache = (const uint8_t *)cache; P.qf = qf; P.seq_len = seq_len; P.cb16 = lay->d_cb16;
     P.partials = partials; P.n_cap = n_cap; P.n_layers = n_layers; P.batch = batch; P.Hkv = Hkv; P.G = G;
     P.buf_bytes = buf_bytes;
+    P.pages = pm ? pm->table : nullptr; P.pstride = pm ? pm->table_stride : 0; P.n_pages = pm ? pm->n_pages : 0;
     const int grid = lay->sm_count;
     const size_t smem = decode_smem(W, buf_bytes);
     int rc;
-    switch (W) {
-    case 16: rc = launch_decode_w<16>(P, grid, smem, st); break;
-    case 12: rc = launch_decode_w<12>(P, grid, smem, st); break;
-    case 8: rc = launch_decode_w<8>(P, grid, smem, st); break;
-    default: rc = launch_decode_w<4>(P, grid, smem, st); break;
+    if (pm) {
+        switch (W) {
+        case 16: rc = launch_decode_w<16, true>(P, grid, smem, st); break;
+        case 12: rc = launch_decode_w<12, true>(P, grid, smem, st); break;
+        case 8: rc = launch_decode_w<8, true>(P, grid, smem, st); break;
+        default: rc = launch_decode_w<4, true>(P, grid, smem, st); break;
+        }
+    } else {
+        switch (W) {
+        case 16: rc = launch_decode_w<16, false>(P, grid, smem, st); break;
+        case 12: rc = launch_decode_w<12, false>(P, grid, smem, st); break;
+        case 8: rc = launch_decode_w<8, false>(P, grid, smem, st); break;
+        default: rc = launch_decode_w<4, false>(P, grid, smem, st); break;
+        }
     }
     if (rc != BGTQ_OK) return rc;
     count_launch();

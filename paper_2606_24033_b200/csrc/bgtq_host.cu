@@ -295,7 +295,53 @@ extern "C" int bgtq_quantize_append_layers(const bgtq_layout *lay, int layer0, i
     if (n_new == 0) return BGTQ_OK;
     if (!k_new || !v_new) FAIL(BGTQ_EINVAL, "bgtq_quantize_append: null k_new/v_new");
     return launch_quantize_append(lay, layer0, n_layers, cache, k_new, v_new, dt, batch, n_new, seq_len,
-                                  advance_seq_len, max_tokens, (cudaStream_t)stream);
+                                  advance_seq_len, max_tokens, nullptr, (cudaStream_t)stream);
+}
+
+// ------------------------------------------------------------------ paged cache
+extern "C" size_t bgtq_paged_cache_bytes(const bgtq_layout *lay, int64_t n_pages)
+{
+    if (!lay || n_pages <= 0) return 0;
+    return (size_t)(n_pages * lay->total_stride_sum);
+}
+extern "C" int64_t bgtq_paged_pool_offset(const bgtq_layout *lay, int layer, int kv_head, int64_t n_pages)
+{
+    if (!lay || layer < 0 || layer >= lay->n_layers || kv_head < 0 || kv_head >= lay->n_kv_heads || n_pages <= 0) return -1;
+    const HeadMeta &m = lay->meta[(size_t)layer * lay->n_kv_heads + kv_head];
+    return n_pages * ((int64_t)m.layer_prefix + m.head_prefix);
+}
+extern "C" int bgtq_quantize_append_paged(const bgtq_layout *lay, int layer0, int n_layers, void *cache,
+                                          const void *k_new, const void *v_new, int dt, int batch, int n_new,
+                                          int32_t *seq_len, int advance_seq_len, const int32_t *page_table,
+                                          int table_stride, int64_t n_pages, void *stream)
+{
+    if (!lay || !cache || !seq_len || !page_table) FAIL(BGTQ_EINVAL, "bgtq_quantize_append_paged: null pointer");
+    if (layer0 < 0 || n_layers <= 0 || layer0 + n_layers > lay->n_layers) FAIL(BGTQ_EINVAL, "bgtq_quantize_append_paged: layer out of range");
+    if (dt != BGTQ_F32 && dt != BGTQ_BF16) FAIL(BGTQ_EINVAL, "bgtq_quantize_append_paged: dtype");
+    if (batch <= 0 || n_new < 0 || table_stride <= 0 || n_pages <= 0) FAIL(BGTQ_EINVAL, "bgtq_quantize_append_paged: batch/n_new/table_stride/n_pages");
+    if (batch > 65535 || (int64_t)n_layers * lay->n_kv_heads > 65535) FAIL(BGTQ_EINVAL, "bgtq_quantize_append_paged: batch or layers*heads > 65535");
+    const int64_t max_tokens = (int64_t)table_stride * kTile;
+    if (n_new > max_tokens) FAIL(BGTQ_ECAPACITY, "bgtq_quantize_append_paged: n_new exceeds 128 * table_stride");
+    if (n_new == 0) return BGTQ_OK;
+    if (!k_new || !v_new) FAIL(BGTQ_EINVAL, "bgtq_quantize_append_paged: null k_new/v_new");
+    const PageMap pm{page_table, table_stride, n_pages};
+    return launch_quantize_append(lay, layer0, n_layers, cache, k_new, v_new, dt, batch, n_new, seq_len,
+                                  advance_seq_len, max_tokens, &pm, (cudaStream_t)stream);
+}
+extern "C" int bgtq_decode_attention_paged(const bgtq_layout *lay, int layer0, int n_layers, const void *cache,
+                                           const void *q, const int32_t *seq_len, int batch,
+                                           const int32_t *page_table, int table_stride, int64_t n_pages,
+                                           float softmax_scale, void *out, void *workspace,
+                                           size_t workspace_bytes, void *stream)
+{
+    if (!lay || !cache || !q || !seq_len || !out || !workspace || !page_table) FAIL(BGTQ_EINVAL, "bgtq_decode_attention_paged: null pointer");
+    if (layer0 < 0 || n_layers <= 0 || layer0 + n_layers > lay->n_layers) FAIL(BGTQ_EINVAL, "bgtq_decode_attention_paged: layer range");
+    if (batch <= 0 || table_stride <= 0 || n_pages <= 0) FAIL(BGTQ_EINVAL, "bgtq_decode_attention_paged: batch/table_stride/n_pages");
+    if (!(softmax_scale > 0.0f) || std::isinf(softmax_scale)) FAIL(BGTQ_EINVAL, "bgtq_decode_attention_paged: softmax_scale must be finite and > 0");
+    if (workspace_bytes < decode_ws_bytes(lay, batch, n_layers)) FAIL(BGTQ_EWORKSPACE, "bgtq_decode_attention_paged: workspace too small");
+    const PageMap pm{page_table, table_stride, n_pages};
+    return launch_decode(lay, layer0, n_layers, cache, q, seq_len, batch, (int64_t)table_stride * kTile, softmax_scale,
+                         out, workspace, workspace_bytes, &pm, (cudaStream_t)stream);
 }
 
 extern "C" int bgtq_quantize_append(const bgtq_layout *lay, int layer, void *cache, const void *k_new,
@@ -325,7 +371,7 @@ extern "C" int bgtq_decode_attention_layers(const bgtq_layout *lay, int layer0, 
     if (!(softmax_scale > 0.0f) || std::isinf(softmax_scale)) FAIL(BGTQ_EINVAL, "bgtq_decode_attention: softmax_scale must be finite and > 0");
     if (workspace_bytes < decode_ws_bytes(lay, batch, n_layers)) FAIL(BGTQ_EWORKSPACE, "bgtq_decode_attention: workspace too small");
     return launch_decode(lay, layer0, n_layers, cache, q, seq_len, batch, max_tokens, softmax_scale,
-                         out, workspace, workspace_bytes, (cudaStream_t)stream);
+                         out, workspace, workspace_bytes, nullptr, (cudaStream_t)stream);
 }
 
 extern "C" int bgtq_decode_attention(const bgtq_layout *lay, int layer, const void *cache, const void *q,

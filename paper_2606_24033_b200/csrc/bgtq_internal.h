@@ -68,6 +68,15 @@ __host__ __device__ inline int64_t rot_offset(int m)  // element offset of Pi^(m
     return 4 * ((n - 1) * n * (2 * n - 1) / 6);
 }
 
+// Paged cache (bgtq_*_paged): pools [layer][kv head][page], one page = one 128-token tile of that head;
+// table[seq * table_stride + tile] = page index, the same index in every (layer, head) pool.  table == nullptr:
+// the contiguous layout [layer][seq][kv head][tile].
+struct PageMap {
+    const int32_t *table;
+    int table_stride;
+    int64_t n_pages;
+};
+
 // implemented in the .cu files
 int launch_block_energy(const void *q, int64_t n_q, const void *k, int64_t n_k, int dt, int Hq,
                         int Hkv, int d_h, int pairing, int kind, float *scores, float *eq_out,
@@ -77,10 +86,10 @@ int launch_allocate(const float *scores, int n_heads, int L, int b_min, int b_ma
                     uint8_t *bits, cudaStream_t st);
 int launch_quantize_append(const bgtq_layout *lay, int layer, int n_layers, void *cache, const void *k_new,
                            const void *v_new, int dt, int batch, int n_new, int32_t *seq_len,
-                           int advance, int64_t max_tokens, cudaStream_t st);
+                           int advance, int64_t max_tokens, const PageMap *pm, cudaStream_t st);
 int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *cache,
                   const void *q, const int32_t *seq_len, int batch, int64_t max_tokens,
-                  float scale, void *out, void *ws, size_t ws_bytes, cudaStream_t st);
+                  float scale, void *out, void *ws, size_t ws_bytes, const PageMap *pm, cudaStream_t st);
 size_t decode_ws_bytes(const bgtq_layout *lay, int batch, int n_layers);
 int debug_decode_unit(int b, const uint32_t *words, float *values);
 size_t prefill_ws_bytes(const bgtq_layout *lay, int batch, int n_q);

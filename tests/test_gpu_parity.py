@@ -442,3 +442,89 @@ def test_attention_more_shapes_and_budgets(P, tab128, Hq, Hkv, bk, bv, T):
     """GQA groups 1, 2, 3, 5, 8 and budgets K1V1 .. K6V5 / V8 (greedy allocation at that budget)."""
     err = _attention_case(P, tab128, 90 + T, T, Hq, Hkv, bk, bv, 1, 8, base=5e5)
     assert err.max() <= 2e-3, err
+
+
+def test_paged_cache_append_and_attention(P, tab128):
+    """bgtq_quantize_append_paged + bgtq_decode_attention_paged.  A paged cache holds the same
+    tiles as the contiguous one at addresses given by a page table, so every page must equal the oracle's packed
+    tile byte for byte and attention must match the oracle; pages are scattered, shared across 2 layers, and the
+    sequences grow in uneven chunks (a page boundary inside a chunk, an incremental single token)."""
+    Lyr, B, Hq, Hkv, d = 2, 3, 8, 2, 128
+    lens = [389, 150, 0]
+    probs = [[H.make_problem(160 + 10 * l + b, max(lens[b], 1), Hq, Hkv, 3, 3, 1, 8, rope_base=1e6) for b in range(B)]
+             for l in range(Lyr)]
+    for l in range(Lyr):
+        for b in range(B):
+            probs[l][b].bits = probs[l][0].bits
+    bits = np.stack([probs[l][0].bits for l in range(Lyr)])
+    lay = P.Layout(bits, Hq, d, 3, probs[0][0].rot)
+    table_stride, n_pages = 5, 23
+    rng = np.random.default_rng(7)
+    perm = rng.permutation(n_pages)[:B * table_stride].astype(np.int32).reshape(B, table_stride)   # distinct pages
+    table = torch.from_numpy(perm).cuda()
+    cache = torch.full((lay.paged_cache_bytes(n_pages),), 0xAB, dtype=torch.uint8, device="cuda")   # pages start dirty
+    assert lay.paged_cache_bytes(n_pages) == n_pages * sum(lay.tile_stride(l, h) for l in range(Lyr) for h in range(Hkv))
+    seq = torch.zeros(B, dtype=torch.int32, device="cuda")
+    done = [0] * B
+    for chunk in (100, 1, 49, 239):                       # sequence 1 stops at 150, sequence 2 never grows
+        n_app = [min(chunk, lens[b] - done[b]) for b in range(B)]
+        kk = np.zeros((Lyr, B, chunk, Hkv, d)); vv = np.zeros((Lyr, B, chunk, Hkv, d))
+        for l in range(Lyr):
+            for b in range(B):
+                kk[l, b, :n_app[b]] = probs[l][b].k_post[done[b]:done[b] + n_app[b]]
+                vv[l, b, :n_app[b]] = probs[l][b].v[done[b]:done[b] + n_app[b]]
+        assert all(n in (0, chunk) for n in n_app)
+        # one call for every layer and sequence; a sequence that is done is presented as full, so nothing is appended
+        sq = torch.tensor([done[b] if n_app[b] else table_stride * 128 for b in range(B)], dtype=torch.int32, device="cuda")
+        P.quantize_append_paged(lay, 0, cache, _cuda(kk, torch.float32), _cuda(vv, torch.float32), sq, table, n_pages,
+                                advance_seq_len=(chunk == 100), n_layers=Lyr)
+        if chunk == 100:                                  # the library advanced the lengths (and saturated the full one)
+            assert sq.tolist() == [100, 100, table_stride * 128]
+        seq = torch.tensor([done[b] + n_app[b] for b in range(B)], dtype=torch.int32, device="cuda")
+        done = [done[b] + n_app[b] for b in range(B)]
+        assert seq.tolist() == done
+    assert done == lens
+    host = cache.cpu().numpy()
+    heads = [[H.oracle_heads(probs[l][b], tab128) if lens[b] else None for b in range(B)] for l in range(Lyr)]
+    touched = set()
+    for l in range(Lyr):
+        for b in range(B):
+            if not lens[b]:
+                continue
+            n_t = (lens[b] + 127) // 128
+            for h in range(Hkv):
+                stride = lay.tile_stride(l, h)
+                pool = lay.paged_pool_offset(l, h, n_pages)
+                exp = np.zeros(n_t * stride, dtype=np.uint8)
+                O.pack_region(heads[l][b][h], d, exp)
+                for j in range(n_t):
+                    pg = int(perm[b, j])
+                    touched.add((l, h, pg))
+                    got = host[pool + pg * stride: pool + (pg + 1) * stride]
+                    assert np.array_equal(got, exp[j * stride:(j + 1) * stride]), (l, b, h, j)
+    for l in range(Lyr):                                  # pages no live tile maps to were not written
+        for h in range(Hkv):
+            stride, pool = lay.tile_stride(l, h), lay.paged_pool_offset(l, h, n_pages)
+            for pg in range(n_pages):
+                if (l, h, pg) not in touched:
+                    assert np.all(host[pool + pg * stride: pool + (pg + 1) * stride] == 0xAB)
+    scale = 1.0 / math.sqrt(d)
+    q = np.stack([np.stack([probs[l][b].q_post for b in range(B)]) for l in range(Lyr)])
+    qd = _cuda(q, torch.bfloat16)
+    out_b = P.decode_attention_paged(lay, 0, cache, qd, seq, table, n_pages, scale, lay.new_workspace(B, Lyr), n_layers=Lyr)
+    ws1 = lay.new_workspace(B, 1)
+    out_l = torch.stack([P.decode_attention_paged(lay, l, cache, qd[l].contiguous(), seq, table, n_pages, scale, ws1)
+                         for l in range(Lyr)])
+    torch.cuda.synchronize()
+    for l in range(Lyr):
+        for b in range(B):
+            for name, out in (("batched", out_b), ("per-layer", out_l)):
+                got = out[l, b].double().cpu().numpy()
+                if not lens[b]:
+                    assert np.all(got == 0.0)
+                    continue
+                exp, rv = H.oracle_attention(probs[l][b], heads[l][b], tab128, scale)
+                err = max(np.max(np.abs(got[a] - exp[a])) / rv[a // (Hq // Hkv)] for a in range(Hq))
+                assert err <= 2e-3, (name, l, b, err)
+    with pytest.raises(P.BgtqError):
+        P.decode_attention_paged(lay, 0, cache, qd[0].contiguous(), seq, table, 0, scale, ws1)
