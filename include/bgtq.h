@@ -145,6 +145,20 @@ int bgtq_decode_attention_layers(const bgtq_layout *layout, int layer0, int n_la
                                  int batch, int64_t max_tokens, float softmax_scale, void *out,
                                  void *workspace, size_t workspace_bytes, void *stream);
 
+/* ---- SURVEY.md 8(f).4 "RoPE fused into append": bgtq_quantize_append_layers on PRE-RoPE keys.
+ * k_pre [device] [n_layers, batch, n_new, n_kv_heads, d_h] of dtype dt; the token stored at cache position
+ * t is first rotated block by block (the layout's pairing):
+ *     a' = x_a * cos[t][i] - x_b * sin[t][i],   b' = x_a * sin[t][i] + x_b * cos[t][i]
+ * with rope_cos, rope_sin [device] fp32 [rope_rows, d_h/2] (rope_rows >= max_tokens, else
+ * BGTQ_ECAPACITY), evaluated in fp64 -- both products are exact, so each output is the correctly
+ * rounded value of the expression -- and quantised WITHOUT an intermediate rounding to dt (PAPER.md:122
+ * quantises post-RoPE keys; this saves the separate rotary pass and its K write + read).  V and all
+ * other arguments as for bgtq_quantize_append_layers. */
+int bgtq_quantize_append_rope(const bgtq_layout *layout, int layer0, int n_layers, void *cache,
+                              const void *k_pre, const void *v_new, int dt, int batch, int n_new,
+                              int32_t *seq_len, int advance_seq_len, int64_t max_tokens,
+                              const float *rope_cos, const float *rope_sin, int64_t rope_rows, void *stream);
+
 /* ---- SURVEY.md 8(f).4 "paged sequences": the same two calls over a PAGED cache.
  * The cache is a set of pools, one per (layer, kv head), each of n_pages pages; a page is one
  * 128-token tile of that head (bgtq_tile_stride bytes, the same tile format as the contiguous

@@ -99,6 +99,24 @@ def rope(x: np.ndarray, pos: np.ndarray, base: float, pairing: int = PAIR_HALF) 
     return out
 
 
+def rope_table(x: np.ndarray, cos: np.ndarray, sin: np.ndarray, pairing: int = PAIR_HALF) -> np.ndarray:
+    """RoPE from caller-supplied tables (the fused-append variant): x[n, heads, d_h], cos/sin
+    [n, d_h/2] -> for block i = pair (a(i), b(i)):  a' = x_a cos_i - x_b sin_i,  b' = x_a sin_i + x_b cos_i,
+    each evaluated as two fp64 products and one fp64 sum (plain numpy).  With fp32/bf16-valued x and fp32-valued
+    tables the products are exact, so every output is the correctly rounded value of its expression."""
+    x = _c64(x)
+    n, H, d = x.shape
+    cos, sin = _c64(cos), _c64(sin)
+    assert cos.shape == (n, d // 2) and sin.shape == (n, d // 2)
+    a, b = pair_indices(d, pairing)
+    out = np.empty_like(x)
+    xa, xb = x[:, :, a], x[:, :, b]
+    c, s_ = cos[:, None, :], sin[:, None, :]
+    out[:, :, a] = xa * c - xb * s_
+    out[:, :, b] = xa * s_ + xb * c
+    return out
+
+
 # ----------------------------------------------------------------------------- energy
 def block_energy(q: np.ndarray, k: np.ndarray, pairing: int = PAIR_HALF, kind: str = "qk_avg"):
     """Eq. 4 (PAPER.md:612).  q[N_q, H_q, d_h], k[N_k, H_kv, d_h] -> (s, Eq, Ek) each [H_kv, L]."""

@@ -30,6 +30,7 @@ SYMBOLS = [
     "bgtq_profile_decode_read", "bgtq_decode_attention", "bgtq_decode_attention_layers",
     "bgtq_prefill_workspace_bytes", "bgtq_prefill_attention", "bgtq_fp16_workspace_bytes", "bgtq_fp16_decode_attention", "bgtq_debug_decode_unit", "bgtq_launch_count",
     "bgtq_paged_cache_bytes", "bgtq_paged_pool_offset", "bgtq_quantize_append_paged", "bgtq_decode_attention_paged",
+    "bgtq_quantize_append_rope",
 ]
 
 
@@ -100,6 +101,8 @@ def _load() -> C.CDLL:
     lib.bgtq_paged_pool_offset.argtypes = [vp, i32, i32, i64]
     lib.bgtq_quantize_append_paged.restype = i32
     lib.bgtq_quantize_append_paged.argtypes = [vp, i32, i32, vp, vp, vp, i32, i32, i32, vp, i32, vp, i32, i64, vp]
+    lib.bgtq_quantize_append_rope.restype = i32
+    lib.bgtq_quantize_append_rope.argtypes = [vp, i32, i32, vp, vp, vp, i32, i32, i32, vp, i32, i64, vp, vp, i64, vp]
     lib.bgtq_decode_attention_paged.restype = i32
     lib.bgtq_decode_attention_paged.argtypes = [vp, i32, i32, vp, vp, vp, i32, vp, i32, i64, f32, vp, vp, sz, vp]
     return lib
@@ -252,6 +255,22 @@ def quantize_append(layout: Layout, layer: int, cache: torch.Tensor, k_new: torc
     _check(_lib.bgtq_quantize_append(layout._h, layer, _dev(cache, torch.uint8), _dev(k_new), _dev(v_new),
                                      _dt(k_new), batch, n_new, _dev(seq_len, torch.int32),
                                      1 if advance_seq_len else 0, max_tokens, _stream()))
+
+
+def quantize_append_rope(layout: Layout, layer: int, cache: torch.Tensor, k_pre: torch.Tensor, v_new: torch.Tensor,
+                         seq_len: torch.Tensor, max_tokens: int, rope_cos: torch.Tensor, rope_sin: torch.Tensor,
+                         advance_seq_len: bool = True, n_layers: int = 1) -> None:
+    """bgtq_quantize_append_rope: PRE-RoPE k_pre [batch, n_new, H_kv, d_h] (n_layers = 1) or
+    [n_layers, batch, n_new, H_kv, d_h]; rope_cos, rope_sin fp32 [rows >= max_tokens, d_h/2] (CUDA)."""
+    batch, n_new, Hkv, d = k_pre.shape[-4:]
+    assert v_new.shape == k_pre.shape and Hkv == layout.n_kv_heads and d == layout.d_h
+    assert _dt(k_pre) == _dt(v_new)
+    assert k_pre.dim() == 4 and n_layers == 1 or k_pre.dim() == 5 and k_pre.shape[0] == n_layers
+    assert rope_cos.shape == rope_sin.shape and rope_cos.dim() == 2 and rope_cos.shape[1] == d // 2
+    _check(_lib.bgtq_quantize_append_rope(layout._h, layer, n_layers, _dev(cache, torch.uint8), _dev(k_pre), _dev(v_new),
+                                          _dt(k_pre), batch, n_new, _dev(seq_len, torch.int32),
+                                          1 if advance_seq_len else 0, max_tokens, _dev(rope_cos, torch.float32),
+                                          _dev(rope_sin, torch.float32), rope_cos.shape[0], _stream()))
 
 
 def quantize_append_paged(layout: Layout, layer: int, cache: torch.Tensor, k_new: torch.Tensor,

@@ -61,7 +61,8 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
                        const T *__restrict__ k_new, const T *__restrict__ v_new,
                        const double *__restrict__ cb64, const float *__restrict__ rot_t, int batch,
                        int n_new, int Hkv, const int32_t *__restrict__ seq_len, int64_t n_cap,
-                       int64_t max_tokens, const int32_t *__restrict__ pages, int pstride, int64_t n_pages)
+                       int64_t max_tokens, const int32_t *__restrict__ pages, int pstride, int64_t n_pages,
+                       const float *__restrict__ rope_cos, const float *__restrict__ rope_sin, int pairing)
 {
     extern __shared__ __align__(16) unsigned char smem[];
     const int tid = threadIdx.x;
@@ -137,7 +138,22 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
             if (tok >= nlo && tok < nhi) {
                 int64_t row = ((((int64_t)lrel * batch + s) * n_new + (tok - t0)) * Hkv + h) * kDh;
                 if (c >= 128) v = to_f64(v_new[row + (c - 128)]);
-                else if (c < kdim) v = to_f64(k_new[row + M.coords[c]]);
+                else if (c < kdim) {
+                    const int o = M.coords[c];
+                    v = to_f64(k_new[row + o]);
+                    if (rope_cos) {
+                        // fused RoPE: block i = pair (a, b); a' = x_a cos - x_b sin, b' = x_a sin + x_b cos
+                        // at position tok.  Inputs and table entries have <= 24-bit significands, so both products
+                        // are exact in fp64 and each output is the correctly rounded value of the exact expression.
+                        constexpr int L = kDh / 2;
+                        const bool half = pairing == BGTQ_PAIR_HALF;
+                        const int i = half ? (o & (L - 1)) : (o >> 1);
+                        const bool is_b = half ? (o >= L) : (o & 1);
+                        const double xp = to_f64(k_new[row + (half ? (o ^ L) : (o ^ 1))]);
+                        const double cs = (double)__ldg(rope_cos + tok * L + i), sn = (double)__ldg(rope_sin + tok * L + i);
+                        v = is_b ? __dadd_rn(__dmul_rn(xp, sn), __dmul_rn(v, cs)) : __dadd_rn(__dmul_rn(v, cs), -__dmul_rn(xp, sn));
+                    }
+                }
             }
             xs[e] = v;
         }
@@ -290,7 +306,7 @@ static size_t append_smem_bytes(int max_stride)
 
 int launch_quantize_append(const bgtq_layout *lay, int layer, int n_layers, void *cache, const void *k_new,
                            const void *v_new, int dt, int batch, int n_new, int32_t *seq_len,
-                           int advance, int64_t max_tokens, const PageMap *pm, cudaStream_t st)
+                           int advance, int64_t max_tokens, const PageMap *pm, const RopeTab *rope, cudaStream_t st)
 {
     static bool attr_set = false;
     const int64_t n_cap = (max_tokens + kTile - 1) / kTile;
@@ -307,12 +323,12 @@ int launch_quantize_append(const bgtq_layout *lay, int layer, int n_layers, void
         quantize_append_kernel<float><<<grid, kAppendThreads, smem, st>>>(
             metas, (uint8_t *)cache, (const float *)k_new, (const float *)v_new, lay->d_cb64, lay->d_rot_t,
             batch, n_new, lay->n_kv_heads, seq_len, n_cap, n_cap * kTile, pm ? pm->table : nullptr,
-            pm ? pm->table_stride : 0, pm ? pm->n_pages : 0);
+            pm ? pm->table_stride : 0, pm ? pm->n_pages : 0, rope ? rope->cos : nullptr, rope ? rope->sin : nullptr, lay->pairing);
     } else {
         quantize_append_kernel<__nv_bfloat16><<<grid, kAppendThreads, smem, st>>>(
             metas, (uint8_t *)cache, (const __nv_bfloat16 *)k_new, (const __nv_bfloat16 *)v_new, lay->d_cb64,
             lay->d_rot_t, batch, n_new, lay->n_kv_heads, seq_len, n_cap, n_cap * kTile, pm ? pm->table : nullptr,
-            pm ? pm->table_stride : 0, pm ? pm->n_pages : 0);
+            pm ? pm->table_stride : 0, pm ? pm->n_pages : 0, rope ? rope->cos : nullptr, rope ? rope->sin : nullptr, lay->pairing);
     }
     count_launch();
     CUDA_TRY(cudaGetLastError());

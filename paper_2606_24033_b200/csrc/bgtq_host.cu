@@ -295,7 +295,27 @@ extern "C" int bgtq_quantize_append_layers(const bgtq_layout *lay, int layer0, i
     if (n_new == 0) return BGTQ_OK;
     if (!k_new || !v_new) FAIL(BGTQ_EINVAL, "bgtq_quantize_append: null k_new/v_new");
     return launch_quantize_append(lay, layer0, n_layers, cache, k_new, v_new, dt, batch, n_new, seq_len,
-                                  advance_seq_len, max_tokens, nullptr, (cudaStream_t)stream);
+                                  advance_seq_len, max_tokens, nullptr, nullptr, (cudaStream_t)stream);
+}
+
+// ------------------------------------------------------------------ RoPE fused into append
+extern "C" int bgtq_quantize_append_rope(const bgtq_layout *lay, int layer0, int n_layers, void *cache,
+                                         const void *k_pre, const void *v_new, int dt, int batch, int n_new,
+                                         int32_t *seq_len, int advance_seq_len, int64_t max_tokens,
+                                         const float *rope_cos, const float *rope_sin, int64_t rope_rows, void *stream)
+{
+    if (!lay || !cache || !seq_len || !rope_cos || !rope_sin) FAIL(BGTQ_EINVAL, "bgtq_quantize_append_rope: null pointer");
+    if (layer0 < 0 || n_layers <= 0 || layer0 + n_layers > lay->n_layers) FAIL(BGTQ_EINVAL, "bgtq_quantize_append_rope: layer out of range");
+    if (dt != BGTQ_F32 && dt != BGTQ_BF16) FAIL(BGTQ_EINVAL, "bgtq_quantize_append_rope: dtype");
+    if (batch <= 0 || n_new < 0 || max_tokens <= 0) FAIL(BGTQ_EINVAL, "bgtq_quantize_append_rope: batch/n_new/max_tokens");
+    if (batch > 65535 || (int64_t)n_layers * lay->n_kv_heads > 65535) FAIL(BGTQ_EINVAL, "bgtq_quantize_append_rope: batch or layers*heads > 65535");
+    if (n_new > max_tokens) FAIL(BGTQ_ECAPACITY, "bgtq_quantize_append_rope: n_new exceeds max_tokens");
+    if (rope_rows < max_tokens) FAIL(BGTQ_ECAPACITY, "bgtq_quantize_append_rope: cos/sin tables have fewer rows than max_tokens");
+    if (n_new == 0) return BGTQ_OK;
+    if (!k_pre || !v_new) FAIL(BGTQ_EINVAL, "bgtq_quantize_append_rope: null k_pre/v_new");
+    const RopeTab rt{rope_cos, rope_sin};
+    return launch_quantize_append(lay, layer0, n_layers, cache, k_pre, v_new, dt, batch, n_new, seq_len,
+                                  advance_seq_len, max_tokens, nullptr, &rt, (cudaStream_t)stream);
 }
 
 // ------------------------------------------------------------------ paged cache
@@ -326,7 +346,7 @@ extern "C" int bgtq_quantize_append_paged(const bgtq_layout *lay, int layer0, in
     if (!k_new || !v_new) FAIL(BGTQ_EINVAL, "bgtq_quantize_append_paged: null k_new/v_new");
     const PageMap pm{page_table, table_stride, n_pages};
     return launch_quantize_append(lay, layer0, n_layers, cache, k_new, v_new, dt, batch, n_new, seq_len,
-                                  advance_seq_len, max_tokens, &pm, (cudaStream_t)stream);
+                                  advance_seq_len, max_tokens, &pm, nullptr, (cudaStream_t)stream);
 }
 extern "C" int bgtq_decode_attention_paged(const bgtq_layout *lay, int layer0, int n_layers, const void *cache,
                                            const void *q, const int32_t *seq_len, int batch,

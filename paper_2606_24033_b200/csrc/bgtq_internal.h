@@ -77,6 +77,11 @@ struct PageMap {
     int64_t n_pages;
 };
 
+// RoPE fused into append (bgtq_quantize_append_rope): fp32 tables [rows][d_h/2], row = token position
+struct RopeTab {
+    const float *cos, *sin;
+};
+
 // implemented in the .cu files
 int launch_block_energy(const void *q, int64_t n_q, const void *k, int64_t n_k, int dt, int Hq,
                         int Hkv, int d_h, int pairing, int kind, float *scores, float *eq_out,
@@ -86,7 +91,7 @@ int launch_allocate(const float *scores, int n_heads, int L, int b_min, int b_ma
                     uint8_t *bits, cudaStream_t st);
 int launch_quantize_append(const bgtq_layout *lay, int layer, int n_layers, void *cache, const void *k_new,
                            const void *v_new, int dt, int batch, int n_new, int32_t *seq_len,
-                           int advance, int64_t max_tokens, const PageMap *pm, cudaStream_t st);
+                           int advance, int64_t max_tokens, const PageMap *pm, const RopeTab *rope, cudaStream_t st);
 int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *cache,
                   const void *q, const int32_t *seq_len, int batch, int64_t max_tokens,
                   float scale, void *out, void *ws, size_t ws_bytes, const PageMap *pm, cudaStream_t st);

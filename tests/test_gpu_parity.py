@@ -528,3 +528,51 @@ def test_paged_cache_append_and_attention(P, tab128):
                 assert err <= 2e-3, (name, l, b, err)
     with pytest.raises(P.BgtqError):
         P.decode_attention_paged(lay, 0, cache, qd[0].contiguous(), seq, table, 0, scale, ws1)
+
+
+@pytest.mark.parametrize("kv_dtype,pairing", [("f32", 0), ("bf16", 0), ("bf16", 1)])
+def test_append_with_fused_rope_bit_exact(P, tab128, kv_dtype, pairing):
+    """bgtq_quantize_append_rope on PRE-RoPE keys == oracle rope_table (fp64, no intermediate
+    rounding) -> quantise -> pack, byte for byte; two layers in one call, ragged chunks, both pairings."""
+    import workloads as W
+    Lyr, B, Hq, Hkv, d, T, max_tokens = 2, 1, 8, 2, 128, 300, 384
+    L = d // 2
+    rng = np.random.default_rng(3)
+    base = 1.0e6
+    ang = np.arange(max_tokens, dtype=np.float64)[:, None] * base ** (-2.0 * np.arange(L) / d)[None, :]
+    cos32, sin32 = np.cos(ang).astype(np.float32), np.sin(ang).astype(np.float32)
+    probs, k_pre = [], []
+    for l in range(Lyr):
+        p = H.make_problem(300 + l, T, Hq, Hkv, 3, 3, 1, 8, rope_base=base, kv_dtype=kv_dtype)
+        scales = W.block_scales(300 + l, Hkv, L)
+        kp = W.pre_rope_gaussian(300 + l, 1, T, Hkv, d, scales)
+        kp = W.round_to_bf16(kp).astype(np.float64) if kv_dtype == "bf16" else kp.astype(np.float32).astype(np.float64)
+        p.k_post = O.rope_table(kp, cos32[:T].astype(np.float64), sin32[:T].astype(np.float64), pairing)
+        if pairing == 1:                                   # allocation per interleaved block: any valid bits will do
+            p.bits = np.stack([rng.permutation(p.bits[h]) for h in range(Hkv)])
+        probs.append(p); k_pre.append(kp)
+    bits = np.stack([p.bits for p in probs])
+    lay = P.Layout(bits, Hq, d, 3, probs[0].rot, pairing=pairing)
+    cache = lay.new_cache(B, max_tokens)
+    seq = torch.zeros(B, dtype=torch.int32, device="cuda")
+    tdt = torch.float32 if kv_dtype == "f32" else torch.bfloat16
+    cs, sn = torch.from_numpy(cos32).cuda(), torch.from_numpy(sin32).cuda()
+    t = 0
+    for n in (130, 1, 169):
+        k = _cuda(np.stack([k_pre[l][None, t:t + n] for l in range(Lyr)]), tdt)
+        v = _cuda(np.stack([probs[l].v[None, t:t + n] for l in range(Lyr)]), tdt)
+        P.quantize_append_rope(lay, 0, cache, k, v, seq, max_tokens, cs, sn, n_layers=Lyr)
+        t += n
+    assert int(seq.item()) == T
+    host = cache.cpu().numpy()
+    n_cap = max_tokens // 128
+    for l in range(Lyr):
+        heads = [O.quantize_head(probs[l].k_post[:, h], probs[l].v[:, h], probs[l].bits[h], 3, tab128, pairing=pairing)
+                 for h in range(Hkv)]
+        for h in range(Hkv):
+            stride, off = lay.tile_stride(l, h), lay.region_offset(l, 0, h, B, max_tokens)
+            exp = np.zeros(n_cap * stride, dtype=np.uint8)
+            O.pack_region(heads[h], d, exp)
+            assert np.array_equal(host[off:off + n_cap * stride], exp), (l, h)
+    with pytest.raises(P.BgtqError):                       # tables shorter than the capacity
+        P.quantize_append_rope(lay, 0, cache, k, v, seq, max_tokens, cs[:100].contiguous(), sn[:100].contiguous(), n_layers=Lyr)

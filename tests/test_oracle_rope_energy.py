@@ -117,3 +117,31 @@ def test_energy_generator_closed_form_and_amgm():
     kr = O.rope(k, np.arange(n, dtype=np.float64), 1e4, 0)
     s2, _, _ = O.block_energy(q, kr, 0)
     assert np.allclose(s2, s, rtol=1e-10)
+
+
+@pytest.mark.parametrize("pairing", [0, 1])
+def test_rope_table_pins(pairing):
+    """rope_table (fused-append variant) == rope when handed rope's own angles; hand values; exactness on fp32 data."""
+    rng = np.random.default_rng(11)
+    d, base = 128, 1.0e6
+    x = rng.standard_normal((7, 2, d))
+    pos = np.array([0.0, 1.0, 2.0, 77.0, 4095.0, 65536.0, 131071.0])
+    ang = pos[:, None] * base ** (-2.0 * np.arange(d // 2) / d)[None, :]
+    assert np.allclose(O.rope_table(x, np.cos(ang), np.sin(ang), pairing), O.rope(x, pos, base, pairing), rtol=0, atol=1e-9)   # 1-ulp angle differences x 131071
+    # quarter turn of block 3: (x_a, x_b) = (1, 0) -> (0, 1), (0, 1) -> (-1, 0): counter-clockwise (Q2)
+    a, b = O.pair_indices(d, pairing)
+    e = np.zeros((2, 1, d)); e[0, 0, a[3]] = 1.0; e[1, 0, b[3]] = 1.0
+    c = np.ones((2, d // 2)); s = np.zeros((2, d // 2)); c[:, 3] = 0.0; s[:, 3] = 1.0
+    out = O.rope_table(e, c, s, pairing)
+    assert out[0, 0, a[3]] == 0.0 and out[0, 0, b[3]] == 1.0 and out[1, 0, a[3]] == -1.0 and out[1, 0, b[3]] == 0.0
+    assert np.count_nonzero(out) == 2
+    # fp32 inputs and tables: the result is the correctly rounded exact value (checked with exact rationals)
+    from fractions import Fraction
+    xf = rng.standard_normal((1, 1, d)).astype(np.float32).astype(np.float64)
+    cf = np.cos(ang[3:4]).astype(np.float32).astype(np.float64); sf = np.sin(ang[3:4]).astype(np.float32).astype(np.float64)
+    got = O.rope_table(xf, cf, sf, pairing)
+    for i in (0, 5, 63):
+        exact = Fraction(xf[0, 0, a[i]]) * Fraction(cf[0, i]) - Fraction(xf[0, 0, b[i]]) * Fraction(sf[0, i])
+        assert got[0, 0, a[i]] == float(exact)                 # float(Fraction) rounds to nearest even
+        exact = Fraction(xf[0, 0, a[i]]) * Fraction(sf[0, i]) + Fraction(xf[0, 0, b[i]]) * Fraction(cf[0, i])
+        assert got[0, 0, b[i]] == float(exact)
