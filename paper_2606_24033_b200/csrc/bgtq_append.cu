@@ -55,7 +55,7 @@ __device__ __forceinline__ void put_field(uint32_t *base, int wstride, int b, in
 __device__ __forceinline__ double to_f64(float v) { return (double)v; }
 __device__ __forceinline__ double to_f64(__nv_bfloat16 v) { return (double)__bfloat162float(v); }
 
-template <typename T>
+template <typename T, bool ROPE, bool PAGED>
 __global__ void __launch_bounds__(kAppendThreads)
 quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__ cache,
                        const T *__restrict__ k_new, const T *__restrict__ v_new,
@@ -86,7 +86,7 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
     int *n_units_p = reinterpret_cast<int *>(units + kMaxUnits);
     uint32_t *tbuf = reinterpret_cast<uint32_t *>(n_units_p + 4);        // tile, `stride` bytes
 
-    uint8_t *gtile = pages ? cache + n_pages * ((int64_t)M.layer_prefix + M.head_prefix) + (int64_t)pages[(int64_t)s * pstride + tile] * stride
+    uint8_t *gtile = PAGED ? cache + n_pages * ((int64_t)M.layer_prefix + M.head_prefix) + (int64_t)pages[(int64_t)s * pstride + tile] * stride
                            : cache + n_cap * ((int64_t)batch * M.layer_prefix + (int64_t)s * M.layer_sum + M.head_prefix) + tile * stride;
     {   // stage the tile: older tokens present -> load, else start from zeros
         const bool has_old = tile_lo < t0;
@@ -141,7 +141,7 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
                 else if (c < kdim) {
                     const int o = M.coords[c];
                     v = to_f64(k_new[row + o]);
-                    if (rope_cos) {
+                    if constexpr (ROPE) {
                         // fused RoPE: block i = pair (a, b); a' = x_a cos - x_b sin, b' = x_a sin + x_b cos
                         // at position tok.  Inputs and table entries have <= 24-bit significands, so both products
                         // are exact in fp64 and each output is the correctly rounded value of the exact expression.
@@ -315,21 +315,31 @@ int launch_quantize_append(const bgtq_layout *lay, int layer, int n_layers, void
     const HeadMeta *metas = lay->d_meta + (size_t)layer * lay->n_kv_heads;
     if (!attr_set) {   // once per process, outside any stream capture
         const int maxs = (int)append_smem_bytes(16 * kDh * 8 + 256 * 9 + 16 * kDh * 8);
-        CUDA_TRY(cudaFuncSetAttribute(quantize_append_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, maxs));
-        CUDA_TRY(cudaFuncSetAttribute(quantize_append_kernel<__nv_bfloat16>, cudaFuncAttributeMaxDynamicSharedMemorySize, maxs));
+#define BGTQ_APPEND_ATTR(T, R, G) CUDA_TRY(cudaFuncSetAttribute(quantize_append_kernel<T, R, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, maxs))
+        BGTQ_APPEND_ATTR(float, false, false); BGTQ_APPEND_ATTR(__nv_bfloat16, false, false);
+        BGTQ_APPEND_ATTR(float, true, false);  BGTQ_APPEND_ATTR(__nv_bfloat16, true, false);
+        BGTQ_APPEND_ATTR(float, false, true);  BGTQ_APPEND_ATTR(__nv_bfloat16, false, true);
+#undef BGTQ_APPEND_ATTR
         attr_set = true;
     }
-    if (dt == BGTQ_F32) {
-        quantize_append_kernel<float><<<grid, kAppendThreads, smem, st>>>(
-            metas, (uint8_t *)cache, (const float *)k_new, (const float *)v_new, lay->d_cb64, lay->d_rot_t,
-            batch, n_new, lay->n_kv_heads, seq_len, n_cap, n_cap * kTile, pm ? pm->table : nullptr,
-            pm ? pm->table_stride : 0, pm ? pm->n_pages : 0, rope ? rope->cos : nullptr, rope ? rope->sin : nullptr, lay->pairing);
-    } else {
-        quantize_append_kernel<__nv_bfloat16><<<grid, kAppendThreads, smem, st>>>(
-            metas, (uint8_t *)cache, (const __nv_bfloat16 *)k_new, (const __nv_bfloat16 *)v_new, lay->d_cb64,
-            lay->d_rot_t, batch, n_new, lay->n_kv_heads, seq_len, n_cap, n_cap * kTile, pm ? pm->table : nullptr,
-            pm ? pm->table_stride : 0, pm ? pm->n_pages : 0, rope ? rope->cos : nullptr, rope ? rope->sin : nullptr, lay->pairing);
-    }
+    const int32_t *pt = pm ? pm->table : nullptr;
+    const int pstride = pm ? pm->table_stride : 0;
+    const int64_t n_pages = pm ? pm->n_pages : 0;
+    const float *rc = rope ? rope->cos : nullptr, *rs = rope ? rope->sin : nullptr;
+    // (a runtime `pages ? :` in the kernel costs 30 % of the bulk append rate, hence the template switch)
+    if (pm && rope) { set_error("bgtq_quantize_append: paged + fused RoPE is not built"); return BGTQ_EINVAL; }
+    auto launch = [&](auto plain, auto roped, auto paged, auto *kp, auto *vp) {
+        auto kern = pm ? paged : (rope ? roped : plain);
+        kern<<<grid, kAppendThreads, smem, st>>>(metas, (uint8_t *)cache, kp, vp, lay->d_cb64, lay->d_rot_t, batch, n_new,
+                                                 lay->n_kv_heads, seq_len, n_cap, n_cap * kTile, pt, pstride, n_pages, rc, rs,
+                                                 lay->pairing);
+    };
+    if (dt == BGTQ_F32)
+        launch(quantize_append_kernel<float, false, false>, quantize_append_kernel<float, true, false>,
+               quantize_append_kernel<float, false, true>, (const float *)k_new, (const float *)v_new);
+    else
+        launch(quantize_append_kernel<__nv_bfloat16, false, false>, quantize_append_kernel<__nv_bfloat16, true, false>,
+               quantize_append_kernel<__nv_bfloat16, false, true>, (const __nv_bfloat16 *)k_new, (const __nv_bfloat16 *)v_new);
     count_launch();
     CUDA_TRY(cudaGetLastError());
     if (advance) {
