@@ -208,11 +208,14 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
                     float pf[4];
 #pragma unroll
                     for (int u = 0; u < 4; ++u) pf[u] = __ldg(myrot + (size_t)(k + u) * my_m);
+                    const double p0 = (double)pf[0], p1 = (double)pf[1], p2 = (double)pf[2], p3 = (double)pf[3];
+                    // x[tt][k..k+3] as two 16-byte loads (group starts are even and k is a multiple of 4, so the
+                    // address is 16-byte aligned); per token the chain still runs over k in ascending order
 #pragma unroll
-                    for (int u = 0; u < 4; ++u) {
-                        const double pi = (double)pf[u];
-#pragma unroll
-                        for (int tt = 0; tt < kSub; ++tt) z[tt] = __fma_rn(pi, x[tt * 256 + k + u], z[tt]);
+                    for (int tt = 0; tt < kSub; ++tt) {
+                        const double2 xa = *reinterpret_cast<const double2 *>(x + tt * 256 + k);
+                        const double2 xb = *reinterpret_cast<const double2 *>(x + tt * 256 + k + 2);
+                        z[tt] = __fma_rn(p3, xb.y, __fma_rn(p2, xb.x, __fma_rn(p1, xa.y, __fma_rn(p0, xa.x, z[tt]))));
                     }
                 }
                 for (; k < my_m; ++k) {
