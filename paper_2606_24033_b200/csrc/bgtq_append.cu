@@ -56,7 +56,7 @@ __device__ __forceinline__ double to_f64(float v) { return (double)v; }
 __device__ __forceinline__ double to_f64(__nv_bfloat16 v) { return (double)__bfloat162float(v); }
 
 template <typename T, bool ROPE, bool PAGED>
-__global__ void __launch_bounds__(kAppendThreads)
+__global__ void __launch_bounds__(kAppendThreads, 4)
 quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__ cache,
                        const T *__restrict__ k_new, const T *__restrict__ v_new,
                        const double *__restrict__ cb64, const float *__restrict__ rot_t, int batch,
@@ -125,37 +125,48 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
         my_m = M.gm[g]; my_r = col - M.gstart[g]; my_x0 = M.gstart[g]; my_g = g; my_b = M.gb[g];
     }
     const float *myrot = rot_t + rot_offset(my_m > 0 ? my_m : 2) + my_r;
+    // gather source of column `col`: V coordinate col-128, or the K coordinate stored at grouped position col
+    const T *g_src = col >= 128 ? v_new : k_new;
+    const int g_off = col >= 128 ? col - 128 : (col < kdim ? (int)M.coords[col] : -1);
+    int g_part = -1, g_blk = 0;
+    bool g_isb = false;
+    if (ROPE && col < kdim) {               // RoPE partner of this K coordinate, its block and which member it is
+        const bool half = pairing == BGTQ_PAIR_HALF;
+        g_blk = half ? (g_off & (kDh / 2 - 1)) : (g_off >> 1);
+        g_isb = half ? (g_off >= kDh / 2) : (g_off & 1);
+        g_part = half ? (g_off ^ (kDh / 2)) : (g_off ^ 1);
+    }
 
     for (int i = 0; i < kTile / kSub; ++i) {
         const int64_t base = tile_lo + i * kSub;
         const int64_t nlo = max(lo, base), nhi = min(hi, base + kSub);
         if (nlo >= nhi) continue;
-        // ---- 1. gather the sub-batch: xs[tt][0..127] = K in grouped order, xs[tt][128..255] = V
-        for (int e = tid; e < kSub * 256; e += kAppendThreads) {
-            int tt = e >> 8, c = e & 255;
-            int64_t tok = base + tt;
-            double v = 0.0;
-            if (tok >= nlo && tok < nhi) {
-                int64_t row = ((((int64_t)lrel * batch + s) * n_new + (tok - t0)) * Hkv + h) * kDh;
-                if (c >= 128) v = to_f64(v_new[row + (c - 128)]);
-                else if (c < kdim) {
-                    const int o = M.coords[c];
-                    v = to_f64(k_new[row + o]);
+        // ---- 1. gather the sub-batch: xs[tt][0..127] = K in grouped order, xs[tt][128..255] = V.  Thread c owns
+        //      column c (its source coordinate is fixed), so the kSub loads are independent and in flight together.
+        {
+            const int64_t row0 = ((((int64_t)lrel * batch + s) * n_new + (base - t0)) * Hkv + h) * kDh;
+            const int64_t rstep = (int64_t)Hkv * kDh;
+#pragma unroll 4
+            for (int tt = 0; tt < kSub; ++tt) {
+                const int64_t tok = base + tt;
+                double v = 0.0;
+                if (tok >= nlo && tok < nhi && g_off >= 0) {
+                    const int64_t row = row0 + tt * rstep;
+                    v = to_f64(g_src[row + g_off]);
                     if constexpr (ROPE) {
                         // fused RoPE: block i = pair (a, b); a' = x_a cos - x_b sin, b' = x_a sin + x_b cos
                         // at position tok.  Inputs and table entries have <= 24-bit significands, so both products
                         // are exact in fp64 and each output is the correctly rounded value of the exact expression.
-                        constexpr int L = kDh / 2;
-                        const bool half = pairing == BGTQ_PAIR_HALF;
-                        const int i = half ? (o & (L - 1)) : (o >> 1);
-                        const bool is_b = half ? (o >= L) : (o & 1);
-                        const double xp = to_f64(k_new[row + (half ? (o ^ L) : (o ^ 1))]);
-                        const double cs = (double)__ldg(rope_cos + tok * L + i), sn = (double)__ldg(rope_sin + tok * L + i);
-                        v = is_b ? __dadd_rn(__dmul_rn(xp, sn), __dmul_rn(v, cs)) : __dadd_rn(__dmul_rn(v, cs), -__dmul_rn(xp, sn));
+                        if (g_part >= 0) {
+                            const double xp = to_f64(k_new[row + g_part]);
+                            const double cs = (double)__ldg(rope_cos + tok * (kDh / 2) + g_blk);
+                            const double sn = (double)__ldg(rope_sin + tok * (kDh / 2) + g_blk);
+                            v = g_isb ? __dadd_rn(__dmul_rn(xp, sn), __dmul_rn(v, cs)) : __dadd_rn(__dmul_rn(v, cs), -__dmul_rn(xp, sn));
+                        }
                     }
                 }
+                xs[tt * 256 + tid] = v;
             }
-            xs[e] = v;
         }
         __syncthreads();
         // ---- 2. radii: ss = fma chain, r = sqrt(ss), sigma = r / sqrt(m), h = fp16_rne_sat(r)
@@ -204,6 +215,29 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
                 for (int tt = 0; tt < kSub; ++tt) if (tt == tt_lo) z[tt] = zz;
             } else {
                 int k = 0;
+                // blocks of 4 rotation entries, the next block's loads issued before this block's 64 chained FMAs:
+                // the table is an L2 hit (4 CTAs x 56 KB leave little L1), so its latency has to be covered
+                const int kend4 = my_m & ~3;
+                float pc[4];
+                if (kend4 > 0) {
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) pc[u] = __ldg(myrot + (size_t)u * my_m);
+                }
+                for (; k < kend4; k += 4) {
+                    float pn[4];
+                    const int kn = k + 4 < kend4 ? k + 4 : k;           // (the last block re-reads itself: no branch)
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) pn[u] = __ldg(myrot + (size_t)(kn + u) * my_m);
+                    const double p0 = (double)pc[0], p1 = (double)pc[1], p2 = (double)pc[2], p3 = (double)pc[3];
+#pragma unroll
+                    for (int tt = 0; tt < kSub; ++tt) {
+                        const double2 xa = *reinterpret_cast<const double2 *>(x + tt * 256 + k);
+                        const double2 xb = *reinterpret_cast<const double2 *>(x + tt * 256 + k + 2);
+                        z[tt] = __fma_rn(p3, xb.y, __fma_rn(p2, xb.x, __fma_rn(p1, xa.y, __fma_rn(p0, xa.x, z[tt]))));
+                    }
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) pc[u] = pn[u];
+                }
                 for (; k + 4 <= my_m; k += 4) {
                     float pf[4];
 #pragma unroll
@@ -229,17 +263,34 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
         // ---- 4. scalar quantise: idx = #{k : z > tau_k * sigma}; the predicate is monotone in k
         if (my_m > 0) {
             const double *tb = tau + ((1 << my_b) - 1);
-            const int nthr = (1 << my_b) - 1;
+            // the count is found bit by bit (always my_b probes), all kSub searches side by side so that the
+            // dependent LDS -> DMUL -> DSETP chains of different tokens overlap; same count as any other search
+            // because the predicate is monotone in k
+            const double *sgp = sigma + my_g;
+            if (tt_hi - tt_lo == 1) {                         // decode-time append: one token, one search
+                double zz = 0.0;
 #pragma unroll
-            for (int tt = 0; tt < kSub; ++tt) {
-                if (tt < tt_lo || tt >= tt_hi) continue;
-                double sg = sigma[tt * 9 + my_g];
-                int a = 0, c = nthr;
-                while (a < c) {
-                    int mid = (a + c) >> 1;
-                    if (z[tt] > __dmul_rn(tb[mid], sg)) a = mid + 1; else c = mid;
+                for (int tt = 0; tt < kSub; ++tt) if (tt == tt_lo) zz = z[tt];
+                const double sg = sgp[tt_lo * 9];
+                int a = 0;
+                for (int bit = my_b - 1; bit >= 0; --bit)
+                    if (zz > __dmul_rn(tb[a + (1 << bit) - 1], sg)) a += 1 << bit;
+                idxs[tt_lo * 256 + col] = (uint8_t)a;
+            } else
+#pragma unroll
+            for (int t0h = 0; t0h < kSub; t0h += 8) {         // 8 searches side by side (register budget: 64)
+                int a[8];
+#pragma unroll
+                for (int tt = 0; tt < 8; ++tt) a[tt] = 0;
+                for (int bit = my_b - 1; bit >= 0; --bit) {
+                    const int step = 1 << bit;
+#pragma unroll
+                    for (int tt = 0; tt < 8; ++tt)
+                        if (z[t0h + tt] > __dmul_rn(tb[a[tt] + step - 1], sgp[(t0h + tt) * 9])) a[tt] += step;
                 }
-                idxs[tt * 256 + col] = (uint8_t)a;
+#pragma unroll
+                for (int tt = 0; tt < 8; ++tt)
+                    if (t0h + tt >= tt_lo && t0h + tt < tt_hi) idxs[(t0h + tt) * 256 + col] = (uint8_t)a[tt];
             }
         }
         __syncthreads();
