@@ -1395,7 +1395,18 @@ struct PrefillParams {
 
 struct PUnit { int off, b, nc, ustart, group; };
 
-template <int B>
+// Shared-memory layouts of the unpacked fp16 tiles [row][k] (row = token for K^, dim for V^T):
+//   UMMA = false: 256-byte rows, 16-byte chunks XOR-swizzled with (row & 7)              (ldmatrix path)
+//   UMMA = true : the tcgen05 K-major SWIZZLE_128B operand layout: two [128 x 64] blocks of 16 KB, 128-byte rows,
+//                 chunk ^ (row & 7); 8-row groups 1024 B apart (the SBO of the descriptor)
+template <bool UMMA>
+__device__ __forceinline__ int tile_off(int row, int k)
+{
+    if (UMMA) return (k >> 6) * 16384 + row * 128 + (((((k & 63) >> 3) ^ (row & 7)) << 4) | ((k & 7) << 1));
+    return row * 256 + ((((k >> 3) ^ (row & 7)) << 4) | ((k & 7) << 1));
+}
+
+template <int B, bool UMMA = false>
 __device__ __forceinline__ void prefill_decode_k(const uint32_t *raw, const PUnit &U, int lane, const uint32_t *pools,
                                                  const uint16_t *lut, const __half *kn, unsigned char *khat)
 {
@@ -1405,7 +1416,7 @@ __device__ __forceinline__ void prefill_decode_k(const uint32_t *raw, const PUni
     else load_unit_partial<B>(raw + (U.off >> 2), g8, c, U.nc, w);
     decode_unit<B, true>(w, pools, lut, h);
     if (c < U.nc) {
-        const int col = U.ustart + 2 * c, chunk = col >> 3;
+        const int col = U.ustart + 2 * c;
 #pragma unroll
         for (int i = 0; i < 8; ++i)
 #pragma unroll
@@ -1413,12 +1424,12 @@ __device__ __forceinline__ void prefill_decode_k(const uint32_t *raw, const PUni
                 const int tok = 16 * i + 8 * p + g8;
                 const uint32_t n2 = (uint32_t)__half_as_ushort(kn[U.group * 128 + tok]) * 0x10001u;
                 const uint32_t v = hmul2_u(h[2 * i + p], n2);
-                *reinterpret_cast<uint32_t *>(khat + tok * 256 + ((chunk ^ (tok & 7)) << 4) + (col & 7) * 2) = v;
+                *reinterpret_cast<uint32_t *>(khat + tile_off<UMMA>(tok, col)) = v;
             }
     }
 }
 
-template <int B>
+template <int B, bool UMMA = false>
 __device__ __forceinline__ void prefill_decode_v(const uint32_t *vcodes, int J, int lane, const uint32_t *pools,
                                                  const uint16_t *lut, const __half *vn, unsigned char *vhat_t)
 {
@@ -1436,8 +1447,7 @@ __device__ __forceinline__ void prefill_decode_v(const uint32_t *vcodes, int J, 
                 const int tok = 16 * kp + 8 * o + 2 * c;                       // tokens tok, tok+1
                 const uint32_t n2 = *reinterpret_cast<const uint32_t *>(vn + tok);
                 const uint32_t v = hmul2_u(h[2 * kp + o], n2);
-                const int chunk = tok >> 3;
-                *reinterpret_cast<uint32_t *>(vhat_t + dim * 256 + ((chunk ^ (dim & 7)) << 4) + (tok & 7) * 2) = v;
+                *reinterpret_cast<uint32_t *>(vhat_t + tile_off<UMMA>(dim, tok)) = v;
             }
     }
 }
@@ -1671,6 +1681,280 @@ prefill_kernel(const PrefillParams P)
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 128;" :: "r"(tmem_base_s) : "memory");
 }
 
+// ---------------------------------------------------------------- prefill on the 5th-generation tensor cores
+// Same problem and interface as prefill_kernel, but both contractions run as tcgen05.mma (kind::f16, fp32 accumulators in
+// tensor memory), issued by one thread.  A CTA owns 128 query rows (128/G tokens x G heads of one KV head):
+//   shared memory: Q' [128 rows x 128 coords], K^ [128 tokens x 128 coords], V^T [128 dims x 128 tokens] and
+//                  P [128 rows x 128 tokens], all fp16 in the K-major SWIZZLE_128B operand layout (two 16 KB blocks each),
+//                  + the raw packed tile (TMA bulk copy);
+//   tensor memory: S = Q' K^T in columns [0,128), O in columns [128,256); row r of S / O is TMEM lane r.
+// Per 128-token tile: all 8 warps unpack K^ -> S MMA (async) -> unpack V^T while it runs -> softmax straight out of TMEM
+// (thread = one row x 64 columns: no shuffles; the two column halves meet through shared memory) -> P to shared memory,
+// O rescaled in TMEM when a row maximum moved -> PV MMA (async), which overlaps the next tile's K^ unpack.
+__device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t saddr)
+{
+    // K-major SWIZZLE_128B shared-memory operand: start address >> 4 in bits [0,14); leading byte offset (not used by
+    // swizzled K-major layouts) = 1 in [16,30); stride byte offset = 1024 B (8 rows x 128 B) >> 4 in [32,46);
+    // descriptor version 1 (sm_100) in [46,48); layout type 2 = SWIZZLE_128B in [61,64)
+    return (uint64_t)((saddr & 0x3FFFF) >> 4) | ((uint64_t)1 << 16) | ((uint64_t)(1024 >> 4) << 32) |
+           ((uint64_t)1 << 46) | ((uint64_t)2 << 61);
+}
+__device__ __forceinline__ void umma_f16_ss(uint32_t d_tmem, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+                 :: "r"(d_tmem), "l"(da), "l"(db), "r"(idesc), "r"(accumulate) : "memory");
+}
+// D[128 x 128] (+)= A[128 x 128] . B[128 x 128]^T; each operand = two K blocks of [128 x 64] fp16, 16 KB apart
+__device__ __forceinline__ void umma_128x128x128(uint32_t d_tmem, uint32_t a_s, uint32_t b_s, bool accumulate)
+{
+    // instruction descriptor: D format f32 (1) in [4,6); A, B format f16 (0); both K-major; N >> 3 in [17,23); M >> 4 in [24,29)
+    constexpr uint32_t idesc = (1u << 4) | ((128u >> 3) << 17) | ((128u >> 4) << 24);
+#pragma unroll
+    for (int kb = 0; kb < 2; ++kb)
+#pragma unroll
+        for (int k = 0; k < 4; ++k)                          // UMMA_K = 16 fp16 = 32 bytes inside the 128-byte swizzle row
+            umma_f16_ss(d_tmem, umma_desc_sw128(a_s + kb * 16384 + k * 32), umma_desc_sw128(b_s + kb * 16384 + k * 32), idesc,
+                        (accumulate || kb || k) ? 1u : 0u);
+}
+__device__ __forceinline__ void umma_commit(uint32_t bar)
+{
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(bar) : "memory");
+}
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31]) : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&r)[32])
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};"
+                 :: "r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]), "r"(r[16]), "r"(r[17]), "r"(r[18]), "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]), "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31]) : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+
+constexpr int kTcOperandBytes = 4 * 32768;            // Q', K^, V^T, P
+
+__global__ void __launch_bounds__(256, 1)
+prefill_tc_kernel(const PrefillParams P)
+{
+    extern __shared__ __align__(1024) unsigned char smem[];
+    __shared__ __align__(16) uint16_t lut[kLutHalves];
+    __shared__ uint32_t pools[16];
+    __shared__ __align__(8) uint64_t bars[3];         // raw tile landed / S ready / PV done
+    __shared__ PUnit units[2 * kMaxKSteps];
+    __shared__ int n_units_s;
+    __shared__ uint32_t tmem_base_s;
+    __shared__ __align__(16) __half kn[kMaxGroups * 128];
+    __shared__ __align__(16) __half vn[128];
+    __shared__ float rmax[2][128], rsum[2][128];
+    unsigned char *qs = smem, *khat = smem + 32768, *vhat_t = smem + 65536, *ps = smem + 98304;
+    uint32_t *raw = reinterpret_cast<uint32_t *>(smem + kTcOperandBytes);
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int h = blockIdx.y, b = blockIdx.z, G = P.G;
+    const HeadMeta &M = P.metas[h];
+    const int TQ = 128 / G;
+    int64_t slen = P.seq_len[b];
+    slen = slen > P.n_cap * kTile ? P.n_cap * kTile : slen;
+    const int i_first = blockIdx.x * TQ;
+    const int i_last = min(P.n_q, i_first + TQ) - 1;
+    const int64_t pos0 = slen - P.n_q;                              // position of query token 0
+    if (i_first >= P.n_q || pos0 < 0) return;
+    const int n_tiles = (int)((pos0 + i_last) / kTile) + 1;
+
+    build_lut(P.cb16, lut, tid, 256, true);
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 256;" :: "r"(smem_u32(&tmem_base_s)) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    for (int i = tid; i < (32768 + 32768) / 16; i += 256) reinterpret_cast<uint4 *>(khat)[i] = make_uint4(0, 0, 0, 0);   // K^ (zero-width blocks stay 0), V^T
+    const uint32_t bar_raw = smem_u32(&bars[0]), bar_s = smem_u32(&bars[1]), bar_o = smem_u32(&bars[2]);
+    if (tid == 0) {
+        int nu = 0, j = 0;
+        for (int ks = 0; ks < M.n_ksteps; ++ks) {
+            const KStep &K = M.ksteps[ks];
+            const int g = K.flags >> 4;
+            if (K.flags & 1) j = 0;
+            units[nu++] = PUnit{K.off0, K.b, K.nc0, M.gstart[g] + 8 * j, g};
+            ++j;
+            if (K.off1 != 0xFFFF) { units[nu++] = PUnit{K.off1, K.b, K.nc1, M.gstart[g] + 8 * j, g}; ++j; }
+        }
+        n_units_s = nu;
+        mbar_init(bar_raw, 1);
+        mbar_init(bar_s, 1);
+        mbar_init(bar_o, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        fence_proxy_async();
+    }
+    {   // Q' rows -> the A operand.  Row r = (token r / G, head r % G); rows past n_q are zero.
+        const int r = tid >> 1, half = tid & 1;
+        const int ti = i_first + r / G, n = r % G;
+        const bool valid = ti < P.n_q;
+        const uint4 *src = reinterpret_cast<const uint4 *>(P.qp + ((((size_t)b * P.n_q + (valid ? ti : 0)) * P.Hkv + h) * 8 + n) * kDh + half * 64);
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            const uint4 v = valid ? __ldg(src + j) : make_uint4(0, 0, 0, 0);
+            *reinterpret_cast<uint4 *>(qs + half * 16384 + r * 128 + ((j ^ (r & 7)) << 4)) = v;
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tm = tmem_base_s;
+    if (tid == 0) build_pools(lut, pools);
+    const int n_units = n_units_s, ng = M.n_groups, b_v = M.b_v;
+    const uint8_t *region = P.cache + P.n_cap * ((int64_t)P.batch * M.layer_prefix + (int64_t)b * M.layer_sum + M.head_prefix);
+    const uint32_t raw_s = smem_u32(raw);
+    if (tid == 0) { mbar_expect_tx(bar_raw, M.tile_stride); bulk_g2s(raw_s, region, M.tile_stride, bar_raw); }
+
+    // softmax ownership: TMEM lane quadrant = warp & 3 (a warp can only touch its own quadrant), column half = warp >> 2
+    const int quad = warp & 3, hb = warp >> 2, row = 32 * quad + lane;
+    const int64_t prow = pos0 + i_first + row / G;                  // position of this row's query token
+    const uint32_t t_s = tm + ((uint32_t)(32 * quad) << 16) + 64u * hb, t_o = t_s + 128u;
+    const uint32_t qs_s = smem_u32(qs), khat_s = smem_u32(khat), vhat_s = smem_u32(vhat_t), ps_s = smem_u32(ps);
+    float m_run = -INFINITY, l_run = 0.f;
+    uint32_t ph_raw = 0, ph_s = 0, ph_o = 0;
+
+    for (int t = 0; t < n_tiles; ++t) {
+        // ---- a. raw tile t landed: linearise the norms, unpack K^ (its buffer is free: S(t-1) was waited for), start S
+        mbar_wait(bar_raw, ph_raw);
+        ph_raw ^= 1;
+        for (int idx = tid; idx < (ng + 1) * 128; idx += 256) {
+            const int tau = idx & 127, g = idx >> 7;
+            const int slot = (tau & 7) * 16 + (tau >> 4) * 2 + ((tau >> 3) & 1);
+            const int off = g < ng ? M.knorm_off + 256 * g : M.vnorm_off;
+            const __half v = reinterpret_cast<const __half *>(reinterpret_cast<const unsigned char *>(raw) + off)[slot];
+            if (g < ng) kn[g * 128 + tau] = v; else vn[tau] = v;
+        }
+        __syncthreads();
+        for (int u = warp; u < n_units; u += 8) {
+            const PUnit U = units[u];
+            switch (U.b) {
+            case 1: prefill_decode_k<1, true>(raw, U, lane, pools, lut, kn, khat); break;
+            case 2: prefill_decode_k<2, true>(raw, U, lane, pools, lut, kn, khat); break;
+            case 3: prefill_decode_k<3, true>(raw, U, lane, pools, lut, kn, khat); break;
+            case 4: prefill_decode_k<4, true>(raw, U, lane, pools, lut, kn, khat); break;
+            case 5: prefill_decode_k<5, true>(raw, U, lane, pools, lut, kn, khat); break;
+            case 6: prefill_decode_k<6, true>(raw, U, lane, pools, lut, kn, khat); break;
+            case 7: prefill_decode_k<7, true>(raw, U, lane, pools, lut, kn, khat); break;
+            default: prefill_decode_k<8, true>(raw, U, lane, pools, lut, kn, khat); break;
+            }
+        }
+        fence_proxy_async();                                         // generic-proxy writes of Q', K^ -> visible to the MMA
+        tc_fence_before();
+        __syncthreads();
+        if (tid == 0) {
+            tc_fence_after();
+            umma_128x128x128(tm, qs_s, khat_s, false);               // S = Q' . K^T
+            umma_commit(bar_s);
+        }
+        // ---- b. unpack V^T while S runs (its buffer and P are free once PV(t-1) has completed)
+        if (t > 0) {
+            mbar_wait(bar_o, ph_o);
+            ph_o ^= 1;
+            tc_fence_after();
+        }
+        {
+            const uint32_t *vcodes = raw + (M.vcode_off >> 2);
+            switch (b_v) {
+            case 1: prefill_decode_v<1, true>(vcodes, warp, lane, pools, lut, vn, vhat_t); break;
+            case 2: prefill_decode_v<2, true>(vcodes, warp, lane, pools, lut, vn, vhat_t); break;
+            case 3: prefill_decode_v<3, true>(vcodes, warp, lane, pools, lut, vn, vhat_t); break;
+            case 4: prefill_decode_v<4, true>(vcodes, warp, lane, pools, lut, vn, vhat_t); break;
+            case 5: prefill_decode_v<5, true>(vcodes, warp, lane, pools, lut, vn, vhat_t); break;
+            case 6: prefill_decode_v<6, true>(vcodes, warp, lane, pools, lut, vn, vhat_t); break;
+            case 7: prefill_decode_v<7, true>(vcodes, warp, lane, pools, lut, vn, vhat_t); break;
+            default: prefill_decode_v<8, true>(vcodes, warp, lane, pools, lut, vn, vhat_t); break;
+            }
+        }
+        // ---- c. softmax of this thread's row x 64 columns, straight from tensor memory (log2 domain)
+        mbar_wait(bar_s, ph_s);
+        ph_s ^= 1;
+        tc_fence_after();
+        uint32_t sr[2][32];
+        tmem_ld32(t_s, sr[0]);
+        tmem_ld32(t_s + 32, sr[1]);
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+        const int64_t col0 = (int64_t)t * kTile + 64 * hb;
+        float mx = -INFINITY;
+#pragma unroll
+        for (int i = 0; i < 64; ++i) {
+            float v = __uint_as_float(sr[i >> 5][i & 31]);
+            if (col0 + i > prow) v = -INFINITY;                      // causal mask
+            sr[i >> 5][i & 31] = __float_as_uint(v);
+            mx = fmaxf(mx, v);
+        }
+        rmax[hb][row] = mx;
+        __syncthreads();                                             // (also: every warp is done with the raw tile)
+        if (tid == 0 && t + 1 < n_tiles) {
+            fence_proxy_async();
+            mbar_expect_tx(bar_raw, M.tile_stride);
+            bulk_g2s(raw_s, region + (int64_t)(t + 1) * M.tile_stride, M.tile_stride, bar_raw);
+        }
+        const float mn = fmaxf(m_run, fmaxf(rmax[0][row], rmax[1][row]));   // finite: tile 0 holds position 0
+        const float alpha = fast_exp2(m_run - mn);
+        m_run = mn;
+        float ls = 0.f;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {                                // 8 tokens = one 16-byte chunk of the P row
+            float p[8];
+#pragma unroll
+            for (int e = 0; e < 8; ++e) {
+                p[e] = fast_exp2(__uint_as_float(sr[(8 * j + e) >> 5][(8 * j + e) & 31]) - mn);
+                ls += p[e];
+            }
+            const uint4 v = make_uint4(pack_half2(p[0], p[1]), pack_half2(p[2], p[3]), pack_half2(p[4], p[5]), pack_half2(p[6], p[7]));
+            *reinterpret_cast<uint4 *>(ps + hb * 16384 + row * 128 + ((j ^ (row & 7)) << 4)) = v;
+        }
+        l_run = fmaf(l_run, alpha, ls);
+        if (t > 0 && __any_sync(0xFFFFFFFFu, alpha != 1.f)) {        // a row maximum moved: rescale O in place
+#pragma unroll
+            for (int cb = 0; cb < 2; ++cb) {
+                uint32_t o[32];
+                tmem_ld32(t_o + 32 * cb, o);
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+                for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
+                tmem_st32(t_o + 32 * cb, o);
+            }
+            asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+        }
+        fence_proxy_async();                                         // P, V^T -> visible to the MMA
+        tc_fence_before();
+        __syncthreads();
+        if (tid == 0) {
+            tc_fence_after();
+            umma_128x128x128(tm + 128, ps_s, vhat_s, t > 0);         // O (+)= P . V^
+            umma_commit(bar_o);
+        }
+    }
+    // ---- normalise and store the rotated-domain output rows (fp32); derotate_kernel finishes them
+    mbar_wait(bar_o, ph_o);
+    tc_fence_after();
+    rsum[hb][row] = l_run;
+    __syncthreads();
+    const float inv = 1.f / (rsum[0][row] + rsum[1][row]);
+    const int ti = i_first + row / G, n = row % G;
+#pragma unroll
+    for (int cb = 0; cb < 2; ++cb) {
+        uint32_t o[32];
+        tmem_ld32(t_o + 32 * cb, o);
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+        if (ti < P.n_q) {
+            float4 *dst = reinterpret_cast<float4 *>(P.opart + (((size_t)b * P.n_q + ti) * (P.Hkv * G) + h * G + n) * kDh + 64 * hb + 32 * cb);
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+                dst[i] = make_float4(__uint_as_float(o[4 * i]) * inv, __uint_as_float(o[4 * i + 1]) * inv,
+                                     __uint_as_float(o[4 * i + 2]) * inv, __uint_as_float(o[4 * i + 3]) * inv);
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 256;" :: "r"(tm) : "memory");
+}
+
 // out[row][k] = sum_j Pi^(128)[j][k] * o'[row][j] / sqrt(128)  ->  bf16  (the V de-rotation, once per output row)
 __global__ void __launch_bounds__(128)
 derotate_kernel(const float *__restrict__ opart, const float *__restrict__ rot128, int64_t n_rows,
@@ -1719,9 +2003,12 @@ int launch_prefill(const bgtq_layout *lay, int layer, const void *cache, const v
     count_launch();
     CUDA_TRY(cudaGetLastError());
     const int raw_bytes = (lay->max_stride + 127) / 128 * 128;
-    const size_t smem = 65536 + (size_t)raw_bytes;
+    static int use_tc = -1;                         // BGTQ_PREFILL_MMA_SYNC=1 selects the first-cut mma.sync kernel
+    if (use_tc < 0) { const char *e = getenv("BGTQ_PREFILL_MMA_SYNC"); use_tc = (e && atoi(e) != 0) ? 0 : 1; }
+    const size_t smem = (use_tc ? (size_t)kTcOperandBytes : 65536) + (size_t)raw_bytes;
     if (!attr_set) {
         CUDA_TRY(cudaFuncSetAttribute(prefill_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 65536 + 40 * 1024));
+        CUDA_TRY(cudaFuncSetAttribute(prefill_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcOperandBytes + 40 * 1024));
         attr_set = true;
     }
     PrefillParams P;
@@ -1730,7 +2017,8 @@ int launch_prefill(const bgtq_layout *lay, int layer, const void *cache, const v
     P.raw_bytes = raw_bytes;
     const int TQ = 16 * (8 / G);
     dim3 grid((n_q + TQ - 1) / TQ, Hkv, batch);
-    prefill_kernel<<<grid, 256, smem, st>>>(P);
+    if (use_tc) prefill_tc_kernel<<<grid, 256, smem, st>>>(P);
+    else prefill_kernel<<<grid, 256, smem, st>>>(P);
     count_launch();
     CUDA_TRY(cudaGetLastError());
     derotate_kernel<<<(unsigned)((rows * Hq + 3) / 4), 128, 0, st>>>(opart, lay->d_rot + rot_offset(kDh), (int64_t)(rows * Hq),
