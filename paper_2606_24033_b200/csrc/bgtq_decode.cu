@@ -1431,11 +1431,12 @@ __device__ __forceinline__ void prefill_decode_k(const uint32_t *raw, const PUni
 
 template <int B, bool UMMA = false>
 __device__ __forceinline__ void prefill_decode_v(const uint32_t *vcodes, int J, int lane, const uint32_t *pools,
-                                                 const uint16_t *lut, const __half *vn, unsigned char *vhat_t)
+                                                 const uint16_t *lut, const __half *vn, unsigned char *vhat_t, int only_rho = -1)
 {
     const int gq = lane >> 2, c = lane & 3;
 #pragma unroll
     for (int rho = 0; rho < 2; ++rho) {
+        if (only_rho >= 0 && rho != only_rho) continue;
         uint32_t w[B], h[16];
         load_unit_full<B>(vcodes + (2 * J + rho) * 32 * B, lane, w);
         decode_unit<B, true>(w, pools, lut, h);
@@ -1689,7 +1690,7 @@ prefill_kernel(const PrefillParams P)
 //                  + the raw packed tile (TMA bulk copy);
 //   tensor memory: S = Q' K^T in columns [0,128), O in columns [128,256); row r of S / O is TMEM lane r.
 // Per 128-token tile: all 8 warps unpack K^ -> S MMA (async) -> unpack V^T while it runs -> softmax straight out of TMEM
-// (thread = one row x 64 columns: no shuffles; the two column halves meet through shared memory) -> P to shared memory,
+// (thread = one row x 32 columns: no shuffles; the four column quarters meet through shared memory) -> P to shared memory,
 // O rescaled in TMEM when a row maximum moved -> PV MMA (async), which overlaps the next tile's K^ unpack.
 __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t saddr)
 {
@@ -1736,7 +1737,9 @@ __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::
 
 constexpr int kTcOperandBytes = 4 * 32768;            // Q', K^, V^T, P
 
-__global__ void __launch_bounds__(256, 1)
+constexpr int kTcThreads = 512;                       // 16 warps: 4 per TMEM lane quadrant (32 S / O columns each)
+
+__global__ void __launch_bounds__(kTcThreads, 1)
 prefill_tc_kernel(const PrefillParams P)
 {
     extern __shared__ __align__(1024) unsigned char smem[];
@@ -1748,7 +1751,7 @@ prefill_tc_kernel(const PrefillParams P)
     __shared__ uint32_t tmem_base_s;
     __shared__ __align__(16) __half kn[kMaxGroups * 128];
     __shared__ __align__(16) __half vn[128];
-    __shared__ float rmax[2][128], rsum[2][128];
+    __shared__ float rmax[4][128], rsum[4][128];
     unsigned char *qs = smem, *khat = smem + 32768, *vhat_t = smem + 65536, *ps = smem + 98304;
     uint32_t *raw = reinterpret_cast<uint32_t *>(smem + kTcOperandBytes);
 
@@ -1764,12 +1767,12 @@ prefill_tc_kernel(const PrefillParams P)
     if (i_first >= P.n_q || pos0 < 0) return;
     const int n_tiles = (int)((pos0 + i_last) / kTile) + 1;
 
-    build_lut(P.cb16, lut, tid, 256, true);
+    build_lut(P.cb16, lut, tid, kTcThreads, true);
     if (warp == 0) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 256;" :: "r"(smem_u32(&tmem_base_s)) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
-    for (int i = tid; i < (32768 + 32768) / 16; i += 256) reinterpret_cast<uint4 *>(khat)[i] = make_uint4(0, 0, 0, 0);   // K^ (zero-width blocks stay 0), V^T
+    for (int i = tid; i < (32768 + 32768) / 16; i += kTcThreads) reinterpret_cast<uint4 *>(khat)[i] = make_uint4(0, 0, 0, 0);   // K^ (zero-width blocks stay 0), V^T
     const uint32_t bar_raw = smem_u32(&bars[0]), bar_s = smem_u32(&bars[1]), bar_o = smem_u32(&bars[2]);
     if (tid == 0) {
         int nu = 0, j = 0;
@@ -1789,12 +1792,12 @@ prefill_tc_kernel(const PrefillParams P)
         fence_proxy_async();
     }
     {   // Q' rows -> the A operand.  Row r = (token r / G, head r % G); rows past n_q are zero.
-        const int r = tid >> 1, half = tid & 1;
+        const int r = tid >> 2, half = (tid >> 1) & 1, j0 = (tid & 1) * 4;
         const int ti = i_first + r / G, n = r % G;
         const bool valid = ti < P.n_q;
         const uint4 *src = reinterpret_cast<const uint4 *>(P.qp + ((((size_t)b * P.n_q + (valid ? ti : 0)) * P.Hkv + h) * 8 + n) * kDh + half * 64);
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
+        for (int j = j0; j < j0 + 4; ++j) {
             const uint4 v = valid ? __ldg(src + j) : make_uint4(0, 0, 0, 0);
             *reinterpret_cast<uint4 *>(qs + half * 16384 + r * 128 + ((j ^ (r & 7)) << 4)) = v;
         }
@@ -1809,10 +1812,10 @@ prefill_tc_kernel(const PrefillParams P)
     const uint32_t raw_s = smem_u32(raw);
     if (tid == 0) { mbar_expect_tx(bar_raw, M.tile_stride); bulk_g2s(raw_s, region, M.tile_stride, bar_raw); }
 
-    // softmax ownership: TMEM lane quadrant = warp & 3 (a warp can only touch its own quadrant), column half = warp >> 2
-    const int quad = warp & 3, hb = warp >> 2, row = 32 * quad + lane;
+    // softmax ownership: TMEM lane quadrant = warp & 3 (a warp can only touch its own quadrant), column quarter = warp >> 2
+    const int quad = warp & 3, qb = warp >> 2, row = 32 * quad + lane;
     const int64_t prow = pos0 + i_first + row / G;                  // position of this row's query token
-    const uint32_t t_s = tm + ((uint32_t)(32 * quad) << 16) + 64u * hb, t_o = t_s + 128u;
+    const uint32_t t_s = tm + ((uint32_t)(32 * quad) << 16) + 32u * qb, t_o = t_s + 128u;
     const uint32_t qs_s = smem_u32(qs), khat_s = smem_u32(khat), vhat_s = smem_u32(vhat_t), ps_s = smem_u32(ps);
     float m_run = -INFINITY, l_run = 0.f;
     uint32_t ph_raw = 0, ph_s = 0, ph_o = 0;
@@ -1821,7 +1824,7 @@ prefill_tc_kernel(const PrefillParams P)
         // ---- a. raw tile t landed: linearise the norms, unpack K^ (its buffer is free: S(t-1) was waited for), start S
         mbar_wait(bar_raw, ph_raw);
         ph_raw ^= 1;
-        for (int idx = tid; idx < (ng + 1) * 128; idx += 256) {
+        for (int idx = tid; idx < (ng + 1) * 128; idx += kTcThreads) {
             const int tau = idx & 127, g = idx >> 7;
             const int slot = (tau & 7) * 16 + (tau >> 4) * 2 + ((tau >> 3) & 1);
             const int off = g < ng ? M.knorm_off + 256 * g : M.vnorm_off;
@@ -1829,7 +1832,7 @@ prefill_tc_kernel(const PrefillParams P)
             if (g < ng) kn[g * 128 + tau] = v; else vn[tau] = v;
         }
         __syncthreads();
-        for (int u = warp; u < n_units; u += 8) {
+        for (int u = warp; u < n_units; u += kTcThreads / 32) {
             const PUnit U = units[u];
             switch (U.b) {
             case 1: prefill_decode_k<1, true>(raw, U, lane, pools, lut, kn, khat); break;
@@ -1859,66 +1862,63 @@ prefill_tc_kernel(const PrefillParams P)
         {
             const uint32_t *vcodes = raw + (M.vcode_off >> 2);
             switch (b_v) {
-            case 1: prefill_decode_v<1, true>(vcodes, warp, lane, pools, lut, vn, vhat_t); break;
-            case 2: prefill_decode_v<2, true>(vcodes, warp, lane, pools, lut, vn, vhat_t); break;
-            case 3: prefill_decode_v<3, true>(vcodes, warp, lane, pools, lut, vn, vhat_t); break;
-            case 4: prefill_decode_v<4, true>(vcodes, warp, lane, pools, lut, vn, vhat_t); break;
-            case 5: prefill_decode_v<5, true>(vcodes, warp, lane, pools, lut, vn, vhat_t); break;
-            case 6: prefill_decode_v<6, true>(vcodes, warp, lane, pools, lut, vn, vhat_t); break;
-            case 7: prefill_decode_v<7, true>(vcodes, warp, lane, pools, lut, vn, vhat_t); break;
-            default: prefill_decode_v<8, true>(vcodes, warp, lane, pools, lut, vn, vhat_t); break;
+            case 1: prefill_decode_v<1, true>(vcodes, warp >> 1, lane, pools, lut, vn, vhat_t, warp & 1); break;
+            case 2: prefill_decode_v<2, true>(vcodes, warp >> 1, lane, pools, lut, vn, vhat_t, warp & 1); break;
+            case 3: prefill_decode_v<3, true>(vcodes, warp >> 1, lane, pools, lut, vn, vhat_t, warp & 1); break;
+            case 4: prefill_decode_v<4, true>(vcodes, warp >> 1, lane, pools, lut, vn, vhat_t, warp & 1); break;
+            case 5: prefill_decode_v<5, true>(vcodes, warp >> 1, lane, pools, lut, vn, vhat_t, warp & 1); break;
+            case 6: prefill_decode_v<6, true>(vcodes, warp >> 1, lane, pools, lut, vn, vhat_t, warp & 1); break;
+            case 7: prefill_decode_v<7, true>(vcodes, warp >> 1, lane, pools, lut, vn, vhat_t, warp & 1); break;
+            default: prefill_decode_v<8, true>(vcodes, warp >> 1, lane, pools, lut, vn, vhat_t, warp & 1); break;
             }
         }
         // ---- c. softmax of this thread's row x 64 columns, straight from tensor memory (log2 domain)
         mbar_wait(bar_s, ph_s);
         ph_s ^= 1;
         tc_fence_after();
-        uint32_t sr[2][32];
-        tmem_ld32(t_s, sr[0]);
-        tmem_ld32(t_s + 32, sr[1]);
+        uint32_t sr[32];
+        tmem_ld32(t_s, sr);
         asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-        const int64_t col0 = (int64_t)t * kTile + 64 * hb;
+        const int rel = (int)min((int64_t)1 << 20, prow - ((int64_t)t * kTile + 32 * qb));   // columns i > rel are in the future
         float mx = -INFINITY;
 #pragma unroll
-        for (int i = 0; i < 64; ++i) {
-            float v = __uint_as_float(sr[i >> 5][i & 31]);
-            if (col0 + i > prow) v = -INFINITY;                      // causal mask
-            sr[i >> 5][i & 31] = __float_as_uint(v);
+        for (int i = 0; i < 32; ++i) {
+            float v = __uint_as_float(sr[i]);
+            if (i > rel) v = -INFINITY;                              // causal mask
+            sr[i] = __float_as_uint(v);
             mx = fmaxf(mx, v);
         }
-        rmax[hb][row] = mx;
+        rmax[qb][row] = mx;
         __syncthreads();                                             // (also: every warp is done with the raw tile)
         if (tid == 0 && t + 1 < n_tiles) {
             fence_proxy_async();
             mbar_expect_tx(bar_raw, M.tile_stride);
             bulk_g2s(raw_s, region + (int64_t)(t + 1) * M.tile_stride, M.tile_stride, bar_raw);
         }
-        const float mn = fmaxf(m_run, fmaxf(rmax[0][row], rmax[1][row]));   // finite: tile 0 holds position 0
+        const float mn = fmaxf(fmaxf(m_run, fmaxf(rmax[0][row], rmax[1][row])), fmaxf(rmax[2][row], rmax[3][row]));   // finite: tile 0 holds position 0
         const float alpha = fast_exp2(m_run - mn);
         m_run = mn;
         float ls = 0.f;
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {                                // 8 tokens = one 16-byte chunk of the P row
+        for (int j = 0; j < 4; ++j) {                                // 8 tokens = one 16-byte chunk of the P row
             float p[8];
 #pragma unroll
             for (int e = 0; e < 8; ++e) {
-                p[e] = fast_exp2(__uint_as_float(sr[(8 * j + e) >> 5][(8 * j + e) & 31]) - mn);
+                p[e] = fast_exp2(__uint_as_float(sr[8 * j + e]) - mn);
                 ls += p[e];
             }
             const uint4 v = make_uint4(pack_half2(p[0], p[1]), pack_half2(p[2], p[3]), pack_half2(p[4], p[5]), pack_half2(p[6], p[7]));
-            *reinterpret_cast<uint4 *>(ps + hb * 16384 + row * 128 + ((j ^ (row & 7)) << 4)) = v;
+            const int ch = (qb & 1) * 4 + j;                         // chunk inside the 64-token K block qb >> 1
+            *reinterpret_cast<uint4 *>(ps + (qb >> 1) * 16384 + row * 128 + ((ch ^ (row & 7)) << 4)) = v;
         }
         l_run = fmaf(l_run, alpha, ls);
         if (t > 0 && __any_sync(0xFFFFFFFFu, alpha != 1.f)) {        // a row maximum moved: rescale O in place
+            uint32_t o[32];
+            tmem_ld32(t_o, o);
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
-            for (int cb = 0; cb < 2; ++cb) {
-                uint32_t o[32];
-                tmem_ld32(t_o + 32 * cb, o);
-                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-                for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
-                tmem_st32(t_o + 32 * cb, o);
-            }
+            for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
+            tmem_st32(t_o, o);
             asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
         }
         fence_proxy_async();                                         // P, V^T -> visible to the MMA
@@ -1933,17 +1933,16 @@ prefill_tc_kernel(const PrefillParams P)
     // ---- normalise and store the rotated-domain output rows (fp32); derotate_kernel finishes them
     mbar_wait(bar_o, ph_o);
     tc_fence_after();
-    rsum[hb][row] = l_run;
+    rsum[qb][row] = l_run;
     __syncthreads();
-    const float inv = 1.f / (rsum[0][row] + rsum[1][row]);
+    const float inv = 1.f / ((rsum[0][row] + rsum[1][row]) + (rsum[2][row] + rsum[3][row]));
     const int ti = i_first + row / G, n = row % G;
-#pragma unroll
-    for (int cb = 0; cb < 2; ++cb) {
+    {
         uint32_t o[32];
-        tmem_ld32(t_o + 32 * cb, o);
+        tmem_ld32(t_o, o);
         asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
         if (ti < P.n_q) {
-            float4 *dst = reinterpret_cast<float4 *>(P.opart + (((size_t)b * P.n_q + ti) * (P.Hkv * G) + h * G + n) * kDh + 64 * hb + 32 * cb);
+            float4 *dst = reinterpret_cast<float4 *>(P.opart + (((size_t)b * P.n_q + ti) * (P.Hkv * G) + h * G + n) * kDh + 32 * qb);
 #pragma unroll
             for (int i = 0; i < 8; ++i)
                 dst[i] = make_float4(__uint_as_float(o[4 * i]) * inv, __uint_as_float(o[4 * i + 1]) * inv,
@@ -2017,7 +2016,7 @@ int launch_prefill(const bgtq_layout *lay, int layer, const void *cache, const v
     P.raw_bytes = raw_bytes;
     const int TQ = 16 * (8 / G);
     dim3 grid((n_q + TQ - 1) / TQ, Hkv, batch);
-    if (use_tc) prefill_tc_kernel<<<grid, 256, smem, st>>>(P);
+    if (use_tc) prefill_tc_kernel<<<grid, kTcThreads, smem, st>>>(P);
     else prefill_kernel<<<grid, 256, smem, st>>>(P);
     count_launch();
     CUDA_TRY(cudaGetLastError());
