@@ -1732,16 +1732,27 @@ __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&r)[32
     asm volatile("tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};"
                  :: "r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]), "r"(r[16]), "r"(r[17]), "r"(r[18]), "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]), "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31]) : "memory");
 }
+__device__ __forceinline__ float fmax3(float a, float b, float c)
+{
+    float r;
+    asm("max.f32 %0, %1, %2, %3;" : "=f"(r) : "f"(a), "f"(b), "f"(c));     // FMNMX3 (sm_100)
+    return r;
+}
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 
-constexpr int kTcOperandBytes = 4 * 32768;            // Q', K^, V^T, P
+constexpr int kTcThreads = 512;                       // 16 warps: 4 per TMEM lane quadrant
+__host__ __device__ constexpr int tc_operand_bytes(int RT) { return RT * 32768 + 32768 + 32768 + RT * 32768; }   // Q', K^, V^T, P
 
-constexpr int kTcThreads = 512;                       // 16 warps: 4 per TMEM lane quadrant (32 S / O columns each)
-
+// RT = 128-row query tiles per CTA (1 or 2).  With RT = 2 one unpack of a packed tile serves 256 query rows
+// (32 tokens x 8 heads at G = 8): S0, S1 in TMEM columns [0,256), O0, O1 in [256,512) -- the whole tensor memory --
+// and 192 KB of operands in shared memory, so it is used whenever the raw tile still fits beside them.
+template <int RT>
 __global__ void __launch_bounds__(kTcThreads, 1)
 prefill_tc_kernel(const PrefillParams P)
 {
+    constexpr int NG = 4 / RT;                        // column groups per row: each thread owns 128 / NG columns of one row
+    constexpr int NCH = RT;                           // ... i.e. NCH chunks of 32 columns
     extern __shared__ __align__(1024) unsigned char smem[];
     __shared__ __align__(16) uint16_t lut[kLutHalves];
     __shared__ uint32_t pools[16];
@@ -1751,14 +1762,14 @@ prefill_tc_kernel(const PrefillParams P)
     __shared__ uint32_t tmem_base_s;
     __shared__ __align__(16) __half kn[kMaxGroups * 128];
     __shared__ __align__(16) __half vn[128];
-    __shared__ float rmax[4][128], rsum[4][128];
-    unsigned char *qs = smem, *khat = smem + 32768, *vhat_t = smem + 65536, *ps = smem + 98304;
-    uint32_t *raw = reinterpret_cast<uint32_t *>(smem + kTcOperandBytes);
+    __shared__ float rmax[NG][RT * 128], rsum[NG][RT * 128];
+    unsigned char *qs = smem, *khat = smem + RT * 32768, *vhat_t = khat + 32768, *ps = vhat_t + 32768;
+    uint32_t *raw = reinterpret_cast<uint32_t *>(smem + tc_operand_bytes(RT));
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int h = blockIdx.y, b = blockIdx.z, G = P.G;
     const HeadMeta &M = P.metas[h];
-    const int TQ = 128 / G;
+    const int TQ = RT * 128 / G;
     int64_t slen = P.seq_len[b];
     slen = slen > P.n_cap * kTile ? P.n_cap * kTile : slen;
     const int i_first = blockIdx.x * TQ;
@@ -1769,7 +1780,7 @@ prefill_tc_kernel(const PrefillParams P)
 
     build_lut(P.cb16, lut, tid, kTcThreads, true);
     if (warp == 0) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 256;" :: "r"(smem_u32(&tmem_base_s)) : "memory");
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(smem_u32(&tmem_base_s)), "n"(RT * 256) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
     for (int i = tid; i < (32768 + 32768) / 16; i += kTcThreads) reinterpret_cast<uint4 *>(khat)[i] = make_uint4(0, 0, 0, 0);   // K^ (zero-width blocks stay 0), V^T
@@ -1791,15 +1802,17 @@ prefill_tc_kernel(const PrefillParams P)
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         fence_proxy_async();
     }
-    {   // Q' rows -> the A operand.  Row r = (token r / G, head r % G); rows past n_q are zero.
-        const int r = tid >> 2, half = (tid >> 1) & 1, j0 = (tid & 1) * 4;
-        const int ti = i_first + r / G, n = r % G;
+    {   // Q' rows -> the A operands.  Row r of the CTA = (token r / G, head r % G); rows past n_q are zero.
+        constexpr int TPR = 4 / RT, NV = 4 * RT;                    // threads per row, 16-byte vectors per thread
+        const int r = tid / TPR, part = tid % TPR;
+        const int kb = (part * 8 * NV) >> 6, j0 = ((part * 8 * NV) & 63) >> 3;
+        const int ti = i_first + r / G, n = r % G, rr = r & 127;
         const bool valid = ti < P.n_q;
-        const uint4 *src = reinterpret_cast<const uint4 *>(P.qp + ((((size_t)b * P.n_q + (valid ? ti : 0)) * P.Hkv + h) * 8 + n) * kDh + half * 64);
+        const uint4 *src = reinterpret_cast<const uint4 *>(P.qp + ((((size_t)b * P.n_q + (valid ? ti : 0)) * P.Hkv + h) * 8 + n) * kDh + part * 8 * NV);
 #pragma unroll
-        for (int j = j0; j < j0 + 4; ++j) {
-            const uint4 v = valid ? __ldg(src + j) : make_uint4(0, 0, 0, 0);
-            *reinterpret_cast<uint4 *>(qs + half * 16384 + r * 128 + ((j ^ (r & 7)) << 4)) = v;
+        for (int jj = 0; jj < NV; ++jj) {
+            const uint4 v = valid ? __ldg(src + jj) : make_uint4(0, 0, 0, 0);
+            *reinterpret_cast<uint4 *>(qs + (r >> 7) * 32768 + kb * 16384 + rr * 128 + (((j0 + jj) ^ (rr & 7)) << 4)) = v;
         }
     }
     tc_fence_before();
@@ -1812,11 +1825,14 @@ prefill_tc_kernel(const PrefillParams P)
     const uint32_t raw_s = smem_u32(raw);
     if (tid == 0) { mbar_expect_tx(bar_raw, M.tile_stride); bulk_g2s(raw_s, region, M.tile_stride, bar_raw); }
 
-    // softmax ownership: TMEM lane quadrant = warp & 3 (a warp can only touch its own quadrant), column quarter = warp >> 2
-    const int quad = warp & 3, qb = warp >> 2, row = 32 * quad + lane;
-    const int64_t prow = pos0 + i_first + row / G;                  // position of this row's query token
-    const uint32_t t_s = tm + ((uint32_t)(32 * quad) << 16) + 32u * qb, t_o = t_s + 128u;
+    // softmax ownership: TMEM lane quadrant = warp & 3 (a warp can only touch its own quadrant); the 4 warps of a quadrant
+    // split into RT row tiles x NG column groups
+    const int quad = warp & 3, rt = (warp >> 2) % RT, cg = (warp >> 2) / RT;
+    const int row = 32 * quad + lane, crow = rt * 128 + row, c_lo = cg * (128 / NG);
+    const int64_t prow = pos0 + i_first + crow / G;                 // position of this row's query token
+    const uint32_t t_s = tm + ((uint32_t)(32 * quad) << 16) + (uint32_t)(rt * 128 + c_lo), t_o = t_s + RT * 128u;
     const uint32_t qs_s = smem_u32(qs), khat_s = smem_u32(khat), vhat_s = smem_u32(vhat_t), ps_s = smem_u32(ps);
+    unsigned char *prow_s = ps + rt * 32768 + row * 128;
     float m_run = -INFINITY, l_run = 0.f;
     uint32_t ph_raw = 0, ph_s = 0, ph_o = 0;
 
@@ -1850,7 +1866,8 @@ prefill_tc_kernel(const PrefillParams P)
         __syncthreads();
         if (tid == 0) {
             tc_fence_after();
-            umma_128x128x128(tm, qs_s, khat_s, false);               // S = Q' . K^T
+#pragma unroll
+            for (int r = 0; r < RT; ++r) umma_128x128x128(tm + r * 128, qs_s + r * 32768, khat_s, false);   // S_r = Q'_r . K^T
             umma_commit(bar_s);
         }
         // ---- b. unpack V^T while S runs (its buffer and P are free once PV(t-1) has completed)
@@ -1872,53 +1889,71 @@ prefill_tc_kernel(const PrefillParams P)
             default: prefill_decode_v<8, true>(vcodes, warp >> 1, lane, pools, lut, vn, vhat_t, warp & 1); break;
             }
         }
-        // ---- c. softmax of this thread's row x 64 columns, straight from tensor memory (log2 domain)
+        // ---- c. softmax of this thread's row x (128 / NG) columns, straight from tensor memory (log2 domain), in two
+        //      passes over TMEM (maximum, then exponentials) so that no more than 32 logits are in registers at a time
         mbar_wait(bar_s, ph_s);
         ph_s ^= 1;
         tc_fence_after();
-        uint32_t sr[32];
-        tmem_ld32(t_s, sr);
-        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-        const int rel = (int)min((int64_t)1 << 20, prow - ((int64_t)t * kTile + 32 * qb));   // columns i > rel are in the future
+        const int rel = (int)max((int64_t)-1, min((int64_t)1 << 20, prow - ((int64_t)t * kTile + c_lo)));   // columns > rel are in the future
+        // (all but the last one or two tiles of a row are fully visible: warp-uniform fast path without the mask)
+        const bool nomask = __all_sync(0xFFFFFFFFu, rel >= 128 / NG - 1);
         float mx = -INFINITY;
 #pragma unroll
-        for (int i = 0; i < 32; ++i) {
-            float v = __uint_as_float(sr[i]);
-            if (i > rel) v = -INFINITY;                              // causal mask
-            sr[i] = __float_as_uint(v);
-            mx = fmaxf(mx, v);
+        for (int ch = 0; ch < NCH; ++ch) {
+            uint32_t sr[32];
+            tmem_ld32(t_s + 32 * ch, sr);
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+            if (nomask) {
+#pragma unroll
+                for (int i = 0; i < 32; i += 2) mx = fmax3(mx, __uint_as_float(sr[i]), __uint_as_float(sr[i + 1]));
+            } else {
+#pragma unroll
+                for (int i = 0; i < 32; ++i) mx = fmaxf(mx, 32 * ch + i > rel ? -INFINITY : __uint_as_float(sr[i]));
+            }
         }
-        rmax[qb][row] = mx;
+        rmax[cg][crow] = mx;
         __syncthreads();                                             // (also: every warp is done with the raw tile)
         if (tid == 0 && t + 1 < n_tiles) {
             fence_proxy_async();
             mbar_expect_tx(bar_raw, M.tile_stride);
             bulk_g2s(raw_s, region + (int64_t)(t + 1) * M.tile_stride, M.tile_stride, bar_raw);
         }
-        const float mn = fmaxf(fmaxf(m_run, fmaxf(rmax[0][row], rmax[1][row])), fmaxf(rmax[2][row], rmax[3][row]));   // finite: tile 0 holds position 0
+        float mn = m_run;                                            // finite after tile 0: it holds position 0
+#pragma unroll
+        for (int g2 = 0; g2 < NG; ++g2) mn = fmaxf(mn, rmax[g2][crow]);
         const float alpha = fast_exp2(m_run - mn);
         m_run = mn;
         float ls = 0.f;
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {                                // 8 tokens = one 16-byte chunk of the P row
-            float p[8];
+        for (int ch = 0; ch < NCH; ++ch) {
+            uint32_t sr[32];
+            tmem_ld32(t_s + 32 * ch, sr);
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
-            for (int e = 0; e < 8; ++e) {
-                p[e] = fast_exp2(__uint_as_float(sr[8 * j + e]) - mn);
-                ls += p[e];
+            for (int j = 0; j < 4; ++j) {                            // 8 tokens = one 16-byte chunk of the P row
+                float p[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    const int i = 32 * ch + 8 * j + e;
+                    p[e] = (!nomask && i > rel) ? 0.f : fast_exp2(__uint_as_float(sr[8 * j + e]) - mn);
+                    ls += p[e];
+                }
+                const uint4 v = make_uint4(pack_half2(p[0], p[1]), pack_half2(p[2], p[3]), pack_half2(p[4], p[5]), pack_half2(p[6], p[7]));
+                const int col = c_lo + 32 * ch + 8 * j;              // token column of the chunk: K block col >> 6, chunk (col & 63) >> 3
+                *reinterpret_cast<uint4 *>(prow_s + (col >> 6) * 16384 + ((((col & 63) >> 3) ^ (row & 7)) << 4)) = v;
             }
-            const uint4 v = make_uint4(pack_half2(p[0], p[1]), pack_half2(p[2], p[3]), pack_half2(p[4], p[5]), pack_half2(p[6], p[7]));
-            const int ch = (qb & 1) * 4 + j;                         // chunk inside the 64-token K block qb >> 1
-            *reinterpret_cast<uint4 *>(ps + (qb >> 1) * 16384 + row * 128 + ((ch ^ (row & 7)) << 4)) = v;
         }
         l_run = fmaf(l_run, alpha, ls);
         if (t > 0 && __any_sync(0xFFFFFFFFu, alpha != 1.f)) {        // a row maximum moved: rescale O in place
-            uint32_t o[32];
-            tmem_ld32(t_o, o);
-            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
-            for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
-            tmem_st32(t_o, o);
+            for (int ch = 0; ch < NCH; ++ch) {
+                uint32_t o[32];
+                tmem_ld32(t_o + 32 * ch, o);
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+                for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
+                tmem_st32(t_o + 32 * ch, o);
+            }
             asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
         }
         fence_proxy_async();                                         // P, V^T -> visible to the MMA
@@ -1926,23 +1961,28 @@ prefill_tc_kernel(const PrefillParams P)
         __syncthreads();
         if (tid == 0) {
             tc_fence_after();
-            umma_128x128x128(tm + 128, ps_s, vhat_s, t > 0);         // O (+)= P . V^
+#pragma unroll
+            for (int r = 0; r < RT; ++r) umma_128x128x128(tm + (RT + r) * 128, ps_s + r * 32768, vhat_s, t > 0);   // O_r (+)= P_r . V^
             umma_commit(bar_o);
         }
     }
     // ---- normalise and store the rotated-domain output rows (fp32); derotate_kernel finishes them
     mbar_wait(bar_o, ph_o);
     tc_fence_after();
-    rsum[qb][row] = l_run;
+    rsum[cg][crow] = l_run;
     __syncthreads();
-    const float inv = 1.f / ((rsum[0][row] + rsum[1][row]) + (rsum[2][row] + rsum[3][row]));
-    const int ti = i_first + row / G, n = row % G;
-    {
+    float lt = 0.f;
+#pragma unroll
+    for (int g2 = 0; g2 < NG; ++g2) lt += rsum[g2][crow];
+    const float inv = 1.f / lt;
+    const int ti = i_first + crow / G, n = crow % G;
+#pragma unroll
+    for (int ch = 0; ch < NCH; ++ch) {
         uint32_t o[32];
-        tmem_ld32(t_o, o);
+        tmem_ld32(t_o + 32 * ch, o);
         asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
         if (ti < P.n_q) {
-            float4 *dst = reinterpret_cast<float4 *>(P.opart + (((size_t)b * P.n_q + ti) * (P.Hkv * G) + h * G + n) * kDh + 32 * qb);
+            float4 *dst = reinterpret_cast<float4 *>(P.opart + (((size_t)b * P.n_q + ti) * (P.Hkv * G) + h * G + n) * kDh + c_lo + 32 * ch);
 #pragma unroll
             for (int i = 0; i < 8; ++i)
                 dst[i] = make_float4(__uint_as_float(o[4 * i]) * inv, __uint_as_float(o[4 * i + 1]) * inv,
@@ -1951,7 +1991,7 @@ prefill_tc_kernel(const PrefillParams P)
     }
     tc_fence_before();
     __syncthreads();
-    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 256;" :: "r"(tm) : "memory");
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tm), "n"(RT * 256) : "memory");
 }
 
 // out[row][k] = sum_j Pi^(128)[j][k] * o'[row][j] / sqrt(128)  ->  bf16  (the V de-rotation, once per output row)
@@ -2004,20 +2044,24 @@ int launch_prefill(const bgtq_layout *lay, int layer, const void *cache, const v
     const int raw_bytes = (lay->max_stride + 127) / 128 * 128;
     static int use_tc = -1;                         // BGTQ_PREFILL_MMA_SYNC=1 selects the first-cut mma.sync kernel
     if (use_tc < 0) { const char *e = getenv("BGTQ_PREFILL_MMA_SYNC"); use_tc = (e && atoi(e) != 0) ? 0 : 1; }
-    const size_t smem = (use_tc ? (size_t)kTcOperandBytes : 65536) + (size_t)raw_bytes;
+    // two 128-row query tiles per CTA when the raw tile still fits beside 192 KB of operands (12.5 KB of static tables)
+    const int RT = (tc_operand_bytes(2) + raw_bytes + 13 * 1024 <= 227 * 1024 && (n_q * G > 128)) ? 2 : 1;
+    const size_t smem = (use_tc ? (size_t)tc_operand_bytes(RT) : 65536) + (size_t)raw_bytes;
     if (!attr_set) {
         CUDA_TRY(cudaFuncSetAttribute(prefill_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 65536 + 40 * 1024));
-        CUDA_TRY(cudaFuncSetAttribute(prefill_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcOperandBytes + 40 * 1024));
+        CUDA_TRY(cudaFuncSetAttribute(prefill_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc_operand_bytes(1) + 40 * 1024));
+        CUDA_TRY(cudaFuncSetAttribute(prefill_tc_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 13 * 1024));
         attr_set = true;
     }
     PrefillParams P;
     P.metas = metas; P.cache = (const uint8_t *)cache; P.qp = qp; P.seq_len = seq_len; P.cb16 = lay->d_cb16;
     P.opart = opart; P.n_cap = (max_tokens + kTile - 1) / kTile; P.batch = batch; P.n_q = n_q; P.Hkv = Hkv; P.G = G;
     P.raw_bytes = raw_bytes;
-    const int TQ = 16 * (8 / G);
+    const int TQ = (use_tc ? RT * 128 : 128) / G;
     dim3 grid((n_q + TQ - 1) / TQ, Hkv, batch);
-    if (use_tc) prefill_tc_kernel<<<grid, kTcThreads, smem, st>>>(P);
-    else prefill_kernel<<<grid, 256, smem, st>>>(P);
+    if (!use_tc) prefill_kernel<<<grid, 256, smem, st>>>(P);
+    else if (RT == 2) prefill_tc_kernel<2><<<grid, kTcThreads, smem, st>>>(P);
+    else prefill_tc_kernel<1><<<grid, kTcThreads, smem, st>>>(P);
     count_launch();
     CUDA_TRY(cudaGetLastError());
     derotate_kernel<<<(unsigned)((rows * Hq + 3) / 4), 128, 0, st>>>(opart, lay->d_rot + rot_offset(kDh), (int64_t)(rows * Hq),
