@@ -1417,15 +1417,31 @@ __device__ __forceinline__ void prefill_decode_k(const uint32_t *raw, const PUni
     decode_unit<B, true>(w, pools, lut, h);
     if (c < U.nc) {
         const int col = U.ustart + 2 * c;
+        if (UMMA) {
+            // the norm row of a group is stored so that the 16 tokens of a lane (16 i + 8 p + g8) are 16 consecutive fp16:
+            // `kn` points at the raw row of the unit's group
+            const uint4 *np = reinterpret_cast<const uint4 *>(kn + g8 * 16);
+            const uint4 n0 = np[0], n1 = np[1];
+            const uint32_t nw[8] = {n0.x, n0.y, n0.z, n0.w, n1.x, n1.y, n1.z, n1.w};
 #pragma unroll
-        for (int i = 0; i < 8; ++i)
+            for (int i = 0; i < 8; ++i)
 #pragma unroll
-            for (int p = 0; p < 2; ++p) {
-                const int tok = 16 * i + 8 * p + g8;
-                const uint32_t n2 = (uint32_t)__half_as_ushort(kn[U.group * 128 + tok]) * 0x10001u;
-                const uint32_t v = hmul2_u(h[2 * i + p], n2);
-                *reinterpret_cast<uint32_t *>(khat + tile_off<UMMA>(tok, col)) = v;
-            }
+                for (int p = 0; p < 2; ++p) {
+                    const int tok = 16 * i + 8 * p + g8;
+                    const uint32_t n2 = prmt(nw[i], nw[i], p ? 0x3232 : 0x1010);
+                    *reinterpret_cast<uint32_t *>(khat + tile_off<UMMA>(tok, col)) = hmul2_u(h[2 * i + p], n2);
+                }
+        } else {
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+#pragma unroll
+                for (int p = 0; p < 2; ++p) {
+                    const int tok = 16 * i + 8 * p + g8;
+                    const uint32_t n2 = (uint32_t)__half_as_ushort(kn[U.group * 128 + tok]) * 0x10001u;
+                    const uint32_t v = hmul2_u(h[2 * i + p], n2);
+                    *reinterpret_cast<uint32_t *>(khat + tile_off<UMMA>(tok, col)) = v;
+                }
+        }
     }
 }
 
@@ -1445,7 +1461,7 @@ __device__ __forceinline__ void prefill_decode_v(const uint32_t *vcodes, int J, 
         for (int kp = 0; kp < 8; ++kp)
 #pragma unroll
             for (int o = 0; o < 2; ++o) {
-                const int tok = 16 * kp + 8 * o + 2 * c;                       // tokens tok, tok+1
+                const int tok = 16 * kp + 8 * o + 2 * c;                   // tokens tok, tok+1
                 const uint32_t n2 = *reinterpret_cast<const uint32_t *>(vn + tok);
                 const uint32_t v = hmul2_u(h[2 * kp + o], n2);
                 *reinterpret_cast<uint32_t *>(vhat_t + tile_off<UMMA>(dim, tok)) = v;
@@ -1760,9 +1776,8 @@ prefill_tc_kernel(const PrefillParams P)
     __shared__ PUnit units[2 * kMaxKSteps];
     __shared__ int n_units_s;
     __shared__ uint32_t tmem_base_s;
-    __shared__ __align__(16) __half kn[kMaxGroups * 128];
-    __shared__ __align__(16) __half vn[128];
     __shared__ float rmax[NG][RT * 128], rsum[NG][RT * 128];
+    __shared__ __align__(16) __half vn[128];
     unsigned char *qs = smem, *khat = smem + RT * 32768, *vhat_t = khat + 32768, *ps = vhat_t + 32768;
     uint32_t *raw = reinterpret_cast<uint32_t *>(smem + tc_operand_bytes(RT));
 
@@ -1820,7 +1835,8 @@ prefill_tc_kernel(const PrefillParams P)
     tc_fence_after();
     const uint32_t tm = tmem_base_s;
     if (tid == 0) build_pools(lut, pools);
-    const int n_units = n_units_s, ng = M.n_groups, b_v = M.b_v;
+    __syncthreads();                                                // pools are read by the first unpack
+    const int n_units = n_units_s, b_v = M.b_v;
     const uint8_t *region = P.cache + P.n_cap * ((int64_t)P.batch * M.layer_prefix + (int64_t)b * M.layer_sum + M.head_prefix);
     const uint32_t raw_s = smem_u32(raw);
     if (tid == 0) { mbar_expect_tx(bar_raw, M.tile_stride); bulk_g2s(raw_s, region, M.tile_stride, bar_raw); }
@@ -1840,16 +1856,11 @@ prefill_tc_kernel(const PrefillParams P)
         // ---- a. raw tile t landed: linearise the norms, unpack K^ (its buffer is free: S(t-1) was waited for), start S
         mbar_wait(bar_raw, ph_raw);
         ph_raw ^= 1;
-        for (int idx = tid; idx < (ng + 1) * 128; idx += kTcThreads) {
-            const int tau = idx & 127, g = idx >> 7;
-            const int slot = (tau & 7) * 16 + (tau >> 4) * 2 + ((tau >> 3) & 1);
-            const int off = g < ng ? M.knorm_off + 256 * g : M.vnorm_off;
-            const __half v = reinterpret_cast<const __half *>(reinterpret_cast<const unsigned char *>(raw) + off)[slot];
-            if (g < ng) kn[g * 128 + tau] = v; else vn[tau] = v;
-        }
-        __syncthreads();
+        if (tid < 128)      // V norms in token order for the V^T unpack (K norms are read from the raw rows directly)
+            vn[tid] = reinterpret_cast<const __half *>(reinterpret_cast<const unsigned char *>(raw) + M.vnorm_off)[(tid & 7) * 16 + (tid >> 4) * 2 + ((tid >> 3) & 1)];
         for (int u = warp; u < n_units; u += kTcThreads / 32) {
             const PUnit U = units[u];
+            const __half *kn = reinterpret_cast<const __half *>(reinterpret_cast<const unsigned char *>(raw) + M.knorm_off + 256 * U.group);
             switch (U.b) {
             case 1: prefill_decode_k<1, true>(raw, U, lane, pools, lut, kn, khat); break;
             case 2: prefill_decode_k<2, true>(raw, U, lane, pools, lut, kn, khat); break;

@@ -383,7 +383,8 @@ def test_cfg1_append_then_attend(P, tab128):
 
 # ----------------------------------------------------------------------------- NEXT #1: prefill attention
 @pytest.mark.parametrize("T,n_q,Hq,Hkv,bk,bv", [(40, 40, 8, 1, 3, 3), (300, 77, 16, 2, 3, 3), (333, 333, 8, 2, 2, 2),
-                                              (260, 5, 4, 1, 3, 4)])
+                                              (260, 5, 4, 1, 3, 4), (1100, 190, 8, 2, 3, 3), (515, 130, 2, 2, 4, 2),
+                                              (200, 9, 8, 1, 6, 6)])
 def test_prefill_attention_vs_oracle(P, tab128, T, n_q, Hq, Hkv, bk, bv):
     """bgtq_prefill_attention: causal attention of the last n_q tokens' queries over the packed cache
     against the oracle's plain definition, row by row."""
