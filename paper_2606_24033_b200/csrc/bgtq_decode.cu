@@ -2005,6 +2005,290 @@ prefill_tc_kernel(const PrefillParams P)
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tm), "n"(RT * 256) : "memory");
 }
 
+// ---------------------------------------------------------------- prefill, warp-specialised (two 128-row query tiles per CTA)
+// Same operands, tensor-memory map and arithmetic as prefill_tc_kernel<2>, but the three kinds of work run concurrently
+// on different warps and different pipes instead of in block-wide phases:
+//   warps 0-7   softmax: TMEM lane quadrant = warp & 3, query tile = warp >> 2; a thread owns one whole row (128 logits):
+//               no exchange between threads at all; MUFU-bound
+//   warps 8-14  producers: unpack K^ / V^T of the next tile into the operand buffers (ALU-pipe bound)
+//   warp 15     one thread issues the TMA bulk copies of the packed half tiles and the tcgen05.mma groups
+// and hand over through mbarriers (one completion per tile each; a waiter uses the parity of the tile index):
+//   kfull/vfull  TMA: [K codes|K norms] / [V norms|V codes] of tile t landed
+//   kready/vready  7 producer warps: K^ / V^T(t) written (the raw half is free again)
+//   sfull        tcgen05.commit: S(t) = Q' K^T complete (K^ is free again)
+//   sfree        8 softmax warps: S(t) has been read (S(t+1) may overwrite it)
+//   pready       8 softmax warps: P(t) written, O rescaled
+//   odone        tcgen05.commit: O += P(t) V^(t) complete (V^T and P are free again, O is stable)
+enum { WS_KFULL = 0, WS_VFULL, WS_KREADY, WS_VREADY, WS_SFULL, WS_SFREE, WS_PREADY, WS_ODONE, WS_NBARS };
+constexpr int kWsProducers = 7;
+
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(bar) : "memory");
+}
+
+__global__ void __launch_bounds__(kTcThreads, 1)
+prefill_ws_kernel(const PrefillParams P)
+{
+    constexpr int RT = 2;
+    extern __shared__ __align__(1024) unsigned char smem[];
+    __shared__ __align__(16) uint16_t lut[kLutHalves];
+    __shared__ uint32_t pools[16];
+    __shared__ __align__(8) uint64_t bars[WS_NBARS];
+    __shared__ PUnit units[2 * kMaxKSteps];
+    __shared__ int n_units_s;
+    __shared__ uint32_t tmem_base_s;
+    __shared__ __align__(16) __half vn_w[kWsProducers][128];        // V norms in token order, one private copy per producer warp
+    unsigned char *qs = smem, *khat = smem + RT * 32768, *vhat_t = khat + 32768, *ps = vhat_t + 32768;
+    uint32_t *raw = reinterpret_cast<uint32_t *>(smem + tc_operand_bytes(RT));
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int h = blockIdx.y, b = blockIdx.z, G = P.G;
+    const HeadMeta &M = P.metas[h];
+    const int TQ = RT * 128 / G;
+    int64_t slen = P.seq_len[b];
+    slen = slen > P.n_cap * kTile ? P.n_cap * kTile : slen;
+    const int i_first = blockIdx.x * TQ;
+    const int i_last = min(P.n_q, i_first + TQ) - 1;
+    const int64_t pos0 = slen - P.n_q;                              // position of query token 0
+    if (i_first >= P.n_q || pos0 < 0) return;
+    const int n_tiles = (int)((pos0 + i_last) / kTile) + 1;
+
+    build_lut(P.cb16, lut, tid, kTcThreads, true);
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" :: "r"(smem_u32(&tmem_base_s)) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    for (int i = tid; i < (32768 + 32768) / 16; i += kTcThreads) reinterpret_cast<uint4 *>(khat)[i] = make_uint4(0, 0, 0, 0);   // K^ (zero-width blocks stay 0), V^T
+    uint32_t bar[WS_NBARS];
+#pragma unroll
+    for (int i = 0; i < WS_NBARS; ++i) bar[i] = smem_u32(&bars[i]);
+    if (tid == 0) {
+        int nu = 0, j = 0;
+        for (int ks = 0; ks < M.n_ksteps; ++ks) {
+            const KStep &K = M.ksteps[ks];
+            const int g = K.flags >> 4;
+            if (K.flags & 1) j = 0;
+            units[nu++] = PUnit{K.off0, K.b, K.nc0, M.gstart[g] + 8 * j, g};
+            ++j;
+            if (K.off1 != 0xFFFF) { units[nu++] = PUnit{K.off1, K.b, K.nc1, M.gstart[g] + 8 * j, g}; ++j; }
+        }
+        n_units_s = nu;
+        mbar_init(bar[WS_KFULL], 1);
+        mbar_init(bar[WS_VFULL], 1);
+        mbar_init(bar[WS_KREADY], kWsProducers);
+        mbar_init(bar[WS_VREADY], kWsProducers);
+        mbar_init(bar[WS_SFULL], 1);
+        mbar_init(bar[WS_SFREE], 8);
+        mbar_init(bar[WS_PREADY], 8);
+        mbar_init(bar[WS_ODONE], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        fence_proxy_async();
+    }
+    {   // Q' rows -> the A operands.  Row r of the CTA = (token r / G, head r % G); rows past n_q are zero.
+        constexpr int TPR = 4 / RT, NV = 4 * RT;                    // threads per row, 16-byte vectors per thread
+        const int r = tid / TPR, part = tid % TPR;
+        const int kb = (part * 8 * NV) >> 6, j0 = ((part * 8 * NV) & 63) >> 3;
+        const int ti = i_first + r / G, n = r % G, rr = r & 127;
+        const bool valid = ti < P.n_q;
+        const uint4 *src = reinterpret_cast<const uint4 *>(P.qp + ((((size_t)b * P.n_q + (valid ? ti : 0)) * P.Hkv + h) * 8 + n) * kDh + part * 8 * NV);
+#pragma unroll
+        for (int jj = 0; jj < NV; ++jj) {
+            const uint4 v = valid ? __ldg(src + jj) : make_uint4(0, 0, 0, 0);
+            *reinterpret_cast<uint4 *>(qs + (r >> 7) * 32768 + kb * 16384 + rr * 128 + (((j0 + jj) ^ (rr & 7)) << 4)) = v;
+        }
+    }
+    fence_proxy_async();                                            // Q', zero fill -> visible to the MMA
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tm = tmem_base_s;
+    if (tid == 0) build_pools(lut, pools);
+    __syncthreads();
+    const int n_units = n_units_s, b_v = M.b_v;
+    const uint8_t *region = P.cache + P.n_cap * ((int64_t)P.batch * M.layer_prefix + (int64_t)b * M.layer_sum + M.head_prefix);
+    const uint32_t raw_s = smem_u32(raw), kbytes = M.vnorm_off, vbytes = M.tile_stride - M.vnorm_off;
+    const uint32_t qs_s = smem_u32(qs), khat_s = smem_u32(khat), vhat_s = smem_u32(vhat_t), ps_s = smem_u32(ps);
+
+    if (warp == 15) {
+        // ================= issuer: TMA + tcgen05.mma, one thread
+        if (lane == 0) {
+            mbar_expect_tx(bar[WS_KFULL], kbytes); bulk_g2s(raw_s, region, kbytes, bar[WS_KFULL]);
+            mbar_expect_tx(bar[WS_VFULL], vbytes); bulk_g2s(raw_s + kbytes, region + kbytes, vbytes, bar[WS_VFULL]);
+            for (int t = 0; t < n_tiles; ++t) {
+                const uint32_t par = t & 1, parp = (t - 1) & 1;
+                mbar_wait(bar[WS_KREADY], par);
+                if (t > 0) mbar_wait(bar[WS_SFREE], parp);
+                tc_fence_after();
+#pragma unroll
+                for (int r = 0; r < RT; ++r) umma_128x128x128(tm + r * 128, qs_s + r * 32768, khat_s, false);          // S_r = Q'_r . K^T
+                umma_commit(bar[WS_SFULL]);
+                if (t + 1 < n_tiles) {                               // the producers are done with the raw K half
+                    const uint8_t *src = region + (int64_t)(t + 1) * M.tile_stride;
+                    mbar_expect_tx(bar[WS_KFULL], kbytes); bulk_g2s(raw_s, src, kbytes, bar[WS_KFULL]);
+                }
+                mbar_wait(bar[WS_VREADY], par);
+                mbar_wait(bar[WS_PREADY], par);
+                tc_fence_after();
+#pragma unroll
+                for (int r = 0; r < RT; ++r) umma_128x128x128(tm + (RT + r) * 128, ps_s + r * 32768, vhat_s, t > 0);   // O_r (+)= P_r . V^
+                umma_commit(bar[WS_ODONE]);
+                if (t + 1 < n_tiles) {
+                    const uint8_t *src = region + (int64_t)(t + 1) * M.tile_stride + kbytes;
+                    mbar_expect_tx(bar[WS_VFULL], vbytes); bulk_g2s(raw_s + kbytes, src, vbytes, bar[WS_VFULL]);
+                }
+            }
+        }
+    } else if (warp >= 8) {
+        // ================= producers: unpack K^ and V^T of every tile
+        const int pw = warp - 8;
+        __half *vn = vn_w[pw];
+        for (int t = 0; t < n_tiles; ++t) {
+            const uint32_t par = t & 1, parp = (t - 1) & 1;
+            mbar_wait(bar[WS_KFULL], par);
+            if (t > 0) mbar_wait(bar[WS_SFULL], parp);               // S(t-1) has consumed K^
+            for (int u = pw; u < n_units; u += kWsProducers) {
+                const PUnit U = units[u];
+                const __half *kn = reinterpret_cast<const __half *>(reinterpret_cast<const unsigned char *>(raw) + M.knorm_off + 256 * U.group);
+                switch (U.b) {
+                case 1: prefill_decode_k<1, true>(raw, U, lane, pools, lut, kn, khat); break;
+                case 2: prefill_decode_k<2, true>(raw, U, lane, pools, lut, kn, khat); break;
+                case 3: prefill_decode_k<3, true>(raw, U, lane, pools, lut, kn, khat); break;
+                case 4: prefill_decode_k<4, true>(raw, U, lane, pools, lut, kn, khat); break;
+                case 5: prefill_decode_k<5, true>(raw, U, lane, pools, lut, kn, khat); break;
+                case 6: prefill_decode_k<6, true>(raw, U, lane, pools, lut, kn, khat); break;
+                case 7: prefill_decode_k<7, true>(raw, U, lane, pools, lut, kn, khat); break;
+                default: prefill_decode_k<8, true>(raw, U, lane, pools, lut, kn, khat); break;
+                }
+            }
+            fence_proxy_async();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar[WS_KREADY]);
+            mbar_wait(bar[WS_VFULL], par);
+            if (t > 0) mbar_wait(bar[WS_ODONE], parp);               // PV(t-1) has consumed V^T
+            {
+                const __half *rv = reinterpret_cast<const __half *>(reinterpret_cast<const unsigned char *>(raw) + M.vnorm_off);
+#pragma unroll
+                for (int q4 = 0; q4 < 4; ++q4) {
+                    const int tau = 32 * q4 + lane;
+                    vn[tau] = rv[(tau & 7) * 16 + (tau >> 4) * 2 + ((tau >> 3) & 1)];
+                }
+                __syncwarp();
+                const uint32_t *vcodes = raw + (M.vcode_off >> 2);
+                for (int v = pw; v < 16; v += kWsProducers) {
+                    switch (b_v) {
+                    case 1: prefill_decode_v<1, true>(vcodes, v >> 1, lane, pools, lut, vn, vhat_t, v & 1); break;
+                    case 2: prefill_decode_v<2, true>(vcodes, v >> 1, lane, pools, lut, vn, vhat_t, v & 1); break;
+                    case 3: prefill_decode_v<3, true>(vcodes, v >> 1, lane, pools, lut, vn, vhat_t, v & 1); break;
+                    case 4: prefill_decode_v<4, true>(vcodes, v >> 1, lane, pools, lut, vn, vhat_t, v & 1); break;
+                    case 5: prefill_decode_v<5, true>(vcodes, v >> 1, lane, pools, lut, vn, vhat_t, v & 1); break;
+                    case 6: prefill_decode_v<6, true>(vcodes, v >> 1, lane, pools, lut, vn, vhat_t, v & 1); break;
+                    case 7: prefill_decode_v<7, true>(vcodes, v >> 1, lane, pools, lut, vn, vhat_t, v & 1); break;
+                    default: prefill_decode_v<8, true>(vcodes, v >> 1, lane, pools, lut, vn, vhat_t, v & 1); break;
+                    }
+                }
+            }
+            fence_proxy_async();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar[WS_VREADY]);
+        }
+    } else {
+        // ================= softmax: one thread per query row
+        const int quad = warp & 3, rt = warp >> 2;
+        const int row = 32 * quad + lane, crow = rt * 128 + row;
+        const int64_t prow = pos0 + i_first + crow / G;             // position of this row's query token
+        const uint32_t t_s = tm + ((uint32_t)(32 * quad) << 16) + (uint32_t)(rt * 128), t_o = t_s + RT * 128u;
+        unsigned char *prow_s = ps + rt * 32768 + row * 128;
+        float m_run = -INFINITY, l_run = 0.f;
+        for (int t = 0; t < n_tiles; ++t) {
+            const uint32_t par = t & 1, parp = (t - 1) & 1;
+            mbar_wait(bar[WS_SFULL], par);
+            tc_fence_after();
+            const int rel = (int)max((int64_t)-1, min((int64_t)1 << 20, prow - (int64_t)t * kTile));   // columns > rel are in the future
+            const bool nomask = __all_sync(0xFFFFFFFFu, rel >= 127);
+            float mx = -INFINITY;
+#pragma unroll
+            for (int ch = 0; ch < 4; ++ch) {
+                uint32_t sr[32];
+                tmem_ld32(t_s + 32 * ch, sr);
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                if (nomask) {
+#pragma unroll
+                    for (int i = 0; i < 32; i += 2) mx = fmax3(mx, __uint_as_float(sr[i]), __uint_as_float(sr[i + 1]));
+                } else {
+#pragma unroll
+                    for (int i = 0; i < 32; ++i) mx = fmaxf(mx, 32 * ch + i > rel ? -INFINITY : __uint_as_float(sr[i]));
+                }
+            }
+            const float mn = fmaxf(m_run, mx);                       // finite: tile 0 holds position 0
+            const float alpha = fast_exp2(m_run - mn);
+            m_run = mn;
+            if (t > 0) { mbar_wait(bar[WS_ODONE], parp); tc_fence_after(); }    // PV(t-1) has consumed P; O is stable
+            float ls = 0.f;
+#pragma unroll
+            for (int ch = 0; ch < 4; ++ch) {
+                uint32_t sr[32];
+                tmem_ld32(t_s + 32 * ch, sr);
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {                        // 8 tokens = one 16-byte chunk of the P row
+                    float p[8];
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) {
+                        const int i = 32 * ch + 8 * j + e;
+                        p[e] = (!nomask && i > rel) ? 0.f : fast_exp2(__uint_as_float(sr[8 * j + e]) - mn);
+                        ls += p[e];
+                    }
+                    const uint4 v = make_uint4(pack_half2(p[0], p[1]), pack_half2(p[2], p[3]), pack_half2(p[4], p[5]), pack_half2(p[6], p[7]));
+                    const int col = 32 * ch + 8 * j;
+                    *reinterpret_cast<uint4 *>(prow_s + (col >> 6) * 16384 + ((((col & 63) >> 3) ^ (row & 7)) << 4)) = v;
+                }
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar[WS_SFREE]);               // S(t+1) may be issued while O is rescaled
+            l_run = fmaf(l_run, alpha, ls);
+            if (t > 0 && __any_sync(0xFFFFFFFFu, alpha != 1.f)) {    // a row maximum moved: rescale O in place
+#pragma unroll
+                for (int ch = 0; ch < 4; ++ch) {
+                    uint32_t o[32];
+                    tmem_ld32(t_o + 32 * ch, o);
+                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+                    for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
+                    tmem_st32(t_o + 32 * ch, o);
+                }
+                asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+            }
+            fence_proxy_async();                                     // P -> visible to the MMA
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar[WS_PREADY]);
+        }
+        // ---- normalise and store the rotated-domain output rows (fp32); derotate_kernel finishes them
+        mbar_wait(bar[WS_ODONE], (n_tiles - 1) & 1);
+        tc_fence_after();
+        const float inv = 1.f / l_run;
+        const int ti = i_first + crow / G, n = crow % G;
+#pragma unroll
+        for (int ch = 0; ch < 4; ++ch) {
+            uint32_t o[32];
+            tmem_ld32(t_o + 32 * ch, o);
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+            if (ti < P.n_q) {
+                float4 *dst = reinterpret_cast<float4 *>(P.opart + (((size_t)b * P.n_q + ti) * (P.Hkv * G) + h * G + n) * kDh + 32 * ch);
+#pragma unroll
+                for (int i = 0; i < 8; ++i)
+                    dst[i] = make_float4(__uint_as_float(o[4 * i]) * inv, __uint_as_float(o[4 * i + 1]) * inv,
+                                         __uint_as_float(o[4 * i + 2]) * inv, __uint_as_float(o[4 * i + 3]) * inv);
+            }
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" :: "r"(tm) : "memory");
+}
+
 // out[row][k] = sum_j Pi^(128)[j][k] * o'[row][j] / sqrt(128)  ->  bf16  (the V de-rotation, once per output row)
 __global__ void __launch_bounds__(128)
 derotate_kernel(const float *__restrict__ opart, const float *__restrict__ rot128, int64_t n_rows,
@@ -2062,6 +2346,7 @@ int launch_prefill(const bgtq_layout *lay, int layer, const void *cache, const v
         CUDA_TRY(cudaFuncSetAttribute(prefill_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 65536 + 40 * 1024));
         CUDA_TRY(cudaFuncSetAttribute(prefill_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc_operand_bytes(1) + 40 * 1024));
         CUDA_TRY(cudaFuncSetAttribute(prefill_tc_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 13 * 1024));
+        CUDA_TRY(cudaFuncSetAttribute(prefill_ws_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 13 * 1024));
         attr_set = true;
     }
     PrefillParams P;
@@ -2070,7 +2355,10 @@ int launch_prefill(const bgtq_layout *lay, int layer, const void *cache, const v
     P.raw_bytes = raw_bytes;
     const int TQ = (use_tc ? RT * 128 : 128) / G;
     dim3 grid((n_q + TQ - 1) / TQ, Hkv, batch);
+    static int use_ws = -1;                         // BGTQ_PREFILL_WS=0 selects the phase-synchronous tcgen05 kernel
+    if (use_ws < 0) { const char *e = getenv("BGTQ_PREFILL_WS"); use_ws = (e && atoi(e) == 0) ? 0 : 1; }
     if (!use_tc) prefill_kernel<<<grid, 256, smem, st>>>(P);
+    else if (RT == 2 && use_ws) prefill_ws_kernel<<<grid, kTcThreads, smem, st>>>(P);
     else if (RT == 2) prefill_tc_kernel<2><<<grid, kTcThreads, smem, st>>>(P);
     else prefill_tc_kernel<1><<<grid, kTcThreads, smem, st>>>(P);
     count_launch();
