@@ -400,6 +400,37 @@ def decode_attention_head(q_post: np.ndarray, qh: QuantizedHead, tab: Tables, d_
     return np.stack([attention(q_post[a], K, V, scale) for a in range(q_post.shape[0])])
 
 
+def protected_sets(T: int, n_sink: int, n_recent: int) -> Tuple[np.ndarray, np.ndarray]:
+    """Token index sets of the *protected-buffer* regime: the cache is
+    [sink (fp16) | compressed | recent (fp16)] with the first n_sink tokens and the most recent n_recent
+    tokens kept as fp16.  Returns (protected, compressed) index arrays over tokens 0..T-1 (disjoint, covering);
+    a token that is both among the first n_sink and the last n_recent is protected once."""
+    t = np.arange(T)
+    prot = (t < n_sink) | (t >= T - n_recent)
+    return t[prot], t[~prot]
+
+
+def window_slot(t: int, n_sink: int, n_recent: int) -> int:
+    """Slot of token t in the fp16 window buffer of n_sink + n_recent rows: the sink tokens keep
+    slots 0..n_sink-1, every later token t lives in the ring slot n_sink + (t mod n_recent) while it is recent."""
+    return t if t < n_sink else n_sink + (t % n_recent)
+
+
+def decode_attention_protected_head(q_post: np.ndarray, qh: QuantizedHead, tab: Tables, d_h: int, scale: float,
+                                    k16: np.ndarray, v16: np.ndarray, n_sink: int, n_recent: int) -> np.ndarray:
+    """Decode attention in the protected regime, the plain definition: one exact softmax
+    over ALL T cached tokens, where a protected token contributes its fp16 key / value row (k16, v16 [T, d_h]: the
+    exact post-RoPE rows rounded to fp16 by the caller) and every other token its dequantised packed row.
+    n_sink = n_recent = 0 is decode_attention_head (the paper's buffer-free packed path)."""
+    K, V = dequantize_head(qh, tab, d_h)
+    T = K.shape[0]
+    prot, _ = protected_sets(T, n_sink, n_recent)
+    K = K.copy(); V = V.copy()
+    K[prot] = _c64(k16)[prot]
+    V[prot] = _c64(v16)[prot]
+    return np.stack([attention(q_post[a], K, V, scale) for a in range(q_post.shape[0])])
+
+
 def prefill_attention_head(q_post: np.ndarray, qh: QuantizedHead, tab: Tables, d_h: int, scale: float,
                            pos0: int) -> np.ndarray:
     """Causal prefill attention over the (fully dequantised) packed cache: query token i of the

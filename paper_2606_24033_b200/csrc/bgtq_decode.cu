@@ -1190,11 +1190,12 @@ fp16_decode_kernel(const Fp16Params P)
 static int pick_warps(int buf_bytes)
 {
     const int avail = 227 * 1024 - kStaticSmem;
-    const int cands[6] = {16, 14, 13, 12, 8, 4};
-    int cap = 12;   // measured: 16 warps at 128 registers (spills, no pair table) is slower than 12 at 168
+    const int cands[4] = {16, 12, 8, 4};
+    int cap = 12;   // measured: 16 warps at 128 registers (spills, no pair table) is slower than 12 at 168; 13 / 14 warps
+                    // (152 / 144 registers, small spills, uneven schedulers) run at 545 / 514 us against 429 us
     if (const char *e = getenv("BGTQ_DECODE_WARPS")) cap = atoi(e);   // tuning knob (warps per CTA upper bound)
     if (cap >= 16 && (size_t)16 * buf_bytes <= (size_t)(227 * 1024 - 2560)) return 16;   // W = 16 runs without the pair table
-    for (int i = 0; i < 6; ++i)
+    for (int i = 0; i < 4; ++i)
         if (cands[i] <= cap && (size_t)cands[i] * buf_bytes <= (size_t)avail) return cands[i];
     return 0;
 }
@@ -1304,8 +1305,6 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
     if (pm) {
         switch (W) {
         case 16: rc = launch_decode_w<16, true>(P, grid, smem, st); break;
-        case 14: rc = launch_decode_w<14, true>(P, grid, smem, st); break;
-        case 13: rc = launch_decode_w<13, true>(P, grid, smem, st); break;
         case 12: rc = launch_decode_w<12, true>(P, grid, smem, st); break;
         case 8: rc = launch_decode_w<8, true>(P, grid, smem, st); break;
         default: rc = launch_decode_w<4, true>(P, grid, smem, st); break;
@@ -1313,8 +1312,6 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
     } else {
         switch (W) {
         case 16: rc = launch_decode_w<16, false>(P, grid, smem, st); break;
-        case 14: rc = launch_decode_w<14, false>(P, grid, smem, st); break;
-        case 13: rc = launch_decode_w<13, false>(P, grid, smem, st); break;
         case 12: rc = launch_decode_w<12, false>(P, grid, smem, st); break;
         case 8: rc = launch_decode_w<8, false>(P, grid, smem, st); break;
         default: rc = launch_decode_w<4, false>(P, grid, smem, st); break;

@@ -226,3 +226,64 @@ def test_prefill_oracle_rows_are_decode_steps(tab128):
             assert np.allclose(out[i, a], O.attention(q[i, a], K[:i + 1], V[:i + 1], 0.1), atol=1e-12)
     out2 = O.prefill_attention_head(q[30:], head, tab128, d, 0.1, 30)        # a later chunk of the same sequence
     assert np.allclose(out2, out[30:], atol=1e-12)
+
+
+# ----------------------------------------------------------------------------- protected regime (PAPER.md:286, 813-815)
+def _protected_case(tab128, T, seed=21):
+    rng = np.random.default_rng(seed)
+    d = 128
+    k = rng.standard_normal((T, d)) * np.repeat(np.exp(rng.uniform(-2, 1, 64)), 2)
+    v = rng.standard_normal((T, d))
+    bits = np.array([3] * 64, dtype=np.uint8); bits[:10] = 5; bits[10:25] = 1; bits[25:30] = 4; bits[30:35] = 2
+    head = O.quantize_head(k, v, bits, 2, tab128)                       # K3V2, the AIME budget (PAPER.md:813)
+    k16 = k.astype(np.float16).astype(np.float64)
+    v16 = v.astype(np.float16).astype(np.float64)
+    q = rng.standard_normal((2, d))
+    return head, k16, v16, q, d
+
+
+def test_protected_sets_partition_and_ring_slots():
+    """[sink | compressed | recent] (PAPER.md:813): the sets partition 0..T-1; short sequences are all protected;
+    the ring slot of every currently-recent token is unique and inside the buffer."""
+    for T, ns, nr in [(300, 4, 128), (132, 4, 128), (133, 4, 128), (100, 4, 128), (3, 4, 128), (300, 0, 0), (300, 0, 7), (300, 5, 0)]:
+        prot, comp = O.protected_sets(T, ns, nr)
+        assert sorted(np.concatenate([prot, comp]).tolist()) == list(range(T))
+        assert len(comp) == max(0, T - ns - nr)
+        if len(comp):
+            assert comp[0] == ns and comp[-1] == T - nr - 1
+        slots = [O.window_slot(int(t), ns, nr) for t in prot]
+        assert len(set(slots)) == len(slots) and all(0 <= s < ns + nr for s in slots)
+
+
+def test_protected_attention_limits_and_three_way_merge(tab128):
+    """n_sink = n_recent = 0 is the buffer-free packed path; a window covering every token is textbook softmax attention
+    over the fp16 rows (scipy); in between, the result equals the exact LSE merge of the three segments
+    computed separately -- which is how the GPU evaluates it."""
+    T = 300
+    head, k16, v16, q, d = _protected_case(tab128, T)
+    scale = 1 / math.sqrt(d)
+    none = O.decode_attention_protected_head(q, head, tab128, d, scale, k16, v16, 0, 0)
+    assert np.array_equal(none, O.decode_attention_head(q, head, tab128, d, scale))
+    full = O.decode_attention_protected_head(q, head, tab128, d, scale, k16, v16, 4, T)
+    for a in range(2):
+        assert np.allclose(full[a], scipy_softmax(scale * (k16 @ q[a])) @ v16, rtol=1e-12, atol=1e-14)
+    out = O.decode_attention_protected_head(q, head, tab128, d, scale, k16, v16, 4, 128)
+    K, V = O.dequantize_head(head, tab128, d)
+    for a in range(2):
+        parts = [O.attention_partial(q[a], k16[:4], v16[:4], scale),
+                 O.attention_partial(q[a], K[4:T - 128], V[4:T - 128], scale),
+                 O.attention_partial(q[a], k16[T - 128:], v16[T - 128:], scale)]
+        assert np.allclose(O.merge_partials(parts), out[a], rtol=1e-12, atol=1e-14)
+    # it really differs from both limits, and protecting tokens moves the output towards the unquantised one
+    exact = np.stack([O.attention(q[a], k16, v16, scale) for a in range(2)])
+    assert np.max(np.abs(out - none)) > 1e-4
+    assert np.linalg.norm(out - exact) < np.linalg.norm(none - exact)
+
+
+def test_protected_attention_short_sequences(tab128):
+    """T <= n_sink + n_recent: nothing is served from the compressed cache."""
+    for T in (1, 3, 100, 132):
+        head, k16, v16, q, d = _protected_case(tab128, T, seed=T)
+        out = O.decode_attention_protected_head(q, head, tab128, d, 0.1, k16, v16, 4, 128)
+        for a in range(2):
+            assert np.allclose(out[a], scipy_softmax(0.1 * (k16 @ q[a])) @ v16, rtol=1e-12, atol=1e-14)
