@@ -145,6 +145,32 @@ int bgtq_decode_attention_layers(const bgtq_layout *layout, int layer0, int n_la
                                  int batch, int64_t max_tokens, float softmax_scale, void *out,
                                  void *workspace, size_t workspace_bytes, void *stream);
 
+/* ---- SURVEY.md 8(f).4 "protected windows": decode attention in the paper's *protected-buffer* regime,
+ * the cache is [sink (fp16) | compressed | recent (fp16)] -- the first n_sink tokens and
+ * the most recent n_recent tokens of every sequence are attended from fp16 rows, every other token from the
+ * packed cache; one exact softmax over all seq_len[s] tokens (the three parts are merged by the same
+ * log-sum-exp rule as the key-axis splits).  The paper uses n_sink = 4, n_recent = 128.
+ * win_k, win_v [device] fp16 [n_layers_of_the_layout, batch, n_kv_heads, n_sink + n_recent, d_h]
+ *   (bgtq_window_bytes each): slot j < n_sink holds token j (post-RoPE key / value), slot
+ *   n_sink + (t mod n_recent) holds token t >= n_sink while it is among the last n_recent.  The windows of
+ *   layers [layer0, layer0 + n_layers) are read.  The packed cache still holds EVERY token (append quantises
+ *   as usual); its tokens outside [n_sink, seq_len - n_recent) are skipped / masked, never read as keys.
+ * Limits: 0 <= n_sink < 128, n_recent >= 0, 1 <= n_sink + n_recent <= 1024 (else BGTQ_EINVAL; use
+ *   bgtq_decode_attention_layers for the buffer-free path).  Everything else as bgtq_decode_attention_layers.
+ * bgtq_window_append: fp16 copies (round-to-nearest-even) of the n_new tokens the matching
+ *   bgtq_quantize_append_layers call stores at positions seq_len[s] .. seq_len[s] + n_new - 1, written to their
+ *   window slots; call it BEFORE that append advances seq_len.  k_new (post-RoPE), v_new, dt, batch, n_new as
+ *   there.  Caller owns all buffers. */
+size_t bgtq_window_bytes(const bgtq_layout *layout, int batch, int n_sink, int n_recent);
+int bgtq_window_append(const bgtq_layout *layout, int layer0, int n_layers, const void *k_new,
+                       const void *v_new, int dt, int batch, int n_new, const int32_t *seq_len,
+                       void *win_k, void *win_v, int n_sink, int n_recent, void *stream);
+int bgtq_decode_attention_protected(const bgtq_layout *layout, int layer0, int n_layers, const void *cache,
+                                    const void *q, const int32_t *seq_len, int batch, int64_t max_tokens,
+                                    float softmax_scale, const void *win_k, const void *win_v, int n_sink,
+                                    int n_recent, void *out, void *workspace, size_t workspace_bytes,
+                                    void *stream);
+
 /* ---- SURVEY.md 8(f).4 "RoPE fused into append": bgtq_quantize_append_layers on PRE-RoPE keys.
  * k_pre [device] [n_layers, batch, n_new, n_kv_heads, d_h] of dtype dt; the token stored at cache position
  * t is first rotated block by block (the layout's pairing):

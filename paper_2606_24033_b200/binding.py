@@ -31,6 +31,7 @@ SYMBOLS = [
     "bgtq_prefill_workspace_bytes", "bgtq_prefill_attention", "bgtq_fp16_workspace_bytes", "bgtq_fp16_decode_attention", "bgtq_debug_decode_unit", "bgtq_launch_count",
     "bgtq_paged_cache_bytes", "bgtq_paged_pool_offset", "bgtq_quantize_append_paged", "bgtq_decode_attention_paged",
     "bgtq_quantize_append_rope",
+    "bgtq_window_bytes", "bgtq_window_append", "bgtq_decode_attention_protected",
 ]
 
 
@@ -103,6 +104,12 @@ def _load() -> C.CDLL:
     lib.bgtq_quantize_append_paged.argtypes = [vp, i32, i32, vp, vp, vp, i32, i32, i32, vp, i32, vp, i32, i64, vp]
     lib.bgtq_quantize_append_rope.restype = i32
     lib.bgtq_quantize_append_rope.argtypes = [vp, i32, i32, vp, vp, vp, i32, i32, i32, vp, i32, i64, vp, vp, i64, vp]
+    lib.bgtq_window_bytes.restype = sz
+    lib.bgtq_window_bytes.argtypes = [vp, i32, i32, i32]
+    lib.bgtq_window_append.restype = i32
+    lib.bgtq_window_append.argtypes = [vp, i32, i32, vp, vp, i32, i32, i32, vp, vp, vp, i32, i32, vp]
+    lib.bgtq_decode_attention_protected.restype = i32
+    lib.bgtq_decode_attention_protected.argtypes = [vp, i32, i32, vp, vp, vp, i32, i64, f32, vp, vp, i32, i32, vp, vp, sz, vp]
     lib.bgtq_decode_attention_paged.restype = i32
     lib.bgtq_decode_attention_paged.argtypes = [vp, i32, i32, vp, vp, vp, i32, vp, i32, i64, f32, vp, vp, sz, vp]
     return lib
@@ -339,6 +346,43 @@ def decode_attention(layout: Layout, layer: int, cache: torch.Tensor, q: torch.T
                                              _dev(q, torch.bfloat16), _dev(seq_len, torch.int32), batch,
                                              max_tokens, float(softmax_scale), _dev(out, torch.bfloat16),
                                              _dev(workspace, torch.uint8), workspace.numel(), _stream()))
+    return out
+
+
+def new_windows(layout: Layout, batch: int, n_sink: int, n_recent: int, device="cuda"):
+    """Zeroed fp16 window buffers (win_k, win_v) [n_layers, batch, H_kv, n_sink + n_recent, d_h] (bgtq_window_bytes each)."""
+    shape = (layout.n_layers, batch, layout.n_kv_heads, n_sink + n_recent, layout.d_h)
+    assert int(_lib.bgtq_window_bytes(layout._h, batch, n_sink, n_recent)) == int(np.prod(shape)) * 2
+    return torch.zeros(shape, dtype=torch.float16, device=device), torch.zeros(shape, dtype=torch.float16, device=device)
+
+
+def window_append(layout: Layout, layer: int, k_new: torch.Tensor, v_new: torch.Tensor, seq_len: torch.Tensor,
+                  win_k: torch.Tensor, win_v: torch.Tensor, n_sink: int, n_recent: int, n_layers: int = 1) -> None:
+    """bgtq_window_append: k_new, v_new [batch, n_new, H_kv, d_h] (n_layers = 1) or [n_layers, batch, n_new, H_kv, d_h];
+    call before the quantize_append that advances seq_len."""
+    batch, n_new, Hkv, d = k_new.shape[-4:]
+    assert v_new.shape == k_new.shape and Hkv == layout.n_kv_heads and d == layout.d_h and _dt(k_new) == _dt(v_new)
+    assert k_new.dim() == 4 or k_new.shape[0] == n_layers
+    _check(_lib.bgtq_window_append(layout._h, layer, n_layers, _dev(k_new), _dev(v_new), _dt(k_new), batch, n_new,
+                                   _dev(seq_len, torch.int32), _dev(win_k, torch.float16), _dev(win_v, torch.float16),
+                                   n_sink, n_recent, _stream()))
+
+
+def decode_attention_protected(layout: Layout, layer: int, cache: torch.Tensor, q: torch.Tensor, seq_len: torch.Tensor,
+                               max_tokens: int, softmax_scale: float, win_k: torch.Tensor, win_v: torch.Tensor,
+                               n_sink: int, n_recent: int, workspace: torch.Tensor,
+                               out: Optional[torch.Tensor] = None, n_layers: int = 1) -> torch.Tensor:
+    """bgtq_decode_attention_protected: q bf16 [batch, H_q, d_h] (n_layers = 1) or [n_layers, batch, H_q, d_h]."""
+    if out is None:
+        out = torch.empty_like(q)
+    batch = q.shape[-3]
+    assert q.shape[-2] == layout.n_q_heads and q.shape[-1] == layout.d_h
+    assert q.dim() == 3 or q.shape[0] == n_layers
+    _check(_lib.bgtq_decode_attention_protected(layout._h, layer, n_layers, _dev(cache, torch.uint8), _dev(q, torch.bfloat16),
+                                                _dev(seq_len, torch.int32), batch, max_tokens, float(softmax_scale),
+                                                _dev(win_k, torch.float16), _dev(win_v, torch.float16), n_sink, n_recent,
+                                                _dev(out, torch.bfloat16), _dev(workspace, torch.uint8), workspace.numel(),
+                                                _stream()))
     return out
 
 

@@ -261,7 +261,16 @@ __device__ __forceinline__ int warp_lo(const Sched &s, int c, int w)
     return lo + (int)(((int64_t)w * len) / s.W);
 }
 
-__device__ __forceinline__ void build_prefix(const int32_t *seq_len, int batch, int64_t cap_tokens, int *pre)
+// Protected regime: of the T cached tokens of a sequence the packed cache serves
+// [n_sink, T - n_recent) only -- the first n_sink and the last n_recent tokens are attended from fp16 windows by
+// window_kernel.  Number of packed tokens to scan (tokens below n_sink are masked inside tile 0); 0 when the range is empty.
+__device__ __forceinline__ int64_t packed_len(int64_t T, int n_sink, int n_recent)
+{
+    const int64_t hi = T - n_recent;
+    return hi > n_sink ? hi : 0;
+}
+__device__ __forceinline__ void build_prefix(const int32_t *seq_len, int batch, int64_t cap_tokens, int *pre,
+                                             int n_sink = 0, int n_recent = 0)
 {
     // called by one thread; batch <= kMaxBatch
     int acc = 0;
@@ -269,6 +278,7 @@ __device__ __forceinline__ void build_prefix(const int32_t *seq_len, int batch, 
     for (int b = 0; b < batch; ++b) {
         int64_t n = seq_len[b];
         n = n < 0 ? 0 : (n > cap_tokens ? cap_tokens : n);
+        n = packed_len(n, n_sink, n_recent);
         acc += (int)((n + kTile - 1) / kTile);
         pre[b + 1] = acc;
     }
@@ -396,6 +406,7 @@ struct DecodeParams {
     const int32_t *pages;       // paged cache: [batch][pstride] page index per tile (nullptr: contiguous layout)
     int pstride;
     int64_t n_pages;
+    int n_sink, n_recent;       // protected regime: packed tokens [n_sink, T - n_recent) only (0, 0 = the buffer-free path)
 };
 
 constexpr int kSmemHdr = 0;      // dynamic shared memory holds only the tile buffers (tables are static)
@@ -561,7 +572,7 @@ decode_kernel(const DecodeParams P)
     auto TS = [&](int) {};
 #endif
     build_lut(P.cb16, lut, tid, W * 32, P5);
-    if (tid == 0) build_prefix(P.seq_len, P.batch, P.n_cap * kTile, pre);
+    if (tid == 0) build_prefix(P.seq_len, P.batch, P.n_cap * kTile, pre, P.n_sink, P.n_recent);
     if (PARK && warp == 0) {                                      // 4 warps per lane quadrant x 32 columns
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 128;" :: "r"(smem_u32(&tmem_base_s)) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
@@ -640,6 +651,7 @@ decode_kernel(const DecodeParams P)
         const int knorm_off = M.knorm_off, vnorm_off = M.vnorm_off, vcode_off = M.vcode_off;
         int64_t slen = P.seq_len[tp.b];
         slen = slen > P.n_cap * kTile ? P.n_cap * kTile : slen;
+        slen = packed_len(slen, P.n_sink, P.n_recent);
         // lane g keeps the descriptor of group g: code offset | m << 16 | b << 24 | first k-step << 28
         uint32_t gdesc = 0;
         if (lane < n_groups) {
@@ -732,11 +744,13 @@ decode_kernel(const DecodeParams P)
             TS(5);
             // ======== mask the ragged tail, online softmax (log2 domain)
             const int n_valid = (int)min((int64_t)kTile, slen - (int64_t)t * kTile);
-            if (n_valid < kTile) {
+            const int n_low = t == 0 ? P.n_sink : 0;           // sink tokens are served by the fp16 window (tile 0 only)
+            if (n_valid < kTile || n_low > 0) {
 #pragma unroll
                 for (int i = 0; i < 8; ++i) {
-                    if (16 * i + g8 >= n_valid) Sc[i][0] = Sc[i][1] = -INFINITY;
-                    if (16 * i + 8 + g8 >= n_valid) Sc[i][2] = Sc[i][3] = -INFINITY;
+                    const int r0 = 16 * i + g8, r1 = r0 + 8;
+                    if (r0 >= n_valid || r0 < n_low) Sc[i][0] = Sc[i][1] = -INFINITY;
+                    if (r1 >= n_valid || r1 < n_low) Sc[i][2] = Sc[i][3] = -INFINITY;
                 }
             }
             float mx0 = -INFINITY, mx1 = -INFINITY;
@@ -874,7 +888,7 @@ decode_kernel(const DecodeParams P)
 __global__ void __launch_bounds__(128)
 combine_kernel(const float *__restrict__ partials, const int32_t *__restrict__ seq_len,
                const float *__restrict__ rot128, int n_layers, int batch, int Hkv, int G, int64_t n_cap,
-               int n_ctas, int W, __nv_bfloat16 *__restrict__ out)
+               int n_ctas, int W, __nv_bfloat16 *__restrict__ out, int n_sink = 0, int n_recent = 0, int win_slot = -1)
 {
     constexpr int kMaxSlots = 1024;                     // 32 + n_ctas entries at most (host checks n_ctas)
     __shared__ int pre[kMaxBatch + 1];
@@ -886,19 +900,25 @@ combine_kernel(const float *__restrict__ partials, const int32_t *__restrict__ s
     const int pair = blockIdx.x / G, n = blockIdx.x % G;
     const int h = pair % Hkv, lb = pair / Hkv, b = lb % batch, l = lb / batch;
     const int d = threadIdx.x, lane = d & 31, wq = d >> 5;
-    if (d == 0) build_prefix(seq_len, batch, n_cap * kTile, pre);
+    if (d == 0) build_prefix(seq_len, batch, n_cap * kTile, pre, n_sink, n_recent);
     __syncthreads();
     const Sched S = make_sched(n_layers, batch, Hkv, pre, n_ctas, W);
     const int tiles_b = pre[b + 1] - pre[b];
     __nv_bfloat16 *dst = out + ((size_t)lb * Hkv * G + h * G + n) * kDh;
-    if (tiles_b == 0) { dst[d] = __float2bfloat16(0.f); return; }
+    // protected regime: one more record per pair, written by window_kernel at slot win_slot (relative to the pair's
+    // base, like every slot below); it exists whenever the sequence is not empty
+    const bool has_win = win_slot >= 0 && seq_len[b] > 0;
+    if (tiles_b == 0 && !has_win) { dst[d] = __float2bfloat16(0.f); return; }
     const int start = l * (Hkv * S.tiles_sum) + pre[b] * Hkv + h * tiles_b, stop = start + tiles_b;
     // CTAs whose range meets [start, stop): the decode kernel's balanced split, recomputed
-    int c0 = (int)(((int64_t)start * S.n_ctas) / S.total), c1 = (int)(((int64_t)(stop - 1) * S.n_ctas) / S.total);
-    while (c0 + 1 < S.n_ctas && cta_lo(S, c0 + 1) <= start) ++c0;
-    while (c0 > 0 && cta_lo(S, c0) > start) --c0;
-    while (c1 + 1 < S.n_ctas && cta_lo(S, c1 + 1) <= stop - 1) ++c1;
-    while (c1 > 0 && cta_lo(S, c1) > stop - 1) --c1;
+    int c0 = 0, c1 = 0;
+    if (tiles_b > 0) {
+        c0 = (int)(((int64_t)start * S.n_ctas) / S.total); c1 = (int)(((int64_t)(stop - 1) * S.n_ctas) / S.total);
+        while (c0 + 1 < S.n_ctas && cta_lo(S, c0 + 1) <= start) ++c0;
+        while (c0 > 0 && cta_lo(S, c0) > start) --c0;
+        while (c1 + 1 < S.n_ctas && cta_lo(S, c1 + 1) <= stop - 1) ++c1;
+        while (c1 > 0 && cta_lo(S, c1) > stop - 1) --c1;
+    }
     // slot list in a fixed order: [warps of the first CTA][interior CTAs][warps of the last CTA].  Interior
     // CTAs lie wholly inside the pair, so they merged their warps (one record at the slot of warp 0); a CTA
     // straddling the pair boundary left one record per warp.
@@ -911,14 +931,16 @@ combine_kernel(const float *__restrict__ partials, const int32_t *__restrict__ s
         return (wl < wh && wl < stop && wh > start) ? c * W + w : -1;
     };
     const int n_int = c1 - c0 - 1 > 0 ? c1 - c0 - 1 : 0;
-    const int n_ent = min(kMaxSlots, 16 + n_int + (c1 > c0 ? 16 : 0));
+    const int n_pk = tiles_b > 0 ? min(kMaxSlots - 1, 16 + n_int + (c1 > c0 ? 16 : 0)) : 0;   // records of the packed range
+    const int n_ent = n_pk + (has_win ? 1 : 0);
     pdl_wait();                                         // the decode kernel's partials are complete from here on
     // pass 1: every record's running max -> M, then its weight 2^(m - M) and the merged sum l.  All loads are
     // independent (one record per thread), and the order of every reduction is fixed, so the result does not depend
     // on timing.
     float mloc = -INFINITY;
     for (int e = d; e < n_ent; e += 128) {
-        const int sl = e < 16 ? edge_slot(c0, e) : (e < 16 + n_int ? edge_slot(c0 + 1 + e - 16, 0) : edge_slot(c1, e - 16 - n_int));
+        const int sl = e >= n_pk ? win_slot
+                     : e < 16 ? edge_slot(c0, e) : (e < 16 + n_int ? edge_slot(c0 + 1 + e - 16, 0) : edge_slot(c1, e - 16 - n_int));
         slots[e] = sl;
         const float mw = sl < 0 ? -INFINITY : rec0[(size_t)sl * kPartialFloats];
         wgt[e] = mw;
@@ -962,6 +984,106 @@ combine_kernel(const float *__restrict__ partials, const int32_t *__restrict__ s
 #pragma unroll 32
     for (int j = 0; j < kDh; ++j) r = fmaf(__ldg(rot128 + j * kDh + d), o[j], r);
     dst[d] = __float2bfloat16(r * 0.08838834764831845f);     // 1/sqrt(128)
+}
+
+// ---------------------------------------------------------------- protected regime: fp16 sink / recent windows
+// PAPER.md:286, 813-815 "[sink (fp16) | compressed | recent (fp16)]".  win_k, win_v: fp16
+// [layer][sequence][kv head][n_sink + n_recent][128]; slot j < n_sink holds token j, slot n_sink + (t mod n_recent)
+// holds token t >= n_sink while it is among the last n_recent (a ring: attention does not depend on the order).
+// One CTA per (pair, query head) attends over the valid slots and leaves ONE partial record in the decode kernel's
+// format -- running max and sum in the log2 domain, accumulator in the rotated V domain scaled by sqrt(128), i.e.
+// acc = sqrt(128) Pi (sum_t p_t v_t), so that combine_kernel's Pi^T acc / sqrt(128) returns sum_t p_t v_t -- which
+// combine_kernel merges with the packed range's records by the same exact log-sum-exp rule.
+constexpr int kMaxWindow = 1024;                    // n_sink + n_recent upper bound (shared-memory logits)
+__device__ __forceinline__ bool window_slot_valid(int s, int64_t T, int n_sink, int n_recent)
+{
+    if (s < n_sink) return s < T;
+    const int64_t x = T - 1 - (s - n_sink);         // T-1 - r; the newest token congruent to r is T-1 - (x mod n_recent)
+    if (x < 0) return false;
+    return T - 1 - (x % n_recent) >= n_sink;
+}
+__global__ void __launch_bounds__(128)
+window_kernel(const __half *__restrict__ win_k, const __half *__restrict__ win_v, const __nv_bfloat16 *__restrict__ q,
+              const int32_t *__restrict__ seq_len, const float *__restrict__ rot128_t, float *__restrict__ partials,
+              int batch, int Hkv, int G, int64_t n_cap, int n_sink, int n_recent, float scale_log2e, int win_slot)
+{
+    __shared__ float lg[kMaxWindow];
+    __shared__ float qs[kDh], o[kDh];
+    __shared__ float red[4];
+    const int pair = blockIdx.x / G, n = blockIdx.x % G;
+    const int h = pair % Hkv, lb = pair / Hkv, b = lb % batch;
+    const int d = threadIdx.x, lane = d & 31, wq = d >> 5;
+    const int n_win = n_sink + n_recent;
+    int64_t T = seq_len[b];
+    T = T < 0 ? 0 : (T > n_cap * kTile ? n_cap * kTile : T);
+    qs[d] = __bfloat162float(q[((size_t)lb * Hkv * G + h * G + n) * kDh + d]) * scale_log2e;
+    __syncthreads();
+    const __half *kw = win_k + (size_t)pair * n_win * kDh, *vw = win_v + (size_t)pair * n_win * kDh;
+    // logits: warp wq takes slots wq, wq+4, ...; a lane owns coordinates 4*lane .. 4*lane+3 (one 256-byte row per load)
+    const float4 q4 = *reinterpret_cast<const float4 *>(qs + 4 * lane);
+    float mloc = -INFINITY;
+    for (int s = wq; s < n_win; s += 4) {
+        float v = -INFINITY;
+        if (window_slot_valid(s, T, n_sink, n_recent)) {
+            const uint2 raw = *reinterpret_cast<const uint2 *>(kw + (size_t)s * kDh + 4 * lane);
+            const float2 a = __half22float2(*reinterpret_cast<const __half2 *>(&raw.x));
+            const float2 c = __half22float2(*reinterpret_cast<const __half2 *>(&raw.y));
+            v = fmaf(a.x, q4.x, fmaf(a.y, q4.y, fmaf(c.x, q4.z, c.y * q4.w)));
+#pragma unroll
+            for (int sft = 16; sft; sft >>= 1) v += __shfl_xor_sync(0xffffffffu, v, sft);
+        }
+        if (lane == 0) lg[s] = v;
+        mloc = fmaxf(mloc, v);
+    }
+    if (lane == 0) red[wq] = mloc;
+    __syncthreads();
+    const float Mx = fmaxf(fmaxf(red[0], red[1]), fmaxf(red[2], red[3]));
+    float *rec = partials + (size_t)(win_slot + pair) * kPartialFloats + n * 130;
+    if (Mx == -INFINITY) {                              // empty sequence: an empty record
+        if (d == 0) { rec[0] = -INFINITY; rec[1] = 0.f; }
+        rec[2 + d] = 0.f;
+        return;
+    }
+    // thread d: dimension d of sum_s p_s v_s and (every thread, same fixed order) the sum of the weights
+    float acc = 0.f, lsum = 0.f;
+    for (int s = 0; s < n_win; ++s) {
+        const float lv = lg[s];
+        if (lv == -INFINITY) continue;
+        const float pw = fast_exp2(lv - Mx);
+        lsum += pw;
+        acc = fmaf(pw, __half2float(vw[(size_t)s * kDh + d]), acc);
+    }
+    o[d] = acc;
+    __syncthreads();
+    float r = 0.f;                                      // acc_rot[d] = sqrt(128) * sum_j Pi[d][j] o[j]; rot128_t[j][d] = Pi[d][j]
+#pragma unroll 32
+    for (int j = 0; j < kDh; ++j) r = fmaf(__ldg(rot128_t + j * kDh + d), o[j], r);
+    rec[2 + d] = r * 11.313708498984761f;
+    if (d == 0) { rec[0] = Mx; rec[1] = lsum; }
+}
+
+// fp16 copies of new tokens into the window buffers (the protected regime's companion of quantize_append): token i of the
+// call sits at position seq_len[b] + i; it is stored iff it is a sink token or one of the call's last n_recent tokens
+// (earlier ones would be overwritten inside the same call).  k_new, v_new [n_layers][batch][n_new][Hkv][128], fp32 or bf16.
+template <typename T>
+__global__ void __launch_bounds__(128)
+window_append_kernel(const T *__restrict__ k_new, const T *__restrict__ v_new, const int32_t *__restrict__ seq_len,
+                     __half *__restrict__ win_k, __half *__restrict__ win_v, int batch, int n_new, int Hkv,
+                     int n_sink, int n_recent)
+{
+    const int i = blockIdx.x % n_new, lb = blockIdx.x / n_new, b = lb % batch, d = threadIdx.x;
+    const int64_t t = (int64_t)seq_len[b] + i;
+    int slot;
+    if (t < n_sink) slot = (int)t;
+    else if (n_recent > 0 && i >= n_new - n_recent) slot = n_sink + (int)(t % n_recent);
+    else return;
+    const int n_win = n_sink + n_recent;
+    for (int h = 0; h < Hkv; ++h) {
+        const size_t src = (((size_t)lb * n_new + i) * Hkv + h) * kDh + d;
+        const size_t dst = (((size_t)lb * Hkv + h) * n_win + slot) * kDh + d;
+        win_k[dst] = __float2half_rn((float)k_new[src]);
+        win_v[dst] = __float2half_rn((float)v_new[src]);
+    }
 }
 
 // ---------------------------------------------------------------- comparison path: fp16 KV cache
@@ -1205,7 +1327,7 @@ size_t decode_ws_bytes(const bgtq_layout *lay, int batch, int n_layers)
 {
     const size_t pairs = (size_t)n_layers * batch * lay->n_kv_heads;
     const size_t qf = pairs * kQfHalves * sizeof(__half);
-    const size_t slots = (size_t)lay->sm_count * kMaxWarpsPerSM + pairs;
+    const size_t slots = (size_t)lay->sm_count * kMaxWarpsPerSM + 2 * pairs;   // warp records + one window record per pair
     return qf + slots * kPartialFloats * sizeof(float);
 }
 
@@ -1275,8 +1397,9 @@ static int launch_decode_w(const DecodeParams &P, int grid, size_t smem, cudaStr
 
 int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *cache, const void *q,
                   const int32_t *seq_len, int batch, int64_t max_tokens, float scale, void *out,
-                  void *ws, size_t, const PageMap *pm, cudaStream_t st)
+                  void *ws, size_t, const PageMap *pm, cudaStream_t st, const Window *win)
 {
+    const int n_sink = win ? win->n_sink : 0, n_recent = win ? win->n_recent : 0;
     if (batch > kMaxBatch) { set_error("bgtq_decode_attention: batch > 256"); return BGTQ_EINVAL; }
     const int Hkv = lay->n_kv_heads, Hq = lay->n_q_heads, G = Hq / Hkv;
     const int64_t n_cap = (max_tokens + kTile - 1) / kTile;
@@ -1299,7 +1422,16 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
     P.partials = partials; P.n_cap = n_cap; P.n_layers = n_layers; P.batch = batch; P.Hkv = Hkv; P.G = G;
     P.buf_bytes = buf_bytes;
     P.pages = pm ? pm->table : nullptr; P.pstride = pm ? pm->table_stride : 0; P.n_pages = pm ? pm->n_pages : 0;
+    P.n_sink = n_sink; P.n_recent = n_recent;
     const int grid = lay->sm_count;
+    const int win_slot = win ? lay->sm_count * kMaxWarpsPerSM + pairs : -1;    // first record after the warp records
+    if (win) {   // fp16 windows -> one record per (pair, query head); ordinary launch, complete before decode's pdl_wait returns
+        window_kernel<<<pairs * G, 128, 0, st>>>((const __half *)win->k, (const __half *)win->v, (const __nv_bfloat16 *)q, seq_len,
+                                                 lay->d_rot_t + rot_offset(kDh), partials, batch, Hkv, G, n_cap, n_sink, n_recent,
+                                                 scale * 1.4426950408889634f, win_slot);
+        count_launch();
+        CUDA_TRY(cudaGetLastError());
+    }
     const size_t smem = decode_smem(W, buf_bytes);
     int rc;
     if (pm) {
@@ -1329,8 +1461,23 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
         cfg.gridDim = dim3(pairs * G); cfg.blockDim = dim3(128); cfg.dynamicSmemBytes = 0; cfg.stream = st;
         cfg.attrs = at; cfg.numAttrs = 1;
         cudaLaunchKernelEx(&cfg, combine_kernel, (const float *)partials, seq_len, (const float *)(lay->d_rot + rot_offset(kDh)),
-                           n_layers, batch, Hkv, G, n_cap, grid, W, (__nv_bfloat16 *)out);
+                           n_layers, batch, Hkv, G, n_cap, grid, W, (__nv_bfloat16 *)out, n_sink, n_recent, win_slot);
     }
+    count_launch();
+    CUDA_TRY(cudaGetLastError());
+    return BGTQ_OK;
+}
+
+int launch_window_append(const void *k_new, const void *v_new, int dt, int n_layers, int batch, int n_new, int Hkv,
+                         const int32_t *seq_len, void *win_k, void *win_v, int n_sink, int n_recent, cudaStream_t st)
+{
+    const int grid = n_layers * batch * n_new;
+    if (dt == BGTQ_F32)
+        window_append_kernel<float><<<grid, 128, 0, st>>>((const float *)k_new, (const float *)v_new, seq_len, (__half *)win_k,
+                                                          (__half *)win_v, batch, n_new, Hkv, n_sink, n_recent);
+    else
+        window_append_kernel<__nv_bfloat16><<<grid, 128, 0, st>>>((const __nv_bfloat16 *)k_new, (const __nv_bfloat16 *)v_new, seq_len,
+                                                                  (__half *)win_k, (__half *)win_v, batch, n_new, Hkv, n_sink, n_recent);
     count_launch();
     CUDA_TRY(cudaGetLastError());
     return BGTQ_OK;

@@ -403,6 +403,46 @@ extern "C" int bgtq_decode_attention(const bgtq_layout *lay, int layer, const vo
                                         softmax_scale, out, workspace, workspace_bytes, stream);
 }
 
+extern "C" int bgtq_decode_attention_protected(const bgtq_layout *lay, int layer0, int n_layers, const void *cache,
+                                               const void *q, const int32_t *seq_len, int batch, int64_t max_tokens,
+                                               float softmax_scale, const void *win_k, const void *win_v, int n_sink,
+                                               int n_recent, void *out, void *workspace, size_t workspace_bytes,
+                                               void *stream)
+{
+    if (!lay || !cache || !q || !seq_len || !out || !workspace || !win_k || !win_v) FAIL(BGTQ_EINVAL, "bgtq_decode_attention_protected: null pointer");
+    if (layer0 < 0 || n_layers <= 0 || layer0 + n_layers > lay->n_layers) FAIL(BGTQ_EINVAL, "bgtq_decode_attention_protected: layer range");
+    if (batch <= 0 || max_tokens <= 0) FAIL(BGTQ_EINVAL, "bgtq_decode_attention_protected: batch/max_tokens");
+    if (!(softmax_scale > 0.0f) || std::isinf(softmax_scale)) FAIL(BGTQ_EINVAL, "bgtq_decode_attention_protected: softmax_scale must be finite and > 0");
+    if (n_sink < 0 || n_recent < 0 || n_sink >= BGTQ_TILE_TOKENS || n_sink + n_recent < 1 || n_sink + n_recent > 1024)
+        FAIL(BGTQ_EINVAL, "bgtq_decode_attention_protected: need 0 <= n_sink < 128, n_recent >= 0, 1 <= n_sink + n_recent <= 1024");
+    if (workspace_bytes < decode_ws_bytes(lay, batch, n_layers)) FAIL(BGTQ_EWORKSPACE, "bgtq_decode_attention_protected: workspace too small");
+    const size_t per_layer = (size_t)batch * lay->n_kv_heads * (size_t)(n_sink + n_recent) * lay->d_h;   // fp16 elements
+    const Window win = {(const uint16_t *)win_k + (size_t)layer0 * per_layer, (const uint16_t *)win_v + (size_t)layer0 * per_layer,
+                        n_sink, n_recent};
+    return launch_decode(lay, layer0, n_layers, cache, q, seq_len, batch, max_tokens, softmax_scale, out, workspace,
+                         workspace_bytes, nullptr, (cudaStream_t)stream, &win);
+}
+
+extern "C" size_t bgtq_window_bytes(const bgtq_layout *lay, int batch, int n_sink, int n_recent)
+{
+    if (!lay || batch <= 0 || n_sink < 0 || n_recent < 0) return 0;
+    return (size_t)lay->n_layers * batch * lay->n_kv_heads * (size_t)(n_sink + n_recent) * lay->d_h * 2;
+}
+
+extern "C" int bgtq_window_append(const bgtq_layout *lay, int layer0, int n_layers, const void *k_new, const void *v_new,
+                                  int dt, int batch, int n_new, const int32_t *seq_len, void *win_k, void *win_v,
+                                  int n_sink, int n_recent, void *stream)
+{
+    if (!lay || !k_new || !v_new || !seq_len || !win_k || !win_v) FAIL(BGTQ_EINVAL, "bgtq_window_append: null pointer");
+    if (layer0 < 0 || n_layers <= 0 || layer0 + n_layers > lay->n_layers) FAIL(BGTQ_EINVAL, "bgtq_window_append: layer range");
+    if (dt != BGTQ_F32 && dt != BGTQ_BF16) FAIL(BGTQ_EINVAL, "bgtq_window_append: dtype");
+    if (batch <= 0 || n_new <= 0 || n_sink < 0 || n_recent < 0 || n_sink + n_recent < 1) FAIL(BGTQ_EINVAL, "bgtq_window_append: batch/n_new/window");
+    const size_t per_layer = (size_t)batch * lay->n_kv_heads * (size_t)(n_sink + n_recent) * lay->d_h;
+    return launch_window_append(k_new, v_new, dt, n_layers, batch, n_new, lay->n_kv_heads, seq_len,
+                                (uint16_t *)win_k + (size_t)layer0 * per_layer, (uint16_t *)win_v + (size_t)layer0 * per_layer,
+                                n_sink, n_recent, (cudaStream_t)stream);
+}
+
 extern "C" size_t bgtq_prefill_workspace_bytes(const bgtq_layout *lay, int batch, int n_q)
 {
     if (!lay || batch <= 0 || n_q <= 0) return 0;

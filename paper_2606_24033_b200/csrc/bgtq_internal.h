@@ -77,6 +77,12 @@ struct PageMap {
     int64_t n_pages;
 };
 
+// Protected regime (bgtq_decode_attention_protected): fp16 windows [layer][seq][kv head][n_sink + n_recent][d_h]
+struct Window {
+    const void *k, *v;
+    int n_sink, n_recent;
+};
+
 // RoPE fused into append (bgtq_quantize_append_rope): fp32 tables [rows][d_h/2], row = token position
 struct RopeTab {
     const float *cos, *sin;
@@ -94,7 +100,10 @@ int launch_quantize_append(const bgtq_layout *lay, int layer, int n_layers, void
                            int advance, int64_t max_tokens, const PageMap *pm, const RopeTab *rope, cudaStream_t st);
 int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *cache,
                   const void *q, const int32_t *seq_len, int batch, int64_t max_tokens,
-                  float scale, void *out, void *ws, size_t ws_bytes, const PageMap *pm, cudaStream_t st);
+                  float scale, void *out, void *ws, size_t ws_bytes, const PageMap *pm, cudaStream_t st,
+                  const Window *win = nullptr);
+int launch_window_append(const void *k_new, const void *v_new, int dt, int n_layers, int batch, int n_new, int Hkv,
+                         const int32_t *seq_len, void *win_k, void *win_v, int n_sink, int n_recent, cudaStream_t st);
 size_t decode_ws_bytes(const bgtq_layout *lay, int batch, int n_layers);
 int debug_decode_unit(int b, const uint32_t *words, float *values);
 size_t prefill_ws_bytes(const bgtq_layout *lay, int batch, int n_q);

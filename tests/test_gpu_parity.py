@@ -577,3 +577,124 @@ def test_append_with_fused_rope_bit_exact(P, tab128, kv_dtype, pairing):
             assert np.array_equal(host[off:off + n_cap * stride], exp), (l, h)
     with pytest.raises(P.BgtqError):                       # tables shorter than the capacity
         P.quantize_append_rope(lay, 0, cache, k, v, seq, max_tokens, cs[:100].contiguous(), sn[:100].contiguous(), n_layers=Lyr)
+
+
+# ----------------------------------------------------------------------------- protected regime
+def _protected_expected(p, heads, tab, scale, n_sink, n_recent):
+    k16 = p.k_post.astype(np.float16).astype(np.float64)
+    v16 = p.v.astype(np.float16).astype(np.float64)
+    G = p.Hq // p.Hkv
+    return np.concatenate([O.decode_attention_protected_head(p.q_post[h * G:(h + 1) * G], heads[h], tab, p.d_h, scale,
+                                                             k16[:, h], v16[:, h], n_sink, n_recent) for h in range(p.Hkv)])
+
+
+def _host_windows(p, n_sink, n_recent):
+    """The window buffers as the layout rule defines them (oracle.window_slot), filled on the host."""
+    wk = np.zeros((p.Hkv, n_sink + n_recent, p.d_h), dtype=np.float16); wv = np.zeros_like(wk)
+    prot, _ = O.protected_sets(p.T, n_sink, n_recent)
+    for t in prot:
+        s = O.window_slot(int(t), n_sink, n_recent)
+        wk[:, s] = p.k_post[t].astype(np.float16); wv[:, s] = p.v[t].astype(np.float16)
+    return wk, wv, prot
+
+
+@pytest.mark.parametrize("T,n_sink,n_recent,chunks", [(300, 4, 128, [300]), (700, 4, 128, [100, 250, 1, 349]), (132, 4, 128, [132]),
+                                                      (133, 4, 128, [3, 130]), (100, 4, 128, [100]), (3, 4, 128, [3]),
+                                                      (260, 0, 7, [255, 5]), (260, 5, 0, [2, 258]), (1000, 100, 300, [1000])])
+def test_protected_windows_attention_and_append(P, tab128, T, n_sink, n_recent, chunks):
+    """bgtq_window_append + bgtq_decode_attention_protected == the oracle's one-softmax definition with fp16 rows for
+    the first n_sink / last n_recent tokens; the window slots hold exactly the fp16-rounded rows; the packed cache
+    is untouched by the regime (still bit-exact, checked by _append_and_compare's path below)."""
+    Hq, Hkv = 8, 2
+    p = H.make_problem(900 + T + n_recent, T, Hq, Hkv, 3, 2, 1, 8, rope_base=1e6)       # K3V2: the AIME budget, PAPER.md:813
+    lay = P.Layout(p.bits[None], Hq, p.d_h, p.b_v, p.rot)
+    max_tokens = (T + 127) // 128 * 128 + 128
+    cache = lay.new_cache(1, max_tokens)
+    seq = torch.zeros(1, dtype=torch.int32, device="cuda")
+    win_k, win_v = P.new_windows(lay, 1, n_sink, n_recent)
+    t0 = 0
+    for n in chunks:
+        kk = _cuda(p.k_post[None, t0:t0 + n], torch.float32); vv = _cuda(p.v[None, t0:t0 + n], torch.float32)
+        P.window_append(lay, 0, kk, vv, seq, win_k, win_v, n_sink, n_recent)
+        P.quantize_append(lay, 0, cache, kk, vv, seq, max_tokens)
+        t0 += n
+    assert seq.tolist() == [T]
+    wk, wv, prot = _host_windows(p, n_sink, n_recent)
+    slots = sorted(O.window_slot(int(t), n_sink, n_recent) for t in prot)
+    got_k = win_k[0, 0].cpu().numpy(); got_v = win_v[0, 0].cpu().numpy()
+    assert np.array_equal(got_k[:, slots].view(np.uint16), wk[:, slots].view(np.uint16))
+    assert np.array_equal(got_v[:, slots].view(np.uint16), wv[:, slots].view(np.uint16))
+    heads = H.oracle_heads(p, tab128)
+    scale = 1.0 / math.sqrt(p.d_h)
+    q = _cuda(p.q_post[None], torch.bfloat16)
+    out = P.decode_attention_protected(lay, 0, cache, q, seq, max_tokens, scale, win_k, win_v, n_sink, n_recent,
+                                       lay.new_workspace(1))
+    torch.cuda.synchronize()
+    exp = _protected_expected(p, heads, tab128, scale, n_sink, n_recent)
+    _, rv = H.oracle_attention(p, heads, tab128, scale)
+    got = out[0].double().cpu().numpy()
+    G = Hq // Hkv
+    err = max(np.max(np.abs(got[a] - exp[a])) / rv[a // G] for a in range(Hq))
+    assert err <= 2e-3, err
+    # the buffer-free entry point on the same cache still gives the buffer-free answer (nothing leaked into the packed path)
+    plain = P.decode_attention(lay, 0, cache, q, seq, max_tokens, scale, lay.new_workspace(1))[0].double().cpu().numpy()
+    exp0, _ = H.oracle_attention(p, heads, tab128, scale)
+    assert max(np.max(np.abs(plain[a] - exp0[a])) / rv[a // G] for a in range(Hq)) <= 2e-3
+
+
+def test_protected_windows_layers_and_ragged_batch(P, tab128):
+    """3 layers x 3 sequences (one of them empty, one shorter than the windows) in one launch and per layer."""
+    Lyr, B, Hq, Hkv, d, ns, nr = 3, 3, 8, 2, 128, 4, 128
+    lens = [389, 0, 100]
+    probs = [[H.make_problem(1200 + 10 * l + b, max(lens[b], 1), Hq, Hkv, 3, 2, 1, 8, rope_base=1e6) for b in range(B)] for l in range(Lyr)]
+    for l in range(Lyr):
+        for b in range(B):
+            probs[l][b].bits = probs[l][0].bits
+    lay = P.Layout(np.stack([probs[l][0].bits for l in range(Lyr)]), Hq, d, 2, probs[0][0].rot)
+    max_tokens = 512
+    cache = lay.new_cache(B, max_tokens)
+    win_k, win_v = P.new_windows(lay, B, ns, nr)
+    for l in range(Lyr):
+        for b in range(B):
+            if lens[b] == 0:
+                continue
+            pb = probs[l][b]
+            kk = np.zeros((B, lens[b], Hkv, d)); vv = np.zeros_like(kk)
+            kk[b] = pb.k_post; vv[b] = pb.v
+            seq_l = torch.full((B,), max_tokens, dtype=torch.int32, device="cuda"); seq_l[b] = 0     # the others are "full"
+            P.quantize_append(lay, l, cache, _cuda(kk, torch.float32), _cuda(vv, torch.float32), seq_l, max_tokens,
+                              advance_seq_len=False)
+            wk, wv, _ = _host_windows(pb, ns, nr)
+            win_k[l, b] = torch.from_numpy(wk).cuda(); win_v[l, b] = torch.from_numpy(wv).cuda()
+    seq = torch.tensor(lens, dtype=torch.int32, device="cuda")
+    scale = 1.0 / math.sqrt(d)
+    qd = _cuda(np.stack([np.stack([probs[l][b].q_post for b in range(B)]) for l in range(Lyr)]), torch.bfloat16)
+    out_b = P.decode_attention_protected(lay, 0, cache, qd, seq, max_tokens, scale, win_k, win_v, ns, nr,
+                                         lay.new_workspace(B, Lyr), n_layers=Lyr)
+    ws1 = lay.new_workspace(B, 1)
+    out_l = torch.stack([P.decode_attention_protected(lay, l, cache, qd[l].contiguous(), seq, max_tokens, scale, win_k, win_v,
+                                                      ns, nr, ws1) for l in range(Lyr)])
+    torch.cuda.synchronize()
+    assert torch.all(out_b[:, 1] == 0) and torch.all(out_l[:, 1] == 0)
+    for l in range(Lyr):
+        for b in (0, 2):
+            pb = probs[l][b]
+            heads = H.oracle_heads(pb, tab128)
+            exp = _protected_expected(pb, heads, tab128, scale, ns, nr)
+            _, rv = H.oracle_attention(pb, heads, tab128, scale)
+            for name, out in (("batched", out_b), ("per-layer", out_l)):
+                got = out[l, b].double().cpu().numpy()
+                err = max(np.max(np.abs(got[a] - exp[a])) / rv[a // (Hq // Hkv)] for a in range(Hq))
+                assert err <= 2e-3, (name, l, b, err)
+
+
+def test_protected_argument_errors(P):
+    p = H.make_problem(43, 4, 8, 1, 3, 3, 1, 8)
+    lay = P.Layout(p.bits[None], 8, 128, 3, p.rot)
+    cache = lay.new_cache(1, 128)
+    seq = torch.zeros(1, dtype=torch.int32, device="cuda")
+    q = _cuda(p.q_post[None], torch.bfloat16)
+    wk, wv = P.new_windows(lay, 1, 4, 128)
+    for ns, nr in [(128, 4), (0, 0), (-1, 4), (4, 2000)]:
+        with pytest.raises(P.BgtqError):
+            P.decode_attention_protected(lay, 0, cache, q, seq, 128, 0.1, wk, wv, ns, nr, lay.new_workspace(1))
