@@ -56,6 +56,8 @@ def parse_args():
                     help="also time the fp16-cache comparison kernel (bgtq_fp16_decode_attention) on the same K, V")
     ap.add_argument("--paged", action="store_true",
                     help="also time bgtq_decode_attention_paged on a scattered-page copy of the same cache")
+    ap.add_argument("--protected", action="store_true",
+                    help="also time bgtq_decode_attention_protected (fp16 sink-4 / recent-128 windows, PAPER.md:813) on the same cache")
     ap.add_argument("--alloc", default="greedy", choices=["greedy", "uniform", "paper_like"],
                     help="K allocation: greedy = Block-GTQ from the library's energy->allocate path (the metric's workload); "
                          "uniform = one group at b_k bits (uniform TQ-MSE, PAPER.md:108); paper_like = greedy on scores whose "
@@ -487,6 +489,35 @@ def run_ours(args):
                      "note": "random page table over batch*ceil(max_tokens/128) pages; same tiles, scattered"}
             del pc
 
+        # ---- NEXT #4: protected regime (fp16 sink-4 / recent-128 windows), device-timed
+        protected = None
+        if args.protected:
+            n_sink, n_recent = 4, 128
+            win_k, win_v = P.new_windows(lay, args.batch, n_sink, n_recent)
+            win_k.normal_(); win_v.normal_()              # synthetic fp16 rows (timing only; parity is tests/test_gpu_parity.py)
+            outw = torch.empty_like(q)
+            tms = {}
+            for name in ("buffer_free", "protected"):
+                def call():
+                    if name == "protected":
+                        P.decode_attention_protected(lay, 0, cache, q, seq, wl["max_tokens"], wl["scale"], win_k, win_v,
+                                                     n_sink, n_recent, ws, out=outw, n_layers=Lyr)
+                    else:
+                        P.decode_attention(lay, 0, cache, q, seq, wl["max_tokens"], wl["scale"], ws, out=out, n_layers=Lyr)
+                for _ in range(3):
+                    call()
+                g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                g0.record(stream)
+                for _ in range(10):
+                    call()
+                g1.record(stream)
+                stream.synchronize()
+                tms[name] = g0.elapsed_time(g1) / 10 * 1e3
+            protected = {"attention_call_us": tms["protected"], "buffer_free_attention_call_us": tms["buffer_free"],
+                         "n_sink": n_sink, "n_recent": n_recent, "window_bytes": int(win_k.numel() * 2 * 2),
+                         "note": "q-fold + window_kernel + decode_kernel + combine_kernel over [sink fp16 | packed | recent fp16]"}
+            del win_k, win_v
+
         # ---- NEXT #1: causal prefill attention of the last N cached tokens (layer 0), device-timed
         prefill = None
         if args.prefill_chunk > 0:
@@ -605,7 +636,7 @@ def run_ours(args):
             "e2e": {"value": e2e_val, "unit": "GB/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": e2e_ms},
             "gpu_launches": int(launches_per_step) * args.steps, "gpu_launches_per_step": int(launches_per_step),
-            "comparison": comparison, "prefill": prefill, "paged": paged, "append_bulk": append_bulk,
+            "comparison": comparison, "prefill": prefill, "paged": paged, "protected": protected, "append_bulk": append_bulk,
         }))
     if world > 1:
         dist.destroy_process_group()

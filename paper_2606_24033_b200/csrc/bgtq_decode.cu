@@ -1019,22 +1019,34 @@ window_kernel(const __half *__restrict__ win_k, const __half *__restrict__ win_v
     qs[d] = __bfloat162float(q[((size_t)lb * Hkv * G + h * G + n) * kDh + d]) * scale_log2e;
     __syncthreads();
     const __half *kw = win_k + (size_t)pair * n_win * kDh, *vw = win_v + (size_t)pair * n_win * kDh;
-    // logits: warp wq takes slots wq, wq+4, ...; a lane owns coordinates 4*lane .. 4*lane+3 (one 256-byte row per load)
-    const float4 q4 = *reinterpret_cast<const float4 *>(qs + 4 * lane);
+    // logits: one thread per slot, the whole 256-byte key row in sixteen independent 16-byte loads (one memory latency per
+    // slot instead of one per load); q is read from shared memory (broadcast)
     float mloc = -INFINITY;
-    for (int s = wq; s < n_win; s += 4) {
+    for (int s = d; s < n_win; s += 128) {
         float v = -INFINITY;
         if (window_slot_valid(s, T, n_sink, n_recent)) {
-            const uint2 raw = *reinterpret_cast<const uint2 *>(kw + (size_t)s * kDh + 4 * lane);
-            const float2 a = __half22float2(*reinterpret_cast<const __half2 *>(&raw.x));
-            const float2 c = __half22float2(*reinterpret_cast<const __half2 *>(&raw.y));
-            v = fmaf(a.x, q4.x, fmaf(a.y, q4.y, fmaf(c.x, q4.z, c.y * q4.w)));
+            const uint4 *row = reinterpret_cast<const uint4 *>(kw + (size_t)s * kDh);
+            uint4 raw[16];
 #pragma unroll
-            for (int sft = 16; sft; sft >>= 1) v += __shfl_xor_sync(0xffffffffu, v, sft);
+            for (int c = 0; c < 16; ++c) raw[c] = __ldg(row + c);
+            float a0 = 0.f, a1 = 0.f;
+#pragma unroll
+            for (int c = 0; c < 16; ++c) {
+                const uint32_t wds[4] = {raw[c].x, raw[c].y, raw[c].z, raw[c].w};
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const float2 f = __half22float2(*reinterpret_cast<const __half2 *>(&wds[e]));
+                    a0 = fmaf(f.x, qs[8 * c + 2 * e], a0);
+                    a1 = fmaf(f.y, qs[8 * c + 2 * e + 1], a1);
+                }
+            }
+            v = a0 + a1;
         }
-        if (lane == 0) lg[s] = v;
+        lg[s] = v;
         mloc = fmaxf(mloc, v);
     }
+#pragma unroll
+    for (int sft = 16; sft; sft >>= 1) mloc = fmaxf(mloc, __shfl_xor_sync(0xffffffffu, mloc, sft));
     if (lane == 0) red[wq] = mloc;
     __syncthreads();
     const float Mx = fmaxf(fmaxf(red[0], red[1]), fmaxf(red[2], red[3]));
@@ -1044,14 +1056,18 @@ window_kernel(const __half *__restrict__ win_k, const __half *__restrict__ win_v
         rec[2 + d] = 0.f;
         return;
     }
-    // thread d: dimension d of sum_s p_s v_s and (every thread, same fixed order) the sum of the weights
+    // weights 2^(logit - max) in place (0 for an empty slot), then thread d: dimension d of sum_s p_s v_s and (every
+    // thread, same fixed order) the sum of the weights.  The value loads do not depend on the weights, so the unrolled
+    // loop keeps sixteen of them in flight; an empty slot's row may hold anything and is replaced by 0.
+    for (int s = d; s < n_win; s += 128) lg[s] = lg[s] == -INFINITY ? 0.f : fast_exp2(lg[s] - Mx);
+    __syncthreads();
     float acc = 0.f, lsum = 0.f;
+#pragma unroll 16
     for (int s = 0; s < n_win; ++s) {
-        const float lv = lg[s];
-        if (lv == -INFINITY) continue;
-        const float pw = fast_exp2(lv - Mx);
+        const float pw = lg[s];
+        const float vv = __half2float(vw[(size_t)s * kDh + d]);
         lsum += pw;
-        acc = fmaf(pw, __half2float(vw[(size_t)s * kDh + d]), acc);
+        acc = fmaf(pw, pw != 0.f ? vv : 0.f, acc);
     }
     o[d] = acc;
     __syncthreads();
@@ -1409,6 +1425,15 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
     float *partials = reinterpret_cast<float *>(reinterpret_cast<unsigned char *>(ws) + (size_t)pairs * kQfHalves * sizeof(__half));
     const HeadMeta *metas = lay->d_meta + (size_t)layer0 * Hkv;
 
+    const int win_slot = win ? lay->sm_count * kMaxWarpsPerSM + pairs : -1;    // first record after the warp records
+    if (win) {   // fp16 windows -> one record per (pair, query head).  Launched first so that qfold -> decode -> combine keep their
+                 // programmatic overlap; an ordinary launch, so it has completed before qfold_kernel starts
+        window_kernel<<<pairs * G, 128, 0, st>>>((const __half *)win->k, (const __half *)win->v, (const __nv_bfloat16 *)q, seq_len,
+                                                 lay->d_rot_t + rot_offset(kDh), partials, batch, Hkv, G, n_cap, n_sink, n_recent,
+                                                 scale * 1.4426950408889634f, win_slot);
+        count_launch();
+        CUDA_TRY(cudaGetLastError());
+    }
     qfold_kernel<<<pairs * G, 128, 0, st>>>(metas, lay->d_rot_t, (const __nv_bfloat16 *)q, batch, Hkv, Hq,
                                         scale * 1.4426950408889634f, qf, 0);
     count_launch();
@@ -1424,14 +1449,6 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
     P.pages = pm ? pm->table : nullptr; P.pstride = pm ? pm->table_stride : 0; P.n_pages = pm ? pm->n_pages : 0;
     P.n_sink = n_sink; P.n_recent = n_recent;
     const int grid = lay->sm_count;
-    const int win_slot = win ? lay->sm_count * kMaxWarpsPerSM + pairs : -1;    // first record after the warp records
-    if (win) {   // fp16 windows -> one record per (pair, query head); ordinary launch, complete before decode's pdl_wait returns
-        window_kernel<<<pairs * G, 128, 0, st>>>((const __half *)win->k, (const __half *)win->v, (const __nv_bfloat16 *)q, seq_len,
-                                                 lay->d_rot_t + rot_offset(kDh), partials, batch, Hkv, G, n_cap, n_sink, n_recent,
-                                                 scale * 1.4426950408889634f, win_slot);
-        count_launch();
-        CUDA_TRY(cudaGetLastError());
-    }
     const size_t smem = decode_smem(W, buf_bytes);
     int rc;
     if (pm) {
