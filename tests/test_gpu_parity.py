@@ -319,6 +319,59 @@ def test_full_size_128k_sampled_head(P, tab128):
     assert err <= 2e-3, err
 
 
+@pytest.mark.timeout(900)
+def test_full_size_cfg3_batch4_sampled(P, tab128):
+    """BASELINE.json configs[3] at full size (Llama-3.1-8B layer shape: 32 q / 8 kv heads, K2V2, 131,072 tokens, batch 4 of
+    independent seeds; here with ragged lengths so the balanced split crosses sequence boundaries): the packed region and
+    the attention output of two sampled (sequence, KV head) pairs against the oracle on the SAME input tensors."""
+    from workloads import gpu_synth as GS
+    shp = W.CONFIGS[3]
+    B, T, d, Hq, Hkv = 4, 131072, shp.d_h, shp.n_q_heads, shp.n_kv_heads
+    lens = [T, T - 77, T // 2 + 5, T]
+    _, _, scales = GS.layer_kv(shp.seed0, 8, Hkv, d, shp.rope_base, "cuda")
+    qcal = GS.layer_queries(shp.seed0, shp.n_cal, Hq, scales, d, shp.rope_base, 0, "cuda", tag=4)
+    kcal, _, _ = GS.layer_kv(shp.seed0, 32768, Hkv, d, shp.rope_base, "cuda", chunk_tag=99)
+    bits = P.allocate(P.block_energy(qcal, kcal), shp.b_k * 64, shp.b_min, shp.b_max).cpu().numpy().reshape(1, Hkv, 64)
+    del kcal
+    lay = P.Layout(bits, Hq, d, shp.b_v, tab128.rot)
+    cache = lay.new_cache(B, T)
+    seq = torch.zeros(B, dtype=torch.int32, device="cuda")
+    sampled = {(1, 5): None, (2, 0): None}
+    for c0 in range(0, T, 32768):                 # every sequence gets its own draw; all are filled to T, seq_len is set after
+        k = torch.stack([GS.layer_kv(shp.seed0 + 100 * b, 32768, Hkv, d, shp.rope_base, "cuda", t0=c0, chunk_tag=c0 // 32768)[0] for b in range(B)])
+        v = torch.stack([GS.layer_kv(shp.seed0 + 100 * b, 32768, Hkv, d, shp.rope_base, "cuda", t0=c0, chunk_tag=c0 // 32768)[1] for b in range(B)])
+        P.quantize_append(lay, 0, cache, k, v, seq, T)
+        for (b, h) in sampled:
+            kh, vh = k[b, :, h].double().cpu().numpy(), v[b, :, h].double().cpu().numpy()
+            sampled[(b, h)] = (kh, vh) if sampled[(b, h)] is None else (np.concatenate([sampled[(b, h)][0], kh]),
+                                                                         np.concatenate([sampled[(b, h)][1], vh]))
+        del k, v
+    assert seq.tolist() == [T] * B
+    seq = torch.tensor(lens, dtype=torch.int32, device="cuda")
+    q = torch.stack([GS.layer_queries(shp.seed0 + 100 * b, 1, Hq, scales, d, shp.rope_base, lens[b], "cuda", tag=3,
+                                      dtype=torch.bfloat16)[0] for b in range(B)])
+    scale = 1.0 / math.sqrt(d)
+    out = P.decode_attention(lay, 0, cache, q, seq, T, scale, lay.new_workspace(B, 1))
+    torch.cuda.synchronize()
+    G = Hq // Hkv
+    for (b, h), (kh, vh) in sampled.items():
+        n = lens[b]
+        head = O.quantize_head(kh[:n], vh[:n], bits[0, h], shp.b_v, tab128)
+        stride = lay.tile_stride(0, h)
+        off = lay.region_offset(0, b, h, B, T)
+        n_full = n // 128                          # whole tiles of the attended prefix (the cache holds all T tokens)
+        exp = np.zeros(((n + 127) // 128) * stride, dtype=np.uint8)
+        O.pack_region(head, d, exp)
+        got = cache[off:off + n_full * stride].cpu().numpy()
+        assert np.array_equal(got, exp[:n_full * stride]), ("packed region differs at full size", b, h)
+        q_h = q[b, h * G:(h + 1) * G].double().cpu().numpy()
+        ref = O.decode_attention_head(q_h, head, tab128, d, scale)
+        _, V = O.dequantize_head(head, tab128, d)
+        rv = math.sqrt(np.mean(np.sum(V * V, axis=1)))
+        err = np.max(np.abs(out[b, h * G:(h + 1) * G].double().cpu().numpy() - ref)) / rv
+        assert err <= 2e-3, (b, h, err)
+
+
 # ----------------------------------------------------------------------------- comparison path (not the method)
 @pytest.mark.parametrize("lens", [[1], [300, 77], [1000, 129, 0]])
 def test_fp16_comparison_kernel_vs_plain_attention(P, lens):
