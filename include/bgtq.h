@@ -157,6 +157,7 @@ int bgtq_decode_attention_layers(const bgtq_layout *layout, int layer0, int n_la
  *   as usual); its tokens outside [n_sink, seq_len - n_recent) are skipped / masked, never read as keys.
  * Limits: 0 <= n_sink < 128, n_recent >= 0, 1 <= n_sink + n_recent <= 1024 (else BGTQ_EINVAL; use
  *   bgtq_decode_attention_layers for the buffer-free path).  Everything else as bgtq_decode_attention_layers.
+ *   Contiguous cache layout only (no paged variant).
  * bgtq_window_append: fp16 copies (round-to-nearest-even) of the n_new tokens the matching
  *   bgtq_quantize_append_layers call stores at positions seq_len[s] .. seq_len[s] + n_new - 1, written to their
  *   window slots; call it BEFORE that append advances seq_len.  k_new (post-RoPE), v_new, dt, batch, n_new as

@@ -317,6 +317,19 @@ def test_full_size_128k_sampled_head(P, tab128):
     rv = math.sqrt(np.mean(np.sum(V * V, axis=1)))
     err = np.max(np.abs(out[l, 0, h * G:(h + 1) * G].double().cpu().numpy() - ref)) / rv
     assert err <= 2e-3, err
+    # the protected regime (fp16 sink-4 / recent-128 windows) on the same cache, same launch configuration
+    ns, nr = 4, 128
+    win_k, win_v = P.new_windows(lay, 1, ns, nr)
+    zero = torch.zeros(1, dtype=torch.int32, device="cuda")
+    for ll in range(Lyr):
+        P.window_append(lay, ll, kv[ll][0][None].contiguous(), kv[ll][1][None].contiguous(), zero, win_k, win_v, ns, nr)
+    outp = P.decode_attention_protected(lay, 0, cache, q, seq, max_tokens, scale, win_k, win_v, ns, nr,
+                                        lay.new_workspace(1, Lyr), n_layers=Lyr)
+    torch.cuda.synchronize()
+    refp = O.decode_attention_protected_head(q_h, head, tab128, d, scale, k_h.astype(np.float16).astype(np.float64),
+                                             v_h.astype(np.float16).astype(np.float64), ns, nr)
+    errp = np.max(np.abs(outp[l, 0, h * G:(h + 1) * G].double().cpu().numpy() - refp)) / rv
+    assert errp <= 2e-3, errp
 
 
 @pytest.mark.timeout(900)
