@@ -367,6 +367,10 @@ qfold_kernel(const HeadMeta *__restrict__ metas, const float *__restrict__ rot_t
         if (plain) qf[((size_t)pair * 8 + n) * kDh + tid] = __float2half_rn(acc * sc);
         else out[((ks * 8 + n) * 4 + ((kap & 7) >> 1)) * 4 + (kap >> 3) * 2 + (kap & 1)] = __float2half_rn(acc * sc);
     }
+    // Protected regime: this kernel is launched programmatically behind window_kernel and runs beside it; it must not
+    // COMPLETE before window_kernel has, because the kernels after it only wait for their immediate predecessor.
+    // (A no-op when the launch carries no programmatic dependency.)
+    pdl_wait();
 }
 
 // ---------------------------------------------------------------- TMEM as a register parking space
@@ -994,7 +998,7 @@ combine_kernel(const float *__restrict__ partials, const int32_t *__restrict__ s
 // format -- running max and sum in the log2 domain, accumulator in the rotated V domain scaled by sqrt(128), i.e.
 // acc = sqrt(128) Pi (sum_t p_t v_t), so that combine_kernel's Pi^T acc / sqrt(128) returns sum_t p_t v_t -- which
 // combine_kernel merges with the packed range's records by the same exact log-sum-exp rule.
-constexpr int kMaxWindow = 1024;                    // n_sink + n_recent upper bound (shared-memory logits)
+constexpr int kMaxWindow = 1024;                    // n_sink + n_recent upper bound (shared-memory logits; >= 4 * 128 for the reuse below)
 __device__ __forceinline__ bool window_slot_valid(int s, int64_t T, int n_sink, int n_recent)
 {
     if (s < n_sink) return s < T;
@@ -1010,6 +1014,7 @@ window_kernel(const __half *__restrict__ win_k, const __half *__restrict__ win_v
     __shared__ float lg[kMaxWindow];
     __shared__ float qs[kDh], o[kDh];
     __shared__ float red[4];
+    pdl_trigger();                                      // qfold_kernel may run beside this kernel (it reads nothing of ours)
     const int pair = blockIdx.x / G, n = blockIdx.x % G;
     const int h = pair % Hkv, lb = pair / Hkv, b = lb % batch;
     const int d = threadIdx.x, lane = d & 31, wq = d >> 5;
@@ -1056,20 +1061,40 @@ window_kernel(const __half *__restrict__ win_k, const __half *__restrict__ win_v
         rec[2 + d] = 0.f;
         return;
     }
-    // weights 2^(logit - max) in place (0 for an empty slot), then thread d: dimension d of sum_s p_s v_s and (every
-    // thread, same fixed order) the sum of the weights.  The value loads do not depend on the weights, so the unrolled
-    // loop keeps sixteen of them in flight; an empty slot's row may hold anything and is replaced by 0.
+    // weights 2^(logit - max) in place (0 for an empty slot).  Then warp wq takes slots wq, wq+4, ... and a lane four
+    // dimensions (one 8-byte load per slot), 32 slots' loads in flight at a time -- the value loads do not depend on the
+    // weights; an empty slot's row may hold anything and is replaced by 0.  The four warps' partial sums meet in shared
+    // memory in a fixed order.
     for (int s = d; s < n_win; s += 128) lg[s] = lg[s] == -INFINITY ? 0.f : fast_exp2(lg[s] - Mx);
     __syncthreads();
-    float acc = 0.f, lsum = 0.f;
-#pragma unroll 16
-    for (int s = 0; s < n_win; ++s) {
-        const float pw = lg[s];
-        const float vv = __half2float(vw[(size_t)s * kDh + d]);
-        lsum += pw;
-        acc = fmaf(pw, pw != 0.f ? vv : 0.f, acc);
+    float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f, lw = 0.f;
+    for (int s0 = wq; s0 < n_win; s0 += 4 * 32) {
+        uint2 raw[32];
+#pragma unroll
+        for (int u = 0; u < 32; ++u) {
+            const int s = s0 + 4 * u;
+            raw[u] = s < n_win ? __ldg(reinterpret_cast<const uint2 *>(vw + (size_t)s * kDh + 4 * lane)) : make_uint2(0u, 0u);
+        }
+#pragma unroll
+        for (int u = 0; u < 32; ++u) {
+            const int s = s0 + 4 * u;
+            const float pw = s < n_win ? lg[s] : 0.f;
+            const float2 x = __half22float2(*reinterpret_cast<const __half2 *>(&raw[u].x));
+            const float2 y = __half22float2(*reinterpret_cast<const __half2 *>(&raw[u].y));
+            const bool on = pw != 0.f;
+            lw += pw;
+            a0 = fmaf(pw, on ? x.x : 0.f, a0); a1 = fmaf(pw, on ? x.y : 0.f, a1);
+            a2 = fmaf(pw, on ? y.x : 0.f, a2); a3 = fmaf(pw, on ? y.y : 0.f, a3);
+        }
     }
-    o[d] = acc;
+    float *part = lg;                                   // the logits are dead from here on: reuse as [4][128] + [4]
+    __syncthreads();
+    part[wq * kDh + 4 * lane] = a0; part[wq * kDh + 4 * lane + 1] = a1;
+    part[wq * kDh + 4 * lane + 2] = a2; part[wq * kDh + 4 * lane + 3] = a3;
+    if (lane == 0) red[wq] = lw;
+    __syncthreads();
+    const float lsum = (red[0] + red[1]) + (red[2] + red[3]);
+    o[d] = (part[d] + part[kDh + d]) + (part[2 * kDh + d] + part[3 * kDh + d]);
     __syncthreads();
     float r = 0.f;                                      // acc_rot[d] = sqrt(128) * sum_j Pi[d][j] o[j]; rot128_t[j][d] = Pi[d][j]
 #pragma unroll 32
@@ -1426,16 +1451,28 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
     const HeadMeta *metas = lay->d_meta + (size_t)layer0 * Hkv;
 
     const int win_slot = win ? lay->sm_count * kMaxWarpsPerSM + pairs : -1;    // first record after the warp records
-    if (win) {   // fp16 windows -> one record per (pair, query head).  Launched first so that qfold -> decode -> combine keep their
-                 // programmatic overlap; an ordinary launch, so it has completed before qfold_kernel starts
+    if (win) {   // fp16 windows -> one record per (pair, query head).  An ordinary launch (everything before it, the appends
+                 // included, is complete when it starts); qfold_kernel is then launched programmatically behind it and the
+                 // two run side by side.  Completion order is kept by qfold_kernel's trailing griddepcontrol.wait:
+                 // window -> qfold -> decode -> combine, each waiting for its predecessor only.
         window_kernel<<<pairs * G, 128, 0, st>>>((const __half *)win->k, (const __half *)win->v, (const __nv_bfloat16 *)q, seq_len,
                                                  lay->d_rot_t + rot_offset(kDh), partials, batch, Hkv, G, n_cap, n_sink, n_recent,
                                                  scale * 1.4426950408889634f, win_slot);
         count_launch();
         CUDA_TRY(cudaGetLastError());
     }
-    qfold_kernel<<<pairs * G, 128, 0, st>>>(metas, lay->d_rot_t, (const __nv_bfloat16 *)q, batch, Hkv, Hq,
-                                        scale * 1.4426950408889634f, qf, 0);
+    if (win && !g_prof) {
+        cudaLaunchConfig_t cfg = {};
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.gridDim = dim3(pairs * G); cfg.blockDim = dim3(128); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        cudaLaunchKernelEx(&cfg, qfold_kernel, metas, (const float *)lay->d_rot_t, (const __nv_bfloat16 *)q, batch, Hkv, Hq,
+                           scale * 1.4426950408889634f, qf, 0);
+    } else
+        qfold_kernel<<<pairs * G, 128, 0, st>>>(metas, lay->d_rot_t, (const __nv_bfloat16 *)q, batch, Hkv, Hq,
+                                                scale * 1.4426950408889634f, qf, 0);
     count_launch();
     CUDA_TRY(cudaGetLastError());
 
