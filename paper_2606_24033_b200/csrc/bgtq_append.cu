@@ -19,10 +19,12 @@ namespace bgtq {
 #define CUDA_TRY(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) return cuda_fail(e_, #expr); } while (0)
 
 constexpr int kAppendThreads = 256;
+constexpr int kMetaBytes = (int)((sizeof(HeadMeta) + 15) / 16 * 16);
+static_assert(sizeof(HeadMeta) % 4 == 0, "HeadMeta is copied word by word");
 constexpr int kSub = 16;                       // tokens per sub-batch
 constexpr int kMaxUnits = 2 * kMaxKSteps;
 
-struct UnitDesc { int off; int b; int nc; int ustart; };   // ustart: grouped-order coordinate of slot q=0,c=0
+struct UnitDesc { uint16_t off; uint8_t b, nc; uint16_t ustart, pad; };   // ustart: grouped-order coordinate of slot q=0,c=0 (8 bytes: shared memory is what caps this kernel at 4 CTAs per SM)
 
 // position of bit `bit` of the field of slot k in a unit of width b (DESIGN.md section 4 table)
 __device__ __forceinline__ void field_bit_pos(int b, int k, int bit, int &word, int &pos)
@@ -67,7 +69,6 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
     extern __shared__ __align__(16) unsigned char smem[];
     const int tid = threadIdx.x;
     const int h = blockIdx.y % Hkv, lrel = blockIdx.y / Hkv, s = blockIdx.z;
-    const HeadMeta &M = metas[blockIdx.y];
     const int64_t t0 = seq_len[s];
     const int64_t t_end = min(t0 + (int64_t)n_new, max_tokens);
     const int64_t tile = t0 / kTile + blockIdx.x;
@@ -75,7 +76,6 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
     const int64_t lo = max(t0, tile_lo), hi = min(t_end, tile_lo + kTile);
     if (lo >= hi) return;
 
-    const int stride = M.tile_stride, ng = M.n_groups, kdim = M.kdim, b_v = M.b_v;
     // shared memory carve-up
     double *xs = reinterpret_cast<double *>(smem);                       // [16][256]
     double *tau = xs + kSub * 256;                                       // [512] thresholds (C_b at 2^b-1)
@@ -84,7 +84,18 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
     uint8_t *idxs = reinterpret_cast<uint8_t *>(nrm + kSub * 9 + 8);     // [16][256]
     UnitDesc *units = reinterpret_cast<UnitDesc *>(idxs + kSub * 256);   // [32]
     int *n_units_p = reinterpret_cast<int *>(units + kMaxUnits);
-    uint32_t *tbuf = reinterpret_cast<uint32_t *>(n_units_p + 4);        // tile, `stride` bytes
+    HeadMeta *Msp = reinterpret_cast<HeadMeta *>(n_units_p + 4);         // this head's static metadata (kMetaBytes)
+    uint32_t *tbuf = reinterpret_cast<uint32_t *>(reinterpret_cast<unsigned char *>(Msp) + kMetaBytes);   // tile, `stride` bytes
+    // The metadata is read many times by single threads (unit list, group search, radii); one coalesced copy into
+    // shared memory replaces those dependent global-memory round trips -- they dominated the one-token append.
+    {
+        const uint32_t *msrc = reinterpret_cast<const uint32_t *>(metas + blockIdx.y);
+        uint32_t *mdst = reinterpret_cast<uint32_t *>(Msp);
+        for (int i = tid; i < (int)(sizeof(HeadMeta) / 4); i += kAppendThreads) mdst[i] = __ldg(msrc + i);
+    }
+    __syncthreads();
+    const HeadMeta &M = *Msp;
+    const int stride = M.tile_stride, ng = M.n_groups, kdim = M.kdim, b_v = M.b_v;
 
     uint8_t *gtile = PAGED ? cache + n_pages * ((int64_t)M.layer_prefix + M.head_prefix) + (int64_t)pages[(int64_t)s * pstride + tile] * stride
                            : cache + n_cap * ((int64_t)batch * M.layer_prefix + (int64_t)s * M.layer_sum + M.head_prefix) + tile * stride;
@@ -106,9 +117,9 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
             const KStep &K = M.ksteps[ks];
             int g = K.flags >> 4;
             if (K.flags & 1) j = 0;
-            units[n++] = UnitDesc{K.off0, K.b, K.nc0, M.gstart[g] + 8 * j};
+            units[n++] = UnitDesc{K.off0, K.b, K.nc0, (uint16_t)(M.gstart[g] + 8 * j), 0};
             ++j;
-            if (K.off1 != 0xFFFF) { units[n++] = UnitDesc{K.off1, K.b, K.nc1, M.gstart[g] + 8 * j}; ++j; }
+            if (K.off1 != 0xFFFF) { units[n++] = UnitDesc{K.off1, K.b, K.nc1, (uint16_t)(M.gstart[g] + 8 * j), 0}; ++j; }
         }
         *n_units_p = n;
     }
@@ -355,7 +366,7 @@ __global__ void advance_seq_len_kernel(int32_t *seq_len, int batch, int n_new, i
 static size_t append_smem_bytes(int max_stride)
 {
     return (size_t)kSub * 256 * 8 + 512 * 8 + kSub * 9 * 8 + (kSub * 9 + 8) * 2 + kSub * 256 +
-           kMaxUnits * sizeof(UnitDesc) + 16 + (size_t)max_stride + 64;
+           kMaxUnits * sizeof(UnitDesc) + 16 + kMetaBytes + (size_t)max_stride + 64;
 }
 
 int launch_quantize_append(const bgtq_layout *lay, int layer, int n_layers, void *cache, const void *k_new,
