@@ -305,11 +305,19 @@ def build_workload(args, P, torch, device, seed_shift: int = 0):
                                                  dtype=torch.bfloat16) for b in range(B)]) for l in range(Lyr)])   # [Lyr,B,Hq,d]
     k_new = torch.stack([torch.stack([gen_chunk(l, b, T, 1)[0] for b in range(B)]) for l in range(Lyr)]).contiguous()  # [Lyr,B,1,Hkv,d]
     v_new = torch.randn_like(k_new)
+    # the step's inputs live in ONE device buffer (q | k_new | v_new views), so that the end-to-end leg moves them with a
+    # single host-to-device copy
+    nq, nk = q.numel() * 2, k_new.numel() * 4
+    step_in = torch.empty(nq + 2 * nk, dtype=torch.uint8, device=device)
+    qv = step_in[:nq].view(torch.bfloat16).view(q.shape); qv.copy_(q)
+    kv_ = step_in[nq:nq + nk].view(torch.float32).view(k_new.shape); kv_.copy_(k_new)
+    vv_ = step_in[nq + nk:].view(torch.float32).view(v_new.shape); vv_.copy_(v_new)
+    q, k_new, v_new = qv, kv_, vv_
     tok_bytes = B * sum(lay.token_bytes(l, h) for l in range(Lyr) for h in range(Hkv))
     ws = lay.new_workspace(B, Lyr, device)
     torch.cuda.empty_cache()
     n_th = Lyr * B * T * Hkv
-    return dict(lay=lay, cache=cache, seq=seq, q=q, k_new=k_new, v_new=v_new, ws=ws, max_tokens=max_tokens,
+    return dict(lay=lay, cache=cache, seq=seq, q=q, k_new=k_new, v_new=v_new, step_in=step_in, ws=ws, max_tokens=max_tokens,
                 tok_bytes=tok_bytes, bits=bits, scale=1.0 / math.sqrt(d), fp16=fp16,
                 setup={"block_energy_ms": t_energy, "block_energy_GBs": energy_bytes / (t_energy * 1e-3) / 1e9,
                        "allocate_ms": t_alloc, "allocate_heads": Lyr * Hkv, "layout_create_ms": t_layout,
@@ -583,7 +591,8 @@ def run_ours(args):
             del ac, kk, vv
 
         # ---- end to end through the C-ABI with HOST buffers (pinned), copies inside the timed region
-        hq, hk, hv = q.cpu().pin_memory(), k_new.cpu().pin_memory(), v_new.cpu().pin_memory()
+        step_in = wl["step_in"]                       # q | k_new | v_new, one buffer on each side
+        hin = step_in.cpu().pin_memory()
         hout = torch.empty_like(out, device="cpu").pin_memory()
         n_e2e = max(5, min(args.steps, 30))
         for it in range(3 + n_e2e):
@@ -591,9 +600,7 @@ def run_ours(args):
                 stream.synchronize()
                 b0, b1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 b0.record(stream)
-            q.copy_(hq, non_blocking=True)
-            k_new.copy_(hk, non_blocking=True)
-            v_new.copy_(hv, non_blocking=True)
+            step_in.copy_(hin, non_blocking=True)
             graph.replay()
             hout.copy_(out, non_blocking=True)
             stream.synchronize()
@@ -606,7 +613,7 @@ def run_ours(args):
             e2e_ms = float(t.item())
         seq_e2e = int(seq[0].item()) - n_e2e / 2.0
         e2e_val = world * (seq_e2e * wl["tok_bytes"] + io_bytes) / (e2e_ms * 1e-3) / 1e9
-        h2d = (hq.numel() * 2 + hk.numel() * 4 + hv.numel() * 4)
+        h2d = hin.numel()
         d2h = hout.numel() * 2
 
     cpu_baseline = None
