@@ -28,6 +28,8 @@
 
 namespace bgtq {
 
+static_assert(sizeof(HeadMeta) % 4 == 0 && sizeof(HeadMeta) <= 128 * 4, "qfold_kernel copies HeadMeta with one word per thread");
+
 #define CUDA_TRY(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) return cuda_fail(e_, #expr); } while (0)
 
 #ifndef BGTQ_NORM_IN_OPERAND
@@ -327,11 +329,17 @@ qfold_kernel(const HeadMeta *__restrict__ metas, const float *__restrict__ rot_t
     const int G = Hq / Hkv;
     const int pair = blockIdx.x / G, n = blockIdx.x % G;   // one block per (pair, query head of the group)
     const int h = pair % Hkv, lb = pair / Hkv, l = lb / batch;
-    const HeadMeta &M = metas[l * Hkv + h];
-    __shared__ float qs[kDh];
+    __shared__ __align__(8) HeadMeta Ms;                    // one coalesced copy: the k-step scan and the group search below
+    __shared__ float qs[kDh];                               // were chains of dependent global loads on the critical path
     __shared__ int ksbase[kMaxGroups];
     const int tid = threadIdx.x;
+    {
+        const uint32_t *msrc = reinterpret_cast<const uint32_t *>(metas + l * Hkv + h);
+        if (tid < (int)(sizeof(HeadMeta) / 4)) reinterpret_cast<uint32_t *>(&Ms)[tid] = __ldg(msrc + tid);
+    }
     qs[tid] = __bfloat162float(q[((size_t)lb * Hq + h * G + n) * kDh + tid]);
+    __syncthreads();
+    const HeadMeta &M = Ms;
     if (tid == 0)
         for (int ks = 0; ks < M.n_ksteps; ++ks)
             if (M.ksteps[ks].flags & 1) ksbase[M.ksteps[ks].flags >> 4] = ks;
