@@ -15,7 +15,10 @@
  *   orc_dequantize_group   pinned to the rate law PAPER.md:49 and to brute-force nearest
  *                          centroid; "parity unpinned" against the AUTHORS' codebook /
  *                          rotation / layout (the paper prints none) -- see DESIGN.md.
- *   orc_put_field / get    pinned (round trip, byte accounting PAPER.md:837)
+ *   orc_put_field / get    pinned (round trip, byte accounting PAPER.md:837, hand-worked tests/golden/layout_*.txt)
+ *   orc_*_v2 (BGTQ-v2)     pinned (hand-worked tests/golden/layout_fields_v2.txt, layout_region_v2.txt; bijection; round trip)
+ *   orc_f64_to_f16_bits /
+ *   orc_f16_bits_to_f64    pinned to IEEE binary16 via numpy.float16 (every value, every midpoint, saturation)
  *
  * Build: gcc -O2 -ffp-contract=off -fno-fast-math -shared -fPIC (oracle/build.py).
  * -ffp-contract=off matters: every rounding below is the one written.
@@ -436,6 +439,126 @@ void orc_pack_region(uint8_t *region, long tile_stride, int n_groups, const int 
             else {
                 orc_put_field(W, b_v, slot, vidx[(size_t)t * d_h + u]);
                 for (int w = 0; w < b_v; ++w) memcpy(tile + unit + 4L * (w * 32 + lane), &W[w], 4);
+            }
+        }
+    }
+}
+
+/* ------------------------------------------------------------------ physical layout BGTQ-v2 ("row order")
+ * DESIGN.md section 4b is the specification; this is its independent restatement.
+ * A tile is still 128 tokens, [K codes | K norms | V norms | V codes], but a code word now belongs to ONE row of the
+ * tensor-core operand: token tau = 32*w + l (quadrant w, lane l) owns its K codes, dimension d = 32*w + l owns its V
+ * codes.  A "chunk" is up to 32 slots of one row: K chunk u of group g = grouped coordinates 32u .. 32u+r-1 of the
+ * group (r = min(32, m - 32u)); V chunk c of dimension d = tokens 32c .. 32c+31.  A chunk stores nw(b, r) 32-bit
+ * words per lane, plane-major (word j of lane l at byte 4*(j*32 + l)).
+ *   slot -> bits: b = 1: slot 4Q+e at word 0 bit 8e+7-Q;  b = 2, 3, >= 5: as BGTQ-v1 (orc_put_field);
+ *                 b = 4: magnitudes as b = 3 in words 0 .. nwm-1, sign of slot 4Q+e at word nwm, bit 8e+7-Q
+ *   nw(b, r):     b = 1: 1;  b = 2: ceil(r/16);  b = 3: nwm = min(3, ceil(r/8));  b = 4: nwm + 1;  b >= 5: ceil(r*b/32)
+ * Norm rows are in natural token order (token tau at entry tau).                                                     */
+int orc_chunk_words_v2(int b, int r)
+{
+    int nwm = r > 24 ? 3 : (r + 7) / 8;
+    switch (b) {
+    case 1: return 1;
+    case 2: return (r + 15) / 16;
+    case 3: return nwm;
+    case 4: return nwm + 1;
+    default: return (r * b + 31) / 32;
+    }
+}
+
+void orc_put_field_v2(uint32_t *W, int b, int r, int k, unsigned idx)
+{
+    int word, pos;
+    if (b == 1) setbit(W, 0, 8 * (k & 3) + 7 - (k >> 2), idx);
+    else if (b == 4) {
+        unsigned f = recode4(idx);
+        int nwm = r > 24 ? 3 : (r + 7) / 8;
+        for (int bit = 0; bit < 3; ++bit) { mag3_pos(k, bit, &word, &pos); setbit(W, word, pos, f >> bit); }
+        setbit(W, nwm, 8 * (k & 3) + 7 - (k >> 2), f >> 3);
+    } else orc_put_field(W, b, k, idx);
+}
+
+unsigned orc_get_field_v2(const uint32_t *W, int b, int r, int k)
+{
+    int word, pos;
+    unsigned f = 0;
+    if (b == 1) return getbit(W, 0, 8 * (k & 3) + 7 - (k >> 2));
+    if (b == 4) {
+        int nwm = r > 24 ? 3 : (r + 7) / 8;
+        for (int bit = 0; bit < 3; ++bit) { mag3_pos(k, bit, &word, &pos); f |= getbit(W, word, pos) << bit; }
+        f |= getbit(W, nwm, 8 * (k & 3) + 7 - (k >> 2)) << 3;
+        return decode4(f);
+    }
+    return orc_get_field(W, b, k);
+}
+
+/* bytes of the K codes of ONE quadrant (32 tokens) of a tile */
+long orc_kquad_bytes_v2(int n_groups, const int *gb, const int *gm)
+{
+    long words = 0;
+    for (int g = 0; g < n_groups; ++g)
+        for (int u = 0; 32 * u < gm[g]; ++u) {
+            int r = gm[g] - 32 * u >= 32 ? 32 : gm[g] - 32 * u;
+            words += orc_chunk_words_v2(gb[g], r);
+        }
+    return 128L * words;
+}
+
+/* Same contract as orc_pack_region, BGTQ-v2 layout. */
+void orc_pack_region_v2(uint8_t *region, long tile_stride, int n_groups, const int *gb, const int *gm,
+                        int d_h, int b_v, long t0, long t1, uint8_t *kidx, uint16_t *knorm,
+                        uint8_t *vidx, uint16_t *vnorm, int unpack)
+{
+    int kdim = 0;
+    for (int g = 0; g < n_groups; ++g) kdim += gm[g];
+    long kq = orc_kquad_bytes_v2(n_groups, gb, gm);
+    long knorm_off = 4 * kq;
+    long vnorm_off = knorm_off + 256L * n_groups;
+    long vcode_off = vnorm_off + 256L;
+    for (long t = t0; t < t1; ++t) {
+        uint8_t *tile = region + (t >> 7) * tile_stride;
+        int tau = (int)(t & 127), w = tau >> 5, l = tau & 31;
+        /* ---- K codes: quadrant w -> group -> chunk u -> word planes; lane l = token, slot = coordinate */
+        long coff = (long)w * kq;
+        int ubase = 0;
+        for (int g = 0; g < n_groups; ++g) {
+            int b = gb[g], m = gm[g];
+            for (int u = 0; 32 * u < m; ++u) {
+                int r = m - 32 * u >= 32 ? 32 : m - 32 * u;
+                int nw = orc_chunk_words_v2(b, r);
+                uint32_t W[8];
+                for (int j = 0; j < nw; ++j) memcpy(&W[j], tile + coff + 4L * (j * 32 + l), 4);
+                for (int s = 0; s < r; ++s) {
+                    size_t src = (size_t)t * kdim + ubase + 32 * u + s;
+                    if (unpack) kidx[src] = (uint8_t)orc_get_field_v2(W, b, r, s);
+                    else orc_put_field_v2(W, b, r, s, kidx[src]);
+                }
+                if (!unpack)
+                    for (int j = 0; j < nw; ++j) memcpy(tile + coff + 4L * (j * 32 + l), &W[j], 4);
+                coff += 128L * nw;
+            }
+            uint8_t *np_ = tile + knorm_off + 256L * g + 2L * tau;
+            if (unpack) memcpy(&knorm[(size_t)t * n_groups + g], np_, 2);
+            else memcpy(np_, &knorm[(size_t)t * n_groups + g], 2);
+            ubase += m;
+        }
+        /* ---- V norm */
+        {
+            uint8_t *np_ = tile + vnorm_off + 2L * tau;
+            if (unpack) memcpy(&vnorm[t], np_, 2);
+            else memcpy(np_, &vnorm[t], 2);
+        }
+        /* ---- V codes: dimension d = 32*wq + lane; chunk c = tau>>5; slot = tau&31 */
+        for (int d = 0; d < d_h; ++d) {
+            int wq = d >> 5, lane = d & 31;
+            long unit = vcode_off + (long)((wq * 4 + w) * b_v) * 128;
+            uint32_t W[8];
+            for (int j = 0; j < b_v; ++j) memcpy(&W[j], tile + unit + 4L * (j * 32 + lane), 4);
+            if (unpack) vidx[(size_t)t * d_h + d] = (uint8_t)orc_get_field_v2(W, b_v, 32, l);
+            else {
+                orc_put_field_v2(W, b_v, 32, l, vidx[(size_t)t * d_h + d]);
+                for (int j = 0; j < b_v; ++j) memcpy(tile + unit + 4L * (j * 32 + lane), &W[j], 4);
             }
         }
     }

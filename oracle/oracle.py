@@ -55,6 +55,16 @@ def lib():
         L.orc_pack_region.restype = None
         L.orc_pack_region.argtypes = [u8p, C.c_long, C.c_int, ip, ip, C.c_int, C.c_int, C.c_long,
                                       C.c_long, u8p, u16p, u8p, u16p, C.c_int]
+        L.orc_chunk_words_v2.restype = C.c_int
+        L.orc_chunk_words_v2.argtypes = [C.c_int, C.c_int]
+        L.orc_put_field_v2.restype = None
+        L.orc_put_field_v2.argtypes = [C.POINTER(C.c_uint32), C.c_int, C.c_int, C.c_int, C.c_uint]
+        L.orc_get_field_v2.restype = C.c_uint
+        L.orc_get_field_v2.argtypes = [C.POINTER(C.c_uint32), C.c_int, C.c_int, C.c_int]
+        L.orc_kquad_bytes_v2.restype = C.c_long
+        L.orc_kquad_bytes_v2.argtypes = [C.c_int, ip, ip]
+        L.orc_pack_region_v2.restype = None
+        L.orc_pack_region_v2.argtypes = L.orc_pack_region.argtypes
         _lib = L
     return _lib
 
@@ -295,9 +305,16 @@ def _f16_array(bits: np.ndarray) -> np.ndarray:
 
 
 # ----------------------------------------------------------------------------- physical layout
-def tile_geometry(groups: List[Group], d_h: int, b_v: int):
-    """Byte offsets inside one 128-token tile: [K codes | K norms | V norms | V codes]."""
-    kcode = sum(16 * g.m * g.width for g in groups)
+def tile_geometry(groups: List[Group], d_h: int, b_v: int, version: int = 1):
+    """Byte offsets inside one 128-token tile: [K codes | K norms | V norms | V codes].
+    version 1 = BGTQ-v1 (fragment order, no padding); 2 = BGTQ-v2 (row order: a K chunk of r <= 32 coordinates of one
+    token takes whole 32-bit words)."""
+    if version == 2:
+        gb = np.array([g.width for g in groups] + [0], dtype=np.int32)
+        gm = np.array([g.m for g in groups] + [0], dtype=np.int32)
+        kcode = 4 * int(lib().orc_kquad_bytes_v2(len(groups), _p(gb, C.c_int), _p(gm, C.c_int)))
+    else:
+        kcode = sum(16 * g.m * g.width for g in groups)
     knorm_off = kcode
     vnorm_off = knorm_off + 256 * len(groups)
     vcode_off = vnorm_off + 256
@@ -306,19 +323,19 @@ def tile_geometry(groups: List[Group], d_h: int, b_v: int):
                 stride=stride)
 
 
-def token_bytes(groups: List[Group], d_h: int, b_v: int) -> float:
+def token_bytes(groups: List[Group], d_h: int, b_v: int, version: int = 1) -> float:
     """Packed bytes per token of one KV head = tile stride / 128
-    (= 16*bbar_K + 16*b_V + 2*(n_g+1) at d_h = 128; PAPER.md:837 for the 96-byte ideal)."""
-    return tile_geometry(groups, d_h, b_v)["stride"] / 128.0
+    (v1: = 16*bbar_K + 16*b_V + 2*(n_g+1) at d_h = 128; PAPER.md:837 for the 96-byte ideal)."""
+    return tile_geometry(groups, d_h, b_v, version)["stride"] / 128.0
 
 
 def pack_region(q: QuantizedHead, d_h: int, region: np.ndarray | None = None,
-                t_offset: int = 0) -> np.ndarray:
+                t_offset: int = 0, version: int = 1) -> np.ndarray:
     """Write the T tokens of q at positions [t_offset, t_offset + T) into the packed region of
     one (sequence, layer, KV head); all other fields of ``region`` are preserved.  ``region``
     (uint8, zero-initialised) is created when None."""
     T = q.kidx.shape[0]
-    geo = tile_geometry(q.groups, d_h, q.b_v)
+    geo = tile_geometry(q.groups, d_h, q.b_v, version)
     n_tiles = (t_offset + T + 127) // 128
     if region is None:
         region = np.zeros(n_tiles * geo["stride"], dtype=np.uint8)
@@ -333,24 +350,27 @@ def pack_region(q: QuantizedHead, d_h: int, region: np.ndarray | None = None,
     knorm = np.zeros((t_offset + T, ng), np.uint16); knorm[t_offset:] = q.knorm
     vidx = np.zeros((t_offset + T, d_h), np.uint8); vidx[t_offset:] = q.vidx
     vnorm = np.zeros(t_offset + T, np.uint16); vnorm[t_offset:] = q.vnorm
-    lib().orc_pack_region(_p(region, C.c_uint8), geo["stride"], ng, _p(gb, C.c_int),
-                          _p(gm, C.c_int), d_h, q.b_v, t_offset, t_offset + T,
-                          _p(kidx, C.c_uint8), _p(knorm, C.c_uint16),
-                          _p(vidx, C.c_uint8), _p(vnorm, C.c_uint16), 0)
+    fn = lib().orc_pack_region_v2 if version == 2 else lib().orc_pack_region
+    fn(_p(region, C.c_uint8), geo["stride"], ng, _p(gb, C.c_int),
+       _p(gm, C.c_int), d_h, q.b_v, t_offset, t_offset + T,
+       _p(kidx, C.c_uint8), _p(knorm, C.c_uint16),
+       _p(vidx, C.c_uint8), _p(vnorm, C.c_uint16), 0)
     return region
 
 
-def unpack_region(region: np.ndarray, groups: List[Group], d_h: int, b_v: int, T: int) -> QuantizedHead:
-    geo = tile_geometry(groups, d_h, b_v)
+def unpack_region(region: np.ndarray, groups: List[Group], d_h: int, b_v: int, T: int,
+                  version: int = 1) -> QuantizedHead:
+    geo = tile_geometry(groups, d_h, b_v, version)
     gb = np.array([g.width for g in groups], dtype=np.int32)
     gm = np.array([g.m for g in groups], dtype=np.int32)
     kdim = int(gm.sum())
     q = QuantizedHead(groups, b_v, np.zeros((T, kdim), np.uint8), np.zeros((T, len(groups)), np.uint16),
                       np.zeros((T, d_h), np.uint8), np.zeros(T, np.uint16))
     region = np.ascontiguousarray(region, dtype=np.uint8)
-    lib().orc_pack_region(_p(region, C.c_uint8), geo["stride"], len(groups), _p(gb, C.c_int),
-                          _p(gm, C.c_int), d_h, b_v, 0, T, _p(q.kidx, C.c_uint8),
-                          _p(q.knorm, C.c_uint16), _p(q.vidx, C.c_uint8), _p(q.vnorm, C.c_uint16), 1)
+    fn = lib().orc_pack_region_v2 if version == 2 else lib().orc_pack_region
+    fn(_p(region, C.c_uint8), geo["stride"], len(groups), _p(gb, C.c_int),
+       _p(gm, C.c_int), d_h, b_v, 0, T, _p(q.kidx, C.c_uint8),
+       _p(q.knorm, C.c_uint16), _p(q.vidx, C.c_uint8), _p(q.vnorm, C.c_uint16), 1)
     return q
 
 
@@ -360,6 +380,18 @@ def put_field(W: np.ndarray, b: int, k: int, idx: int) -> None:
 
 def get_field(W: np.ndarray, b: int, k: int) -> int:
     return int(lib().orc_get_field(_p(W, C.c_uint32), b, k))
+
+
+def chunk_words_v2(b: int, r: int) -> int:
+    return int(lib().orc_chunk_words_v2(b, r))
+
+
+def put_field_v2(W: np.ndarray, b: int, r: int, k: int, idx: int) -> None:
+    lib().orc_put_field_v2(_p(W, C.c_uint32), b, r, k, idx)
+
+
+def get_field_v2(W: np.ndarray, b: int, r: int, k: int) -> int:
+    return int(lib().orc_get_field_v2(_p(W, C.c_uint32), b, r, k))
 
 
 # ----------------------------------------------------------------------------- attention

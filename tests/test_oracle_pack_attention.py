@@ -287,3 +287,157 @@ def test_protected_attention_short_sequences(tab128):
         out = O.decode_attention_protected_head(q, head, tab128, d, 0.1, k16, v16, 4, 128)
         for a in range(2):
             assert np.allclose(out[a], scipy_softmax(0.1 * (k16 @ q[a])) @ v16, rtol=1e-12, atol=1e-14)
+
+
+# ----------------------------------------------------------------------------- BGTQ-v2 (row order)
+GOLDEN_V2 = os.path.join(os.path.dirname(__file__), "golden", "layout_fields_v2.txt")
+GOLDEN_REGION_V2 = os.path.join(os.path.dirname(__file__), "golden", "layout_region_v2.txt")
+
+
+def _nw_spec(b, r):
+    """nw(b, r) retyped from DESIGN.md section 4b (not from the oracle)."""
+    nwm = min(3, -(-r // 8))
+    return {1: 1, 2: -(-r // 16), 3: nwm, 4: nwm + 1}.get(b, -(-r * b // 32))
+
+
+def test_v2_golden_field_positions():
+    n = 0
+    for line in open(GOLDEN_V2):
+        line = line.strip()
+        if not line or line.startswith("#"):
+            continue
+        parts = line.split()
+        b, r, k, idx = (int(x) for x in parts[:4])
+        want = [int(x, 16) for x in parts[4:]]
+        assert len(want) == _nw_spec(b, r) == O.chunk_words_v2(b, r), line
+        W = np.zeros(8, dtype=np.uint32)
+        O.put_field_v2(W, b, r, k, idx)
+        assert W[:len(want)].tolist() == want, line
+        assert not W[len(want):].any()
+        assert O.get_field_v2(W, b, r, k) == idx
+        n += 1
+    assert n >= 20
+
+
+@pytest.mark.parametrize("b", range(1, 9))
+def test_v2_chunk_slots_are_disjoint_and_fit(b):
+    """For every chunk size r (even, 2..32): the r slots own disjoint bit sets of exactly b bits inside nw(b, r) words."""
+    for r in range(2, 33, 2):
+        nw = O.chunk_words_v2(b, r)
+        assert nw == _nw_spec(b, r)
+        assert 32 * nw >= r * b
+        seen = np.zeros(8, dtype=np.uint32)
+        for k in range(r):
+            foot = np.zeros(8, dtype=np.uint32)
+            for idx in range(1 << b):
+                W = np.zeros(8, dtype=np.uint32)
+                O.put_field_v2(W, b, r, k, idx)
+                assert O.get_field_v2(W, b, r, k) == idx
+                foot |= W
+            assert not foot[nw:].any(), (b, r, k)
+            assert not (seen & foot).any()
+            seen |= foot
+            assert sum(bin(int(x)).count("1") for x in foot) == b
+    # a full chunk uses every bit
+    assert np.all(seen[:b] == 0xFFFFFFFF)
+
+
+def test_v2_golden_region_positions():
+    """One code / norm written into an otherwise zero head lands on the hand-computed byte."""
+    d, b_v = 128, 2
+    groups = [O.Group(1, np.array([0], np.int64), np.array([0, 64], np.int64)),
+              O.Group(3, np.arange(1, 18, dtype=np.int64), np.concatenate([[i, i + 64] for i in range(1, 18)]).astype(np.int64))]
+    assert [g.m for g in groups] == [2, 34]
+    geo = O.tile_geometry(groups, d, b_v, version=2)
+    assert geo == dict(kcode=2560, knorm_off=2560, vnorm_off=3072, vcode_off=3328, stride=7424)
+    n = 0
+    for line in open(GOLDEN_REGION_V2):
+        line = line.strip()
+        if not line or line.startswith("#"):
+            continue
+        what, index, value, off, byte = line.split()
+        t = 165 if what.endswith("165") else 37
+        T = t + 1
+        q = O.QuantizedHead(groups, b_v, np.zeros((T, 36), np.uint8), np.zeros((T, 2), np.uint16),
+                            np.zeros((T, d), np.uint8), np.zeros(T, np.uint16))
+        if what.startswith("kcode"):
+            q.kidx[t, int(index)] = int(value)
+        elif what == "knorm":
+            q.knorm[t, int(index)] = int(value, 16)
+        elif what == "vnorm":
+            q.vnorm[t] = int(value, 16)
+        else:
+            q.vidx[t, int(index)] = int(value)
+        region = O.pack_region(q, d, version=2)
+        assert region[int(off)] == int(byte, 16), line
+        if what != "knorm" and what != "vnorm":
+            assert np.count_nonzero(region) == 1, line
+        n += 1
+    assert n >= 8
+
+
+@pytest.mark.parametrize("bits_kind", ["mixed", "uniform3", "all8", "zeros_and_ones", "ragged"])
+def test_v2_region_round_trip_and_accounting(bits_kind):
+    rng = np.random.default_rng(6)
+    d = 128
+    bits = {"mixed": rng.integers(0, 9, 64), "uniform3": np.full(64, 3), "all8": np.full(64, 8),
+            "zeros_and_ones": np.array([0, 1] * 32),
+            "ragged": np.array([1] * 1 + [2] * 3 + [3] * 33 + [4] * 13 + [5] * 7 + [6] * 5 + [7] * 1 + [8] * 1)}[bits_kind]
+    b_v = 3
+    T = 128 * 2 + 37
+    q = _random_head(rng, bits, b_v, T)
+    region = O.pack_region(q, d, version=2)
+    geo = O.tile_geometry(q.groups, d, b_v, version=2)
+    # byte accounting from the spec: K codes = 4 quadrants x 128 B x sum of nw over chunks
+    words = sum(_nw_spec(g.width, min(32, g.m - 32 * u)) for g in q.groups for u in range(-(-g.m // 32)))
+    assert geo["kcode"] == 4 * 128 * words
+    assert geo["stride"] == geo["kcode"] + 256 * (len(q.groups) + 1) + 16 * d * b_v
+    # never smaller than the dense v1 tile, and equal to it when every group is a multiple of 32 coordinates
+    v1 = O.tile_geometry(q.groups, d, b_v)["stride"]
+    assert geo["stride"] >= v1
+    if all(g.m % 32 == 0 for g in q.groups):
+        assert geo["stride"] == v1
+    assert region.size == 3 * geo["stride"]
+    u = O.unpack_region(region, q.groups, d, b_v, T, version=2)
+    assert np.array_equal(u.kidx, q.kidx) and np.array_equal(u.knorm, q.knorm)
+    assert np.array_equal(u.vidx, q.vidx) and np.array_equal(u.vnorm, q.vnorm)
+    region2 = np.zeros_like(region)
+    for (t0, t1) in [(0, 1), (1, 100), (100, 129), (129, T)]:
+        part = O.QuantizedHead(q.groups, b_v, q.kidx[t0:t1], q.knorm[t0:t1], q.vidx[t0:t1], q.vnorm[t0:t1])
+        O.pack_region(part, d, region2, t_offset=t0, version=2)
+    assert np.array_equal(region, region2)
+    full = O.unpack_region(region, q.groups, d, b_v, 3 * 128, version=2)
+    o = 0
+    for g in q.groups:
+        assert np.all(full.kidx[T:, o:o + g.m] == (8 if g.width == 4 else 0))
+        o += g.m
+    assert not full.vnorm[T:].any() and not full.knorm[T:].any()
+
+
+def test_v1_golden_region_positions_partial_half_steps_and_norm_slot():
+    """Hand-worked byte positions of BGTQ-v1: trailing partial half-steps (r = 2, 4, 6) and norm_slot."""
+    d = 128
+    n = 0
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "layout_region_v1.txt")):
+        line = line.strip()
+        if not line or line.startswith("#"):
+            continue
+        head, item, where = (x.split() for x in line.split("|"))
+        m, b, b_v = (int(x) for x in head)
+        blocks = np.arange(m // 2, dtype=np.int64)
+        groups = [O.Group(b, blocks, np.concatenate([[i, i + 64] for i in blocks]).astype(np.int64))]
+        t = 45
+        q = O.QuantizedHead(groups, b_v, np.zeros((t + 1, m), np.uint8), np.zeros((t + 1, 1), np.uint16),
+                            np.zeros((t + 1, d), np.uint8), np.zeros(t + 1, np.uint16))
+        if item[0] == "kcode":
+            q.kidx[t, int(item[1])] = int(item[2])
+        elif item[0] == "knorm":
+            q.knorm[t, int(item[1])] = int(item[2], 16)
+        else:
+            q.vnorm[t] = int(item[2], 16)
+        region = O.pack_region(q, d)
+        assert region[int(where[0])] == int(where[1], 16), line
+        if item[0] == "kcode":
+            assert np.count_nonzero(region) == 1, line
+        n += 1
+    assert n >= 6

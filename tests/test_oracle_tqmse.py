@@ -37,7 +37,9 @@ def test_rate_law_m128(b, tab128):
         xh = O.dequantize_group(idx, h, b, tab128)
         rel[i] = np.sum((x - xh) ** 2) / np.sum(x * x)
         assert idx.max() < (1 << b)
-        assert h == O.f16_bits(math.sqrt(float(np.sum(x * x)))) or abs(h - O.f16_bits(math.sqrt(float(np.sum(x * x))))) <= 1
+        # stored norm = IEEE binary16 round-to-nearest-even of the unrounded radius (Q10), checked against numpy's conversion
+        assert h == int(np.array([r], dtype=np.float64).astype(np.float16).view(np.uint16)[0])
+        assert r == pytest.approx(math.sqrt(float(np.sum(x * x))), rel=1e-14)
     D = cb.distortion(cb.lloyd_max_levels(b))
     assert rel.mean() <= C_TQ * 4.0 ** (-b)
     assert rel.mean() == pytest.approx(D, rel=0.06)
@@ -131,3 +133,31 @@ def test_block_gtq_beats_uniform_on_logit_error(tab128):
     mae_b = np.mean(np.abs(q_post @ (k_post - Kb).T))
     mae_u = np.mean(np.abs(q_post @ (k_post - Ku).T))
     assert mae_b < 0.7 * mae_u
+
+
+def test_f16_converters_match_ieee_binary16():
+    """orc_f64_to_f16_bits / orc_f16_bits_to_f64 against numpy.float16 (IEEE binary16, round-to-nearest-even): every
+    fp16 value, every midpoint between adjacent fp16 values and its two double neighbours, subnormals, signed zero,
+    random doubles, and the saturation at 65504 / 65520 (Q10)."""
+    L = O.lib()
+    allbits = np.arange(0x7C00, dtype=np.uint16)                       # every finite non-negative fp16
+    vals = allbits.view(np.float16).astype(np.float64)
+    for h, v in zip(allbits[::7].tolist() + [0, 1, 0x03FF, 0x0400, 0x7BFF], vals[::7].tolist() + [vals[0], vals[1], vals[0x3FF], vals[0x400], vals[0x7BFF]]):
+        assert L.orc_f16_bits_to_f64(h) == v
+        assert L.orc_f16_bits_to_f64(h | 0x8000) == -v or v == 0.0
+    assert math.copysign(1.0, L.orc_f16_bits_to_f64(0x8000)) == -1.0
+    mids = (vals[:-1] + vals[1:]) / 2.0                                # exact in fp64
+    cand = np.concatenate([vals, mids, np.nextafter(mids, np.inf), np.nextafter(mids, -np.inf),
+                           np.nextafter(vals, np.inf), np.nextafter(vals[1:], -np.inf),
+                           np.random.default_rng(0).uniform(0.0, 65504.0, 20000),
+                           np.exp(np.random.default_rng(1).uniform(np.log(1e-9), np.log(65504.0), 20000))])
+    cand = cand[cand < 65520.0]
+    want = cand.astype(np.float16).view(np.uint16)
+    got = np.array([L.orc_f64_to_f16_bits(float(x)) for x in cand], dtype=np.uint16)
+    assert np.array_equal(got, want)
+    got_neg = np.array([L.orc_f64_to_f16_bits(float(-x)) for x in cand[::5]], dtype=np.uint16)
+    assert np.array_equal(got_neg, (-cand[::5]).astype(np.float16).view(np.uint16))
+    # saturation: 65504 is the largest finite value; 65520 (the midpoint to 2^16) and everything above saturate
+    for x, bits in [(65504.0, 0x7BFF), (65519.999, 0x7BFF), (65520.0, 0x7BFF), (1e9, 0x7BFF), (-65520.0, 0xFBFF),
+                    (2.0 ** -25, 0x0000), (np.nextafter(2.0 ** -25, 1.0), 0x0001), (2.0 ** -24, 0x0001), (0.0, 0), (-0.0, 0x8000)]:
+        assert L.orc_f64_to_f16_bits(float(x)) == bits, x
