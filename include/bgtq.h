@@ -91,6 +91,18 @@ int bgtq_allocate(const float *scores, int n_heads, int n_blocks, int b_min, int
 typedef struct bgtq_layout bgtq_layout;
 int bgtq_layout_create(const uint8_t *bits, int n_layers, int n_kv_heads, int n_q_heads, int d_h,
                        int b_v, int pairing, const float *rotations, bgtq_layout **out);
+/* The same with an explicit physical format ("static layout metadata"; DESIGN.md sections 4, 4b):
+ *   BGTQ_FORMAT_V1  "fragment order": code words follow the mma.sync fragment order of the round-1 decode kernel;
+ *                   no padding (16*bbar_K + 16*b_V + 2*(n_groups+1) bytes per token at d_h = 128).
+ *   BGTQ_FORMAT_V2  "row order": a code word belongs to ONE operand row (a token for K, a dimension for V), so the
+ *                   decode kernel can write unpacked 8-bit operand rows straight into tensor memory for tcgen05.mma.
+ *                   K groups are stored in chunks of <= 32 coordinates per token, each chunk rounded up to whole 32-bit
+ *                   words (same bytes as V1 when every group holds a multiple of 32 coordinates).
+ * Every call below works on either format unless stated otherwise; the cache bytes of the two formats differ. */
+typedef enum { BGTQ_FORMAT_V1 = 1, BGTQ_FORMAT_V2 = 2 } bgtq_format;
+int bgtq_layout_create_format(const uint8_t *bits, int n_layers, int n_kv_heads, int n_q_heads, int d_h,
+                              int b_v, int pairing, const float *rotations, int format, bgtq_layout **out);
+int bgtq_layout_format(const bgtq_layout *layout);
 void bgtq_layout_destroy(bgtq_layout *layout);
 
 /* Sizes.  cache: one buffer for all layers, order [layer][sequence][head][tile], which the CALLER

@@ -32,7 +32,9 @@ SYMBOLS = [
     "bgtq_paged_cache_bytes", "bgtq_paged_pool_offset", "bgtq_quantize_append_paged", "bgtq_decode_attention_paged",
     "bgtq_quantize_append_rope",
     "bgtq_window_bytes", "bgtq_window_append", "bgtq_decode_attention_protected",
+    "bgtq_layout_create_format", "bgtq_layout_format",
 ]
+FORMAT_V1, FORMAT_V2 = 1, 2
 
 
 class BgtqError(RuntimeError):
@@ -62,6 +64,10 @@ def _load() -> C.CDLL:
     lib.bgtq_allocate.argtypes = [vp, i32, i32, i32, i32, i32, vp, i32, vp]
     lib.bgtq_layout_create.restype = i32
     lib.bgtq_layout_create.argtypes = [vp, i32, i32, i32, i32, i32, i32, vp, C.POINTER(vp)]
+    lib.bgtq_layout_create_format.restype = i32
+    lib.bgtq_layout_create_format.argtypes = [vp, i32, i32, i32, i32, i32, i32, vp, i32, C.POINTER(vp)]
+    lib.bgtq_layout_format.restype = i32
+    lib.bgtq_layout_format.argtypes = [vp]
     lib.bgtq_layout_destroy.restype = None
     lib.bgtq_layout_destroy.argtypes = [vp]
     lib.bgtq_cache_bytes.restype = sz
@@ -199,16 +205,17 @@ class Layout:
     """bgtq_layout: static metadata of the packed cache for an allocation bits[n_layers, H_kv, L]."""
 
     def __init__(self, bits: np.ndarray, n_q_heads: int, d_h: int, b_v: int, rotations: np.ndarray,
-                 pairing: int = PAIR_HALF):
+                 pairing: int = PAIR_HALF, fmt: int = FORMAT_V1):
         bits = np.ascontiguousarray(bits, dtype=np.uint8)
         assert bits.ndim == 3
         self.n_layers, self.n_kv_heads, _ = bits.shape
         self.n_q_heads, self.d_h, self.b_v = n_q_heads, d_h, b_v
         rot = np.ascontiguousarray(rotations, dtype=np.float32)
         h = C.c_void_p()
-        _check(_lib.bgtq_layout_create(bits.ctypes.data, self.n_layers, self.n_kv_heads, n_q_heads, d_h, b_v,
-                                       pairing, rot.ctypes.data, C.byref(h)))
+        _check(_lib.bgtq_layout_create_format(bits.ctypes.data, self.n_layers, self.n_kv_heads, n_q_heads, d_h, b_v,
+                                              pairing, rot.ctypes.data, fmt, C.byref(h)))
         self._h = h
+        self.fmt = int(_lib.bgtq_layout_format(h))
 
     def __del__(self):
         h = getattr(self, "_h", None)

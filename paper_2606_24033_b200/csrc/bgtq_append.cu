@@ -1,5 +1,5 @@
 // bgtq_append.cu -- quantize-on-append: TQ-MSE per same-width K group and for V
-// (PAPER.md:49, 108), packed into the BGTQ-v1 tile layout.
+// (PAPER.md:49, 108), packed into the BGTQ-v1 or BGTQ-v2 tile layout (DESIGN.md sections 4, 4b).
 //
 // Exactness: the arithmetic is the fp64 sequence of DESIGN.md section 3 -- fma chains in index
 // order, IEEE sqrt / divide, strict '>' against tau_k * sigma -- written with explicit
@@ -51,6 +51,32 @@ __device__ __forceinline__ void put_field(uint32_t *base, int wstride, int b, in
         uint32_t v = base[word * wstride];
         v = (v & ~(1u << pos)) | (((f >> bit) & 1u) << pos);
         base[word * wstride] = v;
+    }
+}
+
+// BGTQ-v2: bits that code f at slot k of a chunk (width b, r slots) contributes to word j of the chunk
+__device__ __forceinline__ void slot_bits_v2(int b, int r, int k, int j, unsigned f, uint32_t &val, uint32_t &mask)
+{
+    if (b == 1) {
+        if (j == 0) { const int pos = 8 * (k & 3) + 7 - (k >> 2); val |= (f & 1u) << pos; mask |= 1u << pos; }
+    } else if (b == 2) {
+        if ((k >> 4) == j) {
+            const int kk = k & 15, Q = kk >> 2, e = kk & 3, pos = 4 * ((Q & 1) * 4 + e) + 2 * (Q >> 1);
+            val |= (f & 3u) << pos; mask |= 3u << pos;
+        }
+    } else if (b == 3 || b == 4) {
+        if (b == 4) f = f >= 8 ? (f - 8) : (8u | (7u - f));            // sign-magnitude storage
+        const int nwm = r > 24 ? 3 : (r + 7) / 8;
+        if (j < nwm) {
+            if (k < 24) {
+                if ((k >> 3) == j) { const int pos = 4 * (k & 7); val |= (f & 7u) << pos; mask |= 7u << pos; }
+            } else { const int pos = 4 * (k - 24) + 3; val |= ((f >> j) & 1u) << pos; mask |= 1u << pos; }
+        } else if (b == 4) { const int pos = 8 * (k & 3) + 7 - (k >> 2); val |= ((f >> 3) & 1u) << pos; mask |= 1u << pos; }
+    } else {
+        const int sh = b * k - 32 * j;                                  // field = bits [b*k, b*k+b) of the stream
+        const uint32_t fm = (1u << b) - 1u;
+        if (sh >= 0 && sh < 32) { val |= f << sh; mask |= fm << sh; }
+        else if (sh < 0 && sh > -b) { val |= f >> (-sh); mask |= fm >> (-sh); }
     }
 }
 
@@ -113,7 +139,7 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
     }
     if (tid == 0) {  // list of half-step units of the K code section
         int n = 0, j = 0;
-        for (int ks = 0; ks < M.n_ksteps; ++ks) {
+        for (int ks = 0; ks < (M.format == 2 ? 0 : M.n_ksteps); ++ks) {   // (BGTQ-v2 packs from M.chunks, step 5)
             const KStep &K = M.ksteps[ks];
             int g = K.flags >> 4;
             if (K.flags & 1) j = 0;
@@ -306,6 +332,39 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
         }
         __syncthreads();
         // ---- 5. pack the sub-batch's fields; each (unit, lane) word set has exactly one owner
+        if (M.format == 2) {
+            // BGTQ-v2: a K word belongs to one token (composed whole), a V word to one dimension and 32 tokens (read-modify-write)
+            const int nch = M.n_ksteps, kq4 = M.kcode_bytes >> 4;        // words of one quadrant's K section
+            for (int it = tid; it < kSub * nch * 8; it += kAppendThreads) {
+                const int j = it & 7, ch = (it >> 3) % nch, tt = (it >> 3) / nch;
+                const Chunk2 C2 = M.chunks[ch];
+                const int64_t tok = base + tt;
+                if (j >= C2.nw || tok < nlo || tok >= nhi) continue;
+                const int tau = i * kSub + tt;
+                uint32_t val = 0, mask = 0;
+                const uint8_t *ip = idxs + tt * 256 + C2.ustart;
+                for (int k = 0; k < C2.r; ++k) slot_bits_v2(C2.b, C2.r, k, j, ip[k], val, mask);
+                tbuf[(tau >> 5) * kq4 + (C2.off >> 2) + j * 32 + (tau & 31)] = val;
+            }
+            const int c = i >> 1, k0 = (i & 1) * kSub;
+            for (int it = tid; it < kDh * b_v; it += kAppendThreads) {
+                const int d = it % kDh, j = it / kDh;
+                uint32_t val = 0, mask = 0;
+                for (int tt = tt_lo; tt < tt_hi; ++tt) slot_bits_v2(b_v, 32, k0 + tt, j, idxs[tt * 256 + 128 + d], val, mask);
+                uint32_t *wp = tbuf + ((M.vcode_off + ((d >> 5) * 4 + c) * b_v * 128) >> 2) + j * 32 + (d & 31);
+                *wp = (*wp & ~mask) | val;
+            }
+            if (tid < kSub * (ng + 1)) {                                   // fp16 norms in natural token order
+                const int tt = tid / (ng + 1), g = tid % (ng + 1);
+                const int64_t tok = base + tt;
+                if (tok >= nlo && tok < nhi) {
+                    const int off = g < ng ? M.knorm_off + 256 * g : M.vnorm_off;
+                    reinterpret_cast<uint16_t *>(reinterpret_cast<uint8_t *>(tbuf) + off)[i * kSub + tt] = nrm[tt * 9 + g];
+                }
+            }
+            __syncthreads();
+            continue;
+        }
         const int kitems = n_units * 32;
         for (int it = tid; it < kitems + 16 * 32; it += kAppendThreads) {
             if (it < kitems) {
@@ -396,7 +455,7 @@ int launch_quantize_append(const bgtq_layout *lay, int layer, int n_layers, void
     auto launch = [&](auto plain, auto roped, auto paged, auto *kp, auto *vp) {
         auto kern = pm ? paged : (rope ? roped : plain);
         kern<<<grid, kAppendThreads, smem, st>>>(metas, (uint8_t *)cache, kp, vp, lay->d_cb64, lay->d_rot_t, batch, n_new,
-                                                 lay->n_kv_heads, seq_len, n_cap, n_cap * kTile, pt, pstride, n_pages, rc, rs,
+                                                 lay->n_kv_heads, seq_len, n_cap, max_tokens, pt, pstride, n_pages, rc, rs,
                                                  lay->pairing);
     };
     if (dt == BGTQ_F32)
@@ -408,7 +467,7 @@ int launch_quantize_append(const bgtq_layout *lay, int layer, int n_layers, void
     count_launch();
     CUDA_TRY(cudaGetLastError());
     if (advance) {
-        advance_seq_len_kernel<<<(batch + 127) / 128, 128, 0, st>>>(seq_len, batch, n_new, n_cap * kTile);
+        advance_seq_len_kernel<<<(batch + 127) / 128, 128, 0, st>>>(seq_len, batch, n_new, max_tokens);
         count_launch();
         CUDA_TRY(cudaGetLastError());
     }

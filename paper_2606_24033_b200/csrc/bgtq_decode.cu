@@ -25,6 +25,7 @@
 #include <vector>
 
 #include "bgtq_internal.h"
+#include "bgtq_device.cuh"
 
 namespace bgtq {
 
@@ -41,79 +42,7 @@ static_assert(sizeof(HeadMeta) % 4 == 0 && sizeof(HeadMeta) <= 128 * 4, "qfold_k
 #ifndef BGTQ_NO_P5
 #define BGTQ_NO_P5 0
 #endif
-constexpr int kMaxWarpsPerSM = 16;
-constexpr int kMaxBatch = 256;
 constexpr int kQfHalves = kMaxKSteps * 8 * 16;      // fp16 q' fragments per (layer, seq, kv head)
-constexpr int kPartialFloats = 8 * 130;             // (m, l, acc[128]) for 8 head slots
-
-// ---------------------------------------------------------------- small PTX wrappers
-__device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t s)
-{
-    uint32_t r;
-    asm("prmt.b32 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(s));
-    return r;
-}
-__device__ __forceinline__ void mma16816(float (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2,
-                                         uint32_t a3, uint32_t b0, uint32_t b1)
-{
-    asm("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
-                 : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
-                 : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
-}
-// same with C = 0 (the zero register): starts an accumulator without a separate zero-fill
-__device__ __forceinline__ void mma16816_z(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2,
-                                           uint32_t a3, uint32_t b0, uint32_t b1)
-{
-    asm("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%10,%10,%10,%10};"
-        : "=f"(d[0]), "=f"(d[1]), "=f"(d[2]), "=f"(d[3])
-        : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1), "f"(0.f));
-}
-__device__ __forceinline__ uint32_t movmatrix_trans(uint32_t x)
-{
-    uint32_t r;
-    asm volatile("movmatrix.sync.aligned.m8n8.trans.b16 %0, %1;" : "=r"(r) : "r"(x));
-    return r;
-}
-__device__ __forceinline__ float fast_exp2(float x)
-{
-    float r;
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
-    return r;
-}
-__device__ __forceinline__ uint32_t pack_half2(float lo, float hi)
-{
-    uint32_t r;
-    asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
-    return r;
-}
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint32_t bar, int count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
-{
-    uint32_t done;
-    do {
-        asm volatile("{\n\t.reg .pred p;\n\t"
-                     "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-                     "selp.u32 %0, 1, 0, p;\n\t}"
-                     : "=r"(done) : "r"(bar), "r"(parity) : "memory");
-    } while (!done);
-}
-__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
-}
-__device__ __forceinline__ void fence_proxy_async()
-{
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-}
 
 // Optional: shifts issued to the FMA pipe (IMAD) instead of the ALU pipe (tuning switches)
 __device__ __forceinline__ uint32_t shl_k(uint32_t x, int k)
@@ -238,82 +167,6 @@ __device__ __forceinline__ void build_pools(const uint16_t *cb16, uint32_t *pool
     pools[1] = plane(3, 0);  pools[2] = plane(3, 1);
     pools[3] = plane(7, 0);  pools[4] = plane(11, 0); pools[5] = plane(7, 1);  pools[6] = plane(11, 1);
     pools[7] = plane(15 + 8, 0); pools[8] = plane(15 + 12, 0); pools[9] = plane(15 + 8, 1); pools[10] = plane(15 + 12, 1);
-}
-
-// ---------------------------------------------------------------- programmatic dependent launch
-// qfold -> decode -> combine are launched back to back on one stream.  decode and combine are launched with the
-// programmatic-stream-serialization attribute: their CTAs may start while the previous kernel is still running
-// (pdl_trigger in that kernel), run their prologue (LUTs, prefix sums, slot lists), and block in pdl_wait until the
-// previous kernel has completed and its writes are visible.  Nothing written by a predecessor is read before pdl_wait.
-__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
-__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
-
-// ---------------------------------------------------------------- work partition
-// Global tile list [layer][sequence][kv head][tile]; pre[] = prefix sums of tiles per sequence.
-struct Sched {
-    int n_layers, batch, Hkv;
-    int tiles_sum;          // sum over sequences of ceil(seq_len/128)
-    int total;              // n_layers * Hkv * tiles_sum
-    int n_ctas, W;          // balanced two-level split: CTA c owns [cta_lo(c), cta_lo(c+1)), its W warps split that evenly
-};
-__device__ __forceinline__ int cta_lo(const Sched &s, int c) { return (int)(((int64_t)c * s.total) / s.n_ctas); }
-__device__ __forceinline__ int warp_lo(const Sched &s, int c, int w)
-{
-    const int lo = cta_lo(s, c), len = cta_lo(s, c + 1) - lo;
-    return lo + (int)(((int64_t)w * len) / s.W);
-}
-
-// Protected regime: of the T cached tokens of a sequence the packed cache serves
-// [n_sink, T - n_recent) only -- the first n_sink and the last n_recent tokens are attended from fp16 windows by
-// window_kernel.  Number of packed tokens to scan (tokens below n_sink are masked inside tile 0); 0 when the range is empty.
-__device__ __forceinline__ int64_t packed_len(int64_t T, int n_sink, int n_recent)
-{
-    const int64_t hi = T - n_recent;
-    return hi > n_sink ? hi : 0;
-}
-__device__ __forceinline__ void build_prefix(const int32_t *seq_len, int batch, int64_t cap_tokens, int *pre,
-                                             int n_sink = 0, int n_recent = 0)
-{
-    // called by one thread; batch <= kMaxBatch
-    int acc = 0;
-    pre[0] = 0;
-    for (int b = 0; b < batch; ++b) {
-        int64_t n = seq_len[b];
-        n = n < 0 ? 0 : (n > cap_tokens ? cap_tokens : n);
-        n = packed_len(n, n_sink, n_recent);
-        acc += (int)((n + kTile - 1) / kTile);
-        pre[b + 1] = acc;
-    }
-}
-
-__device__ __forceinline__ Sched make_sched(int n_layers, int batch, int Hkv, const int *pre, int n_ctas, int W)
-{
-    Sched s;
-    s.n_layers = n_layers; s.batch = batch; s.Hkv = Hkv;
-    s.tiles_sum = pre[batch];
-    s.total = n_layers * Hkv * s.tiles_sum;
-    s.n_ctas = n_ctas; s.W = W;
-    return s;
-}
-
-struct TilePos { int l, b, h, t, tiles_b, pair, pair_start; };
-
-__device__ __forceinline__ TilePos locate(int x, const Sched &s, const int *pre)
-{
-    TilePos p;
-    const int per_layer = s.Hkv * s.tiles_sum;
-    p.l = x / per_layer;
-    const int r = x - p.l * per_layer;
-    int b = 0;
-    while (b + 1 < s.batch && r >= pre[b + 1] * s.Hkv) ++b;
-    p.b = b;
-    p.tiles_b = pre[b + 1] - pre[b];
-    const int r2 = r - pre[b] * s.Hkv;
-    p.h = r2 / p.tiles_b;
-    p.t = r2 - p.h * p.tiles_b;
-    p.pair = (p.l * s.batch + b) * s.Hkv + p.h;
-    p.pair_start = x - p.t;
-    return p;
 }
 
 // ---------------------------------------------------------------- prologue: Q-side rotation fold
@@ -1401,6 +1254,54 @@ int profile_decode_read(double *ms_sum, int *count)
     return BGTQ_OK;
 }
 
+bool profile_decode_on() { return g_prof; }
+int profile_decode_begin(cudaStream_t st)
+{
+    if (!g_prof) return BGTQ_OK;
+    if (g_prof_used == g_prof_events.size()) {
+        cudaEvent_t e0 = nullptr, e1 = nullptr;
+        CUDA_TRY(cudaEventCreate(&e0));
+        CUDA_TRY(cudaEventCreate(&e1));
+        g_prof_events.emplace_back(e0, e1);
+    }
+    CUDA_TRY(cudaEventRecord(g_prof_events[g_prof_used].first, st));
+    return BGTQ_OK;
+}
+int profile_decode_end(cudaStream_t st)
+{
+    if (!g_prof) return BGTQ_OK;
+    CUDA_TRY(cudaEventRecord(g_prof_events[g_prof_used].second, st));
+    ++g_prof_used;
+    return BGTQ_OK;
+}
+
+int launch_combine(const float *partials, const int32_t *seq_len, const float *rot128, int n_layers, int batch, int Hkv, int G,
+                   int64_t n_cap, int n_ctas, int W, void *out, int n_sink, int n_recent, int win_slot, bool pdl, cudaStream_t st)
+{
+    cudaLaunchConfig_t cfg = {};
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
+    cfg.gridDim = dim3(n_layers * batch * Hkv * G); cfg.blockDim = dim3(128); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, combine_kernel, partials, seq_len, rot128, n_layers, batch, Hkv, G, n_cap, n_ctas, W,
+                       (__nv_bfloat16 *)out, n_sink, n_recent, win_slot);
+    count_launch();
+    CUDA_TRY(cudaGetLastError());
+    return BGTQ_OK;
+}
+
+int launch_window(const void *win_k, const void *win_v, const void *q, const int32_t *seq_len, const float *rot128_t,
+                  float *partials, int pairs, int batch, int Hkv, int G, int64_t n_cap, int n_sink, int n_recent,
+                  float scale_log2e, int win_slot, cudaStream_t st)
+{
+    window_kernel<<<pairs * G, 128, 0, st>>>((const __half *)win_k, (const __half *)win_v, (const __nv_bfloat16 *)q, seq_len,
+                                             rot128_t, partials, batch, Hkv, G, n_cap, n_sink, n_recent, scale_log2e, win_slot);
+    count_launch();
+    CUDA_TRY(cudaGetLastError());
+    return BGTQ_OK;
+}
+
 template <int W, bool PAGED>
 static int launch_decode_w(const DecodeParams &P, int grid, size_t smem, cudaStream_t st)
 {
@@ -1409,18 +1310,7 @@ static int launch_decode_w(const DecodeParams &P, int grid, size_t smem, cudaStr
         CUDA_TRY(cudaFuncSetAttribute(decode_kernel<W, PAGED>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - (W == 16 ? 2560 : kStaticSmem)));
         attr_set = true;
     }
-    cudaEvent_t e0 = nullptr, e1 = nullptr;
-    if (g_prof) {
-        if (g_prof_used == g_prof_events.size()) {
-            CUDA_TRY(cudaEventCreate(&e0));
-            CUDA_TRY(cudaEventCreate(&e1));
-            g_prof_events.emplace_back(e0, e1);
-        }
-        e0 = g_prof_events[g_prof_used].first;
-        e1 = g_prof_events[g_prof_used].second;
-        ++g_prof_used;
-        CUDA_TRY(cudaEventRecord(e0, st));
-    }
+    if (int rc = profile_decode_begin(st)) return rc;
     {
         cudaLaunchConfig_t cfg = {};
         cudaLaunchAttribute at[1];
@@ -1440,8 +1330,7 @@ static int launch_decode_w(const DecodeParams &P, int grid, size_t smem, cudaStr
             return BGTQ_ECUDA;
         }
     }
-    if (g_prof) CUDA_TRY(cudaEventRecord(e1, st));
-    return BGTQ_OK;
+    return profile_decode_end(st);
 }
 
 int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *cache, const void *q,
@@ -1463,11 +1352,8 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
                  // included, is complete when it starts); qfold_kernel is then launched programmatically behind it and the
                  // two run side by side.  Completion order is kept by qfold_kernel's trailing griddepcontrol.wait:
                  // window -> qfold -> decode -> combine, each waiting for its predecessor only.
-        window_kernel<<<pairs * G, 128, 0, st>>>((const __half *)win->k, (const __half *)win->v, (const __nv_bfloat16 *)q, seq_len,
-                                                 lay->d_rot_t + rot_offset(kDh), partials, batch, Hkv, G, n_cap, n_sink, n_recent,
-                                                 scale * 1.4426950408889634f, win_slot);
-        count_launch();
-        CUDA_TRY(cudaGetLastError());
+        if (int rc = launch_window(win->k, win->v, q, seq_len, lay->d_rot_t + rot_offset(kDh), partials, pairs, batch, Hkv, G, n_cap,
+                                   n_sink, n_recent, scale * 1.4426950408889634f, win_slot, st)) return rc;
     }
     if (win && !g_prof) {
         cudaLaunchConfig_t cfg = {};
@@ -1515,19 +1401,8 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
     count_launch();
     CUDA_TRY(cudaGetLastError());
 
-    {
-        cudaLaunchConfig_t cfg = {};
-        cudaLaunchAttribute at[1];
-        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-        at[0].val.programmaticStreamSerializationAllowed = g_prof ? 0 : 1;
-        cfg.gridDim = dim3(pairs * G); cfg.blockDim = dim3(128); cfg.dynamicSmemBytes = 0; cfg.stream = st;
-        cfg.attrs = at; cfg.numAttrs = 1;
-        cudaLaunchKernelEx(&cfg, combine_kernel, (const float *)partials, seq_len, (const float *)(lay->d_rot + rot_offset(kDh)),
-                           n_layers, batch, Hkv, G, n_cap, grid, W, (__nv_bfloat16 *)out, n_sink, n_recent, win_slot);
-    }
-    count_launch();
-    CUDA_TRY(cudaGetLastError());
-    return BGTQ_OK;
+    return launch_combine(partials, seq_len, lay->d_rot + rot_offset(kDh), n_layers, batch, Hkv, G, n_cap, grid, W, out, n_sink,
+                          n_recent, win_slot, !g_prof, st);
 }
 
 int launch_window_append(const void *k_new, const void *v_new, int dt, int n_layers, int batch, int n_new, int Hkv,
@@ -2232,10 +2107,6 @@ prefill_tc_kernel(const PrefillParams P)
 enum { WS_KFULL = 0, WS_VFULL, WS_KREADY, WS_VREADY, WS_SFULL, WS_SFREE, WS_PREADY, WS_ODONE, WS_NBARS };
 constexpr int kWsProducers = 7;
 
-__device__ __forceinline__ void mbar_arrive(uint32_t bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(bar) : "memory");
-}
 
 __global__ void __launch_bounds__(kTcThreads, 1)
 prefill_ws_kernel(const PrefillParams P)

@@ -160,11 +160,80 @@ static void build_head_meta(const uint8_t *bits, int d_h, int b_v, int pairing, 
     m.tile_stride = m.vcode_off + 16 * d_h * b_v;
 }
 
+// BGTQ-v2: words per lane of a chunk of r slots at width b
+static int chunk_words(int b, int r)
+{
+    const int nwm = r > 24 ? 3 : (r + 7) / 8;
+    switch (b) {
+    case 1: return 1;
+    case 2: return (r + 15) / 16;
+    case 3: return nwm;
+    case 4: return nwm + 1;
+    default: return (r * b + 31) / 32;
+    }
+}
+
+static void build_head_meta_v2(const uint8_t *bits, int d_h, int b_v, int pairing, HeadMeta &m)
+{
+    std::memset(&m, 0, sizeof(m));
+    const int L = d_h / 2;
+    m.b_v = b_v;
+    m.format = 2;
+    int ng = 0, kdim = 0, off = 0, nch = 0;
+    for (int w = 1; w <= BGTQ_MAX_WIDTH; ++w) {
+        int cnt = 0;
+        for (int i = 0; i < L; ++i)
+            if (bits[i] == w) {
+                int a = pairing == BGTQ_PAIR_HALF ? i : 2 * i;
+                int b = pairing == BGTQ_PAIR_HALF ? i + L : 2 * i + 1;
+                m.coords[kdim + cnt++] = (uint8_t)a;
+                m.coords[kdim + cnt++] = (uint8_t)b;
+            }
+        if (!cnt) continue;
+        m.gb[ng] = (uint8_t)w;
+        m.gm[ng] = (uint16_t)cnt;
+        m.gstart[ng] = (uint16_t)kdim;
+        m.goff[ng] = off;
+        for (int u = 0; 32 * u < cnt; ++u) {
+            Chunk2 &c = m.chunks[nch++];
+            const int r = cnt - 32 * u >= 32 ? 32 : cnt - 32 * u;
+            c.off = (uint16_t)off;
+            c.ustart = (uint16_t)(kdim + 32 * u);
+            c.b = (uint8_t)w;
+            c.r = (uint8_t)r;
+            c.nw = (uint8_t)chunk_words(w, r);
+            c.flags = (uint8_t)((u == 0 ? 1 : 0) | (ng << 4));
+            off += 128 * c.nw;
+        }
+        kdim += cnt;
+        ++ng;
+    }
+    m.n_groups = ng;
+    m.kdim = kdim;
+    m.n_ksteps = nch;
+    m.kcode_bytes = 4 * off;                 // four quadrants of 32 tokens
+    m.knorm_off = m.kcode_bytes;
+    m.vnorm_off = m.knorm_off + 256 * ng;
+    m.vcode_off = m.vnorm_off + 256;
+    m.tile_stride = m.vcode_off + 16 * d_h * b_v;
+}
+
 extern "C" int bgtq_layout_create(const uint8_t *bits, int n_layers, int n_kv_heads, int n_q_heads,
                                   int d_h, int b_v, int pairing, const float *rotations,
                                   bgtq_layout **out)
 {
+    return bgtq_layout_create_format(bits, n_layers, n_kv_heads, n_q_heads, d_h, b_v, pairing, rotations,
+                                     BGTQ_FORMAT_V1, out);
+}
+
+extern "C" int bgtq_layout_format(const bgtq_layout *lay) { return lay ? lay->format : 0; }
+
+extern "C" int bgtq_layout_create_format(const uint8_t *bits, int n_layers, int n_kv_heads, int n_q_heads,
+                                         int d_h, int b_v, int pairing, const float *rotations, int format,
+                                         bgtq_layout **out)
+{
     if (!bits || !rotations || !out) FAIL(BGTQ_EINVAL, "bgtq_layout_create: null pointer");
+    if (format != BGTQ_FORMAT_V1 && format != BGTQ_FORMAT_V2) FAIL(BGTQ_EINVAL, "bgtq_layout_create: format must be BGTQ_FORMAT_V1 or BGTQ_FORMAT_V2");
     if (d_h != kDh) FAIL(BGTQ_EINVAL, "bgtq_layout_create: d_h must be 128");
     if (n_layers <= 0 || n_kv_heads <= 0 || n_q_heads <= 0 || n_q_heads % n_kv_heads)
         FAIL(BGTQ_EINVAL, "bgtq_layout_create: bad layer/head counts");
@@ -179,6 +248,7 @@ extern "C" int bgtq_layout_create(const uint8_t *bits, int n_layers, int n_kv_he
     if (!lay) FAIL(BGTQ_EINVAL, "bgtq_layout_create: out of host memory");
     lay->n_layers = n_layers; lay->n_kv_heads = n_kv_heads; lay->n_q_heads = n_q_heads;
     lay->d_h = d_h; lay->b_v = b_v; lay->pairing = pairing;
+    lay->format = format; lay->d_planes = nullptr;
     lay->d_meta = nullptr; lay->d_rot = nullptr; lay->d_rot_t = nullptr; lay->d_cb16 = nullptr; lay->d_cb64 = nullptr;
     lay->meta.resize((size_t)n_layers * n_kv_heads);
     int64_t prefix = 0;
@@ -187,7 +257,9 @@ extern "C" int bgtq_layout_create(const uint8_t *bits, int n_layers, int n_kv_he
         int64_t lsum = 0;
         for (int h = 0; h < n_kv_heads; ++h) {
             HeadMeta &m = lay->meta[(size_t)l * n_kv_heads + h];
-            build_head_meta(bits + ((size_t)l * n_kv_heads + h) * L, d_h, b_v, pairing, m);
+            if (format == BGTQ_FORMAT_V2) build_head_meta_v2(bits + ((size_t)l * n_kv_heads + h) * L, d_h, b_v, pairing, m);
+            else build_head_meta(bits + ((size_t)l * n_kv_heads + h) * L, d_h, b_v, pairing, m);
+            m.format = format;
             m.layer_prefix = prefix;
             m.head_prefix = lsum;
             lsum += m.tile_stride;
@@ -220,6 +292,10 @@ extern "C" int bgtq_layout_create(const uint8_t *bits, int n_layers, int n_kv_he
             cb16[(1 << b) - 1 + k] = u;
         }
     }
+    std::vector<uint8_t> planes(kPlaneBytes, 0);
+    lay->kappa[0] = 1.f;
+    for (int b = 1; b <= BGTQ_MAX_WIDTH; ++b)
+        codebook_planes(b, &lay->kappa[b], planes.data() + (1 << b) - 1, planes.data() + 512 + (1 << b) - 1);
     cudaError_t e = cudaSuccess;
     int dev = 0;
     if (e == cudaSuccess) e = cudaGetDevice(&dev);
@@ -229,6 +305,8 @@ extern "C" int bgtq_layout_create(const uint8_t *bits, int n_layers, int n_kv_he
     if (e == cudaSuccess) e = cudaMalloc(&lay->d_rot_t, rot_n * sizeof(float));
     if (e == cudaSuccess) e = cudaMalloc(&lay->d_cb16, 512 * sizeof(uint16_t));
     if (e == cudaSuccess) e = cudaMalloc(&lay->d_cb64, 512 * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc(&lay->d_planes, kPlaneBytes);
+    if (e == cudaSuccess) e = cudaMemcpy(lay->d_planes, planes.data(), kPlaneBytes, cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(lay->d_meta, lay->meta.data(), lay->meta.size() * sizeof(HeadMeta), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(lay->d_rot, rotations, rot_n * sizeof(float), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(lay->d_rot_t, rot_t.data(), rot_n * sizeof(float), cudaMemcpyHostToDevice);
@@ -246,7 +324,7 @@ extern "C" void bgtq_layout_destroy(bgtq_layout *lay)
 {
     if (!lay) return;
     cudaFree(lay->d_meta); cudaFree(lay->d_rot); cudaFree(lay->d_rot_t);
-    cudaFree(lay->d_cb16); cudaFree(lay->d_cb64);
+    cudaFree(lay->d_cb16); cudaFree(lay->d_cb64); cudaFree(lay->d_planes);
     delete lay;
 }
 
@@ -275,10 +353,24 @@ extern "C" int64_t bgtq_region_offset(const bgtq_layout *lay, int layer, int seq
     const HeadMeta &m = lay->meta[(size_t)layer * lay->n_kv_heads + kv_head];
     return n_cap_tiles(max_tokens) * ((int64_t)batch * m.layer_prefix + (int64_t)seq * m.layer_sum + m.head_prefix);
 }
+static size_t decode_ws_any(const bgtq_layout *lay, int batch, int n_layers);
 extern "C" size_t bgtq_workspace_bytes(const bgtq_layout *lay, int batch, int n_layers_per_call)
 {
     if (!lay || batch <= 0 || n_layers_per_call <= 0) return 0;
-    return decode_ws_bytes(lay, batch, n_layers_per_call);
+    return decode_ws_any(lay, batch, n_layers_per_call);
+}
+
+// split-KV decode: the BGTQ-v1 mma.sync kernel or the BGTQ-v2 tcgen05 kernel, by the layout's format
+static size_t decode_ws_any(const bgtq_layout *lay, int batch, int n_layers)
+{
+    return lay->format == 2 ? decode2_ws_bytes(lay, batch, n_layers) : decode_ws_bytes(lay, batch, n_layers);
+}
+static int launch_decode_any(const bgtq_layout *lay, int layer0, int n_layers, const void *cache, const void *q,
+                             const int32_t *seq_len, int batch, int64_t max_tokens, float scale, void *out, void *ws,
+                             size_t ws_bytes, const PageMap *pm, cudaStream_t st, const Window *win = nullptr)
+{
+    if (lay->format == 2) return launch_decode2(lay, layer0, n_layers, cache, q, seq_len, batch, max_tokens, scale, out, ws, ws_bytes, pm, st, win);
+    return launch_decode(lay, layer0, n_layers, cache, q, seq_len, batch, max_tokens, scale, out, ws, ws_bytes, pm, st, win);
 }
 
 // ------------------------------------------------------------------ a4 / a5 wrappers
@@ -358,10 +450,10 @@ extern "C" int bgtq_decode_attention_paged(const bgtq_layout *lay, int layer0, i
     if (layer0 < 0 || n_layers <= 0 || layer0 + n_layers > lay->n_layers) FAIL(BGTQ_EINVAL, "bgtq_decode_attention_paged: layer range");
     if (batch <= 0 || table_stride <= 0 || n_pages <= 0) FAIL(BGTQ_EINVAL, "bgtq_decode_attention_paged: batch/table_stride/n_pages");
     if (!(softmax_scale > 0.0f) || std::isinf(softmax_scale)) FAIL(BGTQ_EINVAL, "bgtq_decode_attention_paged: softmax_scale must be finite and > 0");
-    if (workspace_bytes < decode_ws_bytes(lay, batch, n_layers)) FAIL(BGTQ_EWORKSPACE, "bgtq_decode_attention_paged: workspace too small");
+    if (workspace_bytes < decode_ws_any(lay, batch, n_layers)) FAIL(BGTQ_EWORKSPACE, "bgtq_decode_attention_paged: workspace too small");
     const PageMap pm{page_table, table_stride, n_pages};
-    return launch_decode(lay, layer0, n_layers, cache, q, seq_len, batch, (int64_t)table_stride * kTile, softmax_scale,
-                         out, workspace, workspace_bytes, &pm, (cudaStream_t)stream);
+    return launch_decode_any(lay, layer0, n_layers, cache, q, seq_len, batch, (int64_t)table_stride * kTile, softmax_scale,
+                             out, workspace, workspace_bytes, &pm, (cudaStream_t)stream);
 }
 
 extern "C" int bgtq_quantize_append(const bgtq_layout *lay, int layer, void *cache, const void *k_new,
@@ -389,9 +481,9 @@ extern "C" int bgtq_decode_attention_layers(const bgtq_layout *lay, int layer0, 
     if (layer0 < 0 || n_layers <= 0 || layer0 + n_layers > lay->n_layers) FAIL(BGTQ_EINVAL, "bgtq_decode_attention: layer range");
     if (batch <= 0 || max_tokens <= 0) FAIL(BGTQ_EINVAL, "bgtq_decode_attention: batch/max_tokens");
     if (!(softmax_scale > 0.0f) || std::isinf(softmax_scale)) FAIL(BGTQ_EINVAL, "bgtq_decode_attention: softmax_scale must be finite and > 0");
-    if (workspace_bytes < decode_ws_bytes(lay, batch, n_layers)) FAIL(BGTQ_EWORKSPACE, "bgtq_decode_attention: workspace too small");
-    return launch_decode(lay, layer0, n_layers, cache, q, seq_len, batch, max_tokens, softmax_scale,
-                         out, workspace, workspace_bytes, nullptr, (cudaStream_t)stream);
+    if (workspace_bytes < decode_ws_any(lay, batch, n_layers)) FAIL(BGTQ_EWORKSPACE, "bgtq_decode_attention: workspace too small");
+    return launch_decode_any(lay, layer0, n_layers, cache, q, seq_len, batch, max_tokens, softmax_scale,
+                             out, workspace, workspace_bytes, nullptr, (cudaStream_t)stream);
 }
 
 extern "C" int bgtq_decode_attention(const bgtq_layout *lay, int layer, const void *cache, const void *q,
@@ -415,12 +507,12 @@ extern "C" int bgtq_decode_attention_protected(const bgtq_layout *lay, int layer
     if (!(softmax_scale > 0.0f) || std::isinf(softmax_scale)) FAIL(BGTQ_EINVAL, "bgtq_decode_attention_protected: softmax_scale must be finite and > 0");
     if (n_sink < 0 || n_recent < 0 || n_sink >= BGTQ_TILE_TOKENS || n_sink + n_recent < 1 || n_sink + n_recent > 1024)
         FAIL(BGTQ_EINVAL, "bgtq_decode_attention_protected: need 0 <= n_sink < 128, n_recent >= 0, 1 <= n_sink + n_recent <= 1024");
-    if (workspace_bytes < decode_ws_bytes(lay, batch, n_layers)) FAIL(BGTQ_EWORKSPACE, "bgtq_decode_attention_protected: workspace too small");
+    if (workspace_bytes < decode_ws_any(lay, batch, n_layers)) FAIL(BGTQ_EWORKSPACE, "bgtq_decode_attention_protected: workspace too small");
     const size_t per_layer = (size_t)batch * lay->n_kv_heads * (size_t)(n_sink + n_recent) * lay->d_h;   // fp16 elements
     const Window win = {(const uint16_t *)win_k + (size_t)layer0 * per_layer, (const uint16_t *)win_v + (size_t)layer0 * per_layer,
                         n_sink, n_recent};
-    return launch_decode(lay, layer0, n_layers, cache, q, seq_len, batch, max_tokens, softmax_scale, out, workspace,
-                         workspace_bytes, nullptr, (cudaStream_t)stream, &win);
+    return launch_decode_any(lay, layer0, n_layers, cache, q, seq_len, batch, max_tokens, softmax_scale, out, workspace,
+                             workspace_bytes, nullptr, (cudaStream_t)stream, &win);
 }
 
 extern "C" size_t bgtq_window_bytes(const bgtq_layout *lay, int batch, int n_sink, int n_recent)
@@ -456,6 +548,7 @@ extern "C" int bgtq_prefill_attention(const bgtq_layout *lay, int layer, const v
 {
     if (!lay || !cache || !q || !seq_len || !out || !workspace) FAIL(BGTQ_EINVAL, "bgtq_prefill_attention: null pointer");
     if (layer < 0 || layer >= lay->n_layers) FAIL(BGTQ_EINVAL, "bgtq_prefill_attention: layer out of range");
+    if (lay->format != BGTQ_FORMAT_V1) FAIL(BGTQ_EINVAL, "bgtq_prefill_attention: built for BGTQ_FORMAT_V1 layouts only");
     if (batch <= 0 || n_q <= 0 || max_tokens <= 0 || n_q > max_tokens) FAIL(BGTQ_EINVAL, "bgtq_prefill_attention: batch/n_q/max_tokens");
     if (!(softmax_scale > 0.0f) || std::isinf(softmax_scale)) FAIL(BGTQ_EINVAL, "bgtq_prefill_attention: softmax_scale");
     return launch_prefill(lay, layer, cache, q, seq_len, batch, n_q, max_tokens, softmax_scale, out, workspace,

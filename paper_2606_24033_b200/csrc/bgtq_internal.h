@@ -24,26 +24,43 @@ struct KStep {
     uint8_t flags;     // bit0 first step of its group, bit1 last step; bits 4..7 group index
 };
 
+// BGTQ-v2 (row order): one chunk = up to 32 grouped coordinates of one group, one token per lane.
+struct Chunk2 {
+    uint16_t off;      // byte offset of the chunk's first word plane inside a quadrant's K-code section
+    uint16_t ustart;   // grouped-order coordinate of slot 0
+    uint8_t b;         // code width
+    uint8_t r;         // slots in use (even, 2..32)
+    uint8_t nw;        // 32-bit words per lane
+    uint8_t flags;     // bit0 first chunk of its group; bits 4..7 group index
+};
+constexpr int kMaxChunks = 12;    // sum_g ceil(m_g/32) <= 4 + 7
+
 // Static layout metadata of one (layer, KV head)   ("static layout metadata")
 struct HeadMeta {
-    int32_t n_groups, kdim, n_ksteps, b_v;
-    int32_t tile_stride, kcode_bytes, knorm_off, vnorm_off, vcode_off, pad0;
+    int32_t n_groups, kdim, n_ksteps, b_v;      // n_ksteps: k16 steps (v1) / chunks (v2)
+    int32_t tile_stride, kcode_bytes, knorm_off, vnorm_off, vcode_off, format;   // format: 1 = BGTQ-v1, 2 = BGTQ-v2
     int64_t layer_prefix;   // sum of tile strides of all heads of all earlier layers
     int64_t layer_sum;      // sum of tile strides of the heads of this layer
     int64_t head_prefix;    // sum of tile strides of earlier heads of this layer
     int32_t goff[kMaxGroups];      // byte offset of the group's codes inside the tile
     uint16_t gm[kMaxGroups];       // coordinates in the group
     uint16_t gstart[kMaxGroups];   // first grouped-order coordinate of the group
-    uint16_t grot[kMaxGroups];     // unused / reserved
     uint8_t gb[kMaxGroups];        // width of the group
     uint8_t coords[kDh];           // grouped order -> original coordinate (Q9)
-    KStep ksteps[kMaxKSteps];
+    union {
+        KStep ksteps[kMaxKSteps];  // v1
+        Chunk2 chunks[kMaxKSteps]; // v2 (kMaxChunks used); kcode_bytes = 4 * (bytes of one quadrant)
+    };
 };
+static_assert(sizeof(KStep) == 8 && sizeof(Chunk2) == 8, "k-step / chunk descriptors are 8 bytes");
 
 }  // namespace bgtq
 
 struct bgtq_layout {
     int n_layers, n_kv_heads, n_q_heads, d_h, b_v, pairing;
+    int format;                           // 1 = BGTQ-v1 (fragment order), 2 = BGTQ-v2 (row order)
+    uint8_t *d_planes;                    // v2: e4m3 byte planes of the codebooks, see codebook_planes()
+    float kappa[9];                       // v2: plane scale of width b
     int max_stride;                       // largest tile stride over all heads
     std::vector<bgtq::HeadMeta> meta;     // host copy, [layer][kv_head]
     int64_t total_stride_sum;             // sum of tile strides over all (layer, head)
@@ -61,6 +78,11 @@ void set_error(const std::string &msg);
 int cuda_fail(cudaError_t e, const char *what);
 void count_launch(int n = 1);
 void codebook_levels(int b, double *levels);
+// e4m3 byte planes of C_b (v2 decode path): level k of width b is represented as (hi[k] + lo[k]) / kappa with hi, lo
+// e4m3 values; kappa in [32, 64] is chosen per width to minimise the largest relative error (0 for b = 1, 3; < 2e-6 for
+// b = 2; < 2e-4 for b = 4; < 1.3e-3 for b >= 5).  hi, lo receive 2^b bytes each.
+void codebook_planes(int b, float *kappa, uint8_t *hi, uint8_t *lo);
+constexpr int kPlaneBytes = 2 * 512;   // [plane][flat level index (2^b - 1 + k)]
 
 __host__ __device__ inline int64_t rot_offset(int m)  // element offset of Pi^(m), m even: sum of m'^2, m' = 2,4,..,m-2
 {
@@ -105,6 +127,11 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
 int launch_window_append(const void *k_new, const void *v_new, int dt, int n_layers, int batch, int n_new, int Hkv,
                          const int32_t *seq_len, void *win_k, void *win_v, int n_sink, int n_recent, cudaStream_t st);
 size_t decode_ws_bytes(const bgtq_layout *lay, int batch, int n_layers);
+int launch_decode2(const bgtq_layout *lay, int layer0, int n_layers, const void *cache,
+                   const void *q, const int32_t *seq_len, int batch, int64_t max_tokens,
+                   float scale, void *out, void *ws, size_t ws_bytes, const PageMap *pm, cudaStream_t st,
+                   const Window *win = nullptr);
+size_t decode2_ws_bytes(const bgtq_layout *lay, int batch, int n_layers);
 int debug_decode_unit(int b, const uint32_t *words, float *values);
 size_t prefill_ws_bytes(const bgtq_layout *lay, int batch, int n_q);
 int launch_prefill(const bgtq_layout *lay, int layer, const void *cache, const void *q, const int32_t *seq_len,

@@ -119,4 +119,87 @@ void codebook_levels(int b, double *levels)
     }
 }
 
+
+// ---------------------------------------------------------------- e4m3 byte planes (BGTQ-v2 decode path)
+// The v2 decode kernel feeds the 5th-generation tensor cores with 8-bit operands: one PRMT byte lookup yields four
+// operand bytes.  A codebook level v is therefore represented as (hi + lo) / kappa with hi, lo in the e4m3 grid
+// (sign, 4 exponent bits, 3 mantissa bits; finite range +-448), hi = nearest(kappa v), lo = nearest(kappa v - hi).
+// kappa is free (it is divided out of q' in fp32): it is searched on [32, 64] for the smallest worst-case relative
+// error over the levels of the width -- for b <= 3 there are scales at which every level is (almost) exactly a sum of
+// two grid values.
+namespace {
+double e4m3_value(int byte)
+{
+    const int s = byte >> 7, e = (byte >> 3) & 15, m = byte & 7;
+    const double v = e == 0 ? ldexp((double)m, -9) : ldexp(1.0 + m / 8.0, e - 7);
+    return s ? -v : v;
+}
+// nearest finite e4m3 value (round to nearest, ties to even), returned as its byte
+int e4m3_nearest(double x)
+{
+    const int s = x < 0 ? 0x80 : 0;
+    const double a = fabs(x);
+    if (a >= 448.0) return s | 0x7E;
+    int e;
+    (void)frexp(a, &e);                          // a = f * 2^e, f in [0.5, 1): leading bit 2^(e-1)
+    int E = a == 0.0 ? -7 : e - 1;
+    if (E < -6) E = -6;                          // subnormals share the quantum of the smallest normal binade
+    const double q = ldexp(1.0, E - 3);          // quantum: 3 mantissa bits
+    const double r = nearbyint(a / q) * q;       // default rounding mode: ties to even
+    if (r == 0.0) return s;
+    int er;
+    const double fr = frexp(r, &er);             // r = fr * 2^er
+    int Er = er - 1;
+    if (Er < -6) return s | (int)nearbyint(ldexp(r, 9));            // subnormal: m * 2^-9
+    return s | ((Er + 7) << 3) | (int)nearbyint((2.0 * fr - 1.0) * 8.0);
+}
+}  // namespace
+
+static void codebook_planes_search(int b, float *kappa, uint8_t *hi, uint8_t *lo)
+{
+    const int n = 1 << b;
+    double lv[256];
+    codebook_levels(b, lv);
+    if (b == 1) {                                // {-c, +c}: one plane of +-1, the level itself is the scale
+        *kappa = (float)(1.0 / lv[1]);
+        hi[0] = 0xB8; hi[1] = 0x38; lo[0] = lo[1] = 0;
+        return;
+    }
+    double best_k = 64.0, best_err = 1e300;
+    const int steps = b <= 4 ? 200000 : 20000;
+    for (int i = 0; i <= steps; ++i) {
+        const float kf = (float)(32.0 + 32.0 * i / steps);          // the kernel divides by the fp32 value
+        const double k = (double)kf;
+        double worst = 0.0;
+        for (int j = n / 2; j < n && worst < best_err; ++j) {       // positive half (the table is symmetric)
+            const double v = k * lv[j];
+            const double h = e4m3_value(e4m3_nearest(v));
+            const double l = e4m3_value(e4m3_nearest(v - h));
+            worst = fmax(worst, fabs(v - h - l) / v);
+        }
+        if (worst < best_err) { best_err = worst; best_k = k; }
+    }
+    *kappa = (float)best_k;
+    for (int j = 0; j < n; ++j) {
+        const double v = best_k * lv[j];
+        const int hb = e4m3_nearest(v);
+        hi[j] = (uint8_t)hb;
+        lo[j] = (uint8_t)e4m3_nearest(v - e4m3_value(hb));
+    }
+}
+
+
+void codebook_planes(int b, float *kappa, uint8_t *hi, uint8_t *lo)
+{
+    // searched once per process (the result depends on nothing but b)
+    struct Cache { float kappa[9]; uint8_t hi[9][256], lo[9][256]; };
+    static const Cache *cache = [] {
+        Cache *c = new Cache();
+        for (int w = 1; w <= 8; ++w) codebook_planes_search(w, &c->kappa[w], c->hi[w], c->lo[w]);
+        return c;
+    }();
+    *kappa = cache->kappa[b];
+    for (int j = 0; j < (1 << b); ++j) { hi[j] = cache->hi[b][j]; lo[j] = cache->lo[b][j]; }
+}
+
 }  // namespace bgtq
