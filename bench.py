@@ -50,6 +50,8 @@ def parse_args():
     ap.add_argument("--batch", type=int, default=None, help="sequences (default: the config's)")
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config supplying the head shape")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--format", type=int, default=1, choices=[1, 2],
+                    help="physical cache format: 1 = BGTQ-v1 fragment order (mma.sync decode kernel, default), 2 = BGTQ-v2 row order (tcgen05 decode kernel, measured slower: DESIGN.md section 7b)")
     ap.add_argument("--prefill-chunk", type=int, default=0,
                     help="also time bgtq_prefill_attention for the last N cached tokens of layer 0 (NEXT #1, first cut)")
     ap.add_argument("--compare-fp16", action="store_true",
@@ -261,7 +263,7 @@ def build_workload(args, P, torch, device, seed_shift: int = 0):
         bits = P.allocate(sc, shp.b_k * (d // 2), shp.b_min, shp.b_max).cpu().numpy().reshape(Lyr, Hkv, d // 2)
     t0 = time.perf_counter()
     rot = W.rotations(ROT_SEED, d)
-    lay = P.Layout(bits, Hq, d, shp.b_v, rot)
+    lay = P.Layout(bits, Hq, d, shp.b_v, rot, fmt=(1 if getattr(args, "prefill_chunk", 0) else args.format))
     t_layout = (time.perf_counter() - t0) * 1e3
     max_tokens = T + 4096
     cache = lay.new_cache(B, max_tokens, device)
@@ -418,7 +420,7 @@ def run_ours(args):
         except Exception:
             pass
         achieved = alg_bytes / (k_ms * 1e-3) / 1e9
-        roofline = {"bound": "hbm", "kernel": "bgtq::decode_kernel", "achieved": achieved, "peak": peak,
+        roofline = {"bound": "hbm", "kernel": "bgtq::decode2_kernel" if lay.fmt == 2 else "bgtq::decode_kernel", "achieved": achieved, "peak": peak,
                     "peak_source": peak_src, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
                     "kernel_us": k_ms * 1e3, "algorithmic_bytes_per_launch": alg_bytes,
                     "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS}

@@ -38,17 +38,19 @@ namespace bgtq {
 
 #define CUDA_TRY(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) return cuda_fail(e_, #expr); } while (0)
 
-constexpr int kD2Warps = 14;
+constexpr int kQkIssuers = 4, kPvIssuers = 2;                 // a thread issues one tcgen05.mma per ~60 clocks: several issuers in parallel
+constexpr int kD2Warps = 13 + kQkIssuers + kPvIssuers;
 constexpr int kD2Threads = kD2Warps * 32;
-constexpr int kD2Consumers = 13 * 32;                         // every warp but the TMA producer (named barrier 1)
+constexpr int kD2Consumers = (kD2Warps - 1) * 32;             // every warp but the TMA producer (named barrier 1)
 constexpr int kQ2Planes = 3;
 constexpr int kQ2Atoms = (kQ2Planes * kMaxChunks + 3) / 4;    // (chunk, plane) slices of [8 heads x 32 bytes], four per 1 KB atom
 constexpr int kQ2ImageBytes = kQ2Atoms * 1024;
 constexpr int kQ2Stride = kQ2ImageBytes + 128;                // + sigma_n (8 floats)
 constexpr int kP2Bytes = 3 * 1024;                            // P' planes: 12 slices (4 token quarters x 3 planes) = 3 atoms
 constexpr int kMaxStages = 10;
-// tensor memory columns (512 allocated)
-constexpr int kColAKhi = 0, kColAKlo = 96, kColAVhi = 192, kColAVlo = 224, kColS = 256, kColO = 320;   // S: 8 groups x 8; O: 3 planes x 8
+// tensor memory columns (512 allocated).  A_K: 192 columns = one buffer of 12 chunks x (hi, lo) or, when no head has more
+// than 6 chunks, two buffers of 6 chunks; A_V, S, P' double-buffered; O: three planes of 8 heads.
+constexpr int kColAK = 0, kColAV = 192, kColS = 320, kColO = 448;
 constexpr float kRefHeadroom = 5.0f;      // a new reference puts the largest weight at 2^5
 constexpr float kRefLimit = 8.5f;         // weights above 2^8.5 (e4m3 max 448) force a new reference
 
@@ -62,6 +64,7 @@ struct Decode2Params {
     int64_t n_cap;
     int n_layers, batch, Hkv, G;
     int stage_bytes, n_stages;
+    int ak_bufs;                // 2 when every head has <= 6 K chunks, else 1
     float inv_kappa_v;
     const int32_t *pages;
     int pstride;
@@ -315,14 +318,48 @@ __device__ __forceinline__ void umma_commit2(uint32_t bar)
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(bar) : "memory");
 }
 
-// barrier indices (after the ring's full / empty pairs)
-enum { B2_AK_READY = 0, B2_AK_FREE, B2_S_READY, B2_S_FREE, B2_AV_READY, B2_AV_FREE, B2_P_READY0, B2_P_READY1, B2_P_FREE0,
-       B2_P_FREE1, B2_QIMG, B2_COUNT };
+// barrier indices (after the ring's full / empty pairs); [2] = double-buffered, indexed by the use's buffer
+enum { B2_AK_READY = 0, B2_AK_FREE = 2, B2_S_READY = 4, B2_S_FREE = 6, B2_AV_READY = 8, B2_AV_FREE = 10, B2_P_READY = 12,
+       B2_P_FREE = 14, B2_QIMG = 16, B2_COUNT = 17 };
+
+// D[128 x 8] (+)= A . B with the B descriptor given as (constant high part | start address >> 4)
+__device__ __forceinline__ void umma_q8d(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc, uint32_t accumulate)
+{
+    constexpr uint32_t idesc = (1u << 4) | (1u << 17) | (8u << 24);
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::f8f6f4 [%0], [%1], %2, %3, p;\n\t}"
+                 :: "r"(d_tmem), "r"(a_tmem), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
+}
+// D[128 x 24] (+)= A . B, B = three 8-row atoms (SBO = 1024 bytes) of a SWIZZLE_128B image
+__device__ __forceinline__ void umma_n24(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc, uint32_t accumulate)
+{
+    constexpr uint32_t idesc = (1u << 4) | (3u << 17) | (8u << 24);
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::f8f6f4 [%0], [%1], %2, %3, p;\n\t}"
+                 :: "r"(d_tmem), "r"(a_tmem), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ uint64_t bdesc_sw128(uint32_t saddr)
+{
+    return (uint64_t)((saddr & 0x3FFFF) >> 4) | ((uint64_t)1 << 16) | ((uint64_t)(1024 >> 4) << 32) | ((uint64_t)1 << 46) | ((uint64_t)2 << 61);
+}
+
+#ifndef BGTQ_D2_TIMING
+#define BGTQ_D2_TIMING 0
+#endif
+#if BGTQ_D2_TIMING
+#define TWAIT(slot, bar, par) do { long long t0_ = clock64(); mbar_wait(bar, par); twait[slot] += clock64() - t0_; } while (0)
+#else
+#define TWAIT(slot, bar, par) mbar_wait(bar, par)
+#endif
 
 template <bool PAGED>
 __global__ void __launch_bounds__(kD2Threads, 1)
 decode2_kernel(const Decode2Params P)
 {
+#if BGTQ_D2_TIMING
+    long long twait[6] = {0, 0, 0, 0, 0, 0};
+    const long long tstart = clock64();
+#endif
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     // dynamic (1024-byte aligned by hand: the SWIZZLE_128B pattern is a function of the address):
     // [q' image 10 KB][P' planes 2 x 3 KB][ring: n_stages x stage_bytes]
@@ -337,12 +374,14 @@ decode2_kernel(const Decode2Params P)
     __shared__ int pre[kMaxBatch + 1];
     __shared__ __align__(8) uint64_t bars[2 * kMaxStages + B2_COUNT];
     __shared__ uint32_t tmem_base_s;
-    __shared__ float qmax_s[4][8];
+    __shared__ float qmax_s[2][4][8];
     __shared__ float lsum_s[4][8];
-    __shared__ float sigma_s[8];
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int role = warp >> 2, quad = warp & 3;               // role 0 K unpack, 1 softmax, 2 V unpack, 3: warp 12 MMA, warp 13 TMA
+    const int quad = warp & 3;
+    // roles: 0 K unpack (warps 0-3), 1 softmax (4-7), 2 V unpack (8-11), 4 TMA (12), 3 QK^T issue (13 ..), 5 PV issue (the last two)
+    const int role = warp < 12 ? (warp >> 2) : (warp == 12 ? 4 : (warp < 13 + kQkIssuers ? 3 : 5));
+    const int issuer = warp < 13 + kQkIssuers ? warp - 13 : warp - 13 - kQkIssuers;
     pdl_trigger();
 
     for (int i = tid; i < kPlaneBytes; i += kD2Threads) planes_s[i] = __ldg(P.planes + i);
@@ -358,11 +397,12 @@ decode2_kernel(const Decode2Params P)
     auto xbar = [&](int i) { return bar0 + 8u * (2 * kMaxStages + i); };
     if (tid == 32) {
         for (int s = 0; s < P.n_stages; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 12); }
-        mbar_init(xbar(B2_AK_READY), 4);  mbar_init(xbar(B2_AK_FREE), 1);
-        mbar_init(xbar(B2_S_READY), 1);   mbar_init(xbar(B2_S_FREE), 4);
-        mbar_init(xbar(B2_AV_READY), 4);  mbar_init(xbar(B2_AV_FREE), 1);
-        mbar_init(xbar(B2_P_READY0), 4);  mbar_init(xbar(B2_P_READY1), 4);
-        mbar_init(xbar(B2_P_FREE0), 1);   mbar_init(xbar(B2_P_FREE1), 1);
+        for (int b = 0; b < 2; ++b) {
+            mbar_init(xbar(B2_AK_READY + b), 4);  mbar_init(xbar(B2_AK_FREE + b), kQkIssuers);
+            mbar_init(xbar(B2_S_READY + b), kQkIssuers);   mbar_init(xbar(B2_S_FREE + b), 4);
+            mbar_init(xbar(B2_AV_READY + b), 4);  mbar_init(xbar(B2_AV_FREE + b), kPvIssuers);
+            mbar_init(xbar(B2_P_READY + b), 4);   mbar_init(xbar(B2_P_FREE + b), kPvIssuers);
+        }
         mbar_init(xbar(B2_QIMG), 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -389,7 +429,7 @@ decode2_kernel(const Decode2Params P)
     };
 
     // ================================================================ TMA producer: free-runs over the CTA's tile range
-    if (warp == 13) {
+    if (role == 4) {
         if (lane == 0) {
             int it = 0;
             for (int x = x_lo; x < x_hi;) {
@@ -414,15 +454,16 @@ decode2_kernel(const Decode2Params P)
         return;
     }
 
-    // per-role state
+    // Every wait below derives its parity from the tile counter `it` (tiles consumed by this CTA so far): a resource with
+    // nb buffers is used for the (it / nb)-th time by tile it, in buffer it % nb.
     const Pools2 pools = load_pools2(planes_s);
-    uint32_t ph_ak_free = 0, ph_s_free = 0, ph_av_free = 0, ph_ak_ready = 0, ph_s_ready = 0, ph_av_ready = 0;
-    uint32_t ph_p_ready[2] = {0, 0}, ph_p_free[2] = {0, 0}, ph_qimg = 0;
-    int it = 0;                                         // tiles consumed so far by this CTA (ring position)
-    int n_pv = 0;                                       // tiles whose PV has been issued (softmax / MMA bookkeeping)
+    const int nbk = P.ak_bufs;
+    int it = 0, seg = 0;
     const uint32_t lane_base = (uint32_t)(32 * quad) << 16;
+    auto ak_col = [&](int buf, int plane, int ch) { return kColAK + (nbk == 2 ? buf * 96 + plane * 48 : plane * 96) + 8 * ch; };
+    auto av_col = [&](int buf, int plane, int c) { return kColAV + buf * 64 + plane * 32 + 8 * c; };
 
-    for (int x = x_lo; x < x_hi;) {
+    for (int x = x_lo; x < x_hi; ++seg) {
         // ---------------- segment = the part of one (layer, sequence, kv head) inside this CTA's range
         const TilePos tp = locate(x, S, pre);
         const int seg_end = min(x_hi, tp.pair_start + tp.tiles_b);
@@ -431,7 +472,7 @@ decode2_kernel(const Decode2Params P)
             const uint32_t *msrc = reinterpret_cast<const uint32_t *>(P.metas + tp.l * P.Hkv + tp.h);
             if (tid < (int)(sizeof(HeadMeta) / 4)) reinterpret_cast<uint32_t *>(&Ms)[tid] = __ldg(msrc + tid);
         }
-        if (warp == 12 && lane == 0) {                  // q' image of this pair (written by qfold2_kernel)
+        if (role == 3 && issuer == 0 && lane == 0) {    // q' image of this pair (written by qfold2_kernel)
             pdl_wait();
             mbar_expect_tx(xbar(B2_QIMG), kQ2Stride);
             bulk_g2s(smem_u32(qimg_s), P.qimg + (size_t)tp.pair * kQ2Stride, kQ2Stride, xbar(B2_QIMG));
@@ -443,105 +484,124 @@ decode2_kernel(const Decode2Params P)
         slen = slen > P.n_cap * kTile ? P.n_cap * kTile : slen;
         slen = packed_len(slen, P.n_sink, P.n_recent);
         const int n_tiles_seg = seg_end - x;
+        x = seg_end;
 
         if (role == 0) {
             // ======================================================== K unpack: thread = token row `quad*32 + lane`
             const int kq4 = M.kcode_bytes >> 4;                          // words of one quadrant's K-code section
             for (int j = 0; j < n_tiles_seg; ++j, ++it) {
                 const int s = it % P.n_stages;
-                mbar_wait(full_bar(s), (it / P.n_stages) & 1);
+                TWAIT(0, full_bar(s), (it / P.n_stages) & 1);
                 const uint32_t *kc = reinterpret_cast<const uint32_t *>(ring + (size_t)s * P.stage_bytes) + quad * kq4 + lane;
-                if (it > 0) { mbar_wait(xbar(B2_AK_FREE), ph_ak_free); ph_ak_free ^= 1; tc2_fence_after(); }
+                const int buf = it % nbk, use = it / nbk;
+                bool waited = use == 0;
 #pragma unroll 1
                 for (int ch = 0; ch < n_chunks; ++ch) {
                     const Chunk2 C2 = M.chunks[ch];
                     uint32_t hi[8], lo[8];
                     decode_chunk2_any(C2.b, kc + (C2.off >> 2), C2.nw, pools, lut16, pair5, hi, lo);
-                    tmem_st8(tmem + lane_base + kColAKhi + 8 * ch, hi);
-                    if (C2.b > 1) tmem_st8(tmem + lane_base + kColAKlo + 8 * ch, lo);
+                    if (!waited) { TWAIT(1, xbar(B2_AK_FREE + buf), (use - 1) & 1); tc2_fence_after(); waited = true; }
+                    tmem_st8(tmem + lane_base + ak_col(buf, 0, ch), hi);
+                    if (C2.b > 1) tmem_st8(tmem + lane_base + ak_col(buf, 1, ch), lo);
                 }
+#if BGTQ_D2_TIMING
+                long long tq0 = clock64();
+#endif
                 tmem_wait_st();
+#if BGTQ_D2_TIMING
+                twait[3] += clock64() - tq0;
+#endif
                 tc2_fence_before();
                 __syncwarp();
-                if (lane == 0) { mbar_arrive(xbar(B2_AK_READY)); mbar_arrive(empty_bar(s)); }
+                if (lane == 0) { mbar_arrive(xbar(B2_AK_READY + buf)); mbar_arrive(empty_bar(s)); }
             }
         } else if (role == 2) {
             // ======================================================== V unpack: thread = dimension row `quad*32 + lane`
             for (int j = 0; j < n_tiles_seg; ++j, ++it) {
                 const int s = it % P.n_stages;
-                mbar_wait(full_bar(s), (it / P.n_stages) & 1);
+                TWAIT(0, full_bar(s), (it / P.n_stages) & 1);
                 const uint32_t *vc = reinterpret_cast<const uint32_t *>(ring + (size_t)s * P.stage_bytes + M.vcode_off) + quad * 4 * b_v * 32 + lane;
-                if (it > 0) { mbar_wait(xbar(B2_AV_FREE), ph_av_free); ph_av_free ^= 1; tc2_fence_after(); }
+                const int buf = it & 1, use = it >> 1;
+                bool waited = use == 0;
 #pragma unroll 1
                 for (int c = 0; c < 4; ++c) {
                     uint32_t hi[8], lo[8];
                     decode_chunk2_any(b_v, vc + c * b_v * 32, b_v, pools, lut16, pair5, hi, lo);
-                    tmem_st8(tmem + lane_base + kColAVhi + 8 * c, hi);
-                    if (b_v > 1) tmem_st8(tmem + lane_base + kColAVlo + 8 * c, lo);
+                    if (!waited) { TWAIT(1, xbar(B2_AV_FREE + buf), (use - 1) & 1); tc2_fence_after(); waited = true; }
+                    tmem_st8(tmem + lane_base + av_col(buf, 0, c), hi);
+                    if (b_v > 1) tmem_st8(tmem + lane_base + av_col(buf, 1, c), lo);
                 }
                 tmem_wait_st();
                 tc2_fence_before();
                 __syncwarp();
-                if (lane == 0) { mbar_arrive(xbar(B2_AV_READY)); mbar_arrive(empty_bar(s)); }
+                if (lane == 0) { mbar_arrive(xbar(B2_AV_READY + buf)); mbar_arrive(empty_bar(s)); }
             }
-        } else if (warp == 12) {
-            // ======================================================== MMA issue (one thread)
+        } else if (role == 3) {
+            // ======================================================== QK^T issue: S_g = A_K . q' ; issuer i owns the groups g = i (mod kQkIssuers)
             if (lane == 0) {
-                mbar_wait(xbar(B2_QIMG), ph_qimg); ph_qimg ^= 1;
-                const uint32_t qb = smem_u32(qimg_s), pb = smem_u32(pimg_s);
+                mbar_wait(xbar(B2_QIMG), seg & 1);
+                const uint64_t qd = bdesc_sw128(smem_u32(qimg_s));
                 for (int j = 0; j < n_tiles_seg; ++j, ++it) {
-                    // ---- S_g = A_K . q'  for every chunk
-                    mbar_wait(xbar(B2_AK_READY), ph_ak_ready); ph_ak_ready ^= 1;
-                    if (it > 0) { mbar_wait(xbar(B2_S_FREE), ph_s_free); ph_s_free ^= 1; }
+                    const int bufk = it % nbk, sb = it & 1;
+                    TWAIT(1, xbar(B2_AK_READY + bufk), (it / nbk) & 1);
+                    if (it >= 2) TWAIT(2, xbar(B2_S_FREE + sb), ((it >> 1) - 1) & 1);
                     tc2_fence_after();
                     for (int ch = 0; ch < n_chunks; ++ch) {
                         const Chunk2 C2 = M.chunks[ch];
-                        const uint32_t d = tmem + kColS + 8 * (C2.flags >> 4);
-                        const uint32_t ahi = tmem + kColAKhi + 8 * ch, alo = tmem + kColAKlo + 8 * ch;
+                        const int g = C2.flags >> 4;
+                        if (g % kQkIssuers != issuer) continue;
+                        const uint32_t d = tmem + kColS + 64 * sb + 8 * g;
+                        const uint32_t ahi = tmem + ak_col(bufk, 0, ch), alo = tmem + ak_col(bufk, 1, ch);
                         const int sl = 3 * ch;
-                        auto bq = [&](int p) { return qb + (uint32_t)(((sl + p) >> 2) * 1024 + ((sl + p) & 3) * 32); };
-                        umma_q8(d, ahi, bq(0), (C2.flags & 1) ? 0u : 1u);
-                        umma_q8(d, ahi, bq(1), 1u);
-                        umma_q8(d, ahi, bq(2), 1u);
-                        if (C2.b > 1) { umma_q8(d, alo, bq(0), 1u); umma_q8(d, alo, bq(1), 1u); }
+                        auto bq = [&](int p) { return qd + (uint64_t)((((sl + p) >> 2) * 1024 + ((sl + p) & 3) * 32) >> 4); };
+                        umma_q8d(d, ahi, bq(0), (C2.flags & 1) ? 0u : 1u);
+                        umma_q8d(d, ahi, bq(1), 1u);
+                        umma_q8d(d, ahi, bq(2), 1u);
+                        if (C2.b > 1) { umma_q8d(d, alo, bq(0), 1u); umma_q8d(d, alo, bq(1), 1u); }
                     }
-                    umma_commit2(xbar(B2_S_READY));
-                    umma_commit2(xbar(B2_AK_FREE));
-                    // ---- O_p += A_V . P'_p  (three planes of P', one accumulator each)
-                    const int pbuf = it & 1;
-                    mbar_wait(xbar(B2_AV_READY), ph_av_ready); ph_av_ready ^= 1;
-                    mbar_wait(xbar(B2_P_READY0 + pbuf), ph_p_ready[pbuf]); ph_p_ready[pbuf] ^= 1;
+                    umma_commit2(xbar(B2_S_READY + sb));
+                    umma_commit2(xbar(B2_AK_FREE + bufk));
+                }
+            } else it += n_tiles_seg;
+            __syncwarp();
+        } else if (role == 5) {
+            // ======================================================== PV issue: O[128 dims x (3 planes x 8 heads)] += A_V . P'; issuer 0 = hi plane of V, 1 = lo plane
+            if (lane == 0) {
+                const uint64_t pd = bdesc_sw128(smem_u32(pimg_s));
+                for (int j = 0; j < n_tiles_seg; ++j, ++it) {
+                    const int b = it & 1;
+                    TWAIT(1, xbar(B2_AV_READY + b), (it >> 1) & 1);
+                    TWAIT(2, xbar(B2_P_READY + b), (it >> 1) & 1);
                     tc2_fence_after();
-                    const uint32_t pbase = pb + pbuf * kP2Bytes;
-                    for (int c = 0; c < 4; ++c) {
-                        const uint32_t ahi = tmem + kColAVhi + 8 * c, alo = tmem + kColAVlo + 8 * c;
-                        const uint32_t acc = (j > 0 || c > 0) ? 1u : 0u;
-                        auto bp = [&](int p) { const int sl = 3 * c + p; return pbase + (uint32_t)((sl >> 2) * 1024 + (sl & 3) * 32); };
-                        umma_q8(tmem + kColO + 0, ahi, bp(0), acc);
-                        umma_q8(tmem + kColO + 8, ahi, bp(1), acc);
-                        umma_q8(tmem + kColO + 16, ahi, bp(2), acc);
-                        if (b_v > 1) { umma_q8(tmem + kColO + 0, alo, bp(0), 1u); umma_q8(tmem + kColO + 8, alo, bp(1), 1u); }
-                    }
-                    umma_commit2(xbar(B2_AV_FREE));
-                    umma_commit2(xbar(B2_P_FREE0 + pbuf));
+                    if (issuer == 0 || b_v > 1)
+                        for (int c = 0; c < 4; ++c)        // (O was zeroed by the softmax warps before the first P' of the segment)
+                            umma_n24(tmem + kColO, tmem + av_col(b, issuer, c), pd + (uint64_t)((b * kP2Bytes + 32 * c) >> 4), 1u);
+                    umma_commit2(xbar(B2_AV_FREE + b));
+                    umma_commit2(xbar(B2_P_FREE + b));
                 }
             } else it += n_tiles_seg;
             __syncwarp();
         } else {
             // ======================================================== softmax: thread = token row `quad*32 + lane`
-            mbar_wait(xbar(B2_QIMG), ph_qimg); ph_qimg ^= 1;        // sigma_n arrives with the q' image
-            if (tid - 128 < 8) sigma_s[tid - 128] = reinterpret_cast<const float *>(qimg_s + kQ2ImageBytes)[tid - 128];
-            bar_softmax();
+            mbar_wait(xbar(B2_QIMG), seg & 1);                      // sigma_n arrives with the q' image
             float sig[8];
 #pragma unroll
-            for (int n = 0; n < 8; ++n) sig[n] = sigma_s[n];
+            for (int n = 0; n < 8; ++n) sig[n] = reinterpret_cast<const float *>(qimg_s + kQ2ImageBytes)[n];
             float R[8], lacc[8];
 #pragma unroll
             for (int n = 0; n < 8; ++n) { R[n] = -INFINITY; lacc[n] = 0.f; }
             const int row = quad * 32 + lane;
+            {   // O = 0: both PV issuers only ever accumulate.  The previous segment's record has been read (its PV was complete).
+                const uint32_t z[8] = {0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
+                tmem_st8(tmem + lane_base + kColO + 0, z);
+                tmem_st8(tmem + lane_base + kColO + 8, z);
+                tmem_st8(tmem + lane_base + kColO + 16, z);
+                tmem_wait_st();
+                tc2_fence_before();
+            }
             for (int j = 0, t = tp.t; j < n_tiles_seg; ++j, ++t, ++it) {
-                const int s = it % P.n_stages;
-                mbar_wait(full_bar(s), (it / P.n_stages) & 1);
+                const int s = it % P.n_stages, sb = it & 1;
+                TWAIT(0, full_bar(s), (it / P.n_stages) & 1);
                 const unsigned char *tile = ring + (size_t)s * P.stage_bytes;
                 // norms of this token: K groups, V
                 float nk[kMaxGroups];
@@ -556,39 +616,45 @@ decode2_kernel(const Decode2Params P)
                 const int n_valid = (int)min((int64_t)kTile, slen - (int64_t)t * kTile);
                 const int n_low = t == 0 ? P.n_sink : 0;
                 const bool live = row < n_valid && row >= n_low;
-                // ---- logits
-                mbar_wait(xbar(B2_S_READY), ph_s_ready); ph_s_ready ^= 1;
+                // ---- logits: all group accumulators are requested, then one wait
+                TWAIT(1, xbar(B2_S_READY + sb), (it >> 1) & 1);
                 tc2_fence_after();
                 float lg[8];
 #pragma unroll
                 for (int n = 0; n < 8; ++n) lg[n] = 0.f;
 #pragma unroll
-                for (int g = 0; g < kMaxGroups; ++g) {
-                    if (g < n_groups) {
-                        uint32_t sv[8];
-                        tmem_ld8(tmem + lane_base + kColS + 8 * g, sv);
+                for (int g0 = 0; g0 < kMaxGroups; g0 += 4) {        // four groups per round trip to tensor memory
+                    if (g0 < n_groups) {
+                        uint32_t sv[4][8];
+#pragma unroll
+                        for (int g = 0; g < 4; ++g)
+                            if (g0 + g < n_groups) tmem_ld8(tmem + lane_base + kColS + 64 * sb + 8 * (g0 + g), sv[g]);
                         tmem_wait_ld();
 #pragma unroll
-                        for (int n = 0; n < 8; ++n) lg[n] = fmaf(nk[g], __uint_as_float(sv[n]), lg[n]);
+                        for (int g = 0; g < 4; ++g)
+                            if (g0 + g < n_groups) {
+#pragma unroll
+                                for (int n = 0; n < 8; ++n) lg[n] = fmaf(nk[g0 + g], __uint_as_float(sv[g][n]), lg[n]);
+                            }
                     }
                 }
                 tc2_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(xbar(B2_S_FREE));
+                if (lane == 0) mbar_arrive(xbar(B2_S_FREE + sb));
 #pragma unroll
                 for (int n = 0; n < 8; ++n) lg[n] = live ? fmaf(lg[n], sig[n], lgh) : -INFINITY;
-                // ---- reference update (CTA-wide, per head): quadrant maxima meet in shared memory
+                // ---- reference update (CTA-wide, per head): quadrant maxima meet in shared memory (double-buffered by tile parity)
 #pragma unroll
                 for (int n = 0; n < 8; ++n) {
                     const float m = redux_max(lg[n]);
-                    if (lane == n) qmax_s[quad][n] = m;
+                    if (lane == n) qmax_s[sb][quad][n] = m;
                 }
                 bar_softmax();
                 float alpha[8];
                 bool any = false;
 #pragma unroll
                 for (int n = 0; n < 8; ++n) {
-                    const float tm = fmaxf(fmaxf(qmax_s[0][n], qmax_s[1][n]), fmaxf(qmax_s[2][n], qmax_s[3][n]));
+                    const float tm = fmaxf(fmaxf(qmax_s[sb][0][n], qmax_s[sb][1][n]), fmaxf(qmax_s[sb][2][n], qmax_s[sb][3][n]));
                     alpha[n] = 1.f;
                     if (tm > R[n] + kRefLimit) {
                         const float Rn = tm - kRefHeadroom;
@@ -597,11 +663,9 @@ decode2_kernel(const Decode2Params P)
                         any = any || (n < P.G && j > 0);
                     }
                 }
-                bar_softmax();                                      // qmax_s may be overwritten by the next tile from here on
                 if (any) {
-                    // rare: rescale the accumulators in tensor memory.  The PV of tile j-1 must be complete.
-                    const int pb1 = (it - 1) & 1;
-                    mbar_wait(xbar(B2_P_FREE0 + pb1), ph_p_free[pb1]);     // (not consumed: tile it + 1 waits for the same commit)
+                    // rare: rescale the accumulators in tensor memory.  The PV of tile it - 1 must be complete.
+                    mbar_wait(xbar(B2_P_FREE + ((it - 1) & 1)), ((it - 1) >> 1) & 1);
                     tc2_fence_after();
 #pragma unroll
                     for (int p = 0; p < 3; ++p) {
@@ -636,23 +700,21 @@ decode2_kernel(const Decode2Params P)
                     p3[n >> 2] |= c << (8 * (n & 3));
                 }
                 // ---- planes -> shared memory (B operand of PV: row = head, K = token); buffer it & 1
-                const int pbuf = it & 1;
-                if (it >= 2) { mbar_wait(xbar(B2_P_FREE0 + pbuf), ph_p_free[pbuf]); ph_p_free[pbuf] ^= 1; }
-                unsigned char *pi = pimg_s + pbuf * kP2Bytes;
+                if (it >= 2) TWAIT(2, xbar(B2_P_FREE + sb), ((it >> 1) - 1) & 1);
+                unsigned char *pi = pimg_s + sb * kP2Bytes;
 #pragma unroll
                 for (int n = 0; n < 8; ++n) {
-                    pi[sw128_off(3 * quad + 0, n, lane)] = (uint8_t)(p1[n >> 2] >> (8 * (n & 3)));
-                    pi[sw128_off(3 * quad + 1, n, lane)] = (uint8_t)(p2[n >> 2] >> (8 * (n & 3)));
-                    pi[sw128_off(3 * quad + 2, n, lane)] = (uint8_t)(p3[n >> 2] >> (8 * (n & 3)));
+                    pi[sw128_off(0 + quad, n, lane)] = (uint8_t)(p1[n >> 2] >> (8 * (n & 3)));     // atom = plane, 32-byte K slice = token quarter
+                    pi[sw128_off(4 + quad, n, lane)] = (uint8_t)(p2[n >> 2] >> (8 * (n & 3)));
+                    pi[sw128_off(8 + quad, n, lane)] = (uint8_t)(p3[n >> 2] >> (8 * (n & 3)));
                 }
                 fence_proxy_async();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(xbar(B2_P_READY0 + pbuf));
+                if (lane == 0) mbar_arrive(xbar(B2_P_READY + sb));
             }
             // ---------------- segment end: one partial record (R, l, acc[128]) per head; this warp owns dims quad*32 + lane
             {
-                const int last = (it - 1) & 1;                      // PV of the last tile complete
-                mbar_wait(xbar(B2_P_FREE0 + last), ph_p_free[last]);
+                mbar_wait(xbar(B2_P_FREE + ((it - 1) & 1)), ((it - 1) >> 1) & 1);     // PV of the last tile complete
                 tc2_fence_after();
                 float o[8];
                 {
@@ -688,10 +750,12 @@ decode2_kernel(const Decode2Params P)
                 bar_softmax();
             }
         }
-        x = seg_end;
-        n_pv += n_tiles_seg;
     }
-    (void)n_pv;
+#if BGTQ_D2_TIMING
+    if (blockIdx.x == 3 && lane == 0 && (quad == 0 || role >= 3))
+        printf("role %d warp %2d: total %lld  wait full %lld  wait[1] %lld  wait[2] %lld  wait_st %lld tiles %d\n", role, warp, clock64() - tstart,
+               twait[0], twait[1], twait[2], twait[3], it);
+#endif
     tc2_fence_before();
     bar_consumers();
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" :: "r"(tmem) : "memory");
@@ -753,6 +817,7 @@ int launch_decode2(const bgtq_layout *lay, int layer0, int n_layers, const void 
     if (P.n_stages > kMaxStages) P.n_stages = kMaxStages;
     if (P.n_stages < 2) { set_error("bgtq_decode_attention: tile does not fit shared memory"); return BGTQ_EINVAL; }
     P.inv_kappa_v = 1.0f / lay->kappa[lay->b_v];
+    P.ak_bufs = lay->max_chunks <= 6 ? 2 : 1;
     P.pages = pm ? pm->table : nullptr; P.pstride = pm ? pm->table_stride : 0; P.n_pages = pm ? pm->n_pages : 0;
     P.n_sink = n_sink; P.n_recent = n_recent;
     const size_t smem = 17 * 1024 + (size_t)P.n_stages * P.stage_bytes;

@@ -66,10 +66,12 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 {
     uint32_t done;
     do {
+        // (with a suspend-time hint the waiting thread is parked by the hardware until the phase completes -- or the hint,
+        //  in nanoseconds, expires -- instead of re-issuing the test every few dozen clocks and stealing issue slots)
         asm volatile("{\n\t.reg .pred p;\n\t"
-                     "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+                     "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
                      "selp.u32 %0, 1, 0, p;\n\t}"
-                     : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+                     : "=r"(done) : "r"(bar), "r"(parity), "r"(20000u) : "memory");
     } while (!done);
 }
 __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar)

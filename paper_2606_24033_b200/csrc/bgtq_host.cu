@@ -253,6 +253,7 @@ extern "C" int bgtq_layout_create_format(const uint8_t *bits, int n_layers, int 
     lay->meta.resize((size_t)n_layers * n_kv_heads);
     int64_t prefix = 0;
     lay->max_stride = 0;
+    lay->max_chunks = 0;
     for (int l = 0; l < n_layers; ++l) {
         int64_t lsum = 0;
         for (int h = 0; h < n_kv_heads; ++h) {
@@ -264,6 +265,7 @@ extern "C" int bgtq_layout_create_format(const uint8_t *bits, int n_layers, int 
             m.head_prefix = lsum;
             lsum += m.tile_stride;
             if (m.tile_stride > lay->max_stride) lay->max_stride = m.tile_stride;
+            if (format == BGTQ_FORMAT_V2 && m.n_ksteps > lay->max_chunks) lay->max_chunks = m.n_ksteps;
         }
         for (int h = 0; h < n_kv_heads; ++h) lay->meta[(size_t)l * n_kv_heads + h].layer_sum = lsum;
         prefix += lsum;

@@ -62,6 +62,7 @@ struct bgtq_layout {
     uint8_t *d_planes;                    // v2: e4m3 byte planes of the codebooks, see codebook_planes()
     float kappa[9];                       // v2: plane scale of width b
     int max_stride;                       // largest tile stride over all heads
+    int max_chunks;                       // v2: largest number of K chunks over all heads
     std::vector<bgtq::HeadMeta> meta;     // host copy, [layer][kv_head]
     int64_t total_stride_sum;             // sum of tile strides over all (layer, head)
     bgtq::HeadMeta *d_meta;               // device copy
