@@ -127,8 +127,9 @@ int64_t bgtq_tile_stride(const bgtq_layout *layout, int layer, int kv_head);
  * seq_len [device] int32 [batch]: tokens already cached; sequence s receives its n_new tokens at
  *   positions seq_len[s] .. seq_len[s]+n_new-1 and, if advance_seq_len != 0, seq_len[s] is advanced
  *   by n_new (by a kernel on `stream`; a model appends to every layer with the same seq_len and
- *   advances on the last).  Tokens that would not fit in max_tokens are dropped and seq_len
- *   saturates (BGTQ_ECAPACITY if n_new > max_tokens is detectable on the host).
+ *   advances on the last).  Tokens at positions >= max_tokens (the caller's capacity, NOT rounded up to
+ *   a whole tile) are dropped and seq_len saturates at max_tokens (BGTQ_ECAPACITY if n_new > max_tokens
+ *   is detectable on the host).
  * Only the fields of the new tokens change.  One layer per call. */
 int bgtq_quantize_append(const bgtq_layout *layout, int layer, void *cache, const void *k_new,
                          const void *v_new, int dt, int batch, int n_new, int32_t *seq_len,
@@ -173,11 +174,13 @@ int bgtq_decode_attention_layers(const bgtq_layout *layout, int layer0, int n_la
  * bgtq_window_append: fp16 copies (round-to-nearest-even) of the n_new tokens the matching
  *   bgtq_quantize_append_layers call stores at positions seq_len[s] .. seq_len[s] + n_new - 1, written to their
  *   window slots; call it BEFORE that append advances seq_len.  k_new (post-RoPE), v_new, dt, batch, n_new as
- *   there.  Caller owns all buffers. */
+ *   there; max_tokens is that append's capacity: tokens at positions >= max_tokens are dropped here exactly as the
+ *   append drops them (the ring keeps the rows of the tokens that ARE cached).  The window limits of
+ *   bgtq_decode_attention_protected apply (else BGTQ_EINVAL).  Caller owns all buffers. */
 size_t bgtq_window_bytes(const bgtq_layout *layout, int batch, int n_sink, int n_recent);
 int bgtq_window_append(const bgtq_layout *layout, int layer0, int n_layers, const void *k_new,
                        const void *v_new, int dt, int batch, int n_new, const int32_t *seq_len,
-                       void *win_k, void *win_v, int n_sink, int n_recent, void *stream);
+                       int64_t max_tokens, void *win_k, void *win_v, int n_sink, int n_recent, void *stream);
 int bgtq_decode_attention_protected(const bgtq_layout *layout, int layer0, int n_layers, const void *cache,
                                     const void *q, const int32_t *seq_len, int batch, int64_t max_tokens,
                                     float softmax_scale, const void *win_k, const void *win_v, int n_sink,
@@ -225,7 +228,9 @@ int bgtq_decode_attention_paged(const bgtq_layout *layout, int layer0, int n_lay
  * already in the cache (bgtq_quantize_append first): query token i of sequence s sits at position
  * seq_len[s] - n_q + i and attends to cached tokens [0, that position] (itself included).
  * q, out [device] bf16 [batch, n_q, n_q_heads, d_h] (post-RoPE q); seq_len [device] int32 [batch] >= n_q.
- * GQA group must be 1, 2, 4 or 8.  First cut on the legacy mma.sync tensor path. */
+ * A sequence with seq_len[s] < n_q is a caller error the host cannot see: its output rows are zeros.
+ * GQA group must be 1, 2, 4 or 8; BGTQ_FORMAT_V1 layouts only.  Runs on the 5th-generation tensor cores (tcgen05.mma with
+ * accumulators in tensor memory, warp-specialised). */
 size_t bgtq_prefill_workspace_bytes(const bgtq_layout *layout, int batch, int n_q);
 int bgtq_prefill_attention(const bgtq_layout *layout, int layer, const void *cache, const void *q,
                            const int32_t *seq_len, int batch, int n_q, int64_t max_tokens, float softmax_scale,

@@ -113,7 +113,7 @@ def _load() -> C.CDLL:
     lib.bgtq_window_bytes.restype = sz
     lib.bgtq_window_bytes.argtypes = [vp, i32, i32, i32]
     lib.bgtq_window_append.restype = i32
-    lib.bgtq_window_append.argtypes = [vp, i32, i32, vp, vp, i32, i32, i32, vp, vp, vp, i32, i32, vp]
+    lib.bgtq_window_append.argtypes = [vp, i32, i32, vp, vp, i32, i32, i32, vp, i64, vp, vp, i32, i32, vp]
     lib.bgtq_decode_attention_protected.restype = i32
     lib.bgtq_decode_attention_protected.argtypes = [vp, i32, i32, vp, vp, vp, i32, i64, f32, vp, vp, i32, i32, vp, vp, sz, vp]
     lib.bgtq_decode_attention_paged.restype = i32
@@ -364,15 +364,16 @@ def new_windows(layout: Layout, batch: int, n_sink: int, n_recent: int, device="
 
 
 def window_append(layout: Layout, layer: int, k_new: torch.Tensor, v_new: torch.Tensor, seq_len: torch.Tensor,
-                  win_k: torch.Tensor, win_v: torch.Tensor, n_sink: int, n_recent: int, n_layers: int = 1) -> None:
+                  win_k: torch.Tensor, win_v: torch.Tensor, n_sink: int, n_recent: int, n_layers: int = 1,
+                  max_tokens: int = 2**31 - 1) -> None:
     """bgtq_window_append: k_new, v_new [batch, n_new, H_kv, d_h] (n_layers = 1) or [n_layers, batch, n_new, H_kv, d_h];
     call before the quantize_append that advances seq_len."""
     batch, n_new, Hkv, d = k_new.shape[-4:]
     assert v_new.shape == k_new.shape and Hkv == layout.n_kv_heads and d == layout.d_h and _dt(k_new) == _dt(v_new)
     assert k_new.dim() == 4 or k_new.shape[0] == n_layers
     _check(_lib.bgtq_window_append(layout._h, layer, n_layers, _dev(k_new), _dev(v_new), _dt(k_new), batch, n_new,
-                                   _dev(seq_len, torch.int32), _dev(win_k, torch.float16), _dev(win_v, torch.float16),
-                                   n_sink, n_recent, _stream()))
+                                   _dev(seq_len, torch.int32), max_tokens, _dev(win_k, torch.float16),
+                                   _dev(win_v, torch.float16), n_sink, n_recent, _stream()))
 
 
 def decode_attention_protected(layout: Layout, layer: int, cache: torch.Tensor, q: torch.Tensor, seq_len: torch.Tensor,

@@ -432,19 +432,17 @@ int launch_quantize_append(const bgtq_layout *lay, int layer, int n_layers, void
                            const void *v_new, int dt, int batch, int n_new, int32_t *seq_len,
                            int advance, int64_t max_tokens, const PageMap *pm, const RopeTab *rope, cudaStream_t st)
 {
-    static bool attr_set = false;
     const int64_t n_cap = (max_tokens + kTile - 1) / kTile;
     const size_t smem = append_smem_bytes(lay->max_stride);
     dim3 grid((n_new + kTile - 1) / kTile + 1, lay->n_kv_heads * n_layers, batch);
     const HeadMeta *metas = lay->d_meta + (size_t)layer * lay->n_kv_heads;
-    if (!attr_set) {   // once per process, outside any stream capture
+    if (first_use_on_device(1)) {   // once per device, outside any stream capture
         const int maxs = (int)append_smem_bytes(16 * kDh * 8 + 256 * 9 + 16 * kDh * 8);
 #define BGTQ_APPEND_ATTR(T, R, G) CUDA_TRY(cudaFuncSetAttribute(quantize_append_kernel<T, R, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, maxs))
         BGTQ_APPEND_ATTR(float, false, false); BGTQ_APPEND_ATTR(__nv_bfloat16, false, false);
         BGTQ_APPEND_ATTR(float, true, false);  BGTQ_APPEND_ATTR(__nv_bfloat16, true, false);
         BGTQ_APPEND_ATTR(float, false, true);  BGTQ_APPEND_ATTR(__nv_bfloat16, false, true);
 #undef BGTQ_APPEND_ATTR
-        attr_set = true;
     }
     const int32_t *pt = pm ? pm->table : nullptr;
     const int pstride = pm ? pm->table_stride : 0;

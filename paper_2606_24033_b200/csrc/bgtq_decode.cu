@@ -234,29 +234,6 @@ qfold_kernel(const HeadMeta *__restrict__ metas, const float *__restrict__ rot_t
     pdl_wait();
 }
 
-// ---------------------------------------------------------------- TMEM as a register parking space
-// The PV accumulators (32 registers per thread) are idle during the QK^T phase.  With 16 warps per SM the kernel has
-// 128 registers per thread and no shared memory to spare (tile buffers), so they are parked in tensor memory:
-// tcgen05.st / tcgen05.ld move 32 registers of every lane to / from 32 TMEM columns of the warp's lane quadrant.
-__device__ __forceinline__ void tmem_park(uint32_t taddr, const float (&O)[8][4])
-{
-    uint32_t r[32];
-#pragma unroll
-    for (int i = 0; i < 32; ++i) r[i] = __float_as_uint(O[i >> 2][i & 3]);
-    asm volatile("tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};"
-                 :: "r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]), "r"(r[16]), "r"(r[17]), "r"(r[18]), "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]), "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31]) : "memory");
-    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
-}
-__device__ __forceinline__ void tmem_unpark(uint32_t taddr, float (&O)[8][4])
-{
-    uint32_t r[32];
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
-                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31]) : "r"(taddr) : "memory");
-    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-    for (int i = 0; i < 32; ++i) O[i >> 2][i & 3] = __uint_as_float(r[i]);
-}
-
 // ---------------------------------------------------------------- the decode kernel
 struct DecodeParams {
     const HeadMeta *metas;      // [n_layers][Hkv], first layer of this call
@@ -417,13 +394,11 @@ __global__ void __launch_bounds__(W * 32, 1)
 decode_kernel(const DecodeParams P)
 {
     extern __shared__ __align__(128) unsigned char smem[];       // the per-warp tile buffers only
-    constexpr bool P5 = W < 16 && !BGTQ_NO_P5;                                   // the 4 KB 5-bit pair table is dropped where 16 tile buffers need the room
+    constexpr bool P5 = !BGTQ_NO_P5;
     __shared__ __align__(16) uint16_t lut[P5 ? kLutHalves : 512]; // static: constant LDS addresses for the LUTs
     __shared__ uint32_t pools[16];
     __shared__ int pre[kMaxBatch + 1];
     __shared__ __align__(8) uint64_t bars[2 * W];
-    constexpr bool PARK = W == 16;                                // 16 warps: 128 registers -> park O in TMEM during QK^T
-    __shared__ uint32_t tmem_base_s;
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int g8 = lane >> 2, c = lane & 3;
@@ -438,14 +413,7 @@ decode_kernel(const DecodeParams P)
 #endif
     build_lut(P.cb16, lut, tid, W * 32, P5);
     if (tid == 0) build_prefix(P.seq_len, P.batch, P.n_cap * kTile, pre, P.n_sink, P.n_recent);
-    if (PARK && warp == 0) {                                      // 4 warps per lane quadrant x 32 columns
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 128;" :: "r"(smem_u32(&tmem_base_s)) : "memory");
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-    }
-    if (PARK) asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
-    if (PARK) asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-    const uint32_t taddr = PARK ? tmem_base_s + ((uint32_t)(32 * (warp & 3)) << 16) + 32u * (warp >> 2) : 0u;
     if (tid == 0) build_pools(lut, pools);
     const uint32_t kbar = smem_u32(&bars[2 * warp]), vbar = smem_u32(&bars[2 * warp + 1]);
     if (lane == 0) {
@@ -473,7 +441,7 @@ decode_kernel(const DecodeParams P)
             merged_pair = tc.pair;
         }
     }
-    if (!PARK && !merged && x >= x_end) return;               // (with TMEM parking every warp stays for the dealloc barrier)
+    if (!merged && x >= x_end) return;
 
     const uint32_t *tile = reinterpret_cast<const uint32_t *>(smem + kSmemHdr + warp * P.buf_bytes);
     const uint32_t tile_s = smem_u32(tile);
@@ -483,7 +451,7 @@ decode_kernel(const DecodeParams P)
     // (the buffer was only READ through the generic proxy since its last fill, and __syncwarp orders those reads
     // before the copy is issued, so no cross-proxy fence is needed -- the usual consumer-release -> TMA pattern)
     auto issue_at = [&](const uint8_t *src, uint32_t kbytes, uint32_t vbytes, bool want_k, bool want_v) {
-        if (want_k) { mbar_expect_tx(kbar, kbytes); bulk_g2s(tile_s, src, kbytes, kbar); }
+        if (want_k && kbytes) { mbar_expect_tx(kbar, kbytes); bulk_g2s(tile_s, src, kbytes, kbar); }   // (no K group: nothing to copy)
         if (want_v) { mbar_expect_tx(vbar, vbytes); bulk_g2s(tile_s + kbytes, src + kbytes, vbytes, vbar); }
     };
     auto tile_src = [&](const TilePos &tp, const HeadMeta &M) -> const uint8_t * {
@@ -534,14 +502,12 @@ decode_kernel(const DecodeParams P)
         float O[8][4];
 #pragma unroll
         for (int J = 0; J < 8; ++J) O[J][0] = O[J][1] = O[J][2] = O[J][3] = 0.f;
-        if (PARK) tmem_park(taddr, O);              // TMEM is the home of O; registers hold it only during PV
 
         for (int t = tp.t; x < seg_end; ++x, ++t) {
             // ======== QK^T
             // paged: the next tile's page index is fetched a whole QK^T ahead of the copy that needs it
             const int next_page = (PAGED && x + 1 < seg_end) ? __ldg(prow + t + 1) : 0;
-            mbar_wait(kbar, kphase);
-            kphase ^= 1;
+            if (kbytes) { mbar_wait(kbar, kphase); kphase ^= 1; }
             TS(4);
             float Sc[8][4];
 #pragma unroll
@@ -642,7 +608,6 @@ decode_kernel(const DecodeParams P)
             }
             l0 = fmaf(l0, al0, ls0);
             l1 = fmaf(l1, al1, ls1);
-            if (PARK) tmem_unpark(taddr, O);
             if (__any_sync(0xFFFFFFFFu, al0 != 1.f || al1 != 1.f)) {
 #pragma unroll
                 for (int J = 0; J < 8; ++J) { O[J][0] *= al0; O[J][2] *= al0; O[J][1] *= al1; O[J][3] *= al1; }
@@ -677,7 +642,6 @@ decode_kernel(const DecodeParams P)
             }
             __syncwarp();
             TS(7);
-            if (PARK) tmem_park(taddr, O);
             if (x + 1 < seg_end) {
                 if (lane == 0) issue_at(src, kbytes, vbytes, false, true);                   // V half of the next tile
             } else if (x + 1 < x_end) {                                                      // next segment: other layout
@@ -688,7 +652,6 @@ decode_kernel(const DecodeParams P)
         }
 
         // ---------------- write this warp's partial for the pair: slot = warp + pair (unique, see combine)
-        if (PARK) tmem_unpark(taddr, O);
 #pragma unroll
         for (int o = 4; o < 32; o <<= 1) {
             l0 += __shfl_xor_sync(0xFFFFFFFFu, l0, o);
@@ -740,11 +703,6 @@ decode_kernel(const DecodeParams P)
         printf("cta %d warp %d: prologue %llu issue %llu pdlwait %llu ktile %llu qk %llu softmax+vwait %llu pv %llu tail %llu merge %llu total %llu\n", blockIdx.x, warp,
                tst[1] - tst[0], tst[2] - tst[1], tst[3] - tst[2], tst[4] - tst[3], tst[5] - tst[4], tst[6] - tst[5], tst[7] - tst[6], tst[8] - tst[7], tst[9] - tst[8], tst[9] - tst[0]);
 #endif
-    if (PARK) {
-        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-        __syncthreads();
-        if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 128;" :: "r"(tmem_base_s) : "memory");
-    }
 }
 
 // ---------------------------------------------------------------- a6: exact LSE merge + V de-rotation
@@ -971,13 +929,15 @@ template <typename T>
 __global__ void __launch_bounds__(128)
 window_append_kernel(const T *__restrict__ k_new, const T *__restrict__ v_new, const int32_t *__restrict__ seq_len,
                      __half *__restrict__ win_k, __half *__restrict__ win_v, int batch, int n_new, int Hkv,
-                     int n_sink, int n_recent)
+                     int n_sink, int n_recent, int64_t max_tokens)
 {
     const int i = blockIdx.x % n_new, lb = blockIdx.x / n_new, b = lb % batch, d = threadIdx.x;
-    const int64_t t = (int64_t)seq_len[b] + i;
+    const int64_t t0 = seq_len[b], t = t0 + i;
+    if (t >= max_tokens) return;                              // dropped by the append as well (capacity)
+    const int64_t n_kept = min((int64_t)n_new, max_tokens - t0);   // tokens of this call that are cached
     int slot;
     if (t < n_sink) slot = (int)t;
-    else if (n_recent > 0 && i >= n_new - n_recent) slot = n_sink + (int)(t % n_recent);
+    else if (n_recent > 0 && i >= n_kept - n_recent) slot = n_sink + (int)(t % n_recent);
     else return;
     const int n_win = n_sink + n_recent;
     for (int h = 0; h < Hkv; ++h) {
@@ -1213,14 +1173,11 @@ fp16_decode_kernel(const Fp16Params P)
 // ---------------------------------------------------------------- host side
 static int pick_warps(int buf_bytes)
 {
+    // measured: 12 warps at 168 registers beat 13 / 14 / 16 warps (spills, uneven schedulers)
     const int avail = 227 * 1024 - kStaticSmem;
-    const int cands[4] = {16, 12, 8, 4};
-    int cap = 12;   // measured: 16 warps at 128 registers (spills, no pair table) is slower than 12 at 168; 13 / 14 warps
-                    // (152 / 144 registers, small spills, uneven schedulers) run at 545 / 514 us against 429 us
-    if (const char *e = getenv("BGTQ_DECODE_WARPS")) cap = atoi(e);   // tuning knob (warps per CTA upper bound)
-    if (cap >= 16 && (size_t)16 * buf_bytes <= (size_t)(227 * 1024 - 2560)) return 16;   // W = 16 runs without the pair table
-    for (int i = 0; i < 4; ++i)
-        if (cands[i] <= cap && (size_t)cands[i] * buf_bytes <= (size_t)avail) return cands[i];
+    const int cands[3] = {12, 8, 4};
+    for (int i = 0; i < 3; ++i)
+        if ((size_t)cands[i] * buf_bytes <= (size_t)avail) return cands[i];
     return 0;
 }
 static size_t decode_smem(int W, int buf_bytes) { return kSmemHdr + (size_t)W * buf_bytes; }
@@ -1305,11 +1262,8 @@ int launch_window(const void *win_k, const void *win_v, const void *q, const int
 template <int W, bool PAGED>
 static int launch_decode_w(const DecodeParams &P, int grid, size_t smem, cudaStream_t st)
 {
-    static bool attr_set = false;
-    if (!attr_set) {   // once per process, outside any stream capture
-        CUDA_TRY(cudaFuncSetAttribute(decode_kernel<W, PAGED>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - (W == 16 ? 2560 : kStaticSmem)));
-        attr_set = true;
-    }
+    if (first_use_on_device(8 + (W / 4) * 2 + (PAGED ? 1 : 0)))   // once per device, outside any stream capture
+        CUDA_TRY(cudaFuncSetAttribute(decode_kernel<W, PAGED>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - kStaticSmem));
     if (int rc = profile_decode_begin(st)) return rc;
     {
         cudaLaunchConfig_t cfg = {};
@@ -1370,7 +1324,9 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
     count_launch();
     CUDA_TRY(cudaGetLastError());
 
-    const int buf_bytes = (lay->max_stride + 127) / 128 * 128;   // 128-byte aligned tile buffers
+    // 128-byte aligned tile buffers; a warp's buffer also receives its partial record when the CTA merges its warps
+    const int buf_bytes = (std::max(lay->max_stride, (int)(kPartialFloats * sizeof(float))) + 127) / 128 * 128;
+    if (lay->sm_count + 32 >= 1024) { set_error("bgtq_decode_attention: more SMs than combine_kernel's slot list holds"); return BGTQ_EINVAL; }
     const int W = pick_warps(buf_bytes);
     if (!W) { set_error("bgtq_decode_attention: tile does not fit shared memory"); return BGTQ_EINVAL; }
     DecodeParams P;
@@ -1384,14 +1340,12 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
     int rc;
     if (pm) {
         switch (W) {
-        case 16: rc = launch_decode_w<16, true>(P, grid, smem, st); break;
         case 12: rc = launch_decode_w<12, true>(P, grid, smem, st); break;
         case 8: rc = launch_decode_w<8, true>(P, grid, smem, st); break;
         default: rc = launch_decode_w<4, true>(P, grid, smem, st); break;
         }
     } else {
         switch (W) {
-        case 16: rc = launch_decode_w<16, false>(P, grid, smem, st); break;
         case 12: rc = launch_decode_w<12, false>(P, grid, smem, st); break;
         case 8: rc = launch_decode_w<8, false>(P, grid, smem, st); break;
         default: rc = launch_decode_w<4, false>(P, grid, smem, st); break;
@@ -1406,15 +1360,15 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
 }
 
 int launch_window_append(const void *k_new, const void *v_new, int dt, int n_layers, int batch, int n_new, int Hkv,
-                         const int32_t *seq_len, void *win_k, void *win_v, int n_sink, int n_recent, cudaStream_t st)
+                         const int32_t *seq_len, int64_t max_tokens, void *win_k, void *win_v, int n_sink, int n_recent, cudaStream_t st)
 {
     const int grid = n_layers * batch * n_new;
     if (dt == BGTQ_F32)
         window_append_kernel<float><<<grid, 128, 0, st>>>((const float *)k_new, (const float *)v_new, seq_len, (__half *)win_k,
-                                                          (__half *)win_v, batch, n_new, Hkv, n_sink, n_recent);
+                                                          (__half *)win_v, batch, n_new, Hkv, n_sink, n_recent, max_tokens);
     else
         window_append_kernel<__nv_bfloat16><<<grid, 128, 0, st>>>((const __nv_bfloat16 *)k_new, (const __nv_bfloat16 *)v_new, seq_len,
-                                                                  (__half *)win_k, (__half *)win_v, batch, n_new, Hkv, n_sink, n_recent);
+                                                                  (__half *)win_k, (__half *)win_v, batch, n_new, Hkv, n_sink, n_recent, max_tokens);
     count_launch();
     CUDA_TRY(cudaGetLastError());
     return BGTQ_OK;
@@ -1431,7 +1385,6 @@ int launch_fp16_decode(int n_layers, int batch, int Hq, int Hkv, const void *k_c
                        void *ws, size_t ws_bytes, cudaStream_t st)
 {
     static int sm_count = 0;
-    static bool attr_set = false;
     if (!sm_count) {
         int dev = 0;
         CUDA_TRY(cudaGetDevice(&dev));
@@ -1440,9 +1393,8 @@ int launch_fp16_decode(int n_layers, int batch, int Hq, int Hkv, const void *k_c
     if (batch > kMaxBatch) { set_error("bgtq_fp16_decode_attention: batch > 256"); return BGTQ_EINVAL; }
     if (ws_bytes < fp16_ws_bytes(sm_count, batch, n_layers, Hkv)) { set_error("bgtq_fp16_decode_attention: workspace too small"); return BGTQ_EWORKSPACE; }
     const size_t smem = (size_t)kFp16Warps * kFp16Buf;
-    if (!attr_set) {
+    if (first_use_on_device(2)) {
         CUDA_TRY(cudaFuncSetAttribute(fp16_decode_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = true;
     }
     Fp16Params P;
     P.k_cache = (const __half *)k_cache; P.v_cache = (const __half *)v_cache; P.q = (const __nv_bfloat16 *)q;
@@ -1552,235 +1504,6 @@ __device__ __forceinline__ void prefill_decode_v(const uint32_t *vcodes, int J, 
                 *reinterpret_cast<uint32_t *>(vhat_t + tile_off<UMMA>(dim, tok)) = v;
             }
     }
-}
-
-__global__ void __launch_bounds__(256, 2)
-prefill_kernel(const PrefillParams P)
-{
-    extern __shared__ __align__(128) unsigned char smem[];
-    __shared__ __align__(16) uint16_t lut[kLutHalves];
-    __shared__ uint32_t pools[16];
-    __shared__ __align__(8) uint64_t bar;
-    __shared__ PUnit units[2 * kMaxKSteps];
-    __shared__ int n_units_s;
-    __shared__ uint32_t tmem_base_s;                  // O (64 registers per thread) lives in tensor memory outside the PV phase,
-                                                      // which brings the kernel under 128 registers -> two CTAs per SM
-    __shared__ __align__(16) __half kn[kMaxGroups * 128];
-    __shared__ __align__(16) __half vn[128];
-    unsigned char *khat = smem;                       // [128 tokens][128 coords] fp16, 16-byte chunks XOR-swizzled
-    unsigned char *vhat_t = smem + 32768;             // [128 dims][128 tokens] fp16, swizzled
-    uint32_t *raw = reinterpret_cast<uint32_t *>(smem + 65536);
-
-    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g8 = lane >> 2, c = lane & 3;
-    const int h = blockIdx.y, b = blockIdx.z, G = P.G;
-    const HeadMeta &M = P.metas[h];
-    const int TQ = 16 * (8 / G);
-    const int n = warp % G, sb = warp / G;                         // head within the group, 16-token sub-block
-    int64_t slen = P.seq_len[b];
-    slen = slen > P.n_cap * kTile ? P.n_cap * kTile : slen;
-    const int i_first = blockIdx.x * TQ;
-    const int i_last = min(P.n_q, i_first + TQ) - 1;
-    const int64_t pos0 = slen - P.n_q;                              // position of query token 0
-    if (i_first >= P.n_q || pos0 < 0) return;
-    const int n_tiles = (int)((pos0 + i_last) / kTile) + 1;
-
-    build_lut(P.cb16, lut, tid, 256, true);
-    if (warp == 0) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 128;" :: "r"(smem_u32(&tmem_base_s)) : "memory");
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-    }
-    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-    for (int i = tid; i < 65536 / 16; i += 256) reinterpret_cast<uint4 *>(smem)[i] = make_uint4(0, 0, 0, 0);
-    if (tid == 0) {
-        int nu = 0, j = 0;
-        for (int ks = 0; ks < M.n_ksteps; ++ks) {
-            const KStep &K = M.ksteps[ks];
-            const int g = K.flags >> 4;
-            if (K.flags & 1) j = 0;
-            units[nu++] = PUnit{K.off0, K.b, K.nc0, M.gstart[g] + 8 * j, g};
-            ++j;
-            if (K.off1 != 0xFFFF) { units[nu++] = PUnit{K.off1, K.b, K.nc1, M.gstart[g] + 8 * j, g}; ++j; }
-        }
-        n_units_s = nu;
-        mbar_init(smem_u32(&bar), 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        fence_proxy_async();
-    }
-    __syncthreads();
-    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-    const uint32_t taddr = tmem_base_s + ((uint32_t)(32 * (warp & 3)) << 16) + 64u * (warp >> 2);
-    if (tid == 0) build_pools(lut, pools);
-    const int n_units = n_units_s, ng = M.n_groups, b_v = M.b_v;
-    const uint8_t *region = P.cache + P.n_cap * ((int64_t)P.batch * M.layer_prefix + (int64_t)b * M.layer_sum + M.head_prefix);
-    const uint32_t bar_s = smem_u32(&bar), raw_s = smem_u32(raw);
-    if (tid == 0) { mbar_expect_tx(bar_s, M.tile_stride); bulk_g2s(raw_s, region, M.tile_stride, bar_s); }
-
-    // this warp's 16 query rows: tokens i_first + sb*16 + {g8, g8+8}, head n; A fragments of q' for 8 k-steps
-    const int ti0 = i_first + sb * 16 + g8, ti1 = ti0 + 8;
-    const int64_t p0 = pos0 + ti0, p1 = pos0 + ti1;
-    uint32_t Qa[8][4];
-    {
-        const bool v0 = warp < 8 / G * G && ti0 < P.n_q, v1 = warp < 8 / G * G && ti1 < P.n_q;
-        const __half *q0 = P.qp + ((((size_t)b * P.n_q + (v0 ? ti0 : 0)) * P.Hkv + h) * 8 + n) * kDh;
-        const __half *q1 = P.qp + ((((size_t)b * P.n_q + (v1 ? ti1 : 0)) * P.Hkv + h) * 8 + n) * kDh;
-#pragma unroll
-        for (int ks = 0; ks < 8; ++ks) {
-            Qa[ks][0] = v0 ? *reinterpret_cast<const uint32_t *>(q0 + 16 * ks + 2 * c) : 0u;
-            Qa[ks][1] = v1 ? *reinterpret_cast<const uint32_t *>(q1 + 16 * ks + 2 * c) : 0u;
-            Qa[ks][2] = v0 ? *reinterpret_cast<const uint32_t *>(q0 + 16 * ks + 8 + 2 * c) : 0u;
-            Qa[ks][3] = v1 ? *reinterpret_cast<const uint32_t *>(q1 + 16 * ks + 8 + 2 * c) : 0u;
-        }
-    }
-    float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;
-    float O[16][4];
-#pragma unroll
-    for (int nd = 0; nd < 16; ++nd) O[nd][0] = O[nd][1] = O[nd][2] = O[nd][3] = 0.f;
-    tmem_park(taddr, reinterpret_cast<float (&)[8][4]>(O[0]));
-    tmem_park(taddr + 32, reinterpret_cast<float (&)[8][4]>(O[8]));
-    const uint32_t khat_s = smem_u32(khat), vhat_s = smem_u32(vhat_t);
-    uint32_t phase = 0;
-
-    for (int t = 0; t < n_tiles; ++t) {
-        // ---- stage + unpack tile t (all warps)
-        mbar_wait(bar_s, phase);
-        phase ^= 1;
-        for (int idx = tid; idx < (ng + 1) * 128; idx += 256) {      // linearise the norm rows
-            const int tau = idx & 127, g = idx >> 7;
-            const int slot = (tau & 7) * 16 + (tau >> 4) * 2 + ((tau >> 3) & 1);
-            const int off = g < ng ? M.knorm_off + 256 * g : M.vnorm_off;
-            const __half v = reinterpret_cast<const __half *>(reinterpret_cast<const unsigned char *>(raw) + off)[slot];
-            if (g < ng) kn[g * 128 + tau] = v; else vn[tau] = v;
-        }
-        __syncthreads();
-        for (int u = warp; u < n_units; u += 8) {
-            const PUnit U = units[u];
-            switch (U.b) {
-            case 1: prefill_decode_k<1>(raw, U, lane, pools, lut, kn, khat); break;
-            case 2: prefill_decode_k<2>(raw, U, lane, pools, lut, kn, khat); break;
-            case 3: prefill_decode_k<3>(raw, U, lane, pools, lut, kn, khat); break;
-            case 4: prefill_decode_k<4>(raw, U, lane, pools, lut, kn, khat); break;
-            case 5: prefill_decode_k<5>(raw, U, lane, pools, lut, kn, khat); break;
-            case 6: prefill_decode_k<6>(raw, U, lane, pools, lut, kn, khat); break;
-            case 7: prefill_decode_k<7>(raw, U, lane, pools, lut, kn, khat); break;
-            default: prefill_decode_k<8>(raw, U, lane, pools, lut, kn, khat); break;
-            }
-        }
-        {
-            const uint32_t *vcodes = raw + (M.vcode_off >> 2);
-            switch (b_v) {
-            case 1: prefill_decode_v<1>(vcodes, warp, lane, pools, lut, vn, vhat_t); break;
-            case 2: prefill_decode_v<2>(vcodes, warp, lane, pools, lut, vn, vhat_t); break;
-            case 3: prefill_decode_v<3>(vcodes, warp, lane, pools, lut, vn, vhat_t); break;
-            case 4: prefill_decode_v<4>(vcodes, warp, lane, pools, lut, vn, vhat_t); break;
-            case 5: prefill_decode_v<5>(vcodes, warp, lane, pools, lut, vn, vhat_t); break;
-            case 6: prefill_decode_v<6>(vcodes, warp, lane, pools, lut, vn, vhat_t); break;
-            case 7: prefill_decode_v<7>(vcodes, warp, lane, pools, lut, vn, vhat_t); break;
-            default: prefill_decode_v<8>(vcodes, warp, lane, pools, lut, vn, vhat_t); break;
-            }
-        }
-        __syncthreads();
-        if (tid == 0 && t + 1 < n_tiles) {                          // raw buffer is free: request the next tile
-            fence_proxy_async();
-            mbar_expect_tx(bar_s, M.tile_stride);
-            bulk_g2s(raw_s, region + (int64_t)(t + 1) * M.tile_stride, M.tile_stride, bar_s);
-        }
-        // ---- S = q' . K^T for this warp's 16 rows x 128 tokens of the tile (log2 domain)
-        float S[16][4];
-#pragma unroll
-        for (int nt = 0; nt < 16; ++nt) {
-            S[nt][0] = S[nt][1] = S[nt][2] = S[nt][3] = 0.f;
-#pragma unroll
-            for (int ks = 0; ks < 8; ks += 2) {
-                uint32_t r[4];
-                const int tok = 8 * nt + (lane & 7), ch = 2 * ks + (lane >> 3);
-                ldmatrix_x4(r, khat_s + tok * 256 + ((ch ^ (tok & 7)) << 4));
-                mma16816(S[nt], Qa[ks][0], Qa[ks][1], Qa[ks][2], Qa[ks][3], r[0], r[1]);
-                mma16816(S[nt], Qa[ks + 1][0], Qa[ks + 1][1], Qa[ks + 1][2], Qa[ks + 1][3], r[2], r[3]);
-            }
-        }
-        // ---- causal mask + online softmax per row (rows g8 and g8+8; columns 2c, 2c+1 of every n-tile)
-        const int64_t col0 = (int64_t)t * kTile + 2 * c;
-        if (col0 + 126 > (p0 < p1 ? p0 : p1)) {
-#pragma unroll
-            for (int nt = 0; nt < 16; ++nt) {
-                const int64_t j = col0 + 8 * nt;
-                if (j > p0) S[nt][0] = -INFINITY;
-                if (j + 1 > p0) S[nt][1] = -INFINITY;
-                if (j > p1) S[nt][2] = -INFINITY;
-                if (j + 1 > p1) S[nt][3] = -INFINITY;
-            }
-        }
-        float mx0 = -INFINITY, mx1 = -INFINITY;
-#pragma unroll
-        for (int nt = 0; nt < 16; ++nt) {
-            mx0 = fmaxf(mx0, fmaxf(S[nt][0], S[nt][1]));
-            mx1 = fmaxf(mx1, fmaxf(S[nt][2], S[nt][3]));
-        }
-#pragma unroll
-        for (int o = 1; o < 4; o <<= 1) {
-            mx0 = fmaxf(mx0, __shfl_xor_sync(0xFFFFFFFFu, mx0, o));
-            mx1 = fmaxf(mx1, __shfl_xor_sync(0xFFFFFFFFu, mx1, o));
-        }
-        const float mn0 = fmaxf(m0, mx0), mn1 = fmaxf(m1, mx1);
-        // a row whose causal prefix has not started yet (cannot happen: tile 0 always holds token 0) would give -inf
-        const float al0 = fast_exp2(m0 - mn0), al1 = fast_exp2(m1 - mn1);
-        m0 = mn0; m1 = mn1;
-        float ls0 = 0.f, ls1 = 0.f;
-#pragma unroll
-        for (int nt = 0; nt < 16; ++nt) {
-            S[nt][0] = fast_exp2(S[nt][0] - mn0); S[nt][1] = fast_exp2(S[nt][1] - mn0);
-            S[nt][2] = fast_exp2(S[nt][2] - mn1); S[nt][3] = fast_exp2(S[nt][3] - mn1);
-            ls0 += S[nt][0] + S[nt][1];
-            ls1 += S[nt][2] + S[nt][3];
-        }
-        l0 = fmaf(l0, al0, ls0);
-        l1 = fmaf(l1, al1, ls1);
-        uint32_t Pp[16][2];                                           // P as fp16 A fragments; S is dead from here
-#pragma unroll
-        for (int nt = 0; nt < 16; ++nt) { Pp[nt][0] = pack_half2(S[nt][0], S[nt][1]); Pp[nt][1] = pack_half2(S[nt][2], S[nt][3]); }
-        tmem_unpark(taddr, reinterpret_cast<float (&)[8][4]>(O[0]));
-        tmem_unpark(taddr + 32, reinterpret_cast<float (&)[8][4]>(O[8]));
-#pragma unroll
-        for (int nd = 0; nd < 16; ++nd) { O[nd][0] *= al0; O[nd][1] *= al0; O[nd][2] *= al1; O[nd][3] *= al1; }
-        // ---- O += P . V^   (A = P from the S fragments, B = V^T[dim][token] via ldmatrix)
-#pragma unroll
-        for (int kp = 0; kp < 8; ++kp) {
-            const uint32_t a0 = Pp[2 * kp][0], a1 = Pp[2 * kp][1], a2 = Pp[2 * kp + 1][0], a3 = Pp[2 * kp + 1][1];
-#pragma unroll
-            for (int nd = 0; nd < 16; nd += 2) {
-                uint32_t r[4];
-                const int dim = 8 * (nd + (lane >> 4)) + (lane & 7), ch = 2 * kp + ((lane >> 3) & 1);
-                ldmatrix_x4(r, vhat_s + dim * 256 + ((ch ^ (dim & 7)) << 4));
-                mma16816(O[nd], a0, a1, a2, a3, r[0], r[1]);
-                mma16816(O[nd + 1], a0, a1, a2, a3, r[2], r[3]);
-            }
-        }
-        tmem_park(taddr, reinterpret_cast<float (&)[8][4]>(O[0]));
-        tmem_park(taddr + 32, reinterpret_cast<float (&)[8][4]>(O[8]));
-        __syncthreads();                                              // K^/V^ are overwritten by the next tile
-    }
-    tmem_unpark(taddr, reinterpret_cast<float (&)[8][4]>(O[0]));
-    tmem_unpark(taddr + 32, reinterpret_cast<float (&)[8][4]>(O[8]));
-    // ---- normalise and store the rotated-domain output rows (fp32); derotate_kernel finishes them
-#pragma unroll
-    for (int o = 1; o < 4; o <<= 1) {
-        l0 += __shfl_xor_sync(0xFFFFFFFFu, l0, o);
-        l1 += __shfl_xor_sync(0xFFFFFFFFu, l1, o);
-    }
-    const float i0 = 1.f / l0, i1 = 1.f / l1;
-    if (ti0 < P.n_q) {
-        float *dst = P.opart + (((size_t)b * P.n_q + ti0) * (P.Hkv * G) + h * G + n) * kDh;
-#pragma unroll
-        for (int nd = 0; nd < 16; ++nd) *reinterpret_cast<float2 *>(dst + 8 * nd + 2 * c) = make_float2(O[nd][0] * i0, O[nd][1] * i0);
-    }
-    if (ti1 < P.n_q) {
-        float *dst = P.opart + (((size_t)b * P.n_q + ti1) * (P.Hkv * G) + h * G + n) * kDh;
-#pragma unroll
-        for (int nd = 0; nd < 16; ++nd) *reinterpret_cast<float2 *>(dst + 8 * nd + 2 * c) = make_float2(O[nd][2] * i1, O[nd][3] * i1);
-    }
-    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-    __syncthreads();
-    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 128;" :: "r"(tmem_base_s) : "memory");
 }
 
 // ---------------------------------------------------------------- prefill on the 5th-generation tensor cores
@@ -2403,7 +2126,6 @@ int launch_prefill(const bgtq_layout *lay, int layer, const void *cache, const v
                    int batch, int n_q, int64_t max_tokens, float scale, void *out, void *ws, size_t ws_bytes,
                    cudaStream_t st)
 {
-    static bool attr_set = false;
     const int Hkv = lay->n_kv_heads, Hq = lay->n_q_heads, G = Hq / Hkv;
     if (G != 1 && G != 2 && G != 4 && G != 8) { set_error("bgtq_prefill_attention: GQA group must be 1, 2, 4 or 8"); return BGTQ_EINVAL; }
     if (ws_bytes < prefill_ws_bytes(lay, batch, n_q)) { set_error("bgtq_prefill_attention: workspace too small"); return BGTQ_EWORKSPACE; }
@@ -2418,29 +2140,24 @@ int launch_prefill(const bgtq_layout *lay, int layer, const void *cache, const v
     count_launch();
     CUDA_TRY(cudaGetLastError());
     const int raw_bytes = (lay->max_stride + 127) / 128 * 128;
-    static int use_tc = -1;                         // BGTQ_PREFILL_MMA_SYNC=1 selects the first-cut mma.sync kernel
-    if (use_tc < 0) { const char *e = getenv("BGTQ_PREFILL_MMA_SYNC"); use_tc = (e && atoi(e) != 0) ? 0 : 1; }
-    // two 128-row query tiles per CTA when the raw tile still fits beside 192 KB of operands (12.5 KB of static tables)
+    // two 128-row query tiles per CTA (warp-specialised kernel) when the raw tile still fits beside 192 KB of operands
+    // (12.5 KB of static tables) and there is more than one tile of query rows; else one tile per CTA
     const int RT = (tc_operand_bytes(2) + raw_bytes + 13 * 1024 <= 227 * 1024 && (n_q * G > 128)) ? 2 : 1;
-    const size_t smem = (use_tc ? (size_t)tc_operand_bytes(RT) : 65536) + (size_t)raw_bytes;
-    if (!attr_set) {
-        CUDA_TRY(cudaFuncSetAttribute(prefill_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 65536 + 40 * 1024));
+    const size_t smem = (size_t)tc_operand_bytes(RT) + (size_t)raw_bytes;
+    if (first_use_on_device(3)) {
         CUDA_TRY(cudaFuncSetAttribute(prefill_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc_operand_bytes(1) + 40 * 1024));
-        CUDA_TRY(cudaFuncSetAttribute(prefill_tc_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 13 * 1024));
         CUDA_TRY(cudaFuncSetAttribute(prefill_ws_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 13 * 1024));
-        attr_set = true;
     }
     PrefillParams P;
     P.metas = metas; P.cache = (const uint8_t *)cache; P.qp = qp; P.seq_len = seq_len; P.cb16 = lay->d_cb16;
     P.opart = opart; P.n_cap = (max_tokens + kTile - 1) / kTile; P.batch = batch; P.n_q = n_q; P.Hkv = Hkv; P.G = G;
     P.raw_bytes = raw_bytes;
-    const int TQ = (use_tc ? RT * 128 : 128) / G;
+    const int TQ = RT * 128 / G;
     dim3 grid((n_q + TQ - 1) / TQ, Hkv, batch);
-    static int use_ws = -1;                         // BGTQ_PREFILL_WS=0 selects the phase-synchronous tcgen05 kernel
-    if (use_ws < 0) { const char *e = getenv("BGTQ_PREFILL_WS"); use_ws = (e && atoi(e) == 0) ? 0 : 1; }
-    if (!use_tc) prefill_kernel<<<grid, 256, smem, st>>>(P);
-    else if (RT == 2 && use_ws) prefill_ws_kernel<<<grid, kTcThreads, smem, st>>>(P);
-    else if (RT == 2) prefill_tc_kernel<2><<<grid, kTcThreads, smem, st>>>(P);
+    // a sequence shorter than the chunk (seq_len < n_q, a caller error the host cannot see) leaves its rows untouched
+    // in the kernels: start from zeros so that the output is defined
+    CUDA_TRY(cudaMemsetAsync(opart, 0, rows * Hq * kDh * sizeof(float), st));
+    if (RT == 2) prefill_ws_kernel<<<grid, kTcThreads, smem, st>>>(P);
     else prefill_tc_kernel<1><<<grid, kTcThreads, smem, st>>>(P);
     count_launch();
     CUDA_TRY(cudaGetLastError());

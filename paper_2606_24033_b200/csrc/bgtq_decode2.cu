@@ -821,11 +821,9 @@ int launch_decode2(const bgtq_layout *lay, int layer0, int n_layers, const void 
     P.pages = pm ? pm->table : nullptr; P.pstride = pm ? pm->table_stride : 0; P.n_pages = pm ? pm->n_pages : 0;
     P.n_sink = n_sink; P.n_recent = n_recent;
     const size_t smem = 17 * 1024 + (size_t)P.n_stages * P.stage_bytes;
-    static bool attr_set = false;
-    if (!attr_set) {
+    if (first_use_on_device(4)) {
         CUDA_TRY(cudaFuncSetAttribute(decode2_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - static_smem));
         CUDA_TRY(cudaFuncSetAttribute(decode2_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - static_smem));
-        attr_set = true;
     }
     if (int rc = profile_decode_begin(st)) return rc;
     {

@@ -3,6 +3,7 @@
 #include <atomic>
 #include <cmath>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #include <cuda_fp16.h>
@@ -21,6 +22,17 @@ int cuda_fail(cudaError_t e, const char *what)
     return BGTQ_ECUDA;
 }
 void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+bool first_use_on_device(int key)
+{
+    static std::mutex mu;
+    static bool seen[32][64] = {};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64 || key < 0 || key >= 32) return true;
+    std::lock_guard<std::mutex> lock(mu);
+    const bool first = !seen[key][dev];
+    seen[key][dev] = true;
+    return first;
+}
 
 }  // namespace bgtq
 
@@ -524,15 +536,18 @@ extern "C" size_t bgtq_window_bytes(const bgtq_layout *lay, int batch, int n_sin
 }
 
 extern "C" int bgtq_window_append(const bgtq_layout *lay, int layer0, int n_layers, const void *k_new, const void *v_new,
-                                  int dt, int batch, int n_new, const int32_t *seq_len, void *win_k, void *win_v,
-                                  int n_sink, int n_recent, void *stream)
+                                  int dt, int batch, int n_new, const int32_t *seq_len, int64_t max_tokens, void *win_k,
+                                  void *win_v, int n_sink, int n_recent, void *stream)
 {
+    if (max_tokens <= 0) FAIL(BGTQ_EINVAL, "bgtq_window_append: max_tokens");
+    if (n_sink >= BGTQ_TILE_TOKENS || n_sink + n_recent > 1024)
+        FAIL(BGTQ_EINVAL, "bgtq_window_append: need 0 <= n_sink < 128, 1 <= n_sink + n_recent <= 1024");
     if (!lay || !k_new || !v_new || !seq_len || !win_k || !win_v) FAIL(BGTQ_EINVAL, "bgtq_window_append: null pointer");
     if (layer0 < 0 || n_layers <= 0 || layer0 + n_layers > lay->n_layers) FAIL(BGTQ_EINVAL, "bgtq_window_append: layer range");
     if (dt != BGTQ_F32 && dt != BGTQ_BF16) FAIL(BGTQ_EINVAL, "bgtq_window_append: dtype");
     if (batch <= 0 || n_new <= 0 || n_sink < 0 || n_recent < 0 || n_sink + n_recent < 1) FAIL(BGTQ_EINVAL, "bgtq_window_append: batch/n_new/window");
     const size_t per_layer = (size_t)batch * lay->n_kv_heads * (size_t)(n_sink + n_recent) * lay->d_h;
-    return launch_window_append(k_new, v_new, dt, n_layers, batch, n_new, lay->n_kv_heads, seq_len,
+    return launch_window_append(k_new, v_new, dt, n_layers, batch, n_new, lay->n_kv_heads, seq_len, max_tokens,
                                 (uint16_t *)win_k + (size_t)layer0 * per_layer, (uint16_t *)win_v + (size_t)layer0 * per_layer,
                                 n_sink, n_recent, (cudaStream_t)stream);
 }

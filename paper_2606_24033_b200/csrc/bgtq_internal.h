@@ -78,6 +78,9 @@ namespace bgtq {
 void set_error(const std::string &msg);
 int cuda_fail(cudaError_t e, const char *what);
 void count_launch(int n = 1);
+// true exactly once per (key, current CUDA device): kernel function attributes are per device and must be set on each
+// device the library is used on (thread-safe)
+bool first_use_on_device(int key);
 void codebook_levels(int b, double *levels);
 // e4m3 byte planes of C_b (v2 decode path): level k of width b is represented as (hi[k] + lo[k]) / kappa with hi, lo
 // e4m3 values; kappa in [32, 64] is chosen per width to minimise the largest relative error (0 for b = 1, 3; < 2e-6 for
@@ -126,7 +129,8 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
                   float scale, void *out, void *ws, size_t ws_bytes, const PageMap *pm, cudaStream_t st,
                   const Window *win = nullptr);
 int launch_window_append(const void *k_new, const void *v_new, int dt, int n_layers, int batch, int n_new, int Hkv,
-                         const int32_t *seq_len, void *win_k, void *win_v, int n_sink, int n_recent, cudaStream_t st);
+                         const int32_t *seq_len, int64_t max_tokens, void *win_k, void *win_v, int n_sink, int n_recent,
+                         cudaStream_t st);
 size_t decode_ws_bytes(const bgtq_layout *lay, int batch, int n_layers);
 int launch_decode2(const bgtq_layout *lay, int layer0, int n_layers, const void *cache,
                    const void *q, const int32_t *seq_len, int batch, int64_t max_tokens,

@@ -764,3 +764,119 @@ def test_protected_argument_errors(P):
     for ns, nr in [(128, 4), (0, 0), (-1, 4), (4, 2000)]:
         with pytest.raises(P.BgtqError):
             P.decode_attention_protected(lay, 0, cache, q, seq, 128, 0.1, wk, wv, ns, nr, lay.new_workspace(1))
+
+
+# ----------------------------------------------------------------------------- capacity that is not a whole number of tiles
+@pytest.mark.parametrize("fmt", [1, 2])
+def test_append_past_a_capacity_that_is_not_a_tile_multiple(P, tab128, fmt):
+    """max_tokens = 1000 (not a multiple of 128): tokens at positions >= 1000 are dropped, seq_len saturates at 1000 and the
+    bytes equal the oracle's packing of the first 1000 tokens -- also with the fused-RoPE append, whose cos / sin tables
+    have exactly max_tokens rows (nothing beyond them may be read)."""
+    T, cap = 1030, 1000
+    p = H.make_problem(77, T, 4, 2, 3, 3, 1, 8, rope_base=1e6)
+    lay = P.Layout(p.bits[None], p.Hq, p.d_h, p.b_v, p.rot, fmt=fmt)
+    cache = lay.new_cache(1, cap)
+    seq = torch.zeros(1, dtype=torch.int32, device="cuda")
+    for (a, b) in [(0, 990), (990, 1030)]:
+        P.quantize_append(lay, 0, cache, _cuda(p.k_post[None, a:b], torch.float32), _cuda(p.v[None, a:b], torch.float32), seq, cap)
+    assert seq.tolist() == [cap]
+    heads = H.oracle_heads(p, tab128, 0, cap)
+    host = cache.cpu().numpy()
+    for h in range(p.Hkv):
+        stride = lay.tile_stride(0, h)
+        off = lay.region_offset(0, 0, h, 1, cap)
+        exp = np.zeros(8 * stride, dtype=np.uint8)
+        O.pack_region(heads[h], p.d_h, exp, version=fmt)
+        assert np.array_equal(host[off:off + 8 * stride], exp), h
+    # one more append at capacity: nothing changes
+    P.quantize_append(lay, 0, cache, _cuda(p.k_post[None, :5], torch.float32), _cuda(p.v[None, :5], torch.float32), seq, cap)
+    assert seq.tolist() == [cap] and np.array_equal(cache.cpu().numpy(), host)
+    # attention over the saturated cache
+    scale = 1.0 / math.sqrt(p.d_h)
+    out = P.decode_attention(lay, 0, cache, _cuda(p.q_post[None], torch.bfloat16), seq, cap, scale, lay.new_workspace(1))
+    pc = H.Problem(p.d_h, p.Hq, p.Hkv, cap, p.b_v, p.bits, p.k_post[:cap], p.v[:cap], p.q_post, p.scores, p.rot)
+    exp, rv = H.oracle_attention(pc, heads, tab128, scale)
+    got = out[0].double().cpu().numpy()
+    assert max(np.max(np.abs(got[a] - exp[a])) / rv[a // 2] for a in range(p.Hq)) <= 2e-3
+
+
+def test_rope_append_with_tables_of_exactly_max_tokens_rows(P, tab128):
+    T, cap, d = 1010, 1000, 128
+    p = H.make_problem(78, T, 4, 2, 3, 3, 1, 8, rope_base=1e6)
+    scales = W.block_scales(78, 2, 64)
+    k_pre = W.pre_rope_gaussian(78, 1, T, 2, d, scales).astype(np.float32).astype(np.float64)
+    inv = 1e6 ** (-np.arange(64) / 64.0)
+    ang = np.arange(cap)[:, None] * inv[None, :]
+    cos, sin = np.cos(ang).astype(np.float32), np.sin(ang).astype(np.float32)      # exactly `cap` rows
+    lay = P.Layout(p.bits[None], p.Hq, d, p.b_v, p.rot)
+    cache = lay.new_cache(1, cap)
+    seq = torch.zeros(1, dtype=torch.int32, device="cuda")
+    for (a, b) in [(0, 995), (995, 1010)]:
+        P.quantize_append_rope(lay, 0, cache, _cuda(k_pre[None, None, a:b], torch.float32), _cuda(p.v[None, None, a:b], torch.float32),
+                               seq, cap, torch.from_numpy(cos).cuda(), torch.from_numpy(sin).cuda(), n_layers=1)
+    torch.cuda.synchronize()
+    assert seq.tolist() == [cap]
+    k_rot = O.rope_table(k_pre[:cap], cos.astype(np.float64), sin.astype(np.float64))
+    host = cache.cpu().numpy()
+    for h in range(2):
+        head = O.quantize_head(k_rot[:, h], p.v[:cap, h], p.bits[h], p.b_v, tab128)
+        stride = lay.tile_stride(0, h)
+        off = lay.region_offset(0, 0, h, 1, cap)
+        exp = np.zeros(8 * stride, dtype=np.uint8)
+        O.pack_region(head, d, exp)
+        assert np.array_equal(host[off:off + 8 * stride], exp), h
+
+
+@pytest.mark.parametrize("bits_kind", ["mostly_zero", "all_zero"])
+def test_attention_sparse_keys_b_v1_multi_cta(P, tab128, bits_kind):
+    """Tile stride below the partial-record size (zero-width K blocks, b_V = 1) at a context long enough for CTAs to merge
+    their warps' records in shared memory; and a head without any K group (every logit 0: uniform attention)."""
+    T = 128 * 640
+    p = H.make_problem(79, T, 8, 1, 3, 1, 0, 8, rope_base=1e6, n_cal=32)
+    p.bits[:] = 0
+    if bits_kind == "mostly_zero":
+        p.bits[0, :6] = [1, 1, 2, 1, 0, 1]
+    lay = P.Layout(p.bits[None], p.Hq, p.d_h, 1, p.rot)
+    assert lay.tile_stride(0, 0) < 8 * 130 * 4
+    cache = lay.new_cache(1, T)
+    seq = torch.zeros(1, dtype=torch.int32, device="cuda")
+    P.quantize_append(lay, 0, cache, _cuda(p.k_post[None], torch.float32), _cuda(p.v[None], torch.float32), seq, T)
+    scale = 1.0 / math.sqrt(p.d_h)
+    out = P.decode_attention(lay, 0, cache, _cuda(p.q_post[None], torch.bfloat16), seq, T, scale, lay.new_workspace(1))
+    torch.cuda.synchronize()
+    heads = H.oracle_heads(p, tab128)
+    exp, rv = H.oracle_attention(p, heads, tab128, scale)
+    got = out[0].double().cpu().numpy()
+    err = max(np.max(np.abs(got[a] - exp[a])) / rv[0] for a in range(p.Hq))
+    assert err <= 2e-3, err
+
+
+def test_window_append_respects_capacity(P, tab128):
+    """Tokens beyond max_tokens are dropped by bgtq_window_append exactly as by the append: the ring keeps the rows of the
+    last n_recent CACHED tokens, and the protected attention over the saturated cache matches the oracle on those tokens."""
+    T, cap, ns, nr = 300, 256, 4, 64
+    p = H.make_problem(80, T, 8, 2, 3, 2, 1, 8, rope_base=1e6)
+    lay = P.Layout(p.bits[None], p.Hq, p.d_h, p.b_v, p.rot)
+    cache = lay.new_cache(1, cap)
+    seq = torch.zeros(1, dtype=torch.int32, device="cuda")
+    win_k, win_v = P.new_windows(lay, 1, ns, nr)
+    for (a, b) in [(0, 200), (200, 300)]:
+        kk, vv = _cuda(p.k_post[None, a:b], torch.float32), _cuda(p.v[None, a:b], torch.float32)
+        P.window_append(lay, 0, kk, vv, seq, win_k, win_v, ns, nr, max_tokens=cap)
+        P.quantize_append(lay, 0, cache, kk, vv, seq, cap)
+    assert seq.tolist() == [cap]
+    pc = H.Problem(p.d_h, p.Hq, p.Hkv, cap, p.b_v, p.bits, p.k_post[:cap], p.v[:cap], p.q_post, p.scores, p.rot)
+    wk, wv, prot = _host_windows(pc, ns, nr)
+    slots = sorted(O.window_slot(int(t), ns, nr) for t in prot)
+    assert np.array_equal(win_k[0, 0].cpu().numpy()[:, slots].view(np.uint16), wk[:, slots].view(np.uint16))
+    assert np.array_equal(win_v[0, 0].cpu().numpy()[:, slots].view(np.uint16), wv[:, slots].view(np.uint16))
+    heads = H.oracle_heads(pc, tab128)
+    scale = 1.0 / math.sqrt(p.d_h)
+    out = P.decode_attention_protected(lay, 0, cache, _cuda(p.q_post[None], torch.bfloat16), seq, cap, scale, win_k, win_v, ns, nr,
+                                       lay.new_workspace(1))
+    exp = _protected_expected(pc, heads, tab128, scale, ns, nr)
+    _, rv = H.oracle_attention(pc, heads, tab128, scale)
+    got = out[0].double().cpu().numpy()
+    assert max(np.max(np.abs(got[a] - exp[a])) / rv[a // 4] for a in range(p.Hq)) <= 2e-3
+    with pytest.raises(P.BgtqError):
+        P.window_append(lay, 0, _cuda(p.k_post[None, :1], torch.float32), _cuda(p.v[None, :1], torch.float32), seq, win_k, win_v, 128, 64)
