@@ -156,3 +156,105 @@ def codebook(b: int, table: np.ndarray | None = None) -> np.ndarray:
     if table is None:
         table = codebook_table()
     return table[(1 << b) - 1:(1 << (b + 1)) - 1]
+
+
+# ----------------------------------------------------------------------------- exact-density codebooks
+# TQ-MSE "scalar-quantizes the rotated coordinates" of a NORMALISED vector.  A coordinate of
+# sqrt(m) * u, u uniform on the unit sphere of R^m (what a Haar rotation makes of any unit vector), has the density
+#     f_m(x) = c_m (1 - x^2/m)^((m-3)/2),  |x| < sqrt(m),   c_m = Gamma(m/2) / (sqrt(pi m) Gamma((m-1)/2)),
+# which tends to N(0,1) as m grows but is visibly different for the small groups the allocator produces (m = 2 is the
+# arcsine law, m = 3 is uniform).  C_{b,m} = Lloyd-Max quantiser of f_m, symmetric, ascending, rounded to fp16.
+def _sphere_const(m: int) -> float:
+    return math.exp(math.lgamma(m / 2.0) - math.lgamma((m - 1) / 2.0)) / math.sqrt(math.pi * m)
+
+
+def sphere_pdf(x: float, m: int) -> float:
+    u = 1.0 - x * x / m
+    if u <= 0.0:
+        return math.inf if (m == 2 and u == 0.0) else 0.0
+    return _sphere_const(m) * u ** ((m - 3) / 2.0)
+
+
+def _sphere_mass(a: float, b: float, m: int) -> float:
+    """P(a < X < b), 0 <= a < b <= sqrt(m): regularised incomplete beta, I_{x^2/m}(1/2, (m-1)/2) = P(|X| < x)."""
+    from scipy.special import betainc
+    fa = betainc(0.5, (m - 1) / 2.0, min(a * a / m, 1.0))
+    fb = betainc(0.5, (m - 1) / 2.0, min(b * b / m, 1.0))
+    return 0.5 * (fb - fa)
+
+
+def _sphere_first_moment(a: float, b: float, m: int) -> float:
+    """int_a^b x f_m(x) dx = [-(m/(m-1)) c_m (1 - x^2/m)^((m-1)/2)]_a^b."""
+    G = lambda x: -(m / (m - 1.0)) * _sphere_const(m) * max(1.0 - x * x / m, 0.0) ** ((m - 1) / 2.0)
+    return G(b) - G(a)
+
+
+def sphere_lloyd_max_positive(n_pos: int, m: int, tol: float = 1e-13, max_iter: int = 500) -> np.ndarray:
+    """The n_pos positive levels of the symmetric 2*n_pos-level Lloyd-Max quantiser of f_m (Newton on the centroid
+    conditions, as lloyd_max_positive; the support ends at sqrt(m))."""
+    top = math.sqrt(m)
+    c = lloyd_max_positive(n_pos)
+    if c[-1] >= 0.98 * top:
+        c = c * (0.98 * top / c[-1])
+    for _ in range(max_iter):
+        t = np.empty(n_pos + 1)
+        t[0] = 0.0
+        t[1:n_pos] = 0.5 * (c[:-1] + c[1:])
+        t[n_pos] = top
+        F = np.empty(n_pos)
+        Jm = np.zeros((n_pos, n_pos))
+        for k in range(n_pos):
+            a, b = t[k], t[k + 1]
+            P = _sphere_mass(a, b, m)
+            g = _sphere_first_moment(a, b, m) / P
+            dga = sphere_pdf(a, m) * (g - a) / P
+            dgb = 0.0 if k + 1 == n_pos else sphere_pdf(b, m) * (b - g) / P
+            F[k] = c[k] - g
+            Jm[k, k] = 1.0
+            if k > 0:
+                Jm[k, k - 1] -= 0.5 * dga
+                Jm[k, k] -= 0.5 * dga
+            if k + 1 < n_pos:
+                Jm[k, k] -= 0.5 * dgb
+                Jm[k, k + 1] -= 0.5 * dgb
+        step = np.linalg.solve(Jm, F)
+        lam = 1.0
+        while lam > 1e-8:
+            cn = c - lam * step
+            if cn[0] > 0 and np.all(np.diff(cn) > 0) and cn[-1] < top:
+                break
+            lam *= 0.5
+        c = cn
+        if np.max(np.abs(F)) < tol and lam == 1.0:
+            break
+    return c
+
+
+@lru_cache(maxsize=None)
+def sphere_levels(b: int, m: int) -> np.ndarray:
+    """All 2^b levels of C_{b,m}, ascending, fp64, NOT yet rounded to fp16."""
+    if b == 0:
+        return np.zeros(1)
+    pos = sphere_lloyd_max_positive(1 << (b - 1), m)
+    return np.concatenate([-pos[::-1], pos])
+
+
+def sphere_distortion(levels: np.ndarray, m: int) -> float:
+    """E[(X - Q(X))^2] for X ~ f_m and nearest-level quantisation: E X^2 = 1, so D = 1 - 2 sum c_k M1_k + sum c_k^2 P_k."""
+    lv = np.asarray(levels, dtype=np.float64)
+    pos = lv[lv > 0]
+    top = math.sqrt(m)
+    t = np.concatenate([[0.0], 0.5 * (pos[:-1] + pos[1:]), [top]])
+    D = 1.0
+    for k, c in enumerate(pos):
+        a, b = min(t[k], top), min(t[k + 1], top)
+        if b <= a:
+            continue
+        D += 2.0 * (c * c * _sphere_mass(a, b, m) - 2.0 * c * _sphere_first_moment(a, b, m))
+    return D
+
+
+@lru_cache(maxsize=None)
+def sphere_codebook(b: int, m: int) -> np.ndarray:
+    """C_{b,m} rounded to fp16-representable values (fp64 array)."""
+    return f16_round(sphere_levels(b, m))

@@ -202,10 +202,16 @@ def groups_from_bits(bits: Sequence[int], d_h: int, pairing: int = PAIR_HALF) ->
 
 
 class Tables:
-    """Codebooks (oracle's own Lloyd-Max, fp16-rounded) + the rotation table passed in as data."""
+    """Codebooks (oracle's own Lloyd-Max, fp16-rounded) + the rotation table passed in as data.
+    cb_kind "gaussian": one table per width, the Lloyd-Max quantiser of N(0,1) (reading Q7);
+    cb_kind "sphere":   one table per (width, group size m): the Lloyd-Max quantiser of the exact density of a rotated
+                        coordinate of a normalised m-vector (oracle/codebook.py sphere_codebook)."""
 
-    def __init__(self, rotations_flat: np.ndarray, d_h: int, cb_table: np.ndarray | None = None):
+    def __init__(self, rotations_flat: np.ndarray, d_h: int, cb_table: np.ndarray | None = None,
+                 cb_kind: str = "gaussian"):
+        assert cb_kind in ("gaussian", "sphere")
         self.d_h = d_h
+        self.cb_kind = cb_kind
         self.cb = _cb.codebook_table() if cb_table is None else _c64(cb_table)
         self.rot = np.ascontiguousarray(rotations_flat, dtype=np.float32)
         self.off = {}
@@ -215,7 +221,10 @@ class Tables:
             o += m * m
         assert o == self.rot.size
 
-    def C(self, b: int) -> np.ndarray:
+    def C(self, b: int, m: int | None = None) -> np.ndarray:
+        if self.cb_kind == "sphere":
+            assert m is not None
+            return np.ascontiguousarray(_cb.sphere_codebook(b, m))
         return np.ascontiguousarray(self.cb[(1 << b) - 1:(1 << (b + 1)) - 1])
 
     def Pi(self, m: int) -> np.ndarray:
@@ -228,7 +237,7 @@ def quantize_group(x: np.ndarray, b: int, tab: Tables):
     Returns (idx uint8[m], h_bits, r)."""
     x = _c64(x)
     m = len(x)
-    Pi, Cb = tab.Pi(m), tab.C(b)
+    Pi, Cb = tab.Pi(m), tab.C(b, m)
     idx = np.zeros(m, dtype=np.uint8)
     h = C.c_uint16(0)
     r = C.c_double(0.0)
@@ -241,7 +250,7 @@ def dequantize_group(idx: np.ndarray, h_bits: int, b: int, tab: Tables) -> np.nd
     """Oracle step 6: xhat = (h/sqrt(m)) * Pi^T C[idx]."""
     idx = np.ascontiguousarray(idx, dtype=np.uint8)
     m = len(idx)
-    Pi, Cb = tab.Pi(m), tab.C(b)
+    Pi, Cb = tab.Pi(m), tab.C(b, m)
     out = np.empty(m)
     lib().orc_dequantize_group(_p(idx, C.c_uint8), m, int(h_bits), _p(Pi, C.c_float),
                                _p(Cb, C.c_double), _p(out, C.c_double))

@@ -74,3 +74,18 @@ def oracle_attention(p: Problem, heads: List[O.QuantizedHead], tab: O.Tables, sc
         for a in range(h * G, (h + 1) * G):
             out[a] = O.attention(p.q_post[a], K, V, scale)
     return out, rv
+
+
+def record_error(name: str, got: np.ndarray, exp: np.ndarray, rv: float, **extra) -> float:
+    """Achieved attention error of a parity case: max-abs / R_V (the bar of north_star) and max-abs / max|o| (how large
+    the error is against the output itself).  Appended to gpurun_out/achieved_errors.jsonl when that folder exists, so
+    that BASELINE.md can quote measured numbers; returns max-abs / R_V."""
+    import json
+    import os
+    d = float(np.max(np.abs(got - exp)))
+    rec = {"case": name, "max_abs_over_R_V": d / rv, "max_abs_over_max_abs_o": d / float(np.max(np.abs(exp))), **extra}
+    out = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
+    if os.path.isdir(out):
+        with open(os.path.join(out, "achieved_errors.jsonl"), "a") as f:
+            f.write(json.dumps(rec) + "\n")
+    return d / rv
