@@ -299,11 +299,11 @@ def dequantize_head(q: QuantizedHead, tab: Tables, d_h: int) -> Tuple[np.ndarray
     K = np.zeros((T, d_h))
     o = 0
     for gi, g in enumerate(q.groups):
-        Cb, Pi = tab.C(g.width), tab.Pi(g.m).astype(np.float64)
+        Cb, Pi = tab.C(g.width, g.m), tab.Pi(g.m).astype(np.float64)
         h = np.array([f16_value(x) for x in q.knorm[:, gi]]) if T < 64 else _f16_array(q.knorm[:, gi])
         K[:, g.coords] = (h / math.sqrt(g.m))[:, None] * (Cb[q.kidx[:, o:o + g.m]] @ Pi)
         o += g.m
-    Cv, Piv = tab.C(q.b_v), tab.Pi(d_h).astype(np.float64)
+    Cv, Piv = tab.C(q.b_v, d_h), tab.Pi(d_h).astype(np.float64)
     hv = _f16_array(q.vnorm)
     V = (hv / math.sqrt(d_h))[:, None] * (Cv[q.vidx] @ Piv)
     return K, V
@@ -486,3 +486,39 @@ def prefill_attention_head(q_post: np.ndarray, qh: QuantizedHead, tab: Tables, d
         for a in range(G):
             out[i, a] = attention(q_post[i, a], K[:T], V[:T], scale)
     return out
+
+
+# ----------------------------------------------------------------------------- RoPE-logit MAE (App. B.3)
+def rope_logit_mae(q_pre: np.ndarray, k_pre: np.ndarray, bits: np.ndarray, tab: Tables, base: float,
+                   offsets: np.ndarray | None = None, pairing: int = PAIR_HALF) -> float:
+    """MAE = E_h E_{g in G(h)} E_(q,k) E_{Delta in D} | q^T R_Delta k - q^T R_Delta khat |, K-only: khat is the TQ-MSE /
+    Block-GTQ reconstruction of the PRE-RoPE key under the allocation bits[h] (uniform TQ-MSE = all blocks at one width,
+    PAPER.md:108), the analytic rotation R_Delta is applied identically to k and khat, D = 50 evenly spaced offsets in
+    [-1024, 1024].  q_pre [N, Hq, d], k_pre [N, Hkv, d] are paired sample by sample; bits [Hkv, d/2]."""
+    q_pre, k_pre = np.asarray(q_pre, np.float64), np.asarray(k_pre, np.float64)
+    N, Hq, d = q_pre.shape
+    Hkv = k_pre.shape[1]
+    G = Hq // Hkv
+    if offsets is None:
+        offsets = np.linspace(-1024.0, 1024.0, 50)
+    a, b = pair_indices(d, pairing)
+    theta = np.array([base ** (-2.0 * i / d) for i in range(d // 2)])
+    total, count = 0.0, 0
+    for h in range(Hkv):
+        groups = groups_from_bits(bits[h], d, pairing)
+        khat = np.zeros((N, d))
+        for t in range(N):
+            for g in groups:
+                idx, hb, _ = quantize_group(k_pre[t, h, g.coords], g.width, tab)
+                khat[t, g.coords] = dequantize_group(idx, hb, g.width, tab)
+        e = k_pre[:, h] - khat                                      # [N, d]
+        ea, eb = e[:, a], e[:, b]                                  # block members
+        for gq in range(h * G, (h + 1) * G):
+            qa, qb = q_pre[:, gq][:, a], q_pre[:, gq][:, b]
+            # q^(i)T R(phi) e^(i) = cos(phi) (qa ea + qb eb) + sin(phi) (qb ea - qa eb),  phi = Delta * theta_i
+            dot, cross = qa * ea + qb * eb, qb * ea - qa * eb     # [N, L]
+            for D in offsets:
+                phi = D * theta
+                total += float(np.sum(np.abs(dot @ np.cos(phi) + cross @ np.sin(phi))))
+                count += N
+    return total / count

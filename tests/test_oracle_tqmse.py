@@ -161,3 +161,58 @@ def test_f16_converters_match_ieee_binary16():
     for x, bits in [(65504.0, 0x7BFF), (65519.999, 0x7BFF), (65520.0, 0x7BFF), (1e9, 0x7BFF), (-65520.0, 0xFBFF),
                     (2.0 ** -25, 0x0000), (np.nextafter(2.0 ** -25, 1.0), 0x0001), (2.0 ** -24, 0x0001), (0.0, 0), (-0.0, 0x8000)]:
         assert L.orc_f64_to_f16_bits(float(x)) == bits, x
+
+
+@pytest.mark.parametrize("m", [2, 4, 10, 26])
+def test_rate_law_small_groups_exact_density(m, rot128):
+    """PAPER.md:49 at the group sizes the allocator really produces: with the exact-density codebooks the relative error
+    of TQ-MSE on m-vectors equals the table's distortion D(b, m) (the norm is restored exactly up to fp16) and obeys
+    C_TQ 4^-b; with the shared Gaussian table it is larger."""
+    tabs = O.Tables(rot128, 128, cb_kind="sphere")
+    tabg = O.Tables(rot128, 128)
+    rng = np.random.default_rng(m)
+    x = (rng.standard_normal((3000, m)) * 2.0).astype(np.float32).astype(np.float64)
+    for b in (2, 3, 4):
+        es = eg = 0.0
+        for row in x:
+            i1, h1, _ = O.quantize_group(row, b, tabs)
+            i2, h2, _ = O.quantize_group(row, b, tabg)
+            es += np.sum((row - O.dequantize_group(i1, h1, b, tabs)) ** 2) / np.sum(row * row)
+            eg += np.sum((row - O.dequantize_group(i2, h2, b, tabg)) ** 2) / np.sum(row * row)
+        es /= len(x); eg /= len(x)
+        D = cb.sphere_distortion(cb.sphere_codebook(b, m), m)
+        assert es == pytest.approx(D, rel=0.08), (m, b)
+        assert es <= C_TQ * 4.0 ** (-b)
+        assert es < eg
+
+
+def test_rope_logit_mae_echo_of_table_1():
+    """PAPER.md:532 (50 offsets in [-1024, 1024], K-only): on synthetic heads with log-uniform block energies Block-GTQ's
+    allocation beats uniform TQ-MSE at the same budget (the direction of Tables 1 and 11), with either codebook family,
+    and the exact-density codebooks do not hurt."""
+    import workloads as W
+    d, Hq, Hkv, base = 128, 4, 2, 1.0e6
+    rot = W.rotations(20260624, d)
+    tg, ts = O.Tables(rot, d), O.Tables(rot, d, cb_kind="sphere")
+    scales = W.block_scales(5, Hkv, d // 2)
+    s, _, _ = O.block_energy(W.pre_rope_gaussian(5, 4, 256, Hq, d, scales), W.pre_rope_gaussian(5, 1, 256, Hkv, d, scales))
+    q, k = W.pre_rope_gaussian(5, 5, 48, Hq, d, scales), W.pre_rope_gaussian(5, 6, 48, Hkv, d, scales)
+    for bbar in (2, 3):
+        greedy = np.stack([O.allocate(s[h], bbar * 64, 1, 8) for h in range(Hkv)])
+        uniform = np.full_like(greedy, bbar)
+        mu, mg = O.rope_logit_mae(q, k, uniform, tg, base), O.rope_logit_mae(q, k, greedy, tg, base)
+        ms = O.rope_logit_mae(q, k, greedy, ts, base)
+        assert mg < 0.75 * mu
+        assert ms < 1.02 * mg
+    # the definition itself: Delta = 0 only, one block stored -> |q^(i) . e^(i)| averaged
+    one = np.zeros((Hkv, 64), dtype=np.int64); one[:, 0] = 8
+    m0 = O.rope_logit_mae(q, k, one, tg, base, offsets=np.array([0.0]))
+    want = 0.0
+    for h in range(Hkv):
+        g = O.groups_from_bits(one[h], d)[0]
+        for t in range(len(q)):
+            idx, hb, _ = O.quantize_group(k[t, h, g.coords], 8, tg)
+            e = k[t, h].copy(); e[g.coords] -= O.dequantize_group(idx, hb, 8, tg)
+            for a in range(h * 2, h * 2 + 2):
+                want += abs(float(q[t, a] @ e))
+    assert m0 == pytest.approx(want / (len(q) * Hq), rel=1e-12)
