@@ -100,6 +100,14 @@ int bgtq_layout_create(const uint8_t *bits, int n_layers, int n_kv_heads, int n_
  *                   words (same bytes as V1 when every group holds a multiple of 32 coordinates).
  * Every call below works on either format unless stated otherwise; the cache bytes of the two formats differ. */
 typedef enum { BGTQ_FORMAT_V1 = 1, BGTQ_FORMAT_V2 = 2 } bgtq_format;
+/* OR-ed into `format`: exact-density TQ-MSE codebooks (reading Q7b in DESIGN.md).  PAPER.md:49 scalar-
+ * quantises the rotated coordinates of a NORMALISED vector; a coordinate of sqrt(m) x (uniform unit vector of R^m) has the
+ * density ~ (1 - x^2/m)^((m-3)/2), not N(0,1).  With this flag the group of m coordinates at width b uses C_{b,m}, the
+ * Lloyd-Max quantiser of that density (fp16-rounded; bgtq_codebook_exact), V uses C_{b_V, d_h}; without it every group
+ * shares C_b = bgtq_codebook(b) (Q7).  Supported by BGTQ_FORMAT_V1: append (all variants), decode attention (contiguous
+ * and protected); prefill, the paged decode and BGTQ_FORMAT_V2 return BGTQ_EINVAL. */
+#define BGTQ_CODEBOOK_EXACT 0x100
+int bgtq_codebook_exact(int b, int m, float *levels);
 int bgtq_layout_create_format(const uint8_t *bits, int n_layers, int n_kv_heads, int n_q_heads, int d_h,
                               int b_v, int pairing, const float *rotations, int format, bgtq_layout **out);
 int bgtq_layout_format(const bgtq_layout *layout);

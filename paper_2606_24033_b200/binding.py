@@ -32,9 +32,10 @@ SYMBOLS = [
     "bgtq_paged_cache_bytes", "bgtq_paged_pool_offset", "bgtq_quantize_append_paged", "bgtq_decode_attention_paged",
     "bgtq_quantize_append_rope",
     "bgtq_window_bytes", "bgtq_window_append", "bgtq_decode_attention_protected",
-    "bgtq_layout_create_format", "bgtq_layout_format",
+    "bgtq_layout_create_format", "bgtq_layout_format", "bgtq_codebook_exact",
 ]
 FORMAT_V1, FORMAT_V2 = 1, 2
+CODEBOOK_EXACT = 0x100
 
 
 class BgtqError(RuntimeError):
@@ -66,6 +67,8 @@ def _load() -> C.CDLL:
     lib.bgtq_layout_create.argtypes = [vp, i32, i32, i32, i32, i32, i32, vp, C.POINTER(vp)]
     lib.bgtq_layout_create_format.restype = i32
     lib.bgtq_layout_create_format.argtypes = [vp, i32, i32, i32, i32, i32, i32, vp, i32, C.POINTER(vp)]
+    lib.bgtq_codebook_exact.restype = i32
+    lib.bgtq_codebook_exact.argtypes = [i32, i32, vp]
     lib.bgtq_layout_format.restype = i32
     lib.bgtq_layout_format.argtypes = [vp]
     lib.bgtq_layout_destroy.restype = None
@@ -166,6 +169,13 @@ def codebook(b: int) -> np.ndarray:
     return out
 
 
+def codebook_exact(b: int, m: int) -> np.ndarray:
+    """bgtq_codebook_exact: the 2^b fp16-representable levels of C_{b,m} (exact-density codebook, float32)."""
+    out = np.zeros(1 << b, dtype=np.float32)
+    _check(_lib.bgtq_codebook_exact(b, m, out.ctypes.data))
+    return out
+
+
 def block_energy(q: torch.Tensor, k: torch.Tensor, pairing: int = PAIR_HALF, kind: int = QK_AVG,
                  return_parts: bool = False):
     """bgtq_block_energy.  q [N_q, H_q, d_h], k [N_k, H_kv, d_h] (CUDA, same dtype) ->
@@ -205,7 +215,7 @@ class Layout:
     """bgtq_layout: static metadata of the packed cache for an allocation bits[n_layers, H_kv, L]."""
 
     def __init__(self, bits: np.ndarray, n_q_heads: int, d_h: int, b_v: int, rotations: np.ndarray,
-                 pairing: int = PAIR_HALF, fmt: int = FORMAT_V1):
+                 pairing: int = PAIR_HALF, fmt: int = FORMAT_V1, exact_codebooks: bool = False):
         bits = np.ascontiguousarray(bits, dtype=np.uint8)
         assert bits.ndim == 3
         self.n_layers, self.n_kv_heads, _ = bits.shape
@@ -213,9 +223,11 @@ class Layout:
         rot = np.ascontiguousarray(rotations, dtype=np.float32)
         h = C.c_void_p()
         _check(_lib.bgtq_layout_create_format(bits.ctypes.data, self.n_layers, self.n_kv_heads, n_q_heads, d_h, b_v,
-                                              pairing, rot.ctypes.data, fmt, C.byref(h)))
+                                              pairing, rot.ctypes.data, fmt | (CODEBOOK_EXACT if exact_codebooks else 0),
+                                              C.byref(h)))
         self._h = h
-        self.fmt = int(_lib.bgtq_layout_format(h))
+        self.fmt = int(_lib.bgtq_layout_format(h)) & 0xFF
+        self.exact_codebooks = bool(int(_lib.bgtq_layout_format(h)) & CODEBOOK_EXACT)
 
     def __del__(self):
         h = getattr(self, "_h", None)

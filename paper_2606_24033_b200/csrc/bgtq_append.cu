@@ -90,7 +90,7 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
                        const double *__restrict__ cb64, const float *__restrict__ rot_t, int batch,
                        int n_new, int Hkv, const int32_t *__restrict__ seq_len, int64_t n_cap,
                        int64_t max_tokens, const int32_t *__restrict__ pages, int pstride, int64_t n_pages,
-                       const float *__restrict__ rope_cos, const float *__restrict__ rope_sin, int pairing)
+                       const float *__restrict__ rope_cos, const float *__restrict__ rope_sin, int pairing, int cb_exact)
 {
     extern __shared__ __align__(16) unsigned char smem[];
     const int tid = threadIdx.x;
@@ -111,7 +111,9 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
     UnitDesc *units = reinterpret_cast<UnitDesc *>(idxs + kSub * 256);   // [32]
     int *n_units_p = reinterpret_cast<int *>(units + kMaxUnits);
     HeadMeta *Msp = reinterpret_cast<HeadMeta *>(n_units_p + 4);         // this head's static metadata (kMetaBytes)
-    uint32_t *tbuf = reinterpret_cast<uint32_t *>(reinterpret_cast<unsigned char *>(Msp) + kMetaBytes);   // tile, `stride` bytes
+    // exact-density codebooks: V has its own table C_{b_V, d_h} (256 more thresholds); else V shares the flat table
+    double *tauV_own = reinterpret_cast<double *>(reinterpret_cast<unsigned char *>(Msp) + kMetaBytes);
+    uint32_t *tbuf = reinterpret_cast<uint32_t *>(reinterpret_cast<unsigned char *>(Msp) + kMetaBytes + (cb_exact ? 256 * 8 : 0));   // tile, `stride` bytes
     // The metadata is read many times by single threads (unit list, group search, radii); one coalesced copy into
     // shared memory replaces those dependent global-memory round trips -- they dominated the one-token append.
     {
@@ -133,10 +135,16 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
             dst[i] = has_old ? src[i] : make_uint4(0, 0, 0, 0);
     }
     // thresholds tau_k = (C[k] + C[k+1]) / 2 (exact in fp64); stored at the level's flat index
+    const double *cbK = cb64 + (cb_exact ? (size_t)blockIdx.y * 1024 : 0);     // this head's tables (exact: [K 512 | V 512])
     for (int i = tid; i < 511; i += kAppendThreads) {
-        double c0 = cb64[i], c1 = cb64[i + 1 < 511 ? i + 1 : i];
+        double c0 = cbK[i], c1 = cbK[i + 1 < 511 ? i + 1 : i];
         tau[i] = __dmul_rn(__dadd_rn(c0, c1), 0.5);
     }
+    if (cb_exact) {
+        const double *cbV = cbK + 512 + ((1 << b_v) - 1);
+        for (int i = tid; i + 1 < (1 << b_v); i += kAppendThreads) tauV_own[i] = __dmul_rn(__dadd_rn(cbV[i], cbV[i + 1]), 0.5);
+    }
+    const double *tauV = cb_exact ? tauV_own : tau + ((1 << b_v) - 1);
     if (tid == 0) {  // list of half-step units of the K code section
         int n = 0, j = 0;
         for (int ks = 0; ks < (M.format == 2 ? 0 : M.n_ksteps); ++ks) {   // (BGTQ-v2 packs from M.chunks, step 5)
@@ -299,7 +307,7 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
         __syncthreads();
         // ---- 4. scalar quantise: idx = #{k : z > tau_k * sigma}; the predicate is monotone in k
         if (my_m > 0) {
-            const double *tb = tau + ((1 << my_b) - 1);
+            const double *tb = col >= 128 ? tauV : tau + ((1 << my_b) - 1);
             // the count is found bit by bit (always my_b probes), all kSub searches side by side so that the
             // dependent LDS -> DMUL -> DSETP chains of different tokens overlap; same count as any other search
             // because the predicate is monotone in k
@@ -422,10 +430,10 @@ __global__ void advance_seq_len_kernel(int32_t *seq_len, int batch, int n_new, i
     }
 }
 
-static size_t append_smem_bytes(int max_stride)
+static size_t append_smem_bytes(int max_stride, bool cb_exact = false)
 {
     return (size_t)kSub * 256 * 8 + 512 * 8 + kSub * 9 * 8 + (kSub * 9 + 8) * 2 + kSub * 256 +
-           kMaxUnits * sizeof(UnitDesc) + 16 + kMetaBytes + (size_t)max_stride + 64;
+           kMaxUnits * sizeof(UnitDesc) + 16 + kMetaBytes + (cb_exact ? 256 * 8 : 0) + (size_t)max_stride + 64;
 }
 
 int launch_quantize_append(const bgtq_layout *lay, int layer, int n_layers, void *cache, const void *k_new,
@@ -433,11 +441,11 @@ int launch_quantize_append(const bgtq_layout *lay, int layer, int n_layers, void
                            int advance, int64_t max_tokens, const PageMap *pm, const RopeTab *rope, cudaStream_t st)
 {
     const int64_t n_cap = (max_tokens + kTile - 1) / kTile;
-    const size_t smem = append_smem_bytes(lay->max_stride);
+    const size_t smem = append_smem_bytes(lay->max_stride, lay->cb_exact != 0);
     dim3 grid((n_new + kTile - 1) / kTile + 1, lay->n_kv_heads * n_layers, batch);
     const HeadMeta *metas = lay->d_meta + (size_t)layer * lay->n_kv_heads;
     if (first_use_on_device(1)) {   // once per device, outside any stream capture
-        const int maxs = (int)append_smem_bytes(16 * kDh * 8 + 256 * 9 + 16 * kDh * 8);
+        const int maxs = (int)append_smem_bytes(16 * kDh * 8 + 256 * 9 + 16 * kDh * 8, true);
 #define BGTQ_APPEND_ATTR(T, R, G) CUDA_TRY(cudaFuncSetAttribute(quantize_append_kernel<T, R, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, maxs))
         BGTQ_APPEND_ATTR(float, false, false); BGTQ_APPEND_ATTR(__nv_bfloat16, false, false);
         BGTQ_APPEND_ATTR(float, true, false);  BGTQ_APPEND_ATTR(__nv_bfloat16, true, false);
@@ -452,9 +460,10 @@ int launch_quantize_append(const bgtq_layout *lay, int layer, int n_layers, void
     if (pm && rope) { set_error("bgtq_quantize_append: paged + fused RoPE is not built"); return BGTQ_EINVAL; }
     auto launch = [&](auto plain, auto roped, auto paged, auto *kp, auto *vp) {
         auto kern = pm ? paged : (rope ? roped : plain);
-        kern<<<grid, kAppendThreads, smem, st>>>(metas, (uint8_t *)cache, kp, vp, lay->d_cb64, lay->d_rot_t, batch, n_new,
+        const double *cb = lay->cb_exact ? lay->d_hcb64 + (size_t)layer * lay->n_kv_heads * 1024 : lay->d_cb64;
+        kern<<<grid, kAppendThreads, smem, st>>>(metas, (uint8_t *)cache, kp, vp, cb, lay->d_rot_t, batch, n_new,
                                                  lay->n_kv_heads, seq_len, n_cap, max_tokens, pt, pstride, n_pages, rc, rs,
-                                                 lay->pairing);
+                                                 lay->pairing, lay->cb_exact);
     };
     if (dt == BGTQ_F32)
         launch(quantize_append_kernel<float, false, false>, quantize_append_kernel<float, true, false>,

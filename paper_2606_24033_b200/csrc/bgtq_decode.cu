@@ -241,6 +241,7 @@ struct DecodeParams {
     const __half *qf;           // q' fragments, [pair][kQfHalves]
     const int32_t *seq_len;
     const uint16_t *cb16;
+    const uint16_t *hcb16;      // exact-density codebooks: [head of the call][2][kHeadLutHalves] (K, V), else nullptr
     float *partials;            // [n_warps + n_pairs][8][130]
     int64_t n_cap;              // tiles of capacity per sequence
     int n_layers, batch, Hkv, G;
@@ -389,14 +390,14 @@ __device__ __forceinline__ void pv_tile(const uint32_t *vcodes, int lane, const 
     }
 }
 
-template <int W, bool PAGED>
+template <int W, bool PAGED, bool EXACT>
 __global__ void __launch_bounds__(W * 32, 1)
 decode_kernel(const DecodeParams P)
 {
     extern __shared__ __align__(128) unsigned char smem[];       // the per-warp tile buffers only
     constexpr bool P5 = !BGTQ_NO_P5;
     __shared__ __align__(16) uint16_t lut[P5 ? kLutHalves : 512]; // static: constant LDS addresses for the LUTs
-    __shared__ uint32_t pools[16];
+    __shared__ uint32_t pools_s[W][2][12];                        // PRMT byte planes per warp: [0] K tables, [1] V table
     __shared__ int pre[kMaxBatch + 1];
     __shared__ __align__(8) uint64_t bars[2 * W];
 
@@ -414,7 +415,8 @@ decode_kernel(const DecodeParams P)
     build_lut(P.cb16, lut, tid, W * 32, P5);
     if (tid == 0) build_prefix(P.seq_len, P.batch, P.n_cap * kTile, pre, P.n_sink, P.n_recent);
     __syncthreads();
-    if (tid == 0) build_pools(lut, pools);
+    if (lane < 2 && !EXACT) build_pools(lut, pools_s[warp][lane]);   // shared codebooks: the same planes for every head
+    const uint32_t *pools = pools_s[warp][0], *poolsV = pools_s[warp][1];
     const uint32_t kbar = smem_u32(&bars[2 * warp]), vbar = smem_u32(&bars[2 * warp + 1]);
     if (lane == 0) {
         mbar_init(kbar, 1);
@@ -482,6 +484,16 @@ decode_kernel(const DecodeParams P)
         const int seg_end = min(x_end, tp.pair_start + tp.tiles_b);
         const int n_groups = M.n_groups, b_v = M.b_v;
         const int knorm_off = M.knorm_off, vnorm_off = M.vnorm_off, vcode_off = M.vcode_off;
+        // codebook tables of this head: shared Gaussian tables in shared memory, or the head's exact-density tables
+        // (global memory, L1-resident: 10 KB per head) with the byte planes rebuilt per segment
+        const uint16_t *lutK = lut, *lutV = lut;
+        if (EXACT) {
+            lutK = P.hcb16 + (size_t)(tp.l * P.Hkv + tp.h) * 2 * kHeadLutHalves;
+            lutV = lutK + kHeadLutHalves;
+            __syncwarp();
+            if (lane < 2) build_pools(lane ? lutV : lutK, pools_s[warp][lane]);
+            __syncwarp();
+        }
         int64_t slen = P.seq_len[tp.b];
         slen = slen > P.n_cap * kTile ? P.n_cap * kTile : slen;
         slen = packed_len(slen, P.n_sink, P.n_recent);
@@ -532,27 +544,27 @@ decode_kernel(const DecodeParams P)
                     nn[i][1] = prmt(xs, xs, 0x3232);
                 }
                 switch ((d >> 24) & 0xF) {
-                case 1: qk_group_n<1, P5>(gcodes, m, lane, qg, pools, lut, nn, Sc); break;
-                case 2: qk_group_n<2, P5>(gcodes, m, lane, qg, pools, lut, nn, Sc); break;
-                case 3: qk_group_n<3, P5>(gcodes, m, lane, qg, pools, lut, nn, Sc); break;
-                case 4: qk_group_n<4, P5>(gcodes, m, lane, qg, pools, lut, nn, Sc); break;
-                case 5: qk_group_n<5, P5>(gcodes, m, lane, qg, pools, lut, nn, Sc); break;
-                case 6: qk_group_n<6, P5>(gcodes, m, lane, qg, pools, lut, nn, Sc); break;
-                case 7: qk_group_n<7, P5>(gcodes, m, lane, qg, pools, lut, nn, Sc); break;
-                default: qk_group_n<8, P5>(gcodes, m, lane, qg, pools, lut, nn, Sc); break;
+                case 1: qk_group_n<1, P5>(gcodes, m, lane, qg, pools, lutK, nn, Sc); break;
+                case 2: qk_group_n<2, P5>(gcodes, m, lane, qg, pools, lutK, nn, Sc); break;
+                case 3: qk_group_n<3, P5>(gcodes, m, lane, qg, pools, lutK, nn, Sc); break;
+                case 4: qk_group_n<4, P5>(gcodes, m, lane, qg, pools, lutK, nn, Sc); break;
+                case 5: qk_group_n<5, P5>(gcodes, m, lane, qg, pools, lutK, nn, Sc); break;
+                case 6: qk_group_n<6, P5>(gcodes, m, lane, qg, pools, lutK, nn, Sc); break;
+                case 7: qk_group_n<7, P5>(gcodes, m, lane, qg, pools, lutK, nn, Sc); break;
+                default: qk_group_n<8, P5>(gcodes, m, lane, qg, pools, lutK, nn, Sc); break;
                 }
             }
 #else
                 float A[8][4];                               // started by the group's first k-step (m >= 2)
                 switch ((d >> 24) & 0xF) {
-                case 1: qk_group<1, P5>(gcodes, m, lane, qg, pools, lut, A); break;
-                case 2: qk_group<2, P5>(gcodes, m, lane, qg, pools, lut, A); break;
-                case 3: qk_group<3, P5>(gcodes, m, lane, qg, pools, lut, A); break;
-                case 4: qk_group<4, P5>(gcodes, m, lane, qg, pools, lut, A); break;
-                case 5: qk_group<5, P5>(gcodes, m, lane, qg, pools, lut, A); break;
-                case 6: qk_group<6, P5>(gcodes, m, lane, qg, pools, lut, A); break;
-                case 7: qk_group<7, P5>(gcodes, m, lane, qg, pools, lut, A); break;
-                default: qk_group<8, P5>(gcodes, m, lane, qg, pools, lut, A); break;
+                case 1: qk_group<1, P5>(gcodes, m, lane, qg, pools, lutK, A); break;
+                case 2: qk_group<2, P5>(gcodes, m, lane, qg, pools, lutK, A); break;
+                case 3: qk_group<3, P5>(gcodes, m, lane, qg, pools, lutK, A); break;
+                case 4: qk_group<4, P5>(gcodes, m, lane, qg, pools, lutK, A); break;
+                case 5: qk_group<5, P5>(gcodes, m, lane, qg, pools, lutK, A); break;
+                case 6: qk_group<6, P5>(gcodes, m, lane, qg, pools, lutK, A); break;
+                case 7: qk_group<7, P5>(gcodes, m, lane, qg, pools, lutK, A); break;
+                default: qk_group<8, P5>(gcodes, m, lane, qg, pools, lutK, A); break;
                 }
                 // scale by the fp16 group norms (fp32, on the accumulators)
                 const uint4 *np = reinterpret_cast<const uint4 *>(tile + ((knorm_off + 256 * g + g8 * 32) >> 2));
@@ -631,14 +643,14 @@ decode_kernel(const DecodeParams P)
             }
             const uint32_t *vcodes = tile + (vcode_off >> 2);
             switch (b_v) {
-            case 1: pv_tile<1, P5>(vcodes, lane, bP, pools, lut, O); break;
-            case 2: pv_tile<2, P5>(vcodes, lane, bP, pools, lut, O); break;
-            case 3: pv_tile<3, P5>(vcodes, lane, bP, pools, lut, O); break;
-            case 4: pv_tile<4, P5>(vcodes, lane, bP, pools, lut, O); break;
-            case 5: pv_tile<5, P5>(vcodes, lane, bP, pools, lut, O); break;
-            case 6: pv_tile<6, P5>(vcodes, lane, bP, pools, lut, O); break;
-            case 7: pv_tile<7, P5>(vcodes, lane, bP, pools, lut, O); break;
-            default: pv_tile<8, P5>(vcodes, lane, bP, pools, lut, O); break;
+            case 1: pv_tile<1, P5>(vcodes, lane, bP, poolsV, lutV, O); break;
+            case 2: pv_tile<2, P5>(vcodes, lane, bP, poolsV, lutV, O); break;
+            case 3: pv_tile<3, P5>(vcodes, lane, bP, poolsV, lutV, O); break;
+            case 4: pv_tile<4, P5>(vcodes, lane, bP, poolsV, lutV, O); break;
+            case 5: pv_tile<5, P5>(vcodes, lane, bP, poolsV, lutV, O); break;
+            case 6: pv_tile<6, P5>(vcodes, lane, bP, poolsV, lutV, O); break;
+            case 7: pv_tile<7, P5>(vcodes, lane, bP, poolsV, lutV, O); break;
+            default: pv_tile<8, P5>(vcodes, lane, bP, poolsV, lutV, O); break;
             }
             __syncwarp();
             TS(7);
@@ -1259,11 +1271,11 @@ int launch_window(const void *win_k, const void *win_v, const void *q, const int
     return BGTQ_OK;
 }
 
-template <int W, bool PAGED>
+template <int W, bool PAGED, bool EXACT = false>
 static int launch_decode_w(const DecodeParams &P, int grid, size_t smem, cudaStream_t st)
 {
-    if (first_use_on_device(8 + (W / 4) * 2 + (PAGED ? 1 : 0)))   // once per device, outside any stream capture
-        CUDA_TRY(cudaFuncSetAttribute(decode_kernel<W, PAGED>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - kStaticSmem));
+    if (first_use_on_device(8 + (W / 4) * 3 + (PAGED ? 1 : 0) + (EXACT ? 2 : 0)))   // once per device, outside any stream capture
+        CUDA_TRY(cudaFuncSetAttribute(decode_kernel<W, PAGED, EXACT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - kStaticSmem));
     if (int rc = profile_decode_begin(st)) return rc;
     {
         cudaLaunchConfig_t cfg = {};
@@ -1272,13 +1284,13 @@ static int launch_decode_w(const DecodeParams &P, int grid, size_t smem, cudaStr
         at[0].val.programmaticStreamSerializationAllowed = g_prof ? 0 : 1;
         cfg.gridDim = dim3(grid); cfg.blockDim = dim3(W * 32); cfg.dynamicSmemBytes = smem; cfg.stream = st;
         cfg.attrs = at; cfg.numAttrs = 1;
-        cudaLaunchKernelEx(&cfg, decode_kernel<W, PAGED>, P);
+        cudaLaunchKernelEx(&cfg, decode_kernel<W, PAGED, EXACT>, P);
     }
     {
         cudaError_t le = cudaPeekAtLastError();
         if (le != cudaSuccess) {
             cudaFuncAttributes fa;
-            cudaFuncGetAttributes(&fa, decode_kernel<W, PAGED>);
+            cudaFuncGetAttributes(&fa, decode_kernel<W, PAGED, EXACT>);
             set_error(std::string("decode launch: ") + cudaGetErrorString(le) + " regs=" + std::to_string(fa.numRegs) + " maxthr=" + std::to_string(fa.maxThreadsPerBlock) + " static=" + std::to_string(fa.sharedSizeBytes) + " dyn=" + std::to_string(smem) + " maxdyn=" + std::to_string(fa.maxDynamicSharedSizeBytes));
             cudaGetLastError();
             return BGTQ_ECUDA;
@@ -1331,6 +1343,7 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
     if (!W) { set_error("bgtq_decode_attention: tile does not fit shared memory"); return BGTQ_EINVAL; }
     DecodeParams P;
     P.metas = metas; P.cache = (const uint8_t *)cache; P.qf = qf; P.seq_len = seq_len; P.cb16 = lay->d_cb16;
+    P.hcb16 = lay->cb_exact ? lay->d_hcb16 + (size_t)layer0 * Hkv * 2 * kHeadLutHalves : nullptr;
     P.partials = partials; P.n_cap = n_cap; P.n_layers = n_layers; P.batch = batch; P.Hkv = Hkv; P.G = G;
     P.buf_bytes = buf_bytes;
     P.pages = pm ? pm->table : nullptr; P.pstride = pm ? pm->table_stride : 0; P.n_pages = pm ? pm->n_pages : 0;
@@ -1338,7 +1351,14 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
     const int grid = lay->sm_count;
     const size_t smem = decode_smem(W, buf_bytes);
     int rc;
-    if (pm) {
+    if (lay->cb_exact) {
+        if (pm) { set_error("bgtq_decode_attention_paged: not built for exact-density codebooks"); return BGTQ_EINVAL; }
+        switch (W) {
+        case 12: rc = launch_decode_w<12, false, true>(P, grid, smem, st); break;
+        case 8: rc = launch_decode_w<8, false, true>(P, grid, smem, st); break;
+        default: rc = launch_decode_w<4, false, true>(P, grid, smem, st); break;
+        }
+    } else if (pm) {
         switch (W) {
         case 12: rc = launch_decode_w<12, true>(P, grid, smem, st); break;
         case 8: rc = launch_decode_w<8, true>(P, grid, smem, st); break;

@@ -238,14 +238,27 @@ extern "C" int bgtq_layout_create(const uint8_t *bits, int n_layers, int n_kv_he
                                      BGTQ_FORMAT_V1, out);
 }
 
-extern "C" int bgtq_layout_format(const bgtq_layout *lay) { return lay ? lay->format : 0; }
+extern "C" int bgtq_layout_format(const bgtq_layout *lay) { return lay ? (lay->format | (lay->cb_exact ? BGTQ_CODEBOOK_EXACT : 0)) : 0; }
+
+extern "C" int bgtq_codebook_exact(int b, int m, float *levels)
+{
+    if (b < 0 || b > BGTQ_MAX_WIDTH || m < 2 || m > 1024 || (m & 1) || !levels)
+        FAIL(BGTQ_EINVAL, "bgtq_codebook_exact: b in 0..8, m even in 2..1024, levels != NULL");
+    double tmp[256];
+    codebook_levels_sphere(b, m, tmp);
+    for (int k = 0; k < (1 << b); ++k) levels[k] = (float)tmp[k];
+    return BGTQ_OK;
+}
 
 extern "C" int bgtq_layout_create_format(const uint8_t *bits, int n_layers, int n_kv_heads, int n_q_heads,
                                          int d_h, int b_v, int pairing, const float *rotations, int format,
                                          bgtq_layout **out)
 {
     if (!bits || !rotations || !out) FAIL(BGTQ_EINVAL, "bgtq_layout_create: null pointer");
+    const int cb_exact = (format & BGTQ_CODEBOOK_EXACT) ? 1 : 0;
+    format &= ~BGTQ_CODEBOOK_EXACT;
     if (format != BGTQ_FORMAT_V1 && format != BGTQ_FORMAT_V2) FAIL(BGTQ_EINVAL, "bgtq_layout_create: format must be BGTQ_FORMAT_V1 or BGTQ_FORMAT_V2");
+    if (cb_exact && format != BGTQ_FORMAT_V1) FAIL(BGTQ_EINVAL, "bgtq_layout_create: BGTQ_CODEBOOK_EXACT is built for BGTQ_FORMAT_V1 layouts");
     if (d_h != kDh) FAIL(BGTQ_EINVAL, "bgtq_layout_create: d_h must be 128");
     if (n_layers <= 0 || n_kv_heads <= 0 || n_q_heads <= 0 || n_q_heads % n_kv_heads)
         FAIL(BGTQ_EINVAL, "bgtq_layout_create: bad layer/head counts");
@@ -261,6 +274,7 @@ extern "C" int bgtq_layout_create_format(const uint8_t *bits, int n_layers, int 
     lay->n_layers = n_layers; lay->n_kv_heads = n_kv_heads; lay->n_q_heads = n_q_heads;
     lay->d_h = d_h; lay->b_v = b_v; lay->pairing = pairing;
     lay->format = format; lay->d_planes = nullptr;
+    lay->cb_exact = cb_exact; lay->d_hcb16 = nullptr; lay->d_hcb64 = nullptr;
     lay->d_meta = nullptr; lay->d_rot = nullptr; lay->d_rot_t = nullptr; lay->d_cb16 = nullptr; lay->d_cb64 = nullptr;
     lay->meta.resize((size_t)n_layers * n_kv_heads);
     int64_t prefix = 0;
@@ -306,6 +320,41 @@ extern "C" int bgtq_layout_create_format(const uint8_t *bits, int n_layers, int 
             cb16[(1 << b) - 1 + k] = u;
         }
     }
+    // exact-density tables per (layer, kv head): flat by width like the shared table; widths without a group keep the
+    // Gaussian levels (never used)
+    std::vector<uint16_t> hcb16;
+    std::vector<double> hcb64;
+    if (cb_exact) {
+        const size_t nh = lay->meta.size();
+        hcb16.assign(nh * 2 * kHeadLutHalves, 0);
+        hcb64.assign(nh * 2 * 512, 0.0);
+        std::vector<std::vector<double>> cache_lv(9 * 65);         // (b, m/2) -> levels, solved once
+        auto levels_of = [&](int b, int m) -> const std::vector<double> & {
+            std::vector<double> &v = cache_lv[(size_t)b * 65 + m / 2];
+            if (v.empty()) { v.resize(1 << b); codebook_levels_sphere(b, m, v.data()); }
+            return v;
+        };
+        for (size_t hi = 0; hi < nh; ++hi) {
+            const HeadMeta &m = lay->meta[hi];
+            for (int side = 0; side < 2; ++side) {
+                uint16_t *t16 = hcb16.data() + (hi * 2 + side) * kHeadLutHalves;
+                double *t64 = hcb64.data() + (hi * 2 + side) * 512;
+                for (int i = 0; i < 512; ++i) { t16[i] = cb16[i < 511 ? i : 510]; t64[i] = cb64[i < 511 ? i : 510]; }
+                auto put = [&](int b, int mm) {
+                    const std::vector<double> &lv = levels_of(b, mm);
+                    for (int k = 0; k < (1 << b); ++k) {
+                        t64[(1 << b) - 1 + k] = lv[k];
+                        __half hv = __double2half(lv[k]);
+                        std::memcpy(&t16[(1 << b) - 1 + k], &hv, 2);
+                    }
+                };
+                if (side == 0) for (int g = 0; g < m.n_groups; ++g) put(m.gb[g], m.gm[g]);
+                else put(b_v, d_h);
+                uint32_t *pair = reinterpret_cast<uint32_t *>(t16 + 512);     // two adjacent 5-bit codes -> fp16x2
+                for (int i = 0; i < 1024; ++i) pair[i] = (uint32_t)t16[31 + (i & 31)] | ((uint32_t)t16[31 + (i >> 5)] << 16);
+            }
+        }
+    }
     std::vector<uint8_t> planes(kPlaneBytes, 0);
     lay->kappa[0] = 1.f;
     for (int b = 1; b <= BGTQ_MAX_WIDTH; ++b)
@@ -319,6 +368,10 @@ extern "C" int bgtq_layout_create_format(const uint8_t *bits, int n_layers, int 
     if (e == cudaSuccess) e = cudaMalloc(&lay->d_rot_t, rot_n * sizeof(float));
     if (e == cudaSuccess) e = cudaMalloc(&lay->d_cb16, 512 * sizeof(uint16_t));
     if (e == cudaSuccess) e = cudaMalloc(&lay->d_cb64, 512 * sizeof(double));
+    if (e == cudaSuccess && cb_exact) e = cudaMalloc(&lay->d_hcb16, hcb16.size() * sizeof(uint16_t));
+    if (e == cudaSuccess && cb_exact) e = cudaMalloc(&lay->d_hcb64, hcb64.size() * sizeof(double));
+    if (e == cudaSuccess && cb_exact) e = cudaMemcpy(lay->d_hcb16, hcb16.data(), hcb16.size() * sizeof(uint16_t), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess && cb_exact) e = cudaMemcpy(lay->d_hcb64, hcb64.data(), hcb64.size() * sizeof(double), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMalloc(&lay->d_planes, kPlaneBytes);
     if (e == cudaSuccess) e = cudaMemcpy(lay->d_planes, planes.data(), kPlaneBytes, cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(lay->d_meta, lay->meta.data(), lay->meta.size() * sizeof(HeadMeta), cudaMemcpyHostToDevice);
@@ -338,7 +391,7 @@ extern "C" void bgtq_layout_destroy(bgtq_layout *lay)
 {
     if (!lay) return;
     cudaFree(lay->d_meta); cudaFree(lay->d_rot); cudaFree(lay->d_rot_t);
-    cudaFree(lay->d_cb16); cudaFree(lay->d_cb64); cudaFree(lay->d_planes);
+    cudaFree(lay->d_cb16); cudaFree(lay->d_cb64); cudaFree(lay->d_planes); cudaFree(lay->d_hcb16); cudaFree(lay->d_hcb64);
     delete lay;
 }
 
@@ -464,6 +517,7 @@ extern "C" int bgtq_decode_attention_paged(const bgtq_layout *lay, int layer0, i
     if (layer0 < 0 || n_layers <= 0 || layer0 + n_layers > lay->n_layers) FAIL(BGTQ_EINVAL, "bgtq_decode_attention_paged: layer range");
     if (batch <= 0 || table_stride <= 0 || n_pages <= 0) FAIL(BGTQ_EINVAL, "bgtq_decode_attention_paged: batch/table_stride/n_pages");
     if (!(softmax_scale > 0.0f) || std::isinf(softmax_scale)) FAIL(BGTQ_EINVAL, "bgtq_decode_attention_paged: softmax_scale must be finite and > 0");
+    if (lay->cb_exact) FAIL(BGTQ_EINVAL, "bgtq_decode_attention_paged: not built for BGTQ_CODEBOOK_EXACT layouts");
     if (workspace_bytes < decode_ws_any(lay, batch, n_layers)) FAIL(BGTQ_EWORKSPACE, "bgtq_decode_attention_paged: workspace too small");
     const PageMap pm{page_table, table_stride, n_pages};
     return launch_decode_any(lay, layer0, n_layers, cache, q, seq_len, batch, (int64_t)table_stride * kTile, softmax_scale,
@@ -565,7 +619,7 @@ extern "C" int bgtq_prefill_attention(const bgtq_layout *lay, int layer, const v
 {
     if (!lay || !cache || !q || !seq_len || !out || !workspace) FAIL(BGTQ_EINVAL, "bgtq_prefill_attention: null pointer");
     if (layer < 0 || layer >= lay->n_layers) FAIL(BGTQ_EINVAL, "bgtq_prefill_attention: layer out of range");
-    if (lay->format != BGTQ_FORMAT_V1) FAIL(BGTQ_EINVAL, "bgtq_prefill_attention: built for BGTQ_FORMAT_V1 layouts only");
+    if (lay->format != BGTQ_FORMAT_V1 || lay->cb_exact) FAIL(BGTQ_EINVAL, "bgtq_prefill_attention: built for BGTQ_FORMAT_V1 layouts with the shared codebooks only");
     if (batch <= 0 || n_q <= 0 || max_tokens <= 0 || n_q > max_tokens) FAIL(BGTQ_EINVAL, "bgtq_prefill_attention: batch/n_q/max_tokens");
     if (!(softmax_scale > 0.0f) || std::isinf(softmax_scale)) FAIL(BGTQ_EINVAL, "bgtq_prefill_attention: softmax_scale");
     return launch_prefill(lay, layer, cache, q, seq_len, batch, n_q, max_tokens, softmax_scale, out, workspace,

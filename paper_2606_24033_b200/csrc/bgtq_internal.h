@@ -70,6 +70,11 @@ struct bgtq_layout {
     float *d_rot_t;                       // transposed: Pi^(m)[j][k] stored at [k][j]
     uint16_t *d_cb16;                     // fp16 bits of the 511 codebook levels (C_b at 2^b-1)
     double *d_cb64;                       // same levels as fp64
+    // exact-density codebooks (cb_exact = 1): one table set per (layer, kv head) -- groups and widths are
+    // 1:1 inside a head, so the table of width w holds C_{w, m_g} of that head's group of width w; V uses C_{b_V, d_h}.
+    int cb_exact;
+    uint16_t *d_hcb16;                    // [head][2][kHeadLutHalves]: K, V: flat fp16 levels (512) + the 5-bit pair table (1024 x 2)
+    double *d_hcb64;                      // [head][2][512]
     int sm_count;
 };
 
@@ -86,6 +91,10 @@ void codebook_levels(int b, double *levels);
 // e4m3 values; kappa in [32, 64] is chosen per width to minimise the largest relative error (0 for b = 1, 3; < 2e-6 for
 // b = 2; < 2e-4 for b = 4; < 1.3e-3 for b >= 5).  hi, lo receive 2^b bytes each.
 void codebook_planes(int b, float *kappa, uint8_t *hi, uint8_t *lo);
+// exact-density codebook C_{b,m}: Lloyd-Max quantiser of the density of a coordinate of sqrt(m) x (uniform unit vector of
+// R^m), rounded to fp16 (m even)
+void codebook_levels_sphere(int b, int m, double *levels);
+constexpr int kHeadLutHalves = 512 + 2048;
 constexpr int kPlaneBytes = 2 * 512;   // [plane][flat level index (2^b - 1 + k)]
 
 __host__ __device__ inline int64_t rot_offset(int m)  // element offset of Pi^(m), m even: sum of m'^2, m' = 2,4,..,m-2
@@ -121,6 +130,7 @@ int launch_block_energy(const void *q, int64_t n_q, const void *k, int64_t n_k, 
 size_t block_energy_ws_bytes(int Hq, int Hkv, int d_h);
 int launch_allocate(const float *scores, int n_heads, int L, int b_min, int b_max, int B,
                     uint8_t *bits, cudaStream_t st);
+int debug_decode_unit_exact(int b, int m, const uint32_t *words, float *values);
 int launch_quantize_append(const bgtq_layout *lay, int layer, int n_layers, void *cache, const void *k_new,
                            const void *v_new, int dt, int batch, int n_new, int32_t *seq_len,
                            int advance, int64_t max_tokens, const PageMap *pm, const RopeTab *rope, cudaStream_t st);

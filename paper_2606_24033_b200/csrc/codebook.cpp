@@ -202,4 +202,88 @@ void codebook_planes(int b, float *kappa, uint8_t *hi, uint8_t *lo)
     for (int j = 0; j < (1 << b); ++j) { hi[j] = cache->hi[b][j]; lo[j] = cache->lo[b][j]; }
 }
 
+
+// ---------------------------------------------------------------- exact-density codebooks (reading Q7b)
+// A coordinate of sqrt(m) * u, u uniform on the unit sphere of R^m (any unit vector after a Haar rotation),
+// has the density f_m(x) ~ (1 - x^2/m)^((m-3)/2) on |x| < sqrt(m).  With x = sqrt(m) sin(phi):
+//     mass(a, b)  ~  I_n(phi_b) - I_n(phi_a),  I_n(phi) = int_0^phi cos^n,  n = m - 2  (m even: I_0 = phi, then the
+//                    recurrence I_n = cos^(n-1) sin / n + (n-1)/n I_(n-2), all terms positive on [0, pi/2])
+//     int x f     ~  sqrt(m) (cos^(n+1)(phi_a) - cos^(n+1)(phi_b)) / (n+1)
+// C_{b,m} = the Lloyd-Max quantiser of f_m (Newton on the centroid equations, as above), rounded to fp16.  Independent of
+// oracle/codebook.py (which uses the incomplete beta function); tests compare the two tables value by value.
+namespace {
+long double cos_power_integral(int n, long double phi)
+{
+    const long double c = cosl(phi), s = sinl(phi);
+    long double I = phi, cp = c;                  // I_0; cp = cos^(k-1) for the next even k = 2
+    for (int k = 2; k <= n; k += 2) {
+        I = cp * s / k + (long double)(k - 1) / k * I;
+        cp *= c * c;
+    }
+    return I;
+}
+
+std::vector<long double> solve_positive_sphere(int n_pos, int m)
+{
+    const int n = m - 2;
+    const long double rm = sqrtl((long double)m), half_pi = acosl(0.0L);
+    std::vector<long double> c = solve_positive(n_pos);
+    if (c[n_pos - 1] >= 0.98L * rm) { const long double f = 0.98L * rm / c[n_pos - 1]; for (auto &v : c) v *= f; }
+    std::vector<long double> t(n_pos + 1), F(n_pos), lo(n_pos), di(n_pos), up(n_pos), step(n_pos), cn(n_pos), cp(n_pos), dp(n_pos);
+    for (int iter = 0; iter < 1000; ++iter) {
+        t[0] = 0.0L;
+        for (int k = 1; k < n_pos; ++k) t[k] = 0.5L * (c[k - 1] + c[k]);
+        long double resid = 0.0L;
+        for (int k = 0; k < n_pos; ++k) {
+            const long double pa = asinl(t[k] / rm), pb = k + 1 < n_pos ? asinl(t[k + 1] / rm) : half_pi;
+            const long double dI = cos_power_integral(n, pb) - cos_power_integral(n, pa);
+            const long double g = rm * (powl(cosl(pa), n + 1) - powl(cosl(pb), n + 1)) / ((n + 1) * dI);
+            // f(x) / mass = cos^(m-3)(phi) / (sqrt(m) dI)
+            const long double fa = powl(cosl(pa), m - 3) / (rm * dI);
+            const long double fb = k + 1 < n_pos ? powl(cosl(pb), m - 3) / (rm * dI) : 0.0L;
+            const long double dga = fa * (g - t[k]), dgb = k + 1 < n_pos ? fb * (t[k + 1] - g) : 0.0L;
+            F[k] = c[k] - g;
+            lo[k] = 0.0L; up[k] = 0.0L; di[k] = 1.0L;
+            if (k > 0) { lo[k] -= 0.5L * dga; di[k] -= 0.5L * dga; }
+            if (k + 1 < n_pos) { di[k] -= 0.5L * dgb; up[k] -= 0.5L * dgb; }
+            resid = fmaxl(resid, fabsl(F[k]));
+        }
+        if (resid < 1e-16L) break;
+        cp[0] = up[0] / di[0];
+        dp[0] = F[0] / di[0];
+        for (int k = 1; k < n_pos; ++k) {
+            const long double den = di[k] - lo[k] * cp[k - 1];
+            cp[k] = up[k] / den;
+            dp[k] = (F[k] - lo[k] * dp[k - 1]) / den;
+        }
+        step[n_pos - 1] = dp[n_pos - 1];
+        for (int k = n_pos - 2; k >= 0; --k) step[k] = dp[k] - cp[k] * step[k + 1];
+        long double lam = 1.0L;
+        for (;;) {
+            bool ok = true;
+            for (int k = 0; k < n_pos; ++k) cn[k] = c[k] - lam * step[k];
+            if (!(cn[0] > 0.0L) || !(cn[n_pos - 1] < rm)) ok = false;
+            for (int k = 1; k < n_pos && ok; ++k) if (!(cn[k] > cn[k - 1])) ok = false;
+            if (ok || lam < 1e-10L) break;
+            lam *= 0.5L;
+        }
+        c = cn;
+    }
+    return c;
+}
+}  // namespace
+
+// levels[0 .. 2^b) of C_{b,m}: ascending, fp16-representable; m even, 2 <= m
+void codebook_levels_sphere(int b, int m, double *levels)
+{
+    if (b == 0) { levels[0] = 0.0; return; }
+    const int n = 1 << (b - 1);
+    std::vector<long double> pos = solve_positive_sphere(n, m);
+    for (int k = 0; k < n; ++k) {
+        const double v = round_to_f16((double)pos[k]);
+        levels[n + k] = v;
+        levels[n - 1 - k] = -v;
+    }
+}
+
 }  // namespace bgtq

@@ -41,6 +41,17 @@ def test_library_codebook_equals_oracle_codebook(B):
         assert np.array_equal(got.astype(np.float16).astype(np.float64), got)      # fp16-representable
 
 
+def test_library_exact_density_codebook_equals_oracle(B):
+    """two independent solvers of the sphere-marginal Lloyd-Max tables (incomplete beta / dense Newton in numpy vs the
+    cos^n recurrence / Thomas solve in long double), bit-equal after rounding to fp16"""
+    for m in (2, 4, 6, 10, 16, 26, 32, 64, 128):
+        for b in range(9):
+            got = B.codebook_exact(b, m).astype(np.float64)
+            assert np.array_equal(got, ocb.sphere_codebook(b, m)), (b, m)
+    with pytest.raises(B.BgtqError):
+        B.codebook_exact(3, 7)
+
+
 @pytest.mark.parametrize("bmin,bmax,bbar", [(0, 8, 3), (1, 8, 3), (1, 8, 2), (0, 4, 1), (3, 3, 3)])
 def test_host_allocator_equals_oracle(B, bmin, bmax, bbar):
     rng = np.random.default_rng(17)

@@ -880,3 +880,44 @@ def test_window_append_respects_capacity(P, tab128):
     assert max(np.max(np.abs(got[a] - exp[a])) / rv[a // 4] for a in range(p.Hq)) <= 2e-3
     with pytest.raises(P.BgtqError):
         P.window_append(lay, 0, _cuda(p.k_post[None, :1], torch.float32), _cuda(p.v[None, :1], torch.float32), seq, win_k, win_v, 128, 64)
+
+
+# ----------------------------------------------------------------------------- exact-density codebooks
+@pytest.mark.parametrize("T,Hq,Hkv,b_k,b_v,bmin,bmax", [(333, 8, 2, 3, 3, 1, 8), (1000, 16, 2, 3, 3, 0, 8), (300, 8, 2, 2, 2, 1, 8),
+                                                       (200, 4, 1, 5, 5, 1, 8), (150, 8, 2, 4, 6, 1, 8)])
+def test_exact_density_codebooks_append_and_attention(P, rot128, T, Hq, Hkv, b_k, b_v, bmin, bmax):
+    """BGTQ_CODEBOOK_EXACT: every group quantises against C_{b, m_g} (V against C_{b_V, 128}); packed bytes bit-exact and
+    attention <= 2e-3 against the oracle run with the same per-(b, m) tables (its own solver)."""
+    tab = O.Tables(rot128, 128, cb_kind="sphere")
+    p = H.make_problem(300 + T, T, Hq, Hkv, b_k, b_v, bmin, bmax, rope_base=1e6)
+    lay = P.Layout(p.bits[None], Hq, p.d_h, b_v, p.rot, exact_codebooks=True)
+    assert lay.exact_codebooks and lay.fmt == 1
+    max_tokens = (T + 127) // 128 * 128
+    cache = lay.new_cache(1, max_tokens)
+    seq = torch.zeros(1, dtype=torch.int32, device="cuda")
+    half = T // 2
+    for (a, b) in [(0, half), (half, T)]:
+        P.quantize_append(lay, 0, cache, _cuda(p.k_post[None, a:b], torch.float32), _cuda(p.v[None, a:b], torch.float32), seq, max_tokens)
+    heads = H.oracle_heads(p, tab)
+    host = cache.cpu().numpy()
+    differs_from_gaussian = False
+    tabg = O.Tables(rot128, 128)
+    for h in range(Hkv):
+        stride = lay.tile_stride(0, h)
+        off = lay.region_offset(0, 0, h, 1, max_tokens)
+        exp = np.zeros((max_tokens // 128) * stride, dtype=np.uint8)
+        O.pack_region(heads[h], p.d_h, exp)
+        assert np.array_equal(host[off:off + exp.size], exp), h
+        hg = O.quantize_head(p.k_post[:, h], p.v[:, h], p.bits[h], b_v, tabg)
+        differs_from_gaussian |= not np.array_equal(hg.kidx, heads[h].kidx)
+    assert differs_from_gaussian                                    # (the tables really are different ones)
+    scale = 1.0 / math.sqrt(p.d_h)
+    out = P.decode_attention(lay, 0, cache, _cuda(p.q_post[None], torch.bfloat16), seq, max_tokens, scale, lay.new_workspace(1))
+    torch.cuda.synchronize()
+    exp, rv = H.oracle_attention(p, heads, tab, scale)
+    got = out[0].double().cpu().numpy()
+    G = Hq // Hkv
+    err = max(H.record_error("exact-density codebooks", got[a], exp[a], rv[a // G], T=T, b_k=b_k, b_v=b_v) for a in range(Hq))
+    assert err <= 2e-3, err
+    with pytest.raises(P.BgtqError):
+        P.prefill_attention(lay, 0, cache, _cuda(p.q_post[None, None], torch.bfloat16), seq, max_tokens, scale)
