@@ -50,6 +50,8 @@ def parse_args():
     ap.add_argument("--batch", type=int, default=None, help="sequences (default: the config's)")
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config supplying the head shape")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--microbench", action="store_true",
+                    help="print the instruction-rate microbenchmarks (bgtq_debug_microbench) that profiles/ and DESIGN.md quote, then exit")
     ap.add_argument("--format", type=int, default=1, choices=[1, 2],
                     help="physical cache format: 1 = BGTQ-v1 fragment order (mma.sync decode kernel, default), 2 = BGTQ-v2 row order (tcgen05 decode kernel, measured slower: DESIGN.md section 7b)")
     ap.add_argument("--prefill-chunk", type=int, default=0,
@@ -651,9 +653,21 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_microbench():
+    """`bench.py --microbench`: one line per microbenchmark (markdown table rows), at 12 warps per SM."""
+    from paper_2606_24033_b200 import binding as P
+    print("| quantity | value |")
+    print("|---|---|")
+    for i in range(P.MICROBENCH_COUNT):
+        name, v = P.microbench(i, 12)
+        print(f"| {name} | {v:.3f} |")
+
+
 def main():
     args = parse_args()
-    if args.impl == "reference":
+    if args.microbench:
+        run_microbench()
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

@@ -265,6 +265,13 @@ int bgtq_debug_decode_unit(int b, const uint32_t *words, float *values);
  * since the last read, and resets.  Do not enable during stream capture. */
 void bgtq_profile_decode(int enable);
 int bgtq_profile_decode_read(double *ms_sum, int *count);
+/* instruction-rate microbenchmarks behind the numbers DESIGN.md section 7 and profiles/ quote (which pipes the unpack
+ * instructions share, what a 3-bit unit costs to unpack, how fast one thread issues tcgen05.mma); `warps` = warps per SM
+ * (4..16) for the pipe and unpack tests.  which in [0, BGTQ_MICROBENCH_COUNT); bgtq_debug_microbench_name gives the
+ * quantity and its unit.  Synchronous, about 10 ms each; not part of the method. */
+#define BGTQ_MICROBENCH_COUNT 21
+const char *bgtq_debug_microbench_name(int which);
+int bgtq_debug_microbench(int which, int warps, double *value);
 /* number of kernels launched by this library since load (bench.py's gpu_launches). */
 int64_t bgtq_launch_count(void);
 

@@ -10,7 +10,7 @@ _BINDING_NAMES = (
     "new_windows", "window_append", "decode_attention_protected",
     "codebook", "fp16_decode_attention", "prefill_attention", "debug_decode_unit", "profile_decode", "profile_decode_read", "launch_count", "lib", "SYMBOLS", "LIB_PATH",
     "F32", "BF16", "PAIR_HALF", "PAIR_INTERLEAVED", "QK_AVG", "QK_MAX", "QK_PRODUCT", "K_ONLY",
-    "Q_ONLY", "TILE_TOKENS", "FORMAT_V1", "FORMAT_V2", "CODEBOOK_EXACT", "codebook_exact",
+    "Q_ONLY", "TILE_TOKENS", "FORMAT_V1", "FORMAT_V2", "CODEBOOK_EXACT", "codebook_exact", "microbench", "MICROBENCH_COUNT",
 )
 
 

@@ -33,7 +33,9 @@ SYMBOLS = [
     "bgtq_quantize_append_rope",
     "bgtq_window_bytes", "bgtq_window_append", "bgtq_decode_attention_protected",
     "bgtq_layout_create_format", "bgtq_layout_format", "bgtq_codebook_exact",
+    "bgtq_debug_microbench", "bgtq_debug_microbench_name",
 ]
+MICROBENCH_COUNT = 21
 FORMAT_V1, FORMAT_V2 = 1, 2
 CODEBOOK_EXACT = 0x100
 
@@ -67,6 +69,10 @@ def _load() -> C.CDLL:
     lib.bgtq_layout_create.argtypes = [vp, i32, i32, i32, i32, i32, i32, vp, C.POINTER(vp)]
     lib.bgtq_layout_create_format.restype = i32
     lib.bgtq_layout_create_format.argtypes = [vp, i32, i32, i32, i32, i32, i32, vp, i32, C.POINTER(vp)]
+    lib.bgtq_debug_microbench.restype = i32
+    lib.bgtq_debug_microbench.argtypes = [i32, i32, C.POINTER(C.c_double)]
+    lib.bgtq_debug_microbench_name.restype = C.c_char_p
+    lib.bgtq_debug_microbench_name.argtypes = [i32]
     lib.bgtq_codebook_exact.restype = i32
     lib.bgtq_codebook_exact.argtypes = [i32, i32, vp]
     lib.bgtq_layout_format.restype = i32
@@ -167,6 +173,13 @@ def codebook(b: int) -> np.ndarray:
     out = np.zeros(1 << b, dtype=np.float32)
     _check(_lib.bgtq_codebook(b, out.ctypes.data))
     return out
+
+
+def microbench(which: int, warps: int = 12):
+    """bgtq_debug_microbench -> (name, value)."""
+    v = C.c_double(0.0)
+    _check(_lib.bgtq_debug_microbench(which, warps, C.byref(v)))
+    return _lib.bgtq_debug_microbench_name(which).decode(), float(v.value)
 
 
 def codebook_exact(b: int, m: int) -> np.ndarray:

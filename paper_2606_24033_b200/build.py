@@ -12,7 +12,7 @@ import sys
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libbgtq.so")
-SOURCES = ["bgtq_host.cu", "bgtq_kernels.cu", "bgtq_append.cu", "bgtq_decode.cu", "bgtq_decode2.cu", "codebook.cpp"]
+SOURCES = ["bgtq_host.cu", "bgtq_kernels.cu", "bgtq_append.cu", "bgtq_decode.cu", "bgtq_decode2.cu", "bgtq_microbench.cu", "codebook.cpp"]
 HEADERS = ["bgtq_internal.h", "bgtq_device.cuh", os.path.join("..", "..", "include", "bgtq.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "--compiler-options", "-fPIC", "-shared"]

@@ -1274,7 +1274,7 @@ int launch_window(const void *win_k, const void *win_v, const void *q, const int
 template <int W, bool PAGED, bool EXACT = false>
 static int launch_decode_w(const DecodeParams &P, int grid, size_t smem, cudaStream_t st)
 {
-    if (first_use_on_device(8 + (W / 4) * 3 + (PAGED ? 1 : 0) + (EXACT ? 2 : 0)))   // once per device, outside any stream capture
+    if (first_use_on_device(8 + (W / 2) * 4 + (PAGED ? 1 : 0) + (EXACT ? 2 : 0)))   // once per device, outside any stream capture
         CUDA_TRY(cudaFuncSetAttribute(decode_kernel<W, PAGED, EXACT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - kStaticSmem));
     if (int rc = profile_decode_begin(st)) return rc;
     {

@@ -25,9 +25,9 @@ void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 bool first_use_on_device(int key)
 {
     static std::mutex mu;
-    static bool seen[32][64] = {};
+    static bool seen[64][64] = {};
     int dev = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64 || key < 0 || key >= 32) return true;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64 || key < 0 || key >= 64) return true;
     std::lock_guard<std::mutex> lock(mu);
     const bool first = !seen[key][dev];
     seen[key][dev] = true;
@@ -532,6 +532,12 @@ extern "C" int bgtq_quantize_append(const bgtq_layout *lay, int layer, void *cac
                                        advance_seq_len, max_tokens, stream);
 }
 
+extern "C" const char *bgtq_debug_microbench_name(int which) { return microbench_name(which); }
+extern "C" int bgtq_debug_microbench(int which, int warps, double *value)
+{
+    if (!value || warps < 1 || warps > 16) FAIL(BGTQ_EINVAL, "bgtq_debug_microbench: value != NULL, warps in 1..16");
+    return microbench_run(which, warps, value);
+}
 extern "C" void bgtq_profile_decode(int enable) { profile_decode_enable(enable); }
 extern "C" int bgtq_profile_decode_read(double *ms_sum, int *count)
 {

@@ -156,6 +156,8 @@ size_t fp16_ws_bytes(int sm_count, int batch, int n_layers, int Hkv);
 int launch_fp16_decode(int n_layers, int batch, int Hq, int Hkv, const void *k_cache, const void *v_cache,
                        const void *q, const int32_t *seq_len, int64_t max_tokens, float scale, void *out,
                        void *ws, size_t ws_bytes, cudaStream_t st);
+const char *microbench_name(int which);
+int microbench_run(int which, int warps, double *value);
 void profile_decode_enable(int enable);
 int profile_decode_read(double *ms_sum, int *count);
 
