@@ -376,16 +376,32 @@ static int norm_slot(int tau) { return (tau & 7) * 16 + (tau >> 4) * 2 + ((tau >
  *   kidx     : [T][kdim] K codes, grouped coordinate order (groups concatenated), kdim = sum gm
  *   knorm    : [T][n_groups] fp16 bits;  vidx: [T][d_h];  vnorm: [T]
  * Only the fields of tokens in [t0,t1) are touched; everything else is preserved.           */
+void orc_pack_region_kv(uint8_t *region, long tile_stride, int n_groups, const int *gb, const int *gm,
+                        int d_h, int n_vgroups, const int *vgb, const int *vgm, long t0, long t1,
+                        uint8_t *kidx, uint16_t *knorm, uint8_t *vidx, uint16_t *vnorm, int unpack);
+
 void orc_pack_region(uint8_t *region, long tile_stride, int n_groups, const int *gb, const int *gm,
                      int d_h, int b_v, long t0, long t1, uint8_t *kidx, uint16_t *knorm,
                      uint8_t *vidx, uint16_t *vnorm, int unpack)
+{
+    /* V: one group of all d_h coordinates at width b_v */
+    orc_pack_region_kv(region, tile_stride, n_groups, gb, gm, d_h, 1, &b_v, &d_h, t0, t1, kidx, knorm, vidx, vnorm, unpack);
+}
+
+/* The general form (V-side groups, reading Q19): V group gv has width vgb[gv] (ascending) and vgm[gv]
+ * coordinates (a multiple of 16: whole V blocks); tile = [K codes | K norms | V norms (n_vgroups rows) | V codes
+ * (groups in order, 16 * vgm * vgb bytes each)].
+ *   vidx  : [T][d_h] V codes in grouped V order (groups concatenated);  vnorm: [T][n_vgroups]                     */
+void orc_pack_region_kv(uint8_t *region, long tile_stride, int n_groups, const int *gb, const int *gm,
+                        int d_h, int n_vgroups, const int *vgb, const int *vgm, long t0, long t1,
+                        uint8_t *kidx, uint16_t *knorm, uint8_t *vidx, uint16_t *vnorm, int unpack)
 {
     int kdim = 0;
     long kcode_bytes = 0;
     for (int g = 0; g < n_groups; ++g) { kdim += gm[g]; kcode_bytes += 16L * gm[g] * gb[g]; }
     long knorm_off = kcode_bytes;
     long vnorm_off = knorm_off + 256L * n_groups;
-    long vcode_off = vnorm_off + 256L;
+    long vcode_off = vnorm_off + 256L * n_vgroups;
     for (long t = t0; t < t1; ++t) {
         uint8_t *tile = region + (t >> 7) * tile_stride;
         int tau = (int)(t & 127);
@@ -420,26 +436,31 @@ void orc_pack_region(uint8_t *region, long tile_stride, int n_groups, const int 
             goff += 16L * m * b;
             ubase += m;
         }
-        /* ---- V norm */
-        {
-            uint8_t *np_ = tile + vnorm_off + 2L * norm_slot(tau);
-            if (unpack) memcpy(&vnorm[t], np_, 2);
-            else memcpy(np_, &vnorm[t], 2);
-        }
-        /* ---- V codes: coord u -> J=u>>4, g=u&7, rho=(u>>3)&1; token -> kappa=tau>>4,
-         *      c=(tau&7)>>1, e=tau&1, o=(tau>>3)&1; unit J*2+rho, lane g*4+c, slot kappa*4+o*2+e */
-        for (int u = 0; u < d_h; ++u) {
-            int J = u >> 4, g = u & 7, rho = (u >> 3) & 1;
-            int kappa = tau >> 4, c = (tau & 7) >> 1, e = tau & 1, o = (tau >> 3) & 1;
-            long unit = vcode_off + (long)(J * 2 + rho) * b_v * 128;
-            int lane = g * 4 + c, slot = kappa * 4 + o * 2 + e;
-            uint32_t W[8];
-            for (int w = 0; w < b_v; ++w) memcpy(&W[w], tile + unit + 4L * (w * 32 + lane), 4);
-            if (unpack) vidx[(size_t)t * d_h + u] = (uint8_t)orc_get_field(W, b_v, slot);
-            else {
-                orc_put_field(W, b_v, slot, vidx[(size_t)t * d_h + u]);
-                for (int w = 0; w < b_v; ++w) memcpy(tile + unit + 4L * (w * 32 + lane), &W[w], 4);
+        /* ---- V: per group its norm, then its codes.  Inside a group, grouped coordinate u -> J=u>>4, g=u&7,
+         *      rho=(u>>3)&1; token -> kappa=tau>>4, c=(tau&7)>>1, e=tau&1, o=(tau>>3)&1; unit J*2+rho of the group,
+         *      lane g*4+c, slot kappa*4+o*2+e */
+        long vgoff = 0;
+        int vbase = 0;
+        for (int gv = 0; gv < n_vgroups; ++gv) {
+            int b_v = vgb[gv], mv = vgm[gv];
+            uint8_t *np_ = tile + vnorm_off + 256L * gv + 2L * norm_slot(tau);
+            if (unpack) memcpy(&vnorm[(size_t)t * n_vgroups + gv], np_, 2);
+            else memcpy(np_, &vnorm[(size_t)t * n_vgroups + gv], 2);
+            for (int u = 0; u < mv; ++u) {
+                int J = u >> 4, g = u & 7, rho = (u >> 3) & 1;
+                int kappa = tau >> 4, c = (tau & 7) >> 1, e = tau & 1, o = (tau >> 3) & 1;
+                long unit = vcode_off + vgoff + (long)(J * 2 + rho) * b_v * 128;
+                int lane = g * 4 + c, slot = kappa * 4 + o * 2 + e;
+                uint32_t W[8];
+                for (int w = 0; w < b_v; ++w) memcpy(&W[w], tile + unit + 4L * (w * 32 + lane), 4);
+                if (unpack) vidx[(size_t)t * d_h + vbase + u] = (uint8_t)orc_get_field(W, b_v, slot);
+                else {
+                    orc_put_field(W, b_v, slot, vidx[(size_t)t * d_h + vbase + u]);
+                    for (int w = 0; w < b_v; ++w) memcpy(tile + unit + 4L * (w * 32 + lane), &W[w], 4);
+                }
             }
+            vgoff += 16L * mv * b_v;
+            vbase += mv;
         }
     }
 }

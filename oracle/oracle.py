@@ -55,6 +55,9 @@ def lib():
         L.orc_pack_region.restype = None
         L.orc_pack_region.argtypes = [u8p, C.c_long, C.c_int, ip, ip, C.c_int, C.c_int, C.c_long,
                                       C.c_long, u8p, u16p, u8p, u16p, C.c_int]
+        L.orc_pack_region_kv.restype = None
+        L.orc_pack_region_kv.argtypes = [u8p, C.c_long, C.c_int, ip, ip, C.c_int, C.c_int, ip, ip, C.c_long,
+                                         C.c_long, u8p, u16p, u8p, u16p, C.c_int]
         L.orc_chunk_words_v2.restype = C.c_int
         L.orc_chunk_words_v2.argtypes = [C.c_int, C.c_int]
         L.orc_put_field_v2.restype = None
@@ -201,6 +204,35 @@ def groups_from_bits(bits: Sequence[int], d_h: int, pairing: int = PAIR_HALF) ->
     return out
 
 
+V_BLOCK = 16   # coordinates per V block (reading Q19: the V-side allocator's unit)
+
+
+def v_groups_from_bits(bits_v: Sequence[int], d_h: int, block: int = V_BLOCK) -> List[Group]:
+    """V-side groups ("a V-side allocator", reading Q19): V block j = coordinates
+    [block*j, block*j + block); blocks of equal width form one group, ascending width, member blocks and their
+    coordinates in ascending order.  Every V block is stored (width >= 1)."""
+    bits_v = np.asarray(bits_v, dtype=np.int64)
+    assert len(bits_v) * block == d_h and bits_v.min() >= 1 and bits_v.max() <= 8
+    out = []
+    for w in range(1, 9):
+        blk = np.nonzero(bits_v == w)[0]
+        if len(blk) == 0:
+            continue
+        coords = (blk[:, None] * block + np.arange(block)[None, :]).reshape(-1)
+        out.append(Group(w, blk, coords))
+    return out
+
+
+def v_block_energy(v: np.ndarray, block: int = V_BLOCK) -> np.ndarray:
+    """V-side score (reading Q19): s^V_j = E_t ||v_t^(j)||^2, the mean squared norm of V block j.  With the
+    TQ-MSE rate law the expected squared error of the attention output contributed by block j is
+    proportional to s^V_j 4^-b_j, the same objective J(b) = sum_j s_j 4^-b_j Alg. 1 minimises for K.
+    v[N, H_kv, d_h] -> s[H_kv, d_h / block].  The plain definition."""
+    v = _c64(v)
+    N, H, d = v.shape
+    return np.mean(np.sum(v.reshape(N, H, d // block, block) ** 2, axis=3), axis=0)
+
+
 class Tables:
     """Codebooks (oracle's own Lloyd-Max, fp16-rounded) + the rotation table passed in as data.
     cb_kind "gaussian": one table per width, the Lloyd-Max quantiser of N(0,1) (reading Q7);
@@ -264,21 +296,30 @@ class QuantizedHead:
     b_v: int
     kidx: np.ndarray      # [T, kdim] uint8, grouped coordinate order
     knorm: np.ndarray     # [T, n_groups] uint16 (fp16 bits)
-    vidx: np.ndarray      # [T, d_h] uint8
-    vnorm: np.ndarray     # [T] uint16
+    vidx: np.ndarray      # [T, d_h] uint8 (grouped V order when vgroups is set)
+    vnorm: np.ndarray     # [T] uint16, or [T, n_vgroups] when vgroups is set
+    vgroups: List[Group] | None = None     # V-side groups (reading Q19); None = one group of all d_h coordinates at b_v
+
+    def v_groups(self, d_h: int) -> List[Group]:
+        return self.vgroups if self.vgroups is not None else [Group(self.b_v, np.arange(d_h // V_BLOCK), np.arange(d_h))]
 
 
 def quantize_head(k_post: np.ndarray, v: np.ndarray, bits: Sequence[int], b_v: int, tab: Tables,
-                  pairing: int = PAIR_HALF) -> QuantizedHead:
+                  pairing: int = PAIR_HALF, bits_v: Sequence[int] | None = None) -> QuantizedHead:
     """Quantise T tokens of one KV head.  k_post[T, d_h] post-RoPE keys, v[T, d_h] (exact values of
     the boundary dtype).  K: one encoder per same-width group; V: one group of all
-    d_h coordinates at width b_v."""
+    d_h coordinates at width b_v, or -- bits_v[d_h/16] given -- one encoder per same-width group of
+    16-coordinate V blocks (reading Q19; b_v is then ignored)."""
     k_post, v = _c64(k_post), _c64(v)
     T, d = k_post.shape
     groups = groups_from_bits(bits, d, pairing)
     kdim = sum(g.m for g in groups)
     q = QuantizedHead(groups, b_v, np.zeros((T, kdim), np.uint8), np.zeros((T, len(groups)), np.uint16),
                       np.zeros((T, d), np.uint8), np.zeros(T, np.uint16))
+    if bits_v is not None:
+        q.vgroups = v_groups_from_bits(bits_v, d)
+        q.b_v = q.vgroups[0].width
+        q.vnorm = np.zeros((T, len(q.vgroups)), np.uint16)
     for t in range(T):
         o = 0
         for gi, g in enumerate(groups):
@@ -286,9 +327,17 @@ def quantize_head(k_post: np.ndarray, v: np.ndarray, bits: Sequence[int], b_v: i
             q.kidx[t, o:o + g.m] = idx
             q.knorm[t, gi] = h
             o += g.m
-        idx, h, _ = quantize_group(v[t], b_v, tab)
-        q.vidx[t] = idx
-        q.vnorm[t] = h
+        if q.vgroups is None:
+            idx, h, _ = quantize_group(v[t], b_v, tab)
+            q.vidx[t] = idx
+            q.vnorm[t] = h
+            continue
+        o = 0
+        for gi, g in enumerate(q.vgroups):
+            idx, h, _ = quantize_group(v[t, g.coords], g.width, tab)
+            q.vidx[t, o:o + g.m] = idx
+            q.vnorm[t, gi] = h
+            o += g.m
     return q
 
 
@@ -303,9 +352,14 @@ def dequantize_head(q: QuantizedHead, tab: Tables, d_h: int) -> Tuple[np.ndarray
         h = np.array([f16_value(x) for x in q.knorm[:, gi]]) if T < 64 else _f16_array(q.knorm[:, gi])
         K[:, g.coords] = (h / math.sqrt(g.m))[:, None] * (Cb[q.kidx[:, o:o + g.m]] @ Pi)
         o += g.m
-    Cv, Piv = tab.C(q.b_v, d_h), tab.Pi(d_h).astype(np.float64)
-    hv = _f16_array(q.vnorm)
-    V = (hv / math.sqrt(d_h))[:, None] * (Cv[q.vidx] @ Piv)
+    V = np.zeros((T, d_h))
+    vnorm = q.vnorm.reshape(T, -1)
+    o = 0
+    for gi, g in enumerate(q.v_groups(d_h)):
+        Cv, Piv = tab.C(g.width, g.m), tab.Pi(g.m).astype(np.float64)
+        hv = _f16_array(vnorm[:, gi])
+        V[:, g.coords] = (hv / math.sqrt(g.m))[:, None] * (Cv[q.vidx[:, o:o + g.m]] @ Piv)
+        o += g.m
     return K, V
 
 
@@ -314,7 +368,7 @@ def _f16_array(bits: np.ndarray) -> np.ndarray:
 
 
 # ----------------------------------------------------------------------------- physical layout
-def tile_geometry(groups: List[Group], d_h: int, b_v: int, version: int = 1):
+def tile_geometry(groups: List[Group], d_h: int, b_v: int, version: int = 1, vgroups: List[Group] | None = None):
     """Byte offsets inside one 128-token tile: [K codes | K norms | V norms | V codes].
     version 1 = BGTQ-v1 (fragment order, no padding); 2 = BGTQ-v2 (row order: a K chunk of r <= 32 coordinates of one
     token takes whole 32-bit words)."""
@@ -326,16 +380,21 @@ def tile_geometry(groups: List[Group], d_h: int, b_v: int, version: int = 1):
         kcode = sum(16 * g.m * g.width for g in groups)
     knorm_off = kcode
     vnorm_off = knorm_off + 256 * len(groups)
-    vcode_off = vnorm_off + 256
-    stride = vcode_off + 16 * d_h * b_v
+    if vgroups is not None:           # V-side groups (reading Q19): one norm row and one code section per group
+        assert version == 1
+        vcode_off = vnorm_off + 256 * len(vgroups)
+        stride = vcode_off + sum(16 * g.m * g.width for g in vgroups)
+    else:
+        vcode_off = vnorm_off + 256
+        stride = vcode_off + 16 * d_h * b_v
     return dict(kcode=kcode, knorm_off=knorm_off, vnorm_off=vnorm_off, vcode_off=vcode_off,
                 stride=stride)
 
 
-def token_bytes(groups: List[Group], d_h: int, b_v: int, version: int = 1) -> float:
+def token_bytes(groups: List[Group], d_h: int, b_v: int, version: int = 1, vgroups: List[Group] | None = None) -> float:
     """Packed bytes per token of one KV head = tile stride / 128
     (v1: = 16*bbar_K + 16*b_V + 2*(n_g+1) at d_h = 128; PAPER.md:837 for the 96-byte ideal)."""
-    return tile_geometry(groups, d_h, b_v, version)["stride"] / 128.0
+    return tile_geometry(groups, d_h, b_v, version, vgroups)["stride"] / 128.0
 
 
 def pack_region(q: QuantizedHead, d_h: int, region: np.ndarray | None = None,
@@ -344,7 +403,7 @@ def pack_region(q: QuantizedHead, d_h: int, region: np.ndarray | None = None,
     one (sequence, layer, KV head); all other fields of ``region`` are preserved.  ``region``
     (uint8, zero-initialised) is created when None."""
     T = q.kidx.shape[0]
-    geo = tile_geometry(q.groups, d_h, q.b_v, version)
+    geo = tile_geometry(q.groups, d_h, q.b_v, version, q.vgroups)
     n_tiles = (t_offset + T + 127) // 128
     if region is None:
         region = np.zeros(n_tiles * geo["stride"], dtype=np.uint8)
@@ -358,6 +417,15 @@ def pack_region(q: QuantizedHead, d_h: int, region: np.ndarray | None = None,
     kidx = np.zeros((t_offset + T, kdim), np.uint8); kidx[t_offset:] = q.kidx
     knorm = np.zeros((t_offset + T, ng), np.uint16); knorm[t_offset:] = q.knorm
     vidx = np.zeros((t_offset + T, d_h), np.uint8); vidx[t_offset:] = q.vidx
+    if q.vgroups is not None:
+        nvg = len(q.vgroups)
+        vgb = np.array([g.width for g in q.vgroups], dtype=np.int32)
+        vgm = np.array([g.m for g in q.vgroups], dtype=np.int32)
+        vnorm = np.zeros((t_offset + T, nvg), np.uint16); vnorm[t_offset:] = q.vnorm
+        lib().orc_pack_region_kv(_p(region, C.c_uint8), geo["stride"], ng, _p(gb, C.c_int), _p(gm, C.c_int), d_h,
+                                 nvg, _p(vgb, C.c_int), _p(vgm, C.c_int), t_offset, t_offset + T,
+                                 _p(kidx, C.c_uint8), _p(knorm, C.c_uint16), _p(vidx, C.c_uint8), _p(vnorm, C.c_uint16), 0)
+        return region
     vnorm = np.zeros(t_offset + T, np.uint16); vnorm[t_offset:] = q.vnorm
     fn = lib().orc_pack_region_v2 if version == 2 else lib().orc_pack_region
     fn(_p(region, C.c_uint8), geo["stride"], ng, _p(gb, C.c_int),
@@ -368,14 +436,23 @@ def pack_region(q: QuantizedHead, d_h: int, region: np.ndarray | None = None,
 
 
 def unpack_region(region: np.ndarray, groups: List[Group], d_h: int, b_v: int, T: int,
-                  version: int = 1) -> QuantizedHead:
-    geo = tile_geometry(groups, d_h, b_v, version)
+                  version: int = 1, vgroups: List[Group] | None = None) -> QuantizedHead:
+    geo = tile_geometry(groups, d_h, b_v, version, vgroups)
     gb = np.array([g.width for g in groups], dtype=np.int32)
     gm = np.array([g.m for g in groups], dtype=np.int32)
     kdim = int(gm.sum())
     q = QuantizedHead(groups, b_v, np.zeros((T, kdim), np.uint8), np.zeros((T, len(groups)), np.uint16),
                       np.zeros((T, d_h), np.uint8), np.zeros(T, np.uint16))
     region = np.ascontiguousarray(region, dtype=np.uint8)
+    if vgroups is not None:
+        q.vgroups, q.b_v = vgroups, vgroups[0].width
+        q.vnorm = np.zeros((T, len(vgroups)), np.uint16)
+        vgb = np.array([g.width for g in vgroups], dtype=np.int32)
+        vgm = np.array([g.m for g in vgroups], dtype=np.int32)
+        lib().orc_pack_region_kv(_p(region, C.c_uint8), geo["stride"], len(groups), _p(gb, C.c_int), _p(gm, C.c_int), d_h,
+                                 len(vgroups), _p(vgb, C.c_int), _p(vgm, C.c_int), 0, T, _p(q.kidx, C.c_uint8),
+                                 _p(q.knorm, C.c_uint16), _p(q.vidx, C.c_uint8), _p(q.vnorm, C.c_uint16), 1)
+        return q
     fn = lib().orc_pack_region_v2 if version == 2 else lib().orc_pack_region
     fn(_p(region, C.c_uint8), geo["stride"], len(groups), _p(gb, C.c_int),
        _p(gm, C.c_int), d_h, b_v, 0, T, _p(q.kidx, C.c_uint8),

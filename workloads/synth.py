@@ -112,6 +112,16 @@ def values_gaussian(seed, stream: int, n: int, n_heads: int, d_h: int) -> np.nda
     return rng.standard_normal((n, n_heads, d_h))
 
 
+def values_block_scaled(seed, stream: int, n: int, n_heads: int, d_h: int, block: int = 16,
+                        lo: float = 0.05, hi: float = 5.0) -> np.ndarray:
+    """V entries whose 16-coordinate blocks have per-(head, block) variances drawn log-uniform over [lo, hi]:
+    an input with something for a V-side allocator to find (reading Q19 / section 5).  fp64."""
+    rng = np.random.default_rng([int(seed), int(stream), 0x7B10C])
+    var = np.exp(np.log(lo) + rng.random((n_heads, d_h // block)) * (np.log(hi) - np.log(lo)))
+    x = rng.standard_normal((n, n_heads, d_h))
+    return x * np.repeat(np.sqrt(var), block, axis=1)[None, :, :]
+
+
 def f32_to_bf16_bits(x: np.ndarray) -> np.ndarray:
     """fp32 -> bf16 bit patterns (uint16), round-to-nearest-even (finite inputs)."""
     u = np.ascontiguousarray(x, dtype=np.float32).view(np.uint32)
