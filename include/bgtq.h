@@ -111,6 +111,29 @@ int bgtq_codebook_exact(int b, int m, float *levels);
 int bgtq_layout_create_format(const uint8_t *bits, int n_layers, int n_kv_heads, int n_q_heads, int d_h,
                               int b_v, int pairing, const float *rotations, int format, bgtq_layout **out);
 int bgtq_layout_format(const bgtq_layout *layout);
+
+/* ---- V-side allocator ("Adding a V-side allocator to Block-GTQ is a natural extension",
+ * PAPER.md:318; the paper gives no construction, reading Q19 is the one built here).
+ * A V block is BGTQ_V_BLOCK = 16 consecutive coordinates of the head (d_h/16 blocks).  Its score is the mean squared block
+ * norm  s^V[h][j] = 1/n sum_t sum_{u<16} v[t][h][16j+u]^2  (bgtq_v_block_energy): by the TQ-MSE rate law
+ * the squared error block j adds to an attention output is proportional to s^V_j 4^-b_j, the objective Alg. 1 minimises,
+ * so the widths come from bgtq_allocate(scores = s^V, n_blocks = d_h/16, B = bbar_V * d_h/16).  Blocks of equal width form
+ * one V group (ascending width, member blocks ascending), encoded by one TQ-MSE encoder with rotation Pi^(m), m = 16 x
+ * blocks, and one fp16 norm per (token, V group) -- exactly what PAPER.md:108 does for K.
+ *   v [device] [n, n_kv_heads, d_h] of dtype dt; scores [device] float [n_kv_heads, d_h/16]; workspace [device] scratch of
+ *   at least bgtq_v_block_energy_workspace_bytes bytes.  Deterministic.  One layer per call.
+ * bgtq_layout_create_kv: bits_k as `bits` of bgtq_layout_create; bits_v [host] uint8 [n_layers, n_kv_heads, d_h/16], widths
+ *   1..8 (every V block is stored).  Tile = [K codes | K norms | V norms: one row per V group | V codes: groups in order,
+ *   two units of 128*w bytes per block]; all widths of a head equal = the uniform layout, byte for byte (heads may then
+ *   still differ from each other).  BGTQ_FORMAT_V1 only (BGTQ_CODEBOOK_EXACT may be OR-ed in: V group (w, m) uses C_{w,m}).
+ *   Heads with more than one V group are served by append (all variants) and decode attention (contiguous and protected);
+ *   bgtq_prefill_attention and bgtq_decode_attention_paged return BGTQ_EINVAL for such a layout. */
+#define BGTQ_V_BLOCK 16
+size_t bgtq_v_block_energy_workspace_bytes(int n_kv_heads, int d_h);
+int bgtq_v_block_energy(const void *v, int64_t n, int dt, int n_kv_heads, int d_h, float *scores,
+                        void *workspace, size_t workspace_bytes, void *stream);
+int bgtq_layout_create_kv(const uint8_t *bits_k, const uint8_t *bits_v, int n_layers, int n_kv_heads, int n_q_heads,
+                          int d_h, int pairing, const float *rotations, int format, bgtq_layout **out);
 void bgtq_layout_destroy(bgtq_layout *layout);
 
 /* Sizes.  cache: one buffer for all layers, order [layer][sequence][head][tile], which the CALLER

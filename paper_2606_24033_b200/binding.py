@@ -34,6 +34,7 @@ SYMBOLS = [
     "bgtq_window_bytes", "bgtq_window_append", "bgtq_decode_attention_protected",
     "bgtq_layout_create_format", "bgtq_layout_format", "bgtq_codebook_exact",
     "bgtq_debug_microbench", "bgtq_debug_microbench_name",
+    "bgtq_v_block_energy_workspace_bytes", "bgtq_v_block_energy", "bgtq_layout_create_kv",
 ]
 MICROBENCH_COUNT = 21
 FORMAT_V1, FORMAT_V2 = 1, 2
@@ -63,6 +64,12 @@ def _load() -> C.CDLL:
     lib.bgtq_block_energy_workspace_bytes.argtypes = [i32, i32, i32]
     lib.bgtq_block_energy.restype = i32
     lib.bgtq_block_energy.argtypes = [vp, i64, vp, i64, i32, i32, i32, i32, i32, i32, vp, vp, vp, vp, sz, vp]
+    lib.bgtq_v_block_energy_workspace_bytes.restype = sz
+    lib.bgtq_v_block_energy_workspace_bytes.argtypes = [i32, i32]
+    lib.bgtq_v_block_energy.restype = i32
+    lib.bgtq_v_block_energy.argtypes = [vp, i64, i32, i32, i32, vp, vp, sz, vp]
+    lib.bgtq_layout_create_kv.restype = i32
+    lib.bgtq_layout_create_kv.argtypes = [vp, vp, i32, i32, i32, i32, i32, vp, i32, vp]
     lib.bgtq_allocate.restype = i32
     lib.bgtq_allocate.argtypes = [vp, i32, i32, i32, i32, i32, vp, i32, vp]
     lib.bgtq_layout_create.restype = i32
@@ -208,6 +215,19 @@ def block_energy(q: torch.Tensor, k: torch.Tensor, pairing: int = PAIR_HALF, kin
     return (scores, eq, ek) if return_parts else scores
 
 
+V_BLOCK = 16
+
+
+def v_block_energy(v: torch.Tensor) -> torch.Tensor:
+    """bgtq_v_block_energy.  v [N, H_kv, d_h] (CUDA) -> V-side scores [H_kv, d_h/16] float32."""
+    n, Hkv, d = v.shape
+    scores = torch.empty((Hkv, d // V_BLOCK), dtype=torch.float32, device=v.device)
+    nws = int(_lib.bgtq_v_block_energy_workspace_bytes(Hkv, d))
+    ws = torch.empty(nws, dtype=torch.uint8, device=v.device)
+    _check(_lib.bgtq_v_block_energy(_dev(v), n, _dt(v), Hkv, d, _dev(scores), _dev(ws), nws, _stream()))
+    return scores
+
+
 def allocate(scores, total_bits: int, b_min: int, b_max: int):
     """bgtq_allocate.  scores [n_heads, L] float32: a CUDA tensor runs the device kernel and returns
     a CUDA uint8 tensor; a numpy array runs the library's host variant."""
@@ -228,16 +248,24 @@ class Layout:
     """bgtq_layout: static metadata of the packed cache for an allocation bits[n_layers, H_kv, L]."""
 
     def __init__(self, bits: np.ndarray, n_q_heads: int, d_h: int, b_v: int, rotations: np.ndarray,
-                 pairing: int = PAIR_HALF, fmt: int = FORMAT_V1, exact_codebooks: bool = False):
+                 pairing: int = PAIR_HALF, fmt: int = FORMAT_V1, exact_codebooks: bool = False,
+                 bits_v: np.ndarray | None = None):
+        """bits_v [n_layers, H_kv, d_h/16] (V-side allocator, bgtq_layout_create_kv) replaces the uniform width b_v."""
         bits = np.ascontiguousarray(bits, dtype=np.uint8)
         assert bits.ndim == 3
         self.n_layers, self.n_kv_heads, _ = bits.shape
         self.n_q_heads, self.d_h, self.b_v = n_q_heads, d_h, b_v
         rot = np.ascontiguousarray(rotations, dtype=np.float32)
         h = C.c_void_p()
-        _check(_lib.bgtq_layout_create_format(bits.ctypes.data, self.n_layers, self.n_kv_heads, n_q_heads, d_h, b_v,
-                                              pairing, rot.ctypes.data, fmt | (CODEBOOK_EXACT if exact_codebooks else 0),
-                                              C.byref(h)))
+        flags = fmt | (CODEBOOK_EXACT if exact_codebooks else 0)
+        if bits_v is not None:
+            bits_v = np.ascontiguousarray(bits_v, dtype=np.uint8)
+            assert bits_v.shape == (self.n_layers, self.n_kv_heads, d_h // V_BLOCK)
+            _check(_lib.bgtq_layout_create_kv(bits.ctypes.data, bits_v.ctypes.data, self.n_layers, self.n_kv_heads,
+                                              n_q_heads, d_h, pairing, rot.ctypes.data, flags, C.byref(h)))
+        else:
+            _check(_lib.bgtq_layout_create_format(bits.ctypes.data, self.n_layers, self.n_kv_heads, n_q_heads, d_h, b_v,
+                                                  pairing, rot.ctypes.data, flags, C.byref(h)))
         self._h = h
         self.fmt = int(_lib.bgtq_layout_format(h)) & 0xFF
         self.exact_codebooks = bool(int(_lib.bgtq_layout_format(h)) & CODEBOOK_EXACT)

@@ -90,7 +90,8 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
                        const double *__restrict__ cb64, const float *__restrict__ rot_t, int batch,
                        int n_new, int Hkv, const int32_t *__restrict__ seq_len, int64_t n_cap,
                        int64_t max_tokens, const int32_t *__restrict__ pages, int pstride, int64_t n_pages,
-                       const float *__restrict__ rope_cos, const float *__restrict__ rope_sin, int pairing, int cb_exact)
+                       const float *__restrict__ rope_cos, const float *__restrict__ rope_sin, int pairing, int cb_exact,
+                       int max_rows)
 {
     extern __shared__ __align__(16) unsigned char smem[];
     const int tid = threadIdx.x;
@@ -105,15 +106,16 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
     // shared memory carve-up
     double *xs = reinterpret_cast<double *>(smem);                       // [16][256]
     double *tau = xs + kSub * 256;                                       // [512] thresholds (C_b at 2^b-1)
-    double *sigma = tau + 512;                                           // [16][9]
-    uint16_t *nrm = reinterpret_cast<uint16_t *>(sigma + kSub * 9);      // [16][9] (+pad)
-    uint8_t *idxs = reinterpret_cast<uint8_t *>(nrm + kSub * 9 + 8);     // [16][256]
+    double *sigma = tau + 512;                                           // [16][ns], ns = K groups + V groups of this head (<= max_rows)
+    uint16_t *nrm = reinterpret_cast<uint16_t *>(sigma + kSub * max_rows);   // [16][ns] (+pad)
+    uint8_t *idxs = reinterpret_cast<uint8_t *>(nrm + kSub * max_rows + 8);  // [16][256]
     UnitDesc *units = reinterpret_cast<UnitDesc *>(idxs + kSub * 256);   // [32]
     int *n_units_p = reinterpret_cast<int *>(units + kMaxUnits);
     HeadMeta *Msp = reinterpret_cast<HeadMeta *>(n_units_p + 4);         // this head's static metadata (kMetaBytes)
-    // exact-density codebooks: V has its own table C_{b_V, d_h} (256 more thresholds); else V shares the flat table
+    // exact-density codebooks: V has its own flat table (C_{w, m} of the V group of width w; 512 more thresholds); else V
+    // shares the flat table of K
     double *tauV_own = reinterpret_cast<double *>(reinterpret_cast<unsigned char *>(Msp) + kMetaBytes);
-    uint32_t *tbuf = reinterpret_cast<uint32_t *>(reinterpret_cast<unsigned char *>(Msp) + kMetaBytes + (cb_exact ? 256 * 8 : 0));   // tile, `stride` bytes
+    uint32_t *tbuf = reinterpret_cast<uint32_t *>(reinterpret_cast<unsigned char *>(Msp) + kMetaBytes + (cb_exact ? 512 * 8 : 0));   // tile, `stride` bytes
     // The metadata is read many times by single threads (unit list, group search, radii); one coalesced copy into
     // shared memory replaces those dependent global-memory round trips -- they dominated the one-token append.
     {
@@ -123,7 +125,8 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
     }
     __syncthreads();
     const HeadMeta &M = *Msp;
-    const int stride = M.tile_stride, ng = M.n_groups, kdim = M.kdim, b_v = M.b_v;
+    const int stride = M.tile_stride, ng = M.n_groups, kdim = M.kdim, b_v = M.b_v;     // (b_v: BGTQ-v2 packing only)
+    const int nvg = M.n_vgroups, ns = ng + nvg;
 
     uint8_t *gtile = PAGED ? cache + n_pages * ((int64_t)M.layer_prefix + M.head_prefix) + (int64_t)pages[(int64_t)s * pstride + tile] * stride
                            : cache + n_cap * ((int64_t)batch * M.layer_prefix + (int64_t)s * M.layer_sum + M.head_prefix) + tile * stride;
@@ -141,10 +144,10 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
         tau[i] = __dmul_rn(__dadd_rn(c0, c1), 0.5);
     }
     if (cb_exact) {
-        const double *cbV = cbK + 512 + ((1 << b_v) - 1);
-        for (int i = tid; i + 1 < (1 << b_v); i += kAppendThreads) tauV_own[i] = __dmul_rn(__dadd_rn(cbV[i], cbV[i + 1]), 0.5);
+        const double *cbV = cbK + 512;
+        for (int i = tid; i < 511; i += kAppendThreads) tauV_own[i] = __dmul_rn(__dadd_rn(cbV[i], cbV[i + 1 < 511 ? i + 1 : i]), 0.5);
     }
-    const double *tauV = cb_exact ? tauV_own : tau + ((1 << b_v) - 1);
+    const double *tauV = cb_exact ? tauV_own : tau;
     if (tid == 0) {  // list of half-step units of the K code section
         int n = 0, j = 0;
         for (int ks = 0; ks < (M.format == 2 ? 0 : M.n_ksteps); ++ks) {   // (BGTQ-v2 packs from M.chunks, step 5)
@@ -160,10 +163,13 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
     __syncthreads();
     const int n_units = *n_units_p;
 
-    // this thread's row of the rotation: col < kdim -> K group row, col >= 128 -> V row
+    // this thread's row of the rotation: col < kdim -> K group row, col >= 128 -> row of its V group (grouped V order)
     const int col = tid;
     int my_m = 0, my_r = 0, my_x0 = 0, my_g = 0, my_b = 0;
-    if (col >= 128) { my_m = kDh; my_r = col - 128; my_x0 = 128; my_g = ng; my_b = b_v; }
+    if (col >= 128) {
+        const int gv = M.vbg[(col - 128) >> 4];
+        my_m = 16 * M.vgcnt[gv]; my_x0 = 128 + 16 * M.vgstart[gv]; my_r = col - my_x0; my_g = ng + gv; my_b = M.vgb[gv];
+    }
     else if (col < kdim) {
         int g = 0;
         while (g + 1 < ng && col >= M.gstart[g + 1]) ++g;
@@ -172,7 +178,7 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
     const float *myrot = rot_t + rot_offset(my_m > 0 ? my_m : 2) + my_r;
     // gather source of column `col`: V coordinate col-128, or the K coordinate stored at grouped position col
     const T *g_src = col >= 128 ? v_new : k_new;
-    const int g_off = col >= 128 ? col - 128 : (col < kdim ? (int)M.coords[col] : -1);
+    const int g_off = col >= 128 ? 16 * M.vblk[(col - 128) >> 4] + (col & 15) : (col < kdim ? (int)M.coords[col] : -1);
     int g_part = -1, g_blk = 0;
     bool g_isb = false;
     if (ROPE && col < kdim) {               // RoPE partner of this K coordinate, its block and which member it is
@@ -187,7 +193,7 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
         const int64_t nlo = max(lo, base), nhi = min(hi, base + kSub);
         if (nlo >= nhi) continue;
         // ---- 1. gather the sub-batch: xs[tt][0..127] = K in grouped order, xs[tt][128..255] = V.  Thread c owns
-        //      column c (its source coordinate is fixed), so the kSub loads are independent and in flight together.
+        //      (grouped V order) column c (its source coordinate is fixed), so the kSub loads are independent and in flight together.
         {
             const int64_t row0 = ((((int64_t)lrel * batch + s) * n_new + (base - t0)) * Hkv + h) * kDh;
             const int64_t rstep = (int64_t)Hkv * kDh;
@@ -215,18 +221,18 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
         }
         __syncthreads();
         // ---- 2. radii: ss = fma chain, r = sqrt(ss), sigma = r / sqrt(m), h = fp16_rne_sat(r)
-        if (tid < kSub * (ng + 1) && base + tid / (ng + 1) >= nlo && base + tid / (ng + 1) < nhi) {
-            int tt = tid / (ng + 1), g = tid % (ng + 1);
-            int x0 = g < ng ? M.gstart[g] : 128, m = g < ng ? M.gm[g] : kDh;
+        if (tid < kSub * ns && base + tid / ns >= nlo && base + tid / ns < nhi) {
+            int tt = tid / ns, g = tid % ns;
+            int x0 = g < ng ? M.gstart[g] : 128 + 16 * M.vgstart[g - ng], m = g < ng ? M.gm[g] : 16 * M.vgcnt[g - ng];
             const double *x = xs + tt * 256 + x0;
             double ss = 0.0;
             for (int j = 0; j < m; ++j) ss = __fma_rn(x[j], x[j], ss);
             double r = __dsqrt_rn(ss);
-            sigma[tt * 9 + g] = __ddiv_rn(r, __dsqrt_rn((double)m));
+            sigma[tt * ns + g] = __ddiv_rn(r, __dsqrt_rn((double)m));
             __half hv = __double2half(r);
             uint16_t hb = __half_as_ushort(hv);
             if (r >= 65520.0) hb = 0x7BFF;
-            nrm[tt * 9 + g] = hb;
+            nrm[tt * ns + g] = hb;
         }
         // ---- 3. rotation: z[tt] = fma chain over k of Pi[r][k] * x_k (k ascending: the oracle's order).
         //      Rotation rows are read 4 at a time ahead of the chain; a single new token (decode-time
@@ -307,7 +313,7 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
         __syncthreads();
         // ---- 4. scalar quantise: idx = #{k : z > tau_k * sigma}; the predicate is monotone in k
         if (my_m > 0) {
-            const double *tb = col >= 128 ? tauV : tau + ((1 << my_b) - 1);
+            const double *tb = (col >= 128 ? tauV : tau) + ((1 << my_b) - 1);
             // the count is found bit by bit (always my_b probes), all kSub searches side by side so that the
             // dependent LDS -> DMUL -> DSETP chains of different tokens overlap; same count as any other search
             // because the predicate is monotone in k
@@ -316,7 +322,7 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
                 double zz = 0.0;
 #pragma unroll
                 for (int tt = 0; tt < kSub; ++tt) if (tt == tt_lo) zz = z[tt];
-                const double sg = sgp[tt_lo * 9];
+                const double sg = sgp[tt_lo * ns];
                 int a = 0;
                 for (int bit = my_b - 1; bit >= 0; --bit)
                     if (zz > __dmul_rn(tb[a + (1 << bit) - 1], sg)) a += 1 << bit;
@@ -331,7 +337,7 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
                     const int step = 1 << bit;
 #pragma unroll
                     for (int tt = 0; tt < 8; ++tt)
-                        if (z[t0h + tt] > __dmul_rn(tb[a[tt] + step - 1], sgp[(t0h + tt) * 9])) a[tt] += step;
+                        if (z[t0h + tt] > __dmul_rn(tb[a[tt] + step - 1], sgp[(t0h + tt) * ns])) a[tt] += step;
                 }
 #pragma unroll
                 for (int tt = 0; tt < 8; ++tt)
@@ -362,12 +368,12 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
                 uint32_t *wp = tbuf + ((M.vcode_off + ((d >> 5) * 4 + c) * b_v * 128) >> 2) + j * 32 + (d & 31);
                 *wp = (*wp & ~mask) | val;
             }
-            if (tid < kSub * (ng + 1)) {                                   // fp16 norms in natural token order
-                const int tt = tid / (ng + 1), g = tid % (ng + 1);
+            if (tid < kSub * ns) {                                         // fp16 norms in natural token order (one V group)
+                const int tt = tid / ns, g = tid % ns;
                 const int64_t tok = base + tt;
                 if (tok >= nlo && tok < nhi) {
                     const int off = g < ng ? M.knorm_off + 256 * g : M.vnorm_off;
-                    reinterpret_cast<uint16_t *>(reinterpret_cast<uint8_t *>(tbuf) + off)[i * kSub + tt] = nrm[tt * 9 + g];
+                    reinterpret_cast<uint16_t *>(reinterpret_cast<uint8_t *>(tbuf) + off)[i * kSub + tt] = nrm[tt * ns + g];
                 }
             }
             __syncthreads();
@@ -389,27 +395,28 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
                         put_field(wbase, lanes, U.b, i * 4 + p * 2 + q, idxs[tt * 256 + U.ustart + 2 * c + q]);
                 }
             } else {
-                const int v = it - kitems, unit = v >> 5, lane = v & 31;   // unit = 2J + rho
+                const int v = it - kitems, unit = v >> 5, lane = v & 31;   // unit = 2J' + rho, J' = grouped V block
                 const int gq = lane >> 2, c = lane & 3;
-                const int u = 16 * (unit >> 1) + 8 * (unit & 1) + gq;
-                uint32_t *wbase = tbuf + ((M.vcode_off + unit * 128 * b_v) >> 2) + lane;
+                const int u = 16 * (unit >> 1) + 8 * (unit & 1) + gq;      // grouped V coordinate
+                const int bw = M.vbw[unit >> 1];
+                uint32_t *wbase = tbuf + ((M.vboff[unit >> 1] + (unit & 1) * 128 * bw) >> 2) + lane;
                 for (int o = 0; o < 2; ++o)
                     for (int e = 0; e < 2; ++e) {
                         int tt = 8 * o + 2 * c + e;
                         int64_t tok = base + tt;
                         if (tok < nlo || tok >= nhi) continue;
-                        put_field(wbase, 32, b_v, i * 4 + o * 2 + e, idxs[tt * 256 + 128 + u]);
+                        put_field(wbase, 32, bw, i * 4 + o * 2 + e, idxs[tt * 256 + 128 + u]);
                     }
             }
         }
-        if (tid < kSub * (ng + 1)) {   // fp16 norms: token tau at entry (tau&7)*16 + (tau>>4)*2 + ((tau>>3)&1)
-            int tt = tid / (ng + 1), g = tid % (ng + 1);
+        if (tid < kSub * ns) {   // fp16 norms: token tau at entry (tau&7)*16 + (tau>>4)*2 + ((tau>>3)&1)
+            int tt = tid / ns, g = tid % ns;
             int64_t tok = base + tt;
             if (tok >= nlo && tok < nhi) {
                 int t128 = i * kSub + tt;
                 int slot = (t128 & 7) * 16 + (t128 >> 4) * 2 + ((t128 >> 3) & 1);
-                int off = g < ng ? M.knorm_off + 256 * g : M.vnorm_off;
-                reinterpret_cast<uint16_t *>(reinterpret_cast<uint8_t *>(tbuf) + off)[slot] = nrm[tt * 9 + g];
+                int off = g < ng ? M.knorm_off + 256 * g : M.vnorm_off + 256 * (g - ng);
+                reinterpret_cast<uint16_t *>(reinterpret_cast<uint8_t *>(tbuf) + off)[slot] = nrm[tt * ns + g];
             }
         }
         __syncthreads();
@@ -430,10 +437,10 @@ __global__ void advance_seq_len_kernel(int32_t *seq_len, int batch, int n_new, i
     }
 }
 
-static size_t append_smem_bytes(int max_stride, bool cb_exact = false)
+static size_t append_smem_bytes(int max_stride, int max_rows, bool cb_exact = false)
 {
-    return (size_t)kSub * 256 * 8 + 512 * 8 + kSub * 9 * 8 + (kSub * 9 + 8) * 2 + kSub * 256 +
-           kMaxUnits * sizeof(UnitDesc) + 16 + kMetaBytes + (cb_exact ? 256 * 8 : 0) + (size_t)max_stride + 64;
+    return (size_t)kSub * 256 * 8 + 512 * 8 + kSub * max_rows * 8 + (kSub * max_rows + 8) * 2 + kSub * 256 +
+           kMaxUnits * sizeof(UnitDesc) + 16 + kMetaBytes + (cb_exact ? 512 * 8 : 0) + (size_t)max_stride + 64;
 }
 
 int launch_quantize_append(const bgtq_layout *lay, int layer, int n_layers, void *cache, const void *k_new,
@@ -441,11 +448,11 @@ int launch_quantize_append(const bgtq_layout *lay, int layer, int n_layers, void
                            int advance, int64_t max_tokens, const PageMap *pm, const RopeTab *rope, cudaStream_t st)
 {
     const int64_t n_cap = (max_tokens + kTile - 1) / kTile;
-    const size_t smem = append_smem_bytes(lay->max_stride, lay->cb_exact != 0);
+    const size_t smem = append_smem_bytes(lay->max_stride, lay->max_rows, lay->cb_exact != 0);
     dim3 grid((n_new + kTile - 1) / kTile + 1, lay->n_kv_heads * n_layers, batch);
     const HeadMeta *metas = lay->d_meta + (size_t)layer * lay->n_kv_heads;
     if (first_use_on_device(1)) {   // once per device, outside any stream capture
-        const int maxs = (int)append_smem_bytes(16 * kDh * 8 + 256 * 9 + 16 * kDh * 8, true);
+        const int maxs = (int)append_smem_bytes(16 * kDh * 8 + 256 * 16 + 16 * kDh * 8, 16, true);
 #define BGTQ_APPEND_ATTR(T, R, G) CUDA_TRY(cudaFuncSetAttribute(quantize_append_kernel<T, R, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, maxs))
         BGTQ_APPEND_ATTR(float, false, false); BGTQ_APPEND_ATTR(__nv_bfloat16, false, false);
         BGTQ_APPEND_ATTR(float, true, false);  BGTQ_APPEND_ATTR(__nv_bfloat16, true, false);
@@ -463,7 +470,7 @@ int launch_quantize_append(const bgtq_layout *lay, int layer, int n_layers, void
         const double *cb = lay->cb_exact ? lay->d_hcb64 + (size_t)layer * lay->n_kv_heads * 1024 : lay->d_cb64;
         kern<<<grid, kAppendThreads, smem, st>>>(metas, (uint8_t *)cache, kp, vp, cb, lay->d_rot_t, batch, n_new,
                                                  lay->n_kv_heads, seq_len, n_cap, max_tokens, pt, pstride, n_pages, rc, rs,
-                                                 lay->pairing, lay->cb_exact);
+                                                 lay->pairing, lay->cb_exact, lay->max_rows);
     };
     if (dt == BGTQ_F32)
         launch(quantize_append_kernel<float, false, false>, quantize_append_kernel<float, true, false>,

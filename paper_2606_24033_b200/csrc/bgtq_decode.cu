@@ -390,7 +390,24 @@ __device__ __forceinline__ void pv_tile(const uint32_t *vcodes, int lane, const 
     }
 }
 
-template <int W, bool PAGED, bool EXACT>
+// PV of one 16-dimension V block (two units of width B): O0 += V^T[16 dims x 128 tokens] . P[128 tokens x 8 heads]
+template <int B, bool P5>
+__device__ __forceinline__ void pv_block(const uint32_t *u0, int lane, const uint32_t (&bP)[8][2],
+                                         const uint32_t *pools, const uint16_t *lut, float (&O0)[4])
+{
+    uint32_t w0[B], w1[B], h0[16], h1[16];
+    load_unit_full<B>(u0, lane, w0);
+    load_unit_full<B>(u0 + 32 * B, lane, w1);
+    decode_unit<B, P5>(w0, pools, lut, h0);
+    decode_unit<B, P5>(w1, pools, lut, h1);
+#pragma unroll
+    for (int kp = 0; kp < 8; ++kp)
+        mma16816(O0, h0[2 * kp], h1[2 * kp], h0[2 * kp + 1], h1[2 * kp + 1], bP[kp][0], bP[kp][1]);
+}
+
+// VG: heads may hold several V groups (V-side allocator, reading Q19): the accumulator and the partial record are in
+// GROUPED V order (block J' of the record = original block vblk[J']), every V group brings its own norm row and width.
+template <int W, bool PAGED, bool EXACT, bool VG>
 __global__ void __launch_bounds__(W * 32, 1)
 decode_kernel(const DecodeParams P)
 {
@@ -503,6 +520,12 @@ decode_kernel(const DecodeParams P)
             int ksb = 0;
             for (int g = 0; g < lane; ++g) ksb += (M.gm[g] + 15) >> 4;
             gdesc = (uint32_t)M.goff[lane] | ((uint32_t)(M.gm[lane] & 0xFF) << 16) | ((uint32_t)M.gb[lane] << 24) | ((uint32_t)ksb << 28);
+        }
+        // lane J' keeps the descriptor of grouped V block J': unit offset | width << 16 | V group << 20 | first of its group << 24
+        uint32_t vdesc = 0;
+        if (VG && lane < kMaxGroups) {
+            const int gv = M.vbg[lane];
+            vdesc = (uint32_t)M.vboff[lane] | ((uint32_t)M.vbw[lane] << 16) | ((uint32_t)gv << 20) | (M.vgstart[gv] == lane ? 1u << 24 : 0u);
         }
         const uint2 *qfp = reinterpret_cast<const uint2 *>(P.qf + (size_t)tp.pair * kQfHalves) + lane;
         const uint8_t *src = tile_src(tp, M);                     // current tile of this segment (advanced per tile)
@@ -630,7 +653,42 @@ decode_kernel(const DecodeParams P)
             vphase ^= 1;
             TS(6);
             uint32_t bP[8][2];
-            {
+            if constexpr (VG) {
+#pragma unroll 1
+                for (int Jg = 0; Jg < kMaxGroups; ++Jg) {
+                    const uint32_t d = __shfl_sync(0xFFFFFFFFu, vdesc, Jg);
+                    if (d >> 24) {                         // first block of a V group: P * (its norms) -> B fragments
+                        const uint4 *np = reinterpret_cast<const uint4 *>(tile + ((vnorm_off + 256 * ((d >> 20) & 0xF) + g8 * 32) >> 2));
+                        const uint4 n0 = np[0], n1 = np[1];
+                        const uint32_t nw[8] = {n0.x, n0.y, n0.z, n0.w, n1.x, n1.y, n1.z, n1.w};
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) {
+                            const float2 nf = __half22float2(*reinterpret_cast<const __half2 *>(&nw[i]));
+                            bP[i][0] = movmatrix_trans(pack_half2(Sc[i][0] * nf.x, Sc[i][1] * nf.x));
+                            bP[i][1] = movmatrix_trans(pack_half2(Sc[i][2] * nf.y, Sc[i][3] * nf.y));
+                        }
+                    }
+                    const uint32_t *u0 = tile + ((d & 0xFFFF) >> 2);
+                    switch ((d >> 16) & 0xF) {
+                    case 1: pv_block<1, P5>(u0, lane, bP, poolsV, lutV, O[0]); break;
+                    case 2: pv_block<2, P5>(u0, lane, bP, poolsV, lutV, O[0]); break;
+                    case 3: pv_block<3, P5>(u0, lane, bP, poolsV, lutV, O[0]); break;
+                    case 4: pv_block<4, P5>(u0, lane, bP, poolsV, lutV, O[0]); break;
+                    case 5: pv_block<5, P5>(u0, lane, bP, poolsV, lutV, O[0]); break;
+                    case 6: pv_block<6, P5>(u0, lane, bP, poolsV, lutV, O[0]); break;
+                    case 7: pv_block<7, P5>(u0, lane, bP, poolsV, lutV, O[0]); break;
+                    default: pv_block<8, P5>(u0, lane, bP, poolsV, lutV, O[0]); break;
+                    }
+                    // rotate the accumulator blocks: after the eight blocks O is back in grouped order
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        const float t0 = O[0][e];
+#pragma unroll
+                        for (int J = 0; J < 7; ++J) O[J][e] = O[J + 1][e];
+                        O[7][e] = t0;
+                    }
+                }
+            } else {
                 const uint4 *np = reinterpret_cast<const uint4 *>(tile + ((vnorm_off + g8 * 32) >> 2));
                 const uint4 n0 = np[0], n1 = np[1];
                 const uint32_t nw[8] = {n0.x, n0.y, n0.z, n0.w, n1.x, n1.y, n1.z, n1.w};
@@ -641,16 +699,18 @@ decode_kernel(const DecodeParams P)
                     bP[i][1] = movmatrix_trans(pack_half2(Sc[i][2] * nf.y, Sc[i][3] * nf.y));
                 }
             }
-            const uint32_t *vcodes = tile + (vcode_off >> 2);
-            switch (b_v) {
-            case 1: pv_tile<1, P5>(vcodes, lane, bP, poolsV, lutV, O); break;
-            case 2: pv_tile<2, P5>(vcodes, lane, bP, poolsV, lutV, O); break;
-            case 3: pv_tile<3, P5>(vcodes, lane, bP, poolsV, lutV, O); break;
-            case 4: pv_tile<4, P5>(vcodes, lane, bP, poolsV, lutV, O); break;
-            case 5: pv_tile<5, P5>(vcodes, lane, bP, poolsV, lutV, O); break;
-            case 6: pv_tile<6, P5>(vcodes, lane, bP, poolsV, lutV, O); break;
-            case 7: pv_tile<7, P5>(vcodes, lane, bP, poolsV, lutV, O); break;
-            default: pv_tile<8, P5>(vcodes, lane, bP, poolsV, lutV, O); break;
+            if constexpr (!VG) {
+                const uint32_t *vcodes = tile + (vcode_off >> 2);
+                switch (b_v) {
+                case 1: pv_tile<1, P5>(vcodes, lane, bP, poolsV, lutV, O); break;
+                case 2: pv_tile<2, P5>(vcodes, lane, bP, poolsV, lutV, O); break;
+                case 3: pv_tile<3, P5>(vcodes, lane, bP, poolsV, lutV, O); break;
+                case 4: pv_tile<4, P5>(vcodes, lane, bP, poolsV, lutV, O); break;
+                case 5: pv_tile<5, P5>(vcodes, lane, bP, poolsV, lutV, O); break;
+                case 6: pv_tile<6, P5>(vcodes, lane, bP, poolsV, lutV, O); break;
+                case 7: pv_tile<7, P5>(vcodes, lane, bP, poolsV, lutV, O); break;
+                default: pv_tile<8, P5>(vcodes, lane, bP, poolsV, lutV, O); break;
+                }
             }
             __syncwarp();
             TS(7);
@@ -723,7 +783,8 @@ decode_kernel(const DecodeParams P)
 __global__ void __launch_bounds__(128)
 combine_kernel(const float *__restrict__ partials, const int32_t *__restrict__ seq_len,
                const float *__restrict__ rot128, int n_layers, int batch, int Hkv, int G, int64_t n_cap,
-               int n_ctas, int W, __nv_bfloat16 *__restrict__ out, int n_sink = 0, int n_recent = 0, int win_slot = -1)
+               int n_ctas, int W, __nv_bfloat16 *__restrict__ out, int n_sink = 0, int n_recent = 0, int win_slot = -1,
+               const HeadMeta *__restrict__ metas = nullptr, const float *__restrict__ rot_base = nullptr)
 {
     constexpr int kMaxSlots = 1024;                     // 32 + n_ctas entries at most (host checks n_ctas)
     __shared__ int pre[kMaxBatch + 1];
@@ -814,6 +875,18 @@ combine_kernel(const float *__restrict__ partials, const int32_t *__restrict__ s
     __syncthreads();
     o[d] = ((red[0][d] + red[1][d]) + (red[2][d] + red[3][d])) / lsum;
     __syncthreads();
+    if (metas) {
+        // V-side groups (reading Q19): record position d is grouped V coordinate d.  Its group of m coordinates starts at
+        // s: out[coord(d)] = sum_j Pi^(m)[j][d - s] o[s + j] / sqrt(m), coord(d) = 16 * vblk[d >> 4] + (d & 15).
+        const HeadMeta &M = metas[l * Hkv + h];
+        const int gv = M.vbg[d >> 4], s = 16 * M.vgstart[gv], m = 16 * M.vgcnt[gv];
+        const float *R = rot_base + rot_offset(m) + (d - s);
+        float r = 0.f;
+#pragma unroll 16
+        for (int j = 0; j < m; ++j) r = fmaf(__ldg(R + j * m), o[s + j], r);
+        dst[16 * M.vblk[d >> 4] + (d & 15)] = __float2bfloat16(r / sqrtf((float)m));
+        return;
+    }
     if (rot128 == nullptr) { dst[d] = __float2bfloat16(o[d]); return; }    // fp16-cache comparison path: no rotation
     float r = 0.f;
 #pragma unroll 32
@@ -840,7 +913,8 @@ __device__ __forceinline__ bool window_slot_valid(int s, int64_t T, int n_sink, 
 __global__ void __launch_bounds__(128)
 window_kernel(const __half *__restrict__ win_k, const __half *__restrict__ win_v, const __nv_bfloat16 *__restrict__ q,
               const int32_t *__restrict__ seq_len, const float *__restrict__ rot128_t, float *__restrict__ partials,
-              int batch, int Hkv, int G, int64_t n_cap, int n_sink, int n_recent, float scale_log2e, int win_slot)
+              int batch, int Hkv, int G, int64_t n_cap, int n_sink, int n_recent, float scale_log2e, int win_slot,
+              const HeadMeta *__restrict__ metas = nullptr, const float *__restrict__ rot_t_base = nullptr)
 {
     __shared__ float lg[kMaxWindow];
     __shared__ float qs[kDh], o[kDh];
@@ -927,6 +1001,19 @@ window_kernel(const __half *__restrict__ win_k, const __half *__restrict__ win_v
     const float lsum = (red[0] + red[1]) + (red[2] + red[3]);
     o[d] = (part[d] + part[kDh + d]) + (part[2 * kDh + d] + part[3 * kDh + d]);
     __syncthreads();
+    if (metas) {
+        // V-side groups: the record is in grouped V order, each group rotated by its own Pi^(m) and scaled by sqrt(m):
+        // rec[s + r] = sqrt(m) sum_u Pi^(m)[r][u] o[coord(s + u)]  (the inverse of combine_kernel's per-group de-rotation)
+        const HeadMeta &M = metas[(lb / batch) * Hkv + h];
+        const int gv = M.vbg[d >> 4], s = 16 * M.vgstart[gv], m = 16 * M.vgcnt[gv];
+        const float *T = rot_t_base + rot_offset(m) + (d - s);
+        float r = 0.f;
+#pragma unroll 16
+        for (int u = 0; u < m; ++u) r = fmaf(__ldg(T + u * m), o[16 * M.vblk[(s + u) >> 4] + (u & 15)], r);
+        rec[2 + d] = r * sqrtf((float)m);
+        if (d == 0) { rec[0] = Mx; rec[1] = lsum; }
+        return;
+    }
     float r = 0.f;                                      // acc_rot[d] = sqrt(128) * sum_j Pi[d][j] o[j]; rot128_t[j][d] = Pi[d][j]
 #pragma unroll 32
     for (int j = 0; j < kDh; ++j) r = fmaf(__ldg(rot128_t + j * kDh + d), o[j], r);
@@ -1245,7 +1332,8 @@ int profile_decode_end(cudaStream_t st)
 }
 
 int launch_combine(const float *partials, const int32_t *seq_len, const float *rot128, int n_layers, int batch, int Hkv, int G,
-                   int64_t n_cap, int n_ctas, int W, void *out, int n_sink, int n_recent, int win_slot, bool pdl, cudaStream_t st)
+                   int64_t n_cap, int n_ctas, int W, void *out, int n_sink, int n_recent, int win_slot, bool pdl, cudaStream_t st,
+                   const HeadMeta *metas, const float *rot_base)
 {
     cudaLaunchConfig_t cfg = {};
     cudaLaunchAttribute at[1];
@@ -1254,7 +1342,7 @@ int launch_combine(const float *partials, const int32_t *seq_len, const float *r
     cfg.gridDim = dim3(n_layers * batch * Hkv * G); cfg.blockDim = dim3(128); cfg.dynamicSmemBytes = 0; cfg.stream = st;
     cfg.attrs = at; cfg.numAttrs = 1;
     cudaLaunchKernelEx(&cfg, combine_kernel, partials, seq_len, rot128, n_layers, batch, Hkv, G, n_cap, n_ctas, W,
-                       (__nv_bfloat16 *)out, n_sink, n_recent, win_slot);
+                       (__nv_bfloat16 *)out, n_sink, n_recent, win_slot, metas, rot_base);
     count_launch();
     CUDA_TRY(cudaGetLastError());
     return BGTQ_OK;
@@ -1262,20 +1350,21 @@ int launch_combine(const float *partials, const int32_t *seq_len, const float *r
 
 int launch_window(const void *win_k, const void *win_v, const void *q, const int32_t *seq_len, const float *rot128_t,
                   float *partials, int pairs, int batch, int Hkv, int G, int64_t n_cap, int n_sink, int n_recent,
-                  float scale_log2e, int win_slot, cudaStream_t st)
+                  float scale_log2e, int win_slot, cudaStream_t st, const HeadMeta *metas, const float *rot_t_base)
 {
     window_kernel<<<pairs * G, 128, 0, st>>>((const __half *)win_k, (const __half *)win_v, (const __nv_bfloat16 *)q, seq_len,
-                                             rot128_t, partials, batch, Hkv, G, n_cap, n_sink, n_recent, scale_log2e, win_slot);
+                                             rot128_t, partials, batch, Hkv, G, n_cap, n_sink, n_recent, scale_log2e, win_slot,
+                                             metas, rot_t_base);
     count_launch();
     CUDA_TRY(cudaGetLastError());
     return BGTQ_OK;
 }
 
-template <int W, bool PAGED, bool EXACT = false>
+template <int W, bool PAGED, bool EXACT = false, bool VG = false>
 static int launch_decode_w(const DecodeParams &P, int grid, size_t smem, cudaStream_t st)
 {
-    if (first_use_on_device(8 + (W / 2) * 4 + (PAGED ? 1 : 0) + (EXACT ? 2 : 0)))   // once per device, outside any stream capture
-        CUDA_TRY(cudaFuncSetAttribute(decode_kernel<W, PAGED, EXACT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - kStaticSmem));
+    if (first_use_on_device(8 + (W / 2) * 8 + (PAGED ? 1 : 0) + (EXACT ? 2 : 0) + (VG ? 4 : 0)))   // once per device, outside any stream capture
+        CUDA_TRY(cudaFuncSetAttribute(decode_kernel<W, PAGED, EXACT, VG>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - kStaticSmem));
     if (int rc = profile_decode_begin(st)) return rc;
     {
         cudaLaunchConfig_t cfg = {};
@@ -1284,13 +1373,13 @@ static int launch_decode_w(const DecodeParams &P, int grid, size_t smem, cudaStr
         at[0].val.programmaticStreamSerializationAllowed = g_prof ? 0 : 1;
         cfg.gridDim = dim3(grid); cfg.blockDim = dim3(W * 32); cfg.dynamicSmemBytes = smem; cfg.stream = st;
         cfg.attrs = at; cfg.numAttrs = 1;
-        cudaLaunchKernelEx(&cfg, decode_kernel<W, PAGED, EXACT>, P);
+        cudaLaunchKernelEx(&cfg, decode_kernel<W, PAGED, EXACT, VG>, P);
     }
     {
         cudaError_t le = cudaPeekAtLastError();
         if (le != cudaSuccess) {
             cudaFuncAttributes fa;
-            cudaFuncGetAttributes(&fa, decode_kernel<W, PAGED, EXACT>);
+            cudaFuncGetAttributes(&fa, decode_kernel<W, PAGED, EXACT, VG>);
             set_error(std::string("decode launch: ") + cudaGetErrorString(le) + " regs=" + std::to_string(fa.numRegs) + " maxthr=" + std::to_string(fa.maxThreadsPerBlock) + " static=" + std::to_string(fa.sharedSizeBytes) + " dyn=" + std::to_string(smem) + " maxdyn=" + std::to_string(fa.maxDynamicSharedSizeBytes));
             cudaGetLastError();
             return BGTQ_ECUDA;
@@ -1319,7 +1408,8 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
                  // two run side by side.  Completion order is kept by qfold_kernel's trailing griddepcontrol.wait:
                  // window -> qfold -> decode -> combine, each waiting for its predecessor only.
         if (int rc = launch_window(win->k, win->v, q, seq_len, lay->d_rot_t + rot_offset(kDh), partials, pairs, batch, Hkv, G, n_cap,
-                                   n_sink, n_recent, scale * 1.4426950408889634f, win_slot, st)) return rc;
+                                   n_sink, n_recent, scale * 1.4426950408889634f, win_slot, st,
+                                   lay->v_grouped ? metas : nullptr, lay->d_rot_t)) return rc;
     }
     if (win && !g_prof) {
         cudaLaunchConfig_t cfg = {};
@@ -1351,7 +1441,21 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
     const int grid = lay->sm_count;
     const size_t smem = decode_smem(W, buf_bytes);
     int rc;
-    if (lay->cb_exact) {
+    if (lay->v_grouped) {
+        if (pm) { set_error("bgtq_decode_attention_paged: not built for V-side groups"); return BGTQ_EINVAL; }
+        if (lay->cb_exact)
+            switch (W) {
+            case 12: rc = launch_decode_w<12, false, true, true>(P, grid, smem, st); break;
+            case 8: rc = launch_decode_w<8, false, true, true>(P, grid, smem, st); break;
+            default: rc = launch_decode_w<4, false, true, true>(P, grid, smem, st); break;
+            }
+        else
+            switch (W) {
+            case 12: rc = launch_decode_w<12, false, false, true>(P, grid, smem, st); break;
+            case 8: rc = launch_decode_w<8, false, false, true>(P, grid, smem, st); break;
+            default: rc = launch_decode_w<4, false, false, true>(P, grid, smem, st); break;
+            }
+    } else if (lay->cb_exact) {
         if (pm) { set_error("bgtq_decode_attention_paged: not built for exact-density codebooks"); return BGTQ_EINVAL; }
         switch (W) {
         case 12: rc = launch_decode_w<12, false, true>(P, grid, smem, st); break;
@@ -1376,7 +1480,7 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
     CUDA_TRY(cudaGetLastError());
 
     return launch_combine(partials, seq_len, lay->d_rot + rot_offset(kDh), n_layers, batch, Hkv, G, n_cap, grid, W, out, n_sink,
-                          n_recent, win_slot, !g_prof, st);
+                          n_recent, win_slot, !g_prof, st, lay->v_grouped ? metas : nullptr, lay->d_rot);
 }
 
 int launch_window_append(const void *k_new, const void *v_new, int dt, int n_layers, int batch, int n_new, int Hkv,

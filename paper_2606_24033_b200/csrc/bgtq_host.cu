@@ -118,9 +118,51 @@ extern "C" int bgtq_block_energy(const void *q, int64_t n_q, const void *k, int6
                                eq_out, ek_out, workspace, workspace_bytes, (cudaStream_t)stream);
 }
 
+extern "C" size_t bgtq_v_block_energy_workspace_bytes(int n_kv_heads, int d_h)
+{
+    if (n_kv_heads <= 0 || d_h <= 0) return 0;
+    return block_energy_ws_bytes(0, n_kv_heads, d_h);
+}
+
+extern "C" int bgtq_v_block_energy(const void *v, int64_t n, int dt, int n_kv_heads, int d_h, float *scores,
+                                   void *workspace, size_t workspace_bytes, void *stream)
+{
+    if (!scores || !workspace) FAIL(BGTQ_EINVAL, "bgtq_v_block_energy: null scores/workspace");
+    if (n <= 0 || !v) FAIL(BGTQ_EINVAL, "bgtq_v_block_energy: bad v/n");
+    if (dt != BGTQ_F32 && dt != BGTQ_BF16) FAIL(BGTQ_EINVAL, "bgtq_v_block_energy: dtype");
+    if (n_kv_heads <= 0) FAIL(BGTQ_EINVAL, "bgtq_v_block_energy: heads");
+    if (d_h <= 0 || d_h % BGTQ_V_BLOCK || d_h > 1024) FAIL(BGTQ_EINVAL, "bgtq_v_block_energy: d_h must be a multiple of 16, <= 1024");
+    if (workspace_bytes < block_energy_ws_bytes(0, n_kv_heads, d_h)) FAIL(BGTQ_EWORKSPACE, "bgtq_v_block_energy: workspace too small");
+    return launch_v_block_energy(v, n, dt, n_kv_heads, d_h, scores, workspace, (cudaStream_t)stream);
+}
+
 // ------------------------------------------------------------------ a3: layout build
 // Grouping, tile geometry and the k-step program of DESIGN.md section 4.
-static void build_head_meta(const uint8_t *bits, int d_h, int b_v, int pairing, HeadMeta &m)
+// V side (reading Q19): same-width groups of 16-coordinate V blocks, ascending width, member blocks ascending; one fp16
+// norm row per group, then the groups' code sections (two units of 128 * w bytes per block).  bits_v: 8 widths in 1..8.
+// Needs m.vnorm_off; sets everything after it.  All widths equal = the uniform layout of PAPER.md:27, byte for byte.
+static void build_v_side(const uint8_t *bits_v, HeadMeta &m)
+{
+    int nvg = 0, jg = 0;
+    for (int w = 1; w <= BGTQ_MAX_WIDTH; ++w) {
+        int cnt = 0;
+        for (int j = 0; j < kMaxGroups; ++j)
+            if (bits_v[j] == w) {
+                if (!cnt) { m.vgb[nvg] = (uint8_t)w; m.vgstart[nvg] = (uint8_t)jg; }
+                m.vblk[jg] = (uint8_t)j; m.vbg[jg] = (uint8_t)nvg; m.vbw[jg] = (uint8_t)w;
+                ++cnt; ++jg;
+            }
+        if (cnt) m.vgcnt[nvg++] = (uint8_t)cnt;
+    }
+    m.n_vgroups = (uint8_t)nvg;
+    m.b_v = m.vgb[0];
+    m.vcode_off = m.vnorm_off + 256 * nvg;
+    int off = m.vcode_off;
+    for (int j = 0; j < kMaxGroups; ++j) { m.vboff[j] = (uint16_t)off; off += 2 * 128 * m.vbw[j]; }
+    m.tile_stride = off;
+}
+
+static void build_head_meta(const uint8_t *bits, int d_h, int b_v, const uint8_t *bits_v, int pairing, HeadMeta &m)
 {
     std::memset(&m, 0, sizeof(m));
     const int L = d_h / 2;
@@ -168,8 +210,9 @@ static void build_head_meta(const uint8_t *bits, int d_h, int b_v, int pairing, 
     m.kcode_bytes = off;
     m.knorm_off = off;
     m.vnorm_off = off + 256 * ng;
-    m.vcode_off = m.vnorm_off + 256;
-    m.tile_stride = m.vcode_off + 16 * d_h * b_v;
+    uint8_t uni[kMaxGroups];
+    for (int j = 0; j < kMaxGroups; ++j) uni[j] = (uint8_t)b_v;
+    build_v_side(bits_v ? bits_v : uni, m);
 }
 
 // BGTQ-v2: words per lane of a chunk of r slots at width b
@@ -228,6 +271,9 @@ static void build_head_meta_v2(const uint8_t *bits, int d_h, int b_v, int pairin
     m.vnorm_off = m.knorm_off + 256 * ng;
     m.vcode_off = m.vnorm_off + 256;
     m.tile_stride = m.vcode_off + 16 * d_h * b_v;
+    m.n_vgroups = 1;                         // (row order keeps one V group: bits_v is a BGTQ-v1 feature)
+    m.vgb[0] = (uint8_t)b_v; m.vgcnt[0] = kMaxGroups;
+    for (int j = 0; j < kMaxGroups; ++j) { m.vblk[j] = (uint8_t)j; m.vbw[j] = (uint8_t)b_v; }
 }
 
 extern "C" int bgtq_layout_create(const uint8_t *bits, int n_layers, int n_kv_heads, int n_q_heads,
@@ -250,9 +296,32 @@ extern "C" int bgtq_codebook_exact(int b, int m, float *levels)
     return BGTQ_OK;
 }
 
+static int layout_create_impl(const uint8_t *bits, const uint8_t *bits_v, int n_layers, int n_kv_heads, int n_q_heads,
+                              int d_h, int b_v, int pairing, const float *rotations, int format, bgtq_layout **out);
+
 extern "C" int bgtq_layout_create_format(const uint8_t *bits, int n_layers, int n_kv_heads, int n_q_heads,
                                          int d_h, int b_v, int pairing, const float *rotations, int format,
                                          bgtq_layout **out)
+{
+    if (b_v < 1 || b_v > BGTQ_MAX_WIDTH) FAIL(BGTQ_EINVAL, "bgtq_layout_create: b_v in 1..8");
+    return layout_create_impl(bits, nullptr, n_layers, n_kv_heads, n_q_heads, d_h, b_v, pairing, rotations, format, out);
+}
+
+extern "C" int bgtq_layout_create_kv(const uint8_t *bits_k, const uint8_t *bits_v, int n_layers, int n_kv_heads,
+                                     int n_q_heads, int d_h, int pairing, const float *rotations, int format,
+                                     bgtq_layout **out)
+{
+    if (!bits_v) FAIL(BGTQ_EINVAL, "bgtq_layout_create_kv: null pointer");
+    if (d_h != kDh) FAIL(BGTQ_EINVAL, "bgtq_layout_create_kv: d_h must be 128");
+    if ((format & ~BGTQ_CODEBOOK_EXACT) != BGTQ_FORMAT_V1) FAIL(BGTQ_EINVAL, "bgtq_layout_create_kv: V-side widths are built for BGTQ_FORMAT_V1 layouts");
+    if (n_layers > 0 && n_kv_heads > 0)
+        for (size_t i = 0; i < (size_t)n_layers * n_kv_heads * (d_h / BGTQ_V_BLOCK); ++i)
+            if (bits_v[i] < 1 || bits_v[i] > BGTQ_MAX_WIDTH) FAIL(BGTQ_EINVAL, "bgtq_layout_create_kv: V widths must be 1..8");
+    return layout_create_impl(bits_k, bits_v, n_layers, n_kv_heads, n_q_heads, d_h, 0, pairing, rotations, format, out);
+}
+
+static int layout_create_impl(const uint8_t *bits, const uint8_t *bits_v, int n_layers, int n_kv_heads, int n_q_heads,
+                              int d_h, int b_v, int pairing, const float *rotations, int format, bgtq_layout **out)
 {
     if (!bits || !rotations || !out) FAIL(BGTQ_EINVAL, "bgtq_layout_create: null pointer");
     const int cb_exact = (format & BGTQ_CODEBOOK_EXACT) ? 1 : 0;
@@ -263,7 +332,6 @@ extern "C" int bgtq_layout_create_format(const uint8_t *bits, int n_layers, int 
     if (n_layers <= 0 || n_kv_heads <= 0 || n_q_heads <= 0 || n_q_heads % n_kv_heads)
         FAIL(BGTQ_EINVAL, "bgtq_layout_create: bad layer/head counts");
     if (n_q_heads / n_kv_heads > 8) FAIL(BGTQ_EINVAL, "bgtq_layout_create: GQA group size must be <= 8");
-    if (b_v < 1 || b_v > BGTQ_MAX_WIDTH) FAIL(BGTQ_EINVAL, "bgtq_layout_create: b_v in 1..8");
     if (pairing != BGTQ_PAIR_HALF && pairing != BGTQ_PAIR_INTERLEAVED) FAIL(BGTQ_EINVAL, "bgtq_layout_create: pairing");
     const int L = d_h / 2;
     for (size_t i = 0; i < (size_t)n_layers * n_kv_heads * L; ++i)
@@ -280,13 +348,18 @@ extern "C" int bgtq_layout_create_format(const uint8_t *bits, int n_layers, int 
     int64_t prefix = 0;
     lay->max_stride = 0;
     lay->max_chunks = 0;
+    lay->v_grouped = 0;
+    lay->max_rows = 1;
     for (int l = 0; l < n_layers; ++l) {
         int64_t lsum = 0;
         for (int h = 0; h < n_kv_heads; ++h) {
             HeadMeta &m = lay->meta[(size_t)l * n_kv_heads + h];
             if (format == BGTQ_FORMAT_V2) build_head_meta_v2(bits + ((size_t)l * n_kv_heads + h) * L, d_h, b_v, pairing, m);
-            else build_head_meta(bits + ((size_t)l * n_kv_heads + h) * L, d_h, b_v, pairing, m);
+            else build_head_meta(bits + ((size_t)l * n_kv_heads + h) * L, d_h, b_v,
+                                 bits_v ? bits_v + ((size_t)l * n_kv_heads + h) * kMaxGroups : nullptr, pairing, m);
             m.format = format;
+            if (m.n_vgroups > 1) lay->v_grouped = 1;
+            if (m.n_groups + m.n_vgroups > lay->max_rows) lay->max_rows = m.n_groups + m.n_vgroups;
             m.layer_prefix = prefix;
             m.head_prefix = lsum;
             lsum += m.tile_stride;
@@ -349,7 +422,7 @@ extern "C" int bgtq_layout_create_format(const uint8_t *bits, int n_layers, int 
                     }
                 };
                 if (side == 0) for (int g = 0; g < m.n_groups; ++g) put(m.gb[g], m.gm[g]);
-                else put(b_v, d_h);
+                else for (int g = 0; g < m.n_vgroups; ++g) put(m.vgb[g], 16 * m.vgcnt[g]);
                 uint32_t *pair = reinterpret_cast<uint32_t *>(t16 + 512);     // two adjacent 5-bit codes -> fp16x2
                 for (int i = 0; i < 1024; ++i) pair[i] = (uint32_t)t16[31 + (i & 31)] | ((uint32_t)t16[31 + (i >> 5)] << 16);
             }
@@ -517,7 +590,7 @@ extern "C" int bgtq_decode_attention_paged(const bgtq_layout *lay, int layer0, i
     if (layer0 < 0 || n_layers <= 0 || layer0 + n_layers > lay->n_layers) FAIL(BGTQ_EINVAL, "bgtq_decode_attention_paged: layer range");
     if (batch <= 0 || table_stride <= 0 || n_pages <= 0) FAIL(BGTQ_EINVAL, "bgtq_decode_attention_paged: batch/table_stride/n_pages");
     if (!(softmax_scale > 0.0f) || std::isinf(softmax_scale)) FAIL(BGTQ_EINVAL, "bgtq_decode_attention_paged: softmax_scale must be finite and > 0");
-    if (lay->cb_exact) FAIL(BGTQ_EINVAL, "bgtq_decode_attention_paged: not built for BGTQ_CODEBOOK_EXACT layouts");
+    if (lay->cb_exact || lay->v_grouped) FAIL(BGTQ_EINVAL, "bgtq_decode_attention_paged: not built for BGTQ_CODEBOOK_EXACT layouts or V-side groups");
     if (workspace_bytes < decode_ws_any(lay, batch, n_layers)) FAIL(BGTQ_EWORKSPACE, "bgtq_decode_attention_paged: workspace too small");
     const PageMap pm{page_table, table_stride, n_pages};
     return launch_decode_any(lay, layer0, n_layers, cache, q, seq_len, batch, (int64_t)table_stride * kTile, softmax_scale,
@@ -625,7 +698,7 @@ extern "C" int bgtq_prefill_attention(const bgtq_layout *lay, int layer, const v
 {
     if (!lay || !cache || !q || !seq_len || !out || !workspace) FAIL(BGTQ_EINVAL, "bgtq_prefill_attention: null pointer");
     if (layer < 0 || layer >= lay->n_layers) FAIL(BGTQ_EINVAL, "bgtq_prefill_attention: layer out of range");
-    if (lay->format != BGTQ_FORMAT_V1 || lay->cb_exact) FAIL(BGTQ_EINVAL, "bgtq_prefill_attention: built for BGTQ_FORMAT_V1 layouts with the shared codebooks only");
+    if (lay->format != BGTQ_FORMAT_V1 || lay->cb_exact || lay->v_grouped) FAIL(BGTQ_EINVAL, "bgtq_prefill_attention: built for BGTQ_FORMAT_V1 layouts with the shared codebooks and one V group per head only");
     if (batch <= 0 || n_q <= 0 || max_tokens <= 0 || n_q > max_tokens) FAIL(BGTQ_EINVAL, "bgtq_prefill_attention: batch/n_q/max_tokens");
     if (!(softmax_scale > 0.0f) || std::isinf(softmax_scale)) FAIL(BGTQ_EINVAL, "bgtq_prefill_attention: softmax_scale");
     return launch_prefill(lay, layer, cache, q, seq_len, batch, n_q, max_tokens, softmax_scale, out, workspace,

@@ -47,21 +47,35 @@ struct HeadMeta {
     uint16_t gstart[kMaxGroups];   // first grouped-order coordinate of the group
     uint8_t gb[kMaxGroups];        // width of the group
     uint8_t coords[kDh];           // grouped order -> original coordinate (Q9)
+    // V side (reading Q19): same-width groups of 16-coordinate V blocks, ascending width; a uniform V width is one group of
+    // all 8 blocks.  "Grouped block" J' = position of a block in the grouped order (the order of the accumulator and of the
+    // V code section); the tile holds one fp16 norm row per V group at vnorm_off + 256 * gv.
+    uint8_t n_vgroups, vpad[3];
+    uint8_t vgb[kMaxGroups];       // width of V group gv
+    uint8_t vgcnt[kMaxGroups];     // blocks in the group (m = 16 * vgcnt)
+    uint8_t vgstart[kMaxGroups];   // first grouped block of the group
+    uint8_t vblk[kMaxGroups];      // grouped block -> original block (coordinates 16 * vblk .. + 15)
+    uint8_t vbg[kMaxGroups];       // grouped block -> V group
+    uint8_t vbw[kMaxGroups];       // grouped block -> width
+    uint16_t vboff[kMaxGroups];    // grouped block -> byte offset of its first unit inside the tile
     union {
         KStep ksteps[kMaxKSteps];  // v1
         Chunk2 chunks[kMaxKSteps]; // v2 (kMaxChunks used); kcode_bytes = 4 * (bytes of one quadrant)
     };
 };
 static_assert(sizeof(KStep) == 8 && sizeof(Chunk2) == 8, "k-step / chunk descriptors are 8 bytes");
+static_assert(kDh / 16 == kMaxGroups, "eight V blocks of 16 coordinates");
 
 }  // namespace bgtq
 
 struct bgtq_layout {
-    int n_layers, n_kv_heads, n_q_heads, d_h, b_v, pairing;
+    int n_layers, n_kv_heads, n_q_heads, d_h, b_v, pairing;     // b_v: the uniform V width, 0 when widths come from bits_v
+    int v_grouped;                        // 1 when some head has more than one V group (V-side allocator, reading Q19)
     int format;                           // 1 = BGTQ-v1 (fragment order), 2 = BGTQ-v2 (row order)
     uint8_t *d_planes;                    // v2: e4m3 byte planes of the codebooks, see codebook_planes()
     float kappa[9];                       // v2: plane scale of width b
     int max_stride;                       // largest tile stride over all heads
+    int max_rows;                         // largest number of norm rows (K groups + V groups) over all heads
     int max_chunks;                       // v2: largest number of K chunks over all heads
     std::vector<bgtq::HeadMeta> meta;     // host copy, [layer][kv_head]
     int64_t total_stride_sum;             // sum of tile strides over all (layer, head)
@@ -128,6 +142,7 @@ int launch_block_energy(const void *q, int64_t n_q, const void *k, int64_t n_k, 
                         int Hkv, int d_h, int pairing, int kind, float *scores, float *eq_out,
                         float *ek_out, void *ws, size_t ws_bytes, cudaStream_t st);
 size_t block_energy_ws_bytes(int Hq, int Hkv, int d_h);
+int launch_v_block_energy(const void *v, int64_t n, int dt, int Hkv, int d_h, float *scores, void *ws, cudaStream_t st);
 int launch_allocate(const float *scores, int n_heads, int L, int b_min, int b_max, int B,
                     uint8_t *bits, cudaStream_t st);
 int debug_decode_unit_exact(int b, int m, const uint32_t *words, float *values);

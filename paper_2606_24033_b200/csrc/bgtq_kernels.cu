@@ -179,6 +179,42 @@ int launch_block_energy(const void *q, int64_t n_q, const void *k, int64_t n_k, 
     return BGTQ_OK;
 }
 
+// V-side score (reading Q19): s^V[h][j] = mean_t ||v_t^(j)||^2 over the 16 coordinates of V block j.  Same two passes:
+// the streaming pass above, then one CTA per (kv head, block) reduces its 16 columns' partials in fp64, fixed order.
+__global__ void __launch_bounds__(128)
+energy_final_v_kernel(const float *__restrict__ pv, int cv, int64_t n, int Hkv, int d_h, float *__restrict__ scores)
+{
+    const int nb = d_h / BGTQ_V_BLOCK;
+    const int h = blockIdx.x / nb, j = blockIdx.x % nb;
+    double sv = 0.0;
+    for (int c = threadIdx.x; c < cv; c += 128) {
+        const float *row = pv + ((int64_t)c * Hkv + h) * d_h + BGTQ_V_BLOCK * j;
+#pragma unroll
+        for (int u = 0; u < BGTQ_V_BLOCK; ++u) sv += (double)row[u];
+    }
+    __shared__ double s1[128];
+    s1[threadIdx.x] = sv;
+    __syncthreads();
+    for (int w = 64; w > 0; w >>= 1) {
+        if (threadIdx.x < w) s1[threadIdx.x] += s1[threadIdx.x + w];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) scores[h * nb + j] = (float)(s1[0] / (double)n);
+}
+
+int launch_v_block_energy(const void *v, int64_t n, int dt, int Hkv, int d_h, float *scores, void *ws, cudaStream_t st)
+{
+    float *pv = (float *)ws;
+    const int cv = energy_chunks(n), rv = Hkv * d_h;
+    dim3 grid(cv, (rv / 8 + kEnergyThreads - 1) / kEnergyThreads);
+    if (dt == BGTQ_F32) energy_partial_kernel<float><<<grid, kEnergyThreads, 0, st>>>((const float *)v, n, rv, cv, pv);
+    else energy_partial_kernel<__nv_bfloat16><<<grid, kEnergyThreads, 0, st>>>((const __nv_bfloat16 *)v, n, rv, cv, pv);
+    energy_final_v_kernel<<<Hkv * (d_h / BGTQ_V_BLOCK), 128, 0, st>>>(pv, cv, n, Hkv, d_h, scores);
+    count_launch(2);
+    CUDA_TRY(cudaGetLastError());
+    return BGTQ_OK;
+}
+
 // ============================================================================ a2: Alg. 1 on the device
 // One warp per head.  Each lane scans blocks lane, lane+32, ...; the warp arg-max
 // takes the largest key, ties to the smallest index (Q4).  key = 3/4 * s * 4^-b, exact in fp64.
