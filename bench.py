@@ -261,10 +261,11 @@ def build_workload(args, P, torch, device, seed_shift: int = 0):
         k = torch.cat(ks) if len(ks) > 1 else ks[0]
         qcal = GS.layer_queries(seed_of(l, 0), shp.n_cal, Hq, scales, d, shp.rope_base, 0, device, tag=4)
         if l == 0:
-            P.block_energy(qcal, k)                               # warm-up (allocator, caches)
+            ews = P.block_energy_workspace(Hq, Hkv, d, device)    # caller-owned scratch, reused by every layer
+            P.block_energy(qcal, k, workspace=ews)                # warm-up (module load, caches)
         e0, e1 = ev(), ev()
         e0.record()
-        scores.append(P.block_energy(qcal, k))
+        scores.append(P.block_energy(qcal, k, workspace=ews))
         e1.record()
         torch.cuda.synchronize()
         t_energy += e0.elapsed_time(e1)

@@ -196,8 +196,13 @@ def codebook_exact(b: int, m: int) -> np.ndarray:
     return out
 
 
+def block_energy_workspace(n_q_heads: int, n_kv_heads: int, d_h: int, device="cuda") -> torch.Tensor:
+    """Caller-owned scratch for block_energy / v_block_energy (reusable across calls)."""
+    return torch.empty(int(_lib.bgtq_block_energy_workspace_bytes(n_q_heads, n_kv_heads, d_h)), dtype=torch.uint8, device=device)
+
+
 def block_energy(q: torch.Tensor, k: torch.Tensor, pairing: int = PAIR_HALF, kind: int = QK_AVG,
-                 return_parts: bool = False):
+                 return_parts: bool = False, workspace: Optional[torch.Tensor] = None):
     """bgtq_block_energy.  q [N_q, H_q, d_h], k [N_k, H_kv, d_h] (CUDA, same dtype) ->
     scores [H_kv, d_h/2] float32 (and Eq, Ek)."""
     nq, Hq, d = q.shape
@@ -208,7 +213,8 @@ def block_energy(q: torch.Tensor, k: torch.Tensor, pairing: int = PAIR_HALF, kin
     eq = torch.empty_like(scores) if return_parts else None
     ek = torch.empty_like(scores) if return_parts else None
     nws = int(_lib.bgtq_block_energy_workspace_bytes(Hq, Hkv, d))
-    ws = torch.empty(nws, dtype=torch.uint8, device=k.device)
+    ws = workspace if workspace is not None else torch.empty(nws, dtype=torch.uint8, device=k.device)
+    nws = ws.numel()
     _check(_lib.bgtq_block_energy(_dev(q) if nq else None, nq, _dev(k) if nk else None, nk, _dt(k), Hq, Hkv, d,
                                   pairing, kind, _dev(scores), _dev(eq) if return_parts else None,
                                   _dev(ek) if return_parts else None, _dev(ws), nws, _stream()))
@@ -218,12 +224,13 @@ def block_energy(q: torch.Tensor, k: torch.Tensor, pairing: int = PAIR_HALF, kin
 V_BLOCK = 16
 
 
-def v_block_energy(v: torch.Tensor) -> torch.Tensor:
+def v_block_energy(v: torch.Tensor, workspace: Optional[torch.Tensor] = None) -> torch.Tensor:
     """bgtq_v_block_energy.  v [N, H_kv, d_h] (CUDA) -> V-side scores [H_kv, d_h/16] float32."""
     n, Hkv, d = v.shape
     scores = torch.empty((Hkv, d // V_BLOCK), dtype=torch.float32, device=v.device)
     nws = int(_lib.bgtq_v_block_energy_workspace_bytes(Hkv, d))
-    ws = torch.empty(nws, dtype=torch.uint8, device=v.device)
+    ws = workspace if workspace is not None else torch.empty(nws, dtype=torch.uint8, device=v.device)
+    nws = ws.numel()
     _check(_lib.bgtq_v_block_energy(_dev(v), n, _dt(v), Hkv, d, _dev(scores), _dev(ws), nws, _stream()))
     return scores
 

@@ -1,5 +1,6 @@
 // bgtq_kernels.cu -- block-energy reduction (a1), device allocator (a2), quantize-on-append (a4).
 // Hand-written CUDA for sm_100a.  Shares nothing with oracle/.
+#include <cooperative_groups.h>
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
 
@@ -10,9 +11,9 @@ namespace bgtq {
 #define CUDA_TRY(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) return cuda_fail(e_, #expr); } while (0)
 
 // ============================================================================ a1: block energy
-// Eq. 4: two plain means of squared block norms.  Pass 1 streams the activations once
-// (HBM-bound, 16-byte loads, fp32 partial sums over <= ~N/512 tokens per column), pass 2 reduces the
-// partials in fp64 in a fixed order and applies the score kind.
+// Eq. 4: two plain means of squared block norms, ONE cooperative launch.  Phase 1 streams the activations
+// once (HBM-bound, 16-byte loads, fp32 partial sums over <= ~N/512 tokens per column), phase 2 (after a grid-wide barrier)
+// reduces the partials in fp64 in a fixed order and applies the score kind.
 constexpr int kEnergyMaxChunks = 512;
 constexpr int kEnergyThreads = 256;
 
@@ -33,21 +34,19 @@ __device__ __forceinline__ void load8(const __nv_bfloat16 *p, float v[8])
     }
 }
 
+// one work item of pass 1: token chunk c of a tensor with rows of row_elems elements, column slab `slab`
 template <typename T>
-__global__ void __launch_bounds__(kEnergyThreads)
-energy_partial_kernel(const T *__restrict__ x, int64_t n, int row_elems, int n_chunks,
-                      float *__restrict__ partial)
+__device__ __forceinline__ void energy_partial_item(const T *__restrict__ x, int64_t n, int row_elems, int n_chunks, int c,
+                                                    int slab, float *__restrict__ partial, float *red)
 {
     // A row (one token, all heads) is row_elems/8 threads wide; when that is narrower than the CTA the spare
     // threads take other tokens of the chunk (token lanes) and a fixed-order shared-memory reduction joins them.
-    __shared__ float red[kEnergyThreads * 8];
     const int row_threads = row_elems / 8;
     const int ct = row_threads < kEnergyThreads ? row_threads : kEnergyThreads;   // column threads in this CTA
     const int TS = kEnergyThreads / ct;                                            // token lanes
     const int tsub = threadIdx.x / ct, cidx = threadIdx.x % ct;
-    const int col0 = (blockIdx.y * ct + cidx) * 8;
+    const int col0 = (slab * ct + cidx) * 8;
     const bool active = tsub < TS && col0 < row_elems;
-    const int c = blockIdx.x;
     const int64_t per = (n + n_chunks - 1) / n_chunks;
     const int64_t t_lo = c * per, t_hi = min(n, t_lo + per);
     float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
@@ -74,6 +73,7 @@ energy_partial_kernel(const T *__restrict__ x, int64_t n, int row_elems, int n_c
         }
     }
     if (TS > 1) {
+        __syncthreads();                               // (red may still be read by the previous item)
 #pragma unroll
         for (int e = 0; e < 8; ++e) red[threadIdx.x * 8 + e] = acc[e];
         __syncthreads();
@@ -90,50 +90,84 @@ energy_partial_kernel(const T *__restrict__ x, int64_t n, int row_elems, int n_c
     }
 }
 
-// one CTA of 128 threads per (kv head h, block i): fixed-order fp64 reduction of the partials
-__global__ void __launch_bounds__(128)
-energy_final_kernel(const float *__restrict__ pq, int cq, int64_t n_q, const float *__restrict__ pk,
-                    int ck, int64_t n_k, int Hq, int Hkv, int d_h, int pairing, int kind,
-                    float *__restrict__ scores, float *__restrict__ eq_out, float *__restrict__ ek_out)
+struct EnergyParams {
+    const void *q, *k;                 // k: the keys, or the values for the V-side score (v_mode)
+    int64_t n_q, n_k;
+    int rq, rk, cq, ck, sq, sk;        // row elements, token chunks, column slabs per chunk
+    float *pq, *pk;
+    int Hq, Hkv, d_h, pairing, kind, v_mode;
+    float *scores, *eq_out, *ek_out;
+};
+
+// ONE launch (cooperative: all CTAs are resident).  Phase 1: the work items (tensor, token chunk, column slab) of q and k
+// are dealt round-robin to the CTAs; grid-wide barrier; phase 2: output (kv head, block) o is reduced by CTA o mod grid
+// from the partials in fp64, in a fixed order, and the score kind is applied.
+template <typename T>
+__global__ void __launch_bounds__(kEnergyThreads)
+energy_kernel(const EnergyParams P)
 {
-    const int L = d_h / 2, G = Hq / Hkv;
-    const int h = blockIdx.x / L, i = blockIdx.x % L;
-    const int a = pairing == BGTQ_PAIR_HALF ? i : 2 * i;
-    const int b = pairing == BGTQ_PAIR_HALF ? i + L : 2 * i + 1;
-    double sq = 0.0, sk = 0.0;
-    if (n_q > 0)
-        for (int c = threadIdx.x; c < cq; c += 128)
-            for (int g = h * G; g < h * G + G; ++g) {
-                const float *row = pq + ((int64_t)c * Hq + g) * d_h;
-                sq += (double)row[a] + (double)row[b];
-            }
-    if (n_k > 0)
-        for (int c = threadIdx.x; c < ck; c += 128) {
-            const float *row = pk + ((int64_t)c * Hkv + h) * d_h;
-            sk += (double)row[a] + (double)row[b];
-        }
-    __shared__ double s1[128], s2[128];
-    s1[threadIdx.x] = sq;
-    s2[threadIdx.x] = sk;
-    __syncthreads();
-    for (int w = 64; w > 0; w >>= 1) {
-        if (threadIdx.x < w) { s1[threadIdx.x] += s1[threadIdx.x + w]; s2[threadIdx.x] += s2[threadIdx.x + w]; }
-        __syncthreads();
+    __shared__ float red[kEnergyThreads * 8];
+    const int items_q = P.n_q > 0 ? P.cq * P.sq : 0, items_k = P.n_k > 0 ? P.ck * P.sk : 0;
+    // the large tensor first: its items are the long ones
+    for (int it = blockIdx.x; it < items_q + items_k; it += gridDim.x) {
+        if (it < items_k) energy_partial_item<T>((const T *)P.k, P.n_k, P.rk, P.ck, it / P.sk, it % P.sk, P.pk, red);
+        else { const int j = it - items_k; energy_partial_item<T>((const T *)P.q, P.n_q, P.rq, P.cq, j / P.sq, j % P.sq, P.pq, red); }
     }
-    if (threadIdx.x == 0) {
-        double eq = n_q > 0 ? s1[0] / ((double)n_q * (double)G) : 0.0;
-        double ek = n_k > 0 ? s2[0] / (double)n_k : 0.0;
-        double s;
-        switch (kind) {
-        case BGTQ_QK_AVG: s = 0.5 * (eq + ek); break;
-        case BGTQ_QK_MAX: s = eq > ek ? eq : ek; break;
-        case BGTQ_QK_PRODUCT: s = sqrt(eq * ek); break;
-        case BGTQ_K_ONLY: s = ek; break;
-        default: s = eq; break;
+    __threadfence();
+    cooperative_groups::this_grid().sync();
+    double *s1 = reinterpret_cast<double *>(red), *s2 = s1 + kEnergyThreads;
+    const int d_h = P.d_h, L = d_h / 2, G = P.v_mode ? 1 : P.Hq / P.Hkv;
+    const int nb = P.v_mode ? d_h / BGTQ_V_BLOCK : L;
+    for (int o = blockIdx.x; o < P.Hkv * nb; o += gridDim.x) {
+        const int h = o / nb, i = o % nb;
+        double sq = 0.0, sk = 0.0;
+        if (P.v_mode) {
+            for (int c = threadIdx.x; c < P.ck; c += kEnergyThreads) {
+                const float *row = P.pk + ((int64_t)c * P.Hkv + h) * d_h + BGTQ_V_BLOCK * i;
+#pragma unroll
+                for (int u = 0; u < BGTQ_V_BLOCK; ++u) sk += (double)__ldcg(row + u);
+            }
+        } else {
+            const int a = P.pairing == BGTQ_PAIR_HALF ? i : 2 * i;
+            const int b = P.pairing == BGTQ_PAIR_HALF ? i + L : 2 * i + 1;
+            if (P.n_q > 0)
+                for (int c = threadIdx.x; c < P.cq; c += kEnergyThreads)
+                    for (int g = h * G; g < h * G + G; ++g) {
+                        const float *row = P.pq + ((int64_t)c * P.Hq + g) * d_h;
+                        sq += (double)__ldcg(row + a) + (double)__ldcg(row + b);
+                    }
+            if (P.n_k > 0)
+                for (int c = threadIdx.x; c < P.ck; c += kEnergyThreads) {
+                    const float *row = P.pk + ((int64_t)c * P.Hkv + h) * d_h;
+                    sk += (double)__ldcg(row + a) + (double)__ldcg(row + b);
+                }
         }
-        scores[h * L + i] = (float)s;
-        if (eq_out) eq_out[h * L + i] = (float)eq;
-        if (ek_out) ek_out[h * L + i] = (float)ek;
+#pragma unroll
+        for (int w = 16; w > 0; w >>= 1) { sq += __shfl_xor_sync(0xffffffffu, sq, w); sk += __shfl_xor_sync(0xffffffffu, sk, w); }
+        __syncthreads();
+        if ((threadIdx.x & 31) == 0) { s1[threadIdx.x >> 5] = sq; s2[threadIdx.x >> 5] = sk; }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            sq = 0.0; sk = 0.0;
+            for (int w = 0; w < kEnergyThreads / 32; ++w) { sq += s1[w]; sk += s2[w]; }
+            s1[0] = sq; s2[0] = sk;
+        }
+        if (threadIdx.x == 0) {
+            if (P.v_mode) { P.scores[o] = (float)(s2[0] / (double)P.n_k); continue; }
+            const double eq = P.n_q > 0 ? s1[0] / ((double)P.n_q * (double)G) : 0.0;
+            const double ek = P.n_k > 0 ? s2[0] / (double)P.n_k : 0.0;
+            double s;
+            switch (P.kind) {
+            case BGTQ_QK_AVG: s = 0.5 * (eq + ek); break;
+            case BGTQ_QK_MAX: s = eq > ek ? eq : ek; break;
+            case BGTQ_QK_PRODUCT: s = sqrt(eq * ek); break;
+            case BGTQ_K_ONLY: s = ek; break;
+            default: s = eq; break;
+            }
+            P.scores[o] = (float)s;
+            if (P.eq_out) P.eq_out[o] = (float)eq;
+            if (P.ek_out) P.ek_out[o] = (float)ek;
+        }
     }
 }
 
@@ -142,77 +176,72 @@ size_t block_energy_ws_bytes(int Hq, int Hkv, int d_h)
     return (size_t)kEnergyMaxChunks * (size_t)(Hq + Hkv) * d_h * sizeof(float);
 }
 
-static int energy_chunks(int64_t n)
+static int energy_chunks(int64_t n, int row_elems, int max_chunks = kEnergyMaxChunks)
 {
-    int64_t c = (n + 31) / 32;
-    if (c > kEnergyMaxChunks) c = kEnergyMaxChunks;
+    // a chunk gives each of its threads four tokens (one round of four loads in flight); more tokens per chunk only when
+    // the chunk count is capped.  Wide rows (queries: one thread column per 8 elements, no token lanes) get short chunks,
+    // so a few hundred calibration tokens still spread over the whole GPU instead of eight CTAs walking 32 rows each.
+    const int row_threads = row_elems / 8;
+    const int ct = row_threads < kEnergyThreads ? (row_threads > 0 ? row_threads : 1) : kEnergyThreads;
+    const int min_per = 4 * (kEnergyThreads / ct);
+    int64_t c = (n + min_per - 1) / min_per;
+    if (c > max_chunks) c = max_chunks;
     if (c < 1) c = 1;
     // make every chunk non-empty: per = ceil(n/c) tokens, chunks = ceil(n/per)
     if (n > 0) { int64_t per = (n + c - 1) / c; c = (n + per - 1) / per; }
     return (int)c;
 }
 
+static int launch_energy(EnergyParams &P, int dt, cudaStream_t st, int max_chunks = kEnergyMaxChunks)
+{
+    static int blocks_per_sm[64][2] = {};          // occupancy of the two instantiations per device (cooperative grid size)
+    int dev = 0, sms = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const int ti = dt == BGTQ_F32 ? 0 : 1;
+    if (dev < 64 && blocks_per_sm[dev][ti] == 0) {
+        int nb = 0;
+        if (ti == 0) CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, energy_kernel<float>, kEnergyThreads, 0));
+        else CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, energy_kernel<__nv_bfloat16>, kEnergyThreads, 0));
+        blocks_per_sm[dev][ti] = nb < 1 ? 1 : (nb > 4 ? 4 : nb);
+    }
+    P.cq = energy_chunks(P.n_q, P.rq, max_chunks); P.ck = energy_chunks(P.n_k, P.rk, max_chunks);
+    P.sq = (P.rq / 8 + kEnergyThreads - 1) / kEnergyThreads;       // narrow rows: one slab, spare threads take tokens
+    P.sk = (P.rk / 8 + kEnergyThreads - 1) / kEnergyThreads;
+    if (P.sq < 1) P.sq = 1;
+    if (P.sk < 1) P.sk = 1;
+    const int items = (P.n_q > 0 ? P.cq * P.sq : 0) + (P.n_k > 0 ? P.ck * P.sk : 0);
+    const int outs = P.Hkv * (P.v_mode ? P.d_h / BGTQ_V_BLOCK : P.d_h / 2);
+    int grid = sms * (dev < 64 ? blocks_per_sm[dev][ti] : 1);
+    const int want = items > outs ? items : outs;
+    if (grid > want) grid = want;
+    void *args[] = {&P};
+    if (dt == BGTQ_F32) CUDA_TRY(cudaLaunchCooperativeKernel((const void *)energy_kernel<float>, dim3(grid), dim3(kEnergyThreads), args, 0, st));
+    else CUDA_TRY(cudaLaunchCooperativeKernel((const void *)energy_kernel<__nv_bfloat16>, dim3(grid), dim3(kEnergyThreads), args, 0, st));
+    count_launch();
+    return BGTQ_OK;
+}
+
 int launch_block_energy(const void *q, int64_t n_q, const void *k, int64_t n_k, int dt, int Hq,
                         int Hkv, int d_h, int pairing, int kind, float *scores, float *eq_out,
                         float *ek_out, void *ws, size_t, cudaStream_t st)
 {
-    float *pq = (float *)ws;
-    float *pk = pq + (size_t)kEnergyMaxChunks * Hq * d_h;
-    const int cq = energy_chunks(n_q), ck = energy_chunks(n_k);
-    const int rq = Hq * d_h, rk = Hkv * d_h;
-    if (n_q > 0) {
-        dim3 grid(cq, (rq / 8 + kEnergyThreads - 1) / kEnergyThreads);   // narrow rows: one slab, spare threads take tokens
-        if (dt == BGTQ_F32) energy_partial_kernel<float><<<grid, kEnergyThreads, 0, st>>>((const float *)q, n_q, rq, cq, pq);
-        else energy_partial_kernel<__nv_bfloat16><<<grid, kEnergyThreads, 0, st>>>((const __nv_bfloat16 *)q, n_q, rq, cq, pq);
-        count_launch();
-    }
-    if (n_k > 0) {
-        dim3 grid(ck, (rk / 8 + kEnergyThreads - 1) / kEnergyThreads);
-        if (dt == BGTQ_F32) energy_partial_kernel<float><<<grid, kEnergyThreads, 0, st>>>((const float *)k, n_k, rk, ck, pk);
-        else energy_partial_kernel<__nv_bfloat16><<<grid, kEnergyThreads, 0, st>>>((const __nv_bfloat16 *)k, n_k, rk, ck, pk);
-        count_launch();
-    }
-    energy_final_kernel<<<Hkv * (d_h / 2), 128, 0, st>>>(pq, cq, n_q, pk, ck, n_k, Hq, Hkv, d_h, pairing,
-                                                         kind, scores, eq_out, ek_out);
-    count_launch();
-    CUDA_TRY(cudaGetLastError());
-    return BGTQ_OK;
+    EnergyParams P = {};
+    P.q = q; P.k = k; P.n_q = n_q; P.n_k = n_k; P.rq = Hq * d_h; P.rk = Hkv * d_h;
+    P.pq = (float *)ws; P.pk = P.pq + (size_t)kEnergyMaxChunks * Hq * d_h;
+    P.Hq = Hq; P.Hkv = Hkv; P.d_h = d_h; P.pairing = pairing; P.kind = kind; P.v_mode = 0;
+    P.scores = scores; P.eq_out = eq_out; P.ek_out = ek_out;
+    return launch_energy(P, dt, st);
 }
 
-// V-side score (reading Q19): s^V[h][j] = mean_t ||v_t^(j)||^2 over the 16 coordinates of V block j.  Same two passes:
-// the streaming pass above, then one CTA per (kv head, block) reduces its 16 columns' partials in fp64, fixed order.
-__global__ void __launch_bounds__(128)
-energy_final_v_kernel(const float *__restrict__ pv, int cv, int64_t n, int Hkv, int d_h, float *__restrict__ scores)
-{
-    const int nb = d_h / BGTQ_V_BLOCK;
-    const int h = blockIdx.x / nb, j = blockIdx.x % nb;
-    double sv = 0.0;
-    for (int c = threadIdx.x; c < cv; c += 128) {
-        const float *row = pv + ((int64_t)c * Hkv + h) * d_h + BGTQ_V_BLOCK * j;
-#pragma unroll
-        for (int u = 0; u < BGTQ_V_BLOCK; ++u) sv += (double)row[u];
-    }
-    __shared__ double s1[128];
-    s1[threadIdx.x] = sv;
-    __syncthreads();
-    for (int w = 64; w > 0; w >>= 1) {
-        if (threadIdx.x < w) s1[threadIdx.x] += s1[threadIdx.x + w];
-        __syncthreads();
-    }
-    if (threadIdx.x == 0) scores[h * nb + j] = (float)(s1[0] / (double)n);
-}
-
+// V-side score (reading Q19): s^V[h][j] = mean_t ||v_t^(j)||^2 over the 16 coordinates of V block j -- the same kernel,
+// phase 2 sums the 16 columns of a block.
 int launch_v_block_energy(const void *v, int64_t n, int dt, int Hkv, int d_h, float *scores, void *ws, cudaStream_t st)
 {
-    float *pv = (float *)ws;
-    const int cv = energy_chunks(n), rv = Hkv * d_h;
-    dim3 grid(cv, (rv / 8 + kEnergyThreads - 1) / kEnergyThreads);
-    if (dt == BGTQ_F32) energy_partial_kernel<float><<<grid, kEnergyThreads, 0, st>>>((const float *)v, n, rv, cv, pv);
-    else energy_partial_kernel<__nv_bfloat16><<<grid, kEnergyThreads, 0, st>>>((const __nv_bfloat16 *)v, n, rv, cv, pv);
-    energy_final_v_kernel<<<Hkv * (d_h / BGTQ_V_BLOCK), 128, 0, st>>>(pv, cv, n, Hkv, d_h, scores);
-    count_launch(2);
-    CUDA_TRY(cudaGetLastError());
-    return BGTQ_OK;
+    EnergyParams P = {};
+    P.k = v; P.n_k = n; P.rq = d_h; P.rk = Hkv * d_h; P.pq = (float *)ws; P.pk = (float *)ws;
+    P.Hq = Hkv; P.Hkv = Hkv; P.d_h = d_h; P.v_mode = 1; P.scores = scores;
+    return launch_energy(P, dt, st);
 }
 
 // ============================================================================ a2: Alg. 1 on the device
