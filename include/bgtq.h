@@ -67,6 +67,22 @@ int bgtq_block_energy(const void *q, int64_t n_q, const void *k, int64_t n_k, in
                       float *scores, float *eq_out, float *ek_out,
                       void *workspace, size_t workspace_bytes, void *stream);
 
+/* The same computation for callers that cannot allocate device memory (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): no workspace argument -- the partial sums live in a file-scope device array of
+ * the library, 4 MiB per GPU that loads the library, held until the process exits.  The call allocates nothing (no
+ * cudaMalloc / cudaFree, no allocating library routine); the array's device address is looked up once per device.
+ * Limit: (n_q_heads + n_kv_heads) * d_h <= bgtq_block_energy_static_max_row_elems() = 8192 (e.g. 48 + 16 heads at
+ * d_h = 128); beyond it the call returns BGTQ_EWORKSPACE and launches nothing -- use bgtq_block_energy.  n_q, n_k are
+ * not limited.  Token chunks are capped at 128 per tensor (workspace path: 512), so fp32 partial sums group differently:
+ * results agree with bgtq_block_energy to ~1e-6 relative, not bit for bit.  Deterministic.
+ * ALL calls share the one array (it keeps the last call's contents; nothing in it needs clearing, a call reads only what
+ * it has written): calls that overlap on the GPU -- other streams, concurrently replayed graphs, several host threads on
+ * one device -- RACE.  Serialise them (one stream) or use bgtq_block_energy with a workspace per call. */
+int bgtq_block_energy_static_max_row_elems(void);
+int bgtq_block_energy_static(const void *q, int64_t n_q, const void *k, int64_t n_k, int dt,
+                             int n_q_heads, int n_kv_heads, int d_h, int pairing, int kind,
+                             float *scores, float *eq_out, float *ek_out, void *stream);
+
 /* ---- a2: greedy marginal-gain allocation, Alg. 1, optimal by Thm. 1.
  * Per head: b_i = b_min; repeat B - L*b_min times: give one bit to the block with the largest
  * Delta_i = 3/4 * s_i * 4^-b_i among those with b_i < b_max; ties -> smallest i (Q4).

@@ -35,6 +35,7 @@ SYMBOLS = [
     "bgtq_layout_create_format", "bgtq_layout_format", "bgtq_codebook_exact",
     "bgtq_debug_microbench", "bgtq_debug_microbench_name",
     "bgtq_v_block_energy_workspace_bytes", "bgtq_v_block_energy", "bgtq_layout_create_kv",
+    "bgtq_block_energy_static", "bgtq_block_energy_static_max_row_elems",
 ]
 MICROBENCH_COUNT = 21
 FORMAT_V1, FORMAT_V2 = 1, 2
@@ -64,6 +65,10 @@ def _load() -> C.CDLL:
     lib.bgtq_block_energy_workspace_bytes.argtypes = [i32, i32, i32]
     lib.bgtq_block_energy.restype = i32
     lib.bgtq_block_energy.argtypes = [vp, i64, vp, i64, i32, i32, i32, i32, i32, i32, vp, vp, vp, vp, sz, vp]
+    lib.bgtq_block_energy_static.restype = i32
+    lib.bgtq_block_energy_static.argtypes = [vp, i64, vp, i64, i32, i32, i32, i32, i32, i32, vp, vp, vp, vp]
+    lib.bgtq_block_energy_static_max_row_elems.restype = i32
+    lib.bgtq_block_energy_static_max_row_elems.argtypes = []
     lib.bgtq_v_block_energy_workspace_bytes.restype = sz
     lib.bgtq_v_block_energy_workspace_bytes.argtypes = [i32, i32]
     lib.bgtq_v_block_energy.restype = i32
@@ -219,6 +224,25 @@ def block_energy(q: torch.Tensor, k: torch.Tensor, pairing: int = PAIR_HALF, kin
                                   pairing, kind, _dev(scores), _dev(eq) if return_parts else None,
                                   _dev(ek) if return_parts else None, _dev(ws), nws, _stream()))
     return (scores, eq, ek) if return_parts else scores
+
+
+def block_energy_static(q: torch.Tensor, k: torch.Tensor, scores: torch.Tensor, pairing: int = PAIR_HALF,
+                        kind: int = QK_AVG, eq: Optional[torch.Tensor] = None, ek: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """bgtq_block_energy_static: block_energy without any allocation -- the caller passes the output tensor(s)
+    [H_kv, d_h/2] float32, the scratch is the library's static 4 MiB device array (shared by all calls: do not overlap
+    calls on the GPU).  Limit (H_q + H_kv) * d_h <= block_energy_static_max_row_elems()."""
+    nq, Hq, d = q.shape
+    nk, Hkv, d2 = k.shape
+    assert d == d2 and _dt(q) == _dt(k) and scores.shape == (Hkv, d // 2)
+    _check(_lib.bgtq_block_energy_static(_dev(q) if nq else None, nq, _dev(k) if nk else None, nk, _dt(k), Hq, Hkv, d,
+                                         pairing, kind, _dev(scores, torch.float32),
+                                         _dev(eq, torch.float32) if eq is not None else None,
+                                         _dev(ek, torch.float32) if ek is not None else None, _stream()))
+    return scores
+
+
+def block_energy_static_max_row_elems() -> int:
+    return int(_lib.bgtq_block_energy_static_max_row_elems())
 
 
 V_BLOCK = 16

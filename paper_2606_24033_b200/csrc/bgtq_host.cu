@@ -118,6 +118,23 @@ extern "C" int bgtq_block_energy(const void *q, int64_t n_q, const void *k, int6
                                eq_out, ek_out, workspace, workspace_bytes, (cudaStream_t)stream);
 }
 
+extern "C" int bgtq_block_energy_static_max_row_elems(void) { return block_energy_static_max_row_elems(); }
+
+extern "C" int bgtq_block_energy_static(const void *q, int64_t n_q, const void *k, int64_t n_k, int dt,
+                                        int n_q_heads, int n_kv_heads, int d_h, int pairing, int kind,
+                                        float *scores, float *eq_out, float *ek_out, void *stream)
+{
+    if (!scores) FAIL(BGTQ_EINVAL, "bgtq_block_energy_static: null scores");
+    if (n_q < 0 || n_k < 0 || (n_q > 0 && !q) || (n_k > 0 && !k)) FAIL(BGTQ_EINVAL, "bgtq_block_energy_static: bad q/k");
+    if (dt != BGTQ_F32 && dt != BGTQ_BF16) FAIL(BGTQ_EINVAL, "bgtq_block_energy_static: dtype");
+    if (n_kv_heads <= 0 || n_q_heads <= 0 || n_q_heads % n_kv_heads) FAIL(BGTQ_EINVAL, "bgtq_block_energy_static: heads");
+    if (d_h <= 0 || d_h % 8 || d_h > 1024) FAIL(BGTQ_EINVAL, "bgtq_block_energy_static: d_h must be a multiple of 8, <= 1024");
+    if (pairing != BGTQ_PAIR_HALF && pairing != BGTQ_PAIR_INTERLEAVED) FAIL(BGTQ_EINVAL, "bgtq_block_energy_static: pairing");
+    if (kind < 0 || kind > BGTQ_Q_ONLY) FAIL(BGTQ_EINVAL, "bgtq_block_energy_static: score kind");
+    return launch_block_energy_static(q, n_q, k, n_k, dt, n_q_heads, n_kv_heads, d_h, pairing, kind, scores, eq_out, ek_out,
+                                      (cudaStream_t)stream);
+}
+
 extern "C" size_t bgtq_v_block_energy_workspace_bytes(int n_kv_heads, int d_h)
 {
     if (n_kv_heads <= 0 || d_h <= 0) return 0;

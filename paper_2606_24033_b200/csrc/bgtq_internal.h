@@ -142,6 +142,9 @@ int launch_block_energy(const void *q, int64_t n_q, const void *k, int64_t n_k, 
                         int Hkv, int d_h, int pairing, int kind, float *scores, float *eq_out,
                         float *ek_out, void *ws, size_t ws_bytes, cudaStream_t st);
 size_t block_energy_ws_bytes(int Hq, int Hkv, int d_h);
+int launch_block_energy_static(const void *q, int64_t n_q, const void *k, int64_t n_k, int dt, int Hq, int Hkv, int d_h,
+                               int pairing, int kind, float *scores, float *eq_out, float *ek_out, cudaStream_t st);
+int block_energy_static_max_row_elems();
 int launch_v_block_energy(const void *v, int64_t n, int dt, int Hkv, int d_h, float *scores, void *ws, cudaStream_t st);
 int launch_allocate(const float *scores, int n_heads, int L, int b_min, int b_max, int B,
                     uint8_t *bits, cudaStream_t st);

@@ -4,6 +4,9 @@
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
 
+#include <mutex>
+#include <string>
+
 #include "bgtq_internal.h"
 
 namespace bgtq {
@@ -232,6 +235,51 @@ int launch_block_energy(const void *q, int64_t n_q, const void *k, int64_t n_k, 
     P.Hq = Hq; P.Hkv = Hkv; P.d_h = d_h; P.pairing = pairing; P.kind = kind; P.v_mode = 0;
     P.scores = scores; P.eq_out = eq_out; P.ek_out = ek_out;
     return launch_energy(P, dt, st);
+}
+
+// ---- bgtq_block_energy_static: the same kernel with its partial sums in a file-scope device array instead of a caller
+// workspace, for callers that cannot allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc).
+// 4 MiB per GPU that loads the library, held until exit.  Every call uses the SAME array: calls that overlap on the GPU
+// (different streams, or graphs replayed concurrently) race.  Nothing in it has to start at zero -- phase 2 reads exactly the
+// entries phase 1 of the same call has written (every chunk < cq / ck, every column), so stale contents are never read.
+constexpr int kStaticEnergyChunks = 128;                                  // token chunks per tensor (the workspace path: 512)
+constexpr int kStaticEnergyRowElems = 8192;                               // (n_q_heads + n_kv_heads) * d_h at most
+constexpr size_t kStaticEnergyFloats = (size_t)kStaticEnergyChunks * kStaticEnergyRowElems;   // 1,048,576 floats = 4 MiB
+static __device__ __align__(256) float g_energy_scratch[kStaticEnergyFloats];
+
+int block_energy_static_max_row_elems() { return kStaticEnergyRowElems; }
+
+int launch_block_energy_static(const void *q, int64_t n_q, const void *k, int64_t n_k, int dt, int Hq, int Hkv, int d_h,
+                               int pairing, int kind, float *scores, float *eq_out, float *ek_out, cudaStream_t st)
+{
+    if ((int64_t)(Hq + Hkv) * d_h > kStaticEnergyRowElems) {
+        set_error("bgtq_block_energy_static: (n_q_heads + n_kv_heads) * d_h = " + std::to_string((int64_t)(Hq + Hkv) * d_h) +
+                  " exceeds the static scratch limit of " + std::to_string(kStaticEnergyRowElems) + " (4 MiB); use bgtq_block_energy with a workspace");
+        return BGTQ_EWORKSPACE;
+    }
+    // device address of the array: in host code `g_energy_scratch` is only a handle, never a pointer a kernel may use.
+    // Looked up once per device, with that device current.
+    static float *scratch_of[64] = {};
+    static std::mutex mu;
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    float *scratch = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(mu);
+        if (dev >= 0 && dev < 64 && scratch_of[dev]) scratch = scratch_of[dev];
+        else {
+            void *ptr = nullptr;
+            CUDA_TRY(cudaGetSymbolAddress(&ptr, g_energy_scratch));
+            scratch = static_cast<float *>(ptr);
+            if (dev >= 0 && dev < 64) scratch_of[dev] = scratch;
+        }
+    }
+    EnergyParams P = {};
+    P.q = q; P.k = k; P.n_q = n_q; P.n_k = n_k; P.rq = Hq * d_h; P.rk = Hkv * d_h;
+    P.pq = scratch; P.pk = scratch + (size_t)kStaticEnergyChunks * Hq * d_h;
+    P.Hq = Hq; P.Hkv = Hkv; P.d_h = d_h; P.pairing = pairing; P.kind = kind; P.v_mode = 0;
+    P.scores = scores; P.eq_out = eq_out; P.ek_out = ek_out;
+    return launch_energy(P, dt, st, kStaticEnergyChunks);
 }
 
 // V-side score (reading Q19): s^V[h][j] = mean_t ||v_t^(j)||^2 over the 16 coordinates of V block j -- the same kernel,
