@@ -173,7 +173,12 @@ __device__ __forceinline__ void build_pools(const uint16_t *cb16, uint32_t *pool
 // q'_g = Pi^(m_g) q_g * (scale*log2e/sqrt(m_g))  ("Q-side rotation"), rounded to fp16 and
 // written in B-fragment order: qf[pair][kstep][head slot n (8)][c (4)][coords 2c, 2c+1, 8+2c, 9+2c], i.e. one
 // 8-byte load per lane (n*4+c) and k-step; zero padded.
-__global__ void __launch_bounds__(128)
+// Latency-shaped (it sits on the critical path of every decode call, 8.6 us per layer before): four threads share one
+// output -- thread part p takes k = p, p+4, ... -- so that a group of up to 64 coordinates needs ONE round of 16 independent
+// rotation loads per thread instead of four, and the ragged tail is a masked round instead of a serial loop.
+// PARTS = 1 (one thread per output) serves the launches with many blocks, where throughput counts.
+template <int PARTS>
+__global__ void __launch_bounds__(PARTS * kDh)
 qfold_kernel(const HeadMeta *__restrict__ metas, const float *__restrict__ rot_t,
              const __nv_bfloat16 *__restrict__ q, int batch, int Hkv, int Hq, float scale_log2e,
              __half *__restrict__ qf, int plain)
@@ -190,7 +195,9 @@ qfold_kernel(const HeadMeta *__restrict__ metas, const float *__restrict__ rot_t
         const uint32_t *msrc = reinterpret_cast<const uint32_t *>(metas + l * Hkv + h);
         if (tid < (int)(sizeof(HeadMeta) / 4)) reinterpret_cast<uint32_t *>(&Ms)[tid] = __ldg(msrc + tid);
     }
-    qs[tid] = __bfloat162float(q[((size_t)lb * Hq + h * G + n) * kDh + tid]);
+    constexpr int kQfoldThreads = PARTS * kDh;
+    constexpr int q0 = PARTS > 1 ? kDh : 0;                 // (another warp set than the metadata copy)
+    if (tid >= q0 && tid < q0 + kDh) qs[tid - q0] = __bfloat162float(q[((size_t)lb * Hq + h * G + n) * kDh + tid - q0]);
     __syncthreads();
     const HeadMeta &M = Ms;
     if (tid == 0)
@@ -199,33 +206,38 @@ qfold_kernel(const HeadMeta *__restrict__ metas, const float *__restrict__ rot_t
     // zero padding: this head's slots (and, from block n = 0, the unused head slots n >= G)
     uint2 *out2 = reinterpret_cast<uint2 *>(qf + (size_t)pair * kQfHalves);     // [kstep][8][4] of 4 halves
     if (!plain)
-        for (int e = tid; e < kMaxKSteps * 32; e += 128) {
+        for (int e = tid; e < kMaxKSteps * 32; e += kQfoldThreads) {
             const int nn = (e >> 2) & 7;
             if (nn == n || (n == 0 && nn >= G)) out2[e] = make_uint2(0u, 0u);
         }
     __syncthreads();
     // plain layout (prefill): q'[pair][head slot n][128] in grouped coordinate order, zero beyond kdim
-    if (plain && tid >= M.kdim) qf[((size_t)pair * 8 + n) * kDh + tid] = __float2half(0.f);
-    if (tid < M.kdim) {
+    if (plain && tid < kDh && tid >= M.kdim) qf[((size_t)pair * 8 + n) * kDh + tid] = __float2half(0.f);
+    const int ro = tid / PARTS, part = tid % PARTS;         // output (grouped coordinate) and the part of its dot product
+    const bool act = ro < M.kdim;
+    float acc = 0.f, sc = 0.f;
+    int ks = 0, kap = 0;
+    if (act) {
         int g = 0;
-        while (g + 1 < M.n_groups && tid >= M.gstart[g + 1]) ++g;
-        const int m = M.gm[g], x0 = M.gstart[g], r = tid - x0;
+        while (g + 1 < M.n_groups && ro >= M.gstart[g + 1]) ++g;
+        const int m = M.gm[g], x0 = M.gstart[g], r = ro - x0;
         const float *T = rot_t + rot_offset(m) + r;
-        const float sc = scale_log2e / sqrtf((float)m) * (BGTQ_NORM_IN_OPERAND ? 64.f : 1.f);   // 2^6: see qk_group_n
-        const int ks = ksbase[g] + (r >> 4), kap = r & 15;
+        sc = scale_log2e / sqrtf((float)m) * (BGTQ_NORM_IN_OPERAND ? 64.f : 1.f);   // 2^6: see qk_group_n
+        ks = ksbase[g] + (r >> 4); kap = r & 15;
         const uint8_t *co = M.coords + x0;
-        float acc = 0.f;
-        int k = 0;
-        for (; k + 16 <= m; k += 16) {                  // 16 independent rotation loads in flight per thread
+        for (int k0 = 0; k0 < m; k0 += 16 * PARTS) {        // 16 independent rotation loads in flight per thread
             float tv[16];
 #pragma unroll
-            for (int u = 0; u < 16; ++u) tv[u] = __ldg(T + (size_t)(k + u) * m);
+            for (int u = 0; u < 16; ++u) { const int k = k0 + part + PARTS * u; tv[u] = k < m ? __ldg(T + (size_t)k * m) : 0.f; }
 #pragma unroll
-            for (int u = 0; u < 16; ++u) acc = fmaf(tv[u], qs[co[k + u]], acc);
+            for (int u = 0; u < 16; ++u) { const int k = k0 + part + PARTS * u; acc = fmaf(tv[u], k < m ? qs[co[k]] : 0.f, acc); }
         }
-        for (; k < m; ++k) acc = fmaf(__ldg(T + (size_t)k * m), qs[co[k]], acc);
+    }
+#pragma unroll
+    for (int sft = 1; sft < PARTS; sft <<= 1) acc += __shfl_xor_sync(0xffffffffu, acc, sft);   // the parts of an output are adjacent lanes; fixed order
+    if (act && part == 0) {
         __half *out = qf + (size_t)pair * kQfHalves;
-        if (plain) qf[((size_t)pair * 8 + n) * kDh + tid] = __float2half_rn(acc * sc);
+        if (plain) qf[((size_t)pair * 8 + n) * kDh + ro] = __float2half_rn(acc * sc);
         else out[((ks * 8 + n) * 4 + ((kap & 7) >> 1)) * 4 + (kap >> 3) * 2 + (kap & 1)] = __float2half_rn(acc * sc);
     }
     // Protected regime: this kernel is launched programmatically behind window_kernel and runs beside it; it must not
@@ -780,23 +792,31 @@ decode_kernel(const DecodeParams P)
 // ---------------------------------------------------------------- a6: exact LSE merge + V de-rotation
 // M = max_w m_w; l = sum_w l_w 2^(m_w-M); o' = sum_w acc_w 2^(m_w-M) / l, then
 // out = Pi^(128)^T o' / sqrt(128)  (dequantisation of V, applied once because it is linear) -> bf16.
-__global__ void __launch_bounds__(128)
+// Latency-shaped like qfold_kernel (it ends every decode call): 512 threads per (pair, query head), one record per thread in
+// pass 1 (its running max and sum in one round trip), 16 warps over the records in pass 2, four threads per output
+// dimension in the de-rotation.  Every reduction has a fixed order, so the result does not depend on timing.
+// PARTS = 1 (128 threads) serves the launches with many blocks.
+template <int PARTS>
+__global__ void __launch_bounds__(PARTS * kDh)
 combine_kernel(const float *__restrict__ partials, const int32_t *__restrict__ seq_len,
                const float *__restrict__ rot128, int n_layers, int batch, int Hkv, int G, int64_t n_cap,
-               int n_ctas, int W, __nv_bfloat16 *__restrict__ out, int n_sink = 0, int n_recent = 0, int win_slot = -1,
-               const HeadMeta *__restrict__ metas = nullptr, const float *__restrict__ rot_base = nullptr)
+               int n_ctas, int W, __nv_bfloat16 *__restrict__ out, int n_sink, int n_recent, int win_slot,
+               const HeadMeta *__restrict__ metas, const float *__restrict__ rot_base)
 {
+    constexpr int kCombineThreads = PARTS * kDh;
     constexpr int kMaxSlots = 1024;                     // 32 + n_ctas entries at most (host checks n_ctas)
+    constexpr int NW = kCombineThreads / 32;
     __shared__ int pre[kMaxBatch + 1];
     __shared__ float o[kDh];
     __shared__ int slots[kMaxSlots];
-    __shared__ float wgt[kMaxSlots];
-    __shared__ float red[4][kDh + 4];
-    __shared__ float wred[2][4];
+    __shared__ float wgt[kMaxSlots], lrec[kMaxSlots];
+    __shared__ float red[NW][kDh + 4];
+    __shared__ float wred[2][NW];
     const int pair = blockIdx.x / G, n = blockIdx.x % G;
     const int h = pair % Hkv, lb = pair / Hkv, b = lb % batch, l = lb / batch;
-    const int d = threadIdx.x, lane = d & 31, wq = d >> 5;
-    if (d == 0) build_prefix(seq_len, batch, n_cap * kTile, pre, n_sink, n_recent);
+    const int t = threadIdx.x, lane = t & 31, wq = t >> 5;
+    const int d = t & (kDh - 1), part = t >> 7;         // de-rotation: output dimension and the part of its dot product
+    if (t == 0) build_prefix(seq_len, batch, n_cap * kTile, pre, n_sink, n_recent);
     __syncthreads();
     const Sched S = make_sched(n_layers, batch, Hkv, pre, n_ctas, W);
     const int tiles_b = pre[b + 1] - pre[b];
@@ -804,7 +824,7 @@ combine_kernel(const float *__restrict__ partials, const int32_t *__restrict__ s
     // protected regime: one more record per pair, written by window_kernel at slot win_slot (relative to the pair's
     // base, like every slot below); it exists whenever the sequence is not empty
     const bool has_win = win_slot >= 0 && seq_len[b] > 0;
-    if (tiles_b == 0 && !has_win) { dst[d] = __float2bfloat16(0.f); return; }
+    if (tiles_b == 0 && !has_win) { if (t < kDh) dst[t] = __float2bfloat16(0.f); return; }
     const int start = l * (Hkv * S.tiles_sum) + pre[b] * Hkv + h * tiles_b, stop = start + tiles_b;
     // CTAs whose range meets [start, stop): the decode kernel's balanced split, recomputed
     int c0 = 0, c1 = 0;
@@ -830,40 +850,43 @@ combine_kernel(const float *__restrict__ partials, const int32_t *__restrict__ s
     const int n_pk = tiles_b > 0 ? min(kMaxSlots - 1, 16 + n_int + (c1 > c0 ? 16 : 0)) : 0;   // records of the packed range
     const int n_ent = n_pk + (has_win ? 1 : 0);
     pdl_wait();                                         // the decode kernel's partials are complete from here on
-    // pass 1: every record's running max -> M, then its weight 2^(m - M) and the merged sum l.  All loads are
-    // independent (one record per thread), and the order of every reduction is fixed, so the result does not depend
-    // on timing.
+    // pass 1: every record's running max and sum (one round trip: the two loads are independent) -> M
     float mloc = -INFINITY;
-    for (int e = d; e < n_ent; e += 128) {
+    for (int e = t; e < n_ent; e += kCombineThreads) {
         const int sl = e >= n_pk ? win_slot
                      : e < 16 ? edge_slot(c0, e) : (e < 16 + n_int ? edge_slot(c0 + 1 + e - 16, 0) : edge_slot(c1, e - 16 - n_int));
         slots[e] = sl;
-        const float mw = sl < 0 ? -INFINITY : rec0[(size_t)sl * kPartialFloats];
-        wgt[e] = mw;
-        mloc = fmaxf(mloc, mw);
+        const float2 ml = sl < 0 ? make_float2(-INFINITY, 0.f) : *reinterpret_cast<const float2 *>(rec0 + (size_t)sl * kPartialFloats);
+        wgt[e] = ml.x;
+        lrec[e] = ml.y;
+        mloc = fmaxf(mloc, ml.x);
     }
 #pragma unroll
     for (int s = 16; s; s >>= 1) mloc = fmaxf(mloc, __shfl_xor_sync(0xffffffffu, mloc, s));
     if (lane == 0) wred[0][wq] = mloc;
     __syncthreads();
-    const float Mx = fmaxf(fmaxf(wred[0][0], wred[0][1]), fmaxf(wred[0][2], wred[0][3]));
+    float Mx = wred[0][0];
+#pragma unroll
+    for (int w = 1; w < NW; ++w) Mx = fmaxf(Mx, wred[0][w]);
+    // weights 2^(m - M) and the merged sum l
     float lloc = 0.f;
-    for (int e = d; e < n_ent; e += 128) {
-        const int sl = slots[e];
+    for (int e = t; e < n_ent; e += kCombineThreads) {
         const float mw = wgt[e];
-        const float f = (sl < 0 || mw == -INFINITY) ? 0.f : exp2f(mw - Mx);
+        const float f = (slots[e] < 0 || mw == -INFINITY) ? 0.f : exp2f(mw - Mx);
         wgt[e] = f;
-        if (f != 0.f) lloc = fmaf(rec0[(size_t)sl * kPartialFloats + 1], f, lloc);
+        lloc = fmaf(lrec[e], f, lloc);
     }
 #pragma unroll
     for (int s = 16; s; s >>= 1) lloc += __shfl_xor_sync(0xffffffffu, lloc, s);
     if (lane == 0) wred[1][wq] = lloc;
     __syncthreads();
-    const float lsum = (wred[1][0] + wred[1][1]) + (wred[1][2] + wred[1][3]);
-    // pass 2: warp wq accumulates records wq, wq+4, ...; a lane owns dims 2*lane, 2*lane+1, 64+2*lane, 65+2*lane
+    float lsum = 0.f;
+#pragma unroll
+    for (int w = 0; w < NW; ++w) lsum += wred[1][w];
+    // pass 2: warp wq accumulates records wq, wq+16, ...; a lane owns dims 2*lane, 2*lane+1, 64+2*lane, 65+2*lane
     float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
 #pragma unroll 4
-    for (int e = wq; e < n_ent; e += 4) {
+    for (int e = wq; e < n_ent; e += NW) {
         const float f = wgt[e];
         if (f == 0.f) continue;
         const float *rec = rec0 + (size_t)slots[e] * kPartialFloats + 2;
@@ -873,25 +896,35 @@ combine_kernel(const float *__restrict__ partials, const int32_t *__restrict__ s
     }
     red[wq][2 * lane] = a0; red[wq][2 * lane + 1] = a1; red[wq][64 + 2 * lane] = a2; red[wq][65 + 2 * lane] = a3;
     __syncthreads();
-    o[d] = ((red[0][d] + red[1][d]) + (red[2][d] + red[3][d])) / lsum;
+    if (t < kDh) {
+        float acc = 0.f;
+#pragma unroll
+        for (int w = 0; w < NW; ++w) acc += red[w][t];
+        o[t] = acc / lsum;
+    }
     __syncthreads();
+    if (rot128 == nullptr && metas == nullptr) { if (t < kDh) dst[t] = __float2bfloat16(o[t]); return; }   // fp16-cache comparison path: no rotation
+    // de-rotation of output dimension d: four threads take a quarter of the dot product each (32 independent loads)
+    float r = 0.f, inv = 0.08838834764831845f;          // 1/sqrt(128)
+    int od = d;
     if (metas) {
         // V-side groups (reading Q19): record position d is grouped V coordinate d.  Its group of m coordinates starts at
         // s: out[coord(d)] = sum_j Pi^(m)[j][d - s] o[s + j] / sqrt(m), coord(d) = 16 * vblk[d >> 4] + (d & 15).
         const HeadMeta &M = metas[l * Hkv + h];
-        const int gv = M.vbg[d >> 4], s = 16 * M.vgstart[gv], m = 16 * M.vgcnt[gv];
+        const int gv = M.vbg[d >> 4], s = 16 * M.vgstart[gv], m = 16 * M.vgcnt[gv], mq = m / PARTS;
         const float *R = rot_base + rot_offset(m) + (d - s);
-        float r = 0.f;
-#pragma unroll 16
-        for (int j = 0; j < m; ++j) r = fmaf(__ldg(R + j * m), o[s + j], r);
-        dst[16 * M.vblk[d >> 4] + (d & 15)] = __float2bfloat16(r / sqrtf((float)m));
-        return;
-    }
-    if (rot128 == nullptr) { dst[d] = __float2bfloat16(o[d]); return; }    // fp16-cache comparison path: no rotation
-    float r = 0.f;
+#pragma unroll 4
+        for (int j = part * mq; j < (part + 1) * mq; ++j) r = fmaf(__ldg(R + j * m), o[s + j], r);
+        inv = rsqrtf((float)m);
+        od = 16 * M.vblk[d >> 4] + (d & 15);
+    } else {
 #pragma unroll 32
-    for (int j = 0; j < kDh; ++j) r = fmaf(__ldg(rot128 + j * kDh + d), o[j], r);
-    dst[d] = __float2bfloat16(r * 0.08838834764831845f);     // 1/sqrt(128)
+        for (int j = part * (kDh / PARTS); j < (part + 1) * (kDh / PARTS); ++j) r = fmaf(__ldg(rot128 + j * kDh + d), o[j], r);
+    }
+    if (PARTS == 1) { dst[od] = __float2bfloat16(r * inv); return; }
+    red[part][d] = r;
+    __syncthreads();
+    if (t < kDh) dst[od] = __float2bfloat16(((red[0][t] + red[1][t]) + (red[2][t] + red[3][t])) * inv);
 }
 
 // ---------------------------------------------------------------- protected regime: fp16 sink / recent windows
@@ -1270,6 +1303,7 @@ fp16_decode_kernel(const Fp16Params P)
 }
 
 // ---------------------------------------------------------------- host side
+constexpr int kLatencyShapedBlocks = 160;       // up to this many blocks qfold / combine run four threads per output
 static int pick_warps(int buf_bytes)
 {
     // measured: 12 warps at 168 registers beat 13 / 14 / 16 warps (spills, uneven schedulers)
@@ -1339,9 +1373,11 @@ int launch_combine(const float *partials, const int32_t *seq_len, const float *r
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
-    cfg.gridDim = dim3(n_layers * batch * Hkv * G); cfg.blockDim = dim3(128); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+    // few blocks (a per-layer call): the latency-shaped 512-thread variant; many blocks: 128 threads
+    const bool wide = n_layers * batch * Hkv * G <= kLatencyShapedBlocks;
+    cfg.gridDim = dim3(n_layers * batch * Hkv * G); cfg.blockDim = dim3(wide ? 4 * kDh : kDh); cfg.dynamicSmemBytes = 0; cfg.stream = st;
     cfg.attrs = at; cfg.numAttrs = 1;
-    cudaLaunchKernelEx(&cfg, combine_kernel, partials, seq_len, rot128, n_layers, batch, Hkv, G, n_cap, n_ctas, W,
+    cudaLaunchKernelEx(&cfg, wide ? combine_kernel<4> : combine_kernel<1>, partials, seq_len, rot128, n_layers, batch, Hkv, G, n_cap, n_ctas, W,
                        (__nv_bfloat16 *)out, n_sink, n_recent, win_slot, metas, rot_base);
     count_launch();
     CUDA_TRY(cudaGetLastError());
@@ -1411,18 +1447,22 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
                                    n_sink, n_recent, scale * 1.4426950408889634f, win_slot, st,
                                    lay->v_grouped ? metas : nullptr, lay->d_rot_t)) return rc;
     }
+    const bool wideq = pairs * G <= kLatencyShapedBlocks;       // few blocks: the latency-shaped 512-thread variant
     if (win && !g_prof) {
         cudaLaunchConfig_t cfg = {};
         cudaLaunchAttribute at[1];
         at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
         at[0].val.programmaticStreamSerializationAllowed = 1;
-        cfg.gridDim = dim3(pairs * G); cfg.blockDim = dim3(128); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+        cfg.gridDim = dim3(pairs * G); cfg.blockDim = dim3(wideq ? 4 * kDh : kDh); cfg.dynamicSmemBytes = 0; cfg.stream = st;
         cfg.attrs = at; cfg.numAttrs = 1;
-        cudaLaunchKernelEx(&cfg, qfold_kernel, metas, (const float *)lay->d_rot_t, (const __nv_bfloat16 *)q, batch, Hkv, Hq,
+        cudaLaunchKernelEx(&cfg, wideq ? qfold_kernel<4> : qfold_kernel<1>, metas, (const float *)lay->d_rot_t, (const __nv_bfloat16 *)q, batch, Hkv, Hq,
                            scale * 1.4426950408889634f, qf, 0);
-    } else
-        qfold_kernel<<<pairs * G, 128, 0, st>>>(metas, lay->d_rot_t, (const __nv_bfloat16 *)q, batch, Hkv, Hq,
-                                                scale * 1.4426950408889634f, qf, 0);
+    } else if (wideq)
+        qfold_kernel<4><<<pairs * G, 4 * kDh, 0, st>>>(metas, lay->d_rot_t, (const __nv_bfloat16 *)q, batch, Hkv, Hq,
+                                                       scale * 1.4426950408889634f, qf, 0);
+    else
+        qfold_kernel<1><<<pairs * G, kDh, 0, st>>>(metas, lay->d_rot_t, (const __nv_bfloat16 *)q, batch, Hkv, Hq,
+                                                   scale * 1.4426950408889634f, qf, 0);
     count_launch();
     CUDA_TRY(cudaGetLastError());
 
@@ -1527,8 +1567,9 @@ int launch_fp16_decode(int n_layers, int batch, int Hq, int Hkv, const void *k_c
     fp16_decode_kernel<<<sm_count, kFp16Warps * 32, smem, st>>>(P);
     count_launch();
     CUDA_TRY(cudaGetLastError());
-    combine_kernel<<<n_layers * batch * Hkv * P.G, 128, 0, st>>>(P.partials, seq_len, nullptr, n_layers, batch, Hkv, P.G,
-                                                                 P.n_cap, sm_count, kFp16Warps, (__nv_bfloat16 *)out);
+    combine_kernel<1><<<n_layers * batch * Hkv * P.G, kDh, 0, st>>>(P.partials, seq_len, nullptr, n_layers, batch, Hkv, P.G,
+                                                                 P.n_cap, sm_count, kFp16Warps, (__nv_bfloat16 *)out, 0, 0, -1,
+                                                                    (const HeadMeta *)nullptr, (const float *)nullptr);
     count_launch();
     CUDA_TRY(cudaGetLastError());
     return BGTQ_OK;
@@ -2259,7 +2300,7 @@ int launch_prefill(const bgtq_layout *lay, int layer, const void *cache, const v
     float *opart = reinterpret_cast<float *>(reinterpret_cast<unsigned char *>(ws) + rows * Hkv * 8 * kDh * sizeof(__half));
     const HeadMeta *metas = lay->d_meta + (size_t)layer * Hkv;
     // q' for every query token: the decode q-fold with (batch * n_q) rows, plain layout
-    qfold_kernel<<<(unsigned)(rows * Hkv * G), 128, 0, st>>>(metas, lay->d_rot_t, (const __nv_bfloat16 *)q, (int)rows, Hkv, Hq,
+    qfold_kernel<1><<<(unsigned)(rows * Hkv * G), kDh, 0, st>>>(metas, lay->d_rot_t, (const __nv_bfloat16 *)q, (int)rows, Hkv, Hq,
                                                              scale * 1.4426950408889634f, qp, 1);
     count_launch();
     CUDA_TRY(cudaGetLastError());
