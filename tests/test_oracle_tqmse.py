@@ -216,3 +216,17 @@ def test_rope_logit_mae_echo_of_table_1():
             for a in range(h * 2, h * 2 + 2):
                 want += abs(float(q[t, a] @ e))
     assert m0 == pytest.approx(want / (len(q) * Hq), rel=1e-12)
+    # a non-zero offset against explicit rotations (oracle.rope is pinned on its own): q^T R_Delta (k - khat) with
+    # R_Delta = RoPE at position Delta applied to the error vector
+    D = 37.0
+    mD = O.rope_logit_mae(q, k, one, tg, base, offsets=np.array([D]))
+    want = 0.0
+    for h in range(Hkv):
+        g = O.groups_from_bits(one[h], d)[0]
+        for t in range(len(q)):
+            idx, hb, _ = O.quantize_group(k[t, h, g.coords], 8, tg)
+            e = k[t, h].copy(); e[g.coords] -= O.dequantize_group(idx, hb, 8, tg)
+            re = O.rope(e[None, None, :], np.array([D]), base)[0, 0]
+            for a in range(h * 2, h * 2 + 2):
+                want += abs(float(q[t, a] @ re))
+    assert mD == pytest.approx(want / (len(q) * Hq), rel=1e-10)
