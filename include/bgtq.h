@@ -298,6 +298,10 @@ int bgtq_fp16_decode_attention(int n_layers, int batch, int n_q_heads, int n_kv_
 /* decode one unit (b words per lane, 32 lanes, plane-major as in a tile) with the kernel's own
  * unpack routine: words [host] uint32 [b*32] -> values [host] float [32 lanes][32 slots]. */
 int bgtq_debug_decode_unit(int b, const uint32_t *words, float *values);
+/* bgtq_quantize_append* with >= 16 new tokens per sequence runs the tensor-core fast path (TF32 hi/lo products, codes inside
+ * a guard band of a threshold recomputed with the exact fp64 chain: same bytes as the exact kernel).  on != 0 forces the
+ * exact fp64 kernel for every call of the process (tests compare the two; bench.py times both).  Returns the old setting. */
+int bgtq_debug_append_exact_only(int on);
 /* measurement hook for bench.py's roofline: while enabled, every decode call records a CUDA event
  * pair on its stream around the split-KV decode kernel alone (not the q-fold / combine kernels);
  * _read synchronises those events, returns the summed milliseconds and the number of launches

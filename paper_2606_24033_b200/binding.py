@@ -35,7 +35,7 @@ SYMBOLS = [
     "bgtq_layout_create_format", "bgtq_layout_format", "bgtq_codebook_exact",
     "bgtq_debug_microbench", "bgtq_debug_microbench_name",
     "bgtq_v_block_energy_workspace_bytes", "bgtq_v_block_energy", "bgtq_layout_create_kv",
-    "bgtq_block_energy_static", "bgtq_block_energy_static_max_row_elems",
+    "bgtq_block_energy_static", "bgtq_block_energy_static_max_row_elems", "bgtq_debug_append_exact_only",
 ]
 MICROBENCH_COUNT = 21
 FORMAT_V1, FORMAT_V2 = 1, 2
@@ -67,6 +67,8 @@ def _load() -> C.CDLL:
     lib.bgtq_block_energy.argtypes = [vp, i64, vp, i64, i32, i32, i32, i32, i32, i32, vp, vp, vp, vp, sz, vp]
     lib.bgtq_block_energy_static.restype = i32
     lib.bgtq_block_energy_static.argtypes = [vp, i64, vp, i64, i32, i32, i32, i32, i32, i32, vp, vp, vp, vp]
+    lib.bgtq_debug_append_exact_only.restype = i32
+    lib.bgtq_debug_append_exact_only.argtypes = [i32]
     lib.bgtq_block_energy_static_max_row_elems.restype = i32
     lib.bgtq_block_energy_static_max_row_elems.argtypes = []
     lib.bgtq_v_block_energy_workspace_bytes.restype = sz
@@ -241,6 +243,11 @@ def block_energy_static(q: torch.Tensor, k: torch.Tensor, scores: torch.Tensor, 
     return scores
 
 
+def append_exact_only(on: bool) -> bool:
+    """bgtq_debug_append_exact_only: force the exact fp64 append kernel for bulk appends (test / bench hook)."""
+    return bool(_lib.bgtq_debug_append_exact_only(1 if on else 0))
+
+
 def block_energy_static_max_row_elems() -> int:
     return int(_lib.bgtq_block_energy_static_max_row_elems())
 
@@ -303,7 +310,7 @@ class Layout:
 
     def __del__(self):
         h = getattr(self, "_h", None)
-        if h:
+        if h and _lib is not None:            # (module globals are already gone at interpreter shutdown)
             _lib.bgtq_layout_destroy(h)
             self._h = None
 

@@ -18,6 +18,9 @@ namespace bgtq {
 
 #define CUDA_TRY(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) return cuda_fail(e_, #expr); } while (0)
 
+#ifndef BGTQ_APPEND_PHASES
+#define BGTQ_APPEND_PHASES 0
+#endif
 constexpr int kAppendThreads = 256;
 constexpr int kMetaBytes = (int)((sizeof(HeadMeta) + 15) / 16 * 16);
 static_assert(sizeof(HeadMeta) % 4 == 0, "HeadMeta is copied word by word");
@@ -54,6 +57,61 @@ __device__ __forceinline__ void put_field(uint32_t *base, int wstride, int b, in
     }
 }
 
+// The four slots 4i .. 4i+3 of a unit (one sub-batch's contribution to a lane: two tokens x two coordinates for K, four
+// tokens for V) written with one read-modify-write per word they touch instead of one per bit: at every width the four
+// fields are neighbours (DESIGN.md section 4 table).  pm: which of the four are present (tokens of this call).
+__device__ __forceinline__ void rmw(uint32_t *w, uint32_t val, uint32_t mask) { if (mask) *w = (*w & ~mask) | val; }
+__device__ __forceinline__ void pack4(uint32_t *wb, int ws, int b, int i, const unsigned (&f)[4], unsigned pm)
+{
+    uint32_t val = 0, mask = 0;
+    if (b == 1) {                                                  // slot 2j+e at bit (15-j) + 16e
+#pragma unroll
+        for (int s = 0; s < 4; ++s)
+            if ((pm >> s) & 1) { const int pos = 15 - (2 * i + (s >> 1)) + 16 * (s & 1); val |= (f[s] & 1u) << pos; mask |= 1u << pos; }
+        rmw(wb, val, mask);
+    } else if (b == 2) {                                           // word i>>2; Q = i&3, e = s
+#pragma unroll
+        for (int s = 0; s < 4; ++s)
+            if ((pm >> s) & 1) { const int pos = 4 * ((i & 1) * 4 + s) + 2 * ((i & 3) >> 1); val |= (f[s] & 3u) << pos; mask |= 3u << pos; }
+        rmw(wb + (i >> 2) * ws, val, mask);
+    } else if (b <= 4) {
+        unsigned g[4];
+#pragma unroll
+        for (int s = 0; s < 4; ++s) g[s] = b == 4 ? (f[s] >= 8 ? f[s] - 8 : (8u | (7u - f[s]))) : f[s];   // width 4: sign-magnitude
+        if (i < 6) {                                               // slots 0..23: word k>>3, nibble k&7
+#pragma unroll
+            for (int s = 0; s < 4; ++s)
+                if ((pm >> s) & 1) { const int pos = 4 * ((i & 1) * 4 + s); val |= (g[s] & 7u) << pos; mask |= 7u << pos; }
+            rmw(wb + (i >> 1) * ws, val, mask);
+        } else {                                                   // slots 24..31: bit j of the field at word j, bit 4(k-24)+3
+#pragma unroll
+            for (int bit = 0; bit < 3; ++bit) {
+                val = 0; mask = 0;
+#pragma unroll
+                for (int s = 0; s < 4; ++s)
+                    if ((pm >> s) & 1) { const int pos = 4 * (4 * (i - 6) + s) + 3; val |= ((g[s] >> bit) & 1u) << pos; mask |= 1u << pos; }
+                rmw(wb + bit * ws, val, mask);
+            }
+        }
+        if (b == 4) {                                              // sign of slot 4Q+e (Q = i, e = s): word 3, bit 8e+7-Q
+            val = 0; mask = 0;
+#pragma unroll
+            for (int s = 0; s < 4; ++s)
+                if ((pm >> s) & 1) { const int pos = 8 * s + 7 - i; val |= ((g[s] >> 3) & 1u) << pos; mask |= 1u << pos; }
+            rmw(wb + 3 * ws, val, mask);
+        }
+    } else {                                                       // widths 5..8: bits [b*k, b*k+b) of the stream, k = 4i .. 4i+3
+        unsigned long long v64 = 0, m64 = 0;
+        const unsigned long long fm = (1ull << b) - 1ull;
+#pragma unroll
+        for (int s = 0; s < 4; ++s)
+            if ((pm >> s) & 1) { v64 |= (unsigned long long)(f[s] & fm) << (s * b); m64 |= fm << (s * b); }
+        const int start = 4 * i * b, word = start >> 5, sh = start & 31;
+        rmw(wb + word * ws, (uint32_t)(v64 << sh), (uint32_t)(m64 << sh));
+        if (sh + 4 * b > 32) rmw(wb + (word + 1) * ws, (uint32_t)(v64 >> (32 - sh)), (uint32_t)(m64 >> (32 - sh)));
+    }
+}
+
 // BGTQ-v2: bits that code f at slot k of a chunk (width b, r slots) contributes to word j of the chunk
 __device__ __forceinline__ void slot_bits_v2(int b, int r, int k, int j, unsigned f, uint32_t &val, uint32_t &mask)
 {
@@ -80,21 +138,55 @@ __device__ __forceinline__ void slot_bits_v2(int b, int r, int k, int j, unsigne
     }
 }
 
+// ---- fast path (FAST = true; bulk appends): z ~ X Pi^T of a 16-token sub-batch on the tensor cores, exact recheck near thresholds
+// One work item = 16 outputs (two n-tiles sharing their A fragments) of one rotation group; mma.sync.m16n8k8 TF32 with hi/lo
+// splits of both operands (the split of Pi is precomputed: rot_hl = {tf32(Pi), Pi - tf32(Pi)}, row-major like the rotation table).
+struct FastItem { uint16_t x0; uint8_t m, n0, b, sidx, isv, pad; };   // x0: first column of the group in a row of xs; n0: first output
+constexpr int kMaxFastItems = 32;              // sum_g ceil(m_g / 16) <= 16 for K, 8 for V
+constexpr int kFastWarps = kAppendThreads / 32;
+constexpr int kFastPerWarp = kMaxFastItems / kFastWarps;
+constexpr int kFastQueue = kSub * 256;         // every (token, column) of a sub-batch may need the exact chain
+// Three TF32 products per k-step (hi/lo splits of x and Pi; lo x lo dropped): |z - z_exact| <= ~1.3e-5 sqrt(m) sigma (dropped term
+// 2^-22, TF32 truncation of the lo operands 2^-21, fp32 accumulation of 48 MMAs at <= 2^-22 of ||x|| each; ||x|| = sqrt(m) sigma
+// bounds every partial sum); the guard band is 4.5x that plus the fp32 rounding of tau * sigma.  A code whose z is inside the
+// band of a neighbouring threshold (0.1-2 % of the codes) is recomputed with the exact fp64 chain, so the packed bytes are
+// identical to the exact kernel's.  (A single TF32 product with its 1.2e-3 sqrt(m) sigma worst-case band was measured too:
+// 2-10 % rechecks, slower overall.)
+__device__ __forceinline__ float fast_guard(int m) { return 6.0e-5f * sqrtf((float)m) + 2.0e-5f; }
+__device__ __forceinline__ uint32_t tf32_rna(float x)
+{
+    uint32_t r;
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x));
+    return r;
+}
+__device__ __forceinline__ void mma_tf32(float (&c)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1)
+{
+    asm volatile("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                 : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3]) : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+
 __device__ __forceinline__ double to_f64(float v) { return (double)v; }
 __device__ __forceinline__ double to_f64(__nv_bfloat16 v) { return (double)__bfloat162float(v); }
 
-template <typename T, bool ROPE, bool PAGED>
-__global__ void __launch_bounds__(kAppendThreads, 4)
+template <typename T, bool ROPE, bool PAGED, bool FAST>
+__global__ void __launch_bounds__(kAppendThreads, FAST ? 3 : 4)
 quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__ cache,
                        const T *__restrict__ k_new, const T *__restrict__ v_new,
                        const double *__restrict__ cb64, const float *__restrict__ rot_t, int batch,
                        int n_new, int Hkv, const int32_t *__restrict__ seq_len, int64_t n_cap,
                        int64_t max_tokens, const int32_t *__restrict__ pages, int pstride, int64_t n_pages,
                        const float *__restrict__ rope_cos, const float *__restrict__ rope_sin, int pairing, int cb_exact,
-                       int max_rows)
+                       int max_rows, const float2 *__restrict__ rot_hl)
 {
     extern __shared__ __align__(16) unsigned char smem[];
     const int tid = threadIdx.x;
+#if BGTQ_APPEND_PHASES
+    long long aph_t[8] = {0, 0, 0, 0, 0, 0, 0, 0}, aph_last = clock64();
+    int aph_cur = 7;
+#define APH(i) do { const long long now_ = clock64(); aph_t[aph_cur] += now_ - aph_last; aph_last = now_; aph_cur = (i); } while (0)
+#else
+#define APH(i) do { } while (0)
+#endif
     const int h = blockIdx.y % Hkv, lrel = blockIdx.y / Hkv, s = blockIdx.z;
     const int64_t t0 = seq_len[s];
     const int64_t t_end = min(t0 + (int64_t)n_new, max_tokens);
@@ -115,7 +207,13 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
     // exact-density codebooks: V has its own flat table (C_{w, m} of the V group of width w; 512 more thresholds); else V
     // shares the flat table of K
     double *tauV_own = reinterpret_cast<double *>(reinterpret_cast<unsigned char *>(Msp) + kMetaBytes);
-    uint32_t *tbuf = reinterpret_cast<uint32_t *>(reinterpret_cast<unsigned char *>(Msp) + kMetaBytes + (cb_exact ? 512 * 8 : 0));   // tile, `stride` bytes
+    unsigned char *after_tabs = reinterpret_cast<unsigned char *>(Msp) + kMetaBytes + (cb_exact ? 512 * 8 : 0);
+    // fast path: fp32 thresholds (K table, V table), work items, recheck queue
+    float *tau32 = reinterpret_cast<float *>(after_tabs);                           // [2][512]
+    FastItem *items = reinterpret_cast<FastItem *>(tau32 + 1024);                   // [kMaxFastItems]
+    uint16_t *queue = reinterpret_cast<uint16_t *>(items + kMaxFastItems);          // [kFastQueue]
+    int *qcount = reinterpret_cast<int *>(queue + kFastQueue);                      // [0] entries, [1] items
+    uint32_t *tbuf = reinterpret_cast<uint32_t *>(after_tabs + (FAST ? 1024 * 4 + kMaxFastItems * sizeof(FastItem) + kFastQueue * 2 + 16 : 0));   // tile, `stride` bytes
     // The metadata is read many times by single threads (unit list, group search, radii); one coalesced copy into
     // shared memory replaces those dependent global-memory round trips -- they dominated the one-token append.
     {
@@ -159,8 +257,20 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
             if (K.off1 != 0xFFFF) { units[n++] = UnitDesc{K.off1, K.b, K.nc1, (uint16_t)(M.gstart[g] + 8 * j), 0}; ++j; }
         }
         *n_units_p = n;
+        if (FAST) {                               // n-tiles of every rotation group of this head
+            int ni = 0;
+            for (int g = 0; g < ng; ++g)
+                for (int n0 = 0; n0 < M.gm[g]; n0 += 16) items[ni++] = FastItem{M.gstart[g], (uint8_t)M.gm[g], (uint8_t)n0, M.gb[g], (uint8_t)g, 0, 0};
+            for (int gv = 0; gv < nvg; ++gv)
+                for (int n0 = 0; n0 < 16 * M.vgcnt[gv]; n0 += 16)
+                    items[ni++] = FastItem{(uint16_t)(128 + 16 * M.vgstart[gv]), (uint8_t)(16 * M.vgcnt[gv]), (uint8_t)n0, M.vgb[gv], (uint8_t)(ng + gv), 1, 0};
+            qcount[1] = ni;
+        }
     }
     __syncthreads();
+    if (FAST)
+        for (int i = tid; i < 1022; i += kAppendThreads) tau32[i + (i >= 511 ? 1 : 0)] = (float)(i < 511 ? tau[i] : tauV[i - 511]);
+    const int n_items = FAST ? qcount[1] : 0;
     const int n_units = *n_units_p;
 
     // this thread's row of the rotation: col < kdim -> K group row, col >= 128 -> row of its V group (grouped V order)
@@ -192,6 +302,7 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
         const int64_t base = tile_lo + i * kSub;
         const int64_t nlo = max(lo, base), nhi = min(hi, base + kSub);
         if (nlo >= nhi) continue;
+        APH(0);
         // ---- 1. gather the sub-batch: xs[tt][0..127] = K in grouped order, xs[tt][128..255] = V.  Thread c owns
         //      (grouped V order) column c (its source coordinate is fixed), so the kSub loads are independent and in flight together.
         {
@@ -220,6 +331,7 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
             }
         }
         __syncthreads();
+        APH(1);
         // ---- 2. radii: ss = fma chain, r = sqrt(ss), sigma = r / sqrt(m), h = fp16_rne_sat(r)
         if (tid < kSub * ns && base + tid / ns >= nlo && base + tid / ns < nhi) {
             int tt = tid / ns, g = tid % ns;
@@ -234,117 +346,248 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
             if (r >= 65520.0) hb = 0x7BFF;
             nrm[tt * ns + g] = hb;
         }
-        // ---- 3. rotation: z[tt] = fma chain over k of Pi[r][k] * x_k (k ascending: the oracle's order).
-        //      Rotation rows are read 4 at a time ahead of the chain; a single new token (decode-time
-        //      append) takes the scalar path so that the step is latency- not throughput-shaped.
         const int tt_lo = (int)(nlo - base), tt_hi = (int)(nhi - base);
-        double z[kSub];
+        if constexpr (FAST) {
+            APH(2);
+            // ---- 3'. z ~ X Pi^T on the tensor cores: warp w takes items w, w+8, ...; accumulators stay in registers
+            const int warp = tid >> 5, lane = tid & 31, fg = lane >> 2, fc = lane & 3;
+            if (tid == 0) qcount[0] = 0;
+            float acc[kFastPerWarp][2][4];
 #pragma unroll
-        for (int tt = 0; tt < kSub; ++tt) z[tt] = 0.0;
-        if (my_m > 0) {
-            const double *x = xs + my_x0;
-            if (tt_hi - tt_lo == 1) {
-                const double *x1 = x + tt_lo * 256;
-                double zz = 0.0;
-                int k = 0;
-                for (; k + 32 <= my_m; k += 32) {            // 32 independent loads in flight, then the chain
-                    float pf[32];
+            for (int ii = 0; ii < kFastPerWarp; ++ii) {
 #pragma unroll
-                    for (int u = 0; u < 32; ++u) pf[u] = __ldg(myrot + (size_t)(k + u) * my_m);
-#pragma unroll
-                    for (int u = 0; u < 32; ++u) zz = __fma_rn((double)pf[u], x1[k + u], zz);
-                }
-                for (; k + 8 <= my_m; k += 8) {
-                    float pf[8];
-#pragma unroll
-                    for (int u = 0; u < 8; ++u) pf[u] = __ldg(myrot + (size_t)(k + u) * my_m);
-#pragma unroll
-                    for (int u = 0; u < 8; ++u) zz = __fma_rn((double)pf[u], x1[k + u], zz);
-                }
-                for (; k < my_m; ++k) zz = __fma_rn((double)__ldg(myrot + (size_t)k * my_m), x1[k], zz);
-#pragma unroll
-                for (int tt = 0; tt < kSub; ++tt) if (tt == tt_lo) z[tt] = zz;
-            } else {
-                int k = 0;
-                // blocks of 4 rotation entries, the next block's loads issued before this block's 64 chained FMAs:
-                // the table is an L2 hit (4 CTAs x 56 KB leave little L1), so its latency has to be covered
-                const int kend4 = my_m & ~3;
-                float pc[4];
-                if (kend4 > 0) {
-#pragma unroll
-                    for (int u = 0; u < 4; ++u) pc[u] = __ldg(myrot + (size_t)u * my_m);
-                }
-                for (; k < kend4; k += 4) {
-                    float pn[4];
-                    const int kn = k + 4 < kend4 ? k + 4 : k;           // (the last block re-reads itself: no branch)
-#pragma unroll
-                    for (int u = 0; u < 4; ++u) pn[u] = __ldg(myrot + (size_t)(kn + u) * my_m);
-                    const double p0 = (double)pc[0], p1 = (double)pc[1], p2 = (double)pc[2], p3 = (double)pc[3];
-#pragma unroll
-                    for (int tt = 0; tt < kSub; ++tt) {
-                        const double2 xa = *reinterpret_cast<const double2 *>(x + tt * 256 + k);
-                        const double2 xb = *reinterpret_cast<const double2 *>(x + tt * 256 + k + 2);
-                        z[tt] = __fma_rn(p3, xb.y, __fma_rn(p2, xb.x, __fma_rn(p1, xa.y, __fma_rn(p0, xa.x, z[tt]))));
+                for (int e = 0; e < 4; ++e) acc[ii][0][e] = acc[ii][1][e] = 0.f;
+                const int item = warp + ii * kFastWarps;
+                if (item < n_items) {
+                    const FastItem it = items[item];
+                    const int m = it.m, nA = it.n0 + fg, nB = nA + 8;
+                    const bool two = it.n0 + 8 < m;                                // (warp-uniform) the second n-tile exists
+                    const double *xa = xs + fg * 256 + it.x0;                     // token row fg; row fg + 8 is 8 * 256 further
+                    const float2 *RA = rot_hl + rot_offset(m) + (size_t)(nA < m ? nA : 0) * m;   // B(k, n) = Pi^(m)[n][k]
+                    const float2 *RB = rot_hl + rot_offset(m) + (size_t)(nB < m ? nB : 0) * m;
+                    const float2 zero2 = make_float2(0.f, 0.f);
+                    auto ldb = [&](const float2 *R, bool vn, int k) { return (vn && k < m) ? __ldg(R + k) : zero2; };
+                    float2 pa0 = ldb(RA, nA < m, fc), pa1 = ldb(RA, nA < m, fc + 4);
+                    float2 pb0 = ldb(RB, nB < m, fc), pb1 = ldb(RB, nB < m, fc + 4);
+                    for (int k0 = 0; k0 < m; k0 += 8) {
+                        const float2 ca0 = pa0, ca1 = pa1, cb0 = pb0, cb1 = pb1;
+                        pa0 = ldb(RA, nA < m, k0 + 8 + fc); pa1 = ldb(RA, nA < m, k0 + 12 + fc);     // next k-step, in flight during the MMAs
+                        if (two) { pb0 = ldb(RB, nB < m, k0 + 8 + fc); pb1 = ldb(RB, nB < m, k0 + 12 + fc); }
+                        const int ka = k0 + fc, kb = ka + 4;
+                        const bool va = ka < m, vb = kb < m;
+                        const float a0 = va ? (float)xa[ka] : 0.f, a1 = va ? (float)xa[8 * 256 + ka] : 0.f;
+                        const float a2 = vb ? (float)xa[kb] : 0.f, a3 = vb ? (float)xa[8 * 256 + kb] : 0.f;
+                        const uint32_t ah[4] = {tf32_rna(a0), tf32_rna(a1), tf32_rna(a2), tf32_rna(a3)};
+                        const uint32_t al[4] = {__float_as_uint(a0 - __uint_as_float(ah[0])), __float_as_uint(a1 - __uint_as_float(ah[1])),
+                                                __float_as_uint(a2 - __uint_as_float(ah[2])), __float_as_uint(a3 - __uint_as_float(ah[3]))};
+                        mma_tf32(acc[ii][0], al, __float_as_uint(ca0.x), __float_as_uint(ca1.x));   // small terms first
+                        mma_tf32(acc[ii][0], ah, __float_as_uint(ca0.y), __float_as_uint(ca1.y));
+                        mma_tf32(acc[ii][0], ah, __float_as_uint(ca0.x), __float_as_uint(ca1.x));
+                        if (two) {
+                            mma_tf32(acc[ii][1], al, __float_as_uint(cb0.x), __float_as_uint(cb1.x));
+                            mma_tf32(acc[ii][1], ah, __float_as_uint(cb0.y), __float_as_uint(cb1.y));
+                            mma_tf32(acc[ii][1], ah, __float_as_uint(cb0.x), __float_as_uint(cb1.x));
+                        }
                     }
-#pragma unroll
-                    for (int u = 0; u < 4; ++u) pc[u] = pn[u];
-                }
-                for (; k + 4 <= my_m; k += 4) {
-                    float pf[4];
-#pragma unroll
-                    for (int u = 0; u < 4; ++u) pf[u] = __ldg(myrot + (size_t)(k + u) * my_m);
-                    const double p0 = (double)pf[0], p1 = (double)pf[1], p2 = (double)pf[2], p3 = (double)pf[3];
-                    // x[tt][k..k+3] as two 16-byte loads (group starts are even and k is a multiple of 4, so the
-                    // address is 16-byte aligned); per token the chain still runs over k in ascending order
-#pragma unroll
-                    for (int tt = 0; tt < kSub; ++tt) {
-                        const double2 xa = *reinterpret_cast<const double2 *>(x + tt * 256 + k);
-                        const double2 xb = *reinterpret_cast<const double2 *>(x + tt * 256 + k + 2);
-                        z[tt] = __fma_rn(p3, xb.y, __fma_rn(p2, xb.x, __fma_rn(p1, xa.y, __fma_rn(p0, xa.x, z[tt]))));
-                    }
-                }
-                for (; k < my_m; ++k) {
-                    const double pi = (double)__ldg(myrot + (size_t)k * my_m);
-#pragma unroll
-                    for (int tt = 0; tt < kSub; ++tt) z[tt] = __fma_rn(pi, x[tt * 256 + k], z[tt]);
                 }
             }
-        }
-        __syncthreads();
-        // ---- 4. scalar quantise: idx = #{k : z > tau_k * sigma}; the predicate is monotone in k
-        if (my_m > 0) {
-            const double *tb = (col >= 128 ? tauV : tau) + ((1 << my_b) - 1);
-            // the count is found bit by bit (always my_b probes), all kSub searches side by side so that the
-            // dependent LDS -> DMUL -> DSETP chains of different tokens overlap; same count as any other search
-            // because the predicate is monotone in k
-            const double *sgp = sigma + my_g;
-            if (tt_hi - tt_lo == 1) {                         // decode-time append: one token, one search
-                double zz = 0.0;
+            __syncthreads();                                                       // sigma of step 2 is complete
+            APH(3);
+            // ---- 4'. codes from z where it is clear of the neighbouring thresholds; the rest go to the queue
 #pragma unroll
-                for (int tt = 0; tt < kSub; ++tt) if (tt == tt_lo) zz = z[tt];
-                const double sg = sgp[tt_lo * ns];
+            for (int ii = 0; ii < kFastPerWarp; ++ii) {
+                const int item = warp + ii * kFastWarps;
+                if (item < n_items) {
+                    const FastItem it = items[item];
+                    const float *tb = tau32 + (it.isv ? 512 : 0) + ((1 << it.b) - 1);
+                    const float gc = fast_guard(it.m);
+                    const int L = 1 << it.b;
+                    // the eight searches of a lane side by side (the probes of one search are a dependent LDS -> FMUL -> FSETP chain)
+                    float z8[8], sg8[8];
+                    int a8[8];
+                    bool ok[8];
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) {
+                        const int tt = fg + 8 * ((e >> 1) & 1), nl = it.n0 + 8 * (e >> 2) + 2 * fc + (e & 1);
+                        ok[e] = nl < it.m && tt >= tt_lo && tt < tt_hi;
+                        z8[e] = acc[ii][e >> 2][e & 3];
+                        sg8[e] = ok[e] ? (float)sigma[tt * ns + it.sidx] : 0.f;
+                        a8[e] = 0;
+                    }
+                    for (int bit = it.b - 1; bit >= 0; --bit) {
+                        const int step = 1 << bit;
+#pragma unroll
+                        for (int e = 0; e < 8; ++e)
+                            if (z8[e] > tb[a8[e] + step - 1] * sg8[e]) a8[e] += step;
+                    }
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) {
+                        if (!ok[e]) continue;
+                        const int tt = fg + 8 * ((e >> 1) & 1), col = it.x0 + it.n0 + 8 * (e >> 2) + 2 * fc + (e & 1);
+                        const int a = a8[e];
+                        const float z = z8[e], sg = sg8[e], gd = gc * sg;
+                        const float tlo = tb[a > 0 ? a - 1 : 0] * sg, thi = tb[a < L - 1 ? a : 0] * sg;
+                        const bool risky = (a > 0 && !(z - tlo > gd)) || (a < L - 1 && !(thi - z > gd));
+                        idxs[tt * 256 + col] = (uint8_t)a;
+                        if (risky) queue[atomicAdd(&qcount[0], 1)] = (uint16_t)((tt << 8) | col);
+                    }
+                }
+            }
+            __syncthreads();
+            APH(4);
+            // ---- 4''. the exact fp64 chain (oracle order) for the queued (token, column) pairs
+            const int qn = qcount[0];
+            for (int e = tid; e < qn; e += kAppendThreads) {
+                const int ent = queue[e], tt = ent >> 8, col = ent & 255;
+                int m, x0, sidx, b;
+                const double *tb;
+                if (col >= 128) {
+                    const int gv = M.vbg[(col - 128) >> 4];
+                    m = 16 * M.vgcnt[gv]; x0 = 128 + 16 * M.vgstart[gv]; sidx = ng + gv; b = M.vgb[gv]; tb = tauV + ((1 << b) - 1);
+                } else {
+                    int g = 0;
+                    while (g + 1 < ng && col >= M.gstart[g + 1]) ++g;
+                    m = M.gm[g]; x0 = M.gstart[g]; sidx = g; b = M.gb[g]; tb = tau + ((1 << b) - 1);
+                }
+                // row (col - x0) of Pi^(m), contiguous: hi + lo is the fp32 entry exactly; 16-byte loads, 16 in flight
+                const float4 *Rq = reinterpret_cast<const float4 *>(rot_hl + rot_offset(m) + (size_t)(col - x0) * m);
+                const double *x = xs + tt * 256 + x0;
+                double zz = 0.0;
+                int k = 0;
+                for (; k + 32 <= m; k += 32) {
+                    float4 pf[16];
+#pragma unroll
+                    for (int u = 0; u < 16; ++u) pf[u] = __ldg(Rq + (k >> 1) + u);
+#pragma unroll
+                    for (int u = 0; u < 16; ++u) {
+                        zz = __fma_rn((double)(pf[u].x + pf[u].y), x[k + 2 * u], zz);
+                        zz = __fma_rn((double)(pf[u].z + pf[u].w), x[k + 2 * u + 1], zz);
+                    }
+                }
+                for (; k < m; k += 2) {                                          // (m is even)
+                    const float4 p = __ldg(Rq + (k >> 1));
+                    zz = __fma_rn((double)(p.x + p.y), x[k], zz);
+                    zz = __fma_rn((double)(p.z + p.w), x[k + 1], zz);
+                }
+                const double sg = sigma[tt * ns + sidx];
                 int a = 0;
-                for (int bit = my_b - 1; bit >= 0; --bit)
+                for (int bit = b - 1; bit >= 0; --bit)
                     if (zz > __dmul_rn(tb[a + (1 << bit) - 1], sg)) a += 1 << bit;
-                idxs[tt_lo * 256 + col] = (uint8_t)a;
-            } else
-#pragma unroll
-            for (int t0h = 0; t0h < kSub; t0h += 8) {         // 8 searches side by side (register budget: 64)
-                int a[8];
-#pragma unroll
-                for (int tt = 0; tt < 8; ++tt) a[tt] = 0;
-                for (int bit = my_b - 1; bit >= 0; --bit) {
-                    const int step = 1 << bit;
-#pragma unroll
-                    for (int tt = 0; tt < 8; ++tt)
-                        if (z[t0h + tt] > __dmul_rn(tb[a[tt] + step - 1], sgp[(t0h + tt) * ns])) a[tt] += step;
+                idxs[tt * 256 + col] = (uint8_t)a;
+            }
+        } else {
+            // ---- 3. rotation: z[tt] = fma chain over k of Pi[r][k] * x_k (k ascending: the oracle's order).
+            //      Rotation rows are read 4 at a time ahead of the chain; a single new token (decode-time
+            //      append) takes the scalar path so that the step is latency- not throughput-shaped.
+            double z[kSub];
+    #pragma unroll
+            for (int tt = 0; tt < kSub; ++tt) z[tt] = 0.0;
+            if (my_m > 0) {
+                const double *x = xs + my_x0;
+                if (tt_hi - tt_lo == 1) {
+                    const double *x1 = x + tt_lo * 256;
+                    double zz = 0.0;
+                    int k = 0;
+                    for (; k + 32 <= my_m; k += 32) {            // 32 independent loads in flight, then the chain
+                        float pf[32];
+    #pragma unroll
+                        for (int u = 0; u < 32; ++u) pf[u] = __ldg(myrot + (size_t)(k + u) * my_m);
+    #pragma unroll
+                        for (int u = 0; u < 32; ++u) zz = __fma_rn((double)pf[u], x1[k + u], zz);
+                    }
+                    for (; k + 8 <= my_m; k += 8) {
+                        float pf[8];
+    #pragma unroll
+                        for (int u = 0; u < 8; ++u) pf[u] = __ldg(myrot + (size_t)(k + u) * my_m);
+    #pragma unroll
+                        for (int u = 0; u < 8; ++u) zz = __fma_rn((double)pf[u], x1[k + u], zz);
+                    }
+                    for (; k < my_m; ++k) zz = __fma_rn((double)__ldg(myrot + (size_t)k * my_m), x1[k], zz);
+    #pragma unroll
+                    for (int tt = 0; tt < kSub; ++tt) if (tt == tt_lo) z[tt] = zz;
+                } else {
+                    int k = 0;
+                    // blocks of 4 rotation entries, the next block's loads issued before this block's 64 chained FMAs:
+                    // the table is an L2 hit (4 CTAs x 56 KB leave little L1), so its latency has to be covered
+                    const int kend4 = my_m & ~3;
+                    float pc[4];
+                    if (kend4 > 0) {
+    #pragma unroll
+                        for (int u = 0; u < 4; ++u) pc[u] = __ldg(myrot + (size_t)u * my_m);
+                    }
+                    for (; k < kend4; k += 4) {
+                        float pn[4];
+                        const int kn = k + 4 < kend4 ? k + 4 : k;           // (the last block re-reads itself: no branch)
+    #pragma unroll
+                        for (int u = 0; u < 4; ++u) pn[u] = __ldg(myrot + (size_t)(kn + u) * my_m);
+                        const double p0 = (double)pc[0], p1 = (double)pc[1], p2 = (double)pc[2], p3 = (double)pc[3];
+    #pragma unroll
+                        for (int tt = 0; tt < kSub; ++tt) {
+                            const double2 xa = *reinterpret_cast<const double2 *>(x + tt * 256 + k);
+                            const double2 xb = *reinterpret_cast<const double2 *>(x + tt * 256 + k + 2);
+                            z[tt] = __fma_rn(p3, xb.y, __fma_rn(p2, xb.x, __fma_rn(p1, xa.y, __fma_rn(p0, xa.x, z[tt]))));
+                        }
+    #pragma unroll
+                        for (int u = 0; u < 4; ++u) pc[u] = pn[u];
+                    }
+                    for (; k + 4 <= my_m; k += 4) {
+                        float pf[4];
+    #pragma unroll
+                        for (int u = 0; u < 4; ++u) pf[u] = __ldg(myrot + (size_t)(k + u) * my_m);
+                        const double p0 = (double)pf[0], p1 = (double)pf[1], p2 = (double)pf[2], p3 = (double)pf[3];
+                        // x[tt][k..k+3] as two 16-byte loads (group starts are even and k is a multiple of 4, so the
+                        // address is 16-byte aligned); per token the chain still runs over k in ascending order
+    #pragma unroll
+                        for (int tt = 0; tt < kSub; ++tt) {
+                            const double2 xa = *reinterpret_cast<const double2 *>(x + tt * 256 + k);
+                            const double2 xb = *reinterpret_cast<const double2 *>(x + tt * 256 + k + 2);
+                            z[tt] = __fma_rn(p3, xb.y, __fma_rn(p2, xb.x, __fma_rn(p1, xa.y, __fma_rn(p0, xa.x, z[tt]))));
+                        }
+                    }
+                    for (; k < my_m; ++k) {
+                        const double pi = (double)__ldg(myrot + (size_t)k * my_m);
+    #pragma unroll
+                        for (int tt = 0; tt < kSub; ++tt) z[tt] = __fma_rn(pi, x[tt * 256 + k], z[tt]);
+                    }
                 }
-#pragma unroll
-                for (int tt = 0; tt < 8; ++tt)
-                    if (t0h + tt >= tt_lo && t0h + tt < tt_hi) idxs[(t0h + tt) * 256 + col] = (uint8_t)a[tt];
+            }
+            __syncthreads();
+            // ---- 4. scalar quantise: idx = #{k : z > tau_k * sigma}; the predicate is monotone in k
+            if (my_m > 0) {
+                const double *tb = (col >= 128 ? tauV : tau) + ((1 << my_b) - 1);
+                // the count is found bit by bit (always my_b probes), all kSub searches side by side so that the
+                // dependent LDS -> DMUL -> DSETP chains of different tokens overlap; same count as any other search
+                // because the predicate is monotone in k
+                const double *sgp = sigma + my_g;
+                if (tt_hi - tt_lo == 1) {                         // decode-time append: one token, one search
+                    double zz = 0.0;
+    #pragma unroll
+                    for (int tt = 0; tt < kSub; ++tt) if (tt == tt_lo) zz = z[tt];
+                    const double sg = sgp[tt_lo * ns];
+                    int a = 0;
+                    for (int bit = my_b - 1; bit >= 0; --bit)
+                        if (zz > __dmul_rn(tb[a + (1 << bit) - 1], sg)) a += 1 << bit;
+                    idxs[tt_lo * 256 + col] = (uint8_t)a;
+                } else
+    #pragma unroll
+                for (int t0h = 0; t0h < kSub; t0h += 8) {         // 8 searches side by side (register budget: 64)
+                    int a[8];
+    #pragma unroll
+                    for (int tt = 0; tt < 8; ++tt) a[tt] = 0;
+                    for (int bit = my_b - 1; bit >= 0; --bit) {
+                        const int step = 1 << bit;
+    #pragma unroll
+                        for (int tt = 0; tt < 8; ++tt)
+                            if (z[t0h + tt] > __dmul_rn(tb[a[tt] + step - 1], sgp[(t0h + tt) * ns])) a[tt] += step;
+                    }
+    #pragma unroll
+                    for (int tt = 0; tt < 8; ++tt)
+                        if (t0h + tt >= tt_lo && t0h + tt < tt_hi) idxs[(t0h + tt) * 256 + col] = (uint8_t)a[tt];
+                }
             }
         }
         __syncthreads();
+        APH(5);
         // ---- 5. pack the sub-batch's fields; each (unit, lane) word set has exactly one owner
         if (M.format == 2) {
             // BGTQ-v2: a K word belongs to one token (composed whole), a V word to one dimension and 32 tokens (read-modify-write)
@@ -385,14 +628,26 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
                 const UnitDesc U = units[it >> 5];
                 const int lp = it & 31, lanes = 8 * U.nc;
                 if (lp >= lanes) continue;
-                const int g8 = lp / U.nc, c = lp % U.nc;
+                // lp = g8 * nc + c with nc in 1..4 lanes per row: no integer division (nc = 3: g8 = lp * 11 >> 5 for lp < 24)
+                const int g8 = U.nc == 4 ? lp >> 2 : (U.nc == 2 ? lp >> 1 : (U.nc == 1 ? lp : (lp * 11) >> 5)), c = lp - g8 * U.nc;
                 uint32_t *wbase = tbuf + (U.off >> 2) + lp;
-                for (int p = 0; p < 2; ++p) {
-                    int tt = 8 * p + g8;
-                    int64_t tok = base + tt;
-                    if (tok < nlo || tok >= nhi) continue;
-                    for (int q = 0; q < 2; ++q)
-                        put_field(wbase, lanes, U.b, i * 4 + p * 2 + q, idxs[tt * 256 + U.ustart + 2 * c + q]);
+                if constexpr (FAST) {
+                    unsigned f[4], pm = 0;
+#pragma unroll
+                    for (int sl = 0; sl < 4; ++sl) {                   // slot 4i + 2p + q: token row 8p + g8, coordinate 2c + q
+                        const int tt = 8 * (sl >> 1) + g8;
+                        f[sl] = idxs[tt * 256 + U.ustart + 2 * c + (sl & 1)];
+                        if (tt >= tt_lo && tt < tt_hi) pm |= 1u << sl;
+                    }
+                    pack4(wbase, lanes, U.b, i, f, pm);
+                } else {                                               // (64-register budget: the word-wise packer makes the rotation loop spill)
+                    for (int p = 0; p < 2; ++p) {
+                        int tt = 8 * p + g8;
+                        int64_t tok = base + tt;
+                        if (tok < nlo || tok >= nhi) continue;
+                        for (int q = 0; q < 2; ++q)
+                            put_field(wbase, lanes, U.b, i * 4 + p * 2 + q, idxs[tt * 256 + U.ustart + 2 * c + q]);
+                    }
                 }
             } else {
                 const int v = it - kitems, unit = v >> 5, lane = v & 31;   // unit = 2J' + rho, J' = grouped V block
@@ -400,13 +655,24 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
                 const int u = 16 * (unit >> 1) + 8 * (unit & 1) + gq;      // grouped V coordinate
                 const int bw = M.vbw[unit >> 1];
                 uint32_t *wbase = tbuf + ((M.vboff[unit >> 1] + (unit & 1) * 128 * bw) >> 2) + lane;
-                for (int o = 0; o < 2; ++o)
-                    for (int e = 0; e < 2; ++e) {
-                        int tt = 8 * o + 2 * c + e;
-                        int64_t tok = base + tt;
-                        if (tok < nlo || tok >= nhi) continue;
-                        put_field(wbase, 32, bw, i * 4 + o * 2 + e, idxs[tt * 256 + 128 + u]);
+                if constexpr (FAST) {
+                    unsigned f[4], pm = 0;
+#pragma unroll
+                    for (int sl = 0; sl < 4; ++sl) {                   // slot 4i + 2o + e: token row 8o + 2c + e
+                        const int tt = 8 * (sl >> 1) + 2 * c + (sl & 1);
+                        f[sl] = idxs[tt * 256 + 128 + u];
+                        if (tt >= tt_lo && tt < tt_hi) pm |= 1u << sl;
                     }
+                    pack4(wbase, 32, bw, i, f, pm);
+                } else {
+                    for (int o = 0; o < 2; ++o)
+                        for (int e = 0; e < 2; ++e) {
+                            int tt = 8 * o + 2 * c + e;
+                            int64_t tok = base + tt;
+                            if (tok < nlo || tok >= nhi) continue;
+                            put_field(wbase, 32, bw, i * 4 + o * 2 + e, idxs[tt * 256 + 128 + u]);
+                        }
+                }
             }
         }
         if (tid < kSub * ns) {   // fp16 norms: token tau at entry (tau&7)*16 + (tau>>4)*2 + ((tau>>3)&1)
@@ -421,11 +687,19 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
         }
         __syncthreads();
     }
+    APH(6);
     {   // write the tile back
         uint4 *dst = reinterpret_cast<uint4 *>(gtile);
         const uint4 *src = reinterpret_cast<const uint4 *>(tbuf);
         for (int i = tid; i < stride / 16; i += kAppendThreads) dst[i] = src[i];
     }
+#if BGTQ_APPEND_PHASES
+    APH(7);
+    if ((tid == 0 || tid == 200) && blockIdx.x == 3 && blockIdx.y == 0 && blockIdx.z == 0)
+        printf("append phases (tid %d, FAST %d): gather %lld radii %lld mma %lld quant %lld recheck %lld pack %lld writeback %lld setup %lld\n", tid, (int)FAST,
+               aph_t[0], aph_t[1], aph_t[2], aph_t[3], aph_t[4], aph_t[5], aph_t[6], aph_t[7]);
+#endif
+#undef APH
 }
 
 __global__ void advance_seq_len_kernel(int32_t *seq_len, int batch, int n_new, int64_t max_tokens)
@@ -437,23 +711,36 @@ __global__ void advance_seq_len_kernel(int32_t *seq_len, int batch, int n_new, i
     }
 }
 
-static size_t append_smem_bytes(int max_stride, int max_rows, bool cb_exact = false)
+static size_t append_smem_bytes(int max_stride, int max_rows, bool cb_exact = false, bool fast = false)
 {
     return (size_t)kSub * 256 * 8 + 512 * 8 + kSub * max_rows * 8 + (kSub * max_rows + 8) * 2 + kSub * 256 +
-           kMaxUnits * sizeof(UnitDesc) + 16 + kMetaBytes + (cb_exact ? 512 * 8 : 0) + (size_t)max_stride + 64;
+           kMaxUnits * sizeof(UnitDesc) + 16 + kMetaBytes + (cb_exact ? 512 * 8 : 0) +
+           (fast ? 1024 * 4 + kMaxFastItems * sizeof(FastItem) + kFastQueue * 2 + 16 : 0) + (size_t)max_stride + 64;
 }
+
+// Bulk appends (>= kFastMinTokens new tokens per sequence) take the tensor-core fast path; the decode-time append keeps the
+// latency-shaped exact kernel.  Both write identical bytes.
+constexpr int kFastMinTokens = 16;
 
 int launch_quantize_append(const bgtq_layout *lay, int layer, int n_layers, void *cache, const void *k_new,
                            const void *v_new, int dt, int batch, int n_new, int32_t *seq_len,
                            int advance, int64_t max_tokens, const PageMap *pm, const RopeTab *rope, cudaStream_t st)
 {
     const int64_t n_cap = (max_tokens + kTile - 1) / kTile;
-    const size_t smem = append_smem_bytes(lay->max_stride, lay->max_rows, lay->cb_exact != 0);
+    // The fast kernel runs 3 CTAs per SM (80 registers, 12 KB more shared memory), the exact one 4: a grid that fits one wave of
+    // the exact kernel but not of the fast one would lose more to the second wave than the fast path gains (measured: 514
+    // CTAs, 30 vs 39 G codes/s), so those grids keep the exact kernel.
+    const int64_t n_cta = (int64_t)((n_new + kTile - 1) / kTile + 1) * lay->n_kv_heads * n_layers * batch;
+    const bool fast = n_new >= kFastMinTokens && !append_exact_only() &&
+                      (n_cta <= 3 * (int64_t)lay->sm_count || n_cta > 8 * (int64_t)lay->sm_count);
+    const size_t smem = append_smem_bytes(lay->max_stride, lay->max_rows, lay->cb_exact != 0, fast);
     dim3 grid((n_new + kTile - 1) / kTile + 1, lay->n_kv_heads * n_layers, batch);
     const HeadMeta *metas = lay->d_meta + (size_t)layer * lay->n_kv_heads;
     if (first_use_on_device(1)) {   // once per device, outside any stream capture
-        const int maxs = (int)append_smem_bytes(16 * kDh * 8 + 256 * 16 + 16 * kDh * 8, 16, true);
-#define BGTQ_APPEND_ATTR(T, R, G) CUDA_TRY(cudaFuncSetAttribute(quantize_append_kernel<T, R, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, maxs))
+        const int maxs = (int)append_smem_bytes(16 * kDh * 8 + 256 * 16 + 16 * kDh * 8, 16, true, true);
+#define BGTQ_APPEND_ATTR(T, R, G) \
+        CUDA_TRY(cudaFuncSetAttribute(quantize_append_kernel<T, R, G, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, maxs)); \
+        CUDA_TRY(cudaFuncSetAttribute(quantize_append_kernel<T, R, G, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, maxs))
         BGTQ_APPEND_ATTR(float, false, false); BGTQ_APPEND_ATTR(__nv_bfloat16, false, false);
         BGTQ_APPEND_ATTR(float, true, false);  BGTQ_APPEND_ATTR(__nv_bfloat16, true, false);
         BGTQ_APPEND_ATTR(float, false, true);  BGTQ_APPEND_ATTR(__nv_bfloat16, false, true);
@@ -470,14 +757,14 @@ int launch_quantize_append(const bgtq_layout *lay, int layer, int n_layers, void
         const double *cb = lay->cb_exact ? lay->d_hcb64 + (size_t)layer * lay->n_kv_heads * 1024 : lay->d_cb64;
         kern<<<grid, kAppendThreads, smem, st>>>(metas, (uint8_t *)cache, kp, vp, cb, lay->d_rot_t, batch, n_new,
                                                  lay->n_kv_heads, seq_len, n_cap, max_tokens, pt, pstride, n_pages, rc, rs,
-                                                 lay->pairing, lay->cb_exact, lay->max_rows);
+                                                 lay->pairing, lay->cb_exact, lay->max_rows, lay->d_rot_hl);
     };
-    if (dt == BGTQ_F32)
-        launch(quantize_append_kernel<float, false, false>, quantize_append_kernel<float, true, false>,
-               quantize_append_kernel<float, false, true>, (const float *)k_new, (const float *)v_new);
-    else
-        launch(quantize_append_kernel<__nv_bfloat16, false, false>, quantize_append_kernel<__nv_bfloat16, true, false>,
-               quantize_append_kernel<__nv_bfloat16, false, true>, (const __nv_bfloat16 *)k_new, (const __nv_bfloat16 *)v_new);
+#define BGTQ_APPEND_LAUNCH(T, F) \
+        launch(quantize_append_kernel<T, false, false, F>, quantize_append_kernel<T, true, false, F>, \
+               quantize_append_kernel<T, false, true, F>, (const T *)k_new, (const T *)v_new)
+    if (dt == BGTQ_F32) { if (fast) BGTQ_APPEND_LAUNCH(float, true); else BGTQ_APPEND_LAUNCH(float, false); }
+    else { if (fast) BGTQ_APPEND_LAUNCH(__nv_bfloat16, true); else BGTQ_APPEND_LAUNCH(__nv_bfloat16, false); }
+#undef BGTQ_APPEND_LAUNCH
     count_launch();
     CUDA_TRY(cudaGetLastError());
     if (advance) {

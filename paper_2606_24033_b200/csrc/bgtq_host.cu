@@ -118,6 +118,13 @@ extern "C" int bgtq_block_energy(const void *q, int64_t n_q, const void *k, int6
                                eq_out, ek_out, workspace, workspace_bytes, (cudaStream_t)stream);
 }
 
+static std::atomic<bool> g_append_exact_only{false};
+namespace bgtq {
+bool append_exact_only() { return g_append_exact_only.load(); }
+void set_append_exact_only(bool on) { g_append_exact_only.store(on); }
+}  // namespace bgtq
+extern "C" int bgtq_debug_append_exact_only(int on) { return g_append_exact_only.exchange(on != 0) ? 1 : 0; }
+
 extern "C" int bgtq_block_energy_static_max_row_elems(void) { return block_energy_static_max_row_elems(); }
 
 extern "C" int bgtq_block_energy_static(const void *q, int64_t n_q, const void *k, int64_t n_k, int dt,
@@ -360,7 +367,7 @@ static int layout_create_impl(const uint8_t *bits, const uint8_t *bits_v, int n_
     lay->d_h = d_h; lay->b_v = b_v; lay->pairing = pairing;
     lay->format = format; lay->d_planes = nullptr;
     lay->cb_exact = cb_exact; lay->d_hcb16 = nullptr; lay->d_hcb64 = nullptr;
-    lay->d_meta = nullptr; lay->d_rot = nullptr; lay->d_rot_t = nullptr; lay->d_cb16 = nullptr; lay->d_cb64 = nullptr;
+    lay->d_meta = nullptr; lay->d_rot = nullptr; lay->d_rot_t = nullptr; lay->d_rot_hl = nullptr; lay->d_cb16 = nullptr; lay->d_cb64 = nullptr;
     lay->meta.resize((size_t)n_layers * n_kv_heads);
     int64_t prefix = 0;
     lay->max_stride = 0;
@@ -396,6 +403,15 @@ static int layout_create_impl(const uint8_t *bits, const uint8_t *bits_v, int n_
         float *T = rot_t.data() + rot_offset(m);
         for (int j = 0; j < m; ++j)
             for (int k = 0; k < m; ++k) T[(size_t)k * m + j] = P[(size_t)j * m + k];
+    }
+    std::vector<float2> rot_hl((size_t)rot_n);        // hi = Pi rounded to TF32 (10-bit mantissa, ties away), lo = Pi - hi (exact)
+    for (int64_t i = 0; i < rot_n; ++i) {
+        uint32_t u;
+        std::memcpy(&u, &rotations[i], 4);
+        u = (u + 0x1000u) & 0xFFFFE000u;
+        float hi;
+        std::memcpy(&hi, &u, 4);
+        rot_hl[(size_t)i] = make_float2(hi, rotations[i] - hi);
     }
     std::vector<uint16_t> cb16(512, 0);
     std::vector<double> cb64(512, 0.0);
@@ -456,6 +472,8 @@ static int layout_create_impl(const uint8_t *bits, const uint8_t *bits_v, int n_
     if (e == cudaSuccess) e = cudaMalloc(&lay->d_meta, lay->meta.size() * sizeof(HeadMeta));
     if (e == cudaSuccess) e = cudaMalloc(&lay->d_rot, rot_n * sizeof(float));
     if (e == cudaSuccess) e = cudaMalloc(&lay->d_rot_t, rot_n * sizeof(float));
+    if (e == cudaSuccess) e = cudaMalloc(&lay->d_rot_hl, rot_n * sizeof(float2));
+    if (e == cudaSuccess) e = cudaMemcpy(lay->d_rot_hl, rot_hl.data(), rot_n * sizeof(float2), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMalloc(&lay->d_cb16, 512 * sizeof(uint16_t));
     if (e == cudaSuccess) e = cudaMalloc(&lay->d_cb64, 512 * sizeof(double));
     if (e == cudaSuccess && cb_exact) e = cudaMalloc(&lay->d_hcb16, hcb16.size() * sizeof(uint16_t));
@@ -480,7 +498,7 @@ static int layout_create_impl(const uint8_t *bits, const uint8_t *bits_v, int n_
 extern "C" void bgtq_layout_destroy(bgtq_layout *lay)
 {
     if (!lay) return;
-    cudaFree(lay->d_meta); cudaFree(lay->d_rot); cudaFree(lay->d_rot_t);
+    cudaFree(lay->d_meta); cudaFree(lay->d_rot); cudaFree(lay->d_rot_t); cudaFree(lay->d_rot_hl);
     cudaFree(lay->d_cb16); cudaFree(lay->d_cb64); cudaFree(lay->d_planes); cudaFree(lay->d_hcb16); cudaFree(lay->d_hcb64);
     delete lay;
 }

@@ -82,6 +82,7 @@ struct bgtq_layout {
     bgtq::HeadMeta *d_meta;               // device copy
     float *d_rot;                         // rotation table, row-major Pi^(m)[j][k]
     float *d_rot_t;                       // transposed: Pi^(m)[j][k] stored at [k][j]
+    float2 *d_rot_hl;                     // row-major {tf32(Pi), Pi - tf32(Pi)}: operands of the append fast path
     uint16_t *d_cb16;                     // fp16 bits of the 511 codebook levels (C_b at 2^b-1)
     double *d_cb64;                       // same levels as fp64
     // exact-density codebooks (cb_exact = 1): one table set per (layer, kv head) -- groups and widths are
@@ -148,6 +149,9 @@ int block_energy_static_max_row_elems();
 int launch_v_block_energy(const void *v, int64_t n, int dt, int Hkv, int d_h, float *scores, void *ws, cudaStream_t st);
 int launch_allocate(const float *scores, int n_heads, int L, int b_min, int b_max, int B,
                     uint8_t *bits, cudaStream_t st);
+// test hook (bgtq_debug_append_exact_only): force the exact fp64 append kernel for bulk appends too
+bool append_exact_only();
+void set_append_exact_only(bool on);
 int debug_decode_unit_exact(int b, int m, const uint32_t *words, float *values);
 int launch_quantize_append(const bgtq_layout *lay, int layer, int n_layers, void *cache, const void *k_new,
                            const void *v_new, int dt, int batch, int n_new, int32_t *seq_len,

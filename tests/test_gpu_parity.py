@@ -921,3 +921,34 @@ def test_exact_density_codebooks_append_and_attention(P, rot128, T, Hq, Hkv, b_k
     assert err <= 2e-3, err
     with pytest.raises(P.BgtqError):
         P.prefill_attention(lay, 0, cache, _cuda(p.q_post[None, None], torch.bfloat16), seq, max_tokens, scale)
+
+
+# ----------------------------------------------------------------------------- a4 fast path (tensor cores + exact recheck)
+@pytest.mark.parametrize("kv_dtype,n_new", [("f32", 1000), ("bf16", 16), ("f32", 130)])
+def test_append_fast_path_writes_the_exact_kernels_bytes(P, tab128, kv_dtype, n_new):
+    """Bulk appends (>= 16 tokens) run the TF32 tensor-core path with an exact fp64 recheck inside the guard band; the
+    bytes must equal those of the exact fp64 kernel (forced with the test hook) and of the oracle, for every width 1..8
+    on both sides of the cache."""
+    p = H.make_problem(77, n_new, 8, 2, 3, 3, 1, 8, kv_dtype=kv_dtype)
+    p.bits[0, :] = np.resize(np.arange(1, 9), 64)            # every K width, eight groups of 16 coordinates
+    bits_v = np.array([[1, 2, 3, 4, 5, 6, 7, 8], [3] * 8], np.uint8)
+    lay = P.Layout(p.bits[None], p.Hq, p.d_h, 0, p.rot, bits_v=bits_v[None])
+    tdt = torch.float32 if kv_dtype == "f32" else torch.bfloat16
+    k, v = _cuda(p.k_post[None], tdt), _cuda(p.v[None], tdt)
+    caches = []
+    try:
+        for exact_only in (False, True):
+            assert P.append_exact_only(exact_only) in (False, True)
+            cache = lay.new_cache(1, 1024)
+            seq = torch.zeros(1, dtype=torch.int32, device="cuda")
+            P.quantize_append(lay, 0, cache, k, v, seq, 1024)
+            caches.append(cache.cpu().numpy())
+    finally:
+        P.append_exact_only(False)
+    assert np.array_equal(caches[0], caches[1])
+    for h in range(2):
+        qh = O.quantize_head(p.k_post[:, h], p.v[:, h], p.bits[h], 0, tab128, bits_v=bits_v[h])
+        stride, off = lay.tile_stride(0, h), lay.region_offset(0, 0, h, 1, 1024)
+        exp = np.zeros(8 * stride, dtype=np.uint8)
+        O.pack_region(qh, p.d_h, exp)
+        assert np.array_equal(caches[0][off:off + 8 * stride], exp), h
