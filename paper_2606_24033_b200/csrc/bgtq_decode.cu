@@ -225,12 +225,24 @@ qfold_kernel(const HeadMeta *__restrict__ metas, const float *__restrict__ rot_t
         sc = scale_log2e / sqrtf((float)m) * (BGTQ_NORM_IN_OPERAND ? 64.f : 1.f);   // 2^6: see qk_group_n
         ks = ksbase[g] + (r >> 4); kap = r & 15;
         const uint8_t *co = M.coords + x0;
-        for (int k0 = 0; k0 < m; k0 += 16 * PARTS) {        // 16 independent rotation loads in flight per thread
-            float tv[16];
+        if constexpr (PARTS == 1) {                         // throughput form: full rounds unmasked, scalar tail
+            int k = 0;
+            for (; k + 16 <= m; k += 16) {
+                float tv[16];
 #pragma unroll
-            for (int u = 0; u < 16; ++u) { const int k = k0 + part + PARTS * u; tv[u] = k < m ? __ldg(T + (size_t)k * m) : 0.f; }
+                for (int u = 0; u < 16; ++u) tv[u] = __ldg(T + (size_t)(k + u) * m);
 #pragma unroll
-            for (int u = 0; u < 16; ++u) { const int k = k0 + part + PARTS * u; acc = fmaf(tv[u], k < m ? qs[co[k]] : 0.f, acc); }
+                for (int u = 0; u < 16; ++u) acc = fmaf(tv[u], qs[co[k + u]], acc);
+            }
+            for (; k < m; ++k) acc = fmaf(__ldg(T + (size_t)k * m), qs[co[k]], acc);
+        } else {
+            for (int k0 = 0; k0 < m; k0 += 16 * PARTS) {    // 16 independent rotation loads in flight per thread, masked tail round
+                float tv[16];
+#pragma unroll
+                for (int u = 0; u < 16; ++u) { const int k = k0 + part + PARTS * u; tv[u] = k < m ? __ldg(T + (size_t)k * m) : 0.f; }
+#pragma unroll
+                for (int u = 0; u < 16; ++u) { const int k = k0 + part + PARTS * u; acc = fmaf(tv[u], k < m ? qs[co[k]] : 0.f, acc); }
+            }
         }
     }
 #pragma unroll
