@@ -2187,42 +2187,79 @@ prefill_ws_kernel(const PrefillParams P)
             tc_fence_after();
             const int rel = (int)max((int64_t)-1, min((int64_t)1 << 20, prow - (int64_t)t * kTile));   // columns > rel are in the future
             const bool nomask = __all_sync(0xFFFFFFFFu, rel >= 127);
-            float mx = -INFINITY;
+            float alpha = 1.f, ls = 0.f;
+            bool two_pass = t == 0 || !nomask;
+            if (!two_pass) {
+                // ---- ONE pass over S with the running REFERENCE m_run instead of this tile's maximum: p = 2^(s - m_run).  softmax
+                // does not care which reference is subtracted as long as nothing overflows; a row whose tile maximum exceeds the
+                // reference by more than 2^8 (p would leave the comfortable fp16 range) sends the warp to the two-pass path below,
+                // which moves the reference and rescales O.  Saves the second TMEM read and the max -> exp dependency; the next
+                // chunk's tcgen05.ld is in flight while this chunk's exponentials run.
+                mbar_wait(bar[WS_ODONE], parp); tc_fence_after();          // PV(t-1) has consumed P; O is stable
+                float mx = -INFINITY;
+                uint32_t sa[32], sb[32];
+                tmem_ld32(t_s, sa);
 #pragma unroll
-            for (int ch = 0; ch < 4; ++ch) {
-                uint32_t sr[32];
-                tmem_ld32(t_s + 32 * ch, sr);
-                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-                if (nomask) {
+                for (int ch = 0; ch < 4; ++ch) {
+                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                    uint32_t (&cur)[32] = (ch & 1) ? sb : sa;
+                    uint32_t (&nxt)[32] = (ch & 1) ? sa : sb;
+                    if (ch < 3) tmem_ld32(t_s + 32 * (ch + 1), nxt);
 #pragma unroll
-                    for (int i = 0; i < 32; i += 2) mx = fmax3(mx, __uint_as_float(sr[i]), __uint_as_float(sr[i + 1]));
-                } else {
+                    for (int j = 0; j < 4; ++j) {                        // 8 tokens = one 16-byte chunk of the P row
+                        float p[8];
 #pragma unroll
-                    for (int i = 0; i < 32; ++i) mx = fmaxf(mx, 32 * ch + i > rel ? -INFINITY : __uint_as_float(sr[i]));
-                }
-            }
-            const float mn = fmaxf(m_run, mx);                       // finite: tile 0 holds position 0
-            const float alpha = fast_exp2(m_run - mn);
-            m_run = mn;
-            if (t > 0) { mbar_wait(bar[WS_ODONE], parp); tc_fence_after(); }    // PV(t-1) has consumed P; O is stable
-            float ls = 0.f;
-#pragma unroll
-            for (int ch = 0; ch < 4; ++ch) {
-                uint32_t sr[32];
-                tmem_ld32(t_s + 32 * ch, sr);
-                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {                        // 8 tokens = one 16-byte chunk of the P row
-                    float p[8];
-#pragma unroll
-                    for (int e = 0; e < 8; ++e) {
-                        const int i = 32 * ch + 8 * j + e;
-                        p[e] = (!nomask && i > rel) ? 0.f : fast_exp2(__uint_as_float(sr[8 * j + e]) - mn);
-                        ls += p[e];
+                        for (int e = 0; e < 8; e += 2) {
+                            const float x0 = __uint_as_float(cur[8 * j + e]), x1 = __uint_as_float(cur[8 * j + e + 1]);
+                            mx = fmax3(mx, x0, x1);
+                            p[e] = fast_exp2(x0 - m_run); p[e + 1] = fast_exp2(x1 - m_run);
+                            ls += p[e] + p[e + 1];
+                        }
+                        const uint4 v = make_uint4(pack_half2(p[0], p[1]), pack_half2(p[2], p[3]), pack_half2(p[4], p[5]), pack_half2(p[6], p[7]));
+                        const int col = 32 * ch + 8 * j;
+                        *reinterpret_cast<uint4 *>(prow_s + (col >> 6) * 16384 + ((((col & 63) >> 3) ^ (row & 7)) << 4)) = v;
                     }
-                    const uint4 v = make_uint4(pack_half2(p[0], p[1]), pack_half2(p[2], p[3]), pack_half2(p[4], p[5]), pack_half2(p[6], p[7]));
-                    const int col = 32 * ch + 8 * j;
-                    *reinterpret_cast<uint4 *>(prow_s + (col >> 6) * 16384 + ((((col & 63) >> 3) ^ (row & 7)) << 4)) = v;
+                }
+                two_pass = __any_sync(0xFFFFFFFFu, mx > m_run + 8.f);
+            }
+            if (two_pass) {
+                float mx = -INFINITY;
+#pragma unroll
+                for (int ch = 0; ch < 4; ++ch) {
+                    uint32_t sr[32];
+                    tmem_ld32(t_s + 32 * ch, sr);
+                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                    if (nomask) {
+#pragma unroll
+                        for (int i = 0; i < 32; i += 2) mx = fmax3(mx, __uint_as_float(sr[i]), __uint_as_float(sr[i + 1]));
+                    } else {
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) mx = fmaxf(mx, 32 * ch + i > rel ? -INFINITY : __uint_as_float(sr[i]));
+                    }
+                }
+                const float mn = fmaxf(m_run, mx);                       // finite: tile 0 holds position 0
+                alpha = fast_exp2(m_run - mn);
+                m_run = mn;
+                if (t > 0) { mbar_wait(bar[WS_ODONE], parp); tc_fence_after(); }    // PV(t-1) has consumed P; O is stable (a no-op after a one-pass attempt)
+                ls = 0.f;
+#pragma unroll
+                for (int ch = 0; ch < 4; ++ch) {
+                    uint32_t sr[32];
+                    tmem_ld32(t_s + 32 * ch, sr);
+                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {                        // 8 tokens = one 16-byte chunk of the P row
+                        float p[8];
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) {
+                            const int i = 32 * ch + 8 * j + e;
+                            p[e] = (!nomask && i > rel) ? 0.f : fast_exp2(__uint_as_float(sr[8 * j + e]) - mn);
+                            ls += p[e];
+                        }
+                        const uint4 v = make_uint4(pack_half2(p[0], p[1]), pack_half2(p[2], p[3]), pack_half2(p[4], p[5]), pack_half2(p[6], p[7]));
+                        const int col = 32 * ch + 8 * j;
+                        *reinterpret_cast<uint4 *>(prow_s + (col >> 6) * 16384 + ((((col & 63) >> 3) ^ (row & 7)) << 4)) = v;
+                    }
                 }
             }
             tc_fence_before();
