@@ -2096,10 +2096,12 @@ prefill_ws_kernel(const PrefillParams P)
         if (lane == 0) {
             mbar_expect_tx(bar[WS_KFULL], kbytes); bulk_g2s(raw_s, region, kbytes, bar[WS_KFULL]);
             mbar_expect_tx(bar[WS_VFULL], vbytes); bulk_g2s(raw_s + kbytes, region + kbytes, vbytes, bar[WS_VFULL]);
-            for (int t = 0; t < n_tiles; ++t) {
-                const uint32_t par = t & 1, parp = (t - 1) & 1;
-                mbar_wait(bar[WS_KREADY], par);
-                if (t > 0) mbar_wait(bar[WS_SFREE], parp);
+            // Issue order S(0), [S(t+1), O(t)] for t = 0 ..: S(t+1) = Q'K^T of the NEXT tile goes to the tensor pipe ahead of
+            // O(t) += P(t) V^(t), so the softmax warps get S(t+1) one MMA sooner (the S buffer is free as soon as softmax(t) has
+            // read it, which is just before P(t) is ready).
+            auto issue_s = [&](int t) {
+                mbar_wait(bar[WS_KREADY], t & 1);
+                if (t > 0) mbar_wait(bar[WS_SFREE], (t - 1) & 1);
                 tc_fence_after();
 #pragma unroll
                 for (int r = 0; r < RT; ++r) umma_128x128x128(tm + r * 128, qs_s + r * 32768, khat_s, false);          // S_r = Q'_r . K^T
@@ -2108,8 +2110,16 @@ prefill_ws_kernel(const PrefillParams P)
                     const uint8_t *src = region + (int64_t)(t + 1) * M.tile_stride;
                     mbar_expect_tx(bar[WS_KFULL], kbytes); bulk_g2s(raw_s, src, kbytes, bar[WS_KFULL]);
                 }
-                mbar_wait(bar[WS_VREADY], par);
-                mbar_wait(bar[WS_PREADY], par);
+            };
+            issue_s(0);
+            for (int t = 0; t < n_tiles; ++t) {
+                const uint32_t par = t & 1;
+                // whichever is ready first; S(t+1) ahead of O(t) when both are
+                bool s_done = t + 1 >= n_tiles;
+                for (;;) {
+                    if (!s_done && mbar_test(bar[WS_KREADY], (t + 1) & 1) && mbar_test(bar[WS_SFREE], par)) { issue_s(t + 1); s_done = true; }
+                    if (mbar_test(bar[WS_VREADY], par) && mbar_test(bar[WS_PREADY], par)) break;
+                }
                 tc_fence_after();
 #pragma unroll
                 for (int r = 0; r < RT; ++r) umma_128x128x128(tm + (RT + r) * 128, ps_s + r * 32768, vhat_s, t > 0);   // O_r (+)= P_r . V^
@@ -2118,6 +2128,7 @@ prefill_ws_kernel(const PrefillParams P)
                     const uint8_t *src = region + (int64_t)(t + 1) * M.tile_stride + kbytes;
                     mbar_expect_tx(bar[WS_VFULL], vbytes); bulk_g2s(raw_s + kbytes, src, vbytes, bar[WS_VFULL]);
                 }
+                if (!s_done) issue_s(t + 1);
             }
         }
     } else if (warp >= 8) {
@@ -2188,14 +2199,13 @@ prefill_ws_kernel(const PrefillParams P)
             const int rel = (int)max((int64_t)-1, min((int64_t)1 << 20, prow - (int64_t)t * kTile));   // columns > rel are in the future
             const bool nomask = __all_sync(0xFFFFFFFFu, rel >= 127);
             float alpha = 1.f, ls = 0.f;
-            bool two_pass = t == 0 || !nomask;
+            bool two_pass = t == 0 || !nomask, s_freed = false;
             if (!two_pass) {
                 // ---- ONE pass over S with the running REFERENCE m_run instead of this tile's maximum: p = 2^(s - m_run).  softmax
                 // does not care which reference is subtracted as long as nothing overflows; a row whose tile maximum exceeds the
                 // reference by more than 2^8 (p would leave the comfortable fp16 range) sends the warp to the two-pass path below,
                 // which moves the reference and rescales O.  Saves the second TMEM read and the max -> exp dependency; the next
                 // chunk's tcgen05.ld is in flight while this chunk's exponentials run.
-                mbar_wait(bar[WS_ODONE], parp); tc_fence_after();          // PV(t-1) has consumed P; O is stable
                 float mx = -INFINITY;
                 uint32_t sa[32], sb[32];
                 tmem_ld32(t_s, sa);
@@ -2205,13 +2215,24 @@ prefill_ws_kernel(const PrefillParams P)
                     uint32_t (&cur)[32] = (ch & 1) ? sb : sa;
                     uint32_t (&nxt)[32] = (ch & 1) ? sa : sb;
                     if (ch < 3) tmem_ld32(t_s + 32 * (ch + 1), nxt);
+                    else {                                               // the last chunk is in registers: decide now, then S(t+1) may be issued
+#pragma unroll
+                        for (int i = 0; i < 32; i += 2) mx = fmax3(mx, __uint_as_float(cur[i]), __uint_as_float(cur[i + 1]));
+                        two_pass = __any_sync(0xFFFFFFFFu, mx > m_run + 8.f);
+                        if (two_pass) break;                             // (S is read again below: it must not be released)
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(bar[WS_SFREE]);
+                        s_freed = true;
+                    }
+                    if (ch == 0) { mbar_wait(bar[WS_ODONE], parp); tc_fence_after(); }   // before the first P store: PV(t-1) has consumed P
 #pragma unroll
                     for (int j = 0; j < 4; ++j) {                        // 8 tokens = one 16-byte chunk of the P row
                         float p[8];
 #pragma unroll
                         for (int e = 0; e < 8; e += 2) {
                             const float x0 = __uint_as_float(cur[8 * j + e]), x1 = __uint_as_float(cur[8 * j + e + 1]);
-                            mx = fmax3(mx, x0, x1);
+                            if (ch < 3) mx = fmax3(mx, x0, x1);
                             p[e] = fast_exp2(x0 - m_run); p[e + 1] = fast_exp2(x1 - m_run);
                             ls += p[e] + p[e + 1];
                         }
@@ -2220,7 +2241,6 @@ prefill_ws_kernel(const PrefillParams P)
                         *reinterpret_cast<uint4 *>(prow_s + (col >> 6) * 16384 + ((((col & 63) >> 3) ^ (row & 7)) << 4)) = v;
                     }
                 }
-                two_pass = __any_sync(0xFFFFFFFFu, mx > m_run + 8.f);
             }
             if (two_pass) {
                 float mx = -INFINITY;
@@ -2264,7 +2284,7 @@ prefill_ws_kernel(const PrefillParams P)
             }
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive(bar[WS_SFREE]);               // S(t+1) may be issued while O is rescaled
+            if (lane == 0 && !s_freed) mbar_arrive(bar[WS_SFREE]);   // S(t+1) may be issued while O is rescaled
             l_run = fmaf(l_run, alpha, ls);
             if (t > 0 && __any_sync(0xFFFFFFFFu, alpha != 1.f)) {    // a row maximum moved: rescale O in place
 #pragma unroll
