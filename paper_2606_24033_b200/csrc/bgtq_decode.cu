@@ -2005,10 +2005,14 @@ prefill_tc_kernel(const PrefillParams P)
 //   pready       8 softmax warps: P(t) written, O rescaled
 //   odone        tcgen05.commit: O += P(t) V^(t) complete (V^T and P are free again, O is stable)
 enum { WS_KFULL = 0, WS_VFULL, WS_KREADY, WS_VREADY, WS_SFULL, WS_SFREE, WS_PREADY, WS_ODONE, WS_NBARS };
-constexpr int kWsProducers = 7;
+#ifndef BGTQ_WS_PRODUCERS
+#define BGTQ_WS_PRODUCERS 11
+#endif
+constexpr int kWsProducers = BGTQ_WS_PRODUCERS;     // unpack warps (they are the critical path: 7 were busy 87 % of the time)
+constexpr int kWsThreads = 32 * (8 + kWsProducers + 1);   // 8 softmax warps, the producers, one issuer warp
 
 
-__global__ void __launch_bounds__(kTcThreads, 1)
+__global__ void __launch_bounds__(kWsThreads, 1)
 prefill_ws_kernel(const PrefillParams P)
 {
     constexpr int RT = 2;
@@ -2035,12 +2039,12 @@ prefill_ws_kernel(const PrefillParams P)
     if (i_first >= P.n_q || pos0 < 0) return;
     const int n_tiles = (int)((pos0 + i_last) / kTile) + 1;
 
-    build_lut(P.cb16, lut, tid, kTcThreads, true);
+    build_lut(P.cb16, lut, tid, kWsThreads, true);
     if (warp == 0) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" :: "r"(smem_u32(&tmem_base_s)) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
-    for (int i = tid; i < (32768 + 32768) / 16; i += kTcThreads) reinterpret_cast<uint4 *>(khat)[i] = make_uint4(0, 0, 0, 0);   // K^ (zero-width blocks stay 0), V^T
+    for (int i = tid; i < (32768 + 32768) / 16; i += kWsThreads) reinterpret_cast<uint4 *>(khat)[i] = make_uint4(0, 0, 0, 0);   // K^ (zero-width blocks stay 0), V^T
     uint32_t bar[WS_NBARS];
 #pragma unroll
     for (int i = 0; i < WS_NBARS; ++i) bar[i] = smem_u32(&bars[i]);
@@ -2066,7 +2070,7 @@ prefill_ws_kernel(const PrefillParams P)
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         fence_proxy_async();
     }
-    {   // Q' rows -> the A operands.  Row r of the CTA = (token r / G, head r % G); rows past n_q are zero.
+    if (tid < 512) {   // Q' rows -> the A operands.  Row r of the CTA = (token r / G, head r % G); rows past n_q are zero.
         constexpr int TPR = 4 / RT, NV = 4 * RT;                    // threads per row, 16-byte vectors per thread
         const int r = tid / TPR, part = tid % TPR;
         const int kb = (part * 8 * NV) >> 6, j0 = ((part * 8 * NV) & 63) >> 3;
@@ -2091,7 +2095,7 @@ prefill_ws_kernel(const PrefillParams P)
     const uint32_t raw_s = smem_u32(raw), kbytes = M.vnorm_off, vbytes = M.tile_stride - M.vnorm_off;
     const uint32_t qs_s = smem_u32(qs), khat_s = smem_u32(khat), vhat_s = smem_u32(vhat_t), ps_s = smem_u32(ps);
 
-    if (warp == 15) {
+    if (warp == 8 + kWsProducers) {
         // ================= issuer: TMA + tcgen05.mma, one thread
         if (lane == 0) {
             mbar_expect_tx(bar[WS_KFULL], kbytes); bulk_g2s(raw_s, region, kbytes, bar[WS_KFULL]);
@@ -2391,7 +2395,7 @@ int launch_prefill(const bgtq_layout *lay, int layer, const void *cache, const v
     // a sequence shorter than the chunk (seq_len < n_q, a caller error the host cannot see) leaves its rows untouched
     // in the kernels: start from zeros so that the output is defined
     CUDA_TRY(cudaMemsetAsync(opart, 0, rows * Hq * kDh * sizeof(float), st));
-    if (RT == 2) prefill_ws_kernel<<<grid, kTcThreads, smem, st>>>(P);
+    if (RT == 2) prefill_ws_kernel<<<grid, kWsThreads, smem, st>>>(P);
     else prefill_tc_kernel<1><<<grid, kTcThreads, smem, st>>>(P);
     count_launch();
     CUDA_TRY(cudaGetLastError());
