@@ -2119,19 +2119,21 @@ prefill_ws_kernel(const PrefillParams P)
             for (int t = 0; t < n_tiles; ++t) {
                 const uint32_t par = t & 1;
                 // whichever is ready first; S(t+1) ahead of O(t) when both are
-                bool s_done = t + 1 >= n_tiles;
+                bool s_done = t + 1 >= n_tiles, v_req = t + 1 >= n_tiles;
                 for (;;) {
                     if (!s_done && mbar_test(bar[WS_KREADY], (t + 1) & 1) && mbar_test(bar[WS_SFREE], par)) { issue_s(t + 1); s_done = true; }
-                    if (mbar_test(bar[WS_VREADY], par) && mbar_test(bar[WS_PREADY], par)) break;
+                    const bool vr = mbar_test(bar[WS_VREADY], par);
+                    if (vr && !v_req) {                              // the producers are done with the raw V half: fetch the next one now
+                        const uint8_t *src = region + (int64_t)(t + 1) * M.tile_stride + kbytes;
+                        mbar_expect_tx(bar[WS_VFULL], vbytes); bulk_g2s(raw_s + kbytes, src, vbytes, bar[WS_VFULL]);
+                        v_req = true;
+                    }
+                    if (vr && mbar_test(bar[WS_PREADY], par)) break;
                 }
                 tc_fence_after();
 #pragma unroll
                 for (int r = 0; r < RT; ++r) umma_128x128x128(tm + (RT + r) * 128, ps_s + r * 32768, vhat_s, t > 0);   // O_r (+)= P_r . V^
                 umma_commit(bar[WS_ODONE]);
-                if (t + 1 < n_tiles) {
-                    const uint8_t *src = region + (int64_t)(t + 1) * M.tile_stride + kbytes;
-                    mbar_expect_tx(bar[WS_VFULL], vbytes); bulk_g2s(raw_s + kbytes, src, vbytes, bar[WS_VFULL]);
-                }
                 if (!s_done) issue_s(t + 1);
             }
         }
