@@ -233,6 +233,30 @@ def run_reference(args):
     }))
 
 
+# ----------------------------------------------------------------------------- N > 1: replicas only
+def max_over_ranks(ms: float, world: int, device) -> float:
+    """Device time of the slowest rank (the contract's max-over-ranks); identity for one rank.  Any backend: the GPU arm
+    calls it under NCCL, tests/test_bench_cli.py under gloo."""
+    if world == 1:
+        return ms
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def replica_value(bytes_per_step_per_rank: float, ms_max: float, steps: int, world: int) -> float:
+    """Whole-job GB/s of `world` independent replicas (weak scaling, no data-path collective): every rank moves its own
+    bytes, the job takes as long as its slowest rank."""
+    return world * bytes_per_step_per_rank / (ms_max / steps * 1e-3) / 1e9
+
+
+def replica_seed_shift(rank: int) -> int:
+    """Seed shift of a replica: rank r draws its own workload (bench.build_workload(seed_shift=r))."""
+    return rank
+
+
 # ----------------------------------------------------------------------------- GPU arm
 def build_workload(args, P, torch, device, seed_shift: int = 0):
     """Calibrate (energy -> allocate -> layout) and fill the packed cache through the library.
@@ -366,7 +390,7 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=device)
     Lyr = args.layers
-    wl = build_workload(args, P, torch, device, seed_shift=rank)
+    wl = build_workload(args, P, torch, device, seed_shift=replica_seed_shift(rank))
     lay, cache, seq, q, k_new, v_new, ws = (wl[k] for k in ("lay", "cache", "seq", "q", "k_new", "v_new", "ws"))
     out = torch.empty_like(q)
 
@@ -407,15 +431,12 @@ def run_ours(args):
         per = np.array([(e0 if i == 0 else marks[i - 1]).elapsed_time(marks[i]) * 1e3 for i in range(args.steps)])
         step_stats = {"median": float(np.median(per)), "mean": float(per.mean()), "p5": float(np.percentile(per, 5)),
                       "p95": float(np.percentile(per, 95))}
-        if world > 1:
-            t = torch.tensor([ms], device=device, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
+        ms = max_over_ranks(ms, world, device)
         ms_step = ms / args.steps
         seq_avg = seq_start + (args.steps + 1) / 2.0
         io_bytes = 2 * q.numel() * 2 + 2 * k_new.numel() * 4
         bytes_step = seq_avg * wl["tok_bytes"] + io_bytes
-        value = world * bytes_step / (ms_step * 1e-3) / 1e9
+        value = replica_value(bytes_step, ms, args.steps, world)
 
         # ---- roofline of the dominant kernel (split-KV decode), timed alone with CUDA events on its stream
         P.profile_decode(True)
@@ -643,10 +664,7 @@ def run_ours(args):
         b1.record(stream)
         stream.synchronize()
         e2e_ms = b0.elapsed_time(b1) / n_e2e
-        if world > 1:
-            t = torch.tensor([e2e_ms], device=device, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            e2e_ms = float(t.item())
+        e2e_ms = max_over_ranks(e2e_ms, world, device)
         seq_e2e = int(seq[0].item()) - n_e2e / 2.0
         e2e_val = world * (seq_e2e * wl["tok_bytes"] + io_bytes) / (e2e_ms * 1e-3) / 1e9
         h2d = hin.numel()

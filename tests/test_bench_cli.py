@@ -31,3 +31,39 @@ def test_reference_arm_under_torchrun_world2():
     assert r.returncode == 0, r.stderr[-2000:]
     lines = _json_lines(r.stdout)
     assert len(lines) == 1 and lines[0]["n_gpus"] == 2 and lines[0]["impl"] == "reference"
+
+
+def _gloo_worker(rank, world, port, q):
+    import torch
+    import torch.distributed as dist
+    sys.path.insert(0, ROOT)
+    import bench
+    dist.init_process_group("gloo", init_method=f"tcp://127.0.0.1:{port}", rank=rank, world_size=world)
+    try:
+        ms_local = [3.0, 5.0][rank]                          # the second replica is the slow one
+        dist.barrier()
+        ms = bench.max_over_ranks(ms_local, world, torch.device("cpu"))
+        q.put((rank, ms, bench.replica_value(1.0e9, ms, 10, world), bench.replica_seed_shift(rank)))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_replica_aggregation_world2_gloo():
+    """bench.py --gpus N (N > 1) runs independent replicas: per-rank seeds, barrier, max-over-ranks time, whole-job value =
+    N x per-rank bytes / slowest rank's time.  The host logic, exercised with two gloo processes on CPU."""
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_gloo_worker, args=(r, 2, 29647, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    got = sorted(q.get(timeout=120) for _ in range(2))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert [g[0] for g in got] == [0, 1]
+    assert all(g[1] == 5.0 for g in got)                    # both ranks see the slowest rank's time
+    assert all(abs(g[2] - 2 * 1.0e9 / (0.5e-3) / 1e9) < 1e-9 for g in got)     # 2 replicas x 1 GB per step / 0.5 ms per step
+    assert [g[3] for g in got] == [0, 1]                    # distinct workloads per replica
+    import bench
+    assert bench.max_over_ranks(7.0, 1, None) == 7.0 and bench.replica_value(2.0e9, 4.0, 2, 1) == 1000.0
