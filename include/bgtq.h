@@ -60,7 +60,8 @@ int bgtq_codebook(int b, float *levels);
  * q [device] [n_q, n_q_heads, d_h], k [device] [n_k, n_kv_heads, d_h], both of dtype `dt`.
  * scores [device] float [n_kv_heads, d_h/2]; eq_out / ek_out [device] same shape, may be NULL.
  * workspace [device], at least bgtq_block_energy_workspace_bytes(...) bytes; contents scratch.
- * Deterministic (fixed reduction order).  One layer per call. */
+ * Deterministic (fixed reduction order).  One layer per call, ONE kernel launch (a cooperative launch: a grid-wide
+ * barrier separates the streaming pass from the fp64 reduction; needs a device with cooperative-launch support). */
 size_t bgtq_block_energy_workspace_bytes(int n_q_heads, int n_kv_heads, int d_h);
 int bgtq_block_energy(const void *q, int64_t n_q, const void *k, int64_t n_k, int dt,
                       int n_q_heads, int n_kv_heads, int d_h, int pairing, int kind,
@@ -168,8 +169,11 @@ int64_t bgtq_tile_stride(const bgtq_layout *layout, int layer, int kv_head);
 
 /* ---- a4: quantize-on-append.  TQ-MSE per same-width K group and for
  * V as one group; code streams + fp16 norms written in the layout the decode kernel reads
- * (PAPER.md:112, 122).  Arithmetic is the exact fp64 sequence of DESIGN.md section 3 (codes,
- * norms and bytes are bit-exact against the oracle).
+ * (PAPER.md:112, 122).  The result is the exact fp64 sequence of DESIGN.md section 3 (codes, norms and
+ * bytes are bit-exact against the oracle).  A call with fewer than 16 new tokens per sequence evaluates that
+ * sequence directly; a bulk append evaluates the rotation on the tensor cores (TF32, hi/lo split) and
+ * recomputes with the exact fp64 chain every code whose rotated value lies within a guard band of a
+ * quantisation threshold -- the same bytes, checked against the exact kernel (bgtq_debug_append_exact_only).
  * k_new, v_new [device] [batch, n_new, n_kv_heads, d_h] of dtype dt (post-RoPE K).
  * seq_len [device] int32 [batch]: tokens already cached; sequence s receives its n_new tokens at
  *   positions seq_len[s] .. seq_len[s]+n_new-1 and, if advance_seq_len != 0, seq_len[s] is advanced
