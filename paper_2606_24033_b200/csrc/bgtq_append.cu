@@ -365,18 +365,12 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
                     const double *xa = xs + fg * 256 + it.x0;                     // token row fg; row fg + 8 is 8 * 256 further
                     const float2 *RA = rot_hl + rot_offset(m) + (size_t)(nA < m ? nA : 0) * m;   // B(k, n) = Pi^(m)[n][k]
                     const float2 *RB = rot_hl + rot_offset(m) + (size_t)(nB < m ? nB : 0) * m;
-                    const float2 zero2 = make_float2(0.f, 0.f);
-                    auto ldb = [&](const float2 *R, bool vn, int k) { return (vn && k < m) ? __ldg(R + k) : zero2; };
-                    float2 pa0 = ldb(RA, nA < m, fc), pa1 = ldb(RA, nA < m, fc + 4);
-                    float2 pb0 = ldb(RB, nB < m, fc), pb1 = ldb(RB, nB < m, fc + 4);
-                    for (int k0 = 0; k0 < m; k0 += 8) {
-                        const float2 ca0 = pa0, ca1 = pa1, cb0 = pb0, cb1 = pb1;
-                        pa0 = ldb(RA, nA < m, k0 + 8 + fc); pa1 = ldb(RA, nA < m, k0 + 12 + fc);     // next k-step, in flight during the MMAs
-                        if (two) { pb0 = ldb(RB, nB < m, k0 + 8 + fc); pb1 = ldb(RB, nB < m, k0 + 12 + fc); }
-                        const int ka = k0 + fc, kb = ka + 4;
-                        const bool va = ka < m, vb = kb < m;
-                        const float a0 = va ? (float)xa[ka] : 0.f, a1 = va ? (float)xa[8 * 256 + ka] : 0.f;
-                        const float a2 = vb ? (float)xa[kb] : 0.f, a3 = vb ? (float)xa[8 * 256 + kb] : 0.f;
+                    // operand pointers of this lane: B rows are clamped to row 0 for outputs beyond the group (their accumulators
+                    // are never read), so the full k-steps need no predicates at all; only a ragged last k-step is masked
+                    const float2 *pA = RA + fc, *pB = RB + fc;
+                    const double *px = xa + fc;
+                    auto kstep = [&](const float2 ca0, const float2 ca1, const float2 cb0, const float2 cb1,
+                                     const float a0, const float a1, const float a2, const float a3) {
                         const uint32_t ah[4] = {tf32_rna(a0), tf32_rna(a1), tf32_rna(a2), tf32_rna(a3)};
                         const uint32_t al[4] = {__float_as_uint(a0 - __uint_as_float(ah[0])), __float_as_uint(a1 - __uint_as_float(ah[1])),
                                                 __float_as_uint(a2 - __uint_as_float(ah[2])), __float_as_uint(a3 - __uint_as_float(ah[3]))};
@@ -388,6 +382,19 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
                             mma_tf32(acc[ii][1], ah, __float_as_uint(cb0.y), __float_as_uint(cb1.y));
                             mma_tf32(acc[ii][1], ah, __float_as_uint(cb0.x), __float_as_uint(cb1.x));
                         }
+                    };
+                    const int kfull = m & ~7;
+#pragma unroll 2
+                    for (int k0 = 0; k0 < kfull; k0 += 8)
+                        kstep(__ldg(pA + k0), __ldg(pA + k0 + 4), __ldg(pB + k0), __ldg(pB + k0 + 4),
+                              (float)px[k0], (float)px[8 * 256 + k0], (float)px[k0 + 4], (float)px[8 * 256 + k0 + 4]);
+                    if (kfull < m) {                                   // ragged tail: k >= m contributes zero
+                        const bool va = kfull + fc < m, vb = kfull + fc + 4 < m;
+                        const float2 zero2 = make_float2(0.f, 0.f);
+                        kstep(va ? __ldg(pA + kfull) : zero2, vb ? __ldg(pA + kfull + 4) : zero2,
+                              va ? __ldg(pB + kfull) : zero2, vb ? __ldg(pB + kfull + 4) : zero2,
+                              va ? (float)px[kfull] : 0.f, va ? (float)px[8 * 256 + kfull] : 0.f,
+                              vb ? (float)px[kfull + 4] : 0.f, vb ? (float)px[8 * 256 + kfull + 4] : 0.f);
                     }
                 }
             }
