@@ -25,23 +25,60 @@ def _nvcc() -> str:
     return "nvcc"
 
 
-def needs_build() -> bool:
-    if not os.path.exists(LIB):
+OBJ = os.path.join(_HERE, "_obj")          # per-source objects (git-ignored): only stale sources are recompiled, in parallel
+
+
+def _deps(src: str) -> list:
+    return [os.path.join(CSRC, src)] + [os.path.join(CSRC, h) for h in HEADERS] + [os.path.abspath(__file__)]
+
+
+def _obj(src: str) -> str:
+    return os.path.join(OBJ, os.path.splitext(src)[0] + ".o")
+
+
+def _stale(target: str, deps: list) -> bool:
+    if not os.path.exists(target):
         return True
-    t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, s) for s in SOURCES + HEADERS] + [os.path.abspath(__file__)]
+    t = os.path.getmtime(target)
     return any(os.path.getmtime(d) > t for d in deps)
+
+
+def needs_build() -> bool:
+    return _stale(LIB, [d for s in SOURCES for d in _deps(s)])
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not needs_build():
         return LIB
-    cmd = [_nvcc()] + NVCC_FLAGS + os.environ.get("BGTQ_EXTRA_NVCC", "").split() + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SOURCES
-    res = subprocess.run(cmd, cwd=CSRC, capture_output=True, text=True)
+    from concurrent.futures import ThreadPoolExecutor
+    os.makedirs(OBJ, exist_ok=True)
+    extra = os.environ.get("BGTQ_EXTRA_NVCC", "").split()
+    flags = [f for f in NVCC_FLAGS if f != "-shared"] + extra + (["-Xptxas", "-v"] if verbose else [])
+    tag = os.path.join(OBJ, "flags.txt")        # objects built with other flags are stale
+    if not os.path.exists(tag) or open(tag).read() != " ".join(flags):
+        force = True
+
+    def compile_one(src: str):
+        if not force and not _stale(_obj(src), _deps(src)):
+            return None
+        return subprocess.run([_nvcc()] + flags + ["-c", src, "-o", _obj(src)], cwd=CSRC, capture_output=True, text=True)
+
+    with ThreadPoolExecutor(max_workers=min(len(SOURCES), os.cpu_count() or 1)) as pool:
+        results = list(pool.map(compile_one, SOURCES))
+    failed = False
+    for res in results:
+        if res is not None and (verbose or res.returncode != 0):
+            sys.stderr.write(res.stdout + res.stderr)
+        failed |= res is not None and res.returncode != 0
+    if failed:
+        raise RuntimeError("nvcc failed building libbgtq.so")
+    with open(tag, "w") as f:
+        f.write(" ".join(flags))
+    res = subprocess.run([_nvcc(), "-shared", "-o", LIB] + [_obj(s) for s in SOURCES], cwd=CSRC, capture_output=True, text=True)
     if verbose or res.returncode != 0:
         sys.stderr.write(res.stdout + res.stderr)
     if res.returncode != 0:
-        raise RuntimeError("nvcc failed building libbgtq.so")
+        raise RuntimeError("nvcc failed linking libbgtq.so")
     return LIB
 
 

@@ -296,36 +296,40 @@ __device__ __forceinline__ void load_unit_partial(const uint32_t *unit, int g8, 
     for (int i = 0; i < B; ++i) w[i] = act ? wp[i * 8 * nc] : 0u;
 }
 
-// QK^T of one same-width group: all its k16 steps, 8 m-tiles each.  m = coordinates in the
-// group; units of 8 coordinates are contiguous (128*B bytes each), only the last may be partial.
+// word i of this lane at unit[off + i * stride].  Full unit: off = lane, stride = 32.  The group's trailing partial unit
+// (nc = 1..3 lanes per token row hold data, compacted to 8*nc lanes per plane): off = g8*nc + c, stride = 8*nc.  Lanes
+// c >= nc read in-bounds words they do not own (the next plane, the next unit or the K norms that follow the codes in the
+// same half-tile copy): whatever they decode is a finite codebook value and meets the zero rows of q' (qfold_kernel pads
+// every k-step with zeros), so no predicate and no zero fill is needed.
+template <int B>
+__device__ __forceinline__ void load_unit_at(const uint32_t *unit, int off, int stride, uint32_t (&w)[B])
+{
+#pragma unroll
+    for (int i = 0; i < B; ++i) w[i] = unit[off + i * stride];
+}
+
+// QK^T of one same-width group.  m = coordinates in the group; units of 8 coordinates are contiguous
+// (128*B bytes each), only the last may be partial.  Units are taken in pairs (one m16n8k16 step per pair and m-tile); an
+// odd last unit is one m16n8k8 step on the first half of its q' fragment.  The group's first step starts the
+// accumulators (C = 0).
 template <int B, bool P5>
 __device__ __forceinline__ void qk_group(const uint32_t *gcodes, int m, int lane, const uint2 *__restrict__ qfp,
                                          const uint32_t *pools, const uint16_t *lut, float (&A)[8][4])
 {
-    // One loop over the group's k16 steps.  A unit holds 8 coordinates; only the group's last unit may be partial
-    // (nc = lanes per token row that hold data: 4 = full) and the last k-step may lack its second unit (nc1 = 0).
-    // A single loader covers full and partial units (word w of lane g8*nc+c at w*8*nc), so every width
-    // instantiates the unpack twice instead of five times (smaller code, one path).
     const int g8 = lane >> 2, c = lane & 3;
-    const int n_full = m >> 3, rem = (m & 7) >> 1, n_half = n_full + (rem ? 1 : 0);
+    const int n_full = m >> 3, rem = (m & 7) >> 1, n_units = n_full + (rem ? 1 : 0);
+    const int offp = rem ? g8 * rem + c : lane, strp = rem ? 8 * rem : 32;     // addressing of the group's LAST unit
     const uint32_t *u0 = gcodes;
-    bool first = true;                                      // the group's first k-step starts the accumulators (C = 0)
+    bool first = true;
 #pragma unroll 1
-    for (int j = 0; j < n_half; j += 2) {
-        const int nc0 = j < n_full ? 4 : rem;
-        const int nc1 = j + 1 < n_half ? (j + 1 < n_full ? 4 : rem) : 0;
-        uint32_t w0[B], h0[16], h1[16];
+    for (int p = n_units >> 1; p > 0; --p) {
+        uint32_t w0[B], w1[B], h0[16], h1[16];
         const uint2 bq = __ldg(qfp);
-        load_unit_partial<B>(u0, g8, c, nc0, w0);
+        const bool last1 = p == 1 && !(n_units & 1);            // this pair's second unit is the group's last unit
+        load_unit_full<B>(u0, lane, w0);
+        load_unit_at<B>(u0 + 32 * B, last1 ? offp : lane, last1 ? strp : 32, w1);
         decode_unit<B, P5>(w0, pools, lut, h0);
-        if (nc1) {
-            uint32_t w1[B];
-            load_unit_partial<B>(u0 + 32 * B, g8, c, nc1, w1);
-            decode_unit<B, P5>(w1, pools, lut, h1);
-        } else {
-#pragma unroll
-            for (int i = 0; i < 16; ++i) h1[i] = 0u;
-        }
+        decode_unit<B, P5>(w1, pools, lut, h1);
         if (first) {
 #pragma unroll
             for (int i = 0; i < 8; ++i) mma16816_z(A[i], h0[2 * i], h0[2 * i + 1], h1[2 * i], h1[2 * i + 1], bq.x, bq.y);
@@ -336,6 +340,19 @@ __device__ __forceinline__ void qk_group(const uint32_t *gcodes, int m, int lane
         }
         u0 += 64 * B;
         qfp += 32;
+    }
+    if (n_units & 1) {
+        uint32_t w0[B], h0[16];
+        const uint32_t b0 = __ldg(reinterpret_cast<const uint32_t *>(qfp));
+        load_unit_at<B>(u0, offp, strp, w0);
+        decode_unit<B, P5>(w0, pools, lut, h0);
+        if (first) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) mma1688_z(A[i], h0[2 * i], h0[2 * i + 1], b0);
+        } else {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) mma1688(A[i], h0[2 * i], h0[2 * i + 1], b0);
+        }
     }
 }
 
@@ -396,21 +413,37 @@ __device__ __forceinline__ void qk_group_n(const uint32_t *gcodes, int m, int la
 }
 
 // PV of one tile: 16 units of width B -> O[J] += V^T[16 dims x 128 tokens] . P[128 tokens x 8 heads]
+// The eight k-steps of a block go to four accumulators (O[J] and three temporaries started with C = 0), so that four
+// independent HMMAs are in flight instead of one chain of eight; the words of the next block are requested before the
+// MMAs of the current one.
 template <int B, bool P5>
 __device__ __forceinline__ void pv_tile(const uint32_t *vcodes, int lane, const uint32_t (&bP)[8][2],
                                         const uint32_t *pools, const uint16_t *lut, float (&O)[8][4])
 {
+    uint32_t w0[B], w1[B];
+    load_unit_full<B>(vcodes, lane, w0);
+    load_unit_full<B>(vcodes + 32 * B, lane, w1);
 #pragma unroll 1
     for (int J = 0; J < 8; ++J) {
-        uint32_t w0[B], w1[B], h0[16], h1[16];
-        const uint32_t *u0 = vcodes + (2 * J) * 32 * B;
-        load_unit_full<B>(u0, lane, w0);
-        load_unit_full<B>(u0 + 32 * B, lane, w1);
+        uint32_t h0[16], h1[16];
         decode_unit<B, P5>(w0, pools, lut, h0);
         decode_unit<B, P5>(w1, pools, lut, h1);
+        if (J < 7) {
+            const uint32_t *u0 = vcodes + (2 * J + 2) * 32 * B;
+            load_unit_full<B>(u0, lane, w0);
+            load_unit_full<B>(u0 + 32 * B, lane, w1);
+        }
+        float T[3][4];
+        mma16816(O[J], h0[0], h1[0], h0[1], h1[1], bP[0][0], bP[0][1]);
 #pragma unroll
-        for (int kp = 0; kp < 8; ++kp)
-            mma16816(O[J], h0[2 * kp], h1[2 * kp], h0[2 * kp + 1], h1[2 * kp + 1], bP[kp][0], bP[kp][1]);
+        for (int kp = 1; kp < 4; ++kp)
+            mma16816_z(T[kp - 1], h0[2 * kp], h1[2 * kp], h0[2 * kp + 1], h1[2 * kp + 1], bP[kp][0], bP[kp][1]);
+        mma16816(O[J], h0[8], h1[8], h0[9], h1[9], bP[4][0], bP[4][1]);
+#pragma unroll
+        for (int kp = 5; kp < 8; ++kp)
+            mma16816(T[kp - 5], h0[2 * kp], h1[2 * kp], h0[2 * kp + 1], h1[2 * kp + 1], bP[kp][0], bP[kp][1]);
+#pragma unroll
+        for (int e = 0; e < 4; ++e) O[J][e] += (T[0][e] + T[1][e]) + T[2][e];
     }
 }
 
