@@ -176,7 +176,7 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
                        int n_new, int Hkv, const int32_t *__restrict__ seq_len, int64_t n_cap,
                        int64_t max_tokens, const int32_t *__restrict__ pages, int pstride, int64_t n_pages,
                        const float *__restrict__ rope_cos, const float *__restrict__ rope_sin, int pairing, int cb_exact,
-                       int max_rows, const float2 *__restrict__ rot_hl)
+                       int max_rows, const float2 *__restrict__ rot_hl, int skip_full)
 {
     extern __shared__ __align__(16) unsigned char smem[];
     const int tid = threadIdx.x;
@@ -194,6 +194,7 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
     const int64_t tile_lo = tile * kTile;
     const int64_t lo = max(t0, tile_lo), hi = min(t_end, tile_lo + kTile);
     if (lo >= hi) return;
+    if (skip_full && lo == tile_lo && hi == tile_lo + kTile) return;      // whole tiles of new tokens: quantize_tile_kernel
 
     // shared memory carve-up
     double *xs = reinterpret_cast<double *>(smem);                       // [16][256]
@@ -709,6 +710,317 @@ quantize_append_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__
 #undef APH
 }
 
+// ---------------------------------------------------------------- bulk path: a whole tile per pass
+// quantize_tile_kernel: one CTA (512 threads) quantises a tile whose 128 tokens are ALL new (bulk prefill appends), in ONE
+// pass instead of eight 16-token sub-batches: every phase (gather, radii, rotation, threshold search, recheck, packing) runs
+// once over 128 tokens, so its latency is paid once per tile and the rotation operands are read once per tile instead of
+// eight times.  Same arithmetic as the FAST sub-batch path (three TF32 products with hi/lo splits, fast_guard band, exact
+// fp64 chain in oracle order for every code inside the band; radii by the exact fp64 chains), hence the same bytes as the
+// exact kernel.  Partly filled first / last tiles of the same call are left to quantize_append_kernel (skip_full = 1).
+// Not for fused RoPE (the rotated keys are not fp32 values), paged caches or BGTQ-v2.
+constexpr int kTileThreads = 512;
+constexpr int kTileWarps = kTileThreads / 32;
+constexpr int kXsLd = 260;                 // floats per token row of xs: 256 + 4, so the A-fragment reads (row g, column c) hit 32 banks
+constexpr int kTileQueue = 6144;           // recheck queue; when more codes than that sit inside a band every code is rechecked
+
+__device__ __forceinline__ float to_f32(float v) { return v; }
+__device__ __forceinline__ float to_f32(__nv_bfloat16 v) { return __bfloat162float(v); }
+
+static size_t tile_smem_bytes(int max_stride, int max_rows, bool cb_exact)
+{
+    return (size_t)kTile * kXsLd * 4 + (size_t)kTile * max_rows * 8 + 512 * 8 * (cb_exact ? 2 : 1) + 1024 * 4 +
+           (size_t)kTile * max_rows * 2 + 16 + (size_t)kTile * 256 + kMaxUnits * sizeof(UnitDesc) + kMaxFastItems * sizeof(FastItem) +
+           16 + kMetaBytes + (size_t)kTileQueue * 2 + (size_t)max_stride + 64;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(kTileThreads, 1)
+quantize_tile_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__ cache,
+                     const T *__restrict__ k_new, const T *__restrict__ v_new, const double *__restrict__ cb64, int batch,
+                     int n_new, int Hkv, const int32_t *__restrict__ seq_len, int64_t n_cap, int64_t max_tokens,
+                     int cb_exact, int max_rows, const float2 *__restrict__ rot_hl)
+{
+    extern __shared__ __align__(16) unsigned char smem[];
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int h = blockIdx.y % Hkv, lrel = blockIdx.y / Hkv, s = blockIdx.z;
+    const int64_t t0 = seq_len[s];
+    const int64_t t_end = min(t0 + (int64_t)n_new, max_tokens);
+    const int64_t tile = t0 / kTile + blockIdx.x;
+    const int64_t tile_lo = tile * kTile;
+    if (t0 > tile_lo || t_end < tile_lo + kTile) return;                  // not a whole tile of new tokens
+
+    float *xs = reinterpret_cast<float *>(smem);                          // [128][kXsLd]: K in grouped order | V in grouped order
+    double *sigma = reinterpret_cast<double *>(xs + kTile * kXsLd);       // [128][ns]
+    double *tau = sigma + kTile * max_rows;                               // [512] (+ [512] V thresholds with exact-density codebooks)
+    float *tau32 = reinterpret_cast<float *>(tau + (cb_exact ? 1024 : 512));   // [2][512]
+    uint16_t *nrm = reinterpret_cast<uint16_t *>(tau32 + 1024);           // [128][ns]
+    uint8_t *idxs = reinterpret_cast<uint8_t *>(nrm + kTile * max_rows + 8);   // [128][256]
+    UnitDesc *units = reinterpret_cast<UnitDesc *>(idxs + kTile * 256);   // [32]
+    FastItem *items = reinterpret_cast<FastItem *>(units + kMaxUnits);    // [32]
+    int *cnt = reinterpret_cast<int *>(items + kMaxFastItems);            // [0] queue entries, [1] K items, [2] V items, [3] K units
+    HeadMeta *Msp = reinterpret_cast<HeadMeta *>(cnt + 4);
+    uint16_t *queue = reinterpret_cast<uint16_t *>(reinterpret_cast<unsigned char *>(Msp) + kMetaBytes);
+    uint32_t *tbuf = reinterpret_cast<uint32_t *>(queue + kTileQueue);    // the tile, `stride` bytes (16-byte aligned)
+    {
+        const uint32_t *msrc = reinterpret_cast<const uint32_t *>(metas + blockIdx.y);
+        uint32_t *mdst = reinterpret_cast<uint32_t *>(Msp);
+        for (int i = tid; i < (int)(sizeof(HeadMeta) / 4); i += kTileThreads) mdst[i] = __ldg(msrc + i);
+    }
+    __syncthreads();
+    const HeadMeta &M = *Msp;
+    const int stride = M.tile_stride, ng = M.n_groups, kdim = M.kdim;
+    const int nvg = M.n_vgroups, ns = ng + nvg;
+    uint8_t *gtile = cache + n_cap * ((int64_t)batch * M.layer_prefix + (int64_t)s * M.layer_sum + M.head_prefix) + tile * stride;
+    for (int i = tid; i < stride / 16; i += kTileThreads) reinterpret_cast<uint4 *>(tbuf)[i] = make_uint4(0, 0, 0, 0);
+    const double *cbK = cb64 + (cb_exact ? (size_t)blockIdx.y * 1024 : 0);
+    for (int i = tid; i < 511; i += kTileThreads) tau[i] = __dmul_rn(__dadd_rn(cbK[i], cbK[i + 1 < 511 ? i + 1 : i]), 0.5);
+    if (cb_exact) {
+        const double *cbV = cbK + 512;
+        for (int i = tid; i < 511; i += kTileThreads) tau[512 + i] = __dmul_rn(__dadd_rn(cbV[i], cbV[i + 1 < 511 ? i + 1 : i]), 0.5);
+    }
+    const double *tauV = cb_exact ? tau + 512 : tau;
+    if (tid == 0) {
+        int n = 0, j = 0;
+        for (int ks = 0; ks < M.n_ksteps; ++ks) {
+            const KStep &K = M.ksteps[ks];
+            const int g = K.flags >> 4;
+            if (K.flags & 1) j = 0;
+            units[n++] = UnitDesc{K.off0, K.b, K.nc0, (uint16_t)(M.gstart[g] + 8 * j), 0};
+            ++j;
+            if (K.off1 != 0xFFFF) { units[n++] = UnitDesc{K.off1, K.b, K.nc1, (uint16_t)(M.gstart[g] + 8 * j), 0}; ++j; }
+        }
+        cnt[3] = n;
+        int ni = 0;
+        for (int g = 0; g < ng; ++g)
+            for (int n0 = 0; n0 < M.gm[g]; n0 += 16) items[ni++] = FastItem{M.gstart[g], (uint8_t)M.gm[g], (uint8_t)n0, M.gb[g], (uint8_t)g, 0, 0};
+        cnt[1] = ni;
+        for (int gv = 0; gv < nvg; ++gv)
+            for (int n0 = 0; n0 < 16 * M.vgcnt[gv]; n0 += 16)
+                items[ni++] = FastItem{(uint16_t)(128 + 16 * M.vgstart[gv]), (uint8_t)(16 * M.vgcnt[gv]), (uint8_t)n0, M.vgb[gv], (uint8_t)(ng + gv), 1, 0};
+        cnt[2] = ni - cnt[1];
+        cnt[0] = 0;
+    }
+    // ---- 1. gather: thread (column c = tid & 255, token half tid >> 8); inputs are fp32 / bf16 values, exact in fp32
+    {
+        const int col = tid & 255, th = tid >> 8;
+        const T *g_src = col >= 128 ? v_new : k_new;
+        const int g_off = col >= 128 ? 16 * M.vblk[(col - 128) >> 4] + (col & 15) : (col < kdim ? (int)M.coords[col] : -1);
+        const int64_t rstep = (int64_t)Hkv * kDh;
+        const int64_t row0 = ((((int64_t)lrel * batch + s) * n_new + (tile_lo - t0)) * Hkv + h) * kDh + (int64_t)th * 64 * rstep;
+        float *xcol = xs + (size_t)th * 64 * kXsLd + col;
+        if (g_off >= 0) {
+#pragma unroll 8
+            for (int tt = 0; tt < 64; ++tt) xcol[tt * kXsLd] = to_f32(g_src[row0 + tt * rstep + g_off]);
+        } else {
+            for (int tt = 0; tt < 64; ++tt) xcol[tt * kXsLd] = 0.f;
+        }
+    }
+    __syncthreads();
+    for (int i = tid; i < 1022; i += kTileThreads) tau32[i + (i >= 511 ? 1 : 0)] = (float)(i < 511 ? tau[i] : tauV[i - 511]);
+    // ---- 2. radii (exact fp64 chains in oracle order).  The long V chains go first, one per thread of the low warps; the
+    //      second round is dealt from the other end so that no thread gets two long chains.
+    {
+        const int total = kTile * ns, nv = kTile * nvg;
+        int w = tid;
+        for (int r = 0; w < total; ++r, w = kTileThreads * r + ((r & 1) ? kTileThreads - 1 - tid : tid)) {
+            int tt, g;
+            if (w < nv) { tt = w / nvg; g = ng + w % nvg; } else { tt = (w - nv) / ng; g = (w - nv) % ng; }
+            const int x0 = g < ng ? M.gstart[g] : 128 + 16 * M.vgstart[g - ng], m = g < ng ? M.gm[g] : 16 * M.vgcnt[g - ng];
+            const float *x = xs + tt * kXsLd + x0;
+            double ss = 0.0;
+            for (int j = 0; j < m; ++j) { const double xv = (double)x[j]; ss = __fma_rn(xv, xv, ss); }
+            const double r2 = __dsqrt_rn(ss);
+            sigma[tt * ns + g] = __ddiv_rn(r2, __dsqrt_rn((double)m));
+            uint16_t hb = __half_as_ushort(__double2half(r2));
+            if (r2 >= 65520.0) hb = 0x7BFF;
+            nrm[tt * ns + g] = hb;
+        }
+    }
+    __syncthreads();
+    // ---- 3. z ~ X Pi^T on the tensor cores and the threshold search.  Work unit = (item: 16 outputs of one rotation group,
+    //      half: 4 m-tiles = 64 tokens); V units (m = 128, the long ones) are dealt first.
+    {
+        const int fg = lane >> 2, fc = lane & 3;
+        const int nki = cnt[1], nvi = cnt[2], n_work = 2 * (nki + nvi);
+        for (int u = warp; u < n_work; u += kTileWarps) {
+            const int item = u < 2 * nvi ? nki + (u >> 1) : ((u - 2 * nvi) >> 1), half = u & 1;
+            const FastItem it = items[item];
+            const int m = it.m, nA = it.n0 + fg, nB = nA + 8;
+            const bool two = it.n0 + 8 < m;
+            const float2 *pA = rot_hl + rot_offset(m) + (size_t)(nA < m ? nA : 0) * m + fc;
+            const float2 *pB = rot_hl + rot_offset(m) + (size_t)(nB < m ? nB : 0) * m + fc;
+            const float *px = xs + (size_t)(half * 64 + fg) * kXsLd + it.x0 + fc;
+            float acc[4][2][4];
+#pragma unroll
+            for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+                for (int e = 0; e < 4; ++e) acc[mt][0][e] = acc[mt][1][e] = 0.f;
+            auto kstep = [&](const float2 ca0, const float2 ca1, const float2 cb0, const float2 cb1, int k0, bool va, bool vb) {
+#pragma unroll
+                for (int mt = 0; mt < 4; ++mt) {
+                    const float *pm = px + mt * 16 * kXsLd + k0;
+                    const float a0 = va ? pm[0] : 0.f, a1 = va ? pm[8 * kXsLd] : 0.f, a2 = vb ? pm[4] : 0.f, a3 = vb ? pm[8 * kXsLd + 4] : 0.f;
+                    const uint32_t ah[4] = {tf32_rna(a0), tf32_rna(a1), tf32_rna(a2), tf32_rna(a3)};
+                    const uint32_t al[4] = {__float_as_uint(a0 - __uint_as_float(ah[0])), __float_as_uint(a1 - __uint_as_float(ah[1])),
+                                            __float_as_uint(a2 - __uint_as_float(ah[2])), __float_as_uint(a3 - __uint_as_float(ah[3]))};
+                    mma_tf32(acc[mt][0], al, __float_as_uint(ca0.x), __float_as_uint(ca1.x));   // small terms first
+                    mma_tf32(acc[mt][0], ah, __float_as_uint(ca0.y), __float_as_uint(ca1.y));
+                    mma_tf32(acc[mt][0], ah, __float_as_uint(ca0.x), __float_as_uint(ca1.x));
+                    if (two) {
+                        mma_tf32(acc[mt][1], al, __float_as_uint(cb0.x), __float_as_uint(cb1.x));
+                        mma_tf32(acc[mt][1], ah, __float_as_uint(cb0.y), __float_as_uint(cb1.y));
+                        mma_tf32(acc[mt][1], ah, __float_as_uint(cb0.x), __float_as_uint(cb1.x));
+                    }
+                }
+            };
+            const int kfull = m & ~7;
+#pragma unroll 1
+            for (int k0 = 0; k0 < kfull; k0 += 8)
+                kstep(__ldg(pA + k0), __ldg(pA + k0 + 4), __ldg(pB + k0), __ldg(pB + k0 + 4), k0, true, true);
+            if (kfull < m) {                                   // ragged tail: k >= m contributes zero
+                const bool va = kfull + fc < m, vb = kfull + fc + 4 < m;
+                const float2 zero2 = make_float2(0.f, 0.f);
+                kstep(va ? __ldg(pA + kfull) : zero2, vb ? __ldg(pA + kfull + 4) : zero2,
+                      va ? __ldg(pB + kfull) : zero2, vb ? __ldg(pB + kfull + 4) : zero2, kfull, va, vb);
+            }
+            // codes from z where it is clear of the neighbouring thresholds; the rest go to the queue
+            const float *tb = tau32 + (it.isv ? 512 : 0) + ((1 << it.b) - 1);
+            const float gc = fast_guard(it.m);
+            const int L = 1 << it.b;
+#pragma unroll 1
+            for (int mt = 0; mt < 4; ++mt) {
+                float z8[8], sg8[8];
+                int a8[8];
+                bool ok[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    const int tt = half * 64 + mt * 16 + fg + 8 * ((e >> 1) & 1), nl = it.n0 + 8 * (e >> 2) + 2 * fc + (e & 1);
+                    ok[e] = nl < it.m;
+                    z8[e] = acc[mt][e >> 2][e & 3];
+                    sg8[e] = ok[e] ? (float)sigma[tt * ns + it.sidx] : 0.f;
+                    a8[e] = 0;
+                }
+                for (int bit = it.b - 1; bit >= 0; --bit) {
+                    const int step = 1 << bit;
+#pragma unroll
+                    for (int e = 0; e < 8; ++e)
+                        if (z8[e] > tb[a8[e] + step - 1] * sg8[e]) a8[e] += step;
+                }
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    if (!ok[e]) continue;
+                    const int tt = half * 64 + mt * 16 + fg + 8 * ((e >> 1) & 1), col = it.x0 + it.n0 + 8 * (e >> 2) + 2 * fc + (e & 1);
+                    const int a = a8[e];
+                    const float z = z8[e], sg = sg8[e], gd = gc * sg;
+                    const float tlo = tb[a > 0 ? a - 1 : 0] * sg, thi = tb[a < L - 1 ? a : 0] * sg;
+                    const bool risky = (a > 0 && !(z - tlo > gd)) || (a < L - 1 && !(thi - z > gd));
+                    idxs[tt * 256 + col] = (uint8_t)a;
+                    if (risky) {
+                        const int pos = atomicAdd(&cnt[0], 1);
+                        if (pos < kTileQueue) queue[pos] = (uint16_t)((tt << 8) | col);
+                    }
+                }
+            }
+        }
+    }
+    __syncthreads();
+    // ---- 4. the exact fp64 chain (oracle order) for the queued (token, column) pairs
+    {
+        auto exact_code = [&](int tt, int col) {
+            int m, x0, sidx, b;
+            const double *tb;
+            if (col >= 128) {
+                const int gv = M.vbg[(col - 128) >> 4];
+                m = 16 * M.vgcnt[gv]; x0 = 128 + 16 * M.vgstart[gv]; sidx = ng + gv; b = M.vgb[gv]; tb = tauV + ((1 << b) - 1);
+            } else {
+                int g = 0;
+                while (g + 1 < ng && col >= M.gstart[g + 1]) ++g;
+                m = M.gm[g]; x0 = M.gstart[g]; sidx = g; b = M.gb[g]; tb = tau + ((1 << b) - 1);
+            }
+            const float4 *Rq = reinterpret_cast<const float4 *>(rot_hl + rot_offset(m) + (size_t)(col - x0) * m);
+            const float *x = xs + tt * kXsLd + x0;
+            double zz = 0.0;
+            int k = 0;
+            for (; k + 32 <= m; k += 32) {
+                float4 pf[16];
+#pragma unroll
+                for (int u = 0; u < 16; ++u) pf[u] = __ldg(Rq + (k >> 1) + u);
+#pragma unroll
+                for (int u = 0; u < 16; ++u) {
+                    zz = __fma_rn((double)(pf[u].x + pf[u].y), (double)x[k + 2 * u], zz);
+                    zz = __fma_rn((double)(pf[u].z + pf[u].w), (double)x[k + 2 * u + 1], zz);
+                }
+            }
+            for (; k < m; k += 2) {
+                const float4 p = __ldg(Rq + (k >> 1));
+                zz = __fma_rn((double)(p.x + p.y), (double)x[k], zz);
+                zz = __fma_rn((double)(p.z + p.w), (double)x[k + 1], zz);
+            }
+            const double sg = sigma[tt * ns + sidx];
+            int a = 0;
+            for (int bit = b - 1; bit >= 0; --bit)
+                if (zz > __dmul_rn(tb[a + (1 << bit) - 1], sg)) a += 1 << bit;
+            idxs[tt * 256 + col] = (uint8_t)a;
+        };
+        const int qn = cnt[0];
+        if (qn <= kTileQueue) {
+            for (int e = tid; e < qn; e += kTileThreads) exact_code(queue[e] >> 8, queue[e] & 255);
+        } else {                                               // (queue overflow: never seen; every code takes the exact chain)
+            for (int e = tid; e < kTile * 256; e += kTileThreads) {
+                const int tt = e >> 8, col = e & 255;
+                if (col >= 128 || col < kdim) exact_code(tt, col);
+            }
+        }
+    }
+    __syncthreads();
+    // ---- 5. pack: one owner per (unit, lane); its eight four-slot groups (one per m-tile) in turn
+    {
+        const int kitems = cnt[3] * 32;
+        for (int itx = tid; itx < kitems + 16 * 32; itx += kTileThreads) {
+            if (itx < kitems) {
+                const UnitDesc U = units[itx >> 5];
+                const int lp = itx & 31, lanes = 8 * U.nc;
+                if (lp >= lanes) continue;
+                const int g8 = U.nc == 4 ? lp >> 2 : (U.nc == 2 ? lp >> 1 : (U.nc == 1 ? lp : (lp * 11) >> 5)), c = lp - g8 * U.nc;
+                uint32_t *wbase = tbuf + (U.off >> 2) + lp;
+                for (int i = 0; i < 8; ++i) {
+                    unsigned f[4];
+#pragma unroll
+                    for (int sl = 0; sl < 4; ++sl)                    // slot 4i + 2p + q: token 16i + 8p + g8, coordinate 2c + q
+                        f[sl] = idxs[(16 * i + 8 * (sl >> 1) + g8) * 256 + U.ustart + 2 * c + (sl & 1)];
+                    pack4(wbase, lanes, U.b, i, f, 15u);
+                }
+            } else {
+                const int v = itx - kitems, unit = v >> 5, ln = v & 31;    // unit = 2J' + rho, J' = grouped V block
+                const int gq = ln >> 2, c = ln & 3;
+                const int u = 16 * (unit >> 1) + 8 * (unit & 1) + gq;      // grouped V coordinate
+                const int bw = M.vbw[unit >> 1];
+                uint32_t *wbase = tbuf + ((M.vboff[unit >> 1] + (unit & 1) * 128 * bw) >> 2) + ln;
+                for (int i = 0; i < 8; ++i) {
+                    unsigned f[4];
+#pragma unroll
+                    for (int sl = 0; sl < 4; ++sl)                    // slot 4i + 2o + e: token 16i + 8o + 2c + e
+                        f[sl] = idxs[(16 * i + 8 * (sl >> 1) + 2 * c + (sl & 1)) * 256 + 128 + u];
+                    pack4(wbase, 32, bw, i, f, 15u);
+                }
+            }
+        }
+        for (int w = tid; w < kTile * ns; w += kTileThreads) {   // fp16 norms: token t at entry (t&7)*16 + (t>>4)*2 + ((t>>3)&1)
+            const int t128 = w / ns, g = w % ns;
+            const int slot = (t128 & 7) * 16 + (t128 >> 4) * 2 + ((t128 >> 3) & 1);
+            const int off = g < ng ? M.knorm_off + 256 * g : M.vnorm_off + 256 * (g - ng);
+            reinterpret_cast<uint16_t *>(reinterpret_cast<uint8_t *>(tbuf) + off)[slot] = nrm[t128 * ns + g];
+        }
+    }
+    __syncthreads();
+    {
+        uint4 *dst = reinterpret_cast<uint4 *>(gtile);
+        const uint4 *src = reinterpret_cast<const uint4 *>(tbuf);
+        for (int i = tid; i < stride / 16; i += kTileThreads) dst[i] = src[i];
+    }
+}
+
+
 __global__ void advance_seq_len_kernel(int32_t *seq_len, int batch, int n_new, int64_t max_tokens)
 {
     int s = blockIdx.x * blockDim.x + threadIdx.x;
@@ -742,6 +1054,10 @@ int launch_quantize_append(const bgtq_layout *lay, int layer, int n_layers, void
                       (n_cta <= 3 * (int64_t)lay->sm_count || n_cta > 8 * (int64_t)lay->sm_count);
     const size_t smem = append_smem_bytes(lay->max_stride, lay->max_rows, lay->cb_exact != 0, fast);
     dim3 grid((n_new + kTile - 1) / kTile + 1, lay->n_kv_heads * n_layers, batch);
+    // whole tiles of new tokens go to quantize_tile_kernel (one pass per tile); the sub-batch kernel keeps the partly
+    // filled first / last tile of every sequence
+    const size_t tsmem = tile_smem_bytes(lay->max_stride, lay->max_rows, lay->cb_exact != 0);
+    const bool tiled = n_new >= kTile && !append_exact_only() && !pm && !rope && lay->format == 1 && tsmem <= 227 * 1024;
     const HeadMeta *metas = lay->d_meta + (size_t)layer * lay->n_kv_heads;
     if (first_use_on_device(1)) {   // once per device, outside any stream capture
         const int maxs = (int)append_smem_bytes(16 * kDh * 8 + 256 * 16 + 16 * kDh * 8, 16, true, true);
@@ -752,6 +1068,8 @@ int launch_quantize_append(const bgtq_layout *lay, int layer, int n_layers, void
         BGTQ_APPEND_ATTR(float, true, false);  BGTQ_APPEND_ATTR(__nv_bfloat16, true, false);
         BGTQ_APPEND_ATTR(float, false, true);  BGTQ_APPEND_ATTR(__nv_bfloat16, false, true);
 #undef BGTQ_APPEND_ATTR
+        CUDA_TRY(cudaFuncSetAttribute(quantize_tile_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        CUDA_TRY(cudaFuncSetAttribute(quantize_tile_kernel<__nv_bfloat16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
     }
     const int32_t *pt = pm ? pm->table : nullptr;
     const int pstride = pm ? pm->table_stride : 0;
@@ -764,8 +1082,20 @@ int launch_quantize_append(const bgtq_layout *lay, int layer, int n_layers, void
         const double *cb = lay->cb_exact ? lay->d_hcb64 + (size_t)layer * lay->n_kv_heads * 1024 : lay->d_cb64;
         kern<<<grid, kAppendThreads, smem, st>>>(metas, (uint8_t *)cache, kp, vp, cb, lay->d_rot_t, batch, n_new,
                                                  lay->n_kv_heads, seq_len, n_cap, max_tokens, pt, pstride, n_pages, rc, rs,
-                                                 lay->pairing, lay->cb_exact, lay->max_rows, lay->d_rot_hl);
+                                                 lay->pairing, lay->cb_exact, lay->max_rows, lay->d_rot_hl, tiled ? 1 : 0);
     };
+    if (tiled) {
+        const double *cb = lay->cb_exact ? lay->d_hcb64 + (size_t)layer * lay->n_kv_heads * 1024 : lay->d_cb64;
+        if (dt == BGTQ_F32)
+            quantize_tile_kernel<float><<<grid, kTileThreads, tsmem, st>>>(metas, (uint8_t *)cache, (const float *)k_new, (const float *)v_new, cb, batch, n_new,
+                                                                         lay->n_kv_heads, seq_len, n_cap, max_tokens, lay->cb_exact, lay->max_rows, lay->d_rot_hl);
+        else
+            quantize_tile_kernel<__nv_bfloat16><<<grid, kTileThreads, tsmem, st>>>(metas, (uint8_t *)cache, (const __nv_bfloat16 *)k_new, (const __nv_bfloat16 *)v_new, cb,
+                                                                                 batch, n_new, lay->n_kv_heads, seq_len, n_cap, max_tokens, lay->cb_exact,
+                                                                                 lay->max_rows, lay->d_rot_hl);
+        count_launch();
+        CUDA_TRY(cudaGetLastError());
+    }
 #define BGTQ_APPEND_LAUNCH(T, F) \
         launch(quantize_append_kernel<T, false, false, F>, quantize_append_kernel<T, true, false, F>, \
                quantize_append_kernel<T, false, true, F>, (const T *)k_new, (const T *)v_new)
