@@ -722,14 +722,59 @@ constexpr int kTileThreads = 512;
 constexpr int kTileWarps = kTileThreads / 32;
 constexpr int kXsLd = 260;                 // floats per token row of xs: 256 + 4, so the A-fragment reads (row g, column c) hit 32 banks
 constexpr int kTileQueue = 6144;           // recheck queue; when more codes than that sit inside a band every code is rechecked
+constexpr int kIdxLd = 260;                // bytes per token row of idxs: 256 + 4, so the packers' byte gathers (8 token rows per warp) hit 8 banks
 
+// All B words of one lane of a unit from its 32 codes (slot k -> f[k]); the bit positions are DESIGN.md section 4's table
+// (field_bit_pos), folded at compile time.
+template <int B>
+__device__ __forceinline__ void pack_unit(const unsigned (&f)[32], uint32_t (&w)[B])
+{
+#pragma unroll
+    for (int j = 0; j < B; ++j) w[j] = 0u;
+#pragma unroll
+    for (int k = 0; k < 32; ++k) {
+        const unsigned g = B == 4 ? (f[k] >= 8 ? f[k] - 8 : (8u | (7u - f[k]))) : f[k];   // width 4: sign-magnitude storage
+#pragma unroll
+        for (int bit = 0; bit < B; ++bit) {
+            int word, pos;
+            field_bit_pos(B, k, bit, word, pos);
+            w[word] |= ((g >> bit) & 1u) << pos;
+        }
+    }
+}
+template <int B>
+__device__ __forceinline__ void pack_store(const unsigned (&f)[32], uint32_t *wbase, int ws)
+{
+    uint32_t w[B];
+    pack_unit<B>(f, w);
+#pragma unroll
+    for (int j = 0; j < B; ++j) wbase[j * ws] = w[j];
+}
+__device__ __forceinline__ void pack_store_b(int b, const unsigned (&f)[32], uint32_t *wbase, int ws)
+{
+    switch (b) {
+    case 1: pack_store<1>(f, wbase, ws); break;
+    case 2: pack_store<2>(f, wbase, ws); break;
+    case 3: pack_store<3>(f, wbase, ws); break;
+    case 4: pack_store<4>(f, wbase, ws); break;
+    case 5: pack_store<5>(f, wbase, ws); break;
+    case 6: pack_store<6>(f, wbase, ws); break;
+    case 7: pack_store<7>(f, wbase, ws); break;
+    case 8: pack_store<8>(f, wbase, ws); break;
+    default: break;
+    }
+}
+
+// hi part of the TF32 split of a finite value: nearest 11-bit significand, ties away (what cvt.rna.tf32 returns for finite
+// inputs, without its NaN / infinity selects; the lo part a - hi is exact in fp32 either way)
+__device__ __forceinline__ uint32_t tf32_near(float a) { return (__float_as_uint(a) + 0x1000u) & 0xffffe000u; }
 __device__ __forceinline__ float to_f32(float v) { return v; }
 __device__ __forceinline__ float to_f32(__nv_bfloat16 v) { return __bfloat162float(v); }
 
 static size_t tile_smem_bytes(int max_stride, int max_rows, bool cb_exact)
 {
     return (size_t)kTile * kXsLd * 4 + (size_t)kTile * max_rows * 8 + 512 * 8 * (cb_exact ? 2 : 1) + 1024 * 4 +
-           (size_t)kTile * max_rows * 2 + 16 + (size_t)kTile * 256 + kMaxUnits * sizeof(UnitDesc) + kMaxFastItems * sizeof(FastItem) +
+           (size_t)kTile * max_rows * 2 + 16 + (size_t)kTile * max_rows * 4 + (size_t)kTile * kIdxLd + kMaxUnits * sizeof(UnitDesc) + kMaxFastItems * sizeof(FastItem) +
            16 + kMetaBytes + (size_t)kTileQueue * 2 + (size_t)max_stride + 64;
 }
 
@@ -743,6 +788,13 @@ quantize_tile_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__ c
     extern __shared__ __align__(16) unsigned char smem[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int h = blockIdx.y % Hkv, lrel = blockIdx.y / Hkv, s = blockIdx.z;
+#if BGTQ_APPEND_PHASES
+    long long tph[10]; int nph = 0;
+#define TPH() do { tph[nph++] = clock64(); } while (0)
+#else
+#define TPH() do { } while (0)
+#endif
+    TPH();
     const int64_t t0 = seq_len[s];
     const int64_t t_end = min(t0 + (int64_t)n_new, max_tokens);
     const int64_t tile = t0 / kTile + blockIdx.x;
@@ -754,8 +806,9 @@ quantize_tile_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__ c
     double *tau = sigma + kTile * max_rows;                               // [512] (+ [512] V thresholds with exact-density codebooks)
     float *tau32 = reinterpret_cast<float *>(tau + (cb_exact ? 1024 : 512));   // [2][512]
     uint16_t *nrm = reinterpret_cast<uint16_t *>(tau32 + 1024);           // [128][ns]
-    uint8_t *idxs = reinterpret_cast<uint8_t *>(nrm + kTile * max_rows + 8);   // [128][256]
-    UnitDesc *units = reinterpret_cast<UnitDesc *>(idxs + kTile * 256);   // [32]
+    float *sig32 = reinterpret_cast<float *>(nrm + kTile * max_rows + 8);   // [128][ns]: (float)sigma, the fast path's scale
+    uint8_t *idxs = reinterpret_cast<uint8_t *>(sig32 + kTile * max_rows);     // [128][kIdxLd]
+    UnitDesc *units = reinterpret_cast<UnitDesc *>(idxs + kTile * kIdxLd);   // [32]
     FastItem *items = reinterpret_cast<FastItem *>(units + kMaxUnits);    // [32]
     int *cnt = reinterpret_cast<int *>(items + kMaxFastItems);            // [0] queue entries, [1] K items, [2] V items, [3] K units
     HeadMeta *Msp = reinterpret_cast<HeadMeta *>(cnt + 4);
@@ -800,6 +853,7 @@ quantize_tile_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__ c
         cnt[2] = ni - cnt[1];
         cnt[0] = 0;
     }
+    TPH();
     // ---- 1. gather: thread (column c = tid & 255, token half tid >> 8); inputs are fp32 / bf16 values, exact in fp32
     {
         const int col = tid & 255, th = tid >> 8;
@@ -809,13 +863,20 @@ quantize_tile_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__ c
         const int64_t row0 = ((((int64_t)lrel * batch + s) * n_new + (tile_lo - t0)) * Hkv + h) * kDh + (int64_t)th * 64 * rstep;
         float *xcol = xs + (size_t)th * 64 * kXsLd + col;
         if (g_off >= 0) {
-#pragma unroll 8
-            for (int tt = 0; tt < 64; ++tt) xcol[tt * kXsLd] = to_f32(g_src[row0 + tt * rstep + g_off]);
+#pragma unroll 1
+            for (int t8 = 0; t8 < 64; t8 += 32) {                  // 32 independent loads in flight per thread
+                T tv[32];
+#pragma unroll
+                for (int tt = 0; tt < 32; ++tt) tv[tt] = g_src[row0 + (t8 + tt) * rstep + g_off];
+#pragma unroll
+                for (int tt = 0; tt < 32; ++tt) xcol[(t8 + tt) * kXsLd] = to_f32(tv[tt]);
+            }
         } else {
             for (int tt = 0; tt < 64; ++tt) xcol[tt * kXsLd] = 0.f;
         }
     }
     __syncthreads();
+    TPH();
     for (int i = tid; i < 1022; i += kTileThreads) tau32[i + (i >= 511 ? 1 : 0)] = (float)(i < 511 ? tau[i] : tauV[i - 511]);
     // ---- 2. radii (exact fp64 chains in oracle order).  The long V chains go first, one per thread of the low warps; the
     //      second round is dealt from the other end so that no thread gets two long chains.
@@ -830,19 +891,28 @@ quantize_tile_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__ c
             double ss = 0.0;
             for (int j = 0; j < m; ++j) { const double xv = (double)x[j]; ss = __fma_rn(xv, xv, ss); }
             const double r2 = __dsqrt_rn(ss);
-            sigma[tt * ns + g] = __ddiv_rn(r2, __dsqrt_rn((double)m));
+            const double sgd = __ddiv_rn(r2, __dsqrt_rn((double)m));
+            sigma[tt * ns + g] = sgd;
+            sig32[tt * ns + g] = (float)sgd;
             uint16_t hb = __half_as_ushort(__double2half(r2));
             if (r2 >= 65520.0) hb = 0x7BFF;
             nrm[tt * ns + g] = hb;
         }
     }
     __syncthreads();
+    TPH();
     // ---- 3. z ~ X Pi^T on the tensor cores and the threshold search.  Work unit = (item: 16 outputs of one rotation group,
     //      half: 4 m-tiles = 64 tokens); V units (m = 128, the long ones) are dealt first.
     {
         const int fg = lane >> 2, fc = lane & 3;
         const int nki = cnt[1], nvi = cnt[2], n_work = 2 * (nki + nvi);
+#if BGTQ_APPEND_PHASES
+        long long tmma = 0, tq = 0; int nun = 0;
+#endif
         for (int u = warp; u < n_work; u += kTileWarps) {
+#if BGTQ_APPEND_PHASES
+            const long long ts0 = clock64(); ++nun;
+#endif
             const int item = u < 2 * nvi ? nki + (u >> 1) : ((u - 2 * nvi) >> 1), half = u & 1;
             const FastItem it = items[item];
             const int m = it.m, nA = it.n0 + fg, nB = nA + 8;
@@ -860,7 +930,7 @@ quantize_tile_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__ c
                 for (int mt = 0; mt < 4; ++mt) {
                     const float *pm = px + mt * 16 * kXsLd + k0;
                     const float a0 = va ? pm[0] : 0.f, a1 = va ? pm[8 * kXsLd] : 0.f, a2 = vb ? pm[4] : 0.f, a3 = vb ? pm[8 * kXsLd + 4] : 0.f;
-                    const uint32_t ah[4] = {tf32_rna(a0), tf32_rna(a1), tf32_rna(a2), tf32_rna(a3)};
+                    const uint32_t ah[4] = {tf32_near(a0), tf32_near(a1), tf32_near(a2), tf32_near(a3)};
                     const uint32_t al[4] = {__float_as_uint(a0 - __uint_as_float(ah[0])), __float_as_uint(a1 - __uint_as_float(ah[1])),
                                             __float_as_uint(a2 - __uint_as_float(ah[2])), __float_as_uint(a3 - __uint_as_float(ah[3]))};
                     mma_tf32(acc[mt][0], al, __float_as_uint(ca0.x), __float_as_uint(ca1.x));   // small terms first
@@ -874,8 +944,8 @@ quantize_tile_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__ c
                 }
             };
             const int kfull = m & ~7;
-#pragma unroll 1
-            for (int k0 = 0; k0 < kfull; k0 += 8)
+#pragma unroll 4
+            for (int k0 = 0; k0 < kfull; k0 += 8)                  // (unrolled: the operand loads of four k-steps are in flight together)
                 kstep(__ldg(pA + k0), __ldg(pA + k0 + 4), __ldg(pB + k0), __ldg(pB + k0 + 4), k0, true, true);
             if (kfull < m) {                                   // ragged tail: k >= m contributes zero
                 const bool va = kfull + fc < m, vb = kfull + fc + 4 < m;
@@ -883,47 +953,56 @@ quantize_tile_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__ c
                 kstep(va ? __ldg(pA + kfull) : zero2, vb ? __ldg(pA + kfull + 4) : zero2,
                       va ? __ldg(pB + kfull) : zero2, vb ? __ldg(pB + kfull + 4) : zero2, kfull, va, vb);
             }
+#if BGTQ_APPEND_PHASES
+            const long long ts1 = clock64(); tmma += ts1 - ts0;
+#endif
             // codes from z where it is clear of the neighbouring thresholds; the rest go to the queue
             const float *tb = tau32 + (it.isv ? 512 : 0) + ((1 << it.b) - 1);
             const float gc = fast_guard(it.m);
-            const int L = 1 << it.b;
-#pragma unroll 1
-            for (int mt = 0; mt < 4; ++mt) {
-                float z8[8], sg8[8];
-                int a8[8];
-                bool ok[8];
+            // Bisection over the 2^b - 1 thresholds, the eight codes of a lane side by side.  Both neighbours of the final
+            // code are among the probed thresholds (the last probe that succeeded, the last that failed), so the smallest
+            // |z - tau sigma| over the probes is the distance to the nearest neighbour: one running minimum replaces the
+            // two extra look-ups of the sub-batch kernel (it can only flag more codes, never fewer).
 #pragma unroll
-                for (int e = 0; e < 8; ++e) {
-                    const int tt = half * 64 + mt * 16 + fg + 8 * ((e >> 1) & 1), nl = it.n0 + 8 * (e >> 2) + 2 * fc + (e & 1);
-                    ok[e] = nl < it.m;
-                    z8[e] = acc[mt][e >> 2][e & 3];
-                    sg8[e] = ok[e] ? (float)sigma[tt * ns + it.sidx] : 0.f;
-                    a8[e] = 0;
-                }
+            for (int mt = 0; mt < 4; ++mt) {
+                const int ttA = half * 64 + mt * 16 + fg;                         // token rows ttA and ttA + 8
+                const float sgA = sig32[ttA * ns + it.sidx], sgB = sig32[(ttA + 8) * ns + it.sidx];
+                uint8_t *ip = idxs + ttA * kIdxLd + it.x0 + it.n0 + 2 * fc;
+                float z8[8], d8[8];
+                int a8[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) { z8[e] = acc[mt][e >> 2][e & 3]; a8[e] = 0; d8[e] = 3.0e38f; }
                 for (int bit = it.b - 1; bit >= 0; --bit) {
                     const int step = 1 << bit;
 #pragma unroll
-                    for (int e = 0; e < 8; ++e)
-                        if (z8[e] > tb[a8[e] + step - 1] * sg8[e]) a8[e] += step;
+                    for (int e = 0; e < 8; ++e) {
+                        const float t = tb[a8[e] + step - 1] * (((e >> 1) & 1) ? sgB : sgA);
+                        d8[e] = fminf(d8[e], fabsf(z8[e] - t));
+                        if (z8[e] > t) a8[e] += step;
+                    }
                 }
 #pragma unroll
                 for (int e = 0; e < 8; ++e) {
-                    if (!ok[e]) continue;
-                    const int tt = half * 64 + mt * 16 + fg + 8 * ((e >> 1) & 1), col = it.x0 + it.n0 + 8 * (e >> 2) + 2 * fc + (e & 1);
-                    const int a = a8[e];
-                    const float z = z8[e], sg = sg8[e], gd = gc * sg;
-                    const float tlo = tb[a > 0 ? a - 1 : 0] * sg, thi = tb[a < L - 1 ? a : 0] * sg;
-                    const bool risky = (a > 0 && !(z - tlo > gd)) || (a < L - 1 && !(thi - z > gd));
-                    idxs[tt * 256 + col] = (uint8_t)a;
-                    if (risky) {
+                    const int nl = it.n0 + 8 * (e >> 2) + 2 * fc + (e & 1);
+                    if (nl >= it.m) continue;
+                    ip[((e >> 1) & 1) * 8 * kIdxLd + 8 * (e >> 2) + (e & 1)] = (uint8_t)a8[e];
+                    if (!(d8[e] > gc * (((e >> 1) & 1) ? sgB : sgA))) {
                         const int pos = atomicAdd(&cnt[0], 1);
-                        if (pos < kTileQueue) queue[pos] = (uint16_t)((tt << 8) | col);
+                        if (pos < kTileQueue) queue[pos] = (uint16_t)(((ttA + 8 * ((e >> 1) & 1)) << 8) | (it.x0 + nl));
                     }
                 }
             }
+#if BGTQ_APPEND_PHASES
+            tq += clock64() - ts1;
+#endif
         }
+#if BGTQ_APPEND_PHASES
+        if ((tid == 0 || tid == 300) && blockIdx.x == 3 && blockIdx.y == 0 && blockIdx.z == 0)
+            printf("tile phase 3 (tid %d): units %d mma %lld quant %lld\n", tid, nun, tmma, tq);
+#endif
     }
     __syncthreads();
+    TPH();
     // ---- 4. the exact fp64 chain (oracle order) for the queued (token, column) pairs
     {
         auto exact_code = [&](int tt, int col) {
@@ -960,7 +1039,7 @@ quantize_tile_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__ c
             int a = 0;
             for (int bit = b - 1; bit >= 0; --bit)
                 if (zz > __dmul_rn(tb[a + (1 << bit) - 1], sg)) a += 1 << bit;
-            idxs[tt * 256 + col] = (uint8_t)a;
+            idxs[tt * kIdxLd + col] = (uint8_t)a;
         };
         const int qn = cnt[0];
         if (qn <= kTileQueue) {
@@ -973,6 +1052,7 @@ quantize_tile_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__ c
         }
     }
     __syncthreads();
+    TPH();
     // ---- 5. pack: one owner per (unit, lane); its eight four-slot groups (one per m-tile) in turn
     {
         const int kitems = cnt[3] * 32;
@@ -983,26 +1063,22 @@ quantize_tile_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__ c
                 if (lp >= lanes) continue;
                 const int g8 = U.nc == 4 ? lp >> 2 : (U.nc == 2 ? lp >> 1 : (U.nc == 1 ? lp : (lp * 11) >> 5)), c = lp - g8 * U.nc;
                 uint32_t *wbase = tbuf + (U.off >> 2) + lp;
-                for (int i = 0; i < 8; ++i) {
-                    unsigned f[4];
+                unsigned f[32];
 #pragma unroll
-                    for (int sl = 0; sl < 4; ++sl)                    // slot 4i + 2p + q: token 16i + 8p + g8, coordinate 2c + q
-                        f[sl] = idxs[(16 * i + 8 * (sl >> 1) + g8) * 256 + U.ustart + 2 * c + (sl & 1)];
-                    pack4(wbase, lanes, U.b, i, f, 15u);
-                }
+                for (int k = 0; k < 32; ++k)                         // slot 4i + 2p + q: token 16i + 8p + g8, coordinate 2c + q
+                    f[k] = idxs[(16 * (k >> 2) + 8 * ((k >> 1) & 1) + g8) * kIdxLd + U.ustart + 2 * c + (k & 1)];
+                pack_store_b(U.b, f, wbase, lanes);
             } else {
                 const int v = itx - kitems, unit = v >> 5, ln = v & 31;    // unit = 2J' + rho, J' = grouped V block
                 const int gq = ln >> 2, c = ln & 3;
                 const int u = 16 * (unit >> 1) + 8 * (unit & 1) + gq;      // grouped V coordinate
                 const int bw = M.vbw[unit >> 1];
                 uint32_t *wbase = tbuf + ((M.vboff[unit >> 1] + (unit & 1) * 128 * bw) >> 2) + ln;
-                for (int i = 0; i < 8; ++i) {
-                    unsigned f[4];
+                unsigned f[32];
 #pragma unroll
-                    for (int sl = 0; sl < 4; ++sl)                    // slot 4i + 2o + e: token 16i + 8o + 2c + e
-                        f[sl] = idxs[(16 * i + 8 * (sl >> 1) + 2 * c + (sl & 1)) * 256 + 128 + u];
-                    pack4(wbase, 32, bw, i, f, 15u);
-                }
+                for (int k = 0; k < 32; ++k)                         // slot 4i + 2o + e: token 16i + 8o + 2c + e
+                    f[k] = idxs[(16 * (k >> 2) + 8 * ((k >> 1) & 1) + 2 * c + (k & 1)) * kIdxLd + 128 + u];
+                pack_store_b(bw, f, wbase, 32);
             }
         }
         for (int w = tid; w < kTile * ns; w += kTileThreads) {   // fp16 norms: token t at entry (t&7)*16 + (t>>4)*2 + ((t>>3)&1)
@@ -1013,11 +1089,19 @@ quantize_tile_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__ c
         }
     }
     __syncthreads();
+    TPH();
     {
         uint4 *dst = reinterpret_cast<uint4 *>(gtile);
         const uint4 *src = reinterpret_cast<const uint4 *>(tbuf);
         for (int i = tid; i < stride / 16; i += kTileThreads) dst[i] = src[i];
     }
+    TPH();
+#if BGTQ_APPEND_PHASES
+    if ((tid == 0 || tid == 300) && blockIdx.x == 3 && blockIdx.y == 0 && blockIdx.z == 0)
+        printf("tile phases (tid %d): setup %lld gather %lld radii %lld mma+quant %lld recheck(%d) %lld pack %lld writeback %lld\n", tid,
+               tph[1] - tph[0], tph[2] - tph[1], tph[3] - tph[2], tph[4] - tph[3], cnt[0], tph[5] - tph[4], tph[6] - tph[5], tph[7] - tph[6]);
+#endif
+#undef TPH
 }
 
 
