@@ -952,3 +952,48 @@ def test_append_fast_path_writes_the_exact_kernels_bytes(P, tab128, kv_dtype, n_
         exp = np.zeros(8 * stride, dtype=np.uint8)
         O.pack_region(qh, p.d_h, exp)
         assert np.array_equal(caches[0][off:off + 8 * stride], exp), h
+
+
+@pytest.mark.parametrize("kv_dtype,n_old,n_new", [("bf16", 0, 300), ("f32", 50, 700), ("bf16", 128, 256)])
+def test_append_whole_tile_path_matches_the_exact_kernel_and_the_oracle(P, tab128, kv_dtype, n_old, n_new):
+    """Bulk appends send every tile whose 128 tokens are all new to quantize_tile_kernel (one pass per tile) and leave
+    the partly filled first / last tile to the sub-batch kernel: an unaligned start (n_old tokens already cached), a
+    ragged end and two sequences of different lengths in one call must give the exact kernel's bytes and the oracle's."""
+    T = n_old + n_new
+    p = H.make_problem(91, T + 64, 8, 2, 3, 3, 1, 8, kv_dtype=kv_dtype)
+    lay = P.Layout(p.bits[None], p.Hq, p.d_h, p.b_v, p.rot)
+    tdt = torch.float32 if kv_dtype == "f32" else torch.bfloat16
+    cap = 1152
+    starts = [n_old, n_old + 64]                                       # the second sequence starts 64 tokens later
+    caches = []
+    try:
+        for exact_only in (False, True):
+            P.append_exact_only(exact_only)
+            cache = lay.new_cache(2, cap)
+            seq = torch.zeros(2, dtype=torch.int32, device="cuda")
+            if n_old:                                                  # older tokens of both sequences
+                k0, v0 = np.stack([p.k_post[:n_old]] * 2), np.stack([p.v[:n_old]] * 2)
+                P.quantize_append(lay, 0, cache, _cuda(k0, tdt), _cuda(v0, tdt), seq, cap)
+            # sequence 1 gets 64 more old tokens through a second call that appends nothing to sequence 0: emulate by
+            # appending them to both and rewinding sequence 0
+            k64 = np.stack([p.k_post[n_old:n_old + 64]] * 2)
+            v64 = np.stack([p.v[n_old:n_old + 64]] * 2)
+            P.quantize_append(lay, 0, cache, _cuda(k64, tdt), _cuda(v64, tdt), seq, cap)
+            seq[0] = n_old
+            knew = np.stack([p.k_post[starts[b]:starts[b] + n_new] for b in range(2)])
+            vnew = np.stack([p.v[starts[b]:starts[b] + n_new] for b in range(2)])
+            P.quantize_append(lay, 0, cache, _cuda(knew, tdt), _cuda(vnew, tdt), seq, cap)
+            assert seq.cpu().tolist() == [starts[0] + n_new, starts[1] + n_new]
+            caches.append(cache.cpu().numpy())
+    finally:
+        P.append_exact_only(False)
+    assert np.array_equal(caches[0], caches[1])
+    n_cap = cap // 128
+    for b in range(2):
+        Tb = starts[b] + n_new
+        for h in range(2):
+            qh = O.quantize_head(p.k_post[:Tb, h], p.v[:Tb, h], p.bits[h], p.b_v, tab128)
+            stride, off = lay.tile_stride(0, h), lay.region_offset(0, b, h, 2, cap)
+            exp = np.zeros(n_cap * stride, dtype=np.uint8)
+            O.pack_region(qh, p.d_h, exp)
+            assert np.array_equal(caches[0][off:off + n_cap * stride], exp), (b, h)
