@@ -643,8 +643,10 @@ def run_ours(args):
             append_bulk = {"tokens_per_seq": n_app, "ms": ms_app, "codes_per_s": vecs * 2 * shp_.d_h / (ms_app * 1e-3),
                            "input_GBs": vecs * 2 * shp_.d_h * 4 / (ms_app * 1e-3) / 1e9,
                            "exact_kernel_ms": ms_exact, "exact_kernel_codes_per_s": vecs * 2 * shp_.d_h / (ms_exact * 1e-3),
-                           "note": "K and V of 8192 tokens per sequence, fp32 in, layer 0; default = TF32 tensor-core rotation with "
-                                   "exact fp64 recheck inside the guard band (bit-identical to the exact fp64 kernel, timed beside it)"}
+                           "note": "K and V of 8192 tokens per sequence, fp32 in, layer 0; default = whole tiles of new tokens in "
+                                   "quantize_tile_kernel (one pass per 128-token tile: TF32 tensor-core rotation, exact fp64 radii, exact "
+                                   "fp64 recheck inside the guard band), partly filled tiles in the 16-token sub-batch kernel; bit-identical "
+                                   "to the exact fp64 kernel, timed beside it"}
             del ac, kk, vv
 
         # ---- end to end through the C-ABI with HOST buffers (pinned), copies inside the timed region

@@ -925,22 +925,34 @@ quantize_tile_kernel(const HeadMeta *__restrict__ metas, uint8_t *__restrict__ c
             for (int mt = 0; mt < 4; ++mt)
 #pragma unroll
                 for (int e = 0; e < 4; ++e) acc[mt][0][e] = acc[mt][1][e] = 0.f;
+            // (the three products of an accumulator are issued eight MMAs apart -- term by term over the four m-tiles and two
+            //  n-tiles -- so that no MMA waits for the one issued just before it)
             auto kstep = [&](const float2 ca0, const float2 ca1, const float2 cb0, const float2 cb1, int k0, bool va, bool vb) {
+                uint32_t ah[4][4], al[4][4];
 #pragma unroll
                 for (int mt = 0; mt < 4; ++mt) {
                     const float *pm = px + mt * 16 * kXsLd + k0;
-                    const float a0 = va ? pm[0] : 0.f, a1 = va ? pm[8 * kXsLd] : 0.f, a2 = vb ? pm[4] : 0.f, a3 = vb ? pm[8 * kXsLd + 4] : 0.f;
-                    const uint32_t ah[4] = {tf32_near(a0), tf32_near(a1), tf32_near(a2), tf32_near(a3)};
-                    const uint32_t al[4] = {__float_as_uint(a0 - __uint_as_float(ah[0])), __float_as_uint(a1 - __uint_as_float(ah[1])),
-                                            __float_as_uint(a2 - __uint_as_float(ah[2])), __float_as_uint(a3 - __uint_as_float(ah[3]))};
-                    mma_tf32(acc[mt][0], al, __float_as_uint(ca0.x), __float_as_uint(ca1.x));   // small terms first
-                    mma_tf32(acc[mt][0], ah, __float_as_uint(ca0.y), __float_as_uint(ca1.y));
-                    mma_tf32(acc[mt][0], ah, __float_as_uint(ca0.x), __float_as_uint(ca1.x));
-                    if (two) {
-                        mma_tf32(acc[mt][1], al, __float_as_uint(cb0.x), __float_as_uint(cb1.x));
-                        mma_tf32(acc[mt][1], ah, __float_as_uint(cb0.y), __float_as_uint(cb1.y));
-                        mma_tf32(acc[mt][1], ah, __float_as_uint(cb0.x), __float_as_uint(cb1.x));
+                    const float a[4] = {va ? pm[0] : 0.f, va ? pm[8 * kXsLd] : 0.f, vb ? pm[4] : 0.f, vb ? pm[8 * kXsLd + 4] : 0.f};
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        ah[mt][e] = tf32_near(a[e]);
+                        al[mt][e] = __float_as_uint(a[e] - __uint_as_float(ah[mt][e]));
                     }
+                }
+#pragma unroll
+                for (int mt = 0; mt < 4; ++mt) {                                   // small terms first
+                    mma_tf32(acc[mt][0], al[mt], __float_as_uint(ca0.x), __float_as_uint(ca1.x));
+                    if (two) mma_tf32(acc[mt][1], al[mt], __float_as_uint(cb0.x), __float_as_uint(cb1.x));
+                }
+#pragma unroll
+                for (int mt = 0; mt < 4; ++mt) {
+                    mma_tf32(acc[mt][0], ah[mt], __float_as_uint(ca0.y), __float_as_uint(ca1.y));
+                    if (two) mma_tf32(acc[mt][1], ah[mt], __float_as_uint(cb0.y), __float_as_uint(cb1.y));
+                }
+#pragma unroll
+                for (int mt = 0; mt < 4; ++mt) {
+                    mma_tf32(acc[mt][0], ah[mt], __float_as_uint(ca0.x), __float_as_uint(ca1.x));
+                    if (two) mma_tf32(acc[mt][1], ah[mt], __float_as_uint(cb0.x), __float_as_uint(cb1.x));
                 }
             };
             const int kfull = m & ~7;
