@@ -316,7 +316,7 @@ int bgtq_profile_decode_read(double *ms_sum, int *count);
  * instructions share, what a 3-bit unit costs to unpack, how fast one thread issues tcgen05.mma); `warps` = warps per SM
  * (4..16) for the pipe and unpack tests.  which in [0, BGTQ_MICROBENCH_COUNT); bgtq_debug_microbench_name gives the
  * quantity and its unit.  Synchronous, about 10 ms each; not part of the method. */
-#define BGTQ_MICROBENCH_COUNT 21
+#define BGTQ_MICROBENCH_COUNT 22
 const char *bgtq_debug_microbench_name(int which);
 int bgtq_debug_microbench(int which, int warps, double *value);
 /* number of kernels launched by this library since load (bench.py's gpu_launches). */

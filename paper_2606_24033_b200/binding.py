@@ -37,7 +37,7 @@ SYMBOLS = [
     "bgtq_v_block_energy_workspace_bytes", "bgtq_v_block_energy", "bgtq_layout_create_kv",
     "bgtq_block_energy_static", "bgtq_block_energy_static_max_row_elems", "bgtq_debug_append_exact_only",
 ]
-MICROBENCH_COUNT = 21
+MICROBENCH_COUNT = 22
 FORMAT_V1, FORMAT_V2 = 1, 2
 CODEBOOK_EXACT = 0x100
 

@@ -86,8 +86,13 @@ __device__ __forceinline__ void mb_hmma(float (&c)[4], uint32_t a0, uint32_t a1,
     asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
                  : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3]) : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
 }
+__device__ __forceinline__ void mb_tf32(float (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0, uint32_t b1)
+{
+    asm volatile("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                 : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3]) : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
 // MODE 0: two units -> fp16 fragments + 8 HMMA (the round-1 PV loop body); 1: fp16 decode only; 2: e4m3 planes decode only;
-// 3: 8 HMMA only (issue rate of the legacy tensor path)
+// 3: 8 HMMA only (issue rate of the legacy tensor path); 4: 8 TF32 m16n8k8 MMAs only (the append fast path's rotation)
 template <int MODE>
 __global__ void __launch_bounds__(512) mb_unpack_kernel(int iters, int units, uint32_t *out, long long *cyc, const uint32_t *src)
 {
@@ -131,6 +136,9 @@ __global__ void __launch_bounds__(512) mb_unpack_kernel(int iters, int units, ui
                 mb_dec3_f8(w1, pools, hi, lo);
 #pragma unroll
                 for (int i = 0; i < 8; ++i) fold ^= hi[i] ^ lo[i];
+            } else if (MODE == 4) {
+#pragma unroll
+                for (int i = 0; i < 8; ++i) mb_tf32(C[i], w0[0], w0[1], w0[2], w1[0], b0, b1);
             } else {
 #pragma unroll
                 for (int i = 0; i < 8; ++i) mb_hmma(C[i], w0[0], w0[1], w0[2], w1[0], b0, b1);
@@ -202,6 +210,7 @@ static const char *const kMbNames[BGTQ_MICROBENCH_COUNT] = {
     "tcgen05.mma M128 N8 K32 (A in TMEM), 1 issuing thread: clocks per MMA",
     "tcgen05.mma, 2 issuing threads: clocks per MMA overall",
     "tcgen05.mma, 4 issuing threads: clocks per MMA overall",
+    "HMMA.1688.TF32 (mma.sync m16n8k8 tf32): clocks per instruction per scheduler",
 };
 
 const char *microbench_name(int which) { return which >= 0 && which < BGTQ_MICROBENCH_COUNT ? kMbNames[which] : nullptr; }
@@ -276,6 +285,7 @@ int microbench_run(int which, int warps, double *value)
     case 18: umma(mb_umma_kernel<1>, 1); break;
     case 19: umma(mb_umma_kernel<2>, 2); break;
     case 20: umma(mb_umma_kernel<4>, 4); break;
+    case 21: unpack(mb_unpack_kernel<4>, 1); *value = *value * 2.0 * 4.0 / 8.0; break;
     default: rc = BGTQ_EINVAL; set_error("bgtq_debug_microbench: unknown benchmark"); break;
     }
     cudaFree(out);
