@@ -174,6 +174,10 @@ int64_t bgtq_tile_stride(const bgtq_layout *layout, int layer, int kv_head);
  * sequence directly; a bulk append evaluates the rotation on the tensor cores (TF32, hi/lo split) and
  * recomputes with the exact fp64 chain every code whose rotated value lies within a guard band of a
  * quantisation threshold -- the same bytes, checked against the exact kernel (bgtq_debug_append_exact_only).
+ * Within a bulk append every tile whose 128 tokens are all new is quantised in one pass by one CTA
+ * (quantize_tile_kernel; contiguous BGTQ-v1 caches, post-RoPE keys); the partly filled first / last tile of a
+ * sequence, paged caches, fused RoPE and BGTQ-v2 take the 16-token sub-batch kernel.  One call may therefore launch two
+ * kernels on `stream`; they touch disjoint tiles.
  * k_new, v_new [device] [batch, n_new, n_kv_heads, d_h] of dtype dt (post-RoPE K).
  * seq_len [device] int32 [batch]: tokens already cached; sequence s receives its n_new tokens at
  *   positions seq_len[s] .. seq_len[s]+n_new-1 and, if advance_seq_len != 0, seq_len[s] is advanced
@@ -302,9 +306,10 @@ int bgtq_fp16_decode_attention(int n_layers, int batch, int n_q_heads, int n_kv_
 /* decode one unit (b words per lane, 32 lanes, plane-major as in a tile) with the kernel's own
  * unpack routine: words [host] uint32 [b*32] -> values [host] float [32 lanes][32 slots]. */
 int bgtq_debug_decode_unit(int b, const uint32_t *words, float *values);
-/* bgtq_quantize_append* with >= 16 new tokens per sequence runs the tensor-core fast path (TF32 hi/lo products, codes inside
- * a guard band of a threshold recomputed with the exact fp64 chain: same bytes as the exact kernel).  on != 0 forces the
- * exact fp64 kernel for every call of the process (tests compare the two; bench.py times both).  Returns the old setting. */
+/* bgtq_quantize_append* with >= 16 new tokens per sequence runs the tensor-core fast paths (TF32 hi/lo products, codes inside
+ * a guard band of a threshold recomputed with the exact fp64 chain: same bytes as the exact kernel; whole tiles of new
+ * tokens in quantize_tile_kernel, the rest in the sub-batch kernel).  on != 0 forces the exact fp64 sub-batch kernel for
+ * every tile of every call of the process (tests compare the two; bench.py times both).  Returns the old setting. */
 int bgtq_debug_append_exact_only(int on);
 /* measurement hook for bench.py's roofline: while enabled, every decode call records a CUDA event
  * pair on its stream around the split-KV decode kernel alone (not the q-fold / combine kernels);
