@@ -1675,8 +1675,10 @@ __device__ __forceinline__ void prefill_decode_k(const uint32_t *raw, const PUni
 #pragma unroll
                 for (int p = 0; p < 2; ++p) {
                     const int tok = 16 * i + 8 * p + g8;
-                    const uint32_t n2 = prmt(nw[i], nw[i], p ? 0x3232 : 0x1010);
-                    *reinterpret_cast<uint32_t *>(khat + tile_off<UMMA>(tok, col)) = hmul2_u(h[2 * i + p], n2);
+                    // (h, h) * (n, n): the half of the norm pair is broadcast by the multiply's operand select, not by a PRMT
+                    const __half2 nn = *reinterpret_cast<const __half2 *>(&nw[i]);
+                    const __half2 pr = __hmul2(*reinterpret_cast<const __half2 *>(&h[2 * i + p]), p ? __high2half2(nn) : __low2half2(nn));
+                    *reinterpret_cast<uint32_t *>(khat + tile_off<UMMA>(tok, col)) = *reinterpret_cast<const uint32_t *>(&pr);
                 }
         } else {
 #pragma unroll
