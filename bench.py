@@ -288,8 +288,9 @@ def build_workload(args, P, torch, device, seed_shift: int = 0):
             ews = P.block_energy_workspace(Hq, Hkv, d, device)    # caller-owned scratch, reused by every layer
             P.block_energy(qcal, k, workspace=ews)                # warm-up (module load, caches)
         e0, e1 = ev(), ev()
-        e0.record()
-        scores.append(P.block_energy(qcal, k, workspace=ews))
+        torch.cuda._sleep(400_000)                            # ~0.2 ms of GPU idling queued first: the host enqueues e0, the
+        e0.record()                                           # (cooperative) launch and e1 meanwhile, so the event pair times the
+        scores.append(P.block_energy(qcal, k, workspace=ews))  # kernel and not the host's launch latency
         e1.record()
         torch.cuda.synchronize()
         t_energy += e0.elapsed_time(e1)
