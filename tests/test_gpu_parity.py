@@ -997,3 +997,28 @@ def test_append_whole_tile_path_matches_the_exact_kernel_and_the_oracle(P, tab12
             exp = np.zeros(n_cap * stride, dtype=np.uint8)
             O.pack_region(qh, p.d_h, exp)
             assert np.array_equal(caches[0][off:off + n_cap * stride], exp), (b, h)
+
+
+@pytest.mark.parametrize("counts", [[1, 3, 5, 7, 9, 11, 13, 15], [2, 4, 6, 8, 10, 12, 14, 8], [17, 1, 1, 1, 1, 1, 1, 41]])
+def test_attention_every_unit_count_and_partial_lane_pattern(P, tab128, counts):
+    """decode_kernel takes a group's 8-coordinate units in pairs (m16n8k16), an odd last unit alone (m16n8k8), and loads a
+    trailing partial unit without predicates (its idle lanes decode words they do not own and meet the zero rows of q').
+    Group sizes m = 2 * counts[w - 1] for width w cover: a single partial unit, odd and even unit counts, 1, 2 and 3 data
+    lanes in the last unit, and a partial unit as the second of a pair -- on tiles that end ragged."""
+    assert sum(counts) == 64
+    Hq, Hkv, T = 8, 2, 517
+    p = H.make_problem(123, T, Hq, Hkv, 3, 3, 1, 8, rope_base=1e4)
+    order = np.random.default_rng(7).permutation(64)
+    for h in range(Hkv):
+        bits = np.concatenate([np.full(c, w + 1) for w, c in enumerate(counts if h == 0 else counts[::-1])])
+        p.bits[h] = bits[order]                                       # widths scattered over the RoPE blocks
+    max_tokens = 640
+    lay, cache, seq, heads = _append_and_compare(P, p, tab128, [T], max_tokens, "f32")
+    scale = 1.0 / math.sqrt(p.d_h)
+    out = P.decode_attention(lay, 0, cache, _cuda(p.q_post[None], torch.bfloat16), seq, max_tokens, scale, lay.new_workspace(1))
+    torch.cuda.synchronize()
+    exp, rv = H.oracle_attention(p, heads, tab128, scale)
+    got = out[0].double().cpu().numpy()
+    G = Hq // Hkv
+    err = max(H.record_error("unit-count / partial-lane patterns", got[a], exp[a], rv[a // G], T=T, b_k=3, b_v=3) for a in range(Hq))
+    assert err <= 2e-3, err
