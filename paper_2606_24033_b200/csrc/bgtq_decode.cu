@@ -181,7 +181,7 @@ template <int PARTS>
 __global__ void __launch_bounds__(PARTS * kDh)
 qfold_kernel(const HeadMeta *__restrict__ metas, const float *__restrict__ rot_t,
              const __nv_bfloat16 *__restrict__ q, int batch, int Hkv, int Hq, float scale_log2e,
-             __half *__restrict__ qf, int plain)
+             __half *__restrict__ qf, int plain, int early_wait = 0)
 {
     pdl_trigger();
     const int G = Hq / Hkv;
@@ -203,14 +203,7 @@ qfold_kernel(const HeadMeta *__restrict__ metas, const float *__restrict__ rot_t
     if (tid == 0)
         for (int ks = 0; ks < M.n_ksteps; ++ks)
             if (M.ksteps[ks].flags & 1) ksbase[M.ksteps[ks].flags >> 4] = ks;
-    // zero padding: this head's slots (and, from block n = 0, the unused head slots n >= G)
-    uint2 *out2 = reinterpret_cast<uint2 *>(qf + (size_t)pair * kQfHalves);     // [kstep][8][4] of 4 halves
-    if (!plain)
-        for (int e = tid; e < kMaxKSteps * 32; e += kQfoldThreads) {
-            const int nn = (e >> 2) & 7;
-            if (nn == n || (n == 0 && nn >= G)) out2[e] = make_uint2(0u, 0u);
-        }
-    __syncthreads();
+    __syncthreads();                                        // ksbase[]
     // plain layout (prefill): q'[pair][head slot n][128] in grouped coordinate order, zero beyond kdim
     if (plain && tid < kDh && tid >= M.kdim) qf[((size_t)pair * 8 + n) * kDh + tid] = __float2half(0.f);
     const int ro = tid / PARTS, part = tid % PARTS;         // output (grouped coordinate) and the part of its dot product
@@ -247,6 +240,18 @@ qfold_kernel(const HeadMeta *__restrict__ metas, const float *__restrict__ rot_t
     }
 #pragma unroll
     for (int sft = 1; sft < PARTS; sft <<= 1) acc += __shfl_xor_sync(0xffffffffu, acc, sft);   // the parts of an output are adjacent lanes; fixed order
+    // Launched programmatically behind the previous decode call's combine_kernel (per-layer chains), this block has come
+    // this far -- metadata, the query row (a caller input, complete before the call), the dot products -- beside it; the
+    // q' workspace may still be read by that call's decode_kernel until its combine_kernel has completed.
+    if (early_wait) pdl_wait();
+    // zero padding: this head's slots (and, from block n = 0, the unused head slots n >= G)
+    uint2 *out2 = reinterpret_cast<uint2 *>(qf + (size_t)pair * kQfHalves);     // [kstep][8][4] of 4 halves
+    if (!plain)
+        for (int e = tid; e < kMaxKSteps * 32; e += kQfoldThreads) {
+            const int nn = (e >> 2) & 7;
+            if (nn == n || (n == 0 && nn >= G)) out2[e] = make_uint2(0u, 0u);
+        }
+    __syncthreads();
     if (act && part == 0) {
         __half *out = qf + (size_t)pair * kQfHalves;
         if (plain) qf[((size_t)pair * 8 + n) * kDh + ro] = __float2half_rn(acc * sc);
@@ -255,7 +260,7 @@ qfold_kernel(const HeadMeta *__restrict__ metas, const float *__restrict__ rot_t
     // Protected regime: this kernel is launched programmatically behind window_kernel and runs beside it; it must not
     // COMPLETE before window_kernel has, because the kernels after it only wait for their immediate predecessor.
     // (A no-op when the launch carries no programmatic dependency.)
-    pdl_wait();
+    if (!early_wait) pdl_wait();
 }
 
 // ---------------------------------------------------------------- the decode kernel
@@ -857,6 +862,7 @@ combine_kernel(const float *__restrict__ partials, const int32_t *__restrict__ s
     __shared__ float wgt[kMaxSlots], lrec[kMaxSlots];
     __shared__ float red[NW][kDh + 4];
     __shared__ float wred[2][NW];
+    pdl_trigger();                                      // the next decode call's qfold_kernel may run its prologue beside this kernel
     const int pair = blockIdx.x / G, n = blockIdx.x % G;
     const int h = pair % Hkv, lb = pair / Hkv, b = lb % batch, l = lb / batch;
     const int t = threadIdx.x, lane = t & 31, wq = t >> 5;
@@ -894,6 +900,13 @@ combine_kernel(const float *__restrict__ partials, const int32_t *__restrict__ s
     const int n_int = c1 - c0 - 1 > 0 ? c1 - c0 - 1 : 0;
     const int n_pk = tiles_b > 0 ? min(kMaxSlots - 1, 16 + n_int + (c1 > c0 ? 16 : 0)) : 0;   // records of the packed range
     const int n_ent = n_pk + (has_win ? 1 : 0);
+    // de-rotation operands of this thread (a static table): requested ahead of the wait, consumed after the merge
+    constexpr int kRotPre = PARTS == 4 ? kDh / PARTS : 1;
+    float rpre[kRotPre];
+    if (PARTS == 4 && rot128 != nullptr && metas == nullptr) {
+#pragma unroll
+        for (int j = 0; j < kRotPre; ++j) rpre[j] = __ldg(rot128 + (part * kRotPre + j) * kDh + d);
+    }
     pdl_wait();                                         // the decode kernel's partials are complete from here on
     // pass 1: every record's running max and sum (one round trip: the two loads are independent) -> M
     float mloc = -INFINITY;
@@ -963,8 +976,13 @@ combine_kernel(const float *__restrict__ partials, const int32_t *__restrict__ s
         inv = rsqrtf((float)m);
         od = 16 * M.vblk[d >> 4] + (d & 15);
     } else {
+        if (PARTS == 4) {
+#pragma unroll
+            for (int j = 0; j < kRotPre; ++j) r = fmaf(rpre[j], o[part * kRotPre + j], r);
+        } else {
 #pragma unroll 32
-        for (int j = part * (kDh / PARTS); j < (part + 1) * (kDh / PARTS); ++j) r = fmaf(__ldg(rot128 + j * kDh + d), o[j], r);
+            for (int j = part * (kDh / PARTS); j < (part + 1) * (kDh / PARTS); ++j) r = fmaf(__ldg(rot128 + j * kDh + d), o[j], r);
+        }
     }
     if (PARTS == 1) { dst[od] = __float2bfloat16(r * inv); return; }
     red[part][d] = r;
@@ -1493,7 +1511,11 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
                                    lay->v_grouped ? metas : nullptr, lay->d_rot_t)) return rc;
     }
     const bool wideq = pairs * G <= kLatencyShapedBlocks;       // few blocks: the latency-shaped 512-thread variant
-    if (win && !g_prof) {
+    if (!g_prof) {
+        // programmatic launch: behind window_kernel (protected regime; the two run side by side, the wait sits at the end of
+        // qfold_kernel) or behind whatever precedes the call on the stream -- in a layer-by-layer decode that is the previous
+        // layer's combine_kernel, which lets this kernel's prologue start early (the wait sits before the first q' write).
+        // A predecessor that never signals (any other kernel) just completes first, as without the attribute.
         cudaLaunchConfig_t cfg = {};
         cudaLaunchAttribute at[1];
         at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
@@ -1501,7 +1523,7 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
         cfg.gridDim = dim3(pairs * G); cfg.blockDim = dim3(wideq ? 4 * kDh : kDh); cfg.dynamicSmemBytes = 0; cfg.stream = st;
         cfg.attrs = at; cfg.numAttrs = 1;
         cudaLaunchKernelEx(&cfg, wideq ? qfold_kernel<4> : qfold_kernel<1>, metas, (const float *)lay->d_rot_t, (const __nv_bfloat16 *)q, batch, Hkv, Hq,
-                           scale * 1.4426950408889634f, qf, 0);
+                           scale * 1.4426950408889634f, qf, 0, win ? 0 : 1);
     } else if (wideq)
         qfold_kernel<4><<<pairs * G, 4 * kDh, 0, st>>>(metas, lay->d_rot_t, (const __nv_bfloat16 *)q, batch, Hkv, Hq,
                                                        scale * 1.4426950408889634f, qf, 0);
