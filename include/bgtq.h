@@ -203,7 +203,13 @@ int bgtq_quantize_append_layers(const bgtq_layout *layout, int layer0, int n_lay
  * bgtq_decode_attention: one layer.  bgtq_decode_attention_layers: layers
  *   [layer0, layer0+n_layers) as independent problems in ONE launch (BASELINE.json cfg2
  *   "36 independent layers").
- * workspace [device] >= bgtq_workspace_bytes(layout, batch, n_layers). */
+ * workspace [device] >= bgtq_workspace_bytes(layout, batch, n_layers).
+ * Stream semantics: the call enqueues three kernels (query fold, split-KV attention, merge) chained by programmatic
+ *   dependent launch; the first of them is itself launched programmatically, so that in a layer-by-layer decode its
+ *   prologue runs beside the previous call's merge kernel.  It reads q BEFORE its griddepcontrol.wait: q (like the cache
+ *   and seq_len) must come from work that precedes the call on `stream` in the ordinary sense -- a kernel that does not
+ *   itself signal griddepcontrol.launch_dependents before it has written q (no kernel of this library writes q).
+ *   The workspace may be shared by consecutive calls on one stream; calls on different streams need their own. */
 int bgtq_decode_attention(const bgtq_layout *layout, int layer, const void *cache, const void *q,
                           const int32_t *seq_len, int batch, int64_t max_tokens,
                           float softmax_scale, void *out, void *workspace, size_t workspace_bytes,
