@@ -1022,3 +1022,38 @@ def test_attention_every_unit_count_and_partial_lane_pattern(P, tab128, counts):
     G = Hq // Hkv
     err = max(H.record_error("unit-count / partial-lane patterns", got[a], exp[a], rv[a // G], T=T, b_k=3, b_v=3) for a in range(Hq))
     assert err <= 2e-3, err
+
+
+def test_back_to_back_per_layer_calls_share_a_workspace(P, tab128):
+    """A layer-by-layer decode issues its calls back to back on one stream with ONE workspace: every call's q-fold kernel is
+    launched programmatically behind the previous call's merge kernel and must not touch the q' workspace before that call
+    is done with it.  40 unsynchronised calls alternating layers and queries == the same calls with a device synchronise
+    after each (bit for bit: every reduction has a fixed order)."""
+    Lyr, Hq, Hkv, d, T = 2, 16, 2, 128, 3000
+    probs = [H.make_problem(140 + l, T, Hq, Hkv, 3, 3, 1, 8, rope_base=1e6) for l in range(Lyr)]
+    bits = np.stack([p.bits for p in probs])
+    lay = P.Layout(bits, Hq, d, 3, probs[0].rot)
+    max_tokens = 3072
+    cache = lay.new_cache(1, max_tokens)
+    for l in range(Lyr):
+        seq = torch.zeros(1, dtype=torch.int32, device="cuda")
+        P.quantize_append(lay, l, cache, _cuda(probs[l].k_post[None], torch.float32), _cuda(probs[l].v[None], torch.float32), seq, max_tokens)
+    rng = np.random.default_rng(5)
+    qs = [_cuda(H.W.round_to_bf16(rng.standard_normal((1, Hq, d)) * 3.0), torch.bfloat16) for _ in range(4)]
+    ws = lay.new_workspace(1, 1)
+    scale = 1.0 / math.sqrt(d)
+    calls = [(i % Lyr, qs[(i * 7) % 4]) for i in range(40)]
+    ref = []
+    for l, q in calls:
+        ref.append(P.decode_attention(lay, l, cache, q, seq, max_tokens, scale, ws).clone())
+        torch.cuda.synchronize()
+    outs = [torch.empty_like(ref[0]) for _ in calls]
+    for (l, q), o in zip(calls, outs):
+        P.decode_attention(lay, l, cache, q, seq, max_tokens, scale, ws, out=o)
+    torch.cuda.synchronize()
+    for i, (a, b) in enumerate(zip(ref, outs)):
+        assert torch.equal(a, b), i
+    exp, rv = H.oracle_attention(probs[0], H.oracle_heads(probs[0], tab128), tab128, scale)    # and the chain still computes the method
+    got = P.decode_attention(lay, 0, cache, _cuda(probs[0].q_post[None], torch.bfloat16), seq, max_tokens, scale, ws)[0].double().cpu().numpy()
+    err = max(np.max(np.abs(got[a] - exp[a])) / rv[a // (Hq // Hkv)] for a in range(Hq))
+    assert err <= 2e-3, err
