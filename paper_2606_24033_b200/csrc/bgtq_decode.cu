@@ -1057,7 +1057,10 @@ window_kernel(const __half *__restrict__ win_k, const __half *__restrict__ win_v
     __syncthreads();
     const float Mx = fmaxf(fmaxf(red[0], red[1]), fmaxf(red[2], red[3]));
     float *rec = partials + (size_t)(win_slot + pair) * kPartialFloats + n * 130;
+    // (launched programmatically behind the previous call's combine_kernel, which may still read the record workspace:
+    //  every write to it comes after a griddepcontrol.wait -- a no-op without a programmatic dependency)
     if (Mx == -INFINITY) {                              // empty sequence: an empty record
+        pdl_wait();
         if (d == 0) { rec[0] = -INFINITY; rec[1] = 0.f; }
         rec[2 + d] = 0.f;
         return;
@@ -1106,6 +1109,7 @@ window_kernel(const __half *__restrict__ win_k, const __half *__restrict__ win_v
         float r = 0.f;
 #pragma unroll 16
         for (int u = 0; u < m; ++u) r = fmaf(__ldg(T + u * m), o[16 * M.vblk[(s + u) >> 4] + (u & 15)], r);
+        pdl_wait();
         rec[2 + d] = r * sqrtf((float)m);
         if (d == 0) { rec[0] = Mx; rec[1] = lsum; }
         return;
@@ -1113,6 +1117,7 @@ window_kernel(const __half *__restrict__ win_k, const __half *__restrict__ win_v
     float r = 0.f;                                      // acc_rot[d] = sqrt(128) * sum_j Pi[d][j] o[j]; rot128_t[j][d] = Pi[d][j]
 #pragma unroll 32
     for (int j = 0; j < kDh; ++j) r = fmaf(__ldg(rot128_t + j * kDh + d), o[j], r);
+    pdl_wait();
     rec[2 + d] = r * 11.313708498984761f;
     if (d == 0) { rec[0] = Mx; rec[1] = lsum; }
 }
@@ -1449,11 +1454,16 @@ int launch_combine(const float *partials, const int32_t *seq_len, const float *r
 
 int launch_window(const void *win_k, const void *win_v, const void *q, const int32_t *seq_len, const float *rot128_t,
                   float *partials, int pairs, int batch, int Hkv, int G, int64_t n_cap, int n_sink, int n_recent,
-                  float scale_log2e, int win_slot, cudaStream_t st, const HeadMeta *metas, const float *rot_t_base)
+                  float scale_log2e, int win_slot, cudaStream_t st, const HeadMeta *metas, const float *rot_t_base, bool pdl)
 {
-    window_kernel<<<pairs * G, 128, 0, st>>>((const __half *)win_k, (const __half *)win_v, (const __nv_bfloat16 *)q, seq_len,
-                                             rot128_t, partials, batch, Hkv, G, n_cap, n_sink, n_recent, scale_log2e, win_slot,
-                                             metas, rot_t_base);
+    cudaLaunchConfig_t cfg = {};
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
+    cfg.gridDim = dim3(pairs * G); cfg.blockDim = dim3(128); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, window_kernel, (const __half *)win_k, (const __half *)win_v, (const __nv_bfloat16 *)q, seq_len,
+                       rot128_t, partials, batch, Hkv, G, n_cap, n_sink, n_recent, scale_log2e, win_slot, metas, rot_t_base);
     count_launch();
     CUDA_TRY(cudaGetLastError());
     return BGTQ_OK;
@@ -1502,19 +1512,20 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
     const HeadMeta *metas = lay->d_meta + (size_t)layer0 * Hkv;
 
     const int win_slot = win ? lay->sm_count * kMaxWarpsPerSM + pairs : -1;    // first record after the warp records
-    if (win) {   // fp16 windows -> one record per (pair, query head).  An ordinary launch (everything before it, the appends
-                 // included, is complete when it starts); qfold_kernel is then launched programmatically behind it and the
-                 // two run side by side.  Completion order is kept by qfold_kernel's trailing griddepcontrol.wait:
-                 // window -> qfold -> decode -> combine, each waiting for its predecessor only.
+    if (win) {   // fp16 windows -> one record per (pair, query head).  Launched programmatically like qfold_kernel below (it
+                 // reads the windows, q and seq_len -- complete in stream order -- and waits before it writes its record, which
+                 // the previous call's combine_kernel may still read); qfold_kernel is launched programmatically behind it and
+                 // the two run side by side.  Completion order: window -> qfold -> decode -> combine, each waiting for its
+                 // predecessor only (qfold_kernel's wait before its first q' write also covers the previous call's decode_kernel).
         if (int rc = launch_window(win->k, win->v, q, seq_len, lay->d_rot_t + rot_offset(kDh), partials, pairs, batch, Hkv, G, n_cap,
                                    n_sink, n_recent, scale * 1.4426950408889634f, win_slot, st,
-                                   lay->v_grouped ? metas : nullptr, lay->d_rot_t)) return rc;
+                                   lay->v_grouped ? metas : nullptr, lay->d_rot_t, !g_prof)) return rc;
     }
     const bool wideq = pairs * G <= kLatencyShapedBlocks;       // few blocks: the latency-shaped 512-thread variant
     if (!g_prof) {
-        // programmatic launch: behind window_kernel (protected regime; the two run side by side, the wait sits at the end of
-        // qfold_kernel) or behind whatever precedes the call on the stream -- in a layer-by-layer decode that is the previous
-        // layer's combine_kernel, which lets this kernel's prologue start early (the wait sits before the first q' write).
+        // programmatic launch: behind window_kernel (protected regime) or behind whatever precedes the call on the stream -- in
+        // a layer-by-layer decode that is the previous layer's combine_kernel, which lets this kernel's prologue and dot
+        // products start early (the wait sits before the first q' write).
         // A predecessor that never signals (any other kernel) just completes first, as without the attribute.
         cudaLaunchConfig_t cfg = {};
         cudaLaunchAttribute at[1];
@@ -1523,7 +1534,7 @@ int launch_decode(const bgtq_layout *lay, int layer0, int n_layers, const void *
         cfg.gridDim = dim3(pairs * G); cfg.blockDim = dim3(wideq ? 4 * kDh : kDh); cfg.dynamicSmemBytes = 0; cfg.stream = st;
         cfg.attrs = at; cfg.numAttrs = 1;
         cudaLaunchKernelEx(&cfg, wideq ? qfold_kernel<4> : qfold_kernel<1>, metas, (const float *)lay->d_rot_t, (const __nv_bfloat16 *)q, batch, Hkv, Hq,
-                           scale * 1.4426950408889634f, qf, 0, win ? 0 : 1);
+                           scale * 1.4426950408889634f, qf, 0, 1);
     } else if (wideq)
         qfold_kernel<4><<<pairs * G, 4 * kDh, 0, st>>>(metas, lay->d_rot_t, (const __nv_bfloat16 *)q, batch, Hkv, Hq,
                                                        scale * 1.4426950408889634f, qf, 0);

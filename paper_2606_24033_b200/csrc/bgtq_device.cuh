@@ -193,7 +193,8 @@ int launch_combine(const float *partials, const int32_t *seq_len, const float *r
                    const HeadMeta *metas = nullptr, const float *rot_base = nullptr);   // metas: heads with V-side groups
 int launch_window(const void *win_k, const void *win_v, const void *q, const int32_t *seq_len, const float *rot128_t,
                   float *partials, int pairs, int batch, int Hkv, int G, int64_t n_cap, int n_sink, int n_recent,
-                  float scale_log2e, int win_slot, cudaStream_t st, const HeadMeta *metas = nullptr, const float *rot_t_base = nullptr);
+                  float scale_log2e, int win_slot, cudaStream_t st, const HeadMeta *metas = nullptr, const float *rot_t_base = nullptr,
+                  bool pdl = false);   // pdl: programmatic launch (the kernel waits before it writes its record)
 // bgtq_profile_decode: event pair around the split-KV kernel of a decode call (no-ops unless enabled)
 bool profile_decode_on();
 int profile_decode_begin(cudaStream_t st);
